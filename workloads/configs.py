@@ -1,0 +1,98 @@
+"""The five BASELINE.json configs (C0..C4, 0-indexed: reading A15) as seeded synthetic inputs,
+plus reduced-size variants of the same recipes for tests the CPU oracle finishes in seconds.
+
+Holds none of the method's arithmetic: geometry, neighbour lists and N(0, sigma) draws only.
+Radial weights w(r), spherical harmonics etc. are computed by each side (oracle / CUDA) itself.
+"""
+import numpy as np
+
+from . import geometry, rng
+
+# name -> recipe.  density 0.1 atoms/A^3 stands in for water at 1 g/cm^3.
+SPECS = {
+    # BASELINE.json:configs[0]
+    "C0": dict(kind="periodic", n_atoms=64, box=10.0, rc=4.0, lmax=1, n=8, dtype="f64", wmode="scalar"),
+    # BASELINE.json:configs[1] -- the config the metric is quoted on
+    "C1": dict(kind="periodic", n_atoms=4096, density=0.1, rc=6.0, lmax=2, n=64, dtype="f32", wmode="scalar"),
+    # BASELINE.json:configs[2] -- two stacked layers, dense per-path mix
+    "C2": dict(kind="periodic", n_atoms=32768, density=0.1, rc=6.0, lmax=2, n=64, dtype="f32", wmode="dense",
+               n_layers=2),
+    # BASELINE.json:configs[3]
+    "C3": dict(kind="periodic", n_atoms=100000, density=0.1, rc=5.0, lmax=3, n=128, dtype="f32", wmode="scalar"),
+    # BASELINE.json:configs[4]
+    "C4": dict(kind="molecules", n_mol=64, rc=6.0, lmax=2, n=32, dtype="f32", wmode="scalar"),
+    # reduced-size variants (same recipes) for CPU-side tests and quick GPU parity
+    "C1s": dict(kind="periodic", n_atoms=200, density=0.1, rc=6.0, lmax=2, n=64, dtype="f32", wmode="scalar"),
+    "C2s": dict(kind="periodic", n_atoms=192, density=0.1, rc=6.0, lmax=2, n=64, dtype="f32", wmode="dense",
+                n_layers=2),
+    "C3s": dict(kind="periodic", n_atoms=150, density=0.1, rc=5.0, lmax=3, n=128, dtype="f32", wmode="scalar"),
+    "C4s": dict(kind="molecules", n_mol=6, rc=6.0, lmax=2, n=32, dtype="f32", wmode="scalar"),
+}
+
+N_BASIS = 8       # Bessel functions (configs[0], configs[1])
+KAPPA = 0.3       # reading A12
+
+
+def num_paths(lmax):
+    """count of parity-allowed (l1,p1,l2->l3) paths (reading A3); pure counting, no CG values"""
+    cnt = 0
+    for l1 in range(lmax + 1):
+        for l2 in range(lmax + 1):
+            cnt += len(range(abs(l1 - l2), min(l1 + l2, lmax) + 1))
+    return 2 * cnt
+
+
+def geometry_for(name, seed=0):
+    s = dict(SPECS[name])
+    if s["kind"] == "periodic":
+        box = s.get("box") or (s["n_atoms"] / s["density"]) ** (1.0 / 3.0)
+        assert s["rc"] < box / 2, "config too small for minimum image"
+        pos = geometry.periodic_box(seed, s["n_atoms"], box)
+        nl = geometry.neighbour_list_periodic(pos, box, s["rc"])
+        nl.update(pos=pos, box=box, mol_ptr=None)
+    else:
+        pos, mol_ptr = geometry.molecules(seed, s["n_mol"])
+        nl = geometry.neighbour_list_open(pos, s["rc"], mol_ptr)
+        nl.update(pos=pos, box=None, mol_ptr=mol_ptr)
+    nl["species"] = geometry.species(seed, pos.shape[0])
+    nl["spec"] = s
+    nl["name"] = name
+    return nl
+
+
+def weights_for(name, seed=0):
+    """Small parameter tensors (float64; each side rounds to its own dtype)."""
+    s = SPECS[name]
+    n, lmax = s["n"], s["lmax"]
+    P = num_paths(lmax)
+    S = rng.STREAMS
+    out = dict(
+        W_r=rng.normal(seed, S["W_r"], (n, N_BASIS)) / np.sqrt(N_BASIS),      # N(0, 1/8)
+        path_w=rng.normal(seed, S["path_w"], (P,)) / np.sqrt(P),              # N(0, 1/#paths), A5
+        q=rng.normal(seed, S["q"], (n,)) / np.sqrt(n),                        # N(0, 1/n), A12
+        kappa=KAPPA,
+    )
+    if s["wmode"] == "dense":
+        L = s["n_layers"]
+        out.update(
+            W_x0=rng.normal(seed, S["W_x0"], (n, N_BASIS)) / np.sqrt(N_BASIS),
+            W_v0=rng.normal(seed, S["W_v0"], (n, N_BASIS)) / np.sqrt(N_BASIS),
+            W_w=rng.normal(seed, S["W_w"], (L, n, n)) / np.sqrt(n),
+            W_p=rng.normal(seed, S["W_p"], (L, P, n, n)) / np.sqrt(n),
+            A_lat=rng.normal(seed, S["A_lat"], (max(L - 1, 1), n, 2 * n)) / np.sqrt(2 * n),
+        )
+    return out
+
+
+def features_for(name, n_edges, seed=0, which="V", e_lo=0, e_hi=None):
+    """V or G ~ N(0,1), shape [e_hi-e_lo, n, dV]; rows are a pure function of the edge index, so
+    any slice can be regenerated on its own."""
+    s = SPECS[name]
+    dV = 2 * (s["lmax"] + 1) ** 2
+    e_hi = n_edges if e_hi is None else e_hi
+    row = s["n"] * dV
+    return rng.normal(seed, rng.STREAMS[which], (e_hi - e_lo, s["n"], dV), offset=e_lo * row)
+
+
+def np_dtype(name):
+    return np.float64 if SPECS[name]["dtype"] == "f64" else np.float32
