@@ -1,0 +1,38 @@
+// plan.h -- internal host-side plan tables of the product library (not part of the ABI).
+// Shares nothing with oracle/: the complex CG coefficients here come from the ladder-operator
+// recursion, not from the Racah sum.
+#pragma once
+#include <cstdint>
+#include <vector>
+
+namespace allegro {
+
+struct PathInfo {
+    int l1, p1, l2, l3, p3, off1, off2, off3;
+};
+struct NonZero {
+    int path, i, j, k;
+    double c;
+};
+
+struct PlanTables {
+    int l_max = 0;
+    int dV = 0, dE = 0;
+    std::vector<PathInfo> paths;
+    std::vector<NonZero> nnz;  // sorted (path, i, j, k)
+};
+
+// <j1 m1 j2 m2 | J M>, Condon-Shortley, all (m1, m2) for one (j1, j2, J): table[(m1+j1)*(2j2+1) + (m2+j2)][M+J]
+void cg_complex_ladder(int j1, int j2, int J, std::vector<double>& table);
+// real-basis block C[m1][m2][M] (reading A2: C = Re T + Im T)
+void cg_real_block(int l1, int l2, int l3, std::vector<double>& C);
+void build_tables(int l_max, PlanTables& t);
+long build_segments(const int32_t* row_ptr, int n_atoms, int tile_edges, int32_t* items, long cap);
+
+}  // namespace allegro
+
+struct allegro_plan {
+    int l_max, n, dtype, wmode;
+    allegro::PlanTables tab;
+    // order in which the generated kernels index the folded coefficient table (== tab.nnz order)
+};
