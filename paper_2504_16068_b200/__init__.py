@@ -1,0 +1,265 @@
+"""paper_2504_16068_b200 -- Python binding of liballegro_b200.so (include/allegro_b200.h).
+
+Argument marshalling only: every step of the hot path runs in the library's CUDA kernels (sm_100a).
+torch is used for device memory and streams.  There is no CPU fallback and nothing here imports the
+oracle: if the shared library is missing the import of any entry point raises.
+
+Names mirror the C ABI without the `allegro_` prefix:
+    Plan(l_max, n, dtype, wmode)            allegro_plan_create / _destroy / _paths / _cg
+    segments_build, env_embed, tp_forward, tp_backward, env_embed_backward, force_gather,
+    radial_forward, radial_backward, edge_energy, segment_sum, launch_count
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liballegro_b200.so")
+_lib = None
+
+F32, F64 = 0, 1
+W_SCALAR, W_DENSE = 0, 1
+_STATUS = {0: "ALLEGRO_OK", 1: "ALLEGRO_EINVAL", 2: "ALLEGRO_EUNSUPPORTED", 3: "ALLEGRO_ECUDA", 4: "ALLEGRO_ENOMEM"}
+
+_vp, _i32p, _f64p = C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_double)
+
+# name -> (restype, argtypes); one row per symbol declared in include/allegro_b200.h
+SIGNATURES = {
+    "allegro_plan_create": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(_vp)]),
+    "allegro_plan_destroy": (None, [_vp]),
+    "allegro_plan_num_paths": (C.c_int, [_vp]),
+    "allegro_plan_dim_v": (C.c_int, [_vp]),
+    "allegro_plan_dim_e": (C.c_int, [_vp]),
+    "allegro_plan_nnz": (C.c_long, [_vp]),
+    "allegro_plan_paths": (C.c_int, [_vp] + [_i32p] * 8),
+    "allegro_plan_cg": (C.c_int, [_vp] + [_i32p] * 4 + [_f64p]),
+    "allegro_cg_real_block": (C.c_int, [C.c_int, C.c_int, C.c_int, _f64p]),
+    "allegro_segments_build": (C.c_int, [_i32p, C.c_int, C.c_int, _i32p, C.c_long, C.POINTER(C.c_long)]),
+    "allegro_env_embed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, C.c_size_t, _vp]),
+    "allegro_tp_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_tp_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
+    "allegro_tp_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_long, C.c_int]),
+    "allegro_env_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
+    "allegro_env_embed_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp]),
+    "allegro_force_gather": (C.c_int, [C.c_int, C.c_long, _vp, _vp, _vp, C.c_int, _vp, _vp]),
+    "allegro_radial_forward": (C.c_int, [C.c_int, C.c_int, C.c_double, C.c_int, C.c_long, _vp, _vp, _vp, _vp]),
+    "allegro_radial_backward": (C.c_int, [C.c_int, C.c_int, C.c_double, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_edge_energy": (C.c_int, [_vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, _vp]),
+    "allegro_segment_sum": (C.c_int, [_vp, C.c_int, _vp, C.c_int, _vp, _vp]),
+    "allegro_status_str": (C.c_char_p, [C.c_int]),
+    "allegro_last_error": (C.c_char_p, []),
+    "allegro_launch_count": (C.c_long, []),
+}
+
+
+class AllegroError(RuntimeError):
+    def __init__(self, status, detail):
+        super().__init__("%s: %s" % (_STATUS.get(status, status), detail))
+        self.status = status
+
+
+def lib():
+    """Load the CUDA library (fails loudly when it has not been built: there is no fallback)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError("liballegro_b200.so not built: run `python -m paper_2504_16068_b200.build` "
+                              "(or __graft_entry__.build()); there is no CPU fallback")
+        L = C.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def _check(status):
+    if status != 0:
+        raise AllegroError(status, lib().allegro_last_error().decode())
+
+
+def _ptr(t):
+    if t is None:
+        return None
+    assert t.is_contiguous(), "tensors handed to the library must be contiguous"
+    return t.data_ptr()
+
+
+def _stream(stream):
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def torch_dtype(dtype):
+    return torch.float32 if dtype == F32 else torch.float64
+
+
+class Plan:
+    """allegro_plan_t: CG table + path plan for (l_max, full parity), n channels, dtype, weight mode."""
+
+    def __init__(self, l_max, n, dtype=F32, wmode=W_SCALAR):
+        h = _vp()
+        _check(lib().allegro_plan_create(l_max, 0, n, dtype, wmode, C.byref(h)))
+        self.h = h
+        self.l_max, self.n, self.dtype, self.wmode = l_max, n, dtype, wmode
+        self.P = lib().allegro_plan_num_paths(h)
+        self.dV = lib().allegro_plan_dim_v(h)
+        self.dE = lib().allegro_plan_dim_e(h)
+        self.nnz = lib().allegro_plan_nnz(h)
+        self.tdtype = torch_dtype(dtype)
+
+    def __del__(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.allegro_plan_destroy(self.h)
+            self.h = None
+
+    def paths(self):
+        names = ["l1", "p1", "l2", "l3", "p3", "off1", "off2", "off3"]
+        arrs = [np.zeros(self.P, dtype=np.int32) for _ in names]
+        _check(lib().allegro_plan_paths(self.h, *[a.ctypes.data_as(_i32p) for a in arrs]))
+        return dict(zip(names, arrs))
+
+    def cg(self):
+        path, i, j, k = [np.zeros(self.nnz, dtype=np.int32) for _ in range(4)]
+        coef = np.zeros(self.nnz)
+        _check(lib().allegro_plan_cg(self.h, *[a.ctypes.data_as(_i32p) for a in (path, i, j, k)], coef.ctypes.data_as(_f64p)))
+        return dict(path=path, i=i, j=j, k=k, coef=coef)
+
+
+def cg_real_block(l1, l2, l3):
+    out = np.zeros((2 * l1 + 1, 2 * l2 + 1, 2 * l3 + 1))
+    _check(lib().allegro_cg_real_block(l1, l2, l3, out.ctypes.data_as(_f64p)))
+    return out
+
+
+def segments_build(row_ptr_host, tile_edges):
+    """HOST int32 row_ptr -> HOST int32 items[n_items, 3] (reading A16)."""
+    rp = np.ascontiguousarray(row_ptr_host, dtype=np.int32)
+    n_atoms = rp.shape[0] - 1
+    cnt = C.c_long(0)
+    _check(lib().allegro_segments_build(rp.ctypes.data_as(_i32p), n_atoms, tile_edges, None, 0, C.byref(cnt)))
+    items = np.zeros((cnt.value, 3), dtype=np.int32)
+    _check(lib().allegro_segments_build(rp.ctypes.data_as(_i32p), n_atoms, tile_edges, items.ctypes.data_as(_i32p), cnt.value,
+                                        C.byref(cnt)))
+    return items
+
+
+def launch_count():
+    return lib().allegro_launch_count()
+
+
+def _n_items(items):
+    return 0 if items is None else items.shape[0]
+
+
+def env_workspace(plan, n_atoms, items):
+    return lib().allegro_env_workspace(plan.h, n_atoms, _n_items(items))
+
+
+def tp_backward_workspace(plan, n_atoms, n_edges, items, want_g_path_w):
+    return lib().allegro_tp_backward_workspace(plan.h, n_atoms, n_edges, _n_items(items), int(bool(want_g_path_w)))
+
+
+def _ws(nbytes, device):
+    return torch.empty(max(int(nbytes), 16), dtype=torch.uint8, device=device)
+
+
+def env_embed(plan, row_ptr, rvec, w, scale=1.0, items=None, Eenv=None, workspace=None, stream=None):
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if Eenv is None:
+        Eenv = torch.empty((n_atoms, plan.n, plan.dE), dtype=plan.tdtype, device=rvec.device)
+    if workspace is None and items is not None:
+        workspace = _ws(env_workspace(plan, n_atoms, items), rvec.device)
+    _check(lib().allegro_env_embed(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(rvec), _ptr(w),
+                                   float(scale), _ptr(Eenv), _ptr(workspace), 0 if workspace is None else workspace.numel(),
+                                   _stream(stream)))
+    return Eenv
+
+
+def tp_forward(plan, row_ptr, V, Eenv, path_w, items=None, out=None, stream=None):
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    if out is None:
+        out = torch.empty_like(V)
+    _check(lib().allegro_tp_forward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(V), _ptr(Eenv),
+                                    _ptr(path_w), _ptr(out), _stream(stream)))
+    return out
+
+
+def tp_backward(plan, row_ptr, G, V, Eenv, path_w, items=None, want_gV=True, want_g_path_w=False, gV=None, gEenv=None,
+                g_path_w=None, workspace=None, stream=None):
+    """-> (gV or None, gEenv, g_path_w or None)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    if gV is None and want_gV:
+        gV = torch.empty_like(V)
+    if gEenv is None:
+        gEenv = torch.empty_like(Eenv)
+    if g_path_w is None and want_g_path_w:
+        g_path_w = torch.empty_like(path_w)
+    if workspace is None:
+        workspace = _ws(tp_backward_workspace(plan, n_atoms, n_edges, items, g_path_w is not None), V.device)
+    _check(lib().allegro_tp_backward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(V),
+                                     _ptr(Eenv), _ptr(path_w), _ptr(gV), _ptr(gEenv), _ptr(g_path_w), _ptr(workspace),
+                                     workspace.numel(), _stream(stream)))
+    return gV, gEenv, g_path_w
+
+
+def env_embed_backward(plan, row_ptr, gEenv, rvec, w, scale=1.0, want_g_w=True, g_rvec=None, g_w=None, stream=None):
+    """-> (g_rvec[E,3], g_w[E,n] or None)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if g_rvec is None:
+        g_rvec = torch.empty_like(rvec)
+    if g_w is None and want_g_w:
+        g_w = torch.empty_like(w)
+    _check(lib().allegro_env_embed_backward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(gEenv), _ptr(rvec), _ptr(w),
+                                            float(scale), _ptr(g_rvec), _ptr(g_w), _stream(stream)))
+    return g_rvec, g_w
+
+
+def _dt(t):
+    return F32 if t.dtype == torch.float32 else F64
+
+
+def force_gather(row_ptr, rev, g_rvec, F=None, stream=None):
+    n_atoms, n_edges = row_ptr.shape[0] - 1, g_rvec.shape[0]
+    if F is None:
+        F = torch.empty((n_atoms, 3), dtype=g_rvec.dtype, device=g_rvec.device)
+    _check(lib().allegro_force_gather(n_atoms, n_edges, _ptr(row_ptr), _ptr(rev), _ptr(g_rvec), _dt(g_rvec), _ptr(F), _stream(stream)))
+    return F
+
+
+def radial_forward(rvec, W_r, r_cut, w=None, stream=None):
+    n, nb = W_r.shape
+    if w is None:
+        w = torch.empty((rvec.shape[0], n), dtype=rvec.dtype, device=rvec.device)
+    _check(lib().allegro_radial_forward(n, nb, float(r_cut), _dt(rvec), rvec.shape[0], _ptr(rvec), _ptr(W_r), _ptr(w), _stream(stream)))
+    return w
+
+
+def radial_backward(rvec, W_r, r_cut, g_w, g_rvec, stream=None):
+    """g_rvec += (sum_n g_w dw/dr) rhat, in place"""
+    n, nb = W_r.shape
+    _check(lib().allegro_radial_backward(n, nb, float(r_cut), _dt(rvec), rvec.shape[0], _ptr(rvec), _ptr(W_r), _ptr(g_w), _ptr(g_rvec),
+                                         _stream(stream)))
+    return g_rvec
+
+
+def edge_energy(plan, out, q, kappa, want_e=True, want_G=True, e_edge=None, G=None, stream=None):
+    """-> (e_edge[E] or None, G or None)"""
+    if e_edge is None and want_e:
+        e_edge = torch.empty((out.shape[0],), dtype=out.dtype, device=out.device)
+    if G is None and want_G:
+        G = torch.empty_like(out)
+    _check(lib().allegro_edge_energy(plan.h, out.shape[0], _ptr(out), _ptr(q), float(kappa), _ptr(e_edge), _ptr(G), _stream(stream)))
+    return e_edge, G
+
+
+def segment_sum(ptr, vals, out=None, stream=None):
+    nseg = ptr.shape[0] - 1
+    if out is None:
+        out = torch.empty((nseg,), dtype=vals.dtype, device=vals.device)
+    _check(lib().allegro_segment_sum(_ptr(ptr), nseg, _ptr(vals), _dt(vals), _ptr(out), _stream(stream)))
+    return out

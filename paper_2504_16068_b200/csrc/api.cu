@@ -1,0 +1,243 @@
+// api.cu -- the C ABI of include/allegro_b200.h: argument checks and dispatch to the per-(dtype, l_max)
+// launchers.  No arithmetic of the method lives here.
+#include <cstdarg>
+#include <cstring>
+#include <new>
+
+#include "common.cuh"
+#include "launch.h"
+
+namespace allegro {
+
+std::atomic<long> g_launches{0};
+static thread_local char t_err[512] = "";
+
+void set_error(const char* fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(t_err, sizeof t_err, fmt, ap);
+    va_end(ap);
+}
+
+// explicit specialisations live in inst_tp.cu / inst_env.cu (one object per dtype and l_max)
+#define ALLEGRO_DECL(T, L)                                                                     \
+    template <> allegro_status_t launch_env_embed<T, L>(const EnvArgs&);                       \
+    template <> allegro_status_t launch_env_embed_backward<T, L>(const EnvBwdArgs&);           \
+    template <> allegro_status_t launch_tp_forward<T, L>(const TpArgs&);                       \
+    template <> allegro_status_t launch_tp_backward<T, L>(const TpArgs&);                      \
+    template <> size_t tp_backward_workspace<T, L>(int, int, long, bool, int, bool);
+ALLEGRO_DECL(float, 1) ALLEGRO_DECL(float, 2) ALLEGRO_DECL(float, 3)
+ALLEGRO_DECL(double, 1) ALLEGRO_DECL(double, 2) ALLEGRO_DECL(double, 3)
+#undef ALLEGRO_DECL
+
+// call F<T, L>(args...) for the plan's dtype and l_max
+#define ALLEGRO_DISPATCH(plan, F, ...)                                   \
+    ((plan)->dtype == ALLEGRO_F32                                        \
+         ? ((plan)->l_max == 1 ? F<float, 1>(__VA_ARGS__)                \
+            : (plan)->l_max == 2 ? F<float, 2>(__VA_ARGS__)              \
+                                 : F<float, 3>(__VA_ARGS__))             \
+         : ((plan)->l_max == 1 ? F<double, 1>(__VA_ARGS__)               \
+            : (plan)->l_max == 2 ? F<double, 2>(__VA_ARGS__)             \
+                                 : F<double, 3>(__VA_ARGS__)))
+
+}  // namespace allegro
+
+using namespace allegro;
+
+extern "C" {
+
+allegro_status_t allegro_plan_create(int l_max, allegro_parity_t parity, int n_channels, allegro_dtype_t dtype, allegro_wmode_t wmode,
+                                     allegro_plan_t** out) {
+    ALLEGRO_CHECK_ARG(out != nullptr, "out is NULL");
+    *out = nullptr;
+    ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
+    ALLEGRO_CHECK_ARG(wmode == ALLEGRO_W_SCALAR || wmode == ALLEGRO_W_DENSE, "bad weight mode");
+    ALLEGRO_CHECK_ARG(n_channels >= 1, "n_channels < 1");
+    if (l_max < 1 || l_max > 3 || parity != ALLEGRO_PARITY_FULL || n_channels > 256) {
+        set_error("allegro_plan_create: unsupported (l_max = %d, parity = %d, n = %d); l_max 1..3, full parity, n <= 256", l_max, (int)parity,
+                  n_channels);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    allegro_plan* p = new (std::nothrow) allegro_plan();
+    if (!p) { set_error("allegro_plan_create: out of host memory"); return ALLEGRO_ENOMEM; }
+    p->l_max = l_max; p->n = n_channels; p->dtype = (int)dtype; p->wmode = (int)wmode;
+    build_tables(l_max, p->tab);
+    *out = p;
+    return ALLEGRO_OK;
+}
+void allegro_plan_destroy(allegro_plan_t* plan) { delete plan; }
+int allegro_plan_num_paths(const allegro_plan_t* plan) { return plan ? (int)plan->tab.paths.size() : -1; }
+int allegro_plan_dim_v(const allegro_plan_t* plan) { return plan ? plan->tab.dV : -1; }
+int allegro_plan_dim_e(const allegro_plan_t* plan) { return plan ? plan->tab.dE : -1; }
+long allegro_plan_nnz(const allegro_plan_t* plan) { return plan ? (long)plan->tab.nnz.size() : -1; }
+
+allegro_status_t allegro_plan_paths(const allegro_plan_t* plan, int32_t* l1, int32_t* p1, int32_t* l2, int32_t* l3, int32_t* p3, int32_t* off1,
+                                    int32_t* off2, int32_t* off3) {
+    ALLEGRO_CHECK_ARG(plan && l1 && p1 && l2 && l3 && p3 && off1 && off2 && off3, "NULL argument");
+    for (size_t p = 0; p < plan->tab.paths.size(); ++p) {
+        const PathInfo& q = plan->tab.paths[p];
+        l1[p] = q.l1; p1[p] = q.p1; l2[p] = q.l2; l3[p] = q.l3; p3[p] = q.p3; off1[p] = q.off1; off2[p] = q.off2; off3[p] = q.off3;
+    }
+    return ALLEGRO_OK;
+}
+allegro_status_t allegro_plan_cg(const allegro_plan_t* plan, int32_t* path, int32_t* i, int32_t* j, int32_t* k, double* coef) {
+    ALLEGRO_CHECK_ARG(plan && path && i && j && k && coef, "NULL argument");
+    for (size_t z = 0; z < plan->tab.nnz.size(); ++z) {
+        const NonZero& q = plan->tab.nnz[z];
+        path[z] = q.path; i[z] = q.i; j[z] = q.j; k[z] = q.k; coef[z] = q.c;
+    }
+    return ALLEGRO_OK;
+}
+allegro_status_t allegro_cg_real_block(int l1, int l2, int l3, double* C) {
+    ALLEGRO_CHECK_ARG(C != nullptr, "C is NULL");
+    ALLEGRO_CHECK_ARG(l1 >= 0 && l2 >= 0 && l3 >= 0 && l1 <= 8 && l2 <= 8 && l3 <= 8, "l out of range 0..8");
+    std::vector<double> c;
+    cg_real_block(l1, l2, l3, c);
+    std::memcpy(C, c.data(), c.size() * sizeof(double));
+    return ALLEGRO_OK;
+}
+allegro_status_t allegro_segments_build(const int32_t* row_ptr_host, int n_atoms, int tile_edges, int32_t* items, long cap, long* n_items) {
+    ALLEGRO_CHECK_ARG(row_ptr_host && n_items, "NULL argument");
+    ALLEGRO_CHECK_ARG(n_atoms >= 0 && tile_edges >= 1 && cap >= 0, "negative size");
+    for (int i = 0; i < n_atoms; ++i) ALLEGRO_CHECK_ARG(row_ptr_host[i + 1] >= row_ptr_host[i], "row_ptr not monotone");
+    *n_items = build_segments(row_ptr_host, n_atoms, tile_edges, items, cap);
+    return ALLEGRO_OK;
+}
+
+#define ALLEGRO_CHECK_GRAPH()                                                                     \
+    ALLEGRO_CHECK_ARG(plan != nullptr, "plan is NULL");                                           \
+    ALLEGRO_CHECK_ARG(n_atoms >= 0 && n_edges >= 0 && n_edges < 2147483647L, "bad n_atoms / n_edges"); \
+    ALLEGRO_CHECK_ARG(row_ptr != nullptr || n_atoms == 0, "row_ptr is NULL")
+
+allegro_status_t allegro_env_embed(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                   long n_items, const void* rvec, const void* w, double scale, void* Eenv, void* workspace,
+                                   size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && w) || n_edges == 0, "rvec / w is NULL");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    ALLEGRO_CHECK_ARG(aligned16(Eenv) && aligned16(w), "Eenv / w not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    const size_t need = allegro_env_workspace(plan, n_atoms, items ? n_items : 0);
+    if (items && (workspace == nullptr || workspace_bytes < need)) {
+        set_error("allegro_env_embed: workspace too small (%zu < %zu bytes)", workspace_bytes, need);
+        return ALLEGRO_ENOMEM;
+    }
+    EnvArgs a{plan->n, n_atoms, n_edges, row_ptr, items, items ? n_items : (long)n_atoms, rvec, w, scale, Eenv, workspace, (cudaStream_t)stream};
+    return ALLEGRO_DISPATCH(plan, launch_env_embed, a);
+}
+
+allegro_status_t allegro_tp_forward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                    long n_items, const void* V, const void* Eenv, const void* path_w, void* out, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((V && out) || n_edges == 0, "V / out is NULL");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr, "path_w is NULL");
+    ALLEGRO_CHECK_ARG(V != out || n_edges == 0, "out aliases V");
+    ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(out) && aligned16(Eenv), "feature tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.out = out; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_forward, a);
+}
+
+allegro_status_t allegro_tp_backward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                     long n_items, const void* G, const void* V, const void* Eenv, const void* path_w, void* gV, void* gEenv,
+                                     void* g_path_w, void* workspace, size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((G && V) || n_edges == 0, "G / V is NULL");
+    ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr, "path_w is NULL");
+    ALLEGRO_CHECK_ARG(gV == nullptr || (gV != G && gV != V), "gV aliases an input");
+    ALLEGRO_CHECK_ARG(aligned16(G) && aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace),
+                      "tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.G = G; a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.gV = gV; a.gEenv = gEenv; a.g_path_w = g_path_w;
+    a.ws = workspace; a.ws_bytes = workspace_bytes; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
+}
+
+size_t allegro_tp_backward_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges, long n_items, int want_g_path_w) {
+    (void)n_edges;
+    if (!plan) return 0;
+    const bool have_items = n_items > 0;
+    const long ni = have_items ? n_items : (long)n_atoms;
+    return ALLEGRO_DISPATCH(plan, tp_backward_workspace, plan->n, n_atoms, ni, have_items, plan->wmode, want_g_path_w != 0);
+}
+size_t allegro_env_workspace(const allegro_plan_t* plan, int n_atoms, long n_items) {
+    (void)n_atoms;
+    if (!plan || n_items <= 0) return 0;
+    return (size_t)n_items * plan->n * plan->tab.dE * (plan->dtype == ALLEGRO_F32 ? 4 : 8);
+}
+
+allegro_status_t allegro_env_embed_backward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const void* gEenv,
+                                            const void* rvec, const void* w, double scale, void* g_rvec, void* g_w, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && w && g_rvec) || n_edges == 0, "rvec / w / g_rvec is NULL");
+    ALLEGRO_CHECK_ARG(gEenv || n_atoms == 0, "gEenv is NULL");
+    EnvBwdArgs a{plan->n, n_atoms, n_edges, row_ptr, gEenv, rvec, w, scale, g_rvec, g_w, (cudaStream_t)stream};
+    return ALLEGRO_DISPATCH(plan, launch_env_embed_backward, a);
+}
+
+allegro_status_t allegro_force_gather(int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* rev, const void* g_rvec,
+                                      allegro_dtype_t dtype, void* F, void* stream) {
+    ALLEGRO_CHECK_ARG(n_atoms >= 0 && n_edges >= 0, "negative size");
+    ALLEGRO_CHECK_ARG((row_ptr && F) || n_atoms == 0, "row_ptr / F is NULL");
+    ALLEGRO_CHECK_ARG((rev && g_rvec) || n_edges == 0, "rev / g_rvec is NULL");
+    ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
+    return dtype == ALLEGRO_F32 ? launch_force_gather<float>(n_atoms, n_edges, row_ptr, rev, g_rvec, F, (cudaStream_t)stream)
+                                : launch_force_gather<double>(n_atoms, n_edges, row_ptr, rev, g_rvec, F, (cudaStream_t)stream);
+}
+
+allegro_status_t allegro_radial_forward(int n_channels, int n_basis, double r_cut, allegro_dtype_t dtype, long n_edges, const void* rvec,
+                                        const void* W_r, void* w, void* stream) {
+    ALLEGRO_CHECK_ARG(n_channels >= 1 && n_basis >= 1 && n_basis <= 16 && r_cut > 0 && n_edges >= 0, "bad size");
+    ALLEGRO_CHECK_ARG(W_r && ((rvec && w) || n_edges == 0), "NULL argument");
+    ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
+    return dtype == ALLEGRO_F32 ? launch_radial_forward<float>(n_channels, n_basis, r_cut, n_edges, rvec, W_r, w, (cudaStream_t)stream)
+                                : launch_radial_forward<double>(n_channels, n_basis, r_cut, n_edges, rvec, W_r, w, (cudaStream_t)stream);
+}
+allegro_status_t allegro_radial_backward(int n_channels, int n_basis, double r_cut, allegro_dtype_t dtype, long n_edges, const void* rvec,
+                                         const void* W_r, const void* g_w, void* g_rvec, void* stream) {
+    ALLEGRO_CHECK_ARG(n_channels >= 1 && n_basis >= 1 && n_basis <= 16 && r_cut > 0 && n_edges >= 0, "bad size");
+    ALLEGRO_CHECK_ARG(W_r && ((rvec && g_w && g_rvec) || n_edges == 0), "NULL argument");
+    ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
+    return dtype == ALLEGRO_F32
+               ? launch_radial_backward<float>(n_channels, n_basis, r_cut, n_edges, rvec, W_r, g_w, g_rvec, (cudaStream_t)stream)
+               : launch_radial_backward<double>(n_channels, n_basis, r_cut, n_edges, rvec, W_r, g_w, g_rvec, (cudaStream_t)stream);
+}
+
+allegro_status_t allegro_edge_energy(const allegro_plan_t* plan, long n_edges, const void* out, const void* q, double kappa, void* e_edge,
+                                     void* G, void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_edges >= 0, "bad argument");
+    ALLEGRO_CHECK_ARG(q && (out || n_edges == 0), "NULL argument");
+    return plan->dtype == ALLEGRO_F32
+               ? launch_edge_energy<float>(plan->n, plan->tab.dV, n_edges, out, q, kappa, e_edge, G, (cudaStream_t)stream)
+               : launch_edge_energy<double>(plan->n, plan->tab.dV, n_edges, out, q, kappa, e_edge, G, (cudaStream_t)stream);
+}
+
+allegro_status_t allegro_segment_sum(const int32_t* ptr, int n_segments, const void* vals, allegro_dtype_t dtype, void* out, void* stream) {
+    ALLEGRO_CHECK_ARG(n_segments >= 0 && ((ptr && out) || n_segments == 0), "bad argument");
+    ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
+    return dtype == ALLEGRO_F32 ? launch_segment_sum<float>(ptr, n_segments, vals, out, (cudaStream_t)stream)
+                                : launch_segment_sum<double>(ptr, n_segments, vals, out, (cudaStream_t)stream);
+}
+
+const char* allegro_status_str(allegro_status_t s) {
+    switch (s) {
+        case ALLEGRO_OK: return "ALLEGRO_OK";
+        case ALLEGRO_EINVAL: return "ALLEGRO_EINVAL";
+        case ALLEGRO_EUNSUPPORTED: return "ALLEGRO_EUNSUPPORTED";
+        case ALLEGRO_ECUDA: return "ALLEGRO_ECUDA";
+        case ALLEGRO_ENOMEM: return "ALLEGRO_ENOMEM";
+    }
+    return "ALLEGRO_?";
+}
+const char* allegro_last_error(void) { return t_err; }
+long allegro_launch_count(void) { return g_launches.load(); }
+
+}  // extern "C"

@@ -49,18 +49,22 @@ __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
-__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+__device__ __forceinline__ bool mbar_try_wait(uint64_t* bar, uint32_t parity) {
+    uint32_t ok;
     asm volatile(
         "{\n"
         ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)),
-        "r"(parity)
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n"
+        : "=r"(ok)
+        : "r"(smem_u32(bar)), "r"(parity)
         : "memory");
+    return ok != 0;
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+    while (!mbar_try_wait(bar, parity)) {
+    }
 }
 // 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP)
 __device__ __forceinline__ void bulk_load(void* dst_smem, const void* src_gmem, uint32_t bytes, uint64_t* bar) {
@@ -141,5 +145,27 @@ __device__ __forceinline__ void get_item(const int* __restrict__ items, const in
         c = (int)it; e0 = row_ptr[it]; e1 = row_ptr[it + 1];
     }
 }
+
+}  // namespace allegro
+
+namespace allegro {
+
+// Sum the per-item partial rows of every centre in item order (A16): item `it` is the first item of its
+// centre iff it == 0 or the previous item names another centre; that CTA adds the centre's partials
+// sequentially, so the result is independent of scheduling.
+template <typename T>
+__global__ void combine_items_kernel(const int* __restrict__ items, long n_items, int rowlen, const T* __restrict__ partial,
+                                     T* __restrict__ dst) {
+    const long it = blockIdx.x;
+    const int c = items[3 * it];
+    if (it > 0 && items[3 * (it - 1)] == c) return;
+    for (int idx = threadIdx.x; idx < rowlen; idx += blockDim.x) {
+        T acc = T(0);
+        for (long k = it; k < n_items && items[3 * k] == c; ++k) acc += partial[(size_t)k * rowlen + idx];
+        dst[(size_t)c * rowlen + idx] = acc;
+    }
+}
+
+__host__ __device__ static inline uint32_t align128(size_t x) { return (uint32_t)((x + 127) / 128 * 128); }
 
 }  // namespace allegro

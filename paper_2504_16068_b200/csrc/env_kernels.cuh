@@ -1,0 +1,197 @@
+// env_kernels.cuh -- real spherical harmonics fused with the environment embedding and its VJP
+// (north_star; "embedding of edge vectors ... to a radial-chemical and spherical harmonics basis").
+//
+// Y_lm is never stored: every kernel re-evaluates it from r_e (3 numbers per edge).  The harmonics here
+// are the explicit Cartesian polynomials for l <= 3 in the convention of reading A1 (real,
+// component-normalised, m = -l..l, Y_1 = sqrt3 (y, z, x)); the oracle uses the Legendre recursion
+// instead, so the two share neither code nor algorithm.
+#pragma once
+#include "common.cuh"
+#include "launch.h"
+
+namespace allegro {
+
+// Y[DE] at the unit vector (x,y,z)
+template <typename T, int L>
+__device__ __forceinline__ void sph_harm(T x, T y, T z, T (&Y)[(L + 1) * (L + 1)]) {
+    Y[0] = T(1);
+    if constexpr (L >= 1) {
+        const T s3 = T(1.7320508075688772935);
+        Y[1] = s3 * y; Y[2] = s3 * z; Y[3] = s3 * x;
+    }
+    if constexpr (L >= 2) {
+        const T s15 = T(3.8729833462074168852), s5h = T(1.1180339887498948482);
+        Y[4] = s15 * x * y;
+        Y[5] = s15 * y * z;
+        Y[6] = s5h * (T(3) * z * z - T(1));
+        Y[7] = s15 * x * z;
+        Y[8] = T(0.5) * s15 * (x * x - y * y);
+    }
+    if constexpr (L >= 3) {
+        const T a = T(2.0916500663351888699);   // sqrt(35/8)
+        const T b = T(10.246950765959598383);   // sqrt(105)
+        const T c = T(1.6201851746019651310);   // sqrt(21/8)
+        const T d = T(1.3228756555322952953);   // sqrt(7)/2
+        const T x2 = x * x, y2 = y * y, z2 = z * z;
+        Y[9] = a * y * (T(3) * x2 - y2);
+        Y[10] = b * x * y * z;
+        Y[11] = c * y * (T(5) * z2 - T(1));
+        Y[12] = d * z * (T(5) * z2 - T(3));
+        Y[13] = c * x * (T(5) * z2 - T(1));
+        Y[14] = T(0.5) * b * z * (x2 - y2);
+        Y[15] = a * x * (x2 - T(3) * y2);
+    }
+}
+
+// g[a] = sum_j gY[j] dY_j/du_a with (x,y,z) treated as independent variables (J~^T gY).  Any other
+// polynomial extension off the sphere differs by a radial term that the projection below removes.
+template <typename T, int L>
+__device__ __forceinline__ void sph_harm_vjp(T x, T y, T z, const T (&gY)[(L + 1) * (L + 1)], T (&g)[3]) {
+    g[0] = g[1] = g[2] = T(0);
+    if constexpr (L >= 1) {
+        const T s3 = T(1.7320508075688772935);
+        g[1] += s3 * gY[1]; g[2] += s3 * gY[2]; g[0] += s3 * gY[3];
+    }
+    if constexpr (L >= 2) {
+        const T s15 = T(3.8729833462074168852), s5 = T(2.2360679774997896964);
+        g[0] += s15 * (y * gY[4] + z * gY[7] + x * gY[8]);
+        g[1] += s15 * (x * gY[4] + z * gY[5] - y * gY[8]);
+        g[2] += s15 * (y * gY[5] + x * gY[7]) + T(3) * s5 * z * gY[6];
+    }
+    if constexpr (L >= 3) {
+        const T a = T(2.0916500663351888699), b = T(10.246950765959598383), c = T(1.6201851746019651310), d = T(1.3228756555322952953);
+        const T x2 = x * x, y2 = y * y, z2 = z * z;
+        const T f = T(5) * z2 - T(1);
+        g[0] += a * (T(6) * x * y * gY[9] + T(3) * (x2 - y2) * gY[15]) + b * (y * z * gY[10] + x * z * gY[14]) + c * f * gY[13];
+        g[1] += a * (T(3) * (x2 - y2) * gY[9] - T(6) * x * y * gY[15]) + b * (x * z * gY[10] - y * z * gY[14]) + c * f * gY[11];
+        g[2] += b * (x * y * gY[10] + T(0.5) * (x2 - y2) * gY[14]) + c * T(10) * z * (y * gY[11] + x * gY[13]) + d * (T(15) * z2 - T(3)) * gY[12];
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Eenv[i][ch][j] = scale * sum_{e in item, CSR order per slot} w[e][ch] Y_j(rhat_e); slots combined in slot order.
+// One CTA per item; thread <-> (edge slot, channel).  With `by_item` the row goes to the item's partial row.
+template <typename T, int L, int THREADS>
+__global__ void __launch_bounds__(THREADS) env_embed_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
+                                                             const T* __restrict__ rvec, const T* __restrict__ w, T scale,
+                                                             T* __restrict__ dst, int by_item) {
+    constexpr int DE = (L + 1) * (L + 1);
+    __shared__ T red[THREADS * DE];
+    const int tid = threadIdx.x;
+    const int nslots = THREADS / n;
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = slot < nslots;
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    T acc[DE];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) acc[j] = T(0);
+    if (active) {
+        for (int e = e0 + slot; e < e1; e += nslots) {
+            const T rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+            const T wv = w[(size_t)e * n + ch];
+            const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+            T Y[DE];
+            sph_harm<T, L>(rx * inv, ry * inv, rz * inv, Y);
+#pragma unroll
+            for (int j = 0; j < DE; ++j) acc[j] = fma(wv, Y[j], acc[j]);
+        }
+#pragma unroll
+        for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = acc[j];
+    }
+    __syncthreads();
+    if (slot == 0) {
+        T* o = dst + ((size_t)(by_item ? (long)blockIdx.x : (long)c) * n + ch) * DE;
+#pragma unroll
+        for (int j = 0; j < DE; ++j) {
+            T s = red[(size_t)ch * DE + j];
+            for (int sl = 1; sl < nslots; ++sl) s += red[((size_t)sl * n + ch) * DE + j];
+            o[j] = scale * s;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// VJP of the embedding.  One CTA per centre; the centre's gEenv row (times scale) stays in registers.
+//   g_w[e][ch] = sum_j gE[ch][j] Y_j(e)
+//   gY_e[j]   = sum_ch gE[ch][j] w[e][ch]   -- fixed-shape reduction over channels: a warp xor tree when the
+//               slot's channels fill whole warps (n % 32 == 0), then the slot's warps in order; otherwise the
+//               channels of the slot in order.
+//   g_r[e]    = (1/|r|)(I - rhat rhat^T) J~^T gY_e
+template <typename T, int L, int THREADS>
+__global__ void __launch_bounds__(THREADS) env_embed_bwd_kernel(int n, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
+                                                                 const T* __restrict__ rvec, const T* __restrict__ w, T scale,
+                                                                 T* __restrict__ g_rvec, T* __restrict__ g_w) {
+    constexpr int DE = (L + 1) * (L + 1);
+    __shared__ T red[THREADS * DE];  // [slot][ch or warp][DE]
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int nslots = THREADS / n;
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = slot < nslots;
+    const bool warp_tree = (n % 32) == 0;
+    const int c = blockIdx.x;
+    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+    const int ntiles = (e1 - e0 + nslots - 1) / nslots;
+    T gE[DE];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) gE[j] = T(0);
+    if (active) {
+        const T* gr = gEenv + ((size_t)c * n + ch) * DE;
+#pragma unroll
+        for (int j = 0; j < DE; ++j) gE[j] = scale * gr[j];
+    }
+    for (int t = 0; t < ntiles; ++t) {
+        const int e = e0 + t * nslots + slot;
+        const bool valid = active && e < e1;
+        T x = T(0), y = T(0), z = T(1), inv = T(1), wv = T(0);
+        if (valid) {
+            const T rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+            inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+            x = rx * inv; y = ry * inv; z = rz * inv;
+            wv = w[(size_t)e * n + ch];
+        }
+        T Y[DE];
+        sph_harm<T, L>(x, y, z, Y);
+        T gw = T(0);
+        T part[DE];
+#pragma unroll
+        for (int j = 0; j < DE; ++j) { gw = fma(gE[j], Y[j], gw); part[j] = gE[j] * wv; }
+        if (valid && g_w) g_w[(size_t)e * n + ch] = gw;
+        if (warp_tree) {
+#pragma unroll
+            for (int j = 0; j < DE; ++j) {
+                T a = part[j];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                part[j] = a;
+            }
+            if (lane == 0 && active) {
+#pragma unroll
+                for (int j = 0; j < DE; ++j) red[((size_t)slot * (n >> 5) + (ch >> 5)) * DE + j] = part[j];
+            }
+        } else if (active) {
+#pragma unroll
+            for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = part[j];
+        }
+        __syncthreads();
+        if (valid && ch == 0) {
+            const int cnt = warp_tree ? (n >> 5) : n;
+            T gY[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) {
+                T s = red[((size_t)slot * cnt) * DE + j];
+                for (int q = 1; q < cnt; ++q) s += red[((size_t)slot * cnt + q) * DE + j];
+                gY[j] = s;
+            }
+            T g[3];
+            sph_harm_vjp<T, L>(x, y, z, gY, g);
+            const T dot = g[0] * x + g[1] * y + g[2] * z;
+            g_rvec[3 * (size_t)e] = (g[0] - dot * x) * inv;
+            g_rvec[3 * (size_t)e + 1] = (g[1] - dot * y) * inv;
+            g_rvec[3 * (size_t)e + 2] = (g[2] - dot * z) * inv;
+        }
+        __syncthreads();
+    }
+}
+
+}  // namespace allegro

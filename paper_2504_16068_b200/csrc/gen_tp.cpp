@@ -118,6 +118,13 @@ static void emit(FILE* f, int L) {
         }
         fprintf(f, "    }\n");
     }
+    // ---------------- per-non-zero tables for the fold kernel (combined tensor = path weight x CG)
+    fprintf(f, "    static __host__ __device__ constexpr int zpath(int z) { constexpr int v[%zu] = {", t.nnz.size());
+    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%d%s", t.nnz[z].path, z + 1 == t.nnz.size() ? "" : ",");
+    fprintf(f, "}; return v[z]; }\n");
+    fprintf(f, "    static __host__ __device__ constexpr double zcoef(int z) { constexpr double v[%zu] = {", t.nnz.size());
+    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%.17g%s", t.nnz[z].c, z + 1 == t.nnz.size() ? "" : ",");
+    fprintf(f, "}; return v[z]; }\n");
     // ---------------- small integer tables for the dense mix
     fprintf(f, "    // t-slot offset of each path, and the out block it mixes into\n");
     fprintf(f, "    static __host__ __device__ constexpr int toff(int p) { constexpr int v[%d] = {", P + 1);

@@ -1,0 +1,81 @@
+// launch.h -- argument packs and launcher declarations shared by api.cu (dispatch) and the
+// per-(dtype, l_max) instantiation units inst_tp.cu / inst_env.cu.  Internal, not part of the ABI.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstddef>
+#include <cstdint>
+
+#include "allegro_b200.h"
+#include "plan.h"
+
+namespace allegro {
+
+struct EnvArgs {
+    int n, n_atoms;
+    long n_edges;
+    const int32_t* row_ptr;
+    const int32_t* items;  // nullable
+    long n_items;          // number of CTAs' worth of work (== n_atoms when items == nullptr)
+    const void* rvec;
+    const void* w;
+    double scale;
+    void* Eenv;
+    void* ws;
+    cudaStream_t st;
+};
+struct EnvBwdArgs {
+    int n, n_atoms;
+    long n_edges;
+    const int32_t* row_ptr;
+    const void* gEenv;
+    const void* rvec;
+    const void* w;
+    double scale;
+    void* g_rvec;
+    void* g_w;  // nullable
+    cudaStream_t st;
+};
+struct TpArgs {
+    const allegro_plan* plan;
+    int n, n_atoms;
+    long n_edges;
+    const int32_t* row_ptr;
+    const int32_t* items;  // nullable
+    long n_items;
+    const void* V;
+    const void* Eenv;
+    const void* path_w;
+    void* out;  // forward
+    // backward
+    const void* G;
+    void* gV;        // nullable
+    void* gEenv;     // required
+    void* g_path_w;  // nullable
+    void* ws;
+    size_t ws_bytes;
+    cudaStream_t st;
+};
+
+template <typename T, int L> allegro_status_t launch_env_embed(const EnvArgs& a);
+template <typename T, int L> allegro_status_t launch_env_embed_backward(const EnvBwdArgs& a);
+template <typename T, int L> allegro_status_t launch_tp_forward(const TpArgs& a);
+template <typename T, int L> allegro_status_t launch_tp_backward(const TpArgs& a);
+template <typename T, int L> size_t tp_backward_workspace(int n, int n_atoms, long n_items, bool have_items, int wmode, bool want_gw);
+
+// dtype-only helpers (misc.cu)
+template <typename T>
+allegro_status_t launch_radial_forward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, void* w, cudaStream_t st);
+template <typename T>
+allegro_status_t launch_radial_backward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, const void* g_w, void* g_rvec,
+                                        cudaStream_t st);
+template <typename T>
+allegro_status_t launch_force_gather(int n_atoms, long E, const int32_t* row_ptr, const int32_t* rev, const void* g_rvec, void* F, cudaStream_t st);
+template <typename T>
+allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, const void* q, double kappa, void* e_edge, void* G, cudaStream_t st);
+template <typename T>
+allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st);
+
+static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+}  // namespace allegro

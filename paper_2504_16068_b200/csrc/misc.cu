@@ -1,0 +1,193 @@
+// misc.cu -- dtype-only helpers of the hot path: radial weights and their chain rule (A8), force
+// assembly (a7), the scalar edge energy of the VJP tests / benchmarks (A12) and the segment sum (A20).
+#include "common.cuh"
+#include "launch.h"
+
+namespace allegro {
+
+constexpr int kMaxBasis = 16;
+constexpr double kPiD = 3.14159265358979323846264338327950288;
+
+// Bessel basis times polynomial cutoff and its derivative w.r.t. |r|, evaluated in double for either dtype
+// (the embedding is "largely in double-precision"); cost is per edge, not per channel.
+//   x = r/rc, B_b = sqrt(2/rc) sin(b pi x)/r, u = 1 - 28x^6 + 48x^7 - 21x^8
+__device__ __forceinline__ void radial_basis(double r, double rc, int nb, double* Bu, double* dBu) {
+    const double x = r / rc;
+    const double x2 = x * x, x5 = x2 * x2 * x, x6 = x5 * x, x7 = x6 * x, x8 = x7 * x;
+    double u = 1.0 - 28.0 * x6 + 48.0 * x7 - 21.0 * x8;
+    double du = (-168.0 * x5 + 336.0 * x6 - 168.0 * x7) / rc;
+    if (x >= 1.0) { u = 0.0; du = 0.0; }
+    const double pre = sqrt(2.0 / rc), ir = 1.0 / r;
+    for (int b = 1; b <= nb; ++b) {
+        const double k = b * kPiD / rc;
+        double sn, cs;
+        sincos(k * r, &sn, &cs);
+        const double B = pre * sn * ir;
+        const double dB = pre * (k * cs * ir - sn * ir * ir);
+        Bu[b - 1] = B * u;
+        if (dBu) dBu[b - 1] = dB * u + B * du;
+    }
+}
+
+constexpr int kRadEdges = 32;  // edges per CTA
+
+// w[e][ch] = sum_b W_r[ch][b] B_b(r_e) u(r_e/rc)
+template <typename T>
+__global__ void __launch_bounds__(256) radial_fwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_r,
+                                                          T* __restrict__ w) {
+    __shared__ double Bs[kRadEdges][kMaxBasis];
+    const long eb = (long)blockIdx.x * kRadEdges;
+    const int cnt = (int)min((long)kRadEdges, E - eb);
+    if ((int)threadIdx.x < cnt) {
+        const long e = eb + threadIdx.x;
+        const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
+        double Bu[kMaxBasis];
+        radial_basis(sqrt(rx * rx + ry * ry + rz * rz), rc, nb, Bu, nullptr);
+        for (int b = 0; b < nb; ++b) Bs[threadIdx.x][b] = Bu[b];
+    }
+    __syncthreads();
+    for (int idx = threadIdx.x; idx < cnt * n; idx += 256) {
+        const int le = idx / n, ch = idx - le * n;
+        double s = 0.0;
+        for (int b = 0; b < nb; ++b) s += (double)W_r[ch * nb + b] * Bs[le][b];
+        w[(size_t)(eb + le) * n + ch] = (T)s;
+    }
+}
+
+// g_rvec[e] += (sum_ch g_w[e][ch] dw[e][ch]/dr) rhat_e.  One warp per edge; channels summed by lane-strided
+// partial sums and a fixed xor tree.
+template <typename T>
+__global__ void __launch_bounds__(256) radial_bwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_r,
+                                                          const T* __restrict__ g_w, T* __restrict__ g_rvec) {
+    const long e = (long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (e >= E) return;
+    const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
+    const double r = sqrt(rx * rx + ry * ry + rz * rz);
+    double Bu[kMaxBasis], dBu[kMaxBasis];
+    radial_basis(r, rc, nb, Bu, dBu);
+    double acc = 0.0;
+    for (int ch = lane; ch < n; ch += 32) {
+        double dw = 0.0;
+        for (int b = 0; b < nb; ++b) dw += (double)W_r[ch * nb + b] * dBu[b];
+        acc += (double)g_w[(size_t)e * n + ch] * dw;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane < 3) {
+        const double comp = lane == 0 ? rx : (lane == 1 ? ry : rz);
+        g_rvec[3 * e + lane] = (T)((double)g_rvec[3 * e + lane] + acc * comp / r);
+    }
+}
+
+// F[a] = sum_{e in row a} (g_r[e] - g_r[rev[e]]): one warp per atom, lane-strided partial sums in CSR
+// order, fixed xor tree (deterministic; no atomics).
+template <typename T>
+__global__ void __launch_bounds__(256) force_gather_kernel(int n_atoms, const int* __restrict__ row_ptr, const int* __restrict__ rev,
+                                                            const T* __restrict__ g_rvec, T* __restrict__ F) {
+    const int a = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (a >= n_atoms) return;
+    T f0 = T(0), f1 = T(0), f2 = T(0);
+    for (int e = row_ptr[a] + lane; e < row_ptr[a + 1]; e += 32) {
+        const size_t r = (size_t)rev[e];
+        f0 += g_rvec[3 * (size_t)e] - g_rvec[3 * r];
+        f1 += g_rvec[3 * (size_t)e + 1] - g_rvec[3 * r + 1];
+        f2 += g_rvec[3 * (size_t)e + 2] - g_rvec[3 * r + 2];
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        f0 += __shfl_xor_sync(0xffffffffu, f0, o);
+        f1 += __shfl_xor_sync(0xffffffffu, f1, o);
+        f2 += __shfl_xor_sync(0xffffffffu, f2, o);
+    }
+    if (lane == 0) { F[3 * (size_t)a] = f0; F[3 * (size_t)a + 1] = f1; F[3 * (size_t)a + 2] = f2; }
+}
+
+// e_edge[e] = sum_ch ( q[ch] out[e][ch][0] + kappa/2 sum_k out[e][ch][k]^2 ),  G = q (x) delta_{k,0} + kappa out.
+// One warp per edge; lanes stride over the n*dV contiguous elements (coalesced), fixed xor tree.
+template <typename T>
+__global__ void __launch_bounds__(256) edge_energy_kernel(int n, int dV, long E, const T* __restrict__ out, const T* __restrict__ q, T kappa,
+                                                           T* __restrict__ e_edge, T* __restrict__ G) {
+    const long e = (long)blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (e >= E) return;
+    const int len = n * dV;
+    const T* o = out + (size_t)e * len;
+    T* g = G ? G + (size_t)e * len : nullptr;
+    T acc = T(0);
+    for (int idx = lane; idx < len; idx += 32) {
+        const T v = o[idx];
+        const int ch = idx / dV, k = idx - ch * dV;
+        T gv = kappa * v;
+        acc = fma(T(0.5) * gv, v, acc);
+        if (k == 0) { const T qc = q[ch]; acc = fma(qc, v, acc); gv += qc; }
+        if (g) g[idx] = gv;
+    }
+#pragma unroll
+    for (int o2 = 16; o2 > 0; o2 >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o2);
+    if (lane == 0 && e_edge) e_edge[e] = acc;
+}
+
+// out[s] = sum_{i in [ptr[s], ptr[s+1])} vals[i]: one warp per segment, lane-strided, fixed xor tree, double accumulator
+template <typename T>
+__global__ void __launch_bounds__(256) segment_sum_kernel(const int* __restrict__ ptr, int nseg, const T* __restrict__ vals, T* __restrict__ out) {
+    const int s = blockIdx.x * 8 + (threadIdx.x >> 5);
+    const int lane = threadIdx.x & 31;
+    if (s >= nseg) return;
+    double acc = 0.0;
+    for (int i = ptr[s] + lane; i < ptr[s + 1]; i += 32) acc += (double)vals[i];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if (lane == 0) out[s] = (T)acc;
+}
+
+// ------------------------------------------------------------------------------------------------ launchers
+template <typename T>
+allegro_status_t launch_radial_forward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, void* w, cudaStream_t st) {
+    if (E == 0) return ALLEGRO_OK;
+    radial_fwd_kernel<T><<<(unsigned)((E + kRadEdges - 1) / kRadEdges), 256, 0, st>>>(n, nb, rc, E, (const T*)rvec, (const T*)W_r, (T*)w);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+template <typename T>
+allegro_status_t launch_radial_backward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, const void* g_w, void* g_rvec,
+                                        cudaStream_t st) {
+    if (E == 0) return ALLEGRO_OK;
+    radial_bwd_kernel<T><<<(unsigned)((E + 7) / 8), 256, 0, st>>>(n, nb, rc, E, (const T*)rvec, (const T*)W_r, (const T*)g_w, (T*)g_rvec);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+template <typename T>
+allegro_status_t launch_force_gather(int n_atoms, long E, const int32_t* row_ptr, const int32_t* rev, const void* g_rvec, void* F, cudaStream_t st) {
+    (void)E;
+    if (n_atoms == 0) return ALLEGRO_OK;
+    force_gather_kernel<T><<<(unsigned)((n_atoms + 7) / 8), 256, 0, st>>>(n_atoms, row_ptr, rev, (const T*)g_rvec, (T*)F);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+template <typename T>
+allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, const void* q, double kappa, void* e_edge, void* G, cudaStream_t st) {
+    if (E == 0) return ALLEGRO_OK;
+    edge_energy_kernel<T><<<(unsigned)((E + 7) / 8), 256, 0, st>>>(n, dV, E, (const T*)out, (const T*)q, (T)kappa, (T*)e_edge, (T*)G);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+template <typename T>
+allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st) {
+    if (nseg == 0) return ALLEGRO_OK;
+    segment_sum_kernel<T><<<(unsigned)((nseg + 7) / 8), 256, 0, st>>>(ptr, nseg, (const T*)vals, (T*)out);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
+#define ALLEGRO_INST(T)                                                                                                               \
+    template allegro_status_t launch_radial_forward<T>(int, int, double, long, const void*, const void*, void*, cudaStream_t);        \
+    template allegro_status_t launch_radial_backward<T>(int, int, double, long, const void*, const void*, const void*, void*, cudaStream_t); \
+    template allegro_status_t launch_force_gather<T>(int, long, const int32_t*, const int32_t*, const void*, void*, cudaStream_t);    \
+    template allegro_status_t launch_edge_energy<T>(int, int, long, const void*, const void*, double, void*, void*, cudaStream_t);    \
+    template allegro_status_t launch_segment_sum<T>(const int32_t*, int, const void*, void*, cudaStream_t);
+ALLEGRO_INST(float)
+ALLEGRO_INST(double)
+
+}  // namespace allegro

@@ -1,0 +1,170 @@
+"""GPU parity: the CUDA library (through the C ABI) against the float64 oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json:north_star's (reading A10): per tensor
+max|d| <= 1e-5 max|ref| (fp32), 1e-11 (fp64); forces <= 1e-4 relative RMS (fp32); integers bit-exact."""
+import numpy as np
+import pytest
+
+import _chain
+
+pytestmark = pytest.mark.gpu
+
+KEYS = ("w", "Eenv", "out", "e_edge", "G", "gV", "gEenv", "g_path_w", "g_w", "g_r_env", "g_r", "F", "E_mol")
+
+
+def _assert_close(ref, got, dt, keys=KEYS, rows=None, label=""):
+    errs = _chain.compare(ref, got, dt, keys, rows)
+    tol = _chain.TOL[dt]
+    bad = {k: v for k, v in errs.items() if not v <= tol}
+    assert not bad, "%s: over tolerance %g: %s (all: %s)" % (label, tol, bad, errs)
+    if "F" in errs and "F" in ref:
+        F = got["F"].cpu().numpy().astype(np.float64)
+        rms = np.linalg.norm(F - ref["F"]) / np.linalg.norm(ref["F"])
+        assert rms <= _chain.FORCE_RMS_TOL[dt], "%s: force relative RMS %g" % (label, rms)
+    return errs
+
+
+# C0 is BASELINE.json:configs[0] in full; the *s variants are the other configs' recipes at sizes the oracle
+# finishes in seconds (they still span many tiles and ragged tails: degrees are not multiples of the slot count)
+@pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
+def test_chain_matches_oracle(name):
+    inp = _chain.make_inputs(name)
+    ref = _chain.oracle_chain(inp)
+    got = _chain.gpu_chain(inp)
+    errs = _assert_close(ref, got, inp["dt"], label=name)
+    print(name, {k: "%.2e" % v for k, v in errs.items()})
+    # sum of forces vanishes (Newton's third law: every edge has its reverse)
+    F = got["F"].cpu().numpy().astype(np.float64)
+    assert np.abs(F.sum(0)).max() <= 1e-3 * np.abs(F).max() * (1.0 if inp["dt"] == np.float32 else 1e-8)
+
+
+def test_c4_fp64_variant():
+    """configs[4] asks for fp32 and fp64: the same molecule batch in double"""
+    inp = _chain.make_inputs("C4s")
+    for k in ("rvec", "V", "W_r", "path_w", "q"):
+        inp[k] = inp[k].astype(np.float64)      # the fp32-rounded values, promoted: same numbers as the fp32 run
+    inp["dt"] = np.float64
+    ref = _chain.oracle_chain(inp)
+    got = _chain.gpu_chain(inp)
+    _assert_close(ref, got, np.float64, label="C4s/f64")
+
+
+@pytest.mark.parametrize("name,T", [("C0", 5), ("C1s", 32), ("C4s", 7)])
+def test_segment_items_split_centres(name, T):
+    """A16: centres split over several items (tile_edges below the degree) give the same result as one item
+    per centre; partial sums are combined in item order"""
+    import oracle as orc
+    import paper_2504_16068_b200 as ab
+    inp = _chain.make_inputs(name)
+    items = ab.segments_build(inp["row_ptr"], T)
+    assert np.array_equal(items, orc.segments(inp["row_ptr"], T))          # integer plan: bit-exact
+    assert items.shape[0] > inp["N"]
+    ref = _chain.oracle_chain(inp)
+    got = _chain.gpu_chain(inp, items=items)
+    _assert_close(ref, got, inp["dt"], label="%s/T=%d" % (name, T))
+
+
+def test_bitwise_determinism():
+    """no float atomics anywhere: two runs give identical bits (reading A11)"""
+    import torch
+    inp = _chain.make_inputs("C1s")
+    dev = _chain.to_device(inp)
+    a = _chain.gpu_chain(inp, dev)
+    b = _chain.gpu_chain(inp, dev)
+    for k in a:
+        if a[k] is not None:
+            assert torch.equal(a[k], b[k]), k
+
+
+def test_empty_and_degenerate_graphs():
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    plan = ab.Plan(2, 32, ab.F32)
+    dev = "cuda"
+    # (i) no atoms, no edges
+    rp = torch.zeros(1, dtype=torch.int32, device=dev)
+    z3 = torch.zeros((0, 3), device=dev)
+    zV = torch.zeros((0, 32, 18), device=dev)
+    zw = torch.zeros((0, 32), device=dev)
+    pw = torch.ones(30, device=dev)
+    E = ab.env_embed(plan, rp, z3, zw)
+    assert E.shape == (0, 32, 9)
+    out = ab.tp_forward(plan, rp, zV, E, pw)
+    gV, gE, gpw = ab.tp_backward(plan, rp, zV, zV, E, pw, want_g_path_w=True)
+    assert out.shape[0] == 0 and float(gpw.abs().sum()) == 0.0
+    # (ii) atoms without neighbours (degree 0) between atoms with neighbours
+    rp = torch.tensor([0, 0, 3, 3, 5, 5], dtype=torch.int32, device=dev)
+    g = torch.Generator(device="cpu").manual_seed(1)
+    rvec = torch.randn((5, 3), generator=g).to(dev)
+    w = torch.randn((5, 32), generator=g).to(dev)
+    V = torch.randn((5, 32, 18), generator=g).to(dev)
+    E = ab.env_embed(plan, rp, rvec, w)
+    assert float(E[0].abs().sum()) == 0.0 and float(E[2].abs().sum()) == 0.0 and float(E[4].abs().sum()) == 0.0
+    out = ab.tp_forward(plan, rp, V, E, pw)
+    gV, gE, _ = ab.tp_backward(plan, rp, out, V, E, pw)
+    assert float(gE[0].abs().sum()) == 0.0 and float(gE[4].abs().sum()) == 0.0
+    assert torch.isfinite(out).all() and torch.isfinite(gV).all() and torch.isfinite(gE).all()
+    import oracle as orc
+    ref = orc.tp_forward(2, rp.cpu().numpy(), V.cpu().numpy(), E.cpu().numpy(), pw.cpu().numpy())
+    assert np.max(np.abs(ref - out.cpu().numpy())) <= 1e-5 * np.max(np.abs(ref))
+
+
+def test_unsupported_and_bad_arguments_fail_loudly():
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    plan = ab.Plan(2, 3, ab.F32)      # 3 channels x 18 comps x 4 B = 216 B rows: not a multiple of 16
+    rp = torch.tensor([0, 1], dtype=torch.int32, device="cuda")
+    V = torch.zeros((1, 3, 18), device="cuda")
+    E = torch.zeros((1, 3, 9), device="cuda")
+    pw = torch.ones(30, device="cuda")
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_forward(plan, rp, V, E, pw)
+    assert ei.value.status == 2
+    plan = ab.Plan(2, 32, ab.F32)
+    V = torch.zeros((1, 32, 18), device="cuda")
+    E = torch.zeros((1, 32, 9), device="cuda")
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_forward(plan, rp, V, E, pw, out=V)      # aliasing
+    assert ei.value.status == 1
+    with pytest.raises(ab.AllegroError) as ei:        # workspace too small
+        ab.tp_backward(plan, rp, V, V.clone(), E, pw, want_g_path_w=True, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+    assert ei.value.status == 4
+
+
+def _check_sampled_centres(inp, got, ranges, label):
+    """oracle on self-contained sub-problems (workloads.inputs.sub_inputs) vs the matching rows of the GPU result"""
+    from workloads.inputs import sub_inputs
+    edge_keys = ("w", "out", "e_edge", "G", "gV", "g_w", "g_r_env", "g_r")
+    for c0, c1 in ranges:
+        sub = sub_inputs(inp, c0, c1)
+        ref = _chain.oracle_chain(sub, want_gw=False, forces=False)
+        e0, e1 = sub["edge_range"]
+        part = {k: got[k][e0:e1] for k in edge_keys}
+        part.update(Eenv=got["Eenv"][c0:c1], gEenv=got["gEenv"][c0:c1])
+        _assert_close(ref, part, inp["dt"], keys=edge_keys + ("Eenv", "gEenv"), label="%s centres [%d,%d)" % (label, c0, c1))
+
+
+def _check_force_gather(inp, got):
+    """F against a float64 host re-summation of the GPU's own g_r (integer gather + sum: size-independent property)"""
+    g_r = got["g_r"].cpu().numpy().astype(np.float64)
+    contrib = g_r - g_r[inp["rev"]]
+    centre = np.repeat(np.arange(inp["N"]), np.diff(inp["row_ptr"]))
+    Fref = np.zeros((inp["N"], 3))
+    np.add.at(Fref, centre, contrib)
+    F = got["F"].cpu().numpy().astype(np.float64)
+    assert np.max(np.abs(F - Fref)) <= _chain.TOL[inp["dt"]] * np.max(np.abs(Fref))
+    assert np.abs(F.sum(0)).max() <= 1e-3 * np.abs(F).max()
+
+
+def test_c1_full_size_sampled_centres():
+    """BASELINE.json:configs[1] at full size in the launch configuration bench.py times (V drawn in device memory);
+    the oracle evaluates seeded centre ranges with their complete neighbourhoods, which is exact because every
+    per-edge / per-centre output depends on one centre only."""
+    from workloads import rng
+    inp = _chain.make_inputs("C1", features="device")
+    got = _chain.gpu_chain(inp, want_gw=False)
+    N = inp["N"]
+    starts = [int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(3), 0, N - 17)]
+    _check_sampled_centres(inp, got, [(c, c + 16) for c in starts + [0, N - 16]], "C1")
+    _check_force_gather(inp, got)
