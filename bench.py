@@ -1,0 +1,294 @@
+"""bench.py -- BASELINE.json's metric on a B200: edges/s of one Allegro tensor-product layer, forward + force VJP
+(fp32, l_max = 2, n = 64) on BASELINE.json:configs[1] (4,096 atoms, ~370k directed edges), seeded synthetic input.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--workload C1|C1s|C4|C3m]
+    torchrun --nnodes=1 --nproc-per-node N ... bench.py --gpus N ...     (one rank per GPU)
+
+A "step" is one pass of the whole hot path (all rows) over one system: radial weights -> Y_lm +
+environment embedding -> tensor product -> edge energy / cotangent -> tensor-product VJP (gV, gEenv) ->
+embedding VJP -> radial chain rule -> force gather -> energy sum.  Every step runs in the library's CUDA kernels.
+
+One JSON line on stdout (rank 0).  `value` = device-timed (CUDA events) edges/s with inputs resident in HBM;
+`e2e` = the same step called with HOST buffers (pinned): H2D of the step's inputs and D2H of forces + energy are
+inside the timed region; `roofline` = the dominant kernel's algorithmic bytes / its CUDA-event time over the
+timed steps, against MEASURED_PEAKS.json; `cpu_baseline` = the float64 oracle timed on the host cores on a
+bounded sample of the same workload.  --impl reference times the oracle alone (rank 0 only).
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+for _p in (ROOT, os.path.join(ROOT, "tests")):
+    if _p not in sys.path:
+        sys.path.insert(0, _p)
+
+METRIC = "edges/s for Allegro TP fwd+force-VJP (fp32, l_max=2, n=64)"
+UNIT = "edges/s"
+FALLBACK_HBM_GBS = 6650.0     # B200_PROFILING.md fallback when MEASURED_PEAKS.json is absent
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="C1")
+    ap.add_argument("--force-only", action="store_true", help="skip dE/dV (valid when V does not depend on positions)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    return ap.parse_args()
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q, "--format=csv,noheader,nounits",
+                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for ln in self.proc.stdout:
+            self.lines.append(ln.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2], "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------------ oracle arm
+def _oracle_sample_step(inp, n_centres):
+    """One oracle step (the chain of tests/_chain.oracle_chain without forces) on the first n_centres centres with
+    their complete neighbourhoods (exact sub-problem: every per-edge / per-centre quantity depends on one centre)."""
+    import _chain
+    from workloads.inputs import sub_inputs
+    sub = sub_inputs(inp, 0, n_centres)
+    t0 = time.perf_counter()
+    _chain.oracle_chain(sub, want_gw=False, forces=False)
+    return sub["E"], time.perf_counter() - t0
+
+
+def cpu_baseline(inp, seconds):
+    """The float64 oracle, as it stands, on a bounded sample: calibrate on 4 centres, then size the sample for
+    about `seconds` of single-threaded CPU work."""
+    N = inp["N"]
+    e_cal, t_cal = _oracle_sample_step(inp, min(4, N))
+    rate = e_cal / max(t_cal, 1e-9)
+    deg = inp["E"] / max(N, 1)
+    nc = int(max(4, min(N, rate * seconds / deg)))
+    e, t = _oracle_sample_step(inp, nc)
+    return {"value": e / t, "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": "float64 C++ oracle chain (radial, env-embed, TP fwd, energy, TP VJP, env VJP; no force gather) on the first "
+                      "%d centres = %d edges of %s, %.1f s, single thread" % (nc, e, inp["name"], t)}
+
+
+def run_reference(args):
+    """--impl reference: the oracle timed on the host cores, each step a bounded sample of the workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    import oracle
+    oracle.build()
+    from workloads.inputs import make_inputs
+    name = args.workload
+    inp = make_inputs(name, features="lazy")
+    steps = max(1, args.steps)
+    per_step = max(0.5, min(10.0, 120.0 / (steps + args.warmup)))
+    e_cal, t_cal = _oracle_sample_step(inp, 4)
+    nc = int(max(4, min(inp["N"], (e_cal / t_cal) * per_step / (inp["E"] / inp["N"]))))
+    for _ in range(args.warmup):
+        _oracle_sample_step(inp, nc)
+    tot_e, tot_t = 0, 0.0
+    for _ in range(steps):
+        e, t = _oracle_sample_step(inp, nc)
+        tot_e += e
+        tot_t += t
+    v = tot_e / tot_t
+    sample = "first %d centres (%d edges) of %s per step, float64 C++ oracle, single thread" % (nc, tot_e // steps, name)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup,
+        "ms_per_step": 1e3 * tot_t / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": name, "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+# ------------------------------------------------------------------------------------------------ CUDA arm
+def _dist_env():
+    return int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1")), int(os.environ.get("LOCAL_RANK", "0"))
+
+
+def run_ours(args):
+    import numpy as np
+    import torch
+    import torch.distributed as dist
+
+    rank, world, local = _dist_env()
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    torch.cuda.set_device(local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import HostStep, SingleLayerStep, to_device
+    from workloads.inputs import make_inputs
+
+    name = args.workload
+    # multi-GPU: the path partitions over independent systems -- rank r owns the system of seed r;
+    # no data-path collective, weak scaling
+    inp = make_inputs(name, seed=rank, features="device")
+    dev = to_device(inp)
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32, ab.W_SCALAR)
+    step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only)
+    E, N = step.E, step.N
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---------------- device-resident timing
+    for _ in range(max(args.warmup, 3)):
+        step.run()
+    barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    n0 = ab.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    marks = []
+    ev0.record()
+    for _ in range(args.steps):
+        step.run(mark=True)
+        marks.append(step.marks)
+    ev1.record()
+    barrier()
+    launches = ab.launch_count() - n0
+    clk = clocks.stop()
+    ms_total = ev0.elapsed_time(ev1)
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    value = world * E / (ms_step * 1e-3)
+
+    # per-call device time (CUDA events on the launching stream, same timed region)
+    per_call = {}
+    for mk in marks:
+        for nm, a, b in mk:
+            per_call.setdefault(nm, []).append(a.elapsed_time(b))
+    per_call_ms = {k: sum(v) / len(v) for k, v in per_call.items()}
+    abytes = step.algorithmic_bytes()
+    peak, peak_src = measured_peaks()
+    top = max(per_call_ms, key=per_call_ms.get)
+    ach = abytes[top] / (per_call_ms[top] * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
+                "traffic": _ncu_traffic(top), "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top],
+                "ms_per_launch": per_call_ms[top]}
+    step_bytes = sum(abytes.values())
+    calls = {k: {"ms": round(per_call_ms[k], 4), "GB/s": round(abytes[k] / (per_call_ms[k] * 1e-3) / 1e9, 1),
+                 "share": round(per_call_ms[k] / sum(per_call_ms.values()), 4)} for k in per_call_ms}
+
+    # ---------------- end to end: host buffers in, forces + energy out, copies inside the timed region
+    host = HostStep(step, inp)
+    for _ in range(3):
+        host.run()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    k_e2e = max(3, min(args.steps, 10))
+    e0.record()
+    for _ in range(k_e2e):
+        host.run()
+    e1.record()
+    barrier()
+    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e_ms = float(t.item()) / k_e2e
+    e2e = {"value": world * E / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.h2d_bytes, "d2h_bytes_per_step": host.d2h_bytes,
+           "ms_per_step": e2e_ms, "steps": k_e2e}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32" if inp["dt"] == np.float32 else "f64", "data": "synthetic",
+            "config": {"workload": "%s: BASELINE.json configs[1] recipe, %d atoms, %d directed edges per GPU, l_max=%d, n=%d, "
+                                   "single TP layer forward + %s" % (name, N, E, inp["lmax"], inp["n"],
+                                                                     "force-only VJP" if args.force_only else "full VJP (gV, gEenv) + forces"),
+                       "atoms": N, "edges": E, "l_max": inp["lmax"], "n_channels": inp["n"], "parallelism": "independent systems per GPU",
+                       "l2": "not flushed: every feature tensor (%.2f GB) exceeds the 126 MB L2" % (abytes["tp_forward"] / 2 / 1e9)},
+            "atom_steps_per_s": world * N / (ms_step * 1e-3),
+            "step_GBps_algorithmic": step_bytes / (ms_step * 1e-3) / 1e9, "step_frac_of_hbm_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
+            "roofline": roofline, "calls": calls, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
+        }
+        if world == 1 and not args.no_cpu_baseline:
+            import oracle
+            oracle.build()
+            line["cpu_baseline"] = cpu_baseline(inp, args.cpu_seconds)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def _ncu_traffic(kernel):
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.json), or None"""
+    p = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f).get(kernel)
+    return None
+
+
+if __name__ == "__main__":
+    a = parse_args()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_ours(a)

@@ -27,10 +27,13 @@ template <typename T> struct Cfg {
 static inline int pick_stages(size_t stage_bytes, size_t extra) {
     // as many stages (<= 3) as fit next to `extra` in the 227 KB a CTA may use; the wrapper decides the
     // occupancy through the total (several CTAs per SM when the stage is small)
-    const size_t cap = 110 * 1024;  // two CTAs per SM
-    int nst = 3;
-    while (nst > 1 && nst * stage_bytes + extra > cap) --nst;
-    return nst;
+    const size_t cap2 = 110 * 1024;  // two CTAs per SM
+    const size_t cap1 = 220 * 1024;  // one CTA per SM
+    if (3 * stage_bytes + extra <= cap2) return 3;
+    if (2 * stage_bytes + extra <= cap2) return 2;
+    if (3 * stage_bytes + extra <= cap1) return 3;
+    if (2 * stage_bytes + extra <= cap1) return 2;
+    return 1;
 }
 
 template <typename T>

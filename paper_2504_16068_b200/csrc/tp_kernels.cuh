@@ -96,7 +96,9 @@ __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __res
             const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
             bulk_store(out + (size_t)eb * n * DV, smem_raw + (size_t)s * stage_bytes, bytes);
             bulk_commit();
-            if (t >= 1 && t - 1 + NST < ntiles) {
+            if constexpr (NST == 1) {
+                if (t + 1 < ntiles) { bulk_wait_read<0>(); issue(t + 1); }  // single stage: store, then refill
+            } else if (t >= 1 && t - 1 + NST < ntiles) {
                 bulk_wait_read<1>();  // the store of tile t-1 has finished reading its stage
                 issue(t - 1 + NST);
             }
@@ -185,7 +187,9 @@ __global__ void __launch_bounds__(THREADS)
                 const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
                 bulk_store(gV + (size_t)eb * n * DV, st, bytes);
                 bulk_commit();
-                if (t >= 1 && t - 1 + NST < ntiles) {
+                if constexpr (NST == 1) {
+                    if (t + 1 < ntiles) { bulk_wait_read<0>(); issue(t + 1); }
+                } else if (t >= 1 && t - 1 + NST < ntiles) {
                     bulk_wait_read<1>();
                     issue(t - 1 + NST);
                 }

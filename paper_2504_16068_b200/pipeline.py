@@ -43,3 +43,107 @@ def gpu_chain(inp, dev=None, items=None, want_gw=True, plan=None):
     if dev.get("edge_mol_ptr") is not None:
         res["E_mol"] = ab.segment_sum(dev["edge_mol_ptr"], e_edge)
     return res
+
+
+class SingleLayerStep:
+    """One MD step of one tensor-product layer with every buffer allocated once (nothing is allocated and no
+    host synchronisation happens inside run()): the object bench.py times.  `want_gV` selects the full VJP
+    (dE/dV as well, what a layer inside a deeper network needs) or the force-only VJP."""
+
+    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None):
+        self.plan, self.dev, self.rc, self.kappa, self.scale = plan, dev, rc, kappa, scale
+        rp, rvec, V = dev["row_ptr"], dev["rvec"], dev["V"]
+        self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
+        self.items = items
+        dt, dv = rvec.dtype, rvec.device
+        n = plan.n
+        self.w = torch.empty((self.E, n), dtype=dt, device=dv)
+        self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
+        self.out = torch.empty_like(V)
+        self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
+        self.G = torch.empty_like(V)
+        self.gV = torch.empty_like(V) if want_gV else None
+        self.gEenv = torch.empty_like(self.Eenv)
+        self.g_path_w = torch.empty((plan.P,), dtype=dt, device=dv) if want_g_path_w else None
+        self.g_r = torch.empty_like(rvec)
+        self.g_w = torch.empty_like(self.w)
+        self.F = torch.empty((self.N, 3), dtype=dt, device=dv)
+        self.e_tot = torch.empty((1,), dtype=dt, device=dv)
+        self.e_ptr = torch.tensor([0, self.E], dtype=torch.int32, device=dv)
+        self.ws_env = torch.empty(max(ab.env_workspace(plan, self.N, items), 16), dtype=torch.uint8, device=dv)
+        self.ws_bwd = torch.empty(max(ab.tp_backward_workspace(plan, self.N, self.E, items, want_g_path_w), 16), dtype=torch.uint8, device=dv)
+        self.marks = None      # optional list of (name, start_event, end_event) filled by run(mark=True)
+
+    def run(self, mark=False):
+        p, d, it = self.plan, self.dev, self.items
+        rp, rvec, V, pw = d["row_ptr"], d["rvec"], d["V"], d["path_w"]
+        ev = []
+
+        def timed(name, fn):
+            if not mark:
+                return fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            r = fn()
+            b.record()
+            ev.append((name, a, b))
+            return r
+
+        timed("radial_forward", lambda: ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w))
+        timed("env_embed", lambda: ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env))
+        timed("tp_forward", lambda: ab.tp_forward(p, rp, V, self.Eenv, pw, items=it, out=self.out))
+        timed("edge_energy", lambda: ab.edge_energy(p, self.out, d["q"], self.kappa, e_edge=self.e_edge, G=self.G))
+        timed("tp_backward", lambda: ab.tp_backward(p, rp, self.G, V, self.Eenv, pw, items=it, want_gV=self.gV is not None,
+                                                    gV=self.gV, gEenv=self.gEenv, g_path_w=self.g_path_w, workspace=self.ws_bwd))
+        timed("env_embed_backward", lambda: ab.env_embed_backward(p, rp, self.gEenv, rvec, self.w, self.scale, g_rvec=self.g_r, g_w=self.g_w))
+        timed("radial_backward", lambda: ab.radial_backward(rvec, d["W_r"], self.rc, self.g_w, self.g_r))
+        timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
+        timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        if mark:
+            self.marks = ev
+        return self.F, self.e_tot
+
+    def algorithmic_bytes(self):
+        """HBM bytes each call must move at least once: dict name -> bytes per step"""
+        p = self.plan
+        s = 4 if p.dtype == ab.F32 else 8
+        E, N, n, dV, dE = self.E, self.N, p.n, p.dV, p.dE
+        feat, env, wrow = E * n * dV * s, N * n * dE * s, E * n * s
+        return {
+            "radial_forward": E * 3 * s + wrow,
+            "env_embed": E * 3 * s + wrow + env + (N + 1) * 4,
+            "tp_forward": 2 * feat + env + (N + 1) * 4,
+            "edge_energy": 2 * feat + E * s,
+            "tp_backward": (3 if self.gV is not None else 2) * feat + 2 * env + (N + 1) * 4,
+            "env_embed_backward": env + E * 3 * s + wrow + wrow + E * 3 * s + (N + 1) * 4,
+            "radial_backward": E * 3 * s + wrow + 2 * E * 3 * s,
+            "force_gather": 2 * E * 3 * s + E * 4 + N * 3 * s + (N + 1) * 4,
+            "segment_sum": E * s,
+        }
+
+
+class HostStep:
+    """The same step called with HOST buffers: every input of the step (row_ptr, rev, rvec, V) sits in pinned host
+    memory and is copied to the device inside run(); forces and the total energy are copied back to pinned host
+    memory and run() returns after they have arrived.  The small parameter tensors (W_r, path_w, q) stay resident."""
+
+    KEYS = ("row_ptr", "rev", "rvec", "V")
+
+    def __init__(self, step, inp=None):
+        self.step = step
+        d = step.dev
+        self.host = {k: torch.empty(d[k].shape, dtype=d[k].dtype, pin_memory=True).copy_(d[k]) for k in self.KEYS}
+        self.F_host = torch.empty(step.F.shape, dtype=step.F.dtype, pin_memory=True)
+        self.e_host = torch.empty(step.e_tot.shape, dtype=step.e_tot.dtype, pin_memory=True)
+        self.h2d_bytes = int(sum(v.numel() * v.element_size() for v in self.host.values()))
+        self.d2h_bytes = int(self.F_host.numel() * self.F_host.element_size() + self.e_host.numel() * self.e_host.element_size())
+
+    def run(self):
+        d = self.step.dev
+        for k in self.KEYS:
+            d[k].copy_(self.host[k], non_blocking=True)
+        self.step.run()
+        self.F_host.copy_(self.step.F, non_blocking=True)
+        self.e_host.copy_(self.step.e_tot, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+        return self.F_host, self.e_host

@@ -4,6 +4,7 @@ Generated in float64 and rounded ONCE to the config's dtype; both the oracle (wh
 double, reading A9) and the CUDA library consume these arrays.  No arithmetic of the method lives here.
 
 features="host"   : V is a numpy array (small configs).
+features="lazy"   : V is not materialised; sub_inputs() draws the rows it needs (CPU-only timing of a sample).
 features="device" : V is drawn directly in device memory by the torch form of the same counter-based
                     generator (full-size configs: C1 is 1.7 GB, C3 86 GB per tensor); whoever needs exact
                     values on the host (the oracle, for the centres it checks) reads them back with
@@ -26,8 +27,11 @@ def make_inputs(name, seed=0, features="host", device="cuda"):
                W_r=np.ascontiguousarray(wts["W_r"].astype(dt)),
                path_w=np.ascontiguousarray(wts["path_w"].astype(dt)),
                q=np.ascontiguousarray(wts["q"].astype(dt)), kappa=wts["kappa"], scale=1.0)
+    inp["seed"] = seed
     if features == "host":
         inp["V"] = np.ascontiguousarray(configs.features_for(name, E, seed, "V").astype(dt))
+    elif features == "lazy":      # rows are drawn on demand by sub_inputs() (a pure function of the edge index)
+        inp["V"] = None
     else:
         import torch
         dV = 2 * (s["lmax"] + 1) ** 2
@@ -45,7 +49,10 @@ def sub_inputs(inp, c_lo, c_hi):
     Forces are not defined on a sub-problem (reverse edges belong to other centres)."""
     rp = inp["row_ptr"]
     e0, e1 = int(rp[c_lo]), int(rp[c_hi])
-    V = inp["V"][e0:e1]
+    if inp["V"] is None:
+        V = configs.features_for(inp["name"], inp["E"], inp["seed"], "V", e0, e1).astype(inp["dt"])
+    else:
+        V = inp["V"][e0:e1]
     if hasattr(V, "detach"):
         V = V.detach().cpu().numpy()
     sub = dict(inp)
