@@ -112,77 +112,69 @@ __global__ void __launch_bounds__(THREADS) env_embed_kernel(int n, const int* __
 }
 
 // ------------------------------------------------------------------------------------------------
-// VJP of the embedding.  One CTA per centre; the centre's gEenv row (times scale) stays in registers.
+// Sum 16 per-lane values over the 32 lanes of a warp with 16 shuffles instead of 80: at each step a lane
+// hands one half of its live values to its partner and keeps the other half (recursive halving).  On
+// return v[0] of lane l holds the total of input index (l >> 1) & 15.  Fixed shape -> deterministic.
+template <typename T>
+__device__ __forceinline__ void warp_reduce16(T (&v)[16], int lane) {
+#pragma unroll
+    for (int h = 8, bit = 16; h >= 1; h >>= 1, bit >>= 1) {
+        const bool up = (lane & bit) != 0;
+#pragma unroll
+        for (int i = 0; i < h; ++i) {
+            const T send = up ? v[i] : v[i + h];
+            const T keep = up ? v[i + h] : v[i];
+            v[i] = keep + __shfl_xor_sync(0xffffffffu, send, bit);
+        }
+    }
+    v[0] += __shfl_xor_sync(0xffffffffu, v[0], 1);
+}
+
+// VJP of the embedding.  One CTA (8 warps) per centre; warp <-> edge, lane <-> channels lane, lane+32, ...
+// (CPL per lane), so w[e][:] and g_w[e][:] are read / written as whole coalesced rows and the centre's gEenv
+// rows (times scale) stay in registers for the whole segment.  No block barrier.
 //   g_w[e][ch] = sum_j gE[ch][j] Y_j(e)
-//   gY_e[j]   = sum_ch gE[ch][j] w[e][ch]   -- fixed-shape reduction over channels: a warp xor tree when the
-//               slot's channels fill whole warps (n % 32 == 0), then the slot's warps in order; otherwise the
-//               channels of the slot in order.
+//   gY_e[j]   = sum_ch gE[ch][j] w[e][ch]   -- lane-local over the lane's channels, then warp_reduce16
 //   g_r[e]    = (1/|r|)(I - rhat rhat^T) J~^T gY_e
-template <typename T, int L, int THREADS>
-__global__ void __launch_bounds__(THREADS) env_embed_bwd_kernel(int n, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
-                                                                 const T* __restrict__ rvec, const T* __restrict__ w, T scale,
-                                                                 T* __restrict__ g_rvec, T* __restrict__ g_w) {
+template <typename T, int L, int CPL>
+__global__ void __launch_bounds__(256) env_embed_bwd_kernel(int n, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
+                                                             const T* __restrict__ rvec, const T* __restrict__ w, T scale,
+                                                             T* __restrict__ g_rvec, T* __restrict__ g_w) {
     constexpr int DE = (L + 1) * (L + 1);
-    __shared__ T red[THREADS * DE];  // [slot][ch or warp][DE]
-    const int tid = threadIdx.x, lane = tid & 31;
-    const int nslots = THREADS / n;
-    const int slot = tid / n, ch = tid - slot * n;
-    const bool active = slot < nslots;
-    const bool warp_tree = (n % 32) == 0;
+    static_assert(DE <= 16, "warp_reduce16 handles l_max <= 3");
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int c = blockIdx.x;
     const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
-    const int ntiles = (e1 - e0 + nslots - 1) / nslots;
-    T gE[DE];
+    T gE[CPL][DE];
 #pragma unroll
-    for (int j = 0; j < DE; ++j) gE[j] = T(0);
-    if (active) {
-        const T* gr = gEenv + ((size_t)c * n + ch) * DE;
+    for (int q = 0; q < CPL; ++q) {
+        const int ch = lane + 32 * q;
 #pragma unroll
-        for (int j = 0; j < DE; ++j) gE[j] = scale * gr[j];
+        for (int j = 0; j < DE; ++j) gE[q][j] = ch < n ? scale * gEenv[((size_t)c * n + ch) * DE + j] : T(0);
     }
-    for (int t = 0; t < ntiles; ++t) {
-        const int e = e0 + t * nslots + slot;
-        const bool valid = active && e < e1;
-        T x = T(0), y = T(0), z = T(1), inv = T(1), wv = T(0);
-        if (valid) {
-            const T rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
-            inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
-            x = rx * inv; y = ry * inv; z = rz * inv;
-            wv = w[(size_t)e * n + ch];
-        }
+    for (int e = e0 + warp; e < e1; e += 8) {
+        const T rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+        const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+        const T x = rx * inv, y = ry * inv, z = rz * inv;
         T Y[DE];
         sph_harm<T, L>(x, y, z, Y);
-        T gw = T(0);
-        T part[DE];
+        T part[16];
 #pragma unroll
-        for (int j = 0; j < DE; ++j) { gw = fma(gE[j], Y[j], gw); part[j] = gE[j] * wv; }
-        if (valid && g_w) g_w[(size_t)e * n + ch] = gw;
-        if (warp_tree) {
+        for (int j = 0; j < 16; ++j) part[j] = T(0);
 #pragma unroll
-            for (int j = 0; j < DE; ++j) {
-                T a = part[j];
+        for (int q = 0; q < CPL; ++q) {
+            const int ch = lane + 32 * q;
+            const T wv = ch < n ? w[(size_t)e * n + ch] : T(0);
+            T gw = T(0);
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-                part[j] = a;
-            }
-            if (lane == 0 && active) {
-#pragma unroll
-                for (int j = 0; j < DE; ++j) red[((size_t)slot * (n >> 5) + (ch >> 5)) * DE + j] = part[j];
-            }
-        } else if (active) {
-#pragma unroll
-            for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = part[j];
+            for (int j = 0; j < DE; ++j) { gw = fma(gE[q][j], Y[j], gw); part[j] = fma(gE[q][j], wv, part[j]); }
+            if (g_w && ch < n) g_w[(size_t)e * n + ch] = gw;
         }
-        __syncthreads();
-        if (valid && ch == 0) {
-            const int cnt = warp_tree ? (n >> 5) : n;
-            T gY[DE];
+        warp_reduce16<T>(part, lane);
+        T gY[DE];
 #pragma unroll
-            for (int j = 0; j < DE; ++j) {
-                T s = red[((size_t)slot * cnt) * DE + j];
-                for (int q = 1; q < cnt; ++q) s += red[((size_t)slot * cnt + q) * DE + j];
-                gY[j] = s;
-            }
+        for (int j = 0; j < DE; ++j) gY[j] = __shfl_sync(0xffffffffu, part[0], 2 * j);
+        if (lane == 0) {
             T g[3];
             sph_harm_vjp<T, L>(x, y, z, gY, g);
             const T dot = g[0] * x + g[1] * y + g[2] * z;
@@ -190,7 +182,6 @@ __global__ void __launch_bounds__(THREADS) env_embed_bwd_kernel(int n, const int
             g_rvec[3 * (size_t)e + 1] = (g[1] - dot * y) * inv;
             g_rvec[3 * (size_t)e + 2] = (g[2] - dot * z) * inv;
         }
-        __syncthreads();
     }
 }
 

@@ -57,6 +57,12 @@ static void emit(FILE* f, int L) {
     const int DT = toff[P];
     fprintf(f, "\n// ======================= l_max = %d: P = %d, nnz = %zu, dV = %d, dE = %d, dT = %d\n", L, P, t.nnz.size(), t.dV,
             t.dE, DT);
+    fprintf(f, "static __device__ const short tpgen_zpath_%d[%zu] = {", L, t.nnz.size());
+    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%d%s", t.nnz[z].path, z + 1 == t.nnz.size() ? "" : ",");
+    fprintf(f, "};\n");
+    fprintf(f, "static __device__ const double tpgen_zcoef_%d[%zu] = {", L, t.nnz.size());
+    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%.17g%s", t.nnz[z].c, z + 1 == t.nnz.size() ? "" : ",");
+    fprintf(f, "};\n");
     fprintf(f, "template <> struct TPGen<%d> {\n", L);
     fprintf(f, "    static constexpr int LMAX = %d, DV = %d, DE = %d, P = %d, NNZ = %zu, DT = %d;\n", L, t.dV, t.dE, P, t.nnz.size(), DT);
     for (int flavour = 0; flavour < 2; ++flavour) {
@@ -118,13 +124,9 @@ static void emit(FILE* f, int L) {
         }
         fprintf(f, "    }\n");
     }
-    // ---------------- per-non-zero tables for the fold kernel (combined tensor = path weight x CG)
-    fprintf(f, "    static __host__ __device__ constexpr int zpath(int z) { constexpr int v[%zu] = {", t.nnz.size());
-    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%d%s", t.nnz[z].path, z + 1 == t.nnz.size() ? "" : ",");
-    fprintf(f, "}; return v[z]; }\n");
-    fprintf(f, "    static __host__ __device__ constexpr double zcoef(int z) { constexpr double v[%zu] = {", t.nnz.size());
-    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%.17g%s", t.nnz[z].c, z + 1 == t.nnz.size() ? "" : ",");
-    fprintf(f, "}; return v[z]; }\n");
+    // ---------------- per-non-zero tables for the fold kernel (combined tensor = path weight x CG): device arrays
+    fprintf(f, "    static __device__ __forceinline__ int zpath(int z) { return tpgen_zpath_%d[z]; }\n", L);
+    fprintf(f, "    static __device__ __forceinline__ double zcoef(int z) { return tpgen_zcoef_%d[z]; }\n", L);
     // ---------------- small integer tables for the dense mix
     fprintf(f, "    // t-slot offset of each path, and the out block it mixes into\n");
     fprintf(f, "    static __host__ __device__ constexpr int toff(int p) { constexpr int v[%d] = {", P + 1);

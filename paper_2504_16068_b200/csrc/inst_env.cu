@@ -44,8 +44,14 @@ allegro_status_t launch_env_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EnvBwdArg
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
-    env_embed_bwd_kernel<T, ALLEGRO_L, kEnvThreads><<<(unsigned)a.n_atoms, kEnvThreads, 0, a.st>>>(
-        a.n, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.w, (T)a.scale, (T*)a.g_rvec, (T*)a.g_w);
+#define ALLEGRO_ENVB(CPL)                                                                          \
+    env_embed_bwd_kernel<T, ALLEGRO_L, CPL><<<(unsigned)a.n_atoms, 256, 0, a.st>>>(                \
+        a.n, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.w, (T)a.scale, (T*)a.g_rvec, (T*)a.g_w)
+    if (a.n <= 32) ALLEGRO_ENVB(1);
+    else if (a.n <= 64) ALLEGRO_ENVB(2);
+    else if (a.n <= 128) ALLEGRO_ENVB(4);
+    else ALLEGRO_ENVB(8);
+#undef ALLEGRO_ENVB
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

@@ -20,6 +20,8 @@ __device__ ALLEGRO_T g_cw_stage[kCwMax];  // fold_kernel writes here; copied dev
 
 namespace allegro {
 
+using Gen = TPGen<ALLEGRO_L>;
+
 template <typename T> struct Cfg {
     static constexpr int THREADS = sizeof(T) == 4 ? 256 : 128;
 };
@@ -40,7 +42,7 @@ template <typename T>
 static allegro_status_t fold_weights(const TpArgs& a) {
     T* stage = nullptr;
     ALLEGRO_CUDA(cudaGetSymbolAddress((void**)&stage, g_cw_stage));
-    fold_kernel<T><<<(Gen::NNZ + 127) / 128, 128, 0, a.st>>>((const T*)a.path_w, stage);
+    fold_kernel<T, ALLEGRO_L><<<(Gen::NNZ + 127) / 128, 128, 0, a.st>>>((const T*)a.path_w, stage);
     ALLEGRO_LAUNCHED();
     ALLEGRO_CUDA(cudaMemcpyToSymbolAsync(c_cw, stage, sizeof(T) * Gen::NNZ, 0, cudaMemcpyDeviceToDevice, a.st));
     return ALLEGRO_OK;
@@ -70,7 +72,7 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     const size_t smem = nst * stage + 64;
 #define ALLEGRO_FWD(NST)                                                                                           \
     {                                                                                                              \
-        auto k = tp_fwd_kernel<T, TH, NST>;                                                                        \
+        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, NST>;                                                                        \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                       \
         k<<<(unsigned)a.n_items, TH, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out); \
     }
@@ -127,7 +129,7 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     const size_t smem = nst * stage + red;
 #define ALLEGRO_BWD(NST, GV, GW)                                                                                          \
     {                                                                                                                     \
-        auto k = tp_bwd_kernel<T, TH, NST, GV, GW>;                                                                       \
+        auto k = tp_bwd_kernel<T, ALLEGRO_L, TH, NST, GV, GW>;                                                                       \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                              \
         k<<<(unsigned)a.n_items, TH, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
                                                    (T*)a.gV, gE_dst, have_items ? 1 : 0, gw_part);                        \

@@ -11,6 +11,8 @@ constexpr double kPiD = 3.14159265358979323846264338327950288;
 // Bessel basis times polynomial cutoff and its derivative w.r.t. |r|, evaluated in double for either dtype
 // (the embedding is "largely in double-precision"); cost is per edge, not per channel.
 //   x = r/rc, B_b = sqrt(2/rc) sin(b pi x)/r, u = 1 - 28x^6 + 48x^7 - 21x^8
+// One sincos per edge; sin(b t), cos(b t) for b >= 2 by the angle-addition recurrence (error growth ~ b eps).
+template <bool WANT_D>
 __device__ __forceinline__ void radial_basis(double r, double rc, int nb, double* Bu, double* dBu) {
     const double x = r / rc;
     const double x2 = x * x, x5 = x2 * x2 * x, x6 = x5 * x, x7 = x6 * x, x8 = x7 * x;
@@ -18,20 +20,27 @@ __device__ __forceinline__ void radial_basis(double r, double rc, int nb, double
     double du = (-168.0 * x5 + 336.0 * x6 - 168.0 * x7) / rc;
     if (x >= 1.0) { u = 0.0; du = 0.0; }
     const double pre = sqrt(2.0 / rc), ir = 1.0 / r;
+    double s1, c1;
+    sincospi(x, &s1, &c1);
+    double sn = s1, cs = c1;
     for (int b = 1; b <= nb; ++b) {
-        const double k = b * kPiD / rc;
-        double sn, cs;
-        sincos(k * r, &sn, &cs);
         const double B = pre * sn * ir;
-        const double dB = pre * (k * cs * ir - sn * ir * ir);
         Bu[b - 1] = B * u;
-        if (dBu) dBu[b - 1] = dB * u + B * du;
+        if (WANT_D) {
+            const double k = b * kPiD / rc;
+            const double dB = pre * (k * cs * ir - sn * ir * ir);
+            dBu[b - 1] = dB * u + B * du;
+        }
+        const double sn2 = sn * c1 + cs * s1;
+        cs = cs * c1 - sn * s1;
+        sn = sn2;
     }
 }
 
-constexpr int kRadEdges = 32;  // edges per CTA
+constexpr int kRadEdges = 64;  // edges per CTA
 
-// w[e][ch] = sum_b W_r[ch][b] B_b(r_e) u(r_e/rc)
+// w[e][ch] = sum_b W_r[ch][b] B_b(r_e) u(r_e/rc).  Phase 1: one thread per edge evaluates the basis into shared
+// memory; phase 2: thread <-> (edge, channel), consecutive threads write consecutive channels (coalesced).
 template <typename T>
 __global__ void __launch_bounds__(256) radial_fwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_r,
                                                           T* __restrict__ w) {
@@ -42,7 +51,7 @@ __global__ void __launch_bounds__(256) radial_fwd_kernel(int n, int nb, double r
         const long e = eb + threadIdx.x;
         const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
         double Bu[kMaxBasis];
-        radial_basis(sqrt(rx * rx + ry * ry + rz * rz), rc, nb, Bu, nullptr);
+        radial_basis<false>(sqrt(rx * rx + ry * ry + rz * rz), rc, nb, Bu, nullptr);
         for (int b = 0; b < nb; ++b) Bs[threadIdx.x][b] = Bu[b];
     }
     __syncthreads();
@@ -54,29 +63,37 @@ __global__ void __launch_bounds__(256) radial_fwd_kernel(int n, int nb, double r
     }
 }
 
-// g_rvec[e] += (sum_ch g_w[e][ch] dw[e][ch]/dr) rhat_e.  One warp per edge; channels summed by lane-strided
-// partial sums and a fixed xor tree.
+// g_rvec[e] += (sum_ch g_w[e][ch] dw[e][ch]/dr) rhat_e.  Phase 1 as above (derivative of the basis); phase 2: one
+// warp per edge, channels summed by lane-strided partial sums and a fixed xor tree.
 template <typename T>
 __global__ void __launch_bounds__(256) radial_bwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_r,
                                                           const T* __restrict__ g_w, T* __restrict__ g_rvec) {
-    const long e = (long)blockIdx.x * 8 + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (e >= E) return;
-    const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
-    const double r = sqrt(rx * rx + ry * ry + rz * rz);
-    double Bu[kMaxBasis], dBu[kMaxBasis];
-    radial_basis(r, rc, nb, Bu, dBu);
-    double acc = 0.0;
-    for (int ch = lane; ch < n; ch += 32) {
-        double dw = 0.0;
-        for (int b = 0; b < nb; ++b) dw += (double)W_r[ch * nb + b] * dBu[b];
-        acc += (double)g_w[(size_t)e * n + ch] * dw;
+    __shared__ double dBs[kRadEdges][kMaxBasis];
+    __shared__ double rh[kRadEdges][3];
+    const long eb = (long)blockIdx.x * kRadEdges;
+    const int cnt = (int)min((long)kRadEdges, E - eb);
+    if ((int)threadIdx.x < cnt) {
+        const long e = eb + threadIdx.x;
+        const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
+        const double r = sqrt(rx * rx + ry * ry + rz * rz);
+        double Bu[kMaxBasis], dBu[kMaxBasis];
+        radial_basis<true>(r, rc, nb, Bu, dBu);
+        for (int b = 0; b < nb; ++b) dBs[threadIdx.x][b] = dBu[b];
+        rh[threadIdx.x][0] = rx / r; rh[threadIdx.x][1] = ry / r; rh[threadIdx.x][2] = rz / r;
     }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int le = warp; le < cnt; le += 8) {
+        const long e = eb + le;
+        double acc = 0.0;
+        for (int ch = lane; ch < n; ch += 32) {
+            double dw = 0.0;
+            for (int b = 0; b < nb; ++b) dw += (double)W_r[ch * nb + b] * dBs[le][b];
+            acc += (double)g_w[(size_t)e * n + ch] * dw;
+        }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane < 3) {
-        const double comp = lane == 0 ? rx : (lane == 1 ? ry : rz);
-        g_rvec[3 * e + lane] = (T)((double)g_rvec[3 * e + lane] + acc * comp / r);
+        for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+        if (lane < 3) g_rvec[3 * e + lane] = (T)((double)g_rvec[3 * e + lane] + acc * rh[le][lane]);
     }
 }
 
@@ -129,17 +146,27 @@ __global__ void __launch_bounds__(256) edge_energy_kernel(int n, int dV, long E,
     if (lane == 0 && e_edge) e_edge[e] = acc;
 }
 
-// out[s] = sum_{i in [ptr[s], ptr[s+1])} vals[i]: one warp per segment, lane-strided, fixed xor tree, double accumulator
+// out[s] = sum_{i in [ptr[s], ptr[s+1])} vals[i]: one CTA per segment, thread-strided partial sums in double, fixed
+// shared-memory tree (deterministic)
+constexpr int kSegThreads = 512;
 template <typename T>
-__global__ void __launch_bounds__(256) segment_sum_kernel(const int* __restrict__ ptr, int nseg, const T* __restrict__ vals, T* __restrict__ out) {
-    const int s = blockIdx.x * 8 + (threadIdx.x >> 5);
-    const int lane = threadIdx.x & 31;
-    if (s >= nseg) return;
-    double acc = 0.0;
-    for (int i = ptr[s] + lane; i < ptr[s + 1]; i += 32) acc += (double)vals[i];
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) out[s] = (T)acc;
+__global__ void __launch_bounds__(kSegThreads) segment_sum_kernel(const int* __restrict__ ptr, int nseg, const T* __restrict__ vals, T* __restrict__ out) {
+    __shared__ double sh[kSegThreads];
+    const int s = blockIdx.x;
+    const int i0 = ptr[s], i1 = ptr[s + 1];
+    double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+    int i = i0 + threadIdx.x;
+    for (; i + 3 * kSegThreads < i1; i += 4 * kSegThreads) {
+        a0 += (double)vals[i]; a1 += (double)vals[i + kSegThreads]; a2 += (double)vals[i + 2 * kSegThreads]; a3 += (double)vals[i + 3 * kSegThreads];
+    }
+    for (; i < i1; i += kSegThreads) a0 += (double)vals[i];
+    sh[threadIdx.x] = (a0 + a1) + (a2 + a3);
+    __syncthreads();
+    for (int o = kSegThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) out[s] = (T)sh[0];
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
@@ -154,7 +181,7 @@ template <typename T>
 allegro_status_t launch_radial_backward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, const void* g_w, void* g_rvec,
                                         cudaStream_t st) {
     if (E == 0) return ALLEGRO_OK;
-    radial_bwd_kernel<T><<<(unsigned)((E + 7) / 8), 256, 0, st>>>(n, nb, rc, E, (const T*)rvec, (const T*)W_r, (const T*)g_w, (T*)g_rvec);
+    radial_bwd_kernel<T><<<(unsigned)((E + kRadEdges - 1) / kRadEdges), 256, 0, st>>>(n, nb, rc, E, (const T*)rvec, (const T*)W_r, (const T*)g_w, (T*)g_rvec);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -176,7 +203,7 @@ allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, cons
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st) {
     if (nseg == 0) return ALLEGRO_OK;
-    segment_sum_kernel<T><<<(unsigned)((nseg + 7) / 8), 256, 0, st>>>(ptr, nseg, (const T*)vals, (T*)out);
+    segment_sum_kernel<T><<<(unsigned)nseg, kSegThreads, 0, st>>>(ptr, nseg, (const T*)vals, (T*)out);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

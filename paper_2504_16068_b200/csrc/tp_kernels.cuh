@@ -20,21 +20,25 @@
 
 namespace allegro {
 
-using Gen = TPGen<ALLEGRO_L>;
-static_assert(Gen::NNZ <= kCwMax, "coefficient table too small");
+// NOTE: l_max is a template parameter of every kernel here.  The translation units inst_tp.cu (one per
+// l_max) would otherwise instantiate kernels with identical mangled names and different bodies, and the
+// linker keeps one of them (ODR): the wrong l_max's code would run.
+static_assert(TPGen<ALLEGRO_L>::NNZ <= kCwMax, "coefficient table too small");
 
 // ------------------------------------------------------------------------------------------------
 // fold: cw[z] = path_w[path(z)] * C_z  (the "combined tensor"), product in double, rounded once
-template <typename T>
+template <typename T, int L>
 __global__ void fold_kernel(const T* __restrict__ path_w, T* __restrict__ cw) {
+    using Gen = TPGen<L>;
     const int z = blockIdx.x * blockDim.x + threadIdx.x;
     if (z < Gen::NNZ) cw[z] = (T)((double)path_w[Gen::zpath(z)] * Gen::zcoef(z));
 }
 
 // ------------------------------------------------------------------------------------------------
-template <typename T, int THREADS, int NST>
+template <typename T, int L, int THREADS, int NST>
 __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                           const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ out) {
+    using Gen = TPGen<L>;
     constexpr int DV = Gen::DV, DE = Gen::DE;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x;
@@ -112,10 +116,11 @@ __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __res
 // bulk-stored; gEenv accumulates in registers over the thread's edges, then over slots in slot order.
 // WANT_GW adds the path-weight gradient: per-thread accumulators -> fixed-shape warp tree -> warps in
 // order -> one partial row per item (reduced over items by gw_final_kernel).
-template <typename T, int THREADS, int NST, bool WANT_GV, bool WANT_GW>
+template <typename T, int L, int THREADS, int NST, bool WANT_GV, bool WANT_GW>
 __global__ void __launch_bounds__(THREADS)
     tp_bwd_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
                   const T* __restrict__ Eenv, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item, T* __restrict__ gw_part) {
+    using Gen = TPGen<L>;
     constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x;
