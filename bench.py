@@ -231,7 +231,7 @@ def run_ours(args):
     roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
                 "traffic": _ncu_traffic(top), "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top],
                 "ms_per_launch": per_call_ms[top]}
-    step_bytes = sum(abytes.values())
+    step_bytes = sum(abytes[k] for k in per_call_ms)
     calls = {k: {"ms": round(per_call_ms[k], 4), "GB/s": round(abytes[k] / (per_call_ms[k] * 1e-3) / 1e9, 1),
                  "share": round(per_call_ms[k] / sum(per_call_ms.values()), 4)} for k in per_call_ms}
 

@@ -6,7 +6,7 @@ oracle: if the shared library is missing the import of any entry point raises.
 
 Names mirror the C ABI without the `allegro_` prefix:
     Plan(l_max, n, dtype, wmode)            allegro_plan_create / _destroy / _paths / _cg
-    segments_build, env_embed, tp_forward, tp_backward, env_embed_backward, force_gather,
+    segments_build, env_embed, tp_forward, tp_forward_energy, tp_backward, env_embed_backward, force_gather,
     radial_forward, radial_backward, edge_energy, segment_sum, launch_count
 """
 import ctypes as C
@@ -39,6 +39,7 @@ SIGNATURES = {
     "allegro_segments_build": (C.c_int, [_i32p, C.c_int, C.c_int, _i32p, C.c_long, C.POINTER(C.c_long)]),
     "allegro_env_embed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_tp_forward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp]),
     "allegro_tp_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_long, C.c_int]),
     "allegro_env_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
@@ -187,6 +188,21 @@ def tp_forward(plan, row_ptr, V, Eenv, path_w, items=None, out=None, stream=None
     _check(lib().allegro_tp_forward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(V), _ptr(Eenv),
                                     _ptr(path_w), _ptr(out), _stream(stream)))
     return out
+
+
+def tp_forward_energy(plan, row_ptr, V, Eenv, path_w, q, kappa, items=None, want_out=True, want_e=True, want_G=True, out=None, e_edge=None,
+                      G=None, stream=None):
+    """-> (out or None, e_edge or None, G or None): tp_forward with the energy / cotangent epilogue fused"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    if out is None and want_out:
+        out = torch.empty_like(V)
+    if e_edge is None and want_e:
+        e_edge = torch.empty((n_edges,), dtype=V.dtype, device=V.device)
+    if G is None and want_G:
+        G = torch.empty_like(V)
+    _check(lib().allegro_tp_forward_energy(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(V), _ptr(Eenv),
+                                           _ptr(path_w), _ptr(q), float(kappa), _ptr(out), _ptr(e_edge), _ptr(G), _stream(stream)))
+    return out, e_edge, G
 
 
 def tp_backward(plan, row_ptr, G, V, Eenv, path_w, items=None, want_gV=True, want_g_path_w=False, gV=None, gEenv=None,

@@ -142,6 +142,29 @@ allegro_status_t allegro_tp_forward(const allegro_plan_t* plan, int n_atoms, lon
     return ALLEGRO_DISPATCH(plan, launch_tp_forward, a);
 }
 
+allegro_status_t allegro_tp_forward_energy(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                           long n_items, const void* V, const void* Eenv, const void* path_w, const void* q, double kappa,
+                                           void* out, void* e_edge, void* G, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG(V || n_edges == 0, "V is NULL");
+    ALLEGRO_CHECK_ARG(out || G, "out and G are both NULL");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr && q != nullptr, "path_w / q is NULL");
+    ALLEGRO_CHECK_ARG((V != out && V != G && (out != G || !out)) || n_edges == 0, "out / G alias V or each other");
+    ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(out) && aligned16(G) && aligned16(Eenv), "feature tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (plan->wmode != ALLEGRO_W_SCALAR) {
+        set_error("allegro_tp_forward_energy: scalar path weights only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.out = out; a.q = q; a.kappa = kappa; a.e_edge = e_edge; a.Gout = G;
+    a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_forward, a);
+}
+
 allegro_status_t allegro_tp_backward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
                                      long n_items, const void* G, const void* V, const void* Eenv, const void* path_w, void* gV, void* gEenv,
                                      void* g_path_w, void* workspace, size_t workspace_bytes, void* stream) {

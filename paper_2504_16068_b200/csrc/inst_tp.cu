@@ -68,15 +68,30 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     if (s != ALLEGRO_OK) return s;
     const int nslots = TH / a.n;
     const size_t stage = align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
-    const int nst = pick_stages(stage, 256);
-    const size_t smem = nst * stage + 64;
-#define ALLEGRO_FWD(NST)                                                                                           \
+    const bool w_out = a.out != nullptr, w_g = a.Gout != nullptr, w_e = a.e_edge != nullptr;
+    const size_t extra = ((w_out && w_g) ? 3 * stage : 0) + 64 + 2 * TH * sizeof(T);
+    const int nst = pick_stages(stage, extra + 128);
+    const size_t smem = nst * stage + extra;
+#define ALLEGRO_FWD(NST, WO, WG, WE)                                                                               \
     {                                                                                                              \
-        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, NST>;                                                                        \
+        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, NST, WO, WG, WE>;                                                 \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                       \
-        k<<<(unsigned)a.n_items, TH, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out); \
+        k<<<(unsigned)a.n_items, TH, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
+                                                   (const T*)a.q, (T)a.kappa, (T*)a.e_edge, (T*)a.Gout);           \
     }
-    if (nst == 3) ALLEGRO_FWD(3) else if (nst == 2) ALLEGRO_FWD(2) else ALLEGRO_FWD(1)
+#define ALLEGRO_FWD_N(WO, WG, WE) \
+    if (nst == 3) ALLEGRO_FWD(3, WO, WG, WE) else if (nst == 2) ALLEGRO_FWD(2, WO, WG, WE) else ALLEGRO_FWD(1, WO, WG, WE)
+    if (w_out && !w_g && !w_e) { ALLEGRO_FWD_N(true, false, false) }
+    else if (w_out && w_g && w_e) { ALLEGRO_FWD_N(true, true, true) }
+    else if (w_out && w_g) { ALLEGRO_FWD_N(true, true, false) }
+    else if (w_out && w_e) { ALLEGRO_FWD_N(true, false, true) }
+    else if (w_g && w_e) { ALLEGRO_FWD_N(false, true, true) }
+    else if (w_g) { ALLEGRO_FWD_N(false, true, false) }
+    else {
+        set_error("tp_forward: nothing to store (out and G are both NULL)");
+        return ALLEGRO_EINVAL;
+    }
+#undef ALLEGRO_FWD_N
 #undef ALLEGRO_FWD
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;

@@ -46,7 +46,12 @@ struct TpArgs {
     const void* V;
     const void* Eenv;
     const void* path_w;
-    void* out;  // forward
+    void* out;  // forward (nullable in the energy variant)
+    // forward energy epilogue (allegro_tp_forward_energy): all nullable
+    const void* q;
+    double kappa;
+    void* e_edge;
+    void* Gout;
     // backward
     const void* G;
     void* gV;        // nullable

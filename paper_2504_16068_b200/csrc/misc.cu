@@ -1,5 +1,7 @@
 // misc.cu -- dtype-only helpers of the hot path: radial weights and their chain rule (A8), force
 // assembly (a7), the scalar edge energy of the VJP tests / benchmarks (A12) and the segment sum (A20).
+#include <cooperative_groups.h>
+
 #include "common.cuh"
 #include "launch.h"
 
@@ -37,59 +39,84 @@ __device__ __forceinline__ void radial_basis(double r, double rc, int nb, double
     }
 }
 
-constexpr int kRadEdges = 64;  // edges per CTA
+constexpr int kRadEdges = 128;  // edges per CTA
 
 // w[e][ch] = sum_b W_r[ch][b] B_b(r_e) u(r_e/rc).  Phase 1: one thread per edge evaluates the basis into shared
-// memory; phase 2: thread <-> (edge, channel), consecutive threads write consecutive channels (coalesced).
-template <typename T>
+// memory; phase 2: warp <-> edge, lane <-> channels lane, lane+32, ... (CPL per lane) whose W_r rows sit in
+// registers as doubles, so a row w[e][:] is written as whole coalesced lines and the inner loop is LDS + DFMA only.
+template <typename T, int CPL, int NB>
 __global__ void __launch_bounds__(256) radial_fwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_r,
                                                           T* __restrict__ w) {
-    __shared__ double Bs[kRadEdges][kMaxBasis];
+    __shared__ double Bs[kRadEdges][NB];
     const long eb = (long)blockIdx.x * kRadEdges;
     const int cnt = (int)min((long)kRadEdges, E - eb);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double Wd[CPL][NB];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Wd[q][b] = (lane + 32 * q < n && b < nb) ? (double)W_r[(lane + 32 * q) * nb + b] : 0.0;
     if ((int)threadIdx.x < cnt) {
         const long e = eb + threadIdx.x;
         const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
         double Bu[kMaxBasis];
         radial_basis<false>(sqrt(rx * rx + ry * ry + rz * rz), rc, nb, Bu, nullptr);
-        for (int b = 0; b < nb; ++b) Bs[threadIdx.x][b] = Bu[b];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Bs[threadIdx.x][b] = b < nb ? Bu[b] : 0.0;
     }
     __syncthreads();
-    for (int idx = threadIdx.x; idx < cnt * n; idx += 256) {
-        const int le = idx / n, ch = idx - le * n;
-        double s = 0.0;
-        for (int b = 0; b < nb; ++b) s += (double)W_r[ch * nb + b] * Bs[le][b];
-        w[(size_t)(eb + le) * n + ch] = (T)s;
+    for (int le = warp; le < cnt; le += 8) {
+        double Bv[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Bv[b] = Bs[le][b];
+#pragma unroll
+        for (int q = 0; q < CPL; ++q) {
+            double s = 0.0;
+#pragma unroll
+            for (int b = 0; b < NB; ++b) s = fma(Wd[q][b], Bv[b], s);
+            if (lane + 32 * q < n) w[(size_t)(eb + le) * n + lane + 32 * q] = (T)s;
+        }
     }
 }
 
-// g_rvec[e] += (sum_ch g_w[e][ch] dw[e][ch]/dr) rhat_e.  Phase 1 as above (derivative of the basis); phase 2: one
-// warp per edge, channels summed by lane-strided partial sums and a fixed xor tree.
-template <typename T>
+// g_rvec[e] += (sum_ch g_w[e][ch] dw[e][ch]/dr) rhat_e.  Same mapping; the channel sum is lane-local over the lane's
+// channels, then a fixed xor tree.
+template <typename T, int CPL, int NB>
 __global__ void __launch_bounds__(256) radial_bwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_r,
                                                           const T* __restrict__ g_w, T* __restrict__ g_rvec) {
-    __shared__ double dBs[kRadEdges][kMaxBasis];
+    __shared__ double dBs[kRadEdges][NB];
     __shared__ double rh[kRadEdges][3];
     const long eb = (long)blockIdx.x * kRadEdges;
     const int cnt = (int)min((long)kRadEdges, E - eb);
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    double Wd[CPL][NB];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Wd[q][b] = (lane + 32 * q < n && b < nb) ? (double)W_r[(lane + 32 * q) * nb + b] : 0.0;
     if ((int)threadIdx.x < cnt) {
         const long e = eb + threadIdx.x;
         const double rx = (double)rvec[3 * e], ry = (double)rvec[3 * e + 1], rz = (double)rvec[3 * e + 2];
         const double r = sqrt(rx * rx + ry * ry + rz * rz);
         double Bu[kMaxBasis], dBu[kMaxBasis];
         radial_basis<true>(r, rc, nb, Bu, dBu);
-        for (int b = 0; b < nb; ++b) dBs[threadIdx.x][b] = dBu[b];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) dBs[threadIdx.x][b] = b < nb ? dBu[b] : 0.0;
         rh[threadIdx.x][0] = rx / r; rh[threadIdx.x][1] = ry / r; rh[threadIdx.x][2] = rz / r;
     }
     __syncthreads();
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int le = warp; le < cnt; le += 8) {
         const long e = eb + le;
+        double Bv[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Bv[b] = dBs[le][b];
         double acc = 0.0;
-        for (int ch = lane; ch < n; ch += 32) {
+#pragma unroll
+        for (int q = 0; q < CPL; ++q) {
             double dw = 0.0;
-            for (int b = 0; b < nb; ++b) dw += (double)W_r[ch * nb + b] * dBs[le][b];
-            acc += (double)g_w[(size_t)e * n + ch] * dw;
+#pragma unroll
+            for (int b = 0; b < NB; ++b) dw = fma(Wd[q][b], Bv[b], dw);
+            if (lane + 32 * q < n) acc = fma((double)g_w[(size_t)e * n + lane + 32 * q], dw, acc);
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
@@ -146,34 +173,65 @@ __global__ void __launch_bounds__(256) edge_energy_kernel(int n, int dV, long E,
     if (lane == 0 && e_edge) e_edge[e] = acc;
 }
 
-// out[s] = sum_{i in [ptr[s], ptr[s+1])} vals[i]: one CTA per segment, thread-strided partial sums in double, fixed
-// shared-memory tree (deterministic)
+// out[s] = sum_{i in [ptr[s], ptr[s+1])} vals[i].  One thread-block CLUSTER of kSegCluster CTAs per segment: every
+// thread adds a strided subset in double, each CTA folds its threads with a fixed shared-memory tree, and CTA 0 of
+// the cluster adds the CTAs' partials in rank order through distributed shared memory (deterministic, no
+// workspace, no atomics).
 constexpr int kSegThreads = 512;
+constexpr int kSegCluster = 8;
 template <typename T>
 __global__ void __launch_bounds__(kSegThreads) segment_sum_kernel(const int* __restrict__ ptr, int nseg, const T* __restrict__ vals, T* __restrict__ out) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
     __shared__ double sh[kSegThreads];
-    const int s = blockIdx.x;
+    const int s = blockIdx.x / kSegCluster;
+    const int rank = (int)cluster.block_rank();
     const int i0 = ptr[s], i1 = ptr[s + 1];
+    constexpr int STRIDE = kSegThreads * kSegCluster;
     double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
-    int i = i0 + threadIdx.x;
-    for (; i + 3 * kSegThreads < i1; i += 4 * kSegThreads) {
-        a0 += (double)vals[i]; a1 += (double)vals[i + kSegThreads]; a2 += (double)vals[i + 2 * kSegThreads]; a3 += (double)vals[i + 3 * kSegThreads];
+    int i = i0 + rank * kSegThreads + threadIdx.x;
+    for (; i + 3 * STRIDE < i1; i += 4 * STRIDE) {
+        a0 += (double)vals[i]; a1 += (double)vals[i + STRIDE]; a2 += (double)vals[i + 2 * STRIDE]; a3 += (double)vals[i + 3 * STRIDE];
     }
-    for (; i < i1; i += kSegThreads) a0 += (double)vals[i];
+    for (; i < i1; i += STRIDE) a0 += (double)vals[i];
     sh[threadIdx.x] = (a0 + a1) + (a2 + a3);
     __syncthreads();
     for (int o = kSegThreads / 2; o > 0; o >>= 1) {
         if ((int)threadIdx.x < o) sh[threadIdx.x] += sh[threadIdx.x + o];
         __syncthreads();
     }
-    if (threadIdx.x == 0) out[s] = (T)sh[0];
+    cluster.sync();
+    if (rank == 0 && threadIdx.x == 0) {
+        double tot = sh[0];
+        for (int r = 1; r < kSegCluster; ++r) tot += *cluster.map_shared_rank(&sh[0], r);
+        out[s] = (T)tot;
+    }
+    cluster.sync();  // keep every CTA's shared memory alive until CTA 0 has read it
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
+// (CPL, NB) instantiations: n <= 32 * CPL channels, nb <= NB basis functions
+#define ALLEGRO_RAD_DISPATCH(KERNEL, ...)                                                     \
+    do {                                                                                      \
+        const unsigned grid = (unsigned)((E + kRadEdges - 1) / kRadEdges);                     \
+        if (nb <= 8) {                                                                        \
+            if (n <= 32) KERNEL<T, 1, 8><<<grid, 256, 0, st>>>(__VA_ARGS__);                   \
+            else if (n <= 64) KERNEL<T, 2, 8><<<grid, 256, 0, st>>>(__VA_ARGS__);              \
+            else if (n <= 128) KERNEL<T, 4, 8><<<grid, 256, 0, st>>>(__VA_ARGS__);             \
+            else KERNEL<T, 8, 8><<<grid, 256, 0, st>>>(__VA_ARGS__);                           \
+        } else {                                                                              \
+            if (n <= 32) KERNEL<T, 1, 16><<<grid, 256, 0, st>>>(__VA_ARGS__);                  \
+            else if (n <= 64) KERNEL<T, 2, 16><<<grid, 256, 0, st>>>(__VA_ARGS__);             \
+            else if (n <= 128) KERNEL<T, 4, 16><<<grid, 256, 0, st>>>(__VA_ARGS__);            \
+            else KERNEL<T, 8, 16><<<grid, 256, 0, st>>>(__VA_ARGS__);                          \
+        }                                                                                     \
+    } while (0)
+
 template <typename T>
 allegro_status_t launch_radial_forward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, void* w, cudaStream_t st) {
     if (E == 0) return ALLEGRO_OK;
-    radial_fwd_kernel<T><<<(unsigned)((E + kRadEdges - 1) / kRadEdges), 256, 0, st>>>(n, nb, rc, E, (const T*)rvec, (const T*)W_r, (T*)w);
+    if (n > 256) { set_error("radial_forward: n = %d unsupported (n <= 256)", n); return ALLEGRO_EUNSUPPORTED; }
+    ALLEGRO_RAD_DISPATCH(radial_fwd_kernel, n, nb, rc, E, (const T*)rvec, (const T*)W_r, (T*)w);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -181,7 +239,8 @@ template <typename T>
 allegro_status_t launch_radial_backward(int n, int nb, double rc, long E, const void* rvec, const void* W_r, const void* g_w, void* g_rvec,
                                         cudaStream_t st) {
     if (E == 0) return ALLEGRO_OK;
-    radial_bwd_kernel<T><<<(unsigned)((E + kRadEdges - 1) / kRadEdges), 256, 0, st>>>(n, nb, rc, E, (const T*)rvec, (const T*)W_r, (const T*)g_w, (T*)g_rvec);
+    if (n > 256) { set_error("radial_backward: n = %d unsupported (n <= 256)", n); return ALLEGRO_EUNSUPPORTED; }
+    ALLEGRO_RAD_DISPATCH(radial_bwd_kernel, n, nb, rc, E, (const T*)rvec, (const T*)W_r, (const T*)g_w, (T*)g_rvec);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -203,7 +262,19 @@ allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, cons
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st) {
     if (nseg == 0) return ALLEGRO_OK;
-    segment_sum_kernel<T><<<(unsigned)nseg, kSegThreads, 0, st>>>(ptr, nseg, (const T*)vals, (T*)out);
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)nseg * kSegCluster);
+    cfg.blockDim = dim3(kSegThreads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = kSegCluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ALLEGRO_CUDA(cudaLaunchKernelEx(&cfg, segment_sum_kernel<T>, ptr, nseg, (const T*)vals, (T*)out));
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

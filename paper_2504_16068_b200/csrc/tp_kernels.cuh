@@ -35,19 +35,30 @@ __global__ void fold_kernel(const T* __restrict__ path_w, T* __restrict__ cw) {
 }
 
 // ------------------------------------------------------------------------------------------------
-template <typename T, int L, int THREADS, int NST>
+// Energy epilogue (reading A12), fused so that `out` is never re-read from HBM:
+//   e_edge[e] = sum_ch ( q[ch] out[e][ch][0] + kappa/2 sum_k out[e][ch][k]^2 ),   G = q (x) delta_{k,0} + kappa out
+// WANT_OUT / WANT_G / WANT_E select which of out, G, e_edge are produced (at least one of out, G).
+// Shared memory: NST stages of V (each becomes the out tile, or the G tile when !WANT_OUT, in place), then
+// 3 G tiles when both out and G are stored, then the mbarriers, then the energy partials.
+template <typename T, int L, int THREADS, int NST, bool WANT_OUT, bool WANT_G, bool WANT_E>
 __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
-                                                          const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ out) {
+                                                          const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ out,
+                                                          const T* __restrict__ q, T kappa, T* __restrict__ e_edge, T* __restrict__ G) {
     using Gen = TPGen<L>;
     constexpr int DV = Gen::DV, DE = Gen::DE;
+    constexpr bool EPI = WANT_G || WANT_E;
+    constexpr bool GBUF = WANT_OUT && WANT_G;  // separate G tiles
+    static_assert(WANT_OUT || WANT_G, "nothing to store");
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int tid = threadIdx.x;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nslots = THREADS / n;
     const int slot = tid / n, ch = tid - slot * n;
     const bool active = slot < nslots;
     const uint32_t row_bytes = (uint32_t)n * DV * sizeof(T);
     const uint32_t stage_bytes = align128((size_t)nslots * row_bytes);
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NST * stage_bytes);
+    unsigned char* gbuf = smem_raw + (size_t)NST * stage_bytes;
+    uint64_t* bars = reinterpret_cast<uint64_t*>(gbuf + (GBUF ? 3 : 0) * (size_t)stage_bytes);
+    T* ered = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(bars) + 64);  // [2][THREADS / 32] or [2][THREADS]
 
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
@@ -74,37 +85,92 @@ __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __res
     }
 
     T E[DE];
+    T qc = T(0);
     if (active) {
         const T* er = Eenv + ((size_t)c * n + ch) * DE;
 #pragma unroll
         for (int j = 0; j < DE; ++j) E[j] = er[j];
+        if constexpr (EPI) qc = q[ch];
     } else {
 #pragma unroll
         for (int j = 0; j < DE; ++j) E[j] = T(0);
     }
+    // how the per-edge energy is summed over the slot's n channels (fixed shape): whole warps -> xor tree + the
+    // slot's warps in order; n a power of two below 32 -> xor tree inside the slot's lanes; otherwise channels in order
+    const bool warp_tree = (n % 32) == 0;
+    const bool sub_tree = n < 32 && (n & (n - 1)) == 0;
 
     for (int t = 0; t < ntiles; ++t) {
         const int s = t % NST;
         mbar_wait(&bars[s], (uint32_t)(t / NST) & 1u);
         const int eb = e0 + t * nslots;
-        if (active && eb + slot < e1) {
+        const bool valid = active && eb + slot < e1;
+        T epart = T(0);
+        if (valid) {
             T* row = reinterpret_cast<T*>(smem_raw + (size_t)s * stage_bytes) + ((size_t)slot * n + ch) * DV;
             T v[DV], o[DV];
             row_load<T, DV>(row, v);
             Gen::template fwd<T>(v, E, o);
-            row_store<T, DV>(row, o);
+            if constexpr (WANT_OUT) row_store<T, DV>(row, o);
+            if constexpr (EPI) {
+                T sq = T(0);
+#pragma unroll
+                for (int k = 0; k < DV; ++k) sq = fma(o[k], o[k], sq);
+                epart = fma(T(0.5) * kappa, sq, qc * o[0]);
+                if constexpr (WANT_G) {
+#pragma unroll
+                    for (int k = 0; k < DV; ++k) o[k] *= kappa;
+                    o[0] += qc;
+                    T* grow = GBUF ? reinterpret_cast<T*>(gbuf + (size_t)(t % 3) * stage_bytes) + ((size_t)slot * n + ch) * DV : row;
+                    row_store<T, DV>(grow, o);
+                }
+            }
+        }
+        if constexpr (WANT_E) {
+            T* er2 = ered + (size_t)(t & 1) * THREADS;
+            if (warp_tree) {
+#pragma unroll
+                for (int o2 = 16; o2 > 0; o2 >>= 1) epart += __shfl_xor_sync(0xffffffffu, epart, o2);
+                if (lane == 0) er2[warp] = epart;
+            } else if (sub_tree) {
+                for (int o2 = n >> 1; o2 > 0; o2 >>= 1) epart += __shfl_xor_sync(0xffffffffu, epart, o2);
+                if (ch == 0 && active) er2[slot] = epart;
+            } else {
+                er2[tid] = epart;
+            }
         }
         fence_proxy_async();
         __syncthreads();
+        if constexpr (WANT_E) {
+            if (valid && ch == 0) {
+                const T* er2 = ered + (size_t)(t & 1) * THREADS;
+                T acc;
+                if (warp_tree) {
+                    const int wps = n >> 5;
+                    acc = er2[slot * wps];
+                    for (int k = 1; k < wps; ++k) acc += er2[slot * wps + k];
+                } else if (sub_tree) {
+                    acc = er2[slot];
+                } else {
+                    acc = er2[slot * n];
+                    for (int k = 1; k < n; ++k) acc += er2[slot * n + k];
+                }
+                e_edge[eb + slot] = acc;
+            }
+        }
         if (tid == 0) {
             const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-            bulk_store(out + (size_t)eb * n * DV, smem_raw + (size_t)s * stage_bytes, bytes);
-            bulk_commit();
+            if constexpr (WANT_OUT) bulk_store(out + (size_t)eb * n * DV, smem_raw + (size_t)s * stage_bytes, bytes);
+            if constexpr (WANT_G)
+                bulk_store(G + (size_t)eb * n * DV, GBUF ? gbuf + (size_t)(t % 3) * stage_bytes : smem_raw + (size_t)s * stage_bytes, bytes);
+            bulk_commit();  // one group per tile: the out and G stores of tile t
             if constexpr (NST == 1) {
                 if (t + 1 < ntiles) { bulk_wait_read<0>(); issue(t + 1); }  // single stage: store, then refill
             } else if (t >= 1 && t - 1 + NST < ntiles) {
-                bulk_wait_read<1>();  // the store of tile t-1 has finished reading its stage
+                bulk_wait_read<1>();  // the stores of tile t-1 have finished reading their stage (and G tile (t-1) % 3)
                 issue(t - 1 + NST);
+            } else if (GBUF && t >= 1) {
+                bulk_wait_read<1>();  // G tile (t-1) % 3 is written again by tile t+2
             }
         }
     }

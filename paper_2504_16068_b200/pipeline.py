@@ -48,9 +48,10 @@ def gpu_chain(inp, dev=None, items=None, want_gw=True, plan=None):
 class SingleLayerStep:
     """One MD step of one tensor-product layer with every buffer allocated once (nothing is allocated and no
     host synchronisation happens inside run()): the object bench.py times.  `want_gV` selects the full VJP
-    (dE/dV as well, what a layer inside a deeper network needs) or the force-only VJP."""
+    (dE/dV as well, what a layer inside a deeper network needs) or the force-only VJP; `fused_energy` uses
+    tp_forward_energy (out, e_edge and G from one kernel) instead of tp_forward followed by edge_energy."""
 
-    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None):
+    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, fused_energy=True, want_out=True):
         self.plan, self.dev, self.rc, self.kappa, self.scale = plan, dev, rc, kappa, scale
         rp, rvec, V = dev["row_ptr"], dev["rvec"], dev["V"]
         self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
@@ -59,7 +60,8 @@ class SingleLayerStep:
         n = plan.n
         self.w = torch.empty((self.E, n), dtype=dt, device=dv)
         self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
-        self.out = torch.empty_like(V)
+        self.fused_energy = fused_energy
+        self.out = torch.empty_like(V) if (want_out or not fused_energy) else None
         self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
         self.G = torch.empty_like(V)
         self.gV = torch.empty_like(V) if want_gV else None
@@ -91,8 +93,12 @@ class SingleLayerStep:
 
         timed("radial_forward", lambda: ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w))
         timed("env_embed", lambda: ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env))
-        timed("tp_forward", lambda: ab.tp_forward(p, rp, V, self.Eenv, pw, items=it, out=self.out))
-        timed("edge_energy", lambda: ab.edge_energy(p, self.out, d["q"], self.kappa, e_edge=self.e_edge, G=self.G))
+        if self.fused_energy:
+            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it,
+                                                                    want_out=self.out is not None, out=self.out, e_edge=self.e_edge, G=self.G))
+        else:
+            timed("tp_forward", lambda: ab.tp_forward(p, rp, V, self.Eenv, pw, items=it, out=self.out))
+            timed("edge_energy", lambda: ab.edge_energy(p, self.out, d["q"], self.kappa, e_edge=self.e_edge, G=self.G))
         timed("tp_backward", lambda: ab.tp_backward(p, rp, self.G, V, self.Eenv, pw, items=it, want_gV=self.gV is not None,
                                                     gV=self.gV, gEenv=self.gEenv, g_path_w=self.g_path_w, workspace=self.ws_bwd))
         timed("env_embed_backward", lambda: ab.env_embed_backward(p, rp, self.gEenv, rvec, self.w, self.scale, g_rvec=self.g_r, g_w=self.g_w))
@@ -114,6 +120,7 @@ class SingleLayerStep:
             "env_embed": E * 3 * s + wrow + env + (N + 1) * 4,
             "tp_forward": 2 * feat + env + (N + 1) * 4,
             "edge_energy": 2 * feat + E * s,
+            "tp_forward_energy": (3 if self.out is not None else 2) * feat + env + E * s + (N + 1) * 4,
             "tp_backward": (3 if self.gV is not None else 2) * feat + 2 * env + (N + 1) * 4,
             "env_embed_backward": env + E * 3 * s + wrow + wrow + E * 3 * s + (N + 1) * 4,
             "radial_backward": E * 3 * s + wrow + 2 * E * 3 * s,

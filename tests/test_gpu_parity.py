@@ -37,6 +37,34 @@ def test_chain_matches_oracle(name):
     assert np.abs(F.sum(0)).max() <= 1e-3 * np.abs(F).max() * (1.0 if inp["dt"] == np.float32 else 1e-8)
 
 
+@pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
+@pytest.mark.parametrize("want_out", [True, False])
+def test_forward_energy_epilogue(name, want_out):
+    """tp_forward_energy (out, e_edge, G from one kernel) against the oracle's tp_forward + edge_energy"""
+    import oracle as orc
+    import paper_2504_16068_b200 as ab
+    inp = _chain.make_inputs(name)
+    dev = _chain.to_device(inp)
+    f8 = lambda a: np.asarray(a, dtype=np.float64)
+    w, _ = orc.radial(f8(inp["W_r"]), inp["rc"], f8(inp["rvec"]))
+    Eenv = orc.env_embed(inp["lmax"], inp["row_ptr"], f8(inp["rvec"]), w, inp["scale"])
+    ref_out = orc.tp_forward(inp["lmax"], inp["row_ptr"], f8(inp["V"]), Eenv, f8(inp["path_w"]))
+    ref_e, ref_G = orc.edge_energy(inp["lmax"], ref_out, f8(inp["q"]), inp["kappa"])
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32)
+    import torch
+    Ed = torch.from_numpy(Eenv.astype(inp["dt"])).cuda()
+    for items in (None, ab.segments_build(inp["row_ptr"], 7)):
+        it = None if items is None else torch.from_numpy(items).cuda()
+        out, e, G = ab.tp_forward_energy(plan, dev["row_ptr"], dev["V"], Ed, dev["path_w"], dev["q"], inp["kappa"], items=it, want_out=want_out)
+        got = dict(out=out, e_edge=e, G=G)
+        assert (out is None) == (not want_out)
+        _assert_close(dict(out=ref_out, e_edge=ref_e, G=ref_G), got, inp["dt"], keys=("out", "e_edge", "G"), label=name)
+    # e_edge only next to out (no G)
+    out, e, G = ab.tp_forward_energy(plan, dev["row_ptr"], dev["V"], Ed, dev["path_w"], dev["q"], inp["kappa"], want_G=False)
+    assert G is None
+    _assert_close(dict(out=ref_out, e_edge=ref_e), dict(out=out, e_edge=e), inp["dt"], keys=("out", "e_edge"), label=name)
+
+
 def test_c4_fp64_variant():
     """configs[4] asks for fp32 and fp64: the same molecule batch in double"""
     inp = _chain.make_inputs("C4s")
@@ -140,7 +168,7 @@ def _check_sampled_centres(inp, got, ranges, label):
         sub = sub_inputs(inp, c0, c1)
         ref = _chain.oracle_chain(sub, want_gw=False, forces=False)
         e0, e1 = sub["edge_range"]
-        part = {k: got[k][e0:e1] for k in edge_keys}
+        part = {k: got[k][e0:e1] for k in edge_keys if got.get(k) is not None}
         part.update(Eenv=got["Eenv"][c0:c1], gEenv=got["gEenv"][c0:c1])
         _assert_close(ref, part, inp["dt"], keys=edge_keys + ("Eenv", "gEenv"), label="%s centres [%d,%d)" % (label, c0, c1))
 
@@ -166,5 +194,19 @@ def test_c1_full_size_sampled_centres():
     got = _chain.gpu_chain(inp, want_gw=False)
     N = inp["N"]
     starts = [int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(3), 0, N - 17)]
-    _check_sampled_centres(inp, got, [(c, c + 16) for c in starts + [0, N - 16]], "C1")
+    ranges = [(c, c + 16) for c in starts + [0, N - 16]]
+    _check_sampled_centres(inp, got, ranges, "C1")
     _check_force_gather(inp, got)
+    # the object bench.py times (preallocated buffers, fused forward + energy epilogue), same checks
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import SingleLayerStep
+    del got
+    dev = _chain.to_device(inp)
+    st = SingleLayerStep(ab.Plan(inp["lmax"], inp["n"], ab.F32), dev, inp["rc"], inp["kappa"], inp["scale"])
+    st.run()
+    got = dict(w=st.w, Eenv=st.Eenv, out=st.out, e_edge=st.e_edge, G=st.G, gV=st.gV, gEenv=st.gEenv, g_w=st.g_w, g_r=st.g_r, F=st.F)
+    _check_sampled_centres(inp, got, ranges, "C1/SingleLayerStep")
+    _check_force_gather(inp, got)
+    e_tot = float(st.e_tot.item())
+    e_ref = float(st.e_edge.double().sum().item())
+    assert abs(e_tot - e_ref) <= 1e-5 * abs(e_ref)
