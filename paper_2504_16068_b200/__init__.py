@@ -41,6 +41,8 @@ SIGNATURES = {
     "allegro_tp_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp]),
     "allegro_tp_forward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp]),
     "allegro_tp_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
+    "allegro_tp_backward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp,
+                                             C.c_size_t, _vp]),
     "allegro_tp_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_long, C.c_int]),
     "allegro_env_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
     "allegro_env_embed_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp]),
@@ -220,6 +222,24 @@ def tp_backward(plan, row_ptr, G, V, Eenv, path_w, items=None, want_gV=True, wan
     _check(lib().allegro_tp_backward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(V),
                                      _ptr(Eenv), _ptr(path_w), _ptr(gV), _ptr(gEenv), _ptr(g_path_w), _ptr(workspace),
                                      workspace.numel(), _stream(stream)))
+    return gV, gEenv, g_path_w
+
+
+def tp_backward_energy(plan, row_ptr, out, V, Eenv, path_w, q, kappa, items=None, want_gV=True, want_g_path_w=False, gV=None, gEenv=None,
+                       g_path_w=None, workspace=None, stream=None):
+    """-> (gV or None, gEenv, g_path_w or None); the cotangent G = q (x) delta + kappa out is formed in registers"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    if gV is None and want_gV:
+        gV = torch.empty_like(V)
+    if gEenv is None:
+        gEenv = torch.empty_like(Eenv)
+    if g_path_w is None and want_g_path_w:
+        g_path_w = torch.empty_like(path_w)
+    if workspace is None:
+        workspace = _ws(tp_backward_workspace(plan, n_atoms, n_edges, items, g_path_w is not None), V.device)
+    _check(lib().allegro_tp_backward_energy(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(out), _ptr(V),
+                                            _ptr(Eenv), _ptr(path_w), _ptr(q), float(kappa), _ptr(gV), _ptr(gEenv), _ptr(g_path_w),
+                                            _ptr(workspace), workspace.numel(), _stream(stream)))
     return gV, gEenv, g_path_w
 
 

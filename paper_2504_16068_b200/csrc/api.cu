@@ -184,6 +184,30 @@ allegro_status_t allegro_tp_backward(const allegro_plan_t* plan, int n_atoms, lo
     return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
 }
 
+allegro_status_t allegro_tp_backward_energy(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                            long n_items, const void* out, const void* V, const void* Eenv, const void* path_w, const void* q,
+                                            double kappa, void* gV, void* gEenv, void* g_path_w, void* workspace, size_t workspace_bytes,
+                                            void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((out && V) || n_edges == 0, "out / V is NULL");
+    ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr && q != nullptr, "path_w / q is NULL");
+    ALLEGRO_CHECK_ARG(gV == nullptr || (gV != out && gV != V), "gV aliases an input");
+    ALLEGRO_CHECK_ARG(aligned16(out) && aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace),
+                      "tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (plan->wmode != ALLEGRO_W_SCALAR) {
+        set_error("allegro_tp_backward_energy: scalar path weights only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.G = out; a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.q = q; a.kappa = kappa; a.gV = gV; a.gEenv = gEenv; a.g_path_w = g_path_w;
+    a.ws = workspace; a.ws_bytes = workspace_bytes; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
+}
+
 size_t allegro_tp_backward_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges, long n_items, int want_g_path_w) {
     (void)n_edges;
     if (!plan) return 0;

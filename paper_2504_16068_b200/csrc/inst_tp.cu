@@ -4,6 +4,8 @@
 #ifndef ALLEGRO_T
 #error "compile with -DALLEGRO_T=float|double -DALLEGRO_L=1|2|3"
 #endif
+#include <cstdlib>
+
 #include "common.cuh"
 
 namespace allegro {
@@ -23,19 +25,23 @@ namespace allegro {
 using Gen = TPGen<ALLEGRO_L>;
 
 template <typename T> struct Cfg {
-    static constexpr int THREADS = sizeof(T) == 4 ? 256 : 128;
+    static constexpr int THREADS = sizeof(T) == 4 ? 256 : 128;  // compute threads; one producer warp is added at launch
 };
 
+// Ring depth: as many stages as fit (<= 4) with two CTAs per SM; if that leaves fewer than 3, one CTA per SM
+// with up to 6 stages.  `extra` = barriers + reduction scratch.  ALLEGRO_NST overrides (experiments).
 static inline int pick_stages(size_t stage_bytes, size_t extra) {
-    // as many stages (<= 3) as fit next to `extra` in the 227 KB a CTA may use; the wrapper decides the
-    // occupancy through the total (several CTAs per SM when the stage is small)
-    const size_t cap2 = 110 * 1024;  // two CTAs per SM
-    const size_t cap1 = 220 * 1024;  // one CTA per SM
-    if (3 * stage_bytes + extra <= cap2) return 3;
-    if (2 * stage_bytes + extra <= cap2) return 2;
-    if (3 * stage_bytes + extra <= cap1) return 3;
-    if (2 * stage_bytes + extra <= cap1) return 2;
-    return 1;
+    const size_t cap2 = 113 * 1024, cap1 = 226 * 1024;
+    int nst = 1;
+    for (int k : {4, 3}) if (k * stage_bytes + extra <= cap2) { nst = k; break; }
+    if (nst == 1) {
+        for (int k : {6, 4, 3, 2}) if (k * stage_bytes + extra <= cap1) { nst = k; break; }
+    }
+    if (const char* e = getenv("ALLEGRO_NST")) {
+        const int k = atoi(e);
+        if (k >= 1 && k <= 6 && k * stage_bytes + extra <= cap1) nst = k;
+    }
+    return nst;
 }
 
 template <typename T>
@@ -67,31 +73,27 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     allegro_status_t s = fold_weights<T>(a);
     if (s != ALLEGRO_OK) return s;
     const int nslots = TH / a.n;
-    const size_t stage = align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
+    const size_t tile = align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
     const bool w_out = a.out != nullptr, w_g = a.Gout != nullptr, w_e = a.e_edge != nullptr;
-    const size_t extra = ((w_out && w_g) ? 3 * stage : 0) + 64 + 2 * TH * sizeof(T);
-    const int nst = pick_stages(stage, extra + 128);
+    const size_t stage = ((w_out && w_g) ? 2 : 1) * tile;
+    const size_t extra = 2 * 6 * 8 + 2 * TH * sizeof(T) + 64;
+    const int nst = pick_stages(stage, extra);
     const size_t smem = nst * stage + extra;
-#define ALLEGRO_FWD(NST, WO, WG, WE)                                                                               \
+#define ALLEGRO_FWD(WO, WG, WE)                                                                                    \
     {                                                                                                              \
-        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, NST, WO, WG, WE>;                                                 \
+        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, WO, WG, WE>;                                                      \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                       \
-        k<<<(unsigned)a.n_items, TH, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
-                                                   (const T*)a.q, (T)a.kappa, (T*)a.e_edge, (T*)a.Gout);           \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(nst, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
+                                                        (const T*)a.q, (T)a.kappa, (T*)a.e_edge, (T*)a.Gout);      \
     }
-#define ALLEGRO_FWD_N(WO, WG, WE) \
-    if (nst == 3) ALLEGRO_FWD(3, WO, WG, WE) else if (nst == 2) ALLEGRO_FWD(2, WO, WG, WE) else ALLEGRO_FWD(1, WO, WG, WE)
-    if (w_out && !w_g && !w_e) { ALLEGRO_FWD_N(true, false, false) }
-    else if (w_out && w_g && w_e) { ALLEGRO_FWD_N(true, true, true) }
-    else if (w_out && w_g) { ALLEGRO_FWD_N(true, true, false) }
-    else if (w_out && w_e) { ALLEGRO_FWD_N(true, false, true) }
-    else if (w_g && w_e) { ALLEGRO_FWD_N(false, true, true) }
-    else if (w_g) { ALLEGRO_FWD_N(false, true, false) }
+    if (w_out && !w_g && !w_e) { ALLEGRO_FWD(true, false, false) }
+    else if (w_out && w_g && w_e) { ALLEGRO_FWD(true, true, true) }
+    else if (w_out && w_e) { ALLEGRO_FWD(true, false, true) }
+    else if (w_g && w_e && !w_out) { ALLEGRO_FWD(false, true, true) }
     else {
-        set_error("tp_forward: nothing to store (out and G are both NULL)");
-        return ALLEGRO_EINVAL;
+        set_error("tp_forward_energy: unsupported output combination (G needs e_edge)");
+        return ALLEGRO_EUNSUPPORTED;
     }
-#undef ALLEGRO_FWD_N
 #undef ALLEGRO_FWD
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
@@ -139,24 +141,29 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
 
     const int nslots = TH / a.n;
     const size_t stage = 2 * (size_t)align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
-    const size_t red = 128 + (size_t)TH * Gen::DE * sizeof(T);
-    const int nst = pick_stages(stage, red + 256);
-    const size_t smem = nst * stage + red;
-#define ALLEGRO_BWD(NST, GV, GW)                                                                                          \
+    const size_t extra = 2 * 6 * 8 + 64;
+    const int nst = pick_stages(stage, extra);
+    const size_t smem = nst * stage + extra;
+    const bool cot = a.q != nullptr;  // tile 0 is `out`; the A12 cotangent is formed in registers
+#define ALLEGRO_BWD(GV, GW, COT)                                                                                          \
     {                                                                                                                     \
-        auto k = tp_bwd_kernel<T, ALLEGRO_L, TH, NST, GV, GW>;                                                                       \
+        auto k = tp_bwd_kernel<T, ALLEGRO_L, TH, GV, GW, COT>;                                                            \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                              \
-        k<<<(unsigned)a.n_items, TH, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
-                                                   (T*)a.gV, gE_dst, have_items ? 1 : 0, gw_part);                        \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(nst, a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
+                                                        (const T*)a.q, (T)a.kappa, (T*)a.gV, gE_dst, have_items ? 1 : 0, gw_part); \
     }
-#define ALLEGRO_BWD_N(GV, GW) \
-    if (nst == 3) ALLEGRO_BWD(3, GV, GW) else if (nst == 2) ALLEGRO_BWD(2, GV, GW) else ALLEGRO_BWD(1, GV, GW)
     const bool want_gv = a.gV != nullptr;
-    if (want_gv && want_gw) { ALLEGRO_BWD_N(true, true) }
-    else if (want_gv) { ALLEGRO_BWD_N(true, false) }
-    else if (want_gw) { ALLEGRO_BWD_N(false, true) }
-    else { ALLEGRO_BWD_N(false, false) }
-#undef ALLEGRO_BWD_N
+    if (cot) {
+        if (want_gv && want_gw) { ALLEGRO_BWD(true, true, true) }
+        else if (want_gv) { ALLEGRO_BWD(true, false, true) }
+        else if (want_gw) { ALLEGRO_BWD(false, true, true) }
+        else { ALLEGRO_BWD(false, false, true) }
+    } else {
+        if (want_gv && want_gw) { ALLEGRO_BWD(true, true, false) }
+        else if (want_gv) { ALLEGRO_BWD(true, false, false) }
+        else if (want_gw) { ALLEGRO_BWD(false, true, false) }
+        else { ALLEGRO_BWD(false, false, false) }
+    }
 #undef ALLEGRO_BWD
     ALLEGRO_LAUNCHED();
     if (have_items) {

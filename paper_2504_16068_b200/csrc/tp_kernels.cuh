@@ -4,25 +4,29 @@
 // Mapping (sm_100a):
 //   * one CTA per segment-plan item = (centre c, edges e0..e1) (A16).  A centre's edges are contiguous
 //     (CSR), so its feature rows V[e0..e1) are ONE contiguous byte range.
-//   * thread <-> (edge slot, channel): THREADS / n slots of n channels.  The centre's environment row
+//   * warp-specialised: CT compute threads + one producer warp.  The producer's elected lane streams tiles
+//     of `nslots` edges through an NST-stage shared-memory ring with 1-D bulk async copies (cp.async.bulk +
+//     mbarrier complete_tx; SASS UBLKCP), issues the bulk stores of finished tiles and refills a stage as
+//     soon as its store has been read out.  Compute warps only ever wait on a "full" mbarrier and signal
+//     "done" with one arrive per warp: there is no block-wide barrier in the steady state, so warps drift
+//     apart by up to NST tiles and HBM latency is covered by the ring, not by occupancy.
+//   * compute thread <-> (edge slot, channel): CT / n slots of n channels.  The centre's environment row
 //     Eenv[c][ch][:] stays in registers for the whole segment (north_star: "staging of each center
-//     atom's environment tile, which is reused across its neighbour edges").
-//   * V (and G) tiles of `nslots` edges stream through an NST-stage shared-memory ring filled by 1-D
-//     bulk async copies (cp.async.bulk + mbarrier complete_tx; SASS UBLKCP).  A thread reads its
-//     channel row with 64/128-bit LDS, runs the generated, fully unrolled sparse CG contraction
-//     (coefficients = constant-bank FFMA operands), writes the result row back IN PLACE and one thread
-//     issues the bulk store of the whole tile (shared -> global).  The outer product V (x) Eenv never
-//     exists anywhere.
-//   * no float atomics: the per-centre sums of gEenv run over slots in a fixed order.
+//     atom's environment tile, which is reused across its neighbour edges").  A thread reads its channel
+//     row with 64/128-bit LDS, runs the generated, fully unrolled sparse CG contraction (coefficients =
+//     constant-bank FFMA operands) and writes the result row back IN PLACE.  The outer product V (x) Eenv
+//     never exists anywhere.
+//   * no float atomics: every reduction has a fixed shape (xor trees, then warps / slots in order).
+//
+// NOTE: l_max is a template parameter of every kernel here.  The translation units inst_tp.cu (one per
+// l_max) would otherwise instantiate kernels with identical mangled names and different bodies, and the
+// linker keeps one of them (ODR): the wrong l_max's code would run.
 #pragma once
 #include "common.cuh"
 #include "launch.h"
 
 namespace allegro {
 
-// NOTE: l_max is a template parameter of every kernel here.  The translation units inst_tp.cu (one per
-// l_max) would otherwise instantiate kernels with identical mangled names and different bodies, and the
-// linker keeps one of them (ODR): the wrong l_max's code would run.
 static_assert(TPGen<ALLEGRO_L>::NNZ <= kCwMax, "coefficient table too small");
 
 // ------------------------------------------------------------------------------------------------
@@ -35,55 +39,138 @@ __global__ void fold_kernel(const T* __restrict__ path_w, T* __restrict__ cw) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Energy epilogue (reading A12), fused so that `out` is never re-read from HBM:
+// The tile ring shared by the kernels below.  A stage holds TILES tiles of `tile_bytes` (tile 0 is
+// overwritten in place by the result that is stored back).  full[s]: the stage's loads have landed
+// (transaction count); done[s]: all compute warps have finished with the stage (one arrive per warp).
+struct Ring {
+    unsigned char* base;
+    uint64_t* full;
+    uint64_t* done;
+    uint32_t tile_bytes, stage_bytes;
+    __device__ __forceinline__ unsigned char* stage(int s) const { return base + (size_t)s * stage_bytes; }
+};
+
+__device__ __forceinline__ void ring_init(const Ring& r, int tid, int compute_warps, int NST) {
+    if (tid == 0) {
+        for (int s = 0; s < NST; ++s) { mbar_init(&r.full[s], 1); mbar_init(&r.done[s], compute_warps); }
+        fence_mbar_init();
+    }
+    __syncthreads();
+}
+
+// compute side: every lane has written its rows; make them visible to the async proxy, then one arrive per warp
+__device__ __forceinline__ void ring_release(uint64_t* done_bar, int lane) {
+    fence_proxy_async();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(done_bar);
+}
+
+// how a per-edge quantity is summed over the n channel threads of a slot (fixed shape -> deterministic)
+//   n % 32 == 0             : xor tree inside each warp, then the slot's warps in order (named barrier per slot)
+//   n power of two below 32 : xor tree inside the slot's lanes
+//   otherwise               : the slot's channels in order (named barrier over all compute threads)
+enum { SUM_WARPS = 0, SUM_SUB = 1, SUM_SERIAL = 2 };
+__device__ __forceinline__ int slot_sum_mode(int n) { return (n % 32) == 0 ? SUM_WARPS : ((n < 32 && (n & (n - 1)) == 0) ? SUM_SUB : SUM_SERIAL); }
+
+// returns the slot total in the thread with ch == 0 (other threads: unspecified).  `buf` holds 2 * CT values
+// (double-buffered by tile parity so that a fast warp cannot overwrite partials that are still being read).
+template <typename T, int CT>
+__device__ __forceinline__ T slot_sum(T x, int mode, int n, int slot, int ch, int tid, int t, T* buf) {
+    T* b = buf + (size_t)(t & 1) * CT;
+    const int lane = tid & 31, warp = tid >> 5;
+    if (mode == SUM_WARPS) {
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        const int wps = n >> 5;
+        if (wps == 1) return x;
+        if (lane == 0) b[warp] = x;
+        named_bar(1 + slot, n);
+        if (ch == 0) {
+            x = b[slot * wps];
+            for (int k = 1; k < wps; ++k) x += b[slot * wps + k];
+        }
+        return x;
+    } else if (mode == SUM_SUB) {
+        for (int o = n >> 1; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
+        return x;
+    } else {
+        b[tid] = x;
+        named_bar(1, CT);
+        if (ch == 0 && slot * n + n <= CT) {
+            x = b[slot * n];
+            for (int k = 1; k < n; ++k) x += b[slot * n + k];
+        }
+        return x;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Forward, optionally with the energy epilogue of reading A12 fused so that `out` is never
+// re-read from HBM:
 //   e_edge[e] = sum_ch ( q[ch] out[e][ch][0] + kappa/2 sum_k out[e][ch][k]^2 ),   G = q (x) delta_{k,0} + kappa out
 // WANT_OUT / WANT_G / WANT_E select which of out, G, e_edge are produced (at least one of out, G).
-// Shared memory: NST stages of V (each becomes the out tile, or the G tile when !WANT_OUT, in place), then
-// 3 G tiles when both out and G are stored, then the mbarriers, then the energy partials.
-template <typename T, int L, int THREADS, int NST, bool WANT_OUT, bool WANT_G, bool WANT_E>
-__global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
+// Stage = [V tile -> out tile (or G tile when !WANT_OUT)] [G tile when both are stored].
+template <typename T, int L, int CT, bool WANT_OUT, bool WANT_G, bool WANT_E>
+__global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                           const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ out,
                                                           const T* __restrict__ q, T kappa, T* __restrict__ e_edge, T* __restrict__ G) {
     using Gen = TPGen<L>;
     constexpr int DV = Gen::DV, DE = Gen::DE;
     constexpr bool EPI = WANT_G || WANT_E;
-    constexpr bool GBUF = WANT_OUT && WANT_G;  // separate G tiles
+    constexpr int TILES = (WANT_OUT && WANT_G) ? 2 : 1;
     static_assert(WANT_OUT || WANT_G, "nothing to store");
     extern __shared__ __align__(128) unsigned char smem_raw[];
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int nslots = THREADS / n;
-    const int slot = tid / n, ch = tid - slot * n;
-    const bool active = slot < nslots;
+    const int nslots = CT / n;
     const uint32_t row_bytes = (uint32_t)n * DV * sizeof(T);
-    const uint32_t stage_bytes = align128((size_t)nslots * row_bytes);
-    unsigned char* gbuf = smem_raw + (size_t)NST * stage_bytes;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(gbuf + (GBUF ? 3 : 0) * (size_t)stage_bytes);
-    T* ered = reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(bars) + 64);  // [2][THREADS / 32] or [2][THREADS]
+    Ring r;
+    r.base = smem_raw;
+    r.tile_bytes = align128((size_t)nslots * row_bytes);
+    r.stage_bytes = TILES * r.tile_bytes;
+    r.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NST * r.stage_bytes);
+    r.done = r.full + NST;
+    T* ebuf = reinterpret_cast<T*>(r.done + NST);  // [2][CT]
 
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
     const int ntiles = (e1 - e0 + nslots - 1) / nslots;
     if (ntiles <= 0) return;
+    ring_init(r, tid, CT / 32, NST);
 
-    if (tid == 0) {
-#pragma unroll
-        for (int s = 0; s < NST; ++s) mbar_init(&bars[s], 1);
-        fence_mbar_init();
-    }
-    __syncthreads();
-
-    auto issue = [&](int t) {
-        const int s = t % NST;
-        const int eb = e0 + t * nslots;
-        const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-        mbar_expect_tx(&bars[s], bytes);
-        bulk_load(smem_raw + (size_t)s * stage_bytes, V + (size_t)eb * n * DV, bytes, &bars[s]);
-    };
-    if (tid == 0) {
+    if (warp == CT / 32) {
+        // ---------------------------------------------------------------- producer
+        if (lane != 0) return;
+        auto issue = [&](int t) {
+            const int s = t % NST;
+            const int eb = e0 + t * nslots;
+            const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
+            mbar_expect_tx(&r.full[s], bytes);
+            bulk_load(r.stage(s), V + (size_t)eb * n * DV, bytes, &r.full[s]);
+        };
         const int pre = ntiles < NST ? ntiles : NST;
         for (int t = 0; t < pre; ++t) issue(t);
+        for (int u = 0; u < ntiles; ++u) {
+            const int s = u % NST;
+            mbar_wait(&r.done[s], (uint32_t)(u / NST) & 1u);
+            const int eb = e0 + u * nslots;
+            const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
+            if constexpr (WANT_OUT) bulk_store(out + (size_t)eb * n * DV, r.stage(s), bytes);
+            if constexpr (WANT_G) bulk_store(G + (size_t)eb * n * DV, r.stage(s) + (TILES - 1) * r.tile_bytes, bytes);
+            bulk_commit();  // one group per tile
+            if (NST == 1) {
+                if (u + 1 < ntiles) { bulk_wait_read<0>(); issue(u + 1); }
+            } else if (u >= 1 && u - 1 + NST < ntiles) {
+                bulk_wait_read<1>();  // the stores of tile u-1 have finished reading their stage
+                issue(u - 1 + NST);
+            }
+        }
+        bulk_wait_read<0>();  // shared memory must outlive the last store's read
+        return;
     }
 
+    // -------------------------------------------------------------------- compute warps
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = slot < nslots;
     T E[DE];
     T qc = T(0);
     if (active) {
@@ -95,19 +182,16 @@ __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __res
 #pragma unroll
         for (int j = 0; j < DE; ++j) E[j] = T(0);
     }
-    // how the per-edge energy is summed over the slot's n channels (fixed shape): whole warps -> xor tree + the
-    // slot's warps in order; n a power of two below 32 -> xor tree inside the slot's lanes; otherwise channels in order
-    const bool warp_tree = (n % 32) == 0;
-    const bool sub_tree = n < 32 && (n & (n - 1)) == 0;
+    const int mode = slot_sum_mode(n);
 
     for (int t = 0; t < ntiles; ++t) {
         const int s = t % NST;
-        mbar_wait(&bars[s], (uint32_t)(t / NST) & 1u);
+        mbar_wait(&r.full[s], (uint32_t)(t / NST) & 1u);
         const int eb = e0 + t * nslots;
         const bool valid = active && eb + slot < e1;
         T epart = T(0);
         if (valid) {
-            T* row = reinterpret_cast<T*>(smem_raw + (size_t)s * stage_bytes) + ((size_t)slot * n + ch) * DV;
+            T* row = reinterpret_cast<T*>(r.stage(s)) + ((size_t)slot * n + ch) * DV;
             T v[DV], o[DV];
             row_load<T, DV>(row, v);
             Gen::template fwd<T>(v, E, o);
@@ -121,162 +205,135 @@ __global__ void __launch_bounds__(THREADS) tp_fwd_kernel(int n, const int* __res
 #pragma unroll
                     for (int k = 0; k < DV; ++k) o[k] *= kappa;
                     o[0] += qc;
-                    T* grow = GBUF ? reinterpret_cast<T*>(gbuf + (size_t)(t % 3) * stage_bytes) + ((size_t)slot * n + ch) * DV : row;
-                    row_store<T, DV>(grow, o);
+                    row_store<T, DV>(reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(row) + (TILES - 1) * r.tile_bytes), o);
                 }
             }
         }
+        ring_release(&r.done[s], lane);
         if constexpr (WANT_E) {
-            T* er2 = ered + (size_t)(t & 1) * THREADS;
-            if (warp_tree) {
-#pragma unroll
-                for (int o2 = 16; o2 > 0; o2 >>= 1) epart += __shfl_xor_sync(0xffffffffu, epart, o2);
-                if (lane == 0) er2[warp] = epart;
-            } else if (sub_tree) {
-                for (int o2 = n >> 1; o2 > 0; o2 >>= 1) epart += __shfl_xor_sync(0xffffffffu, epart, o2);
-                if (ch == 0 && active) er2[slot] = epart;
-            } else {
-                er2[tid] = epart;
-            }
-        }
-        fence_proxy_async();
-        __syncthreads();
-        if constexpr (WANT_E) {
-            if (valid && ch == 0) {
-                const T* er2 = ered + (size_t)(t & 1) * THREADS;
-                T acc;
-                if (warp_tree) {
-                    const int wps = n >> 5;
-                    acc = er2[slot * wps];
-                    for (int k = 1; k < wps; ++k) acc += er2[slot * wps + k];
-                } else if (sub_tree) {
-                    acc = er2[slot];
-                } else {
-                    acc = er2[slot * n];
-                    for (int k = 1; k < n; ++k) acc += er2[slot * n + k];
-                }
-                e_edge[eb + slot] = acc;
-            }
-        }
-        if (tid == 0) {
-            const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-            if constexpr (WANT_OUT) bulk_store(out + (size_t)eb * n * DV, smem_raw + (size_t)s * stage_bytes, bytes);
-            if constexpr (WANT_G)
-                bulk_store(G + (size_t)eb * n * DV, GBUF ? gbuf + (size_t)(t % 3) * stage_bytes : smem_raw + (size_t)s * stage_bytes, bytes);
-            bulk_commit();  // one group per tile: the out and G stores of tile t
-            if constexpr (NST == 1) {
-                if (t + 1 < ntiles) { bulk_wait_read<0>(); issue(t + 1); }  // single stage: store, then refill
-            } else if (t >= 1 && t - 1 + NST < ntiles) {
-                bulk_wait_read<1>();  // the stores of tile t-1 have finished reading their stage (and G tile (t-1) % 3)
-                issue(t - 1 + NST);
-            } else if (GBUF && t >= 1) {
-                bulk_wait_read<1>();  // G tile (t-1) % 3 is written again by tile t+2
-            }
+            const T tot = slot_sum<T, CT>(epart, mode, n, slot, ch, tid, t, ebuf);
+            if (valid && ch == 0) e_edge[eb + slot] = tot;
         }
     }
-    if (tid == 0) bulk_wait_read<0>();
 }
 
 // ------------------------------------------------------------------------------------------------
 // First derivative.  Stage = [G tile | V tile]; gV overwrites the G tile in place and is
 // bulk-stored; gEenv accumulates in registers over the thread's edges, then over slots in slot order.
+// COT: tile 0 is loaded from `out` instead of G and the cotangent of the A12 energy, G = q (x) delta_{k,0} +
+// kappa out, is formed in registers (G never exists in HBM).
 // WANT_GW adds the path-weight gradient: per-thread accumulators -> fixed-shape warp tree -> warps in
 // order -> one partial row per item (reduced over items by gw_final_kernel).
-template <typename T, int L, int THREADS, int NST, bool WANT_GV, bool WANT_GW>
-__global__ void __launch_bounds__(THREADS)
-    tp_bwd_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
-                  const T* __restrict__ Eenv, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item, T* __restrict__ gw_part) {
+template <typename T, int L, int CT, bool WANT_GV, bool WANT_GW, bool COT>
+__global__ void __launch_bounds__(CT + 32)
+    tp_bwd_kernel(int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
+                  const T* __restrict__ Eenv, const T* __restrict__ q, T kappa, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item,
+                  T* __restrict__ gw_part) {
     using Gen = TPGen<L>;
     constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P;
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int tid = threadIdx.x;
-    const int nslots = THREADS / n;
-    const int slot = tid / n, ch = tid - slot * n;
-    const bool active = slot < nslots;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nslots = CT / n;
     const uint32_t row_bytes = (uint32_t)n * DV * sizeof(T);
-    const uint32_t tile_bytes = align128((size_t)nslots * row_bytes);
-    const uint32_t stage_bytes = 2 * tile_bytes;
-    uint64_t* bars = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NST * stage_bytes);
-    T* red = reinterpret_cast<T*>(smem_raw + (size_t)NST * stage_bytes + 128);  // [THREADS][DE] or [warps][P]
+    Ring r;
+    r.base = smem_raw;
+    r.tile_bytes = align128((size_t)nslots * row_bytes);
+    r.stage_bytes = 2 * r.tile_bytes;
+    r.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NST * r.stage_bytes);
+    r.done = r.full + NST;
 
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
     const int ntiles = (e1 - e0 + nslots - 1) / nslots;
+    ring_init(r, tid, CT / 32, NST);
 
-    if (tid == 0) {
+    const bool compute = warp < CT / 32;
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = compute && slot < nslots;
+    T gE[DE];
 #pragma unroll
-        for (int s = 0; s < NST; ++s) mbar_init(&bars[s], 1);
-        fence_mbar_init();
-    }
-    __syncthreads();
-
-    auto issue = [&](int t) {
-        const int s = t % NST;
-        const int eb = e0 + t * nslots;
-        const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-        unsigned char* st = smem_raw + (size_t)s * stage_bytes;
-        mbar_expect_tx(&bars[s], 2 * bytes);
-        bulk_load(st, G + (size_t)eb * n * DV, bytes, &bars[s]);
-        bulk_load(st + tile_bytes, V + (size_t)eb * n * DV, bytes, &bars[s]);
-    };
-    if (tid == 0) {
-        const int pre = ntiles < NST ? ntiles : NST;
-        for (int t = 0; t < pre; ++t) issue(t);
-    }
-
-    T E[DE], gE[DE];
-#pragma unroll
-    for (int j = 0; j < DE; ++j) { E[j] = T(0); gE[j] = T(0); }
-    if (active) {
-        const T* er = Eenv + ((size_t)c * n + ch) * DE;
-#pragma unroll
-        for (int j = 0; j < DE; ++j) E[j] = er[j];
-    }
+    for (int j = 0; j < DE; ++j) gE[j] = T(0);
     T gw[WANT_GW ? P : 1];
 #pragma unroll
     for (int p = 0; p < (WANT_GW ? P : 1); ++p) gw[p] = T(0);
 
-    for (int t = 0; t < ntiles; ++t) {
-        const int s = t % NST;
-        mbar_wait(&bars[s], (uint32_t)(t / NST) & 1u);
-        const int eb = e0 + t * nslots;
-        unsigned char* st = smem_raw + (size_t)s * stage_bytes;
-        if (active && eb + slot < e1) {
-            T* grow = reinterpret_cast<T*>(st) + ((size_t)slot * n + ch) * DV;
-            const T* vrow = reinterpret_cast<const T*>(st + tile_bytes) + ((size_t)slot * n + ch) * DV;
-            T v[DV], g[DV], gv[DV];
-            row_load<T, DV>(grow, g);
-            row_load<T, DV>(vrow, v);
-            Gen::template bwd<T, WANT_GV>(v, E, g, gv, gE);
-            if constexpr (WANT_GW) Gen::template pathw<T>(v, E, g, gw);
-            if constexpr (WANT_GV) row_store<T, DV>(grow, gv);
-        }
-        if constexpr (WANT_GV) fence_proxy_async();
-        __syncthreads();
-        if (tid == 0) {
-            if constexpr (WANT_GV) {
+    if (!compute) {
+        // ---------------------------------------------------------------- producer
+        if (lane == 0) {
+            auto issue = [&](int t) {
+                const int s = t % NST;
+                const int eb = e0 + t * nslots;
                 const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-                bulk_store(gV + (size_t)eb * n * DV, st, bytes);
-                bulk_commit();
-                if constexpr (NST == 1) {
-                    if (t + 1 < ntiles) { bulk_wait_read<0>(); issue(t + 1); }
-                } else if (t >= 1 && t - 1 + NST < ntiles) {
-                    bulk_wait_read<1>();
-                    issue(t - 1 + NST);
+                mbar_expect_tx(&r.full[s], 2 * bytes);
+                bulk_load(r.stage(s), G + (size_t)eb * n * DV, bytes, &r.full[s]);
+                bulk_load(r.stage(s) + r.tile_bytes, V + (size_t)eb * n * DV, bytes, &r.full[s]);
+            };
+            const int pre = ntiles < NST ? ntiles : NST;
+            for (int t = 0; t < pre; ++t) issue(t);
+            for (int u = 0; u < ntiles; ++u) {
+                const int s = u % NST;
+                mbar_wait(&r.done[s], (uint32_t)(u / NST) & 1u);
+                if constexpr (WANT_GV) {
+                    const int eb = e0 + u * nslots;
+                    const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
+                    bulk_store(gV + (size_t)eb * n * DV, r.stage(s), bytes);
+                    bulk_commit();
+                    if (NST == 1) {
+                        if (u + 1 < ntiles) { bulk_wait_read<0>(); issue(u + 1); }
+                    } else if (u >= 1 && u - 1 + NST < ntiles) {
+                        bulk_wait_read<1>();
+                        issue(u - 1 + NST);
+                    }
+                } else {
+                    if (u + NST < ntiles) issue(u + NST);  // every warp is done with stage s
                 }
-            } else {
-                if (t + NST < ntiles) issue(t + NST);  // every thread is done with stage s
             }
+            if constexpr (WANT_GV) bulk_wait_read<0>();
+        }
+    } else {
+        // ---------------------------------------------------------------- compute warps
+        T E[DE];
+        T qc = T(0);
+#pragma unroll
+        for (int j = 0; j < DE; ++j) E[j] = T(0);
+        if (active) {
+            const T* er = Eenv + ((size_t)c * n + ch) * DE;
+#pragma unroll
+            for (int j = 0; j < DE; ++j) E[j] = er[j];
+            if constexpr (COT) qc = q[ch];
+        }
+        for (int t = 0; t < ntiles; ++t) {
+            const int s = t % NST;
+            mbar_wait(&r.full[s], (uint32_t)(t / NST) & 1u);
+            const int eb = e0 + t * nslots;
+            if (active && eb + slot < e1) {
+                T* grow = reinterpret_cast<T*>(r.stage(s)) + ((size_t)slot * n + ch) * DV;
+                const T* vrow = reinterpret_cast<const T*>(r.stage(s) + r.tile_bytes) + ((size_t)slot * n + ch) * DV;
+                T v[DV], g[DV], gv[DV];
+                row_load<T, DV>(grow, g);
+                row_load<T, DV>(vrow, v);
+                if constexpr (COT) {
+#pragma unroll
+                    for (int k = 0; k < DV; ++k) g[k] *= kappa;
+                    g[0] += qc;
+                }
+                Gen::template bwd<T, WANT_GV>(v, E, g, gv, gE);
+                if constexpr (WANT_GW) Gen::template pathw<T>(v, E, g, gw);
+                if constexpr (WANT_GV) row_store<T, DV>(grow, gv);
+            }
+            ring_release(&r.done[s], lane);
         }
     }
+    __syncthreads();  // all tiles are computed and every store has left shared memory: the ring can be reused
 
     // ---- gEenv: slots summed in slot order
+    T* red = reinterpret_cast<T*>(smem_raw);  // [CT][DE], then [warps][P]
     if (active) {
 #pragma unroll
         for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = gE[j];
     }
     __syncthreads();
-    if (slot == 0) {
+    if (compute && slot == 0) {
         T* dst = gE_dst + ((size_t)(gE_by_item ? (long)blockIdx.x : (long)c) * n + ch) * DE;
 #pragma unroll
         for (int j = 0; j < DE; ++j) {
@@ -287,23 +344,21 @@ __global__ void __launch_bounds__(THREADS)
     }
     if constexpr (WANT_GW) {
         __syncthreads();
-        const int lane = tid & 31, warp = tid >> 5;
+        if (compute) {
 #pragma unroll
-        for (int p = 0; p < P; ++p) {
-            T a = gw[p];
+            for (int p = 0; p < P; ++p) {
+                T a = gw[p];
 #pragma unroll
-            for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
-            if (lane == 0) red[warp * P + p] = a;
+                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                if (lane == 0) red[warp * P + p] = a;
+            }
         }
         __syncthreads();
         if (tid < P) {
             T acc = red[tid];
-            for (int wv = 1; wv < THREADS / 32; ++wv) acc += red[wv * P + tid];
+            for (int wv = 1; wv < CT / 32; ++wv) acc += red[wv * P + tid];
             gw_part[(size_t)blockIdx.x * P + tid] = acc;
         }
-    }
-    if constexpr (WANT_GV) {
-        if (tid == 0) bulk_wait_read<0>();
     }
 }
 

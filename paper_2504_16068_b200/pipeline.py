@@ -48,11 +48,15 @@ def gpu_chain(inp, dev=None, items=None, want_gw=True, plan=None):
 class SingleLayerStep:
     """One MD step of one tensor-product layer with every buffer allocated once (nothing is allocated and no
     host synchronisation happens inside run()): the object bench.py times.  `want_gV` selects the full VJP
-    (dE/dV as well, what a layer inside a deeper network needs) or the force-only VJP; `fused_energy` uses
-    tp_forward_energy (out, e_edge and G from one kernel) instead of tp_forward followed by edge_energy."""
+    (dE/dV as well, what a layer inside a deeper network needs) or the force-only VJP.  `mode`:
+      "separate" : tp_forward -> edge_energy -> tp_backward                     (out, G both cross HBM twice)
+      "epilogue" : tp_forward_energy (out, e_edge, G from one kernel) -> tp_backward
+      "onthefly" : tp_forward_energy (out, e_edge) -> tp_backward_energy (cotangent formed from out in registers;
+                   G never exists in HBM)"""
 
-    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, fused_energy=True, want_out=True):
-        self.plan, self.dev, self.rc, self.kappa, self.scale = plan, dev, rc, kappa, scale
+    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, mode="onthefly"):
+        assert mode in ("separate", "epilogue", "onthefly")
+        self.plan, self.dev, self.rc, self.kappa, self.scale, self.mode = plan, dev, rc, kappa, scale, mode
         rp, rvec, V = dev["row_ptr"], dev["rvec"], dev["V"]
         self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
         self.items = items
@@ -60,10 +64,9 @@ class SingleLayerStep:
         n = plan.n
         self.w = torch.empty((self.E, n), dtype=dt, device=dv)
         self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
-        self.fused_energy = fused_energy
-        self.out = torch.empty_like(V) if (want_out or not fused_energy) else None
+        self.out = torch.empty_like(V)
         self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
-        self.G = torch.empty_like(V)
+        self.G = torch.empty_like(V) if mode != "onthefly" else None
         self.gV = torch.empty_like(V) if want_gV else None
         self.gEenv = torch.empty_like(self.Eenv)
         self.g_path_w = torch.empty((plan.P,), dtype=dt, device=dv) if want_g_path_w else None
@@ -91,16 +94,21 @@ class SingleLayerStep:
             ev.append((name, a, b))
             return r
 
+        bw = dict(items=it, want_gV=self.gV is not None, gV=self.gV, gEenv=self.gEenv, g_path_w=self.g_path_w, workspace=self.ws_bwd)
         timed("radial_forward", lambda: ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w))
         timed("env_embed", lambda: ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env))
-        if self.fused_energy:
-            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it,
-                                                                    want_out=self.out is not None, out=self.out, e_edge=self.e_edge, G=self.G))
-        else:
+        if self.mode == "separate":
             timed("tp_forward", lambda: ab.tp_forward(p, rp, V, self.Eenv, pw, items=it, out=self.out))
             timed("edge_energy", lambda: ab.edge_energy(p, self.out, d["q"], self.kappa, e_edge=self.e_edge, G=self.G))
-        timed("tp_backward", lambda: ab.tp_backward(p, rp, self.G, V, self.Eenv, pw, items=it, want_gV=self.gV is not None,
-                                                    gV=self.gV, gEenv=self.gEenv, g_path_w=self.g_path_w, workspace=self.ws_bwd))
+            timed("tp_backward", lambda: ab.tp_backward(p, rp, self.G, V, self.Eenv, pw, **bw))
+        elif self.mode == "epilogue":
+            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it, out=self.out,
+                                                                    e_edge=self.e_edge, G=self.G))
+            timed("tp_backward", lambda: ab.tp_backward(p, rp, self.G, V, self.Eenv, pw, **bw))
+        else:
+            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it, out=self.out,
+                                                                    e_edge=self.e_edge, want_G=False))
+            timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp, self.out, V, self.Eenv, pw, d["q"], self.kappa, **bw))
         timed("env_embed_backward", lambda: ab.env_embed_backward(p, rp, self.gEenv, rvec, self.w, self.scale, g_rvec=self.g_r, g_w=self.g_w))
         timed("radial_backward", lambda: ab.radial_backward(rvec, d["W_r"], self.rc, self.g_w, self.g_r))
         timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
@@ -115,13 +123,15 @@ class SingleLayerStep:
         s = 4 if p.dtype == ab.F32 else 8
         E, N, n, dV, dE = self.E, self.N, p.n, p.dV, p.dE
         feat, env, wrow = E * n * dV * s, N * n * dE * s, E * n * s
+        bwd = (3 if self.gV is not None else 2) * feat + 2 * env + (N + 1) * 4
         return {
             "radial_forward": E * 3 * s + wrow,
             "env_embed": E * 3 * s + wrow + env + (N + 1) * 4,
             "tp_forward": 2 * feat + env + (N + 1) * 4,
             "edge_energy": 2 * feat + E * s,
-            "tp_forward_energy": (3 if self.out is not None else 2) * feat + env + E * s + (N + 1) * 4,
-            "tp_backward": (3 if self.gV is not None else 2) * feat + 2 * env + (N + 1) * 4,
+            "tp_forward_energy": (3 if self.G is not None else 2) * feat + env + E * s + (N + 1) * 4,
+            "tp_backward": bwd,
+            "tp_backward_energy": bwd,
             "env_embed_backward": env + E * 3 * s + wrow + wrow + E * 3 * s + (N + 1) * 4,
             "radial_backward": E * 3 * s + wrow + 2 * E * 3 * s,
             "force_gather": 2 * E * 3 * s + E * 4 + N * 3 * s + (N + 1) * 4,

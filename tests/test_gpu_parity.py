@@ -65,6 +65,34 @@ def test_forward_energy_epilogue(name, want_out):
     _assert_close(dict(out=ref_out, e_edge=ref_e), dict(out=out, e_edge=e), inp["dt"], keys=("out", "e_edge"), label=name)
 
 
+@pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
+@pytest.mark.parametrize("mode", ["separate", "epilogue", "onthefly"])
+def test_single_layer_step_modes(name, mode):
+    """the three call sequences of pipeline.SingleLayerStep (the object bench.py times) give the oracle's forces,
+    energies and gradients; "onthefly" exercises tp_backward_energy (cotangent formed from out in registers)"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import SingleLayerStep
+    inp = _chain.make_inputs(name)
+    ref = _chain.oracle_chain(inp)
+    dev = _chain.to_device(inp)
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32)
+    for items in (None, ab.segments_build(inp["row_ptr"], 9)):
+        it = None if items is None else torch.from_numpy(items).cuda()
+        st = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_g_path_w=True, items=it, mode=mode)
+        st.run()
+        got = dict(w=st.w, Eenv=st.Eenv, out=st.out, e_edge=st.e_edge, G=st.G, gV=st.gV, gEenv=st.gEenv, g_path_w=st.g_path_w,
+                   g_w=st.g_w, g_r=st.g_r, F=st.F)
+        _assert_close(ref, got, inp["dt"], label="%s/%s" % (name, mode))
+        e_ref = float(np.sum(ref["e_edge"]))
+        assert abs(float(st.e_tot.item()) - e_ref) <= _chain.TOL[inp["dt"]] * max(abs(e_ref), float(np.abs(ref["e_edge"]).max()))
+        # force-only VJP (gV = NULL) gives the same gEenv bits or values within tolerance
+        st2 = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=False, items=it, mode=mode)
+        st2.run()
+        _assert_close(ref, dict(gEenv=st2.gEenv, F=st2.F), inp["dt"], keys=("gEenv", "F"), label="%s/%s/force-only" % (name, mode))
+
+
 def test_c4_fp64_variant():
     """configs[4] asks for fp32 and fp64: the same molecule batch in double"""
     inp = _chain.make_inputs("C4s")
