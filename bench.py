@@ -41,6 +41,7 @@ def parse_args():
     ap.add_argument("--workload", default="C1")
     ap.add_argument("--force-only", action="store_true", help="skip dE/dV (valid when V does not depend on positions)")
     ap.add_argument("--mode", default="onthefly", choices=["separate", "epilogue", "onthefly"], help="call sequence (pipeline.SingleLayerStep)")
+    ap.add_argument("--separate-geometry", action="store_true", help="radial / env-embed as four kernels instead of the two fused ones")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -186,7 +187,7 @@ def run_ours(args):
     inp = make_inputs(name, seed=rank, features="device")
     dev = to_device(inp)
     plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32, ab.W_SCALAR)
-    step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only, mode=args.mode)
+    step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only, mode=args.mode, fused_geometry=not args.separate_geometry)
     E, N = step.E, step.N
 
     def barrier():
@@ -264,7 +265,8 @@ def run_ours(args):
                                    "single TP layer forward + %s" % (name, N, E, inp["lmax"], inp["n"],
                                                                      "force-only VJP" if args.force_only else "full VJP (gV, gEenv) + forces"),
                        "atoms": N, "edges": E, "l_max": inp["lmax"], "n_channels": inp["n"], "parallelism": "independent systems per GPU", "mode": args.mode,
-                       "l2": "not flushed: every feature tensor (%.2f GB) exceeds the 126 MB L2" % (abytes["tp_forward"] / 2 / 1e9)},
+                       "l2": "not flushed: every feature tensor (%.2f GB) exceeds the 126 MB L2" % (abytes["tp_forward"] / 2 / 1e9),
+                       "fused_geometry": not args.separate_geometry},
             "atom_steps_per_s": world * N / (ms_step * 1e-3),
             "step_GBps_algorithmic": step_bytes / (ms_step * 1e-3) / 1e9, "step_frac_of_hbm_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
             "roofline": roofline, "calls": calls, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),

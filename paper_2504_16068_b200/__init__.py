@@ -49,6 +49,9 @@ SIGNATURES = {
     "allegro_force_gather": (C.c_int, [C.c_int, C.c_long, _vp, _vp, _vp, C.c_int, _vp, _vp]),
     "allegro_radial_forward": (C.c_int, [C.c_int, C.c_int, C.c_double, C.c_int, C.c_long, _vp, _vp, _vp, _vp]),
     "allegro_radial_backward": (C.c_int, [C.c_int, C.c_int, C.c_double, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_env_radial_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, C.c_int, C.c_double, C.c_double, _vp, _vp, _vp,
+                                             C.c_size_t, _vp]),
+    "allegro_env_radial_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, C.c_double, C.c_double, _vp, _vp, _vp]),
     "allegro_edge_energy": (C.c_int, [_vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_segment_sum": (C.c_int, [_vp, C.c_int, _vp, C.c_int, _vp, _vp]),
     "allegro_status_str": (C.c_char_p, [C.c_int]),
@@ -281,6 +284,33 @@ def radial_backward(rvec, W_r, r_cut, g_w, g_rvec, stream=None):
     _check(lib().allegro_radial_backward(n, nb, float(r_cut), _dt(rvec), rvec.shape[0], _ptr(rvec), _ptr(W_r), _ptr(g_w), _ptr(g_rvec),
                                          _stream(stream)))
     return g_rvec
+
+
+def env_radial_forward(plan, row_ptr, rvec, W_r, r_cut, scale=1.0, items=None, want_w=False, w=None, Eenv=None, workspace=None, stream=None):
+    """-> (Eenv, w or None): radial weights + Y_lm + environment embedding in one kernel"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if Eenv is None:
+        Eenv = torch.empty((n_atoms, plan.n, plan.dE), dtype=plan.tdtype, device=rvec.device)
+    if w is None and want_w:
+        w = torch.empty((n_edges, plan.n), dtype=plan.tdtype, device=rvec.device)
+    if workspace is None and items is not None:
+        workspace = _ws(env_workspace(plan, n_atoms, items), rvec.device)
+    _check(lib().allegro_env_radial_forward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(rvec), _ptr(W_r),
+                                            W_r.shape[1], float(r_cut), float(scale), _ptr(w), _ptr(Eenv), _ptr(workspace),
+                                            0 if workspace is None else workspace.numel(), _stream(stream)))
+    return Eenv, w
+
+
+def env_radial_backward(plan, row_ptr, gEenv, rvec, W_r, r_cut, scale=1.0, want_g_w=False, g_rvec=None, g_w=None, stream=None):
+    """-> (g_rvec[E,3] complete dE/dr_e, g_w or None): embedding VJP + radial chain rule in one kernel"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if g_rvec is None:
+        g_rvec = torch.empty_like(rvec)
+    if g_w is None and want_g_w:
+        g_w = torch.empty((n_edges, plan.n), dtype=plan.tdtype, device=rvec.device)
+    _check(lib().allegro_env_radial_backward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(gEenv), _ptr(rvec), _ptr(W_r), W_r.shape[1],
+                                             float(r_cut), float(scale), _ptr(g_rvec), _ptr(g_w), _stream(stream)))
+    return g_rvec, g_w
 
 
 def edge_energy(plan, out, q, kappa, want_e=True, want_G=True, e_edge=None, G=None, stream=None):

@@ -8,6 +8,7 @@
 #pragma once
 #include "common.cuh"
 #include "launch.h"
+#include "radial.cuh"
 
 namespace allegro {
 
@@ -182,6 +183,183 @@ __global__ void __launch_bounds__(256) env_embed_bwd_kernel(int n, const int* __
             g_rvec[3 * (size_t)e + 1] = (g[1] - dot * y) * inv;
             g_rvec[3 * (size_t)e + 2] = (g[2] - dot * z) * inv;
         }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Fused geometry kernels: radial weights (A8) + Y_lm + environment embedding in one pass, and the matching VJP
+// (embedding VJP + radial chain rule) in one pass.  w[E][n] and g_w[E][n] need not exist in HBM (both are optional
+// outputs): per edge the kernels read r_e (12 bytes) only.  Arithmetic is the same as radial_fwd/bwd_kernel +
+// env_embed(_bwd)_kernel: basis and W_r dot products in double, w rounded once to T, Y_lm and the sums in T.
+// Mapping: CTA per item; chunks of kGeoChunk edges: phase 1, thread per edge -> basis, Y_lm, unit vector into
+// shared memory; phase 2, warp per edge, lane <-> channels lane, lane+32, ... with their W_r rows in registers.
+constexpr int kGeoChunk = 128;
+
+template <typename T, int L, int NB>
+struct GeoSmem {
+    static constexpr int DE = (L + 1) * (L + 1);
+    double Bs[kGeoChunk][NB];
+    double dBs[kGeoChunk][NB];
+    double rh[kGeoChunk][3];
+    T Ys[kGeoChunk][DE];
+    T geo[kGeoChunk][4];  // unit vector, 1/|r|
+};
+
+template <typename T, int L, int NB, bool WANT_D>
+__device__ __forceinline__ void geo_phase1(GeoSmem<T, L, NB>& sm, int le, const T* __restrict__ rvec, size_t e, double rc, int nb) {
+    constexpr int DE = (L + 1) * (L + 1);
+    const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+    const double dx = (double)rx, dy = (double)ry, dz = (double)rz;
+    const double rr = sqrt(dx * dx + dy * dy + dz * dz);
+    double Bu[kMaxBasis], dBu[kMaxBasis];
+    radial_basis<WANT_D>(rr, rc, nb, Bu, dBu);
+#pragma unroll
+    for (int b = 0; b < NB; ++b) {
+        sm.Bs[le][b] = b < nb ? Bu[b] : 0.0;
+        if (WANT_D) sm.dBs[le][b] = b < nb ? dBu[b] : 0.0;
+    }
+    if (WANT_D) { sm.rh[le][0] = dx / rr; sm.rh[le][1] = dy / rr; sm.rh[le][2] = dz / rr; }
+    const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+    const T x = rx * inv, y = ry * inv, z = rz * inv;
+    T Y[DE];
+    sph_harm<T, L>(x, y, z, Y);
+#pragma unroll
+    for (int j = 0; j < DE; ++j) sm.Ys[le][j] = Y[j];
+    sm.geo[le][0] = x; sm.geo[le][1] = y; sm.geo[le][2] = z; sm.geo[le][3] = inv;
+}
+
+template <typename T, int L, int CPL, int NB>
+__global__ void __launch_bounds__(256) env_radial_fwd_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr, const int* __restrict__ items,
+                                                              const T* __restrict__ rvec, const T* __restrict__ W_r, T scale,
+                                                              T* __restrict__ w_out, T* __restrict__ dst, int by_item) {
+    constexpr int DE = (L + 1) * (L + 1);
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    GeoSmem<T, L, NB>& sm = *reinterpret_cast<GeoSmem<T, L, NB>*>(geo_raw);
+    T* red = reinterpret_cast<T*>(geo_raw + sizeof(GeoSmem<T, L, NB>));  // [32 * CPL][DE]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    double Wd[CPL][NB];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Wd[q][b] = (lane + 32 * q < n && b < nb) ? (double)W_r[(lane + 32 * q) * nb + b] : 0.0;
+    T acc[CPL][DE];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q)
+#pragma unroll
+        for (int j = 0; j < DE; ++j) acc[q][j] = T(0);
+
+    for (int cb = e0; cb < e1; cb += kGeoChunk) {
+        const int cnt = min(kGeoChunk, e1 - cb);
+        if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+        __syncthreads();
+        for (int le = warp; le < cnt; le += 8) {
+            double Bv[NB];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) Bv[b] = sm.Bs[le][b];
+            T Y[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) Y[j] = sm.Ys[le][j];
+#pragma unroll
+            for (int q = 0; q < CPL; ++q) {
+                double s = 0.0;
+#pragma unroll
+                for (int b = 0; b < NB; ++b) s = fma(Wd[q][b], Bv[b], s);
+                const T wv = (T)s;
+                if (w_out && lane + 32 * q < n) w_out[(size_t)(cb + le) * n + lane + 32 * q] = wv;
+#pragma unroll
+                for (int j = 0; j < DE; ++j) acc[q][j] = fma(wv, Y[j], acc[q][j]);
+            }
+        }
+        __syncthreads();
+    }
+    // warps folded in warp order through one [n][DE] buffer
+    for (int wv = 0; wv < 8; ++wv) {
+        if (warp == wv) {
+#pragma unroll
+            for (int q = 0; q < CPL; ++q) {
+                const int ch = lane + 32 * q;
+                if (ch < n) {
+#pragma unroll
+                    for (int j = 0; j < DE; ++j) red[ch * DE + j] = (wv == 0 ? T(0) : red[ch * DE + j]) + acc[q][j];
+                }
+            }
+        }
+        __syncthreads();
+    }
+    T* o = dst + (size_t)(by_item ? (long)blockIdx.x : (long)c) * n * DE;
+    for (int idx = tid; idx < n * DE; idx += 256) o[idx] = scale * red[idx];
+}
+
+template <typename T, int L, int CPL, int NB>
+__global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
+                                                              const T* __restrict__ rvec, const T* __restrict__ W_r, T scale,
+                                                              T* __restrict__ g_rvec, T* __restrict__ g_w) {
+    constexpr int DE = (L + 1) * (L + 1);
+    static_assert(DE <= 16, "warp_reduce16 handles l_max <= 3");
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    GeoSmem<T, L, NB>& sm = *reinterpret_cast<GeoSmem<T, L, NB>*>(geo_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int c = blockIdx.x;
+    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+    double Wd[CPL][NB];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) Wd[q][b] = (lane + 32 * q < n && b < nb) ? (double)W_r[(lane + 32 * q) * nb + b] : 0.0;
+    T gE[CPL][DE];
+#pragma unroll
+    for (int q = 0; q < CPL; ++q) {
+        const int ch = lane + 32 * q;
+#pragma unroll
+        for (int j = 0; j < DE; ++j) gE[q][j] = ch < n ? scale * gEenv[((size_t)c * n + ch) * DE + j] : T(0);
+    }
+    for (int cb = e0; cb < e1; cb += kGeoChunk) {
+        const int cnt = min(kGeoChunk, e1 - cb);
+        if (tid < cnt) geo_phase1<T, L, NB, true>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+        __syncthreads();
+        for (int le = warp; le < cnt; le += 8) {
+            const size_t e = (size_t)(cb + le);
+            double Bv[NB], dBv[NB];
+#pragma unroll
+            for (int b = 0; b < NB; ++b) { Bv[b] = sm.Bs[le][b]; dBv[b] = sm.dBs[le][b]; }
+            T Y[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) Y[j] = sm.Ys[le][j];
+            T part[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) part[j] = T(0);
+            double rad = 0.0;
+#pragma unroll
+            for (int q = 0; q < CPL; ++q) {
+                double s = 0.0, ds = 0.0;
+#pragma unroll
+                for (int b = 0; b < NB; ++b) { s = fma(Wd[q][b], Bv[b], s); ds = fma(Wd[q][b], dBv[b], ds); }
+                const T wv = (T)s;
+                T gw = T(0);
+#pragma unroll
+                for (int j = 0; j < DE; ++j) { gw = fma(gE[q][j], Y[j], gw); part[j] = fma(gE[q][j], wv, part[j]); }
+                if (g_w && lane + 32 * q < n) g_w[e * n + lane + 32 * q] = gw;
+                rad = fma((double)gw, ds, rad);
+            }
+            warp_reduce16<T>(part, lane);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) rad += __shfl_xor_sync(0xffffffffu, rad, o);
+            T gY[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) gY[j] = __shfl_sync(0xffffffffu, part[0], 2 * j);
+            if (lane == 0) {
+                const T x = sm.geo[le][0], y = sm.geo[le][1], z = sm.geo[le][2], inv = sm.geo[le][3];
+                T g[3];
+                sph_harm_vjp<T, L>(x, y, z, gY, g);
+                const T dot = g[0] * x + g[1] * y + g[2] * z;
+                g_rvec[3 * e] = (T)((double)((g[0] - dot * x) * inv) + rad * sm.rh[le][0]);
+                g_rvec[3 * e + 1] = (T)((double)((g[1] - dot * y) * inv) + rad * sm.rh[le][1]);
+                g_rvec[3 * e + 2] = (T)((double)((g[2] - dot * z) * inv) + rad * sm.rh[le][2]);
+            }
+        }
+        __syncthreads();
     }
 }
 

@@ -26,9 +26,31 @@ allegro_status_t launch_env_embed<ALLEGRO_T, ALLEGRO_L>(const EnvArgs& a) {
         }
     }
     T* dst = have_items ? (T*)a.ws : (T*)a.Eenv;
+    if (a.W_r != nullptr) {
+        if (a.n > 128 || a.nb > kMaxBasis) {
+            set_error("env_radial_forward: n = %d, n_basis = %d unsupported (n <= 128, n_basis <= %d)", a.n, a.nb, kMaxBasis);
+            return ALLEGRO_EUNSUPPORTED;
+        }
+#define ALLEGRO_GEOF(CPL, NB)                                                                                              \
+    {                                                                                                                      \
+        auto k = env_radial_fwd_kernel<T, ALLEGRO_L, CPL, NB>;                                                             \
+        const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>) + (size_t)32 * CPL * DE * sizeof(T);                         \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
+        k<<<(unsigned)a.n_items, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.W_r, \
+                                                    (T)a.scale, (T*)a.w_out, dst, have_items ? 1 : 0);                     \
+    }
+        if (a.nb <= 8) {
+            if (a.n <= 32) ALLEGRO_GEOF(1, 8) else if (a.n <= 64) ALLEGRO_GEOF(2, 8) else ALLEGRO_GEOF(4, 8)
+        } else {
+            if (a.n <= 32) ALLEGRO_GEOF(1, 16) else if (a.n <= 64) ALLEGRO_GEOF(2, 16) else ALLEGRO_GEOF(4, 16)
+        }
+#undef ALLEGRO_GEOF
+        ALLEGRO_LAUNCHED();
+    } else {
     env_embed_kernel<T, ALLEGRO_L, kEnvThreads><<<(unsigned)a.n_items, kEnvThreads, 0, a.st>>>(
         a.n, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.w, (T)a.scale, dst, have_items ? 1 : 0);
     ALLEGRO_LAUNCHED();
+    }
     if (have_items) {
         combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * DE, (const T*)a.ws, (T*)a.Eenv);
         ALLEGRO_LAUNCHED();
@@ -44,6 +66,28 @@ allegro_status_t launch_env_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EnvBwdArg
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
+    if (a.W_r != nullptr) {
+        if (a.n > 128 || a.nb > kMaxBasis) {
+            set_error("env_radial_backward: n = %d, n_basis = %d unsupported (n <= 128, n_basis <= %d)", a.n, a.nb, kMaxBasis);
+            return ALLEGRO_EUNSUPPORTED;
+        }
+#define ALLEGRO_GEOB(CPL, NB)                                                                                              \
+    {                                                                                                                      \
+        auto k = env_radial_bwd_kernel<T, ALLEGRO_L, CPL, NB>;                                                             \
+        const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>);                                                             \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
+        k<<<(unsigned)a.n_atoms, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec,       \
+                                                    (const T*)a.W_r, (T)a.scale, (T*)a.g_rvec, (T*)a.g_w);                 \
+    }
+        if (a.nb <= 8) {
+            if (a.n <= 32) ALLEGRO_GEOB(1, 8) else if (a.n <= 64) ALLEGRO_GEOB(2, 8) else ALLEGRO_GEOB(4, 8)
+        } else {
+            if (a.n <= 32) ALLEGRO_GEOB(1, 16) else if (a.n <= 64) ALLEGRO_GEOB(2, 16) else ALLEGRO_GEOB(4, 16)
+        }
+#undef ALLEGRO_GEOB
+        ALLEGRO_LAUNCHED();
+        return ALLEGRO_OK;
+    }
 #define ALLEGRO_ENVB(CPL)                                                                          \
     env_embed_bwd_kernel<T, ALLEGRO_L, CPL><<<(unsigned)a.n_atoms, 256, 0, a.st>>>(                \
         a.n, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.w, (T)a.scale, (T*)a.g_rvec, (T*)a.g_w)

@@ -23,6 +23,11 @@ struct EnvArgs {
     void* Eenv;
     void* ws;
     cudaStream_t st;
+    // fused radial variant (allegro_env_radial_forward): W_r != nullptr; w is then an optional OUTPUT (w_out)
+    const void* W_r;
+    int nb;
+    double rc;
+    void* w_out;
 };
 struct EnvBwdArgs {
     int n, n_atoms;
@@ -35,6 +40,10 @@ struct EnvBwdArgs {
     void* g_rvec;
     void* g_w;  // nullable
     cudaStream_t st;
+    // fused radial variant (allegro_env_radial_backward): W_r != nullptr; w is not read
+    const void* W_r;
+    int nb;
+    double rc;
 };
 struct TpArgs {
     const allegro_plan* plan;

@@ -52,17 +52,20 @@ class SingleLayerStep:
       "separate" : tp_forward -> edge_energy -> tp_backward                     (out, G both cross HBM twice)
       "epilogue" : tp_forward_energy (out, e_edge, G from one kernel) -> tp_backward
       "onthefly" : tp_forward_energy (out, e_edge) -> tp_backward_energy (cotangent formed from out in registers;
-                   G never exists in HBM)"""
+                   G never exists in HBM)
+    `fused_geometry`: env_radial_forward / env_radial_backward (w and g_w never exist in HBM) instead of
+    radial_forward + env_embed / env_embed_backward + radial_backward."""
 
-    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, mode="onthefly"):
+    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, mode="onthefly", fused_geometry=True):
         assert mode in ("separate", "epilogue", "onthefly")
         self.plan, self.dev, self.rc, self.kappa, self.scale, self.mode = plan, dev, rc, kappa, scale, mode
+        self.fused_geometry = fused_geometry
         rp, rvec, V = dev["row_ptr"], dev["rvec"], dev["V"]
         self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
         self.items = items
         dt, dv = rvec.dtype, rvec.device
         n = plan.n
-        self.w = torch.empty((self.E, n), dtype=dt, device=dv)
+        self.w = None if fused_geometry else torch.empty((self.E, n), dtype=dt, device=dv)
         self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
         self.out = torch.empty_like(V)
         self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
@@ -71,7 +74,7 @@ class SingleLayerStep:
         self.gEenv = torch.empty_like(self.Eenv)
         self.g_path_w = torch.empty((plan.P,), dtype=dt, device=dv) if want_g_path_w else None
         self.g_r = torch.empty_like(rvec)
-        self.g_w = torch.empty_like(self.w)
+        self.g_w = None if fused_geometry else torch.empty_like(self.w)
         self.F = torch.empty((self.N, 3), dtype=dt, device=dv)
         self.e_tot = torch.empty((1,), dtype=dt, device=dv)
         self.e_ptr = torch.tensor([0, self.E], dtype=torch.int32, device=dv)
@@ -95,8 +98,12 @@ class SingleLayerStep:
             return r
 
         bw = dict(items=it, want_gV=self.gV is not None, gV=self.gV, gEenv=self.gEenv, g_path_w=self.g_path_w, workspace=self.ws_bwd)
-        timed("radial_forward", lambda: ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w))
-        timed("env_embed", lambda: ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env))
+        if self.fused_geometry:
+            timed("env_radial_forward", lambda: ab.env_radial_forward(p, rp, rvec, d["W_r"], self.rc, self.scale, items=it, Eenv=self.Eenv,
+                                                                      workspace=self.ws_env))
+        else:
+            timed("radial_forward", lambda: ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w))
+            timed("env_embed", lambda: ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env))
         if self.mode == "separate":
             timed("tp_forward", lambda: ab.tp_forward(p, rp, V, self.Eenv, pw, items=it, out=self.out))
             timed("edge_energy", lambda: ab.edge_energy(p, self.out, d["q"], self.kappa, e_edge=self.e_edge, G=self.G))
@@ -109,8 +116,11 @@ class SingleLayerStep:
             timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it, out=self.out,
                                                                     e_edge=self.e_edge, want_G=False))
             timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp, self.out, V, self.Eenv, pw, d["q"], self.kappa, **bw))
-        timed("env_embed_backward", lambda: ab.env_embed_backward(p, rp, self.gEenv, rvec, self.w, self.scale, g_rvec=self.g_r, g_w=self.g_w))
-        timed("radial_backward", lambda: ab.radial_backward(rvec, d["W_r"], self.rc, self.g_w, self.g_r))
+        if self.fused_geometry:
+            timed("env_radial_backward", lambda: ab.env_radial_backward(p, rp, self.gEenv, rvec, d["W_r"], self.rc, self.scale, g_rvec=self.g_r))
+        else:
+            timed("env_embed_backward", lambda: ab.env_embed_backward(p, rp, self.gEenv, rvec, self.w, self.scale, g_rvec=self.g_r, g_w=self.g_w))
+            timed("radial_backward", lambda: ab.radial_backward(rvec, d["W_r"], self.rc, self.g_w, self.g_r))
         timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
         timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
         if mark:
@@ -132,6 +142,8 @@ class SingleLayerStep:
             "tp_forward_energy": (3 if self.G is not None else 2) * feat + env + E * s + (N + 1) * 4,
             "tp_backward": bwd,
             "tp_backward_energy": bwd,
+            "env_radial_forward": E * 3 * s + env + (N + 1) * 4,
+            "env_radial_backward": env + 2 * E * 3 * s + (N + 1) * 4,
             "env_embed_backward": env + E * 3 * s + wrow + wrow + E * 3 * s + (N + 1) * 4,
             "radial_backward": E * 3 * s + wrow + 2 * E * 3 * s,
             "force_gather": 2 * E * 3 * s + E * 4 + N * 3 * s + (N + 1) * 4,

@@ -66,8 +66,8 @@ def test_forward_energy_epilogue(name, want_out):
 
 
 @pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
-@pytest.mark.parametrize("mode", ["separate", "epilogue", "onthefly"])
-def test_single_layer_step_modes(name, mode):
+@pytest.mark.parametrize("mode,fused_geometry", [("separate", False), ("epilogue", False), ("onthefly", False), ("onthefly", True)])
+def test_single_layer_step_modes(name, mode, fused_geometry):
     """the three call sequences of pipeline.SingleLayerStep (the object bench.py times) give the oracle's forces,
     energies and gradients; "onthefly" exercises tp_backward_energy (cotangent formed from out in registers)"""
     import torch
@@ -80,7 +80,7 @@ def test_single_layer_step_modes(name, mode):
     plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32)
     for items in (None, ab.segments_build(inp["row_ptr"], 9)):
         it = None if items is None else torch.from_numpy(items).cuda()
-        st = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_g_path_w=True, items=it, mode=mode)
+        st = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_g_path_w=True, items=it, mode=mode, fused_geometry=fused_geometry)
         st.run()
         got = dict(w=st.w, Eenv=st.Eenv, out=st.out, e_edge=st.e_edge, G=st.G, gV=st.gV, gEenv=st.gEenv, g_path_w=st.g_path_w,
                    g_w=st.g_w, g_r=st.g_r, F=st.F)
@@ -88,9 +88,32 @@ def test_single_layer_step_modes(name, mode):
         e_ref = float(np.sum(ref["e_edge"]))
         assert abs(float(st.e_tot.item()) - e_ref) <= _chain.TOL[inp["dt"]] * max(abs(e_ref), float(np.abs(ref["e_edge"]).max()))
         # force-only VJP (gV = NULL) gives the same gEenv bits or values within tolerance
-        st2 = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=False, items=it, mode=mode)
+        st2 = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=False, items=it, mode=mode, fused_geometry=fused_geometry)
         st2.run()
         _assert_close(ref, dict(gEenv=st2.gEenv, F=st2.F), inp["dt"], keys=("gEenv", "F"), label="%s/%s/force-only" % (name, mode))
+
+
+@pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
+def test_fused_geometry_kernels(name):
+    """env_radial_forward / env_radial_backward with their optional outputs w, g_w against the oracle's
+    radial + env_embed / env_embed_backward + radial_backward"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    inp = _chain.make_inputs(name)
+    dev = _chain.to_device(inp)
+    ref = _chain.oracle_chain(inp)
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32)
+    for items in (None, ab.segments_build(inp["row_ptr"], 11)):
+        it = None if items is None else torch.from_numpy(items).cuda()
+        Eenv, w = ab.env_radial_forward(plan, dev["row_ptr"], dev["rvec"], dev["W_r"], inp["rc"], inp["scale"], items=it, want_w=True)
+        _assert_close(ref, dict(Eenv=Eenv, w=w), inp["dt"], keys=("Eenv", "w"), label=name)
+    gE = torch.from_numpy(ref["gEenv"].astype(inp["dt"])).cuda()
+    g_r, g_w = ab.env_radial_backward(plan, dev["row_ptr"], gE, dev["rvec"], dev["W_r"], inp["rc"], inp["scale"], want_g_w=True)
+    _assert_close(ref, dict(g_r=g_r, g_w=g_w), inp["dt"], keys=("g_r", "g_w"), label=name)
+    g_r2, none = ab.env_radial_backward(plan, dev["row_ptr"], gE, dev["rvec"], dev["W_r"], inp["rc"], inp["scale"])
+    assert none is None and torch.equal(g_r, g_r2)
 
 
 def test_c4_fp64_variant():
