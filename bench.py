@@ -42,6 +42,7 @@ def parse_args():
     ap.add_argument("--force-only", action="store_true", help="skip dE/dV (valid when V does not depend on positions)")
     ap.add_argument("--mode", default="onthefly", choices=["separate", "epilogue", "onthefly"], help="call sequence (pipeline.SingleLayerStep)")
     ap.add_argument("--separate-geometry", action="store_true", help="radial / env-embed as four kernels instead of the two fused ones")
+    ap.add_argument("--chunks", type=int, default=1, help="process the centres in this many chunks (C3 defaults to 16)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
@@ -178,7 +179,7 @@ def run_ours(args):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     import paper_2504_16068_b200 as ab
-    from paper_2504_16068_b200.pipeline import HostStep, SingleLayerStep, to_device
+    from paper_2504_16068_b200.pipeline import ChunkedStep, HostStep, SingleLayerStep, to_device
     from workloads.inputs import make_inputs
 
     name = args.workload
@@ -187,7 +188,13 @@ def run_ours(args):
     inp = make_inputs(name, seed=rank, features="device")
     dev = to_device(inp)
     plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32, ab.W_SCALAR)
-    step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only, mode=args.mode, fused_geometry=not args.separate_geometry)
+    chunked = name == "C3" or args.chunks > 1
+    if chunked:      # feature tensors that do not fit HBM four times: V resident, work buffers per centre chunk
+        step = ChunkedStep(plan, dev, inp["row_ptr"], inp["rc"], inp["kappa"], inp["scale"], n_chunks=max(args.chunks, 16 if name == "C3" else 1),
+                           want_gV=not args.force_only)
+    else:
+        step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only, mode=args.mode,
+                               fused_geometry=not args.separate_geometry)
     E, N = step.E, step.N
 
     def barrier():
@@ -222,50 +229,56 @@ def run_ours(args):
 
     # per-call device time (CUDA events on the launching stream, same timed region)
     per_call = {}
-    for mk in marks:
+    for mk in marks:          # one list per step; a chunked step has several entries per name: summed per step
+        tot = {}
         for nm, a, b in mk:
-            per_call.setdefault(nm, []).append(a.elapsed_time(b))
+            tot[nm] = tot.get(nm, 0.0) + a.elapsed_time(b)
+        for nm, v in tot.items():
+            per_call.setdefault(nm, []).append(v)
     per_call_ms = {k: sum(v) / len(v) for k, v in per_call.items()}
     abytes = step.algorithmic_bytes()
     peak, peak_src = measured_peaks()
     top = max(per_call_ms, key=per_call_ms.get)
     ach = abytes[top] / (per_call_ms[top] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": _ncu_traffic(top), "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top],
+                "traffic": _ncu_traffic(name, top) if (args.mode == "onthefly" and not args.force_only) else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top],
                 "ms_per_launch": per_call_ms[top]}
     step_bytes = sum(abytes[k] for k in per_call_ms)
     calls = {k: {"ms": round(per_call_ms[k], 4), "GB/s": round(abytes[k] / (per_call_ms[k] * 1e-3) / 1e9, 1),
                  "share": round(per_call_ms[k] / sum(per_call_ms.values()), 4)} for k in per_call_ms}
 
     # ---------------- end to end: host buffers in, forces + energy out, copies inside the timed region
-    host = HostStep(step, inp)
-    for _ in range(3):
-        host.run()
-    barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    k_e2e = max(3, min(args.steps, 10))
-    e0.record()
-    for _ in range(k_e2e):
-        host.run()
-    e1.record()
-    barrier()
-    t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e_ms = float(t.item()) / k_e2e
-    e2e = {"value": world * E / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.h2d_bytes, "d2h_bytes_per_step": host.d2h_bytes,
-           "ms_per_step": e2e_ms, "steps": k_e2e}
+    if chunked:
+        e2e = None      # the host copy of V alone (86 GB at C3) does not fit pinned memory on the box: no end-to-end arm
+    else:
+        host = HostStep(step, inp)
+        for _ in range(3):
+            host.run()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        k_e2e = max(3, min(args.steps, 10))
+        e0.record()
+        for _ in range(k_e2e):
+            host.run()
+        e1.record()
+        barrier()
+        t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        e2e_ms = float(t.item()) / k_e2e
+        e2e = {"value": world * E / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.h2d_bytes, "d2h_bytes_per_step": host.d2h_bytes,
+               "ms_per_step": e2e_ms, "steps": k_e2e}
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
             "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32" if inp["dt"] == np.float32 else "f64", "data": "synthetic",
-            "config": {"workload": "%s: BASELINE.json configs[1] recipe, %d atoms, %d directed edges per GPU, l_max=%d, n=%d, "
+            "config": {"workload": "%s: BASELINE.json configs recipe, %d atoms, %d directed edges per GPU, l_max=%d, n=%d, "
                                    "single TP layer forward + %s" % (name, N, E, inp["lmax"], inp["n"],
                                                                      "force-only VJP" if args.force_only else "full VJP (gV, gEenv) + forces"),
                        "atoms": N, "edges": E, "l_max": inp["lmax"], "n_channels": inp["n"], "parallelism": "independent systems per GPU", "mode": args.mode,
-                       "l2": "not flushed: every feature tensor (%.2f GB) exceeds the 126 MB L2" % (abytes["tp_forward"] / 2 / 1e9),
+                       "l2": "not flushed: every feature tensor (%.2f GB) exceeds the 126 MB L2" % (E * inp["n"] * plan.dV * (4 if inp["dt"] == np.float32 else 8) / 1e9),
                        "fused_geometry": not args.separate_geometry},
             "atom_steps_per_s": world * N / (ms_step * 1e-3),
             "step_GBps_algorithmic": step_bytes / (ms_step * 1e-3) / 1e9, "step_frac_of_hbm_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
@@ -280,12 +293,12 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
-def _ncu_traffic(kernel):
+def _ncu_traffic(workload, kernel):
     """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.json), or None"""
     p = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(p):
         with open(p) as f:
-            return json.load(f).get(kernel)
+            return json.load(f).get(workload, {}).get(kernel)
     return None
 
 

@@ -176,3 +176,84 @@ class HostStep:
         self.e_host.copy_(self.step.e_tot, non_blocking=True)
         torch.cuda.current_stream().synchronize()
         return self.F_host, self.e_host
+
+
+class ChunkedStep:
+    """The same step for a system whose feature tensors do not fit HBM four times (C3: 85.8 GB per tensor): V stays
+    resident, the centres are processed in `n_chunks` contiguous ranges that reuse one set of chunk-sized work buffers
+    (out, gV), and the per-edge results that the force assembly needs (g_r, e_edge) are written into full-size arrays.
+    Chunks are independent because every per-edge / per-centre quantity depends on one centre (strict locality).
+    Call sequence per chunk: env_radial_forward -> tp_forward_energy -> tp_backward_energy -> env_radial_backward;
+    then one force_gather and one segment_sum over the whole system."""
+
+    def __init__(self, plan, dev, row_ptr_host, rc, kappa, scale=1.0, n_chunks=8, want_gV=True):
+        from .sharding import partition_centres
+        self.plan, self.dev, self.rc, self.kappa, self.scale = plan, dev, rc, kappa, scale
+        rp_h = np.asarray(row_ptr_host, dtype=np.int64)
+        self.N, self.E = rp_h.shape[0] - 1, int(rp_h[-1])
+        self.parts = [p for p in partition_centres(rp_h, n_chunks) if p[1] > p[0]]
+        dv, dt = dev["rvec"].device, dev["rvec"].dtype
+        self.chunks = []
+        emax = 0
+        for c0, c1 in self.parts:
+            e0, e1 = int(rp_h[c0]), int(rp_h[c1])
+            rp_c = torch.from_numpy((rp_h[c0:c1 + 1] - e0).astype(np.int32)).to(dv)
+            self.chunks.append((c0, c1, e0, e1, rp_c))
+            emax = max(emax, e1 - e0)
+        n = plan.n
+        self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
+        self.gEenv = torch.empty_like(self.Eenv)
+        self.out = torch.empty((emax, n, plan.dV), dtype=dt, device=dv)
+        self.gV = torch.empty_like(self.out) if want_gV else None
+        self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
+        self.g_r = torch.empty((self.E, 3), dtype=dt, device=dv)
+        self.F = torch.empty((self.N, 3), dtype=dt, device=dv)
+        self.e_tot = torch.empty((1,), dtype=dt, device=dv)
+        self.e_ptr = torch.tensor([0, self.E], dtype=torch.int32, device=dv)
+        self.ws = torch.empty(16, dtype=torch.uint8, device=dv)
+        self.emax = emax
+
+    def run(self, keep=None, mark=False):
+        """keep: optional dict chunk_index -> dict that receives clones of that chunk's out / gV (parity tests);
+        mark: record CUDA events around every call -> self.marks = [(name, start, end)] (one entry per call and chunk)"""
+        p, d = self.plan, self.dev
+        ev = []
+
+        def timed(name, fn):
+            if not mark:
+                return fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            r = fn()
+            b.record()
+            ev.append((name, a, b))
+            return r
+
+        self.marks = ev
+        for k, (c0, c1, e0, e1, rp_c) in enumerate(self.chunks):
+            m = e1 - e0
+            rvec, V = d["rvec"][e0:e1], d["V"][e0:e1]
+            Eenv, gE = self.Eenv[c0:c1], self.gEenv[c0:c1]
+            out = self.out[:m]
+            gV = None if self.gV is None else self.gV[:m]
+            timed("env_radial_forward", lambda: ab.env_radial_forward(p, rp_c, rvec, d["W_r"], self.rc, self.scale, Eenv=Eenv))
+            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp_c, V, Eenv, d["path_w"], d["q"], self.kappa, out=out,
+                                                                    e_edge=self.e_edge[e0:e1], want_G=False))
+            timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp_c, out, V, Eenv, d["path_w"], d["q"], self.kappa,
+                                                                      want_gV=gV is not None, gV=gV, gEenv=gE, workspace=self.ws))
+            timed("env_radial_backward", lambda: ab.env_radial_backward(p, rp_c, gE, rvec, d["W_r"], self.rc, self.scale,
+                                                                        g_rvec=self.g_r[e0:e1]))
+            if keep is not None and k in keep:
+                keep[k].update(out=out.clone(), gV=None if gV is None else gV.clone())
+        timed("force_gather", lambda: ab.force_gather(d["row_ptr"], d["rev"], self.g_r, F=self.F))
+        timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        return self.F, self.e_tot
+
+    def algorithmic_bytes(self):
+        p = self.plan
+        s = 4 if p.dtype == ab.F32 else 8
+        E, N, n, dV, dE = self.E, self.N, p.n, p.dV, p.dE
+        feat, env = E * n * dV * s, N * n * dE * s
+        return {"env_radial_forward": E * 3 * s + env, "tp_forward_energy": 2 * feat + env + E * s,
+                "tp_backward_energy": (3 if self.gV is not None else 2) * feat + 2 * env, "env_radial_backward": env + 2 * E * 3 * s,
+                "force_gather": 2 * E * 3 * s + E * 4 + N * 3 * s, "segment_sum": E * s}

@@ -261,3 +261,47 @@ def test_c1_full_size_sampled_centres():
     e_tot = float(st.e_tot.item())
     e_ref = float(st.e_edge.double().sum().item())
     assert abs(e_tot - e_ref) <= 1e-5 * abs(e_ref)
+
+
+def test_c4_full_size():
+    """BASELINE.json:configs[4] in full (64 molecules, ~3k atoms, ~138k edges, l_max = 2, n = 32, fp32): forward, force VJP,
+    path-weight gradient and per-molecule energies against the oracle, element by element"""
+    inp = _chain.make_inputs("C4")
+    ref = _chain.oracle_chain(inp)
+    got = _chain.gpu_chain(inp)
+    errs = _assert_close(ref, got, inp["dt"], label="C4")
+    assert "E_mol" in errs and "g_path_w" in errs
+    print("C4", {k: "%.2e" % v for k, v in errs.items()})
+
+
+def test_c3_full_size_chunked_sampled_centres():
+    """BASELINE.json:configs[3] at full size (100,000 atoms, ~5.2 M edges, l_max = 3, n = 128: 86 GB per feature tensor)
+    through pipeline.ChunkedStep, the launch configuration bench.py --workload C3 times; the oracle evaluates seeded
+    centre ranges with their complete neighbourhoods (exact: strict locality) inside the first, a middle and the last chunk"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import ChunkedStep, to_device
+    from workloads.inputs import sub_inputs
+    free, _ = torch.cuda.mem_get_info()
+    if free < 140e9:
+        pytest.skip("needs ~135 GB of free HBM")
+    inp = _chain.make_inputs("C3", features="device")
+    dev = to_device(inp)
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F32)
+    st = ChunkedStep(plan, dev, inp["row_ptr"], inp["rc"], inp["kappa"], inp["scale"], n_chunks=16)
+    nck = len(st.chunks)
+    keep = {0: {}, nck // 2: {}, nck - 1: {}}
+    st.run(keep=keep)
+    torch.cuda.synchronize()
+    for k, kept in keep.items():
+        c0, c1, e0, e1, _ = st.chunks[k]
+        for a in (c0, (c0 + c1) // 2, c1 - 3):
+            sub = sub_inputs(inp, a, a + 3)
+            ref = _chain.oracle_chain(sub, want_gw=False, forces=False)
+            s0, s1 = sub["edge_range"]
+            part = dict(out=kept["out"][s0 - e0:s1 - e0], gV=kept["gV"][s0 - e0:s1 - e0], e_edge=st.e_edge[s0:s1], g_r=st.g_r[s0:s1],
+                        Eenv=st.Eenv[a:a + 3], gEenv=st.gEenv[a:a + 3])
+            _assert_close(ref, part, inp["dt"], keys=tuple(part.keys()), label="C3 chunk %d centres [%d,%d)" % (k, a, a + 3))
+    got = dict(g_r=st.g_r, F=st.F)
+    _check_force_gather(inp, got)
