@@ -1,26 +1,265 @@
-// mix_kernels.cuh -- dense per-path channel mixing (ALLEGRO_W_DENSE; BASELINE.json:configs[2]).
+// mix_kernels.cuh -- dense per-path channel mixing (ALLEGRO_W_DENSE; BASELINE.json:configs[2], reading A5):
+//   t[e][n][p][M]   = sum_{m1 m2} C^p[m1][m2][M] V[e][n][off1(p)+m1] Eenv[c(e)][n][off2(p)+m2]      (un-weighted paths)
+//   out[e][n'][off3(p)+M] = sum_p sum_n W[p][n'][n] t[e][n][p][M]
+// and its VJP  gt[e][n][p][M] = sum_n' W[p][n'][n] G[e][n'][off3(p)+M], then the per-path CG VJP with unit weights.
+//
+// First version (round 1): the 64x64 mixes run on the FP32/FP64 FMA pipe with 128-bit shared-memory operands
+// (t never leaves the SM: PAPER.md:71); the tcgen05 / 3xTF32 tensor-core version is the next step.
+// One CTA per item; thread <-> (edge slot, channel).  Per tile of `nsl` edges:
+//   forward : t (DT values per thread) -> shared tS[slot][col][n]; per path p: W_p -> shared Ws[n'][n] (row stride n+4),
+//             acc[off3(p)+M] += <Ws[n'][:], tS[slot][toff(p)+M][:]>; thread (slot, n') stores its out row.
+//   backward: G rows -> shared gS[slot][k][n']; per path p: W_p^T -> shared; gt[toff(p)+M] += <WsT[n][:], gS[slot][off3(p)+M][:]>;
+//             then the generated per-path VJP (gV row stored, gEenv accumulated in registers over the segment).
 #pragma once
+#include <type_traits>
+#include <utility>
+
 #include "common.cuh"
 #include "launch.h"
 
 namespace allegro {
 
+template <int I, int N, typename F>
+__device__ __forceinline__ void static_for(F&& f) {
+    if constexpr (I < N) {
+        f(std::integral_constant<int, I>{});
+        static_for<I + 1, N>(f);
+    }
+}
+
+// dot product of two 16-byte-aligned shared-memory rows of length n (n * sizeof(T) % 16 == 0), 128-bit loads
+template <typename T>
+__device__ __forceinline__ T dot_rows(const T* __restrict__ a, const T* __restrict__ b, int n, T acc) {
+    constexpr int VEC = 16 / (int)sizeof(T);
+    const int4* a4 = reinterpret_cast<const int4*>(a);
+    const int4* b4 = reinterpret_cast<const int4*>(b);
+    for (int i = 0; i < n / VEC; ++i) {
+        const int4 av = a4[i], bv = b4[i];
+        const T* as = reinterpret_cast<const T*>(&av);
+        const T* bs = reinterpret_cast<const T*>(&bv);
+#pragma unroll
+        for (int k = 0; k < VEC; ++k) acc = fma(as[k], bs[k], acc);
+    }
+    return acc;
+}
+
+template <typename T, int L, int CT>
+__global__ void __launch_bounds__(CT) mix_fwd_kernel(int nsl, int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
+                                                      const T* __restrict__ V, const T* __restrict__ Eenv, const T* __restrict__ W,
+                                                      T* __restrict__ out) {
+    using Gen = TPGen<L>;
+    constexpr int DV = Gen::DV, DE = Gen::DE, DT = Gen::DT, P = Gen::P;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    T* tS = reinterpret_cast<T*>(smem_raw);           // [nsl][DT][n]
+    T* Ws = tS + (size_t)nsl * DT * n;                // [n][n + VEC]
+    const int ldw = n + VEC;
+    const int tid = threadIdx.x;
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = slot < nsl;
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    const int ntiles = (e1 - e0 + nsl - 1) / nsl;
+    T E[DE];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) E[j] = active ? Eenv[((size_t)c * n + ch) * DE + j] : T(0);
+
+    for (int t = 0; t < ntiles; ++t) {
+        const int eb = e0 + t * nsl;
+        const bool valid = active && eb + slot < e1;
+        if (valid) {
+            T v[DV], tt[DT];
+            row_load<T, DV>(V + ((size_t)(eb + slot) * n + ch) * DV, v);
+            Gen::template fwd_paths<T>(v, E, tt);
+#pragma unroll
+            for (int col = 0; col < DT; ++col) tS[((size_t)slot * DT + col) * n + ch] = tt[col];
+        }
+        T acc[DV];
+#pragma unroll
+        for (int k = 0; k < DV; ++k) acc[k] = T(0);
+        static_for<0, P>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int toff = Gen::toff(p), off3 = Gen::off3(p), d3 = Gen::d3(p);
+            __syncthreads();  // tS complete (p == 0) / previous W_p consumed
+            for (int idx = tid; idx < n * n / VEC; idx += CT) {
+                const int r = (idx * VEC) / n, cc = (idx * VEC) - r * n;
+                *reinterpret_cast<int4*>(Ws + (size_t)r * ldw + cc) = *reinterpret_cast<const int4*>(W + (size_t)p * n * n + (size_t)idx * VEC);
+            }
+            __syncthreads();
+            if (valid) {
+#pragma unroll
+                for (int M = 0; M < d3; ++M)
+                    acc[off3 + M] = dot_rows<T>(Ws + (size_t)ch * ldw, tS + ((size_t)slot * DT + toff + M) * n, n, acc[off3 + M]);
+            }
+        });
+        if (valid) row_store<T, DV>(out + ((size_t)(eb + slot) * n + ch) * DV, acc);
+        __syncthreads();  // tS is rewritten by the next tile
+    }
+}
+
+template <typename T, int L, int CT, bool WANT_GV>
+__global__ void __launch_bounds__(CT) mix_bwd_kernel(int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
+                                                      const T* __restrict__ G, const T* __restrict__ V, const T* __restrict__ Eenv,
+                                                      const T* __restrict__ W, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item) {
+    using Gen = TPGen<L>;
+    constexpr int DV = Gen::DV, DE = Gen::DE, DT = Gen::DT, P = Gen::P;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    const int nsl = CT / n;
+    T* gS = reinterpret_cast<T*>(smem_raw);           // [nsl][DV][n]
+    T* WsT = gS + (size_t)nsl * DV * n;               // [n][n + VEC], WsT[a][b] = W_p[b][a]
+    const int ldw = n + VEC;
+    const int tid = threadIdx.x;
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = slot < nsl;
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    const int ntiles = (e1 - e0 + nsl - 1) / nsl;
+    T E[DE], gE[DE];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) { E[j] = active ? Eenv[((size_t)c * n + ch) * DE + j] : T(0); gE[j] = T(0); }
+
+    for (int t = 0; t < ntiles; ++t) {
+        const int eb = e0 + t * nsl;
+        const bool valid = active && eb + slot < e1;
+        if (valid) {
+            T g[DV];
+            row_load<T, DV>(G + ((size_t)(eb + slot) * n + ch) * DV, g);
+#pragma unroll
+            for (int k = 0; k < DV; ++k) gS[((size_t)slot * DV + k) * n + ch] = g[k];
+        }
+        T gt[DT];
+#pragma unroll
+        for (int col = 0; col < DT; ++col) gt[col] = T(0);
+        static_for<0, P>([&](auto pc) {
+            constexpr int p = decltype(pc)::value;
+            constexpr int toff = Gen::toff(p), off3 = Gen::off3(p), d3 = Gen::d3(p);
+            __syncthreads();
+            for (int idx = tid; idx < n * n / VEC; idx += CT) {
+                const int r = (idx * VEC) / n, cc = (idx * VEC) - r * n;  // W_p[r][cc .. cc+VEC)
+                const int4 wv = *reinterpret_cast<const int4*>(W + (size_t)p * n * n + (size_t)idx * VEC);
+                const T* ws = reinterpret_cast<const T*>(&wv);
+#pragma unroll
+                for (int k = 0; k < VEC; ++k) WsT[(size_t)(cc + k) * ldw + r] = ws[k];
+            }
+            __syncthreads();
+            if (valid) {
+#pragma unroll
+                for (int M = 0; M < d3; ++M)
+                    gt[toff + M] = dot_rows<T>(WsT + (size_t)ch * ldw, gS + ((size_t)slot * DV + off3 + M) * n, n, gt[toff + M]);
+            }
+        });
+        if (valid) {
+            T v[DV], gv[DV];
+            row_load<T, DV>(V + ((size_t)(eb + slot) * n + ch) * DV, v);
+            Gen::template bwd_paths<T, WANT_GV>(v, E, gt, gv, gE);
+            if constexpr (WANT_GV) row_store<T, DV>(gV + ((size_t)(eb + slot) * n + ch) * DV, gv);
+        }
+        __syncthreads();  // gS is rewritten by the next tile
+    }
+    // ---- gEenv: slots summed in slot order
+    T* red = reinterpret_cast<T*>(smem_raw);
+    __syncthreads();
+    if (active) {
+#pragma unroll
+        for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = gE[j];
+    }
+    __syncthreads();
+    if (slot == 0) {
+        T* dst = gE_dst + ((size_t)(gE_by_item ? (long)blockIdx.x : (long)c) * n + ch) * DE;
+#pragma unroll
+        for (int j = 0; j < DE; ++j) {
+            T acc = red[(size_t)ch * DE + j];
+            for (int sl = 1; sl < nsl; ++sl) acc += red[((size_t)sl * n + ch) * DE + j];
+            dst[j] = acc;
+        }
+    }
+}
+
+// The dense mode is instantiated for l_max <= 2 (what configs[2] needs): at l_max = 3 a thread would hold 312
+// un-weighted path values, which does not fit the register file.
+#if ALLEGRO_L <= 2
 template <typename T>
 static allegro_status_t launch_mix_forward(const TpArgs& a) {
-    (void)a;
-    set_error("tp_forward: dense weight mode not built yet");
-    return ALLEGRO_EUNSUPPORTED;
+    using Gen = TPGen<ALLEGRO_L>;
+    constexpr int CT = sizeof(T) == 4 ? 256 : 128;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    if (a.n % VEC != 0 || a.n > CT) {
+        set_error("tp_forward (dense): n = %d unsupported (n %% %d == 0, n <= %d)", a.n, VEC, CT);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    const size_t ws_bytes = (size_t)a.n * (a.n + VEC) * sizeof(T);
+    const size_t per_slot = (size_t)Gen::DT * a.n * sizeof(T);
+    int nsl = CT / a.n;
+    while (nsl > 1 && nsl * per_slot + ws_bytes > 200 * 1024) --nsl;
+    const size_t smem = nsl * per_slot + ws_bytes;
+    if (smem > 226 * 1024) {
+        set_error("tp_forward (dense): n = %d needs %zu bytes of shared memory", a.n, smem);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    auto k = mix_fwd_kernel<T, ALLEGRO_L, CT>;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k<<<(unsigned)a.n_items, CT, smem, a.st>>>(nsl, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (const T*)a.path_w, (T*)a.out);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
 }
+
+#else
 template <typename T>
-static allegro_status_t launch_mix_backward(const TpArgs& a) {
-    (void)a;
-    set_error("tp_backward: dense weight mode not built yet");
+static allegro_status_t launch_mix_forward(const TpArgs&) {
+    set_error("tp_forward (dense): dense path weights are built for l_max <= 2");
     return ALLEGRO_EUNSUPPORTED;
 }
+#endif
+
 template <typename T>
 static size_t mix_backward_workspace(int n, long n_items, bool have_items, bool want_gw) {
-    (void)n; (void)n_items; (void)have_items; (void)want_gw;
-    return 0;
+    (void)want_gw;
+    return have_items ? align_up((size_t)n_items * n * TPGen<ALLEGRO_L>::DE * sizeof(T), 256) : 0;
 }
+
+#if ALLEGRO_L <= 2
+template <typename T>
+static allegro_status_t launch_mix_backward(const TpArgs& a) {
+    using Gen = TPGen<ALLEGRO_L>;
+    constexpr int CT = sizeof(T) == 4 ? 256 : 128;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    if (a.n % VEC != 0 || a.n > CT) {
+        set_error("tp_backward (dense): n = %d unsupported (n %% %d == 0, n <= %d)", a.n, VEC, CT);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (a.g_path_w != nullptr) {
+        set_error("tp_backward (dense): the gradient with respect to the dense path weights is not built (forces need only gV, gEenv)");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    const bool have_items = a.items != nullptr;
+    T* gE_dst = have_items ? (T*)a.ws : (T*)a.gEenv;
+    const int nsl = CT / a.n;
+    size_t smem = (size_t)nsl * Gen::DV * a.n * sizeof(T) + (size_t)a.n * (a.n + VEC) * sizeof(T);
+    const size_t red = (size_t)CT * Gen::DE * sizeof(T);
+    if (smem < red) smem = red;
+#define ALLEGRO_MIXB(GV)                                                                                                   \
+    {                                                                                                                      \
+        auto k = mix_bwd_kernel<T, ALLEGRO_L, CT, GV>;                                                                     \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
+        k<<<(unsigned)a.n_items, CT, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
+                                                   (const T*)a.path_w, (T*)a.gV, gE_dst, have_items ? 1 : 0);              \
+    }
+    if (a.gV != nullptr) ALLEGRO_MIXB(true) else ALLEGRO_MIXB(false)
+#undef ALLEGRO_MIXB
+    ALLEGRO_LAUNCHED();
+    if (have_items) {
+        combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, (const T*)a.ws, (T*)a.gEenv);
+        ALLEGRO_LAUNCHED();
+    }
+    return ALLEGRO_OK;
+}
+#else
+template <typename T>
+static allegro_status_t launch_mix_backward(const TpArgs&) {
+    set_error("tp_backward (dense): dense path weights are built for l_max <= 2");
+    return ALLEGRO_EUNSUPPORTED;
+}
+#endif
 
 }  // namespace allegro

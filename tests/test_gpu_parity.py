@@ -305,3 +305,39 @@ def test_c3_full_size_chunked_sampled_centres():
             _assert_close(ref, part, inp["dt"], keys=tuple(part.keys()), label="C3 chunk %d centres [%d,%d)" % (k, a, a + 3))
     got = dict(g_r=st.g_r, F=st.F)
     _check_force_gather(inp, got)
+
+
+@pytest.mark.parametrize("lmax,n,dt,geom", [(2, 64, np.float32, "C1s"), (1, 8, np.float64, "C0"), (1, 128, np.float32, "C0"), (2, 32, np.float64, "C4s")])
+def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
+    """ALLEGRO_W_DENSE (BASELINE.json:configs[2], reading A5): per-path n x n channel mix, forward and VJP (gV, gEenv),
+    against the oracle's dense mode on seeded inputs; also with centres split into items"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, rng
+    g = configs.geometry_for(geom)
+    rp, E, N = g["row_ptr"], g["rvec"].shape[0], g["row_ptr"].shape[0] - 1
+    dV, dE, P = 2 * (lmax + 1) ** 2, (lmax + 1) ** 2, configs.num_paths(lmax)
+    S = rng.STREAMS
+    V = rng.normal(7, S["V"], (E, n, dV)).astype(dt)
+    Ee = (rng.normal(7, S["W_w"], (N, n, dE)) * 0.5).astype(dt)
+    W = (rng.normal(7, S["W_p"], (P, n, n)) / np.sqrt(n)).astype(dt)
+    G = rng.normal(7, S["G"], (E, n, dV)).astype(dt)
+    f8 = lambda a: a.astype(np.float64)
+    ref_out = orc.tp_forward(lmax, rp, f8(V), f8(Ee), f8(W))
+    ref_gV, ref_gE, _ = orc.tp_backward(lmax, rp, f8(G), f8(V), f8(Ee), f8(W), want_gV=True, want_gw=False)
+    plan = ab.Plan(lmax, n, ab.F64 if dt == np.float64 else ab.F32, ab.W_DENSE)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    rpd, Vd, Ed, Wd, Gd = d(rp), d(V), d(Ee), d(W), d(G)
+    for items in (None, ab.segments_build(rp, 6)):
+        it = None if items is None else d(items)
+        out = ab.tp_forward(plan, rpd, Vd, Ed, Wd, items=it)
+        gV, gE, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it)
+        _assert_close(dict(out=ref_out, gV=ref_gV, gEenv=ref_gE), dict(out=out, gV=gV, gEenv=gE), dt, keys=("out", "gV", "gEenv"),
+                      label="dense l%d n%d" % (lmax, n))
+        _, gE2, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it, want_gV=False)
+        _assert_close(dict(gEenv=ref_gE), dict(gEenv=gE2), dt, keys=("gEenv",), label="dense force-only")
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, want_g_path_w=True)
+    assert ei.value.status == 2
