@@ -14,7 +14,7 @@ import subprocess
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_SRCS = ["allegro_oracle.cpp", "model2.cpp"]
+_SRCS = ["allegro_oracle.cpp"]
 _LIB = os.path.join(_HERE, "liballegro_oracle.so")
 _lib = None
 
@@ -50,8 +50,6 @@ def _declare(L):
     L.orc_cg_complex.argtypes = [C.c_int] * 6
     L.orc_nnz.restype = C.c_int64
     L.orc_segments.restype = C.c_int64
-    if hasattr(L, "orc_model2_energy_grad"):
-        L.orc_model2_energy_grad.restype = C.c_double
 
 
 def _d(a):
@@ -238,30 +236,3 @@ def segment_sum(ptr, vals):
     out = np.zeros(nseg)
     lib().orc_segment_sum(_i(ptr), nseg, _d(vals), _d(out))
     return out
-
-
-class _Model2(C.Structure):
-    _fields_ = [("lmax", C.c_int), ("n", C.c_int), ("nb", C.c_int), ("n_layers", C.c_int),
-                ("rc", C.c_double), ("scale", C.c_double),
-                ("W_x0", _f64p), ("W_v0", _f64p), ("W_w", _f64p), ("W_p", _f64p), ("A_lat", _f64p),
-                ("q", _f64p)]
-
-
-def model2_energy_grad(params, row_ptr, rvec, centres=None, taps=False):
-    """Two-layer model of config C2 (reading A19).  params: dict with lmax, n, nb, n_layers, rc,
-    scale, W_x0, W_v0, W_w, W_p, A_lat, q.  -> (energy, g_rvec[E,3], Eenv_taps, V_taps)"""
-    row_ptr, rvec = _i32(row_ptr), _f64(rvec)
-    N = row_ptr.shape[0] - 1
-    E = rvec.shape[0]
-    keep = {k: _f64(params[k]) for k in ("W_x0", "W_v0", "W_w", "W_p", "A_lat", "q")}
-    m = _Model2(int(params["lmax"]), int(params["n"]), int(params["nb"]), int(params["n_layers"]),
-                float(params["rc"]), float(params["scale"]),
-                _d(keep["W_x0"]), _d(keep["W_v0"]), _d(keep["W_w"]), _d(keep["W_p"]), _d(keep["A_lat"]),
-                _d(keep["q"]))
-    c_lo, c_hi = _crange(row_ptr, centres)
-    g_r = np.zeros_like(rvec)
-    L, n, lmax = m.n_layers, m.n, m.lmax
-    Et = np.zeros((L, N, n, dim_e(lmax))) if taps else None
-    Vt = np.zeros((L, E, n, dim_v(lmax))) if taps else None
-    en = lib().orc_model2_energy_grad(C.byref(m), N, _i(row_ptr), c_lo, c_hi, _d(rvec), _d(g_r), _d(Et), _d(Vt))
-    return en, g_r, Et, Vt

@@ -96,23 +96,6 @@ void    orc_edge_energy(int lmax, int n, int64_t E, const double* out, const dou
 /* out[s] = sum_{i = ptr[s]}^{ptr[s+1]-1} vals[i], sequential */
 void    orc_segment_sum(const int32_t* ptr, int nseg, const double* vals, double* out);
 
-/* ---- two-layer model of config C2 (reading A19) --------------------------------------- */
-typedef struct {
-    int lmax, n, nb, n_layers;
-    double rc, scale;
-    const double* W_x0;    /* [n][nb] */
-    const double* W_v0;    /* [n][nb] */
-    const double* W_w;     /* [L][n][n] */
-    const double* W_p;     /* [L][P][n][n] */
-    const double* A_lat;   /* [L-1][n][2n] */
-    const double* q;       /* [n] */
-} orc_model2_t;
-/* Energy of the centres c_lo..c_hi (sum of their edges' readouts) and its gradient
- * g_rvec[e] for their edges (other rows untouched).  Optional taps (nullable), layer-major:
- * Eenv_out[L][N][n][dE], V_out[L][E][n][dV]. */
-double  orc_model2_energy_grad(const orc_model2_t* m, int N, const int32_t* row_ptr, int c_lo,
-                               int c_hi, const double* rvec, double* g_rvec, double* Eenv_out,
-                               double* V_out);
 
 #ifdef __cplusplus
 }

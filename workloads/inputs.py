@@ -61,3 +61,32 @@ def sub_inputs(inp, c_lo, c_hi):
                centre_range=(c_lo, c_hi))
     sub.pop("edge_mol_ptr", None)
     return sub
+
+
+def make_model_inputs(name, seed=0, n=None, lmax=None, n_layers=None):
+    """Inputs of the two-layer model of configs[2] (reading A19): geometry of config `name` plus the dense weights.
+    n / lmax / n_layers override the config's (small oracle-only pins).  Weights are float64 here; each side rounds
+    them to its dtype.  scale = 1/sqrt(E/N) (reading A6)."""
+    g = configs.geometry_for(name, seed)
+    s = dict(g["spec"])
+    n = n or s["n"]
+    lmax = lmax or s["lmax"]
+    L = n_layers or s.get("n_layers", 2)
+    P = configs.num_paths(lmax)
+    S = rng.STREAMS
+    nb = configs.N_BASIS
+    E, N = g["rvec"].shape[0], g["row_ptr"].shape[0] - 1
+    dt = configs.np_dtype(name)
+    params = dict(
+        lmax=lmax, n=n, nb=nb, n_layers=L, rc=s["rc"], scale=1.0 / np.sqrt(E / N),
+        W_x0=rng.normal(seed, S["W_x0"], (n, nb)) / np.sqrt(nb),
+        W_v0=rng.normal(seed, S["W_v0"], (n, nb)) / np.sqrt(nb),
+        W_w=rng.normal(seed, S["W_w"], (L, n, n)) / np.sqrt(n),
+        W_p=rng.normal(seed, S["W_p"], (L, P, n, n)) / np.sqrt(n),
+        A_lat=rng.normal(seed, S["A_lat"], (max(L - 1, 1), n, 2 * n)) / np.sqrt(2 * n),
+        q=rng.normal(seed, S["q"], (n,)) / np.sqrt(n),
+    )
+    for k in ("W_x0", "W_v0", "W_w", "W_p", "A_lat", "q"):      # rounded once to the config's dtype (reading A9)
+        params[k] = np.ascontiguousarray(params[k].astype(dt)).astype(np.float64) if dt == np.float32 else params[k]
+    return dict(name=name, dt=dt, N=N, E=E, row_ptr=g["row_ptr"], rev=g["rev"], rvec=np.ascontiguousarray(g["rvec"].astype(dt)),
+                params=params)
