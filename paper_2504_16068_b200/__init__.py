@@ -54,6 +54,12 @@ SIGNATURES = {
     "allegro_env_radial_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, C.c_double, C.c_double, _vp, _vp, _vp]),
     "allegro_edge_energy": (C.c_int, [_vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_segment_sum": (C.c_int, [_vp, C.c_int, _vp, C.c_int, _vp, _vp]),
+    "allegro_edge_embed": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp]),
+    "allegro_edge_embed_backward": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp, _vp]),
+    "allegro_linear": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_int, C.c_int, _vp, _vp]),
+    "allegro_latent_forward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_latent_backward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_add_inplace": (C.c_int, [C.c_long, C.c_int, _vp, _vp, _vp]),
     "allegro_status_str": (C.c_char_p, [C.c_int]),
     "allegro_last_error": (C.c_char_p, []),
     "allegro_launch_count": (C.c_long, []),
@@ -329,3 +335,57 @@ def segment_sum(ptr, vals, out=None, stream=None):
         out = torch.empty((nseg,), dtype=vals.dtype, device=vals.device)
     _check(lib().allegro_segment_sum(_ptr(ptr), nseg, _ptr(vals), _dt(vals), _ptr(out), _stream(stream)))
     return out
+
+
+# ---------------------------------------------------------------------------------------------------- two-layer model helpers
+def edge_embed(plan, rvec, W_x0, W_v0, r_cut, x0=None, V0=None, stream=None):
+    E = rvec.shape[0]
+    if x0 is None:
+        x0 = torch.empty((E, plan.n), dtype=plan.tdtype, device=rvec.device)
+    if V0 is None:
+        V0 = torch.empty((E, plan.n, plan.dV), dtype=plan.tdtype, device=rvec.device)
+    _check(lib().allegro_edge_embed(plan.h, E, _ptr(rvec), _ptr(W_x0), _ptr(W_v0), W_x0.shape[1], float(r_cut), _ptr(x0), _ptr(V0), _stream(stream)))
+    return x0, V0
+
+
+def edge_embed_backward(plan, rvec, W_x0, W_v0, r_cut, g_x0, gV0, g_rvec, stream=None):
+    """g_rvec += ..., in place"""
+    _check(lib().allegro_edge_embed_backward(plan.h, rvec.shape[0], _ptr(rvec), _ptr(W_x0), _ptr(W_v0), W_x0.shape[1], float(r_cut), _ptr(g_x0),
+                                             _ptr(gV0), _ptr(g_rvec), _stream(stream)))
+    return g_rvec
+
+
+def linear(x, W, transpose_w=False, y=None, accumulate=False, stream=None):
+    """y (+)= x W^T (transpose_w False, W [n_out, n_in]) or x W (transpose_w True, W [n_in, n_out])"""
+    n_in = x.shape[1]
+    n_out = W.shape[1] if transpose_w else W.shape[0]
+    if y is None:
+        assert not accumulate
+        y = torch.empty((x.shape[0], n_out), dtype=x.dtype, device=x.device)
+    _check(lib().allegro_linear(x.shape[0], n_out, n_in, _dt(x), _ptr(x), _ptr(W), int(transpose_w), int(accumulate), _ptr(y), _stream(stream)))
+    return y
+
+
+def latent_forward(rvec, r_cut, x, V, A, z=None, x_new=None, stream=None):
+    """-> (z, x_new)"""
+    if z is None:
+        z = torch.empty_like(x)
+    if x_new is None:
+        x_new = torch.empty_like(x)
+    _check(lib().allegro_latent_forward(x.shape[0], x.shape[1], V.shape[2], float(r_cut), _dt(x), _ptr(rvec), _ptr(x), _ptr(V), _ptr(A), _ptr(z),
+                                        _ptr(x_new), _stream(stream)))
+    return z, x_new
+
+
+def latent_backward(rvec, r_cut, z, g_xnew, A, gV, g_rvec, g_x=None, stream=None):
+    """-> g_x (overwritten); gV[:, :, 0] and g_rvec are accumulated into"""
+    if g_x is None:
+        g_x = torch.empty_like(z)
+    _check(lib().allegro_latent_backward(z.shape[0], z.shape[1], gV.shape[2], float(r_cut), _dt(z), _ptr(rvec), _ptr(z), _ptr(g_xnew), _ptr(A),
+                                         _ptr(g_x), _ptr(gV), _ptr(g_rvec), _stream(stream)))
+    return g_x
+
+
+def add_inplace(y, x, stream=None):
+    _check(lib().allegro_add_inplace(y.numel(), _dt(y), _ptr(y), _ptr(x), _stream(stream)))
+    return y

@@ -2,7 +2,7 @@
 
 Steps: (1) g++ builds the code generator csrc/gen_tp.cpp + csrc/plan.cpp and runs it, which writes
 csrc/generated/tp_gen.cuh (the sparse CG table unrolled into straight-line CUDA, one set per l_max);
-(2) nvcc compiles api.cu, misc.cu, plan.cpp and inst_tp.cu / inst_env.cu once per (dtype, l_max), in
+(2) nvcc compiles api.cu, misc.cu, model.cu, plan.cpp and inst_tp.cu / inst_env.cu once per (dtype, l_max), in
 parallel; (3) nvcc links the shared library next to this file.  Nothing is cached outside the tree.
 
     python -m paper_2504_16068_b200.build [--force] [--jobs N]
@@ -62,7 +62,7 @@ def generate(force=False):
 
 
 def _jobs():
-    jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("plan.o", "plan.cpp", [])]
+    jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("model.o", "model.cu", []), ("plan.o", "plan.cpp", [])]
     for tag, ctype in DTYPES:
         for L in LMAXS:
             d = ["-DALLEGRO_T=%s" % ctype, "-DALLEGRO_L=%d" % L]

@@ -22,6 +22,8 @@ void set_error(const char* fmt, ...) {
 // explicit specialisations live in inst_tp.cu / inst_env.cu (one object per dtype and l_max)
 #define ALLEGRO_DECL(T, L)                                                                     \
     template <> allegro_status_t launch_env_embed<T, L>(const EnvArgs&);                       \
+    template <> allegro_status_t launch_edge_embed<T, L>(const EmbedArgs&);                    \
+    template <> allegro_status_t launch_edge_embed_backward<T, L>(const EmbedArgs&);           \
     template <> allegro_status_t launch_env_embed_backward<T, L>(const EnvBwdArgs&);           \
     template <> allegro_status_t launch_tp_forward<T, L>(const TpArgs&);                       \
     template <> allegro_status_t launch_tp_backward<T, L>(const TpArgs&);                      \
@@ -302,6 +304,56 @@ allegro_status_t allegro_segment_sum(const int32_t* ptr, int n_segments, const v
     ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
     return dtype == ALLEGRO_F32 ? launch_segment_sum<float>(ptr, n_segments, vals, out, (cudaStream_t)stream)
                                 : launch_segment_sum<double>(ptr, n_segments, vals, out, (cudaStream_t)stream);
+}
+
+// ---------------------------------------------------------------------------------------------- two-layer model helpers
+allegro_status_t allegro_edge_embed(const allegro_plan_t* plan, long n_edges, const void* rvec, const void* W_x0, const void* W_v0, int n_basis,
+                                    double r_cut, void* x0, void* V0, void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_edges >= 0, "plan is NULL or n_edges < 0");
+    ALLEGRO_CHECK_ARG((rvec && x0 && V0) || n_edges == 0, "NULL tensor");
+    ALLEGRO_CHECK_ARG(W_x0 && W_v0 && n_basis >= 1 && r_cut > 0, "bad weights / n_basis / r_cut");
+    ALLEGRO_CHECK_ARG(aligned16(V0), "V0 not 16-byte aligned");
+    EmbedArgs a{plan->n, n_basis, r_cut, n_edges, rvec, W_x0, W_v0, x0, V0, nullptr, nullptr, nullptr, (cudaStream_t)stream};
+    return ALLEGRO_DISPATCH(plan, launch_edge_embed, a);
+}
+allegro_status_t allegro_edge_embed_backward(const allegro_plan_t* plan, long n_edges, const void* rvec, const void* W_x0, const void* W_v0,
+                                             int n_basis, double r_cut, const void* g_x0, const void* gV0, void* g_rvec, void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_edges >= 0, "plan is NULL or n_edges < 0");
+    ALLEGRO_CHECK_ARG((rvec && g_x0 && gV0 && g_rvec) || n_edges == 0, "NULL tensor");
+    ALLEGRO_CHECK_ARG(W_x0 && W_v0 && n_basis >= 1 && r_cut > 0, "bad weights / n_basis / r_cut");
+    ALLEGRO_CHECK_ARG(aligned16(gV0), "gV0 not 16-byte aligned");
+    EmbedArgs a{plan->n, n_basis, r_cut, n_edges, rvec, W_x0, W_v0, nullptr, nullptr, g_x0, gV0, g_rvec, (cudaStream_t)stream};
+    return ALLEGRO_DISPATCH(plan, launch_edge_embed_backward, a);
+}
+allegro_status_t allegro_linear(long n_rows, int n_out, int n_in, allegro_dtype_t dtype, const void* x, const void* W, int transpose_w,
+                                int accumulate, void* y, void* stream) {
+    ALLEGRO_CHECK_ARG(n_rows >= 0 && n_out >= 1 && n_in >= 1, "bad size");
+    ALLEGRO_CHECK_ARG((x && y) || n_rows == 0, "x / y is NULL");
+    ALLEGRO_CHECK_ARG(W != nullptr && x != y, "W is NULL or y aliases x");
+    return dtype == ALLEGRO_F32 ? launch_linear<float>(n_rows, n_out, n_in, x, W, transpose_w, accumulate, y, (cudaStream_t)stream)
+                                : launch_linear<double>(n_rows, n_out, n_in, x, W, transpose_w, accumulate, y, (cudaStream_t)stream);
+}
+allegro_status_t allegro_latent_forward(long n_edges, int n_channels, int dim_v, double r_cut, allegro_dtype_t dtype, const void* rvec,
+                                        const void* x, const void* V, const void* A, void* z, void* x_new, void* stream) {
+    ALLEGRO_CHECK_ARG(n_edges >= 0 && n_channels >= 1 && dim_v >= 1 && r_cut > 0, "bad size");
+    ALLEGRO_CHECK_ARG((rvec && x && V && z && x_new) || n_edges == 0, "NULL tensor");
+    ALLEGRO_CHECK_ARG(A != nullptr, "A is NULL");
+    return dtype == ALLEGRO_F32 ? launch_latent_forward<float>(n_edges, n_channels, dim_v, r_cut, rvec, x, V, A, z, x_new, (cudaStream_t)stream)
+                                : launch_latent_forward<double>(n_edges, n_channels, dim_v, r_cut, rvec, x, V, A, z, x_new, (cudaStream_t)stream);
+}
+allegro_status_t allegro_latent_backward(long n_edges, int n_channels, int dim_v, double r_cut, allegro_dtype_t dtype, const void* rvec,
+                                         const void* z, const void* g_xnew, const void* A, void* g_x, void* gV, void* g_rvec, void* stream) {
+    ALLEGRO_CHECK_ARG(n_edges >= 0 && n_channels >= 1 && dim_v >= 1 && r_cut > 0, "bad size");
+    ALLEGRO_CHECK_ARG((rvec && z && g_xnew && g_x && gV && g_rvec) || n_edges == 0, "NULL tensor");
+    ALLEGRO_CHECK_ARG(A != nullptr, "A is NULL");
+    return dtype == ALLEGRO_F32
+               ? launch_latent_backward<float>(n_edges, n_channels, dim_v, r_cut, rvec, z, g_xnew, A, g_x, gV, g_rvec, (cudaStream_t)stream)
+               : launch_latent_backward<double>(n_edges, n_channels, dim_v, r_cut, rvec, z, g_xnew, A, g_x, gV, g_rvec, (cudaStream_t)stream);
+}
+allegro_status_t allegro_add_inplace(long count, allegro_dtype_t dtype, void* y, const void* x, void* stream) {
+    ALLEGRO_CHECK_ARG(count >= 0 && ((x && y) || count == 0), "bad argument");
+    return dtype == ALLEGRO_F32 ? launch_add_inplace<float>(count, y, x, (cudaStream_t)stream)
+                                : launch_add_inplace<double>(count, y, x, (cudaStream_t)stream);
 }
 
 const char* allegro_status_str(allegro_status_t s) {

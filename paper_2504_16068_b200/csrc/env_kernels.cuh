@@ -363,4 +363,109 @@ __global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, doub
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Layer-0 edge embedding of the two-layer model (reading A19; BASELINE.json:configs[2]):
+//   b_e = [B_b(r_e) u(r_e/r_c)],  x0[e][ch] = sum_b W_x0[ch][b] b_e[b],
+//   V0[e][ch][(l, (-1)^l), m] = (sum_b W_v0[ch][b] b_e[b]) Y_lm(rhat_e), other-parity slots 0.
+// CTA per kGeoChunk edges: phase 1 thread per edge (basis in double, Y_lm), phase 2 warp per edge, lanes over channels.
+template <int L>
+__device__ __forceinline__ constexpr int natural_slot(int j) {  // Eenv-style index l^2+l+m -> feature index of (l, (-1)^l, m)
+    int l = 0;
+    while ((l + 1) * (l + 1) <= j) ++l;
+    return 2 * l * l + ((l & 1) ? 2 * l + 1 : 0) + (j - l * l);
+}
+
+template <typename T, int L, int NB>
+__global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_x0,
+                                                          const T* __restrict__ W_v0, T* __restrict__ x0, T* __restrict__ V0) {
+    constexpr int DE = (L + 1) * (L + 1), DV = 2 * DE;
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    GeoSmem<T, L, NB>& sm = *reinterpret_cast<GeoSmem<T, L, NB>*>(geo_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long cb = (long)blockIdx.x * kGeoChunk;
+    const int cnt = (int)min((long)kGeoChunk, E - cb);
+    if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+    __syncthreads();
+    for (int le = warp; le < cnt; le += 8) {
+        const size_t e = (size_t)(cb + le);
+        for (int ch = lane; ch < n; ch += 32) {
+            double sx = 0.0, sv = 0.0;
+            for (int b = 0; b < nb; ++b) {
+                const double bu = sm.Bs[le][b];
+                sx = fma((double)W_x0[ch * nb + b], bu, sx);
+                sv = fma((double)W_v0[ch * nb + b], bu, sv);
+            }
+            x0[e * n + ch] = (T)sx;
+            const T v0 = (T)sv;
+            T row[DV];
+#pragma unroll
+            for (int k = 0; k < DV; ++k) row[k] = T(0);
+#pragma unroll
+            for (int j = 0; j < DE; ++j) row[natural_slot<L>(j)] = v0 * sm.Ys[le][j];
+            row_store<T, DV>(V0 + (e * n + ch) * DV, row);
+        }
+    }
+}
+
+// VJP of the edge embedding: g_rvec[e] += d/dr_e of ( <g_x0[e], x0[e]> + <gV0[e], V0[e]> )
+template <typename T, int L, int NB>
+__global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec,
+                                                              const T* __restrict__ W_x0, const T* __restrict__ W_v0, const T* __restrict__ g_x0,
+                                                              const T* __restrict__ gV0, T* __restrict__ g_rvec) {
+    constexpr int DE = (L + 1) * (L + 1), DV = 2 * DE;
+    static_assert(DE <= 16 && NB <= 16, "warp_reduce16");
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    GeoSmem<T, L, NB>& sm = *reinterpret_cast<GeoSmem<T, L, NB>*>(geo_raw);
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const long cb = (long)blockIdx.x * kGeoChunk;
+    const int cnt = (int)min((long)kGeoChunk, E - cb);
+    if (tid < cnt) geo_phase1<T, L, NB, true>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+    __syncthreads();
+    for (int le = warp; le < cnt; le += 8) {
+        const size_t e = (size_t)(cb + le);
+        T gYp[16];
+        double gbp[16];
+#pragma unroll
+        for (int j = 0; j < 16; ++j) { gYp[j] = T(0); gbp[j] = 0.0; }
+        for (int ch = lane; ch < n; ch += 32) {
+            T row[DV];
+            row_load<T, DV>(gV0 + (e * n + ch) * DV, row);
+            double sv = 0.0;
+            for (int b = 0; b < nb; ++b) sv = fma((double)W_v0[ch * nb + b], sm.Bs[le][b], sv);
+            const T v0 = (T)sv;
+            T gv0 = T(0);
+#pragma unroll
+            for (int j = 0; j < DE; ++j) {
+                const T gj = row[natural_slot<L>(j)];
+                gv0 = fma(gj, sm.Ys[le][j], gv0);
+                gYp[j] = fma(gj, v0, gYp[j]);
+            }
+            const double gx = (double)g_x0[e * n + ch];
+#pragma unroll
+            for (int b = 0; b < NB; ++b)
+                if (b < nb) gbp[b] += gx * (double)W_x0[ch * nb + b] + (double)gv0 * (double)W_v0[ch * nb + b];
+        }
+        warp_reduce16<T>(gYp, lane);
+        warp_reduce16<double>(gbp, lane);
+        T gY[DE];
+#pragma unroll
+        for (int j = 0; j < DE; ++j) gY[j] = __shfl_sync(0xffffffffu, gYp[0], 2 * j);
+        double rad = 0.0;
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const double gb = __shfl_sync(0xffffffffu, gbp[0], 2 * b);
+            rad = fma(gb, sm.dBs[le][b], rad);
+        }
+        if (lane == 0) {
+            const T x = sm.geo[le][0], y = sm.geo[le][1], z = sm.geo[le][2], inv = sm.geo[le][3];
+            T g[3];
+            sph_harm_vjp<T, L>(x, y, z, gY, g);
+            const T dot = g[0] * x + g[1] * y + g[2] * z;
+            g_rvec[3 * e] = (T)((double)g_rvec[3 * e] + (double)((g[0] - dot * x) * inv) + rad * sm.rh[le][0]);
+            g_rvec[3 * e + 1] = (T)((double)g_rvec[3 * e + 1] + (double)((g[1] - dot * y) * inv) + rad * sm.rh[le][1]);
+            g_rvec[3 * e + 2] = (T)((double)g_rvec[3 * e + 2] + (double)((g[2] - dot * z) * inv) + rad * sm.rh[le][2]);
+        }
+    }
+}
+
 }  // namespace allegro

@@ -100,4 +100,49 @@ allegro_status_t launch_env_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EnvBwdArg
     return ALLEGRO_OK;
 }
 
+template <>
+allegro_status_t launch_edge_embed<ALLEGRO_T, ALLEGRO_L>(const EmbedArgs& a) {
+    using T = ALLEGRO_T;
+    if (a.nb > kMaxBasis || ((size_t)(ALLEGRO_L + 1) * (ALLEGRO_L + 1) * 2 * sizeof(T)) % 8 != 0) {
+        set_error("edge_embed: n_basis = %d unsupported (<= %d)", a.nb, kMaxBasis);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (a.n_edges == 0) return ALLEGRO_OK;
+    const unsigned grid = (unsigned)((a.n_edges + kGeoChunk - 1) / kGeoChunk);
+#define ALLEGRO_EMB(NB)                                                                                                     \
+    {                                                                                                                       \
+        auto k = edge_embed_kernel<T, ALLEGRO_L, NB>;                                                                       \
+        const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>);                                                              \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
+        k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0, (T*)a.x0, (T*)a.V0); \
+    }
+    if (a.nb <= 8) ALLEGRO_EMB(8) else ALLEGRO_EMB(16)
+#undef ALLEGRO_EMB
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
+template <>
+allegro_status_t launch_edge_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EmbedArgs& a) {
+    using T = ALLEGRO_T;
+    if (a.nb > kMaxBasis) {
+        set_error("edge_embed_backward: n_basis = %d unsupported (<= %d)", a.nb, kMaxBasis);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (a.n_edges == 0) return ALLEGRO_OK;
+    const unsigned grid = (unsigned)((a.n_edges + kGeoChunk - 1) / kGeoChunk);
+#define ALLEGRO_EMBB(NB)                                                                                                    \
+    {                                                                                                                       \
+        auto k = edge_embed_bwd_kernel<T, ALLEGRO_L, NB>;                                                                   \
+        const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>);                                                              \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
+        k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0,     \
+                                     (const T*)a.g_x0, (const T*)a.gV0, (T*)a.g_rvec);                                     \
+    }
+    if (a.nb <= 8) ALLEGRO_EMBB(8) else ALLEGRO_EMBB(16)
+#undef ALLEGRO_EMBB
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
 }  // namespace allegro

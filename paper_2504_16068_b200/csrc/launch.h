@@ -71,6 +71,22 @@ struct TpArgs {
     cudaStream_t st;
 };
 
+struct EmbedArgs {
+    int n, nb;
+    double rc;
+    long n_edges;
+    const void* rvec;
+    const void* W_x0;
+    const void* W_v0;
+    void* x0;          // forward outputs
+    void* V0;
+    const void* g_x0;  // backward inputs
+    const void* gV0;
+    void* g_rvec;      // backward: accumulated into
+    cudaStream_t st;
+};
+template <typename T, int L> allegro_status_t launch_edge_embed(const EmbedArgs& a);
+template <typename T, int L> allegro_status_t launch_edge_embed_backward(const EmbedArgs& a);
 template <typename T, int L> allegro_status_t launch_env_embed(const EnvArgs& a);
 template <typename T, int L> allegro_status_t launch_env_embed_backward(const EnvBwdArgs& a);
 template <typename T, int L> allegro_status_t launch_tp_forward(const TpArgs& a);
@@ -89,6 +105,18 @@ template <typename T>
 allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, const void* q, double kappa, void* e_edge, void* G, cudaStream_t st);
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st);
+
+// dtype-only pieces of the two-layer model (model.cu)
+template <typename T>
+allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st);
+template <typename T>
+allegro_status_t launch_latent_forward(long E, int n, int dV, double rc, const void* rvec, const void* x, const void* V, const void* A, void* z,
+                                       void* x_new, cudaStream_t st);
+template <typename T>
+allegro_status_t launch_latent_backward(long E, int n, int dV, double rc, const void* rvec, const void* z, const void* g_xnew, const void* A,
+                                        void* g_x, void* gV, void* g_rvec, cudaStream_t st);
+template <typename T>
+allegro_status_t launch_add_inplace(long count, void* y, const void* x, cudaStream_t st);
 
 static inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 

@@ -257,3 +257,82 @@ class ChunkedStep:
         return {"env_radial_forward": E * 3 * s + env, "tp_forward_energy": 2 * feat + env + E * s,
                 "tp_backward_energy": (3 if self.gV is not None else 2) * feat + 2 * env, "env_radial_backward": env + 2 * E * 3 * s,
                 "force_gather": 2 * E * 3 * s + E * 4 + N * 3 * s, "segment_sum": E * s}
+
+
+class TwoLayerStep:
+    """One MD step of the stacked Allegro-style model of BASELINE.json:configs[2] (reading A19) as a sequence of library
+    calls: edge embedding -> per layer [w = W_w x, env_embed, tensor product with dense per-path mix, latent update]
+    -> readout of the l = 0 outputs -> the matching VJPs in reverse -> force gather.  `params` holds device tensors
+    W_x0 [n,nb], W_v0 [n,nb], W_w [L,n,n], W_p [L,P,n,n], A_lat [L-1,n,2n], q [n] and floats rc, scale."""
+
+    def __init__(self, plan_dense, plan_scalar, dev, params):
+        self.pd, self.ps, self.dev, self.p = plan_dense, plan_scalar, dev, params
+        self.L = params["W_w"].shape[0]
+        rp, rvec = dev["row_ptr"], dev["rvec"]
+        self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
+        dt, dv, n, dV = rvec.dtype, rvec.device, plan_dense.n, plan_dense.dV
+        E, N, L = self.E, self.N, self.L
+        new = lambda *shape: torch.empty(shape, dtype=dt, device=dv)
+        self.x = [new(E, n) for _ in range(L)]            # x_0 .. x_{L-1}
+        self.z = [new(E, n) for _ in range(L - 1)]
+        self.V = [new(E, n, dV) for _ in range(L + 1)]    # V_0 .. V_L
+        self.w = [new(E, n) for _ in range(L)]
+        self.Eenv = [new(N, n, plan_dense.dE) for _ in range(L)]
+        self.gEenv = new(N, n, plan_dense.dE)
+        self.cot = [new(E, n, dV), new(E, n, dV)]          # ping-pong cotangents of V_l
+        self.g_w, self.g_x, self.g_x2 = new(E, n), new(E, n), new(E, n)
+        self.g_r, self.g_r_tmp = new(E, 3), new(E, 3)
+        self.e_edge, self.e_tot, self.F = new(E), new(1), new(N, 3)
+        self.e_ptr = torch.tensor([0, E], dtype=torch.int32, device=dv)
+        self.ws = torch.empty(16, dtype=torch.uint8, device=dv)
+        self.marks = None
+
+    def run(self, mark=False):
+        p, d, pd, ps, L = self.p, self.dev, self.pd, self.ps, self.L
+        rp, rvec, rc, scale = d["row_ptr"], d["rvec"], p["rc"], p["scale"]
+        ev = []
+
+        def timed(name, fn):
+            if not mark:
+                return fn()
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            r = fn()
+            b.record()
+            ev.append((name, a, b))
+            return r
+
+        timed("edge_embed", lambda: ab.edge_embed(pd, rvec, p["W_x0"], p["W_v0"], rc, x0=self.x[0], V0=self.V[0]))
+        for l in range(L):
+            timed("linear", lambda: ab.linear(self.x[l], p["W_w"][l], y=self.w[l]))
+            timed("env_embed", lambda: ab.env_embed(ps, rp, rvec, self.w[l], scale, Eenv=self.Eenv[l]))
+            timed("tp_forward_dense", lambda: ab.tp_forward(pd, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
+            if l < L - 1:
+                timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], self.V[l + 1], p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
+        G = self.cot[0]
+        timed("edge_energy", lambda: ab.edge_energy(pd, self.V[L], p["q"], 0.0, e_edge=self.e_edge, G=G))
+        g_x_next, have_gr = None, False
+        for l in reversed(range(L)):
+            g_x = None
+            if l < L - 1:     # x_{l+1} = u SiLU(A [x_l ; V_{l+1}[:,0e]]): cotangent g_x_next; adds to G[:, :, 0] and g_r
+                g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
+                timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], G, self.g_r, g_x=g_x))
+            gVl = self.cot[1] if G is self.cot[0] else self.cot[0]
+            timed("tp_backward_dense", lambda: ab.tp_backward(pd, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
+            if not have_gr:
+                timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r, g_w=self.g_w))
+                have_gr = True
+            else:
+                timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r_tmp, g_w=self.g_w))
+                timed("add_inplace", lambda: ab.add_inplace(self.g_r, self.g_r_tmp))
+            if g_x is None:
+                g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
+                timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x))
+            else:
+                timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x, accumulate=True))
+            G, g_x_next = gVl, g_x
+        timed("edge_embed_backward", lambda: ab.edge_embed_backward(pd, rvec, p["W_x0"], p["W_v0"], rc, g_x_next, G, self.g_r))
+        timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
+        timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        self.marks = ev
+        return self.F, self.e_tot

@@ -341,3 +341,75 @@ def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
     with pytest.raises(ab.AllegroError) as ei:
         ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, want_g_path_w=True)
     assert ei.value.status == 2
+
+
+def _model_device(inp):
+    import torch
+    td = torch.float32 if inp["dt"] == np.float32 else torch.float64
+    p = inp["params"]
+    dev = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).cuda() for k in ("row_ptr", "rev", "rvec")}
+    prm = {k: torch.from_numpy(np.ascontiguousarray(p[k])).to(td).cuda() for k in ("W_x0", "W_v0", "W_w", "W_p", "A_lat", "q")}
+    prm.update(rc=p["rc"], scale=p["scale"])
+    return dev, prm
+
+
+def _two_layer_step(inp):
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import TwoLayerStep
+    p = inp["params"]
+    dt = ab.F32 if inp["dt"] == np.float32 else ab.F64
+    dev, prm = _model_device(inp)
+    st = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm)
+    st.run()
+    return st
+
+
+def test_two_layer_model_c2s():
+    """BASELINE.json:configs[2]'s recipe at 192 atoms (two stacked layers, dense 64x64 per-path mix, latent update, readout of
+    the l = 0 outputs; forward + force backward) against oracle/model2.py: per-layer Eenv and features, per-edge energies,
+    total energy, dE/dr_e and forces"""
+    from oracle import model2
+    import oracle as orc
+    from workloads.inputs import make_model_inputs
+    inp = make_model_inputs("C2s")
+    p = inp["params"]
+    taps = []
+    en, g = model2.energy_grad(p, inp["row_ptr"], inp["rvec"].astype(np.float64), taps)
+    st = _two_layer_step(inp)
+    ref, got = dict(g_r=g, e_edge=taps[-1]["e_edge"], F=orc.force_gather(inp["row_ptr"], inp["rev"], g)), dict(g_r=st.g_r, e_edge=st.e_edge, F=st.F)
+    for l in range(p["n_layers"]):
+        ref.update({"Eenv%d" % l: taps[l]["Eenv"], "V%d" % (l + 1): taps[l]["V_out"], "w%d" % l: taps[l]["w"]})
+        got.update({"Eenv%d" % l: st.Eenv[l], "V%d" % (l + 1): st.V[l + 1], "w%d" % l: st.w[l]})
+    ref["V0"], got["V0"] = taps[0]["V_in"], st.V[0]
+    errs = _assert_close(ref, got, inp["dt"], keys=tuple(ref.keys()), label="C2s")
+    print("C2s", {k: "%.2e" % v for k, v in errs.items()})
+    assert abs(float(st.e_tot.item()) - en) <= 1e-5 * max(abs(en), float(np.abs(taps[-1]["e_edge"]).max()))
+    F = st.F.cpu().numpy().astype(np.float64)
+    assert np.abs(F.sum(0)).max() <= 1e-3 * np.abs(F).max()
+
+
+def test_two_layer_model_c2_full_size_sampled_centres():
+    """configs[2] at full size (32,768 atoms, ~2.95 M edges) in the launch configuration bench.py --workload C2 times;
+    the oracle evaluates seeded centre ranges with their complete neighbourhoods (exact: the model is strictly local)"""
+    import torch
+    from oracle import model2
+    from workloads import rng
+    from workloads.inputs import make_model_inputs
+    free, _ = torch.cuda.mem_get_info()
+    if free < 110e9:
+        pytest.skip("needs ~100 GB of free HBM")
+    inp = make_model_inputs("C2")
+    st = _two_layer_step(inp)
+    torch.cuda.synchronize()
+    rp, N = inp["row_ptr"], inp["N"]
+    starts = [int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(2), 0, N - 5)] + [0, N - 4]
+    for c0 in starts:
+        c1 = c0 + 4
+        e0, e1 = int(rp[c0]), int(rp[c1])
+        sub_rp = (rp[c0:c1 + 1] - rp[c0]).astype(np.int32)
+        taps = []
+        en, g = model2.energy_grad(inp["params"], sub_rp, inp["rvec"][e0:e1].astype(np.float64), taps)
+        ref = dict(g_r=g, e_edge=taps[-1]["e_edge"], V2=taps[1]["V_out"], Eenv1=taps[1]["Eenv"])
+        got = dict(g_r=st.g_r[e0:e1], e_edge=st.e_edge[e0:e1], V2=st.V[2][e0:e1], Eenv1=st.Eenv[1][c0:c1])
+        _assert_close(ref, got, inp["dt"], keys=tuple(ref.keys()), label="C2 centres [%d,%d)" % (c0, c1))
+    _check_force_gather(inp, dict(g_r=st.g_r, F=st.F))
