@@ -183,6 +183,8 @@ def run_ours(args):
     from workloads.inputs import make_inputs
 
     name = args.workload
+    if name in ("C2", "C2s"):
+        return run_two_layer(args, rank, world, local, dist, barrier_factory=None)
     # multi-GPU: the path partitions over independent systems -- rank r owns the system of seed r;
     # no data-path collective, weak scaling
     inp = make_inputs(name, seed=rank, features="device")
@@ -288,6 +290,110 @@ def run_ours(args):
             import oracle
             oracle.build()
             line["cpu_baseline"] = cpu_baseline(inp, args.cpu_seconds)
+        print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
+    """--workload C2: BASELINE.json:configs[2], two stacked layers with the dense per-path mix, forward + force backward as one MD
+    step.  The dominant calls (dense tensor product forward / VJP) run on the FP32 FMA pipe in this round, so the roofline
+    object is an "alu" one: peak = 148 SMs x 128 FP32 lanes x 2 flop x max SM clock (guide unit counts and clocks)."""
+    import numpy as np
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import TwoLayerStep
+    from workloads.inputs import make_model_inputs
+    name = args.workload
+    inp = make_model_inputs(name, seed=rank)
+    p = inp["params"]
+    td = torch.float32 if inp["dt"] == np.float32 else torch.float64
+    dev = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).cuda() for k in ("row_ptr", "rev", "rvec")}
+    prm = {k: torch.from_numpy(np.ascontiguousarray(p[k])).to(td).cuda() for k in ("W_x0", "W_v0", "W_w", "W_p", "A_lat", "q")}
+    prm.update(rc=p["rc"], scale=p["scale"])
+    dt = ab.F32 if inp["dt"] == np.float32 else ab.F64
+    step = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm)
+    E, N = step.E, step.N
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step.run()
+    barrier()
+    clocks = ClockSampler(local)
+    clocks.start()
+    n0 = ab.launch_count()
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    marks = []
+    ev0.record()
+    for _ in range(args.steps):
+        step.run(mark=True)
+        marks.append(step.marks)
+    ev1.record()
+    barrier()
+    launches = ab.launch_count() - n0
+    clk = clocks.stop()
+    t = torch.tensor([ev0.elapsed_time(ev1)], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item()) / args.steps
+    per_call = {}
+    for mk in marks:
+        tot = {}
+        for nm, a, b in mk:
+            tot[nm] = tot.get(nm, 0.0) + a.elapsed_time(b)
+        for nm, v in tot.items():
+            per_call.setdefault(nm, []).append(v)
+    per_call_ms = {k: sum(v) / len(v) for k, v in per_call.items()}
+    flops = step.algorithmic_flops()
+    top = max(per_call_ms, key=per_call_ms.get)
+    sm_max = clk.get("sm_max_mhz") or 1965.0
+    peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+    ach = flops.get(top, 0) / (per_call_ms[top] * 1e-3) / 1e12
+    # end to end: rvec (the positions) in from pinned host memory, forces and energy out, every step
+    h_rvec = torch.empty(dev["rvec"].shape, dtype=dev["rvec"].dtype, pin_memory=True).copy_(dev["rvec"])
+    h_F = torch.empty(step.F.shape, dtype=step.F.dtype, pin_memory=True)
+    h_e = torch.empty(step.e_tot.shape, dtype=step.e_tot.dtype, pin_memory=True)
+
+    def host_step():
+        dev["rvec"].copy_(h_rvec, non_blocking=True)
+        step.run()
+        h_F.copy_(step.F, non_blocking=True)
+        h_e.copy_(step.e_tot, non_blocking=True)
+        torch.cuda.current_stream().synchronize()
+
+    host_step()
+    barrier()
+    k_e2e = max(2, min(args.steps, 5))
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(k_e2e):
+        host_step()
+    e1.record()
+    barrier()
+    e2e_ms = e0.elapsed_time(e1) / k_e2e
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": world * E / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if inp["dt"] == np.float32 else "f64",
+            "data": "synthetic",
+            "config": {"workload": "%s: BASELINE.json configs[2] recipe, %d atoms, %d directed edges per GPU, l_max=%d, n=%d, %d layers with dense "
+                                   "per-path mix, forward + force backward as one MD step" % (name, N, E, p["lmax"], p["n"], p["n_layers"]),
+                       "atoms": N, "edges": E, "l2": "not flushed: feature tensors (%.2f GB each) exceed the 126 MB L2" % (E * p["n"] * step.pd.dV * 4 / 1e9)},
+            "atom_steps_per_s": world * N / (ms_step * 1e-3),
+            "roofline": {"bound": "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                         "peak_source": "148 SMs x 128 FP32 lanes x 2 x %.0f MHz (B200_PROFILING.md unit counts, nvidia-smi max SM clock)" % sm_max},
+            "calls": {k: {"ms": round(v, 4), "share": round(v / sum(per_call_ms.values()), 4)} for k, v in per_call_ms.items()},
+            "clocks": clk,
+            "e2e": {"value": world * E / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h_rvec.numel() * h_rvec.element_size()),
+                    "d2h_bytes_per_step": int(h_F.numel() * h_F.element_size() + h_e.numel() * h_e.element_size()), "ms_per_step": e2e_ms, "steps": k_e2e},
+            "gpu_launches": int(launches),
+        }
         print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -336,3 +336,13 @@ class TwoLayerStep:
         timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
         self.marks = ev
         return self.F, self.e_tot
+
+    def algorithmic_flops(self):
+        """FP32 flops the dense tensor-product calls must execute (sparse CG 806 flop per channel-edge forward,
+        twice that for the VJP; per-path n x n mix 2 n^2 sum_p (2 l3 + 1) per edge), per call name, summed over layers"""
+        pd = self.pd
+        n, L = pd.n, self.L
+        cg_fwd = {1: 2 * 32 + 32, 2: 2 * 274 + 258, 3: 2 * 1222 + 1082}[pd.l_max] * n
+        dT = {1: 22, 2: 102, 3: 312}[pd.l_max]
+        mix = 2 * n * n * dT
+        return {"tp_forward_dense": L * self.E * (cg_fwd + mix), "tp_backward_dense": L * self.E * (2 * cg_fwd + mix)}
