@@ -141,6 +141,49 @@ static void emit(FILE* f, int L) {
     fprintf(f, "};\n");
 }
 
+// Per-path device functions for the dense per-path channel mix (l_max <= 2): un-weighted t_p = C^p (V (x) E) of ONE path and
+// its VJP, with the feature row read through a pointer (shared memory) so that only the path's V block is touched.
+static void emit_paths(FILE* f, int L) {
+    PlanTables t;
+    build_tables(L, t);
+    const int P = (int)t.paths.size();
+    int toff = 0;
+    size_t z = 0;
+    for (int p = 0; p < P; ++p) {
+        const int d3 = 2 * t.paths[p].l3 + 1, off3 = t.paths[p].off3;
+        fprintf(f, "template <> struct TPPath<%d, %d> {\n    static constexpr int D3 = %d, TOFF = %d, OFF3 = %d;\n", L, p, d3, toff, off3);
+        std::vector<Pair> pairs;
+        std::map<std::pair<int, int>, int> idx;
+        for (; z < t.nnz.size() && t.nnz[z].path == p; ++z) {
+            const NonZero& q = t.nnz[z];
+            auto key = std::make_pair(q.i, q.j);
+            if (!idx.count(key)) { idx[key] = (int)pairs.size(); pairs.push_back(Pair{q.i, q.j, {}}); }
+            pairs[idx[key]].terms.push_back(Term{q.k - off3, (int)z, q.c});
+        }
+        fprintf(f, "    template <typename T> static __device__ __forceinline__ void fwd(const T* __restrict__ V, const T (&E)[%d], T (&t)[%d]) {\n", t.dE, d3);
+        std::vector<char> touched(d3, 0);
+        for (const Pair& pr : pairs) {
+            fprintf(f, "        { const T p = V[%d] * E[%d];", pr.i, pr.j);
+            for (const Term& tm : pr.terms) {
+                if (!touched[tm.k]) { fprintf(f, " t[%d] = T(%.17g) * p;", tm.k, tm.c); touched[tm.k] = 1; }
+                else fprintf(f, " t[%d] = fma(T(%.17g), p, t[%d]);", tm.k, tm.c, tm.k);
+            }
+            fprintf(f, " }\n");
+        }
+        for (int k = 0; k < d3; ++k) if (!touched[k]) fprintf(f, "        t[%d] = T(0);\n", k);
+        fprintf(f, "    }\n");
+        fprintf(f, "    template <typename T, bool WANT_GV> static __device__ __forceinline__ void bwd(const T* __restrict__ V, const T (&E)[%d], const T (&gt)[%d], T (&gV)[%d], T (&gE)[%d]) {\n",
+                t.dE, d3, t.dV, t.dE);
+        for (const Pair& pr : pairs) {
+            fprintf(f, "        { T s = T(%.17g) * gt[%d];", pr.terms[0].c, pr.terms[0].k);
+            for (size_t q = 1; q < pr.terms.size(); ++q) fprintf(f, " s = fma(T(%.17g), gt[%d], s);", pr.terms[q].c, pr.terms[q].k);
+            fprintf(f, " gE[%d] = fma(s, V[%d], gE[%d]); if (WANT_GV) gV[%d] = fma(s, E[%d], gV[%d]); }\n", pr.j, pr.i, pr.j, pr.i, pr.j, pr.i);
+        }
+        fprintf(f, "    }\n};\n");
+        toff += d3;
+    }
+}
+
 int main(int argc, char** argv) {
     if (argc < 2) { fprintf(stderr, "usage: gen_tp <out_dir>\n"); return 2; }
     std::string path = std::string(argv[1]) + "/tp_gen.cuh";
@@ -150,6 +193,8 @@ int main(int argc, char** argv) {
     fprintf(f, "// The including file defines ALLEGRO_CW(z): folded coefficient z (constant memory).\n#pragma once\n");
     fprintf(f, "template <int L> struct TPGen;\n");
     for (int L = 1; L <= 3; ++L) emit(f, L);
+    fprintf(f, "\n// per-path functions (dense mix), l_max <= 2\ntemplate <int L, int PTH> struct TPPath;\n");
+    for (int L = 1; L <= 2; ++L) emit_paths(f, L);
     fclose(f);
     return 0;
 }

@@ -106,6 +106,11 @@ allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, cons
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st);
 
+// dense per-path mix, version 2 (inst_mix2.cu, three parts)
+allegro_status_t launch_mix2_forward_f32_l2_n64(const TpArgs& a);
+allegro_status_t launch_mix2_backward_gv_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
+allegro_status_t launch_mix2_backward_nogv_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
+
 // dtype-only pieces of the two-layer model (model.cu)
 template <typename T>
 allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st);

@@ -10,7 +10,9 @@
 //             acc[off3(p)+M] += <Ws[n'][:], tS[slot][toff(p)+M][:]>; thread (slot, n') stores its out row.
 //   backward: G rows -> shared gS[slot][k][n']; per path p: W_p^T -> shared; gt[toff(p)+M] += <WsT[n][:], gS[slot][off3(p)+M][:]>;
 //             then the generated per-path VJP (gV row stored, gEenv accumulated in registers over the segment).
+// fp32, l_max = 2, n = 64 (configs[2]) is served by the faster version in mix2_kernels.cuh (compiled in inst_mix2.cu).
 #pragma once
+#include <cstdlib>
 #include <type_traits>
 #include <utility>
 
@@ -188,6 +190,11 @@ static allegro_status_t launch_mix_forward(const TpArgs& a) {
         set_error("tp_forward (dense): n = %d unsupported (n %% %d == 0, n <= %d)", a.n, VEC, CT);
         return ALLEGRO_EUNSUPPORTED;
     }
+#if ALLEGRO_L == 2
+    if constexpr (sizeof(T) == 4) {
+        if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr) return launch_mix2_forward_f32_l2_n64(a);
+    }
+#endif
     const size_t ws_bytes = (size_t)a.n * (a.n + VEC) * sizeof(T);
     const size_t per_slot = (size_t)Gen::DT * a.n * sizeof(T);
     int nsl = CT / a.n;
@@ -234,6 +241,20 @@ static allegro_status_t launch_mix_backward(const TpArgs& a) {
     }
     const bool have_items = a.items != nullptr;
     T* gE_dst = have_items ? (T*)a.ws : (T*)a.gEenv;
+#if ALLEGRO_L == 2
+    if constexpr (sizeof(T) == 4) {
+        if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr) {
+            allegro_status_t s2 = a.gV ? launch_mix2_backward_gv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0)
+                                       : launch_mix2_backward_nogv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0);
+            if (s2 != ALLEGRO_OK) return s2;
+            if (have_items) {
+                combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, (const T*)a.ws, (T*)a.gEenv);
+                ALLEGRO_LAUNCHED();
+            }
+            return ALLEGRO_OK;
+        }
+    }
+#endif
     const int nsl = CT / a.n;
     size_t smem = (size_t)nsl * Gen::DV * a.n * sizeof(T) + (size_t)a.n * (a.n + VEC) * sizeof(T);
     const size_t red = (size_t)CT * Gen::DE * sizeof(T);

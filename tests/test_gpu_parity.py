@@ -283,6 +283,9 @@ def test_c3_full_size_chunked_sampled_centres():
     import paper_2504_16068_b200 as ab
     from paper_2504_16068_b200.pipeline import ChunkedStep, to_device
     from workloads.inputs import sub_inputs
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 140e9:
         pytest.skip("needs ~135 GB of free HBM")
@@ -395,6 +398,9 @@ def test_two_layer_model_c2_full_size_sampled_centres():
     from oracle import model2
     from workloads import rng
     from workloads.inputs import make_model_inputs
+    import gc
+    gc.collect()
+    torch.cuda.empty_cache()
     free, _ = torch.cuda.mem_get_info()
     if free < 110e9:
         pytest.skip("needs ~100 GB of free HBM")
