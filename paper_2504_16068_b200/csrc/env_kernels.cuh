@@ -364,6 +364,108 @@ __global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, doub
 }
 
 // ------------------------------------------------------------------------------------------------
+// Factorised geometry kernels, used when w / g_w are not requested.  The radial weights are LINEAR in the small basis,
+// w[e][ch] = sum_b W_r[ch][b] Bu_e[b], so the sums over a centre's edges and over channels can be regrouped exactly:
+//   Eenv[c][ch][j] = scale sum_b W_r[ch][b] S_c[b][j],            S_c[b][j] = sum_{e in row c} Bu_e[b] Y_j(e)     (NB x DE per centre)
+//   gY_e[j]        = sum_b Bu_e[b] M_c[b][j],                     M_c[b][j] = scale sum_ch gE[c][ch][j] W_r[ch][b]
+//   sum_ch g_w[e][ch] dw[e][ch]/dr = sum_j Y_j(e) sum_b dBu_e[b] M_c[b][j]
+// Per-edge work no longer scales with the channel count (72 FMAs instead of n x 17), and everything is in double.
+template <typename T, int L, int NB>
+__global__ void __launch_bounds__(kGeoChunk) env_radial_fwd_fact_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr,
+                                                                         const int* __restrict__ items, const T* __restrict__ rvec,
+                                                                         const T* __restrict__ W_r, double scale, T* __restrict__ dst, int by_item) {
+    constexpr int DE = (L + 1) * (L + 1);
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    GeoSmem<T, L, NB>& sm = *reinterpret_cast<GeoSmem<T, L, NB>*>(geo_raw);
+    double* S = reinterpret_cast<double*>(geo_raw + sizeof(GeoSmem<T, L, NB>));  // [NB][DE]
+    const int tid = threadIdx.x;
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    constexpr int R = (NB * DE + kGeoChunk - 1) / kGeoChunk;  // (basis, component) pairs per thread
+    double sacc[R];
+#pragma unroll
+    for (int r = 0; r < R; ++r) sacc[r] = 0.0;
+    for (int cb = e0; cb < e1; cb += kGeoChunk) {
+        const int cnt = min(kGeoChunk, e1 - cb);
+        if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+        __syncthreads();
+#pragma unroll
+        for (int r = 0; r < R; ++r) {
+            const int t = tid + r * kGeoChunk;
+            if (t < NB * DE) {
+                const int b = t / DE, j = t - b * DE;
+                for (int le = 0; le < cnt; ++le) sacc[r] = fma(sm.Bs[le][b], (double)sm.Ys[le][j], sacc[r]);
+            }
+        }
+        __syncthreads();
+    }
+#pragma unroll
+    for (int r = 0; r < R; ++r)
+        if (tid + r * kGeoChunk < NB * DE) S[tid + r * kGeoChunk] = sacc[r];
+    __syncthreads();
+    T* o = dst + (size_t)(by_item ? (long)blockIdx.x : (long)c) * n * DE;
+    for (int idx = tid; idx < n * DE; idx += kGeoChunk) {
+        const int ch = idx / DE, jj = idx - ch * DE;
+        double acc = 0.0;
+        for (int bb = 0; bb < nb; ++bb) acc = fma((double)W_r[ch * nb + bb], S[bb * DE + jj], acc);
+        o[idx] = (T)(scale * acc);
+    }
+}
+
+template <typename T, int L, int NB>
+__global__ void __launch_bounds__(kGeoChunk) env_radial_bwd_fact_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr,
+                                                                         const T* __restrict__ gEenv, const T* __restrict__ rvec,
+                                                                         const T* __restrict__ W_r, double scale, T* __restrict__ g_rvec) {
+    constexpr int DE = (L + 1) * (L + 1);
+    __shared__ double Ms[NB * DE];
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    T* gEs = reinterpret_cast<T*>(geo_raw);  // [n][DE] the centre's gEenv rows
+    T* Wrs = gEs + (size_t)n * DE;           // [n][nb]
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x;
+    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+    for (int idx = tid; idx < n * DE; idx += kGeoChunk) gEs[idx] = gEenv[(size_t)c * n * DE + idx];
+    for (int idx = tid; idx < n * nb; idx += kGeoChunk) Wrs[idx] = W_r[idx];
+    __syncthreads();
+    for (int t = tid; t < NB * DE; t += kGeoChunk) {
+        const int b = t / DE, j = t - b * DE;
+        double m = 0.0;
+        if (b < nb)
+            for (int ch = 0; ch < n; ++ch) m = fma((double)gEs[ch * DE + j], (double)Wrs[ch * nb + b], m);
+        Ms[t] = scale * m;
+    }
+    __syncthreads();
+    for (int e = e0 + tid; e < e1; e += kGeoChunk) {
+        const T rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+        const double dx = (double)rx, dy = (double)ry, dz = (double)rz;
+        const double rr = sqrt(dx * dx + dy * dy + dz * dz);
+        double Bu[kMaxBasis], dBu[kMaxBasis];
+        radial_basis<true>(rr, rc, nb, Bu, dBu);
+        const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+        const T x = rx * inv, y = ry * inv, z = rz * inv;
+        T Y[DE], gY[DE];
+        sph_harm<T, L>(x, y, z, Y);
+        double rad = 0.0;
+#pragma unroll
+        for (int j = 0; j < DE; ++j) {
+            double gy = 0.0, dj = 0.0;
+#pragma unroll
+            for (int b = 0; b < NB; ++b) {
+                if (b < nb) { gy = fma(Bu[b], Ms[b * DE + j], gy); dj = fma(dBu[b], Ms[b * DE + j], dj); }
+            }
+            gY[j] = (T)gy;
+            rad = fma((double)Y[j], dj, rad);
+        }
+        T g[3];
+        sph_harm_vjp<T, L>(x, y, z, gY, g);
+        const T dot = g[0] * x + g[1] * y + g[2] * z;
+        g_rvec[3 * (size_t)e] = (T)((double)((g[0] - dot * x) * inv) + rad * dx / rr);
+        g_rvec[3 * (size_t)e + 1] = (T)((double)((g[1] - dot * y) * inv) + rad * dy / rr);
+        g_rvec[3 * (size_t)e + 2] = (T)((double)((g[2] - dot * z) * inv) + rad * dz / rr);
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Layer-0 edge embedding of the two-layer model (reading A19; BASELINE.json:configs[2]):
 //   b_e = [B_b(r_e) u(r_e/r_c)],  x0[e][ch] = sum_b W_x0[ch][b] b_e[b],
 //   V0[e][ch][(l, (-1)^l), m] = (sum_b W_v0[ch][b] b_e[b]) Y_lm(rhat_e), other-parity slots 0.

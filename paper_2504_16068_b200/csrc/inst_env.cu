@@ -2,6 +2,8 @@
 #ifndef ALLEGRO_T
 #error "compile with -DALLEGRO_T=float|double -DALLEGRO_L=1|2|3"
 #endif
+#include <cstdlib>
+
 #include "env_kernels.cuh"
 
 namespace allegro {
@@ -31,6 +33,18 @@ allegro_status_t launch_env_embed<ALLEGRO_T, ALLEGRO_L>(const EnvArgs& a) {
             set_error("env_radial_forward: n = %d, n_basis = %d unsupported (n <= 128, n_basis <= %d)", a.n, a.nb, kMaxBasis);
             return ALLEGRO_EUNSUPPORTED;
         }
+        if (a.w_out == nullptr && getenv("ALLEGRO_GEO_UNFACTORISED") == nullptr) {   // w not requested: factorised form
+#define ALLEGRO_GEOFF(NB)                                                                                                  \
+    {                                                                                                                      \
+        auto k = env_radial_fwd_fact_kernel<T, ALLEGRO_L, NB>;                                                             \
+        const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>) + (size_t)NB * DE * sizeof(double);                          \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
+        k<<<(unsigned)a.n_items, kGeoChunk, smem, a.st>>>(a.n, a.nb, a.rc, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.W_r, \
+                                                          a.scale, dst, have_items ? 1 : 0);                               \
+    }
+            if (a.nb <= 8) ALLEGRO_GEOFF(8) else ALLEGRO_GEOFF(16)
+#undef ALLEGRO_GEOFF
+        } else {
 #define ALLEGRO_GEOF(CPL, NB)                                                                                              \
     {                                                                                                                      \
         auto k = env_radial_fwd_kernel<T, ALLEGRO_L, CPL, NB>;                                                             \
@@ -45,6 +59,7 @@ allegro_status_t launch_env_embed<ALLEGRO_T, ALLEGRO_L>(const EnvArgs& a) {
             if (a.n <= 32) ALLEGRO_GEOF(1, 16) else if (a.n <= 64) ALLEGRO_GEOF(2, 16) else ALLEGRO_GEOF(4, 16)
         }
 #undef ALLEGRO_GEOF
+        }
         ALLEGRO_LAUNCHED();
     } else {
     env_embed_kernel<T, ALLEGRO_L, kEnvThreads><<<(unsigned)a.n_items, kEnvThreads, 0, a.st>>>(
@@ -70,6 +85,16 @@ allegro_status_t launch_env_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EnvBwdArg
         if (a.n > 128 || a.nb > kMaxBasis) {
             set_error("env_radial_backward: n = %d, n_basis = %d unsupported (n <= 128, n_basis <= %d)", a.n, a.nb, kMaxBasis);
             return ALLEGRO_EUNSUPPORTED;
+        }
+        if (a.g_w == nullptr && getenv("ALLEGRO_GEO_UNFACTORISED") == nullptr) {   // g_w not requested: factorised form
+            constexpr int DEb = (ALLEGRO_L + 1) * (ALLEGRO_L + 1);
+#define ALLEGRO_GEOBF(NB)                                                                                                  \
+    env_radial_bwd_fact_kernel<T, ALLEGRO_L, NB><<<(unsigned)a.n_atoms, kGeoChunk, (size_t)a.n * (DEb + a.nb) * sizeof(T), a.st>>>( \
+        a.n, a.nb, a.rc, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.W_r, a.scale, (T*)a.g_rvec);
+            if (a.nb <= 8) { ALLEGRO_GEOBF(8) } else { ALLEGRO_GEOBF(16) }
+#undef ALLEGRO_GEOBF
+            ALLEGRO_LAUNCHED();
+            return ALLEGRO_OK;
         }
 #define ALLEGRO_GEOB(CPL, NB)                                                                                              \
     {                                                                                                                      \
