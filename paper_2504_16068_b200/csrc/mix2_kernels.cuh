@@ -28,7 +28,7 @@ struct Mix2 {
     static constexpr int CT = 256, EG = CT / N, EPT = 4, TE = EG * EPT, DV = Gen::DV, DE = Gen::DE, P = Gen::P;
     static constexpr int D3MAX = 2 * L + 1, LDT = N + 4;
     static constexpr size_t kVt = (size_t)TE * N * DV * sizeof(float);
-    static constexpr size_t kFwdSmem = kVt + 2 * (size_t)TE * D3MAX * LDT * sizeof(float);
+    static constexpr size_t kFwdSmem = 2 * kVt + (2 * (size_t)TE * D3MAX + N) * LDT * sizeof(float);
     static constexpr size_t kBwdSmem = kVt + (size_t)TE * DV * LDT * sizeof(float);
 };
 
@@ -46,14 +46,50 @@ __device__ __forceinline__ float dot_reg_smem(const float (&wr)[N], const float*
     return acc;
 }
 
+// NC dot products at once against columns that are `stride` floats apart: NC independent accumulation chains
+template <int N, int NC>
+__device__ __forceinline__ void dot_cols(const float (&wr)[N], const float* __restrict__ col0, int stride, float (&acc)[NC]) {
+#pragma unroll
+    for (int k = 0; k < N / 4; ++k) {
+#pragma unroll
+        for (int m = 0; m < NC; ++m) {
+            const float4 c = *reinterpret_cast<const float4*>(col0 + m * stride + 4 * k);
+            float a = acc[m];
+            a = fmaf(wr[4 * k], c.x, a);
+            a = fmaf(wr[4 * k + 1], c.y, a);
+            a = fmaf(wr[4 * k + 2], c.z, a);
+            a = fmaf(wr[4 * k + 3], c.w, a);
+            acc[m] = a;
+        }
+    }
+}
+
+// The loop over paths is a RUN-TIME loop: only the small per-path CG code is selected by a compare chain, the
+// 64-wide inner products exist once per (2 l3 + 1) in {1, 3, 5}.  (A fully unrolled version is 26k FMAs of straight-line
+// code per kernel and stalls on instruction fetch: measured "no_instruction" = 56 % of the warp stall samples.)
+template <int L>
+struct PathTab {
+    using Gen = TPGen<L>;
+    int d3[Gen::P], off3[Gen::P];
+};
+template <int L>
+__host__ __device__ constexpr PathTab<L> make_path_tab() {
+    PathTab<L> t{};
+    for (int p = 0; p < TPGen<L>::P; ++p) { t.d3[p] = TPGen<L>::d3(p); t.off3[p] = TPGen<L>::off3(p); }
+    return t;
+}
+
 template <int L, int N>
 __global__ void __launch_bounds__(256) mix_fwd2_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items, const float* __restrict__ V,
                                                         const float* __restrict__ Eenv, const float* __restrict__ W, float* __restrict__ out) {
     using M2 = Mix2<L, N>;
     constexpr int DV = M2::DV, DE = M2::DE, P = M2::P, EPT = M2::EPT, TE = M2::TE, LDT = M2::LDT, D3MAX = M2::D3MAX;
+    constexpr PathTab<L> tab = make_path_tab<L>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* Vt = reinterpret_cast<float*>(smem_raw);                 // [TE][N][DV]
-    float* tP = reinterpret_cast<float*>(smem_raw + M2::kVt);       // [2][TE * D3MAX][LDT]
+    float* Os = Vt + (size_t)TE * N * DV;                            // [TE][N][DV] out tile (accumulated over paths)
+    float* tP = Os + (size_t)TE * N * DV;                            // [2][TE * D3MAX][LDT]
+    float* Ws = tP + 2 * (size_t)TE * D3MAX * LDT;                   // [N][LDT]
     const int tid = threadIdx.x, ch = tid % N, eg = tid / N;
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
@@ -63,57 +99,73 @@ __global__ void __launch_bounds__(256) mix_fwd2_kernel(const int* __restrict__ r
 
     for (int eb = e0; eb < e1; eb += TE) {
         const int cnt = min(TE, e1 - eb);
-        {   // V tile: one contiguous byte range, 128-bit coalesced loads
+        {   // V tile: one contiguous byte range, 128-bit coalesced loads; out tile zeroed
             const int4* src = reinterpret_cast<const int4*>(V + (size_t)eb * N * DV);
             int4* dst = reinterpret_cast<int4*>(Vt);
-            for (int idx = tid; idx < cnt * N * DV / 4; idx += 256) dst[idx] = src[idx];
+            int4* oz = reinterpret_cast<int4*>(Os);
+            for (int idx = tid; idx < cnt * N * DV / 4; idx += 256) { dst[idx] = src[idx]; oz[idx] = make_int4(0, 0, 0, 0); }
         }
         __syncthreads();
-        float acc[EPT][DV];
-#pragma unroll
-        for (int q = 0; q < EPT; ++q)
-#pragma unroll
-            for (int k = 0; k < DV; ++k) acc[q][k] = 0.f;
-        static_for2<0, P>([&](auto pc) {
-            constexpr int p = decltype(pc)::value;
-            using Pth = TPPath<L, p>;
-            constexpr int D3 = Pth::D3, OFF3 = Pth::OFF3;
+        for (int p = 0; p < P; ++p) {
+            const int d3 = tab.d3[p], off3 = tab.off3[p];
             float* buf = tP + (size_t)(p & 1) * TE * D3MAX * LDT;
+            static_for2<0, P>([&](auto pc) {   // t_p of this thread's (edge, channel) pairs: per-path generated code
+                constexpr int pp = decltype(pc)::value;
+                if (p == pp) {
+                    using Pth = TPPath<L, pp>;
 #pragma unroll
-            for (int q = 0; q < EPT; ++q) {
-                const int el = eg * EPT + q;
-                if (el < cnt) {
-                    float t[D3];
-                    Pth::template fwd<float>(Vt + ((size_t)el * N + ch) * DV, E, t);
+                    for (int q = 0; q < EPT; ++q) {
+                        const int el = eg * EPT + q;
+                        if (el < cnt) {
+                            float t[Pth::D3];
+                            Pth::template fwd<float>(Vt + ((size_t)el * N + ch) * DV, E, t);
 #pragma unroll
-                    for (int M = 0; M < D3; ++M) buf[(el * D3 + M) * LDT + ch] = t[M];
+                            for (int M = 0; M < Pth::D3; ++M) buf[(el * Pth::D3 + M) * LDT + ch] = t[M];
+                        }
+                    }
+                }
+            });
+            {   // W_p: coalesced 128-bit global reads into shared memory (row stride LDT: conflict-free row reads)
+                const float4* w4 = reinterpret_cast<const float4*>(W + (size_t)p * N * N);
+#pragma unroll
+                for (int it = 0; it < N * N / 4 / 256; ++it) {
+                    const int idx = tid + it * 256, r = idx / (N / 4), c4 = idx - r * (N / 4);
+                    *reinterpret_cast<float4*>(Ws + r * LDT + 4 * c4) = w4[idx];
                 }
             }
+            __syncthreads();  // tP[p & 1] and Ws complete
             float wr[N];
-            {
-                const float4* w4 = reinterpret_cast<const float4*>(W + ((size_t)p * N + ch) * N);
 #pragma unroll
-                for (int k = 0; k < N / 4; ++k) {
-                    const float4 w = w4[k];
-                    wr[4 * k] = w.x; wr[4 * k + 1] = w.y; wr[4 * k + 2] = w.z; wr[4 * k + 3] = w.w;
-                }
+            for (int k = 0; k < N / 4; ++k) {
+                const float4 w = *reinterpret_cast<const float4*>(Ws + ch * LDT + 4 * k);
+                wr[4 * k] = w.x; wr[4 * k + 1] = w.y; wr[4 * k + 2] = w.z; wr[4 * k + 3] = w.w;
             }
-            __syncthreads();
+            __syncthreads();  // every row is in registers: Ws may be overwritten by the next path
+            auto gemm = [&](auto dc) {
+                constexpr int D3 = decltype(dc)::value;
 #pragma unroll
-            for (int q = 0; q < EPT; ++q) {
-                const int el = eg * EPT + q;
-                if (el < cnt) {
+                for (int q = 0; q < EPT; ++q) {
+                    const int el = eg * EPT + q;   // rows beyond the ragged tail hold stale values and are never stored
+                    float a[D3];
 #pragma unroll
-                    for (int M = 0; M < D3; ++M) acc[q][OFF3 + M] = dot_reg_smem<N>(wr, buf + (el * D3 + M) * LDT, acc[q][OFF3 + M]);
+                    for (int M = 0; M < D3; ++M) a[M] = 0.f;
+                    dot_cols<N, D3>(wr, buf + (el * D3) * LDT, LDT, a);
+                    float* o = Os + ((size_t)el * N + ch) * DV + off3;
+#pragma unroll
+                    for (int M = 0; M < D3; ++M) o[M] += a[M];
                 }
-            }
-        });
-#pragma unroll
-        for (int q = 0; q < EPT; ++q) {
-            const int el = eg * EPT + q;
-            if (el < cnt) row_store<float, DV>(out + ((size_t)(eb + el) * N + ch) * DV, acc[q]);
+            };
+            if (d3 == 1) gemm(std::integral_constant<int, 1>{});
+            else if (d3 == 3) gemm(std::integral_constant<int, 3>{});
+            else gemm(std::integral_constant<int, (L >= 2 ? 5 : 3)>{});
         }
-        __syncthreads();  // Vt and tP are rewritten by the next tile
+        __syncthreads();
+        {   // out tile: one contiguous byte range, 128-bit coalesced stores
+            int4* dst = reinterpret_cast<int4*>(out + (size_t)eb * N * DV);
+            const int4* src = reinterpret_cast<const int4*>(Os);
+            for (int idx = tid; idx < cnt * N * DV / 4; idx += 256) dst[idx] = src[idx];
+        }
+        __syncthreads();  // Vt, Os and tP are rewritten by the next tile
     }
 }
 
@@ -123,6 +175,7 @@ __global__ void __launch_bounds__(256) mix_bwd2_kernel(const int* __restrict__ r
                                                         float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
     using M2 = Mix2<L, N>;
     constexpr int DV = M2::DV, DE = M2::DE, P = M2::P, EPT = M2::EPT, TE = M2::TE, LDT = M2::LDT, EG = M2::EG;
+    constexpr PathTab<L> tab = make_path_tab<L>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* Vt = reinterpret_cast<float*>(smem_raw);                 // [TE][N][DV]
     float* gS = reinterpret_cast<float*>(smem_raw + M2::kVt);       // [TE * DV][LDT]: gS[(e, k)][n'] = G[e][n'][k]
@@ -151,24 +204,44 @@ __global__ void __launch_bounds__(256) mix_bwd2_kernel(const int* __restrict__ r
         for (int q = 0; q < EPT; ++q)
 #pragma unroll
             for (int k = 0; k < DV; ++k) gv[q][k] = 0.f;
-        static_for2<0, P>([&](auto pc) {
-            constexpr int p = decltype(pc)::value;
-            using Pth = TPPath<L, p>;
-            constexpr int D3 = Pth::D3, OFF3 = Pth::OFF3;
+        for (int p = 0; p < P; ++p) {
+            const int d3 = tab.d3[p], off3 = tab.off3[p];
             float wc[N];  // W_p[n'][ch], n' = 0..N-1 (coalesced across ch)
 #pragma unroll
             for (int k = 0; k < N; ++k) wc[k] = W[((size_t)p * N + k) * N + ch];
+            float gt[EPT][M2::D3MAX];
+            auto gemm = [&](auto dc) {
+                constexpr int D3 = decltype(dc)::value;
 #pragma unroll
-            for (int q = 0; q < EPT; ++q) {
-                const int el = eg * EPT + q;
-                if (el < cnt) {
-                    float gt[D3];
+                for (int q = 0; q < EPT; ++q) {
+                    float a[D3];
 #pragma unroll
-                    for (int M = 0; M < D3; ++M) gt[M] = dot_reg_smem<N>(wc, gS + (el * DV + OFF3 + M) * LDT, 0.f);
-                    Pth::template bwd<float, WANT_GV>(Vt + ((size_t)el * N + ch) * DV, E, gt, gv[q], gE);
+                    for (int M = 0; M < D3; ++M) a[M] = 0.f;
+                    dot_cols<N, D3>(wc, gS + ((eg * EPT + q) * DV + off3) * LDT, LDT, a);
+#pragma unroll
+                    for (int M = 0; M < D3; ++M) gt[q][M] = a[M];
                 }
-            }
-        });
+            };
+            if (d3 == 1) gemm(std::integral_constant<int, 1>{});
+            else if (d3 == 3) gemm(std::integral_constant<int, 3>{});
+            else gemm(std::integral_constant<int, (L >= 2 ? 5 : 3)>{});
+            static_for2<0, P>([&](auto pc) {   // per-path CG VJP: generated code selected by a compare chain
+                constexpr int pp = decltype(pc)::value;
+                if (p == pp) {
+                    using Pth = TPPath<L, pp>;
+#pragma unroll
+                    for (int q = 0; q < EPT; ++q) {
+                        const int el = eg * EPT + q;
+                        if (el < cnt) {
+                            float g3[Pth::D3];
+#pragma unroll
+                            for (int M = 0; M < Pth::D3; ++M) g3[M] = gt[q][M];
+                            Pth::template bwd<float, WANT_GV>(Vt + ((size_t)el * N + ch) * DV, E, g3, gv[q], gE);
+                        }
+                    }
+                }
+            });
+        }
         if constexpr (WANT_GV) {
 #pragma unroll
             for (int q = 0; q < EPT; ++q) {
