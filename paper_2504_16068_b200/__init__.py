@@ -54,6 +54,9 @@ SIGNATURES = {
     "allegro_env_radial_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, C.c_double, C.c_double, _vp, _vp, _vp]),
     "allegro_edge_energy": (C.c_int, [_vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_segment_sum": (C.c_int, [_vp, C.c_int, _vp, C.c_int, _vp, _vp]),
+    "allegro_layer_step_host_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_int, C.c_int]),
+    "allegro_layer_step_host": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, C.c_double, C.c_double,
+                                          C.c_int, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_edge_embed": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp]),
     "allegro_edge_embed_backward": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp, _vp]),
     "allegro_linear": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_int, C.c_int, _vp, _vp]),
@@ -389,3 +392,17 @@ def latent_backward(rvec, r_cut, z, g_xnew, A, gV, g_rvec, g_x=None, stream=None
 def add_inplace(y, x, stream=None):
     _check(lib().allegro_add_inplace(y.numel(), _dt(y), _ptr(y), _ptr(x), _stream(stream)))
     return y
+
+
+def layer_step_host_workspace(plan, n_atoms, n_edges, n_basis, want_gV=True):
+    return lib().allegro_layer_step_host_workspace(plan.h, n_atoms, n_edges, n_basis, int(bool(want_gV)))
+
+
+def layer_step_host(plan, row_ptr, rev, rvec, V, W_r, r_cut, path_w, q, kappa, scale, F, e_tot, workspace, want_gV=True, stream=None):
+    """All tensor arguments except `workspace` are HOST tensors (ideally pinned); F [N,3] and e_tot [1] are filled on return."""
+    for t in (row_ptr, rev, rvec, V, W_r, path_w, q, F, e_tot):
+        assert not t.is_cuda and t.is_contiguous()
+    _check(lib().allegro_layer_step_host(plan.h, row_ptr.shape[0] - 1, rvec.shape[0], _ptr(row_ptr), _ptr(rev), _ptr(rvec), _ptr(V), _ptr(W_r),
+                                         W_r.shape[1], float(r_cut), _ptr(path_w), _ptr(q), float(kappa), float(scale), int(bool(want_gV)),
+                                         _ptr(F), _ptr(e_tot), _ptr(workspace), workspace.numel(), _stream(stream)))
+    return F, e_tot

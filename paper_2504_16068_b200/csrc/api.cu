@@ -306,6 +306,80 @@ allegro_status_t allegro_segment_sum(const int32_t* ptr, int n_segments, const v
                                 : launch_segment_sum<double>(ptr, n_segments, vals, out, (cudaStream_t)stream);
 }
 
+// ---------------------------------------------------------------------------------------------- one-call MD step from HOST buffers
+namespace {
+struct StepLayout {
+    size_t row_ptr, rev, e_ptr, rvec, V, W_r, path_w, q, Eenv, gEenv, out, gV, e_edge, g_r, F, e_tot, total;
+};
+StepLayout step_layout(const allegro_plan_t* plan, int N, long E, int nb, int want_gV) {
+    const size_t s = plan->dtype == ALLEGRO_F32 ? 4 : 8;
+    const size_t n = plan->n, dV = plan->tab.dV, dE = plan->tab.dE, P = plan->tab.paths.size();
+    StepLayout L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += allegro::align_up(bytes ? bytes : 1, 256); return o; };
+    L.row_ptr = take((size_t)(N + 1) * 4); L.rev = take((size_t)E * 4); L.e_ptr = take(8);
+    L.rvec = take((size_t)E * 3 * s); L.V = take((size_t)E * n * dV * s); L.W_r = take(n * nb * s); L.path_w = take(P * s); L.q = take(n * s);
+    L.Eenv = take((size_t)N * n * dE * s); L.gEenv = take((size_t)N * n * dE * s); L.out = take((size_t)E * n * dV * s);
+    L.gV = want_gV ? take((size_t)E * n * dV * s) : 0;
+    L.e_edge = take((size_t)E * s); L.g_r = take((size_t)E * 3 * s); L.F = take((size_t)N * 3 * s); L.e_tot = take(s);
+    L.total = off;
+    return L;
+}
+}  // namespace
+
+size_t allegro_layer_step_host_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges, int n_basis, int want_gV) {
+    if (!plan || n_atoms < 0 || n_edges < 0 || n_basis < 1) return 0;
+    return step_layout(plan, n_atoms, n_edges, n_basis, want_gV).total;
+}
+
+allegro_status_t allegro_layer_step_host(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr_host,
+                                         const int32_t* rev_host, const void* rvec_host, const void* V_host, const void* W_r_host, int n_basis,
+                                         double r_cut, const void* path_w_host, const void* q_host, double kappa, double scale, int want_gV,
+                                         void* F_host, void* e_tot_host, void* workspace, size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_atoms >= 0 && n_edges >= 0 && n_edges < 2147483647L, "bad plan / sizes");
+    ALLEGRO_CHECK_ARG(row_ptr_host && W_r_host && path_w_host && q_host && F_host && e_tot_host, "NULL host argument");
+    ALLEGRO_CHECK_ARG((rev_host && rvec_host && V_host) || n_edges == 0, "NULL host tensor");
+    ALLEGRO_CHECK_ARG(plan->wmode == ALLEGRO_W_SCALAR, "scalar path weights only");
+    const StepLayout L = step_layout(plan, n_atoms, n_edges, n_basis, want_gV);
+    if (workspace == nullptr || workspace_bytes < L.total || !aligned16(workspace)) {
+        set_error("allegro_layer_step_host: workspace too small or misaligned (%zu < %zu bytes)", workspace_bytes, L.total);
+        return ALLEGRO_ENOMEM;
+    }
+    cudaStream_t st = (cudaStream_t)stream;
+    unsigned char* ws = (unsigned char*)workspace;
+    const size_t s = plan->dtype == ALLEGRO_F32 ? 4 : 8;
+    const size_t n = plan->n, dV = plan->tab.dV, P = plan->tab.paths.size();
+    const int32_t e_ptr[2] = {0, (int32_t)n_edges};
+    ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.row_ptr, row_ptr_host, (size_t)(n_atoms + 1) * 4, cudaMemcpyHostToDevice, st));
+    ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.e_ptr, e_ptr, 8, cudaMemcpyHostToDevice, st));
+    if (n_edges > 0) {
+        ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.rev, rev_host, (size_t)n_edges * 4, cudaMemcpyHostToDevice, st));
+        ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.rvec, rvec_host, (size_t)n_edges * 3 * s, cudaMemcpyHostToDevice, st));
+        ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.V, V_host, (size_t)n_edges * n * dV * s, cudaMemcpyHostToDevice, st));
+    }
+    ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.W_r, W_r_host, n * n_basis * s, cudaMemcpyHostToDevice, st));
+    ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.path_w, path_w_host, P * s, cudaMemcpyHostToDevice, st));
+    ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.q, q_host, n * s, cudaMemcpyHostToDevice, st));
+    const int32_t* rp = (const int32_t*)(ws + L.row_ptr);
+    allegro_status_t r;
+    if ((r = allegro_env_radial_forward(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.rvec, ws + L.W_r, n_basis, r_cut, scale, nullptr,
+                                        ws + L.Eenv, nullptr, 0, stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_tp_forward_energy(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.V, ws + L.Eenv, ws + L.path_w, ws + L.q, kappa, ws + L.out,
+                                       ws + L.e_edge, nullptr, stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_tp_backward_energy(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.out, ws + L.V, ws + L.Eenv, ws + L.path_w, ws + L.q, kappa,
+                                        want_gV ? ws + L.gV : nullptr, ws + L.gEenv, nullptr, nullptr, 0, stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_env_radial_backward(plan, n_atoms, n_edges, rp, ws + L.gEenv, ws + L.rvec, ws + L.W_r, n_basis, r_cut, scale, ws + L.g_r,
+                                         nullptr, stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_force_gather(n_atoms, n_edges, rp, (const int32_t*)(ws + L.rev), ws + L.g_r, (allegro_dtype_t)plan->dtype, ws + L.F,
+                                  stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_segment_sum((const int32_t*)(ws + L.e_ptr), 1, ws + L.e_edge, (allegro_dtype_t)plan->dtype, ws + L.e_tot, stream)) != ALLEGRO_OK)
+        return r;
+    ALLEGRO_CUDA(cudaMemcpyAsync(F_host, ws + L.F, (size_t)n_atoms * 3 * s, cudaMemcpyDeviceToHost, st));
+    ALLEGRO_CUDA(cudaMemcpyAsync(e_tot_host, ws + L.e_tot, s, cudaMemcpyDeviceToHost, st));
+    ALLEGRO_CUDA(cudaStreamSynchronize(st));
+    return ALLEGRO_OK;
+}
+
 // ---------------------------------------------------------------------------------------------- two-layer model helpers
 allegro_status_t allegro_edge_embed(const allegro_plan_t* plan, long n_edges, const void* rvec, const void* W_x0, const void* W_v0, int n_basis,
                                     double r_cut, void* x0, void* V0, void* stream) {

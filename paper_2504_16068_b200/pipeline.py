@@ -152,30 +152,28 @@ class SingleLayerStep:
 
 
 class HostStep:
-    """The same step called with HOST buffers: every input of the step (row_ptr, rev, rvec, V) sits in pinned host
-    memory and is copied to the device inside run(); forces and the total energy are copied back to pinned host
-    memory and run() returns after they have arrived.  The small parameter tensors (W_r, path_w, q) stay resident."""
+    """The same step through the C ABI's host entry point allegro_layer_step_host: every input of the step (row_ptr, rev,
+    rvec, V and the small parameter tensors) sits in pinned host memory and is copied to the device inside the call;
+    forces and the total energy come back to pinned host memory before the call returns."""
 
-    KEYS = ("row_ptr", "rev", "rvec", "V")
+    KEYS = ("row_ptr", "rev", "rvec", "V", "W_r", "path_w", "q")
 
     def __init__(self, step, inp=None):
         self.step = step
-        d = step.dev
+        d, p = step.dev, step.plan
         self.host = {k: torch.empty(d[k].shape, dtype=d[k].dtype, pin_memory=True).copy_(d[k]) for k in self.KEYS}
         self.F_host = torch.empty(step.F.shape, dtype=step.F.dtype, pin_memory=True)
         self.e_host = torch.empty(step.e_tot.shape, dtype=step.e_tot.dtype, pin_memory=True)
+        self.want_gV = step.gV is not None
+        nbytes = ab.layer_step_host_workspace(p, step.N, step.E, d["W_r"].shape[1], self.want_gV)
+        self.ws = torch.empty(nbytes, dtype=torch.uint8, device=d["rvec"].device)
         self.h2d_bytes = int(sum(v.numel() * v.element_size() for v in self.host.values()))
         self.d2h_bytes = int(self.F_host.numel() * self.F_host.element_size() + self.e_host.numel() * self.e_host.element_size())
 
     def run(self):
-        d = self.step.dev
-        for k in self.KEYS:
-            d[k].copy_(self.host[k], non_blocking=True)
-        self.step.run()
-        self.F_host.copy_(self.step.F, non_blocking=True)
-        self.e_host.copy_(self.step.e_tot, non_blocking=True)
-        torch.cuda.current_stream().synchronize()
-        return self.F_host, self.e_host
+        h, s = self.host, self.step
+        return ab.layer_step_host(s.plan, h["row_ptr"], h["rev"], h["rvec"], h["V"], h["W_r"], s.rc, h["path_w"], h["q"], s.kappa, s.scale,
+                                  self.F_host, self.e_host, self.ws, want_gV=self.want_gV)
 
 
 class ChunkedStep:

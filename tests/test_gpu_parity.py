@@ -426,3 +426,25 @@ def test_two_layer_model_c2_full_size_sampled_centres():
         got = dict(g_r=st.g_r[e0:e1], e_edge=st.e_edge[e0:e1], V2=st.V[2][e0:e1], Eenv1=st.Eenv[1][c0:c1])
         _assert_close(ref, got, inp["dt"], keys=tuple(ref.keys()), label="C2 centres [%d,%d)" % (c0, c1))
     _check_force_gather(inp, dict(g_r=st.g_r, F=st.F))
+
+
+@pytest.mark.parametrize("name", ["C0", "C1s"])
+def test_host_buffer_step_through_c_abi(name):
+    """allegro_layer_step_host: host buffers in, forces and total energy out in one C-ABI call (bench.py's end-to-end arm)"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import HostStep, SingleLayerStep
+    inp = _chain.make_inputs(name)
+    ref = _chain.oracle_chain(inp, want_gw=False)
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32)
+    st = SingleLayerStep(plan, _chain.to_device(inp), inp["rc"], inp["kappa"], inp["scale"])
+    hs = HostStep(st)
+    F, e = hs.run()
+    _assert_close(ref, dict(F=F), inp["dt"], keys=("F",), label=name + "/host")
+    e_ref = float(np.sum(ref["e_edge"]))
+    assert abs(float(e.item()) - e_ref) <= _chain.TOL[inp["dt"]] * max(abs(e_ref), float(np.abs(ref["e_edge"]).max()))
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.layer_step_host(plan, hs.host["row_ptr"], hs.host["rev"], hs.host["rvec"], hs.host["V"], hs.host["W_r"], inp["rc"], hs.host["path_w"],
+                           hs.host["q"], inp["kappa"], inp["scale"], hs.F_host, hs.e_host, torch.empty(256, dtype=torch.uint8, device="cuda"))
+    assert ei.value.status == 4
