@@ -344,3 +344,31 @@ class TwoLayerStep:
         dT = {1: 22, 2: 102, 3: 312}[pd.l_max]
         mix = 2 * n * n * dT
         return {"tp_forward_dense": L * self.E * (cg_fwd + mix), "tp_backward_dense": L * self.E * (2 * cg_fwd + mix)}
+
+
+class GraphedStep:
+    """A step object (SingleLayerStep / TwoLayerStep / ChunkedStep) captured once into a CUDA graph and replayed: one graph
+    launch per MD step instead of 8-30 kernel launches, which is what bounds small systems (the paper's 25-100 atom
+    molecules).  Buffers are the wrapped step's own (allocated once), so replays read the current contents
+    of dev["rvec"], dev["V"], ... and overwrite F / e_tot in place."""
+
+    def __init__(self, step, warmup=3):
+        self.step = step
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):       # warm up on the capture stream (first calls set function attributes)
+            for _ in range(warmup):
+                step.run()
+        torch.cuda.current_stream().wait_stream(side)
+        torch.cuda.synchronize()
+        self.graph = torch.cuda.CUDAGraph()
+        n0 = ab.launch_count()
+        with torch.cuda.graph(self.graph):
+            step.run()
+        self.kernels_per_step = ab.launch_count() - n0      # kernel nodes of the graph = kernels each replay launches
+        self.F, self.e_tot = step.F, step.e_tot
+        self.marks = None
+
+    def run(self, mark=False):
+        self.graph.replay()
+        return self.F, self.e_tot

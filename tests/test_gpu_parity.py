@@ -448,3 +448,29 @@ def test_host_buffer_step_through_c_abi(name):
         ab.layer_step_host(plan, hs.host["row_ptr"], hs.host["rev"], hs.host["rvec"], hs.host["V"], hs.host["W_r"], inp["rc"], hs.host["path_w"],
                            hs.host["q"], inp["kappa"], inp["scale"], hs.F_host, hs.e_host, torch.empty(256, dtype=torch.uint8, device="cuda"))
     assert ei.value.status == 4
+
+
+def test_cuda_graph_replay_matches_eager():
+    """pipeline.GraphedStep: the step captured into one CUDA graph gives the same bits as the eager call sequence, also after
+    the inputs change in place (an MD loop updates rvec between steps)"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import GraphedStep, SingleLayerStep
+    inp = _chain.make_inputs("C4s")
+    dev = _chain.to_device(inp)
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F32)
+    st = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"])
+    st.run()
+    F0, e0 = st.F.clone(), st.e_tot.clone()
+    gs = GraphedStep(st)
+    st.F.zero_()
+    gs.run()
+    torch.cuda.synchronize()
+    assert torch.equal(gs.F, F0) and torch.equal(gs.e_tot, e0)
+    dev["rvec"].mul_(1.01)                       # new geometry, same graph
+    gs.run()
+    F1 = gs.F.clone()
+    st.run()
+    torch.cuda.synchronize()
+    assert torch.equal(st.F, F1) and not torch.equal(F1, F0)
