@@ -28,7 +28,9 @@ struct Mix2 {
     static constexpr int CT = 256, EG = CT / N, EPT = 4, TE = EG * EPT, DV = Gen::DV, DE = Gen::DE, P = Gen::P;
     static constexpr int D3MAX = 2 * L + 1, LDT = N + 4;
     static constexpr size_t kVt = (size_t)TE * N * DV * sizeof(float);
-    static constexpr size_t kFwdSmem = 2 * kVt + (2 * (size_t)TE * D3MAX + N) * LDT * sizeof(float);
+    static constexpr int EPTF = 2, TEF = EG * EPTF;   // forward tile: 8 edges (n = 64) so that two CTAs fit one SM
+    static constexpr size_t kVtF = (size_t)TEF * N * DV * sizeof(float);
+    static constexpr size_t kFwdSmem = 2 * kVtF + ((size_t)TEF * D3MAX + N) * LDT * sizeof(float);
     static constexpr size_t kBwdSmem = kVt + (size_t)TE * DV * LDT * sizeof(float);
 };
 
@@ -64,6 +66,19 @@ __device__ __forceinline__ void dot_cols(const float (&wr)[N], const float* __re
     }
 }
 
+// 3xTF32 on the tensor cores (legacy mma.sync path; tcgen05 is the next step): x = hi + lo with hi = tf32(x), lo = tf32(x - hi);
+// A.B ~= A_lo.B_hi + A_hi.B_lo + A_hi.B_hi keeps ~21 mantissa bits, enough for the 1e-5 fp32 tolerance (plain TF32 is not).
+__device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
+    const float r = x - __uint_as_float(hi);
+    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(r));
+}
+__device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
+    asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
+                 : "+f"(d[0]), "+f"(d[1]), "+f"(d[2]), "+f"(d[3])
+                 : "r"(a[0]), "r"(a[1]), "r"(a[2]), "r"(a[3]), "r"(b0), "r"(b1));
+}
+
 // The loop over paths is a RUN-TIME loop: only the small per-path CG code is selected by a compare chain, the
 // 64-wide inner products exist once per (2 l3 + 1) in {1, 3, 5}.  (A fully unrolled version is 26k FMAs of straight-line
 // code per kernel and stalls on instruction fetch: measured "no_instruction" = 56 % of the warp stall samples.)
@@ -80,16 +95,16 @@ __host__ __device__ constexpr PathTab<L> make_path_tab() {
 }
 
 template <int L, int N>
-__global__ void __launch_bounds__(256) mix_fwd2_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items, const float* __restrict__ V,
+__global__ void __launch_bounds__(256, 2) mix_fwd2_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items, const float* __restrict__ V,
                                                         const float* __restrict__ Eenv, const float* __restrict__ W, float* __restrict__ out) {
     using M2 = Mix2<L, N>;
-    constexpr int DV = M2::DV, DE = M2::DE, P = M2::P, EPT = M2::EPT, TE = M2::TE, LDT = M2::LDT, D3MAX = M2::D3MAX;
+    constexpr int DV = M2::DV, DE = M2::DE, P = M2::P, EPT = M2::EPTF, TE = M2::TEF, LDT = M2::LDT, D3MAX = M2::D3MAX;
     constexpr PathTab<L> tab = make_path_tab<L>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* Vt = reinterpret_cast<float*>(smem_raw);                 // [TE][N][DV]
     float* Os = Vt + (size_t)TE * N * DV;                            // [TE][N][DV] out tile (accumulated over paths)
-    float* tP = Os + (size_t)TE * N * DV;                            // [2][TE * D3MAX][LDT]
-    float* Ws = tP + 2 * (size_t)TE * D3MAX * LDT;                   // [N][LDT]
+    float* tP = Os + (size_t)TE * N * DV;                            // [TE * D3MAX][LDT]
+    float* Ws = tP + (size_t)TE * D3MAX * LDT;                       // [N][LDT]
     const int tid = threadIdx.x, ch = tid % N, eg = tid / N;
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
@@ -108,7 +123,7 @@ __global__ void __launch_bounds__(256) mix_fwd2_kernel(const int* __restrict__ r
         __syncthreads();
         for (int p = 0; p < P; ++p) {
             const int d3 = tab.d3[p], off3 = tab.off3[p];
-            float* buf = tP + (size_t)(p & 1) * TE * D3MAX * LDT;
+            float* buf = tP;
             static_for2<0, P>([&](auto pc) {   // t_p of this thread's (edge, channel) pairs: per-path generated code
                 constexpr int pp = decltype(pc)::value;
                 if (p == pp) {
@@ -134,30 +149,41 @@ __global__ void __launch_bounds__(256) mix_fwd2_kernel(const int* __restrict__ r
                 }
             }
             __syncthreads();  // tP[p & 1] and Ws complete
-            float wr[N];
+            {   // D[n' (64) x cols (TE * d3)] = W_p . T_p on the tensor cores: warp -> 16 rows (mt) and every other 8-column tile
+                const int lane = tid & 31, warp = tid >> 5, g = lane >> 2, t4 = lane & 3;
+                const int mt = warp & 3, half = warp >> 2;
+                uint32_t ahi[N / 8][4], alo[N / 8][4];
 #pragma unroll
-            for (int k = 0; k < N / 4; ++k) {
-                const float4 w = *reinterpret_cast<const float4*>(Ws + ch * LDT + 4 * k);
-                wr[4 * k] = w.x; wr[4 * k + 1] = w.y; wr[4 * k + 2] = w.z; wr[4 * k + 3] = w.w;
-            }
-            __syncthreads();  // every row is in registers: Ws may be overwritten by the next path
-            auto gemm = [&](auto dc) {
-                constexpr int D3 = decltype(dc)::value;
-#pragma unroll
-                for (int q = 0; q < EPT; ++q) {
-                    const int el = eg * EPT + q;   // rows beyond the ragged tail hold stale values and are never stored
-                    float a[D3];
-#pragma unroll
-                    for (int M = 0; M < D3; ++M) a[M] = 0.f;
-                    dot_cols<N, D3>(wr, buf + (el * D3) * LDT, LDT, a);
-                    float* o = Os + ((size_t)el * N + ch) * DV + off3;
-#pragma unroll
-                    for (int M = 0; M < D3; ++M) o[M] += a[M];
+                for (int kt = 0; kt < N / 8; ++kt) {
+                    const float* w0 = Ws + (mt * 16 + g) * LDT + kt * 8 + t4;
+                    split_tf32(w0[0], ahi[kt][0], alo[kt][0]);
+                    split_tf32(w0[8 * LDT], ahi[kt][1], alo[kt][1]);
+                    split_tf32(w0[4], ahi[kt][2], alo[kt][2]);
+                    split_tf32(w0[8 * LDT + 4], ahi[kt][3], alo[kt][3]);
                 }
-            };
-            if (d3 == 1) gemm(std::integral_constant<int, 1>{});
-            else if (d3 == 3) gemm(std::integral_constant<int, 3>{});
-            else gemm(std::integral_constant<int, (L >= 2 ? 5 : 3)>{});
+                const int ntiles = TE * d3 / 8;
+                for (int nt = half; nt < ntiles; nt += 2) {
+                    float dacc[4] = {0.f, 0.f, 0.f, 0.f};
+                    const float* bcol = buf + (nt * 8 + g) * LDT + t4;
+#pragma unroll
+                    for (int kt = 0; kt < N / 8; ++kt) {
+                        uint32_t bh0, bl0, bh1, bl1;
+                        split_tf32(bcol[kt * 8], bh0, bl0);
+                        split_tf32(bcol[kt * 8 + 4], bh1, bl1);
+                        mma_tf32(dacc, alo[kt], bh0, bh1);
+                        mma_tf32(dacc, ahi[kt], bl0, bl1);
+                        mma_tf32(dacc, ahi[kt], bh0, bh1);
+                    }
+                    // c0: (row g, col 2 t4), c1: (row g, col 2 t4 + 1), c2 / c3: row g + 8; col -> (edge, M) of this path
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) {
+                        const int col = nt * 8 + 2 * t4 + (i & 1), row = mt * 16 + g + ((i & 2) ? 8 : 0);
+                        const int el = col / d3, M = col - el * d3;
+                        Os[((size_t)el * N + row) * DV + off3 + M] += dacc[i];
+                    }
+                }
+            }
+            __syncthreads();  // Ws and tP[p & 1] may be overwritten
         }
         __syncthreads();
         {   // out tile: one contiguous byte range, 128-bit coalesced stores
