@@ -66,12 +66,14 @@ __device__ __forceinline__ void dot_cols(const float (&wr)[N], const float* __re
     }
 }
 
-// 3xTF32 on the tensor cores (legacy mma.sync path; tcgen05 is the next step): x = hi + lo with hi = tf32(x), lo = tf32(x - hi);
+// 3xTF32 on the tensor cores (legacy mma.sync path; tcgen05 is the next step): x = hi + lo;
 // A.B ~= A_lo.B_hi + A_hi.B_lo + A_hi.B_hi keeps ~21 mantissa bits, enough for the 1e-5 fp32 tolerance (plain TF32 is not).
+// The split truncates instead of rounding (cvt.rna.tf32 is a ~5-instruction sequence on sm_100a and dominated the kernel:
+// profiles/r1_final.md): hi = x with the 13 low mantissa bits cleared, lo = x - hi (exact); the tensor core ignores lo's
+// low 13 bits, which leaves a relative error of 2^-20 per product.
 __device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(hi) : "f"(x));
-    const float r = x - __uint_as_float(hi);
-    asm("cvt.rna.tf32.f32 %0, %1;" : "=r"(lo) : "f"(r));
+    hi = __float_as_uint(x) & 0xffffe000u;
+    lo = __float_as_uint(x - __uint_as_float(hi));
 }
 __device__ __forceinline__ void mma_tf32(float (&d)[4], const uint32_t (&a)[4], uint32_t b0, uint32_t b1) {
     asm volatile("mma.sync.aligned.m16n8k8.row.col.f32.tf32.tf32.f32 {%0,%1,%2,%3}, {%4,%5,%6,%7}, {%8,%9}, {%0,%1,%2,%3};"
@@ -161,7 +163,9 @@ __global__ void __launch_bounds__(256, 2) mix_fwd2_kernel(const int* __restrict_
                     split_tf32(w0[4], ahi[kt][2], alo[kt][2]);
                     split_tf32(w0[8 * LDT + 4], ahi[kt][3], alo[kt][3]);
                 }
-                const int ntiles = TE * d3 / 8;
+                auto tiles = [&](auto dc) {   // (2 l3 + 1) as a compile-time constant: column -> (edge, M) without integer division
+                constexpr int D3 = decltype(dc)::value;
+                constexpr int ntiles = TE * D3 / 8;
                 for (int nt = half; nt < ntiles; nt += 2) {
                     float dacc[4] = {0.f, 0.f, 0.f, 0.f};
                     const float* bcol = buf + (nt * 8 + g) * LDT + t4;
@@ -178,12 +182,16 @@ __global__ void __launch_bounds__(256, 2) mix_fwd2_kernel(const int* __restrict_
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         const int col = nt * 8 + 2 * t4 + (i & 1), row = mt * 16 + g + ((i & 2) ? 8 : 0);
-                        const int el = col / d3, M = col - el * d3;
+                        const int el = col / D3, M = col - el * D3;
                         Os[((size_t)el * N + row) * DV + off3 + M] += dacc[i];
                     }
                 }
+                };
+                if (d3 == 1) tiles(std::integral_constant<int, 1>{});
+                else if (d3 == 3) tiles(std::integral_constant<int, 3>{});
+                else tiles(std::integral_constant<int, (L >= 2 ? 5 : 3)>{});
             }
-            __syncthreads();  // Ws and tP[p & 1] may be overwritten
+            __syncthreads();  // Ws and tP may be overwritten
         }
         __syncthreads();
         {   // out tile: one contiguous byte range, 128-bit coalesced stores
