@@ -413,8 +413,8 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
 
 
 def _ncu_traffic(workload, kernel):
-    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.json), or None"""
-    p = os.path.join(ROOT, "profiles", "traffic.json")
+    """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.txt), or None"""
+    p = os.path.join(ROOT, "profiles", "traffic.txt")
     if os.path.exists(p):
         with open(p) as f:
             return json.load(f).get(workload, {}).get(kernel)
