@@ -31,7 +31,7 @@ struct Mix2 {
     static constexpr int EPTF = 2, TEF = EG * EPTF;   // forward tile: 8 edges (n = 64) so that two CTAs fit one SM
     static constexpr size_t kVtF = (size_t)TEF * N * DV * sizeof(float);
     static constexpr size_t kFwdSmem = 2 * kVtF + ((size_t)TEF * D3MAX + N) * LDT * sizeof(float);
-    static constexpr size_t kBwdSmem = kVt + (size_t)TE * DV * LDT * sizeof(float);
+    static constexpr size_t kBwdSmem = kVtF + ((size_t)TEF * DV + (size_t)TEF * D3MAX + N) * LDT * sizeof(float);
 };
 
 template <int N>
@@ -204,16 +204,19 @@ __global__ void __launch_bounds__(256, 2) mix_fwd2_kernel(const int* __restrict_
 }
 
 template <int L, int N, bool WANT_GV>
-__global__ void __launch_bounds__(256) mix_bwd2_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items, const float* __restrict__ G,
-                                                        const float* __restrict__ V, const float* __restrict__ Eenv, const float* __restrict__ W,
-                                                        float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
+__global__ void __launch_bounds__(256, 2) mix_bwd2_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items, const float* __restrict__ G,
+                                                           const float* __restrict__ V, const float* __restrict__ Eenv, const float* __restrict__ W,
+                                                           float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
     using M2 = Mix2<L, N>;
-    constexpr int DV = M2::DV, DE = M2::DE, P = M2::P, EPT = M2::EPT, TE = M2::TE, LDT = M2::LDT, EG = M2::EG;
+    constexpr int DV = M2::DV, DE = M2::DE, P = M2::P, EPT = M2::EPTF, TE = M2::TEF, LDT = M2::LDT, EG = M2::EG, D3MAX = M2::D3MAX;
     constexpr PathTab<L> tab = make_path_tab<L>();
     extern __shared__ __align__(128) unsigned char smem_raw[];
     float* Vt = reinterpret_cast<float*>(smem_raw);                 // [TE][N][DV]
-    float* gS = reinterpret_cast<float*>(smem_raw + M2::kVt);       // [TE * DV][LDT]: gS[(e, k)][n'] = G[e][n'][k]
+    float* gS = Vt + (size_t)TE * N * DV;                            // [TE * DV][LDT]: gS[(e, k)][n'] = G[e][n'][k]
+    float* gtS = gS + (size_t)TE * DV * LDT;                         // [TE * D3MAX][LDT]: gt_p[(e, M)][n]
+    float* Ws = gtS + (size_t)TE * D3MAX * LDT;                      // [N][LDT]: W_p[n'][n]
     const int tid = threadIdx.x, ch = tid % N, eg = tid / N;
+    const int lane = tid & 31, warp = tid >> 5, g = lane >> 2, t4 = lane & 3, mt = warp & 3, half = warp >> 2;
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
     float E[DE], gE[DE];
@@ -226,10 +229,10 @@ __global__ void __launch_bounds__(256) mix_bwd2_kernel(const int* __restrict__ r
             const int4* src = reinterpret_cast<const int4*>(V + (size_t)eb * N * DV);
             int4* dst = reinterpret_cast<int4*>(Vt);
             for (int idx = tid; idx < cnt * N * DV / 4; idx += 256) dst[idx] = src[idx];
-            const float* g = G + (size_t)eb * N * DV;
-            for (int idx = tid; idx < cnt * N * DV; idx += 256) {
+            const float* gp = G + (size_t)eb * N * DV;
+            for (int idx = tid; idx < TE * N * DV; idx += 256) {
                 const int el = idx / (N * DV), rem = idx - el * (N * DV), np = rem / DV, k = rem - np * DV;
-                gS[(el * DV + k) * LDT + np] = g[idx];
+                gS[(el * DV + k) * LDT + np] = el < cnt ? gp[idx] : 0.f;   // zero rows beyond the ragged tail (they feed the MMA)
             }
         }
         __syncthreads();
@@ -240,25 +243,54 @@ __global__ void __launch_bounds__(256) mix_bwd2_kernel(const int* __restrict__ r
             for (int k = 0; k < DV; ++k) gv[q][k] = 0.f;
         for (int p = 0; p < P; ++p) {
             const int d3 = tab.d3[p], off3 = tab.off3[p];
-            float wc[N];  // W_p[n'][ch], n' = 0..N-1 (coalesced across ch)
+            {   // W_p: coalesced 128-bit global reads into shared memory (every warp finished the previous path's MMA
+                // before the "gtS complete" barrier below, so Ws is free)
+                const float4* w4 = reinterpret_cast<const float4*>(W + (size_t)p * N * N);
 #pragma unroll
-            for (int k = 0; k < N; ++k) wc[k] = W[((size_t)p * N + k) * N + ch];
-            float gt[EPT][M2::D3MAX];
-            auto gemm = [&](auto dc) {
-                constexpr int D3 = decltype(dc)::value;
-#pragma unroll
-                for (int q = 0; q < EPT; ++q) {
-                    float a[D3];
-#pragma unroll
-                    for (int M = 0; M < D3; ++M) a[M] = 0.f;
-                    dot_cols<N, D3>(wc, gS + ((eg * EPT + q) * DV + off3) * LDT, LDT, a);
-#pragma unroll
-                    for (int M = 0; M < D3; ++M) gt[q][M] = a[M];
+                for (int it = 0; it < N * N / 4 / 256; ++it) {
+                    const int idx = tid + it * 256, r = idx / (N / 4), c4 = idx - r * (N / 4);
+                    *reinterpret_cast<float4*>(Ws + r * LDT + 4 * c4) = w4[idx];
                 }
-            };
-            if (d3 == 1) gemm(std::integral_constant<int, 1>{});
-            else if (d3 == 3) gemm(std::integral_constant<int, 3>{});
-            else gemm(std::integral_constant<int, (L >= 2 ? 5 : 3)>{});
+            }
+            __syncthreads();  // Ws complete; every thread has consumed the previous path's gtS
+            {   // gt_p[n (64) x cols (TE * d3)] = W_p^T . G_p on the tensor cores (3xTF32)
+                uint32_t ahi[N / 8][4], alo[N / 8][4];
+#pragma unroll
+                for (int kt = 0; kt < N / 8; ++kt) {   // A[row = n][k = n'] = W_p[n'][n]
+                    const float* w0 = Ws + (kt * 8 + t4) * LDT + mt * 16 + g;
+                    split_tf32(w0[0], ahi[kt][0], alo[kt][0]);
+                    split_tf32(w0[8], ahi[kt][1], alo[kt][1]);
+                    split_tf32(w0[4 * LDT], ahi[kt][2], alo[kt][2]);
+                    split_tf32(w0[4 * LDT + 8], ahi[kt][3], alo[kt][3]);
+                }
+                auto tiles = [&](auto dc) {
+                    constexpr int D3 = decltype(dc)::value;
+                    constexpr int ntiles = TE * D3 / 8;
+                    for (int nt = half; nt < ntiles; nt += 2) {
+                        float dacc[4] = {0.f, 0.f, 0.f, 0.f};
+                        const int colb = nt * 8 + g, elb = colb / D3, Mb = colb - elb * D3;
+                        const float* bcol = gS + (elb * DV + off3 + Mb) * LDT + t4;
+#pragma unroll
+                        for (int kt = 0; kt < N / 8; ++kt) {
+                            uint32_t bh0, bl0, bh1, bl1;
+                            split_tf32(bcol[kt * 8], bh0, bl0);
+                            split_tf32(bcol[kt * 8 + 4], bh1, bl1);
+                            mma_tf32(dacc, alo[kt], bh0, bh1);
+                            mma_tf32(dacc, ahi[kt], bl0, bl1);
+                            mma_tf32(dacc, ahi[kt], bh0, bh1);
+                        }
+#pragma unroll
+                        for (int i = 0; i < 4; ++i) {
+                            const int col = nt * 8 + 2 * t4 + (i & 1), row = mt * 16 + g + ((i & 2) ? 8 : 0);
+                            gtS[col * LDT + row] = dacc[i];
+                        }
+                    }
+                };
+                if (d3 == 1) tiles(std::integral_constant<int, 1>{});
+                else if (d3 == 3) tiles(std::integral_constant<int, 3>{});
+                else tiles(std::integral_constant<int, (L >= 2 ? 5 : 3)>{});
+            }
+            __syncthreads();  // gtS complete
             static_for2<0, P>([&](auto pc) {   // per-path CG VJP: generated code selected by a compare chain
                 constexpr int pp = decltype(pc)::value;
                 if (p == pp) {
@@ -269,7 +301,7 @@ __global__ void __launch_bounds__(256) mix_bwd2_kernel(const int* __restrict__ r
                         if (el < cnt) {
                             float g3[Pth::D3];
 #pragma unroll
-                            for (int M = 0; M < Pth::D3; ++M) g3[M] = gt[q][M];
+                            for (int M = 0; M < Pth::D3; ++M) g3[M] = gtS[(el * Pth::D3 + M) * LDT + ch];
                             Pth::template bwd<float, WANT_GV>(Vt + ((size_t)el * N + ch) * DV, E, g3, gv[q], gE);
                         }
                     }
