@@ -167,18 +167,20 @@ __global__ void __launch_bounds__(256, 2) mix_fwd2_kernel(const int* __restrict_
                 constexpr int D3 = decltype(dc)::value;
                 constexpr int ntiles = TE * D3 / 8;
                 for (int nt = half; nt < ntiles; nt += 2) {
-                    float dacc[4] = {0.f, 0.f, 0.f, 0.f};
+                    float dacc[4] = {0.f, 0.f, 0.f, 0.f}, dlo[4] = {0.f, 0.f, 0.f, 0.f}, dmid[4] = {0.f, 0.f, 0.f, 0.f};
                     const float* bcol = buf + (nt * 8 + g) * LDT + t4;
 #pragma unroll
                     for (int kt = 0; kt < N / 8; ++kt) {
                         uint32_t bh0, bl0, bh1, bl1;
                         split_tf32(bcol[kt * 8], bh0, bl0);
                         split_tf32(bcol[kt * 8 + 4], bh1, bl1);
-                        mma_tf32(dacc, alo[kt], bh0, bh1);
-                        mma_tf32(dacc, ahi[kt], bl0, bl1);
+                        mma_tf32(dlo, alo[kt], bh0, bh1);   // three independent accumulation chains (the MMA latency, not its
+                        mma_tf32(dmid, ahi[kt], bl0, bl1);  // throughput, bounds a single chain of 24 dependent MMAs)
                         mma_tf32(dacc, ahi[kt], bh0, bh1);
                     }
                     // c0: (row g, col 2 t4), c1: (row g, col 2 t4 + 1), c2 / c3: row g + 8; col -> (edge, M) of this path
+#pragma unroll
+                    for (int i = 0; i < 4; ++i) dacc[i] += dlo[i] + dmid[i];
 #pragma unroll
                     for (int i = 0; i < 4; ++i) {
                         const int col = nt * 8 + 2 * t4 + (i & 1), row = mt * 16 + g + ((i & 2) ? 8 : 0);
@@ -267,7 +269,7 @@ __global__ void __launch_bounds__(256, 2) mix_bwd2_kernel(const int* __restrict_
                     constexpr int D3 = decltype(dc)::value;
                     constexpr int ntiles = TE * D3 / 8;
                     for (int nt = half; nt < ntiles; nt += 2) {
-                        float dacc[4] = {0.f, 0.f, 0.f, 0.f};
+                        float dacc[4] = {0.f, 0.f, 0.f, 0.f}, dlo[4] = {0.f, 0.f, 0.f, 0.f}, dmid[4] = {0.f, 0.f, 0.f, 0.f};
                         const int colb = nt * 8 + g, elb = colb / D3, Mb = colb - elb * D3;
                         const float* bcol = gS + (elb * DV + off3 + Mb) * LDT + t4;
 #pragma unroll
@@ -275,14 +277,14 @@ __global__ void __launch_bounds__(256, 2) mix_bwd2_kernel(const int* __restrict_
                             uint32_t bh0, bl0, bh1, bl1;
                             split_tf32(bcol[kt * 8], bh0, bl0);
                             split_tf32(bcol[kt * 8 + 4], bh1, bl1);
-                            mma_tf32(dacc, alo[kt], bh0, bh1);
-                            mma_tf32(dacc, ahi[kt], bl0, bl1);
+                            mma_tf32(dlo, alo[kt], bh0, bh1);   // three independent accumulation chains
+                            mma_tf32(dmid, ahi[kt], bl0, bl1);
                             mma_tf32(dacc, ahi[kt], bh0, bh1);
                         }
 #pragma unroll
                         for (int i = 0; i < 4; ++i) {
                             const int col = nt * 8 + 2 * t4 + (i & 1), row = mt * 16 + g + ((i & 2) ? 8 : 0);
-                            gtS[col * LDT + row] = dacc[i];
+                            gtS[col * LDT + row] = dacc[i] + (dlo[i] + dmid[i]);
                         }
                     }
                 };
