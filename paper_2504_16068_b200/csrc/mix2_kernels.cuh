@@ -18,53 +18,19 @@ __device__ __forceinline__ void static_for2(F&& f) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Version 2 (fp32, n = 32 or 64, l_max <= 2): tiles of TE = 4 * (256 / N) edges, t recomputed PER PATH so that only the
-// path's (2 l3 + 1) columns sit in shared memory, and the thread's W_p row (forward: W_p[n'][:], backward: W_p[:][n])
-// held in N registers for the whole tile: the inner product reads its other operand with broadcast 128-bit loads and
-// every weight element loaded from L2 is used for 4 edges x (2 l3 + 1) columns.
+// Tiles of 2 * (256 / N) edges; t is recomputed PER PATH so that only the path's (2 l3 + 1) columns sit in shared memory; W_p is
+// staged once per (tile, path) with coalesced 128-bit loads; the 64 x 64 x columns products run on the tensor cores.
 template <int L, int N>
 struct Mix2 {
     using Gen = TPGen<L>;
-    static constexpr int CT = 256, EG = CT / N, EPT = 4, TE = EG * EPT, DV = Gen::DV, DE = Gen::DE, P = Gen::P;
+    static constexpr int CT = 256, EG = CT / N, DV = Gen::DV, DE = Gen::DE, P = Gen::P;
     static constexpr int D3MAX = 2 * L + 1, LDT = N + 4;
-    static constexpr size_t kVt = (size_t)TE * N * DV * sizeof(float);
-    static constexpr int EPTF = 2, TEF = EG * EPTF;   // forward tile: 8 edges (n = 64) so that two CTAs fit one SM
+    static constexpr int EPTF = 2, TEF = EG * EPTF;   // tile: 8 edges (n = 64) so that two CTAs fit one SM
     static constexpr size_t kVtF = (size_t)TEF * N * DV * sizeof(float);
     static constexpr size_t kFwdSmem = 2 * kVtF + ((size_t)TEF * D3MAX + N) * LDT * sizeof(float);
     static constexpr size_t kBwdSmem = kVtF + ((size_t)TEF * DV + (size_t)TEF * D3MAX + N) * LDT * sizeof(float);
 };
 
-template <int N>
-__device__ __forceinline__ float dot_reg_smem(const float (&wr)[N], const float* __restrict__ col, float acc) {
-    const float4* c4 = reinterpret_cast<const float4*>(col);
-#pragma unroll
-    for (int k = 0; k < N / 4; ++k) {
-        const float4 c = c4[k];
-        acc = fmaf(wr[4 * k], c.x, acc);
-        acc = fmaf(wr[4 * k + 1], c.y, acc);
-        acc = fmaf(wr[4 * k + 2], c.z, acc);
-        acc = fmaf(wr[4 * k + 3], c.w, acc);
-    }
-    return acc;
-}
-
-// NC dot products at once against columns that are `stride` floats apart: NC independent accumulation chains
-template <int N, int NC>
-__device__ __forceinline__ void dot_cols(const float (&wr)[N], const float* __restrict__ col0, int stride, float (&acc)[NC]) {
-#pragma unroll
-    for (int k = 0; k < N / 4; ++k) {
-#pragma unroll
-        for (int m = 0; m < NC; ++m) {
-            const float4 c = *reinterpret_cast<const float4*>(col0 + m * stride + 4 * k);
-            float a = acc[m];
-            a = fmaf(wr[4 * k], c.x, a);
-            a = fmaf(wr[4 * k + 1], c.y, a);
-            a = fmaf(wr[4 * k + 2], c.z, a);
-            a = fmaf(wr[4 * k + 3], c.w, a);
-            acc[m] = a;
-        }
-    }
-}
 
 // 3xTF32 on the tensor cores (legacy mma.sync path; tcgen05 is the next step): x = hi + lo;
 // A.B ~= A_lo.B_hi + A_hi.B_lo + A_hi.B_hi keeps ~21 mantissa bits, enough for the 1e-5 fp32 tolerance (plain TF32 is not).
