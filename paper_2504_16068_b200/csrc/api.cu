@@ -67,7 +67,10 @@ allegro_status_t allegro_plan_create(int l_max, allegro_parity_t parity, int n_c
     *out = p;
     return ALLEGRO_OK;
 }
-void allegro_plan_destroy(allegro_plan_t* plan) { delete plan; }
+void allegro_plan_destroy(allegro_plan_t* plan) {
+    if (plan && plan->dense_img) cudaFree(plan->dense_img);
+    delete plan;
+}
 int allegro_plan_num_paths(const allegro_plan_t* plan) { return plan ? (int)plan->tab.paths.size() : -1; }
 int allegro_plan_dim_v(const allegro_plan_t* plan) { return plan ? plan->tab.dV : -1; }
 int allegro_plan_dim_e(const allegro_plan_t* plan) { return plan ? plan->tab.dE : -1; }

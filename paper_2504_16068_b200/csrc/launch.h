@@ -111,6 +111,9 @@ allegro_status_t launch_mix2_forward_f32_l2_n64(const TpArgs& a);
 allegro_status_t launch_mix2_backward_gv_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
 allegro_status_t launch_mix2_backward_nogv_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
 
+// dense per-path mix on tcgen05 (inst_mix3.cu)
+allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a);
+
 // dtype-only pieces of the two-layer model (model.cu)
 template <typename T>
 allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st);

@@ -192,7 +192,8 @@ static allegro_status_t launch_mix_forward(const TpArgs& a) {
     }
 #if ALLEGRO_L == 2
     if constexpr (sizeof(T) == 4) {
-        if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr) return launch_mix2_forward_f32_l2_n64(a);
+        if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr)
+            return getenv("ALLEGRO_MIX_V2") ? launch_mix2_forward_f32_l2_n64(a) : launch_mix3_forward_f32_l2_n64(a);
     }
 #endif
     const size_t ws_bytes = (size_t)a.n * (a.n + VEC) * sizeof(T);

@@ -34,5 +34,6 @@ long build_segments(const int32_t* row_ptr, int n_atoms, int tile_edges, int32_t
 struct allegro_plan {
     int l_max, n, dtype, wmode;
     allegro::PlanTables tab;
+    mutable void* dense_img = nullptr;  // device: weight images of the tcgen05 dense mix (inst_mix3.cu), plan-owned
     // order in which the generated kernels index the folded coefficient table (== tab.nnz order)
 };
