@@ -32,8 +32,8 @@ __device__ __forceinline__ void static_for3(F&& f) {
 
 struct Mix3 {
     static constexpr int N = 64, L = 2, DV = 18, DE = 9, P = 30;
-    static constexpr int TE = 24, NSLOT = 8, EPS = 3;            // tile edges = 8 slots x 3 edges
-    static constexpr int CT = 512;                                // compute threads (16 warps); + 1 control warp
+    static constexpr int TE = 24, NSLOT = 6, EPS = 4;            // tile edges = 6 slots x 4 consecutive edges
+    static constexpr int CT = 384;                                // compute threads (12 warps, 128 registers each); + 1 control warp
     static constexpr int A_BYTES = 2 * 128 * 128;                 // [2 K-atoms][128 rows][128 B]
     static constexpr int BV_BYTES = 2 * 128 * 128;                // one B variant (hi or lo): [2 K-atoms][<=128 rows][128 B]
     static constexpr int B_BYTES = 2 * BV_BYTES;
@@ -44,6 +44,11 @@ struct Mix3 {
     // TMEM column base of each output block, indexed by off3 (0e:0, 0o:1, 1e:2, 1o:5, 2e:8, 2o:13); N_b = 32 / 80 / 128
     __host__ __device__ static constexpr int dcol(int off3) {
         return off3 == 0 ? 0 : off3 == 1 ? 32 : off3 == 2 ? 64 : off3 == 5 ? 144 : off3 == 8 ? 224 : 352;
+    }
+    // is p the first path (in plan order) that mixes into its output block?
+    __host__ __device__ static constexpr bool first_of_block(int p) {
+        for (int r = 0; r < p; ++r) if (TPGen<2>::off3(r) == TPGen<2>::off3(p)) return false;
+        return true;
     }
     __host__ __device__ static constexpr int ncols(int d3) { return d3 == 1 ? 32 : d3 == 3 ? 80 : 128; }
 };
@@ -79,7 +84,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
     using Gen = TPGen<2>;
     constexpr int DV = M3::DV, DE = M3::DE, P = M3::P, TE = M3::TE;
     extern __shared__ unsigned char smem_raw[];
-    unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~(uintptr_t)1023);
+    unsigned char* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned (128-byte swizzle atoms)
     Mix3Bars* bars = reinterpret_cast<Mix3Bars*>(sm + M3::OFF_BAR);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int c, e0, e1;
@@ -122,33 +127,35 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
             constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 32);
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 128);
-            const uint32_t a0 = smem_u32(sm + M3::OFF_A), b0 = smem_u32(sm + M3::OFF_B);
+            // descriptors of K step 0 of every ring stage; K step j adds (j >> 2) * 16384 + (j & 3) * 32 bytes (16-byte units)
+            uint64_t adesc[M3::NA], bdesc[M3::NB];
+#pragma unroll
+            for (int s = 0; s < M3::NA; ++s) adesc[s] = tc05::sdesc_sw128(smem_u32(sm + M3::OFF_A + s * M3::A_BYTES));
+#pragma unroll
+            for (int s = 0; s < M3::NB; ++s) bdesc[s] = tc05::sdesc_sw128(smem_u32(sm + M3::OFF_B + s * M3::B_BYTES));
             for (int t = 0; t < ntiles; ++t) {
                 if (t > 0) { mbar_wait(&bars->d_empty, (uint32_t)(t - 1) & 1u); tc05::fence_after_sync(); }
-                uint32_t seen = 0;   // bit off3 set once the block's accumulator has been initialised in this tile
-                for (int p = 0; p < P; ++p) {
-                    const int sa = p % M3::NA, sb = p & 1;
+                static_for3<0, P>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int sa = p % M3::NA, sb = p & 1;
+                    constexpr int d3 = Gen::d3(p), off3 = Gen::off3(p);
+                    constexpr uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
+                    constexpr bool first = M3::first_of_block(p);   // first path of its output block: initialises the accumulator
                     const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;          // 15 B-ring turns per tile
                     mbar_wait(&bars->b_full[sb], phb);
                     tc05::fence_after_sync();
-                    const int d3 = Gen::d3(p), off3 = Gen::off3(p);
-                    const uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
                     const uint32_t dcol = tbase + (uint32_t)M3::dcol(off3);
-                    uint32_t acc = (seen >> off3) & 1u;
-                    seen |= 1u << off3;
-                    const uint32_t abase = a0 + sa * M3::A_BYTES, bbase = b0 + sb * M3::B_BYTES;
 #pragma unroll
                     for (int v = 0; v < 2; ++v)          // B variant: hi, lo
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {    // K step of 8 channels
-                            const uint64_t ad = tc05::sdesc_sw128(abase + (j >> 2) * 16384 + (j & 3) * 32);
-                            const uint64_t bd = tc05::sdesc_sw128(bbase + v * M3::BV_BYTES + (j >> 2) * 16384 + (j & 3) * 32);
-                            tc05::mma_tf32(dcol, ad, bd, idesc, acc);
-                            acc = 1u;
+                            const uint64_t koff = (uint64_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
+                            tc05::mma_tf32(dcol, adesc[sa] + koff, bdesc[sb] + (uint64_t)((v * M3::BV_BYTES) >> 4) + koff, idesc,
+                                           (first && v == 0 && j == 0) ? 0u : 1u);
                         }
                     tc05::mma_commit(&bars->b_empty[sb]);
                     tc05::mma_commit(&bars->a_empty[sa]);
-                }
+                });
                 tc05::mma_commit(&bars->d_full);
             }
         }
@@ -158,15 +165,22 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
         float E[DE];
 #pragma unroll
         for (int j = 0; j < DE; ++j) E[j] = Eenv[((size_t)c * 64 + ch) * DE + j];
-        // byte offset of this thread's element inside a B variant, for row group 0: rows are columns (M, e) = M * 24 + 8 i + slot
-        const uint32_t boff = (uint32_t)(ch >> 5) * 16384u + (uint32_t)slot * 128u + (uint32_t)((((ch & 31) >> 2) ^ slot) << 4) + (uint32_t)((ch & 3) << 2);
+        // B rows are the columns (M, e) = M * 24 + e of the problem; this thread writes element (row, k = ch) for its four edges
+        // e = 4 slot + j.  Byte offset inside a B variant for M = 0: row group (e >> 3) * 1024 + (e & 7) * 128, the 16-byte chunk
+        // (ch & 31) >> 2 swizzled with (e & 7); M adds 3 row groups (24 rows).
+        uint32_t boff[M3::EPS];
+#pragma unroll
+        for (int j = 0; j < M3::EPS; ++j) {
+            const uint32_t e = 4u * slot + j, r = e & 7u;
+            boff[j] = (uint32_t)(ch >> 5) * 16384u + (e >> 3) * 1024u + r * 128u + (((((uint32_t)ch & 31u) >> 2) ^ r) << 4) + (((uint32_t)ch & 3u) << 2);
+        }
         const int q = warp & 3, wq = warp >> 2, h = lane >> 4, nl = lane & 15;
         for (int t = 0; t < ntiles; ++t) {
             const int eb = e0 + t * TE;
             float Vr[M3::EPS][DV];
 #pragma unroll
             for (int i = 0; i < M3::EPS; ++i) {
-                const int e = eb + 8 * i + slot;
+                const int e = eb + 4 * slot + i;
                 if (e < e1) {
                     row_load<float, DV>(V + ((size_t)e * 64 + ch) * DV, Vr[i]);
                 } else {
@@ -185,8 +199,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                 // A lo rows: W - tf32(W), two 16-byte chunks per thread (hi rows arrived by TMA)
                 mbar_wait(&bars->a_full[sa], pha);
 #pragma unroll
-                for (int r = 0; r < 2; ++r) {
-                    const int cid = tid + r * M3::CT;
+                for (int cid = tid; cid < 1024; cid += M3::CT) {
                     unsigned char* src = As + (cid >> 9) * 16384 + ((cid >> 7) & 3) * 4096 + (cid & 127) * 16;
                     float4 w = *reinterpret_cast<const float4*>(src);
                     w.x = tf32_lo(w.x); w.y = tf32_lo(w.y); w.z = tf32_lo(w.z); w.w = tf32_lo(w.w);
@@ -194,13 +207,16 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                 }
                 // B: t_p of this thread's three edges, hi (raw) and lo
                 mbar_wait(&bars->b_empty[sb], phb ^ 1u);
+                // launder E so that V.E products are not kept alive (common subexpressions) from one path to the next
+#pragma unroll
+                for (int j = 0; j < DE; ++j) asm volatile("" : "+f"(E[j]));
 #pragma unroll
                 for (int i = 0; i < M3::EPS; ++i) {
                     float tp[Pth::D3];
                     Pth::template fwd<float>(Vr[i], E, tp);
 #pragma unroll
                     for (int M = 0; M < Pth::D3; ++M) {
-                        unsigned char* dst = Bs + boff + (3 * M + i) * 1024;
+                        unsigned char* dst = Bs + boff[i] + 3 * M * 1024;
                         *reinterpret_cast<float*>(dst) = tp[M];
                         *reinterpret_cast<float*>(dst + M3::BV_BYTES) = tf32_lo(tp[M]);
                     }
@@ -209,11 +225,11 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&bars->b_full[sb]);
             });
-            // ---- epilogue: TMEM lane (n', h) -> out rows; warp (q, wq) takes edges 6 wq .. 6 wq + 5, lane h its half of them
+            // ---- epilogue: TMEM lane (n', h) -> out rows; warp (q, wq) takes edges 8 wq .. 8 wq + 7, lane h its half of them
             mbar_wait(&bars->d_full, (uint32_t)t & 1u);
             tc05::fence_after_sync();
-            float o[3][DV];
-            const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(6 * wq);
+            float o[4][DV];
+            const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(8 * wq);
             static_for3<0, 6>([&](auto bc) {
                 constexpr int b = decltype(bc)::value;
                 constexpr int off3 = b == 0 ? 0 : b == 1 ? 1 : b == 2 ? 2 : b == 3 ? 5 : b == 4 ? 8 : 13;
@@ -224,9 +240,9 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                     tc05::tmem_ld8(trow + (uint32_t)(M3::dcol(off3) + M * TE), v);
                     tc05::tmem_ld_wait();
 #pragma unroll
-                    for (int i = 0; i < 3; ++i) {
-                        const float mine = __uint_as_float(h ? v[3 + i] : v[i]);
-                        const float send = __uint_as_float(h ? v[i] : v[3 + i]);
+                    for (int i = 0; i < 4; ++i) {
+                        const float mine = __uint_as_float(h ? v[4 + i] : v[i]);
+                        const float send = __uint_as_float(h ? v[i] : v[4 + i]);
                         o[i][off3 + M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
                     }
                 }
@@ -235,8 +251,8 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars->d_empty);
 #pragma unroll
-            for (int i = 0; i < 3; ++i) {
-                const int e = eb + 6 * wq + 3 * h + i;
+            for (int i = 0; i < 4; ++i) {
+                const int e = eb + 8 * wq + 4 * h + i;
                 if (e < e1) row_store<float, DV>(out + ((size_t)e * 64 + 16 * q + nl) * DV, o[i]);
             }
         }
