@@ -20,6 +20,14 @@
 #include "launch.h"
 #include "tc05.cuh"
 
+#ifdef MIX3_DBG
+#define MIX3_T0() long long dbg_t0 = clock64()
+#define MIX3_ACC(slot, cond) do { const long long dbg_t1 = clock64(); if (cond) mix3_dbg[slot] += dbg_t1 - dbg_t0; dbg_t0 = dbg_t1; } while (0)
+#else
+#define MIX3_T0() do { } while (0)
+#define MIX3_ACC(slot, cond) do { } while (0)
+#endif
+
 namespace allegro {
 
 template <int I, int N, typename F>
@@ -112,7 +120,9 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                 for (int p = 0; p < P; ++p) {
                     const int sa = p % M3::NA;                                   // 30 paths per tile = 10 ring turns: stage and
                     const uint32_t ph = (uint32_t)(p / M3::NA) & 1u;             // parity depend on p only
+                    MIX3_T0();
                     mbar_wait(&bars->a_empty[sa], ph ^ 1u);
+                    MIX3_ACC(3, blockIdx.x == 0);
                     mbar_expect_tx(&bars->a_full[sa], M3::IMG_BYTES);
                     unsigned char* dstA = sm + M3::OFF_A + sa * M3::A_BYTES;
                     const unsigned char* src = reinterpret_cast<const unsigned char*>(img) + (size_t)p * M3::IMG_BYTES;
@@ -134,7 +144,9 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
 #pragma unroll
             for (int s = 0; s < M3::NB; ++s) bdesc[s] = tc05::sdesc_sw128(smem_u32(sm + M3::OFF_B + s * M3::B_BYTES));
             for (int t = 0; t < ntiles; ++t) {
+                MIX3_T0();
                 if (t > 0) { mbar_wait(&bars->d_empty, (uint32_t)(t - 1) & 1u); tc05::fence_after_sync(); }
+                MIX3_ACC(2, blockIdx.x == 0);
                 static_for3<0, P>([&](auto pc) {
                     constexpr int p = decltype(pc)::value;
                     constexpr int sa = p % M3::NA, sb = p & 1;
@@ -143,6 +155,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                     constexpr bool first = M3::first_of_block(p);   // first path of its output block: initialises the accumulator
                     const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;          // 15 B-ring turns per tile
                     mbar_wait(&bars->b_full[sb], phb);
+                    MIX3_ACC(0, blockIdx.x == 0);
                     tc05::fence_after_sync();
                     const uint32_t dcol = tbase + (uint32_t)M3::dcol(off3);
 #pragma unroll
@@ -155,6 +168,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                         }
                     tc05::mma_commit(&bars->b_empty[sb]);
                     tc05::mma_commit(&bars->a_empty[sa]);
+                    MIX3_ACC(1, blockIdx.x == 0);
                 });
                 tc05::mma_commit(&bars->d_full);
             }
@@ -177,6 +191,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
         const int q = warp & 3, wq = warp >> 2, h = lane >> 4, nl = lane & 15;
         for (int t = 0; t < ntiles; ++t) {
             const int eb = e0 + t * TE;
+            MIX3_T0();
             float Vr[M3::EPS][DV];
 #pragma unroll
             for (int i = 0; i < M3::EPS; ++i) {
@@ -196,17 +211,11 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                 const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;
                 unsigned char* As = sm + M3::OFF_A + sa * M3::A_BYTES;
                 unsigned char* Bs = sm + M3::OFF_B + sb * M3::B_BYTES;
-                // A lo rows: W - tf32(W), two 16-byte chunks per thread (hi rows arrived by TMA)
-                mbar_wait(&bars->a_full[sa], pha);
-#pragma unroll
-                for (int cid = tid; cid < 1024; cid += M3::CT) {
-                    unsigned char* src = As + (cid >> 9) * 16384 + ((cid >> 7) & 3) * 4096 + (cid & 127) * 16;
-                    float4 w = *reinterpret_cast<const float4*>(src);
-                    w.x = tf32_lo(w.x); w.y = tf32_lo(w.y); w.z = tf32_lo(w.z); w.w = tf32_lo(w.w);
-                    *reinterpret_cast<float4*>(src + 2048) = w;
-                }
                 // B: t_p of this thread's three edges, hi (raw) and lo
+                MIX3_ACC(10, blockIdx.x == 0 && tid == 0 && p == 0);
                 mbar_wait(&bars->b_empty[sb], phb ^ 1u);
+                if (p == 1 && t > 0) asm volatile("bar.sync 1, %0;" ::"n"(2 * M3::CT) : "memory");
+                MIX3_ACC(4, blockIdx.x == 0 && tid == 0);
                 // launder E so that V.E products are not kept alive (common subexpressions) from one path to the next
 #pragma unroll
                 for (int j = 0; j < DE; ++j) asm volatile("" : "+f"(E[j]));
@@ -221,40 +230,69 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                         *reinterpret_cast<float*>(dst + M3::BV_BYTES) = tf32_lo(tp[M]);
                     }
                 }
+                // A lo rows: W - tf32(W) (hi rows arrive by TMA; waited for after the B work so that the copy's latency is covered)
+                MIX3_ACC(5, blockIdx.x == 0 && tid == 0);
+                mbar_wait(&bars->a_full[sa], pha);
+                MIX3_ACC(6, blockIdx.x == 0 && tid == 0);
+#pragma unroll
+                for (int cid = tid; cid < 1024; cid += M3::CT) {
+                    unsigned char* src = As + (cid >> 9) * 16384 + ((cid >> 7) & 3) * 4096 + (cid & 127) * 16;
+                    float4 w = *reinterpret_cast<const float4*>(src);
+                    w.x = tf32_lo(w.x); w.y = tf32_lo(w.y); w.z = tf32_lo(w.z); w.w = tf32_lo(w.w);
+                    *reinterpret_cast<float4*>(src + 2048) = w;
+                }
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&bars->b_full[sb]);
+                MIX3_ACC(7, blockIdx.x == 0 && tid == 0);
             });
             // ---- epilogue: TMEM lane (n', h) -> out rows; warp (q, wq) takes edges 8 wq .. 8 wq + 7, lane h its half of them
             mbar_wait(&bars->d_full, (uint32_t)t & 1u);
+            MIX3_ACC(8, blockIdx.x == 0 && tid == 0);
             tc05::fence_after_sync();
-            float o[4][DV];
+            // Rows are staged through shared memory (B stage 1 is idle until path 1 of the next tile) so that they leave as
+            // fully coalesced 16-byte stores: per warp a private [4 edges][16 channels][18] block, two half-tiles in turn.
+            float* stg = reinterpret_cast<float*>(sm + M3::OFF_B + M3::B_BYTES) + warp * (4 * 16 * DV);
             const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(8 * wq);
-            static_for3<0, 6>([&](auto bc) {
-                constexpr int b = decltype(bc)::value;
-                constexpr int off3 = b == 0 ? 0 : b == 1 ? 1 : b == 2 ? 2 : b == 3 ? 5 : b == 4 ? 8 : 13;
-                constexpr int d3 = b < 2 ? 1 : b < 4 ? 3 : 5;
 #pragma unroll
-                for (int M = 0; M < d3; ++M) {
-                    uint32_t v[8];
-                    tc05::tmem_ld8(trow + (uint32_t)(M3::dcol(off3) + M * TE), v);
+            for (int hf = 0; hf < 2; ++hf) {     // edges 8 wq + 4 hf + {0..3}: lane half h finalises edges 2 h, 2 h + 1 of them
+                float o[2][DV];
+                static_for3<0, 6>([&](auto bc) {
+                    constexpr int b = decltype(bc)::value;
+                    constexpr int off3 = b == 0 ? 0 : b == 1 ? 1 : b == 2 ? 2 : b == 3 ? 5 : b == 4 ? 8 : 13;
+                    constexpr int d3 = b < 2 ? 1 : b < 4 ? 3 : 5;
+                    uint32_t v[d3][4];
+#pragma unroll
+                    for (int M = 0; M < d3; ++M) tc05::tmem_ld4(trow + (uint32_t)(M3::dcol(off3) + M * TE + 4 * hf), v[M]);
                     tc05::tmem_ld_wait();
 #pragma unroll
-                    for (int i = 0; i < 4; ++i) {
-                        const float mine = __uint_as_float(h ? v[4 + i] : v[i]);
-                        const float send = __uint_as_float(h ? v[i] : v[4 + i]);
-                        o[i][off3 + M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
-                    }
-                }
-            });
-            tc05::fence_before_sync();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bars->d_empty);
+                    for (int M = 0; M < d3; ++M)
 #pragma unroll
-            for (int i = 0; i < 4; ++i) {
-                const int e = eb + 8 * wq + 4 * h + i;
-                if (e < e1) row_store<float, DV>(out + ((size_t)e * 64 + 16 * q + nl) * DV, o[i]);
+                        for (int i = 0; i < 2; ++i) {
+                            const float mine = __uint_as_float(h ? v[M][2 + i] : v[M][i]);
+                            const float send = __uint_as_float(h ? v[M][i] : v[M][2 + i]);
+                            o[i][off3 + M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
+                        }
+                });
+                if (hf == 1) {   // all TMEM reads of this warp are done: the accumulators may be overwritten
+                    tc05::fence_before_sync();
+                    __syncwarp();
+                    if (lane == 0) mbar_arrive(&bars->d_empty);
+                }
+#pragma unroll
+                for (int i = 0; i < 2; ++i) row_store<float, DV>(stg + ((2 * h + i) * 16 + nl) * DV, o[i]);
+                __syncwarp();
+                const int ebase = eb + 8 * wq + 4 * hf;
+#pragma unroll
+                for (int r = 0; r < 9; ++r) {    // 4 edges x 288 floats = 288 float4
+                    const int idx = lane + 32 * r, el = idx / 72, w4 = idx - el * 72;
+                    if (ebase + el < e1)
+                        *reinterpret_cast<float4*>(out + ((size_t)(ebase + el) * 64 + 16 * q) * DV + 4 * w4) = reinterpret_cast<const float4*>(stg)[idx];
+                }
+                __syncwarp();
             }
+            asm volatile("bar.arrive 1, %0;" ::"n"(2 * M3::CT) : "memory");   // staging done; waited for before B stage 1 is rewritten
+            MIX3_ACC(9, blockIdx.x == 0 && tid == 0);
         }
     }
     tc05::fence_before_sync();
