@@ -38,6 +38,25 @@ allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a) {
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
+#else
+allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item) {
+    float *img_f, *img_b;
+    allegro_status_t s = mix3_images(a, &img_f, &img_b);
+    if (s != ALLEGRO_OK) return s;
+    if (a.gV) {
+        auto k = mix3_bwd_kernel<true>;
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
+        k<<<(unsigned)a.n_items, Mix3B::CT + 32, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
+                                                                    img_b, (float*)a.gV, gE_dst, gE_by_item);
+    } else {
+        auto k = mix3_bwd_kernel<false>;
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
+        k<<<(unsigned)a.n_items, Mix3B::CT + 32, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
+                                                                    img_b, nullptr, gE_dst, gE_by_item);
+    }
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
 #endif
 
 }  // namespace allegro

@@ -113,6 +113,7 @@ allegro_status_t launch_mix2_backward_nogv_f32_l2_n64(const TpArgs& a, float* gE
 
 // dense per-path mix on tcgen05 (inst_mix3.cu)
 allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a);
+allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
 
 // dtype-only pieces of the two-layer model (model.cu)
 template <typename T>

@@ -64,7 +64,7 @@ struct Mix3 {
 // Weight images: img_f[p] feeds the forward (A row = output channel n', K = input channel n), img_b[p] the VJP
 // (A row = input channel n, K = output channel n').  Layout [K-atom a][quarter q][row nl][128 B], 16-byte chunk c of a row
 // stored at chunk position c ^ (nl & 7): the bytes land in the "hi" rows of the swizzled A tile by plain bulk copies.
-__global__ void mix3_prep_kernel(const float* __restrict__ W, float* __restrict__ img_f, float* __restrict__ img_b) {
+static __global__ void mix3_prep_kernel(const float* __restrict__ W, float* __restrict__ img_f, float* __restrict__ img_b) {
     const int p = blockIdx.x;
     const float* Wp = W + (size_t)p * 64 * 64;
     for (int idx = threadIdx.x; idx < 64 * 64; idx += blockDim.x) {
@@ -298,6 +298,248 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
     tc05::fence_before_sync();
     __syncthreads();
     if (warp == M3::CT / 32) tc05::tmem_dealloc(tbase, 512);
+}
+
+
+// =====================================================================================================================
+// VJP.  gt_p[e, n, M] = sum_n' W_p[n', n] G[e, n', off3(p) + M] on the tensor cores, then the per-path CG VJP on the CUDA cores:
+//   D_p[128 x N_b] = A_p[128 x 64] . B_b[N_b x 64]^T,   A_p rows = (input channel n, hi/lo) from the transposed weight image,
+//   B_b rows = column (M, e) of block b: G[e, :, off3 + M] over the 64 output channels (K), hi and lo.
+// All six blocks' B operands of a tile of TE = 16 edges stay in shared memory (the cotangent tile transposed once), the paths run
+// in plan order, every D_p goes TMEM -> registers as soon as it is complete (ring of four accumulators), V rows and the gV rows
+// of the thread's four (edge, channel) pairs live in registers for the whole tile.
+struct Mix3B {
+    static constexpr int DV = 18, DE = 9, P = 30;
+    static constexpr int TE = 16, CT = 256;                        // 8 compute warps (<= 168 registers each) + 1 control warp
+    static constexpr int ROWS = 288;                                // sum over blocks of d3 * TE
+    static constexpr int G_ATOM = ROWS * 128, G_VAR = 2 * G_ATOM, G_BYTES = 2 * G_VAR;   // hi, lo: [2 K-atoms][288 rows][128 B]
+    static constexpr int A_BYTES = 2 * 128 * 128, NA = 2, ND = 4;
+    static constexpr int OFF_G = 0, OFF_A = G_BYTES, OFF_BAR = OFF_A + NA * A_BYTES;
+    static constexpr int SMEM = OFF_BAR + 256 + 1024;
+    // first row of a block's B operand, indexed by off3
+    __host__ __device__ static constexpr int rowoff(int off3) {
+        return off3 == 0 ? 0 : off3 == 1 ? 16 : off3 == 2 ? 32 : off3 == 5 ? 80 : off3 == 8 ? 128 : 208;
+    }
+    // component k of a feature row -> row of the (M = 0, e = 0) element of its block + 16 M
+    __host__ __device__ static constexpr int comprow(int k) {
+        return k == 0 ? 0 : k == 1 ? 16 : k < 5 ? 32 + 16 * (k - 2) : k < 8 ? 80 + 16 * (k - 5) : k < 13 ? 128 + 16 * (k - 8) : 208 + 16 * (k - 13);
+    }
+};
+struct Mix3BBars {
+    uint64_t a_full[Mix3B::NA], a_conv[Mix3B::NA], a_empty[Mix3B::NA], d_full[Mix3B::ND], d_empty[Mix3B::ND], g_full;
+    uint32_t tmem_slot;
+};
+
+template <bool WANT_GV>
+__global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
+                                                                    const float* __restrict__ G, const float* __restrict__ V,
+                                                                    const float* __restrict__ Eenv, const float* __restrict__ img,
+                                                                    float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
+    using MB = Mix3B;
+    using Gen = TPGen<2>;
+    constexpr int DV = MB::DV, DE = MB::DE, P = MB::P, TE = MB::TE;
+    extern __shared__ unsigned char smem_raw[];
+    unsigned char* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+    Mix3BBars* bars = reinterpret_cast<Mix3BBars*>(sm + MB::OFF_BAR);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    const int ntiles = (e1 - e0 + TE - 1) / TE;   // 0 for an empty item: only the zero gEenv row is written
+
+    if (tid == 0) {
+        for (int s = 0; s < MB::NA; ++s) { mbar_init(&bars->a_full[s], 1); mbar_init(&bars->a_conv[s], MB::CT / 32); mbar_init(&bars->a_empty[s], 1); }
+        for (int s = 0; s < MB::ND; ++s) { mbar_init(&bars->d_full[s], 1); mbar_init(&bars->d_empty[s], MB::CT / 32); }
+        mbar_init(&bars->g_full, MB::CT / 32);
+        fence_mbar_init();
+    }
+    if (warp == MB::CT / 32) { tc05::tmem_alloc(&bars->tmem_slot, 512); tc05::tmem_relinquish(); }
+    tc05::fence_before_sync();
+    __syncthreads();
+    tc05::fence_after_sync();
+    const uint32_t tbase = bars->tmem_slot;
+
+    if (warp == MB::CT / 32) {
+        if (lane == 0) {
+            // ---- weight images (TMA)
+            for (int t = 0; t < ntiles; ++t)
+                for (int p = 0; p < P; ++p) {
+                    const int sa = p & 1;
+                    const uint32_t ph = (uint32_t)(t + (p >> 1)) & 1u;            // 15 ring turns per tile
+                    mbar_wait(&bars->a_empty[sa], ph ^ 1u);
+                    mbar_expect_tx(&bars->a_full[sa], Mix3::IMG_BYTES);
+                    unsigned char* dstA = sm + MB::OFF_A + sa * MB::A_BYTES;
+                    const unsigned char* src = reinterpret_cast<const unsigned char*>(img) + (size_t)p * Mix3::IMG_BYTES;
+#pragma unroll
+                    for (int a = 0; a < 2; ++a)
+#pragma unroll
+                        for (int q = 0; q < 4; ++q) bulk_load(dstA + a * 16384 + q * 4096, src + (a * 4 + q) * 2048, 2048, &bars->a_full[sa]);
+                }
+        } else if (lane == 1) {
+            // ---- MMA issue
+            constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 16);
+            constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 48);
+            constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
+            uint64_t adesc[MB::NA];
+#pragma unroll
+            for (int s = 0; s < MB::NA; ++s) adesc[s] = tc05::sdesc_sw128(smem_u32(sm + MB::OFF_A + s * MB::A_BYTES));
+            const uint64_t gdesc = tc05::sdesc_sw128(smem_u32(sm + MB::OFF_G));
+            for (int t = 0; t < ntiles; ++t) {
+                mbar_wait(&bars->g_full, (uint32_t)t & 1u);
+                static_for3<0, P>([&](auto pc) {
+                    constexpr int p = decltype(pc)::value;
+                    constexpr int sa = p & 1;
+                    constexpr int d3 = Gen::d3(p), off3 = Gen::off3(p);
+                    constexpr uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
+                    const uint32_t g = (uint32_t)(t * P + p), sd = g & 3u;
+                    mbar_wait(&bars->a_conv[sa], (uint32_t)(t + (p >> 1)) & 1u);
+                    mbar_wait(&bars->d_empty[sd], ((g >> 2) & 1u) ^ 1u);
+                    tc05::fence_after_sync();
+                    const uint32_t dcol = tbase + sd * 128u;
+#pragma unroll
+                    for (int v = 0; v < 2; ++v)
+#pragma unroll
+                        for (int j = 0; j < 8; ++j) {
+                            const uint64_t koff = (uint64_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
+                            const uint64_t goff = (uint64_t)((v * MB::G_VAR + (j >> 2) * MB::G_ATOM + MB::rowoff(off3) * 128 + (j & 3) * 32) >> 4);
+                            tc05::mma_tf32(dcol, adesc[sa] + koff, gdesc + goff, idesc, (v == 0 && j == 0) ? 0u : 1u);
+                        }
+                    tc05::mma_commit(&bars->d_full[sd]);
+                    tc05::mma_commit(&bars->a_empty[sa]);
+                });
+            }
+        }
+    } else {
+        // ---- compute warps.  VJP mapping = TMEM lane: channel n = 16 q + nl, hi/lo partner lane ^ 16; warp (q, wq) reads the columns
+        // of edges 8 wq .. 8 wq + 7, lane half h finalises edges 8 wq + 4 h + {0..3}.
+        const int q = warp & 3, wq = warp >> 2, h = lane >> 4, nl = lane & 15, n = 16 * q + nl;
+        float E[DE], gE[DE];
+#pragma unroll
+        for (int j = 0; j < DE; ++j) { E[j] = Eenv[((size_t)c * 64 + n) * DE + j]; gE[j] = 0.f; }
+        // operand mapping: thread = (slot, n'), rows of edges 4 slot + j; byte offset of element (row of e, k = n') for M = 0, block row 0
+        const int np = tid & 63, slot = tid >> 6;
+        uint32_t goff[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) {
+            const uint32_t e = 4u * slot + j, r = e & 7u;
+            goff[j] = (uint32_t)(np >> 5) * MB::G_ATOM + (e >> 3) * 1024u + r * 128u + (((((uint32_t)np & 31u) >> 2) ^ r) << 4) + (((uint32_t)np & 3u) << 2);
+        }
+        for (int t = 0; t < ntiles; ++t) {
+            const int eb = e0 + t * TE;
+            // (a) cotangent tile -> B operands of all six blocks (hi, lo)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) {
+                const int e = eb + 4 * slot + j;
+                float g[DV];
+                if (e < e1) {
+                    row_load<float, DV>(G + ((size_t)e * 64 + np) * DV, g);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < DV; ++k) g[k] = 0.f;
+                }
+#pragma unroll
+                for (int k = 0; k < DV; ++k) {
+                    unsigned char* dst = sm + MB::OFF_G + goff[j] + (MB::comprow(k) / 8) * 1024;
+                    *reinterpret_cast<float*>(dst) = g[k];
+                    *reinterpret_cast<float*>(dst + MB::G_VAR) = tf32_lo(g[k]);
+                }
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars->g_full);
+            // (b) V rows of this thread's pairs; gV accumulators
+            float Vr[4][DV], gv[4][DV];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                const int e = eb + 8 * wq + 4 * h + i;
+                if (e < e1) {
+                    row_load<float, DV>(V + ((size_t)e * 64 + n) * DV, Vr[i]);
+                } else {
+#pragma unroll
+                    for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
+                }
+#pragma unroll
+                for (int k = 0; k < DV; ++k) gv[i][k] = 0.f;
+            }
+            // (c) paths: convert the next weight image's lo rows, then consume the accumulator of this path
+            auto convert = [&](int sa, uint32_t ph) {
+                unsigned char* As = sm + MB::OFF_A + sa * MB::A_BYTES;
+                mbar_wait(&bars->a_full[sa], ph);
+#pragma unroll
+                for (int cid = tid; cid < 1024; cid += MB::CT) {
+                    unsigned char* src = As + (cid >> 9) * 16384 + ((cid >> 7) & 3) * 4096 + (cid & 127) * 16;
+                    float4 w = *reinterpret_cast<const float4*>(src);
+                    w.x = tf32_lo(w.x); w.y = tf32_lo(w.y); w.z = tf32_lo(w.z); w.w = tf32_lo(w.w);
+                    *reinterpret_cast<float4*>(src + 2048) = w;
+                }
+                fence_proxy_async();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars->a_conv[sa]);
+            };
+            convert(0, (uint32_t)t & 1u);
+            static_for3<0, P>([&](auto pc) {
+                constexpr int p = decltype(pc)::value;
+                using Pth = TPPath<2, p>;
+                constexpr int d3 = Pth::D3;
+                if (p + 1 < P) convert((p + 1) & 1, (uint32_t)(t + ((p + 1) >> 1)) & 1u);
+                const uint32_t g = (uint32_t)(t * P + p), sd = g & 3u;
+                mbar_wait(&bars->d_full[sd], (g >> 2) & 1u);
+                tc05::fence_after_sync();
+                uint32_t v[d3][8];
+                const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + sd * 128u + (uint32_t)(8 * wq);
+#pragma unroll
+                for (int M = 0; M < d3; ++M) tc05::tmem_ld8(trow + (uint32_t)(M * TE), v[M]);
+                tc05::tmem_ld_wait();
+                tc05::fence_before_sync();
+                __syncwarp();
+                if (lane == 0) mbar_arrive(&bars->d_empty[sd]);
+#pragma unroll
+                for (int j = 0; j < DE; ++j) asm volatile("" : "+f"(E[j]));
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    float gt[d3];
+#pragma unroll
+                    for (int M = 0; M < d3; ++M) {
+                        const float mine = __uint_as_float(h ? v[M][4 + i] : v[M][i]);
+                        const float send = __uint_as_float(h ? v[M][i] : v[M][4 + i]);
+                        gt[M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
+                    }
+                    Pth::template bwd<float, WANT_GV>(Vr[i], E, gt, gv[i], gE);
+                }
+            });
+            // (d) gV rows: staged per warp in the (now idle) operand region, stored as coalesced 16-byte vectors
+            if constexpr (WANT_GV) {
+                float* stg = reinterpret_cast<float*>(sm + MB::OFF_G) + warp * (8 * 16 * DV);
+#pragma unroll
+                for (int i = 0; i < 4; ++i) row_store<float, DV>(stg + ((4 * h + i) * 16 + nl) * DV, gv[i]);
+                __syncwarp();
+                const int ebase = eb + 8 * wq;
+#pragma unroll
+                for (int r = 0; r < 18; ++r) {   // 8 edges x 288 floats = 576 float4
+                    const int idx = lane + 32 * r, el = idx / 72, w4 = idx - el * 72;
+                    if (ebase + el < e1)
+                        *reinterpret_cast<float4*>(gV + ((size_t)(ebase + el) * 64 + 16 * q) * DV + 4 * w4) = reinterpret_cast<const float4*>(stg)[idx];
+                }
+            }
+            named_bar(1, MB::CT);   // operand region free for the next tile's cotangent (all MMAs of this tile have completed)
+        }
+        // ---- gEenv: lane halves by shuffle, the two edge groups (wq) through shared memory, fixed order
+#pragma unroll
+        for (int j = 0; j < DE; ++j) gE[j] += __shfl_xor_sync(0xffffffffu, gE[j], 16);
+        float* red = reinterpret_cast<float*>(sm + MB::OFF_G);
+        if (wq == 1 && h == 0) {
+#pragma unroll
+            for (int j = 0; j < DE; ++j) red[n * DE + j] = gE[j];
+        }
+        named_bar(1, MB::CT);
+        if (wq == 0 && h == 0) {
+            float* dst = gE_dst + ((size_t)(gE_by_item ? (long)blockIdx.x : (long)c) * 64 + n) * DE;
+#pragma unroll
+            for (int j = 0; j < DE; ++j) dst[j] = gE[j] + red[n * DE + j];
+        }
+    }
+    tc05::fence_before_sync();
+    __syncthreads();
+    if (warp == MB::CT / 32) { __syncwarp(); tc05::tmem_dealloc(tbase, 512); }
 }
 
 }  // namespace allegro

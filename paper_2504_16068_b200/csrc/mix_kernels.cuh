@@ -245,8 +245,9 @@ static allegro_status_t launch_mix_backward(const TpArgs& a) {
 #if ALLEGRO_L == 2
     if constexpr (sizeof(T) == 4) {
         if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr) {
-            allegro_status_t s2 = a.gV ? launch_mix2_backward_gv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0)
-                                       : launch_mix2_backward_nogv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0);
+            allegro_status_t s2 = getenv("ALLEGRO_MIX_V2") == nullptr ? launch_mix3_backward_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0)
+                                  : a.gV ? launch_mix2_backward_gv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0)
+                                         : launch_mix2_backward_nogv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0);
             if (s2 != ALLEGRO_OK) return s2;
             if (have_items) {
                 combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, (const T*)a.ws, (T*)a.gEenv);
