@@ -21,7 +21,7 @@ static allegro_status_t mix3_images(const TpArgs& a, float** img_f, float** img_
         plan->dense_img = p;
     }
     *img_f = (float*)plan->dense_img;
-    *img_b = *img_f + (size_t)Mix3::P * 4096;
+    *img_b = *img_f + (size_t)Mix3::P * (Mix3::IMG_BYTES / 4);
     mix3_prep_kernel<<<Mix3::P, 256, 0, a.st>>>((const float*)a.path_w, *img_f, *img_b);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;

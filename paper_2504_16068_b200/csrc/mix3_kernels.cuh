@@ -46,7 +46,7 @@ struct Mix3 {
     static constexpr int BV_BYTES = 2 * 128 * 128;                // one B variant (hi or lo): [2 K-atoms][<=128 rows][128 B]
     static constexpr int B_BYTES = 2 * BV_BYTES;
     static constexpr int NA = 3, NB = 2;                          // ring depths
-    static constexpr int IMG_BYTES = 64 * 64 * 4;                 // one path's weight image in global memory (hi rows only)
+    static constexpr int IMG_BYTES = 2 * 128 * 128;               // one path's weight image in global memory (hi and lo rows)
     static constexpr int OFF_A = 0, OFF_B = NA * A_BYTES, OFF_BAR = OFF_B + NB * B_BYTES;
     static constexpr int SMEM = OFF_BAR + 256 + 1024;             // + barrier block + 1024-byte alignment slack
     // TMEM column base of each output block, indexed by off3 (0e:0, 0o:1, 1e:2, 1o:5, 2e:8, 2o:13); N_b = 32 / 80 / 128
@@ -62,17 +62,22 @@ struct Mix3 {
 };
 
 // Weight images: img_f[p] feeds the forward (A row = output channel n', K = input channel n), img_b[p] the VJP
-// (A row = input channel n, K = output channel n').  Layout [K-atom a][quarter q][row nl][128 B], 16-byte chunk c of a row
-// stored at chunk position c ^ (nl & 7): the bytes land in the "hi" rows of the swizzled A tile by plain bulk copies.
+// (A row = input channel n, K = output channel n').  Each image is the complete swizzled A tile, [K-atom a][row 32 q + 16 h + nl][128 B]
+// with the 16-byte chunk c of a row stored at chunk position c ^ (nl & 7): h = 0 rows hold W (the tensor core truncates it to
+// tf32), h = 1 rows the exact remainder W - tf32(W).  One 32 KB bulk copy per path puts it into shared memory.
 static __global__ void mix3_prep_kernel(const float* __restrict__ W, float* __restrict__ img_f, float* __restrict__ img_b) {
     const int p = blockIdx.x;
     const float* Wp = W + (size_t)p * 64 * 64;
     for (int idx = threadIdx.x; idx < 64 * 64; idx += blockDim.x) {
         const int row = idx >> 6, k = idx & 63;
         const int a = k >> 5, q = row >> 4, nl = row & 15, c = (k & 31) >> 2;
-        const int dst = ((a * 4 + q) * 16 + nl) * 32 + ((c ^ (nl & 7)) << 2) + (k & 3);
-        img_f[(size_t)p * 4096 + dst] = Wp[row * 64 + k];   // (n' = row, n = k)
-        img_b[(size_t)p * 4096 + dst] = Wp[k * 64 + row];   // (n = row, n' = k)
+        const int dst = (a * 128 + 32 * q + nl) * 32 + ((c ^ (nl & 7)) << 2) + (k & 3);
+        const float wf = Wp[row * 64 + k], wb = Wp[k * 64 + row];   // (n' = row, n = k) ; (n = row, n' = k)
+        const float wfh = __uint_as_float(__float_as_uint(wf) & 0xffffe000u), wbh = __uint_as_float(__float_as_uint(wb) & 0xffffe000u);
+        img_f[(size_t)p * 8192 + dst] = wf;
+        img_f[(size_t)p * 8192 + dst + 16 * 32] = wf - wfh;
+        img_b[(size_t)p * 8192 + dst] = wb;
+        img_b[(size_t)p * 8192 + dst + 16 * 32] = wb - wbh;
     }
 }
 
@@ -124,13 +129,8 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                     mbar_wait(&bars->a_empty[sa], ph ^ 1u);
                     MIX3_ACC(3, blockIdx.x == 0);
                     mbar_expect_tx(&bars->a_full[sa], M3::IMG_BYTES);
-                    unsigned char* dstA = sm + M3::OFF_A + sa * M3::A_BYTES;
-                    const unsigned char* src = reinterpret_cast<const unsigned char*>(img) + (size_t)p * M3::IMG_BYTES;
-#pragma unroll
-                    for (int a = 0; a < 2; ++a)
-#pragma unroll
-                        for (int q = 0; q < 4; ++q)
-                            bulk_load(dstA + a * 16384 + q * 4096, src + (a * 4 + q) * 2048, 2048, &bars->a_full[sa]);
+                    bulk_load(sm + M3::OFF_A + sa * M3::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * M3::IMG_BYTES,
+                              M3::IMG_BYTES, &bars->a_full[sa]);
                 }
             }
         } else if (lane == 1) {
@@ -138,11 +138,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 128);
             // descriptors of K step 0 of every ring stage; K step j adds (j >> 2) * 16384 + (j & 3) * 32 bytes (16-byte units)
-            uint64_t adesc[M3::NA], bdesc[M3::NB];
-#pragma unroll
-            for (int s = 0; s < M3::NA; ++s) adesc[s] = tc05::sdesc_sw128(smem_u32(sm + M3::OFF_A + s * M3::A_BYTES));
-#pragma unroll
-            for (int s = 0; s < M3::NB; ++s) bdesc[s] = tc05::sdesc_sw128(smem_u32(sm + M3::OFF_B + s * M3::B_BYTES));
+            const uint32_t adesc0 = tc05::sdesc_lo(smem_u32(sm + M3::OFF_A)), bdesc0 = tc05::sdesc_lo(smem_u32(sm + M3::OFF_B));
             for (int t = 0; t < ntiles; ++t) {
                 MIX3_T0();
                 if (t > 0) { mbar_wait(&bars->d_empty, (uint32_t)(t - 1) & 1u); tc05::fence_after_sync(); }
@@ -154,17 +150,20 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                     constexpr uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
                     constexpr bool first = M3::first_of_block(p);   // first path of its output block: initialises the accumulator
                     const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;          // 15 B-ring turns per tile
+                    mbar_wait(&bars->a_full[sa], (uint32_t)(p / M3::NA) & 1u);
                     mbar_wait(&bars->b_full[sb], phb);
                     MIX3_ACC(0, blockIdx.x == 0);
                     tc05::fence_after_sync();
                     const uint32_t dcol = tbase + (uint32_t)M3::dcol(off3);
+                    uint32_t ad = adesc0 + (uint32_t)((sa * M3::A_BYTES) >> 4), bd = bdesc0 + (uint32_t)((sb * M3::B_BYTES) >> 4);
+                    asm volatile("" : "+r"(ad), "+r"(bd));   // opaque per path: keeps the descriptor words from being hoisted and spilled
 #pragma unroll
                     for (int v = 0; v < 2; ++v)          // B variant: hi, lo
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {    // K step of 8 channels
-                            const uint64_t koff = (uint64_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
-                            tc05::mma_tf32(dcol, adesc[sa] + koff, bdesc[sb] + (uint64_t)((v * M3::BV_BYTES) >> 4) + koff, idesc,
-                                           (first && v == 0 && j == 0) ? 0u : 1u);
+                            const uint32_t koff = (uint32_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
+                            tc05::mma_tf32_lo(dcol, ad + koff, bd + (uint32_t)((v * M3::BV_BYTES) >> 4) + koff, tc05::kSdescHiSw128, idesc,
+                                              (first && v == 0 && j == 0) ? 0u : 1u);
                         }
                     tc05::mma_commit(&bars->b_empty[sb]);
                     tc05::mma_commit(&bars->a_empty[sa]);
@@ -207,9 +206,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                 constexpr int p = decltype(pc)::value;
                 using Pth = TPPath<2, p>;
                 constexpr int sa = p % M3::NA, sb = p & 1;
-                constexpr uint32_t pha = (uint32_t)(p / M3::NA) & 1u;
                 const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;
-                unsigned char* As = sm + M3::OFF_A + sa * M3::A_BYTES;
                 unsigned char* Bs = sm + M3::OFF_B + sb * M3::B_BYTES;
                 // B: t_p of this thread's three edges, hi (raw) and lo
                 MIX3_ACC(10, blockIdx.x == 0 && tid == 0 && p == 0);
@@ -230,17 +227,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                         *reinterpret_cast<float*>(dst + M3::BV_BYTES) = tf32_lo(tp[M]);
                     }
                 }
-                // A lo rows: W - tf32(W) (hi rows arrive by TMA; waited for after the B work so that the copy's latency is covered)
                 MIX3_ACC(5, blockIdx.x == 0 && tid == 0);
-                mbar_wait(&bars->a_full[sa], pha);
-                MIX3_ACC(6, blockIdx.x == 0 && tid == 0);
-#pragma unroll
-                for (int cid = tid; cid < 1024; cid += M3::CT) {
-                    unsigned char* src = As + (cid >> 9) * 16384 + ((cid >> 7) & 3) * 4096 + (cid & 127) * 16;
-                    float4 w = *reinterpret_cast<const float4*>(src);
-                    w.x = tf32_lo(w.x); w.y = tf32_lo(w.y); w.z = tf32_lo(w.z); w.w = tf32_lo(w.w);
-                    *reinterpret_cast<float4*>(src + 2048) = w;
-                }
                 fence_proxy_async();
                 __syncwarp();
                 if (lane == 0) mbar_arrive(&bars->b_full[sb]);
@@ -313,12 +300,33 @@ struct Mix3B {
     static constexpr int TE = 16, CT = 256;                        // 8 compute warps (<= 168 registers each) + 1 control warp
     static constexpr int ROWS = 288;                                // sum over blocks of d3 * TE
     static constexpr int G_ATOM = ROWS * 128, G_VAR = 2 * G_ATOM, G_BYTES = 2 * G_VAR;   // hi, lo: [2 K-atoms][288 rows][128 B]
-    static constexpr int A_BYTES = 2 * 128 * 128, NA = 2, ND = 4;
+    static constexpr int A_BYTES = 2 * 128 * 128, NA = 2, ND = 3;   // 30 paths = 10 turns of the accumulator ring: slot and parity depend on p only
     static constexpr int OFF_G = 0, OFF_A = G_BYTES, OFF_BAR = OFF_A + NA * A_BYTES;
     static constexpr int SMEM = OFF_BAR + 256 + 1024;
     // first row of a block's B operand, indexed by off3
     __host__ __device__ static constexpr int rowoff(int off3) {
         return off3 == 0 ? 0 : off3 == 1 ? 16 : off3 == 2 ? 32 : off3 == 5 ? 80 : off3 == 8 ? 128 : 208;
+    }
+    // TMEM columns: accumulator ring at 0, 80, 160; the V rows of a thread's four pairs (72 columns per warp row wq) at 320 ..
+    static constexpr int VCOL = 320;
+    // (l1, p1) block of V that path p reads: first component and width
+    __host__ __device__ static constexpr int off1(int p) {
+        int idx = 0;
+        for (int l1 = 0; l1 <= 2; ++l1)
+            for (int p1 = 0; p1 < 2; ++p1)
+                for (int l2 = 0; l2 <= 2; ++l2)
+                    for (int l3 = (l1 > l2 ? l1 - l2 : l2 - l1); l3 <= (l1 + l2 < 2 ? l1 + l2 : 2); ++l3, ++idx)
+                        if (idx == p) return 2 * l1 * l1 + (p1 ? 2 * l1 + 1 : 0);
+        return -1;
+    }
+    __host__ __device__ static constexpr int d1(int p) {
+        int idx = 0;
+        for (int l1 = 0; l1 <= 2; ++l1)
+            for (int p1 = 0; p1 < 2; ++p1)
+                for (int l2 = 0; l2 <= 2; ++l2)
+                    for (int l3 = (l1 > l2 ? l1 - l2 : l2 - l1); l3 <= (l1 + l2 < 2 ? l1 + l2 : 2); ++l3, ++idx)
+                        if (idx == p) return 2 * l1 + 1;
+        return -1;
     }
     // component k of a feature row -> row of the (M = 0, e = 0) element of its block + 16 M
     __host__ __device__ static constexpr int comprow(int k) {
@@ -326,7 +334,7 @@ struct Mix3B {
     }
 };
 struct Mix3BBars {
-    uint64_t a_full[Mix3B::NA], a_conv[Mix3B::NA], a_empty[Mix3B::NA], d_full[Mix3B::ND], d_empty[Mix3B::ND], g_full;
+    uint64_t a_full[Mix3B::NA], a_empty[Mix3B::NA], d_full[Mix3B::ND], d_empty[Mix3B::ND], g_full;
     uint32_t tmem_slot;
 };
 
@@ -347,7 +355,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
     const int ntiles = (e1 - e0 + TE - 1) / TE;   // 0 for an empty item: only the zero gEenv row is written
 
     if (tid == 0) {
-        for (int s = 0; s < MB::NA; ++s) { mbar_init(&bars->a_full[s], 1); mbar_init(&bars->a_conv[s], MB::CT / 32); mbar_init(&bars->a_empty[s], 1); }
+        for (int s = 0; s < MB::NA; ++s) { mbar_init(&bars->a_full[s], 1); mbar_init(&bars->a_empty[s], 1); }
         for (int s = 0; s < MB::ND; ++s) { mbar_init(&bars->d_full[s], 1); mbar_init(&bars->d_empty[s], MB::CT / 32); }
         mbar_init(&bars->g_full, MB::CT / 32);
         fence_mbar_init();
@@ -367,22 +375,15 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
                     const uint32_t ph = (uint32_t)(t + (p >> 1)) & 1u;            // 15 ring turns per tile
                     mbar_wait(&bars->a_empty[sa], ph ^ 1u);
                     mbar_expect_tx(&bars->a_full[sa], Mix3::IMG_BYTES);
-                    unsigned char* dstA = sm + MB::OFF_A + sa * MB::A_BYTES;
-                    const unsigned char* src = reinterpret_cast<const unsigned char*>(img) + (size_t)p * Mix3::IMG_BYTES;
-#pragma unroll
-                    for (int a = 0; a < 2; ++a)
-#pragma unroll
-                        for (int q = 0; q < 4; ++q) bulk_load(dstA + a * 16384 + q * 4096, src + (a * 4 + q) * 2048, 2048, &bars->a_full[sa]);
+                    bulk_load(sm + MB::OFF_A + sa * MB::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * Mix3::IMG_BYTES,
+                              Mix3::IMG_BYTES, &bars->a_full[sa]);
                 }
         } else if (lane == 1) {
             // ---- MMA issue
             constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 16);
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 48);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
-            uint64_t adesc[MB::NA];
-#pragma unroll
-            for (int s = 0; s < MB::NA; ++s) adesc[s] = tc05::sdesc_sw128(smem_u32(sm + MB::OFF_A + s * MB::A_BYTES));
-            const uint64_t gdesc = tc05::sdesc_sw128(smem_u32(sm + MB::OFF_G));
+            const uint32_t adesc0 = tc05::sdesc_lo(smem_u32(sm + MB::OFF_A)), gdesc0 = tc05::sdesc_lo(smem_u32(sm + MB::OFF_G));
             for (int t = 0; t < ntiles; ++t) {
                 mbar_wait(&bars->g_full, (uint32_t)t & 1u);
                 static_for3<0, P>([&](auto pc) {
@@ -390,18 +391,20 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
                     constexpr int sa = p & 1;
                     constexpr int d3 = Gen::d3(p), off3 = Gen::off3(p);
                     constexpr uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
-                    const uint32_t g = (uint32_t)(t * P + p), sd = g & 3u;
-                    mbar_wait(&bars->a_conv[sa], (uint32_t)(t + (p >> 1)) & 1u);
-                    mbar_wait(&bars->d_empty[sd], ((g >> 2) & 1u) ^ 1u);
+                    constexpr int sd = p % MB::ND;
+                    mbar_wait(&bars->a_full[sa], (uint32_t)(t + (p >> 1)) & 1u);
+                    mbar_wait(&bars->d_empty[sd], ((uint32_t)(p / MB::ND) & 1u) ^ 1u);
                     tc05::fence_after_sync();
-                    const uint32_t dcol = tbase + sd * 128u;
+                    const uint32_t dcol = tbase + sd * 80u;
+                    uint32_t ad = adesc0, gd = gdesc0;   // opaque per path: otherwise all 112 descriptor words are hoisted out of the loops and spilled
+                    asm volatile("" : "+r"(ad), "+r"(gd));
 #pragma unroll
                     for (int v = 0; v < 2; ++v)
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
-                            const uint64_t koff = (uint64_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
-                            const uint64_t goff = (uint64_t)((v * MB::G_VAR + (j >> 2) * MB::G_ATOM + MB::rowoff(off3) * 128 + (j & 3) * 32) >> 4);
-                            tc05::mma_tf32(dcol, adesc[sa] + koff, gdesc + goff, idesc, (v == 0 && j == 0) ? 0u : 1u);
+                            const uint32_t koff = (uint32_t)((sa * MB::A_BYTES + (j >> 2) * 16384 + (j & 3) * 32) >> 4);
+                            const uint32_t goff = (uint32_t)((v * MB::G_VAR + (j >> 2) * MB::G_ATOM + MB::rowoff(off3) * 128 + (j & 3) * 32) >> 4);
+                            tc05::mma_tf32_lo(dcol, ad + koff, gd + goff, tc05::kSdescHiSw128, idesc, (v == 0 && j == 0) ? 0u : 1u);
                         }
                     tc05::mma_commit(&bars->d_full[sd]);
                     tc05::mma_commit(&bars->a_empty[sa]);
@@ -446,48 +449,64 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
             fence_proxy_async();
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars->g_full);
-            // (b) V rows of this thread's pairs; gV accumulators
-            float Vr[4][DV], gv[4][DV];
+            // (b) V rows of this thread's four pairs parked in this thread's TMEM lane (columns VCOL + 72 wq + 18 i + k): registers
+            // hold the gV accumulators; each path reads back only the (l1, p1) block it contracts
+            float gv[4][DV];
+            const uint32_t vrow = tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(MB::VCOL + 72 * wq);
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int e = eb + 8 * wq + 4 * h + i;
+                float vr[DV];
                 if (e < e1) {
-                    row_load<float, DV>(V + ((size_t)e * 64 + n) * DV, Vr[i]);
+                    row_load<float, DV>(V + ((size_t)e * 64 + n) * DV, vr);
                 } else {
 #pragma unroll
-                    for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
+                    for (int k = 0; k < DV; ++k) vr[k] = 0.f;
                 }
+                uint32_t lo16[16], hi2[2];
+#pragma unroll
+                for (int k = 0; k < 16; ++k) lo16[k] = __float_as_uint(vr[k]);
+                hi2[0] = __float_as_uint(vr[16]); hi2[1] = __float_as_uint(vr[17]);
+                tc05::tmem_st16(vrow + (uint32_t)(18 * i), lo16);
+                tc05::tmem_st2(vrow + (uint32_t)(18 * i + 16), hi2);
 #pragma unroll
                 for (int k = 0; k < DV; ++k) gv[i][k] = 0.f;
             }
-            // (c) paths: convert the next weight image's lo rows, then consume the accumulator of this path
-            auto convert = [&](int sa, uint32_t ph) {
-                unsigned char* As = sm + MB::OFF_A + sa * MB::A_BYTES;
-                mbar_wait(&bars->a_full[sa], ph);
-#pragma unroll
-                for (int cid = tid; cid < 1024; cid += MB::CT) {
-                    unsigned char* src = As + (cid >> 9) * 16384 + ((cid >> 7) & 3) * 4096 + (cid & 127) * 16;
-                    float4 w = *reinterpret_cast<const float4*>(src);
-                    w.x = tf32_lo(w.x); w.y = tf32_lo(w.y); w.z = tf32_lo(w.z); w.w = tf32_lo(w.w);
-                    *reinterpret_cast<float4*>(src + 2048) = w;
-                }
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&bars->a_conv[sa]);
-            };
-            convert(0, (uint32_t)t & 1u);
+            tc05::tmem_st_wait();
+            // (c) paths: consume every accumulator as soon as it is complete
             static_for3<0, P>([&](auto pc) {
                 constexpr int p = decltype(pc)::value;
                 using Pth = TPPath<2, p>;
                 constexpr int d3 = Pth::D3;
-                if (p + 1 < P) convert((p + 1) & 1, (uint32_t)(t + ((p + 1) >> 1)) & 1u);
-                const uint32_t g = (uint32_t)(t * P + p), sd = g & 3u;
-                mbar_wait(&bars->d_full[sd], (g >> 2) & 1u);
+                constexpr int sd = p % MB::ND;
+                mbar_wait(&bars->d_full[sd], (uint32_t)(p / MB::ND) & 1u);
                 tc05::fence_after_sync();
+                constexpr int o1 = MB::off1(p), w1 = MB::d1(p);
                 uint32_t v[d3][8];
-                const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + sd * 128u + (uint32_t)(8 * wq);
+                const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + sd * 80u + (uint32_t)(8 * wq);
 #pragma unroll
                 for (int M = 0; M < d3; ++M) tc05::tmem_ld8(trow + (uint32_t)(M * TE), v[M]);
+                float Vb[4][DV];   // only components o1 .. o1 + w1 - 1 are read by this path's code
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    if constexpr (w1 == 1) {
+                        uint32_t x[1];
+                        tc05::tmem_ld1(vrow + (uint32_t)(18 * i + o1), x);
+                        Vb[i][o1] = __uint_as_float(x[0]);
+                    } else if constexpr (w1 == 3) {
+                        uint32_t x[4];
+                        tc05::tmem_ld4(vrow + (uint32_t)(18 * i + o1), x);
+#pragma unroll
+                        for (int k = 0; k < 3; ++k) Vb[i][o1 + k] = __uint_as_float(x[k]);
+                    } else {
+                        uint32_t x[4], y[1];
+                        tc05::tmem_ld4(vrow + (uint32_t)(18 * i + o1), x);
+                        tc05::tmem_ld1(vrow + (uint32_t)(18 * i + o1 + 4), y);
+#pragma unroll
+                        for (int k = 0; k < 4; ++k) Vb[i][o1 + k] = __uint_as_float(x[k]);
+                        Vb[i][o1 + 4] = __uint_as_float(y[0]);
+                    }
+                }
                 tc05::tmem_ld_wait();
                 tc05::fence_before_sync();
                 __syncwarp();
@@ -503,7 +522,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
                         const float send = __uint_as_float(h ? v[M][i] : v[M][4 + i]);
                         gt[M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
                     }
-                    Pth::template bwd<float, WANT_GV>(Vr[i], E, gt, gv[i], gE);
+                    Pth::template bwd<float, WANT_GV>(Vb[i], E, gt, gv[i], gE);
                 }
             });
             // (d) gV rows: staged per warp in the (now idle) operand region, stored as coalesced 16-byte vectors
