@@ -34,7 +34,7 @@ allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a) {
     if (s != ALLEGRO_OK) return s;
     auto k = mix3_fwd_kernel<0>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3::SMEM));
-    k<<<(unsigned)a.n_items, Mix3::CT + 32, Mix3::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out);
+    k<<<(unsigned)a.n_items, Mix3::CT + 64, Mix3::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -46,12 +46,12 @@ allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst,
     if (a.gV) {
         auto k = mix3_bwd_kernel<true>;
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
-        k<<<(unsigned)a.n_items, Mix3B::CT + 32, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
+        k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
                                                                     img_b, (float*)a.gV, gE_dst, gE_by_item);
     } else {
         auto k = mix3_bwd_kernel<false>;
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
-        k<<<(unsigned)a.n_items, Mix3B::CT + 32, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
+        k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
                                                                     img_b, nullptr, gE_dst, gE_by_item);
     }
     ALLEGRO_LAUNCHED();

@@ -90,7 +90,7 @@ struct Mix3Bars {
 __device__ __forceinline__ float tf32_lo(float x) { return x - __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 
 template <int DUMMY = 0>
-__global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
+__global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                    const float* __restrict__ V, const float* __restrict__ Eenv,
                                                                    const float* __restrict__ img, float* __restrict__ out) {
     using M3 = Mix3;
@@ -118,9 +118,9 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
     tc05::fence_after_sync();
     const uint32_t tbase = bars->tmem_slot;
 
-    if (warp == M3::CT / 32) {
-        // ================= control warp: lane 0 streams the weight images (TMA), lane 1 issues the MMAs
-        if (lane == 0) {
+    if (warp >= M3::CT / 32) {
+        // ================= two control warps (one thread each, so that neither spins inside the other's warp): weight images (TMA), MMA issue
+        if (warp == M3::CT / 32 && lane == 0) {
             for (int t = 0; t < ntiles; ++t) {
                 for (int p = 0; p < P; ++p) {
                     const int sa = p % M3::NA;                                   // 30 paths per tile = 10 ring turns: stage and
@@ -133,7 +133,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                               M3::IMG_BYTES, &bars->a_full[sa]);
                 }
             }
-        } else if (lane == 1) {
+        } else if (warp == M3::CT / 32 + 1) {   // the whole warp walks the loop; one elected lane issues
             constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 32);
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 128);
@@ -142,7 +142,7 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
             for (int t = 0; t < ntiles; ++t) {
                 MIX3_T0();
                 if (t > 0) { mbar_wait(&bars->d_empty, (uint32_t)(t - 1) & 1u); tc05::fence_after_sync(); }
-                MIX3_ACC(2, blockIdx.x == 0);
+                MIX3_ACC(2, blockIdx.x == 0 && lane == 0);
                 static_for3<0, P>([&](auto pc) {
                     constexpr int p = decltype(pc)::value;
                     constexpr int sa = p % M3::NA, sb = p & 1;
@@ -152,9 +152,10 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                     const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;          // 15 B-ring turns per tile
                     mbar_wait(&bars->a_full[sa], (uint32_t)(p / M3::NA) & 1u);
                     mbar_wait(&bars->b_full[sb], phb);
-                    MIX3_ACC(0, blockIdx.x == 0);
+                    MIX3_ACC(0, blockIdx.x == 0 && lane == 0);
                     tc05::fence_after_sync();
                     const uint32_t dcol = tbase + (uint32_t)M3::dcol(off3);
+                    if (tc05::elect_one()) {
                     uint32_t ad = adesc0 + (uint32_t)((sa * M3::A_BYTES) >> 4), bd = bdesc0 + (uint32_t)((sb * M3::B_BYTES) >> 4);
                     asm volatile("" : "+r"(ad), "+r"(bd));   // opaque per path: keeps the descriptor words from being hoisted and spilled
 #pragma unroll
@@ -167,9 +168,11 @@ __global__ void __launch_bounds__(Mix3::CT + 32, 1) mix3_fwd_kernel(const int* _
                         }
                     tc05::mma_commit(&bars->b_empty[sb]);
                     tc05::mma_commit(&bars->a_empty[sa]);
-                    MIX3_ACC(1, blockIdx.x == 0);
+                    if (p == P - 1) tc05::mma_commit(&bars->d_full);
+                    }
+                    __syncwarp();
+                    MIX3_ACC(1, blockIdx.x == 0 && lane == 0);
                 });
-                tc05::mma_commit(&bars->d_full);
             }
         }
     } else {
@@ -339,7 +342,7 @@ struct Mix3BBars {
 };
 
 template <bool WANT_GV>
-__global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
+__global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                     const float* __restrict__ G, const float* __restrict__ V,
                                                                     const float* __restrict__ Eenv, const float* __restrict__ img,
                                                                     float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
@@ -366,8 +369,8 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
     tc05::fence_after_sync();
     const uint32_t tbase = bars->tmem_slot;
 
-    if (warp == MB::CT / 32) {
-        if (lane == 0) {
+    if (warp >= MB::CT / 32) {
+        if (warp == MB::CT / 32 && lane == 0) {
             // ---- weight images (TMA)
             for (int t = 0; t < ntiles; ++t)
                 for (int p = 0; p < P; ++p) {
@@ -378,8 +381,8 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
                     bulk_load(sm + MB::OFF_A + sa * MB::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * Mix3::IMG_BYTES,
                               Mix3::IMG_BYTES, &bars->a_full[sa]);
                 }
-        } else if (lane == 1) {
-            // ---- MMA issue
+        } else if (warp == MB::CT / 32 + 1) {
+            // ---- MMA issue: the whole warp walks the loop, one elected lane issues
             constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 16);
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 48);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
@@ -396,6 +399,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
                     mbar_wait(&bars->d_empty[sd], ((uint32_t)(p / MB::ND) & 1u) ^ 1u);
                     tc05::fence_after_sync();
                     const uint32_t dcol = tbase + sd * 80u;
+                    if (tc05::elect_one()) {
                     uint32_t ad = adesc0, gd = gdesc0;   // opaque per path: otherwise all 112 descriptor words are hoisted out of the loops and spilled
                     asm volatile("" : "+r"(ad), "+r"(gd));
 #pragma unroll
@@ -408,6 +412,8 @@ __global__ void __launch_bounds__(Mix3B::CT + 32, 1) mix3_bwd_kernel(const int* 
                         }
                     tc05::mma_commit(&bars->d_full[sd]);
                     tc05::mma_commit(&bars->a_empty[sa]);
+                    }
+                    __syncwarp();
                 });
             }
         }

@@ -37,6 +37,19 @@ __host__ __device__ __forceinline__ uint32_t sw128_off(uint32_t r, uint32_t chun
     return (r >> 3) * 1024u + (r & 7u) * 128u + ((chunk ^ (r & 7u)) << 4);
 }
 
+// one lane of a converged warp (the same lane every time): lets the compiler keep MMA operands in uniform registers
+__device__ __forceinline__ bool elect_one() {
+    uint32_t pred;
+    asm volatile(
+        "{\n"
+        ".reg .pred P;\n"
+        "elect.sync _|P, 0xffffffff;\n"
+        "selp.u32 %0, 1, 0, P;\n"
+        "}\n"
+        : "=r"(pred));
+    return pred != 0;
+}
+
 // ---- instruction descriptor (upper 32 bits of the "idesc" operand): D = fp32, A / B format, K-major both, M, N
 enum : uint32_t { FMT_F16 = 0, FMT_BF16 = 1, FMT_TF32 = 2 };
 __host__ __device__ constexpr uint32_t make_idesc(uint32_t fmt_a, uint32_t fmt_b, uint32_t M, uint32_t N) {
