@@ -329,7 +329,10 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
     prm = {k: torch.from_numpy(np.ascontiguousarray(p[k])).to(td).cuda() for k in ("W_x0", "W_v0", "W_w", "W_p", "A_lat", "q")}
     prm.update(rc=p["rc"], scale=p["scale"])
     dt = ab.F32 if inp["dt"] == np.float32 else ab.F64
-    step = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm)
+    # last layer: its output feeds only the readout of the l = 0 outputs (configs[2]), so the plan is restricted to the 0e block
+    plan_last = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
+    plan_last.set_out_blocks(0x1)
+    step = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=plan_last)
     E, N = step.E, step.N
 
     def barrier():

@@ -29,6 +29,9 @@ _vp, _i32p, _f64p = C.c_void_p, C.POINTER(C.c_int32), C.POINTER(C.c_double)
 SIGNATURES = {
     "allegro_plan_create": (C.c_int, [C.c_int, C.c_int, C.c_int, C.c_int, C.c_int, C.POINTER(_vp)]),
     "allegro_plan_destroy": (None, [_vp]),
+    "allegro_plan_bind_weights": (C.c_int, [_vp, _vp, _vp]),
+    "allegro_plan_set_out_blocks": (C.c_int, [_vp, C.c_uint]),
+    "allegro_plan_set_in_blocks": (C.c_int, [_vp, C.c_uint]),
     "allegro_plan_num_paths": (C.c_int, [_vp]),
     "allegro_plan_dim_v": (C.c_int, [_vp]),
     "allegro_plan_dim_e": (C.c_int, [_vp]),
@@ -131,6 +134,18 @@ class Plan:
         if getattr(self, "h", None) and _lib is not None:
             _lib.allegro_plan_destroy(self.h)
             self.h = None
+
+    def bind_weights(self, path_w, stream=None):
+        """scalar mode: fold path_w into the plan's combined tensor; later calls may pass path_w=None (CUDA-graph capturable)"""
+        _check(lib().allegro_plan_bind_weights(self.h, _ptr(path_w), _stream(stream)))
+
+    def set_out_blocks(self, block_mask):
+        """compute only the output blocks of block_mask (bit b = block b in component order 0e, 0o, 1e, ...)"""
+        _check(lib().allegro_plan_set_out_blocks(self.h, int(block_mask)))
+
+    def set_in_blocks(self, block_mask):
+        """input blocks of V that are present (same bit order); the others are taken as zero and never read"""
+        _check(lib().allegro_plan_set_in_blocks(self.h, int(block_mask)))
 
     def paths(self):
         names = ["l1", "p1", "l2", "l3", "p3", "off1", "off2", "off3"]

@@ -63,8 +63,6 @@ def generate(force=False):
 
 def _jobs():
     jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("model.o", "model.cu", []), ("plan.o", "plan.cpp", [])]
-    for part in (0, 1, 2):      # the long poles first
-        jobs.insert(part, ("inst_mix2_p%d.o" % part, "inst_mix2.cu", ["-DALLEGRO_MIX2_PART=%d" % part]))
     for part in (0, 1):
         jobs.insert(0, ("inst_mix3_p%d.o" % part, "inst_mix3.cu", ["-DALLEGRO_MIX3_PART=%d" % part]))
     for tag, ctype in DTYPES:

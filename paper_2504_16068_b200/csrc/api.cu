@@ -42,6 +42,35 @@ ALLEGRO_DECL(double, 1) ALLEGRO_DECL(double, 2) ALLEGRO_DECL(double, 3)
             : (plan)->l_max == 2 ? F<double, 2>(__VA_ARGS__)             \
                                  : F<double, 3>(__VA_ARGS__)))
 
+// cw[z] = path_w[path(z)] * C_z (0 for paths into a masked-out output block), product in double, rounded once to the plan's dtype
+static void fold_host(const allegro_plan* plan, const void* path_w_host) {
+    const size_t nnz = plan->tab.nnz.size();
+    plan->cw.resize(nnz);
+    for (size_t z = 0; z < nnz; ++z) {
+        const NonZero& q = plan->tab.nnz[z];
+        double w = plan->dtype == ALLEGRO_F32 ? (double)((const float*)path_w_host)[q.path] : ((const double*)path_w_host)[q.path];
+        if (!plan->path_active(q.path)) w = 0.0;
+        const double c = w * q.c;
+        plan->cw[z] = plan->dtype == ALLEGRO_F32 ? (double)(float)c : c;
+    }
+    plan->cw_bound = true;
+}
+
+allegro_status_t bind_scalar_weights(const allegro_plan* plan, const void* path_w_dev, cudaStream_t st) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    ALLEGRO_CUDA(cudaStreamIsCapturing(st, &cs));
+    if (cs != cudaStreamCaptureStatusNone) {
+        set_error("scalar path weights cannot be read back while the stream is capturing: call allegro_plan_bind_weights first and pass path_w = NULL");
+        return ALLEGRO_EINVAL;
+    }
+    double host[128];   // P <= 68 values of at most 8 bytes
+    const size_t bytes = plan->tab.paths.size() * (plan->dtype == ALLEGRO_F32 ? 4 : 8);
+    ALLEGRO_CUDA(cudaMemcpyAsync(host, path_w_dev, bytes, cudaMemcpyDeviceToHost, st));
+    ALLEGRO_CUDA(cudaStreamSynchronize(st));
+    fold_host(plan, host);
+    return ALLEGRO_OK;
+}
+
 }  // namespace allegro
 
 using namespace allegro;
@@ -70,6 +99,27 @@ allegro_status_t allegro_plan_create(int l_max, allegro_parity_t parity, int n_c
 void allegro_plan_destroy(allegro_plan_t* plan) {
     if (plan && plan->dense_img) cudaFree(plan->dense_img);
     delete plan;
+}
+allegro_status_t allegro_plan_set_out_blocks(allegro_plan_t* plan, unsigned block_mask) {
+    ALLEGRO_CHECK_ARG(plan != nullptr, "plan is NULL");
+    const unsigned full = (1u << (2 * (plan->l_max + 1))) - 1u;
+    ALLEGRO_CHECK_ARG((block_mask & full) != 0, "empty block mask");
+    plan->out_blocks = block_mask & full;
+    plan->cw_bound = false;   // a bound table was folded for the previous mask
+    return ALLEGRO_OK;
+}
+allegro_status_t allegro_plan_set_in_blocks(allegro_plan_t* plan, unsigned block_mask) {
+    ALLEGRO_CHECK_ARG(plan != nullptr, "plan is NULL");
+    const unsigned full = (1u << (2 * (plan->l_max + 1))) - 1u;
+    ALLEGRO_CHECK_ARG((block_mask & full) != 0, "empty block mask");
+    plan->in_blocks = block_mask & full;
+    plan->cw_bound = false;
+    return ALLEGRO_OK;
+}
+allegro_status_t allegro_plan_bind_weights(allegro_plan_t* plan, const void* path_w, void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && path_w != nullptr, "plan / path_w is NULL");
+    ALLEGRO_CHECK_ARG(plan->wmode == ALLEGRO_W_SCALAR, "scalar path weights only (dense weights are read by every call)");
+    return bind_scalar_weights(plan, path_w, (cudaStream_t)stream);
 }
 int allegro_plan_num_paths(const allegro_plan_t* plan) { return plan ? (int)plan->tab.paths.size() : -1; }
 int allegro_plan_dim_v(const allegro_plan_t* plan) { return plan ? plan->tab.dV : -1; }
@@ -166,7 +216,8 @@ allegro_status_t allegro_tp_forward(const allegro_plan_t* plan, int n_atoms, lon
     ALLEGRO_CHECK_GRAPH();
     ALLEGRO_CHECK_ARG((V && out) || n_edges == 0, "V / out is NULL");
     ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
-    ALLEGRO_CHECK_ARG(path_w != nullptr, "path_w is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr || plan->wmode == ALLEGRO_W_SCALAR, "path_w is NULL (dense mode)");
+    ALLEGRO_CHECK_ARG(plan->wmode != ALLEGRO_W_DENSE || aligned16(path_w), "dense path_w not 16-byte aligned");
     ALLEGRO_CHECK_ARG(V != out || n_edges == 0, "out aliases V");
     ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(out) && aligned16(Eenv), "feature tensor not 16-byte aligned");
     ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
@@ -184,7 +235,7 @@ allegro_status_t allegro_tp_forward_energy(const allegro_plan_t* plan, int n_ato
     ALLEGRO_CHECK_ARG(V || n_edges == 0, "V is NULL");
     ALLEGRO_CHECK_ARG(out || G, "out and G are both NULL");
     ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
-    ALLEGRO_CHECK_ARG(path_w != nullptr && q != nullptr, "path_w / q is NULL");
+    ALLEGRO_CHECK_ARG(q != nullptr, "q is NULL");
     ALLEGRO_CHECK_ARG((V != out && V != G && (out != G || !out)) || n_edges == 0, "out / G alias V or each other");
     ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(out) && aligned16(G) && aligned16(Eenv), "feature tensor not 16-byte aligned");
     ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
@@ -206,7 +257,8 @@ allegro_status_t allegro_tp_backward(const allegro_plan_t* plan, int n_atoms, lo
     ALLEGRO_CHECK_GRAPH();
     ALLEGRO_CHECK_ARG((G && V) || n_edges == 0, "G / V is NULL");
     ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
-    ALLEGRO_CHECK_ARG(path_w != nullptr, "path_w is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr || plan->wmode == ALLEGRO_W_SCALAR, "path_w is NULL (dense mode)");
+    ALLEGRO_CHECK_ARG(plan->wmode != ALLEGRO_W_DENSE || aligned16(path_w), "dense path_w not 16-byte aligned");
     ALLEGRO_CHECK_ARG(gV == nullptr || (gV != G && gV != V), "gV aliases an input");
     ALLEGRO_CHECK_ARG(aligned16(G) && aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace),
                       "tensor not 16-byte aligned");
@@ -226,7 +278,7 @@ allegro_status_t allegro_tp_backward_energy(const allegro_plan_t* plan, int n_at
     ALLEGRO_CHECK_GRAPH();
     ALLEGRO_CHECK_ARG((out && V) || n_edges == 0, "out / V is NULL");
     ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
-    ALLEGRO_CHECK_ARG(path_w != nullptr && q != nullptr, "path_w / q is NULL");
+    ALLEGRO_CHECK_ARG(q != nullptr, "q is NULL");
     ALLEGRO_CHECK_ARG(gV == nullptr || (gV != out && gV != V), "gV aliases an input");
     ALLEGRO_CHECK_ARG(aligned16(out) && aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace),
                       "tensor not 16-byte aligned");
@@ -351,7 +403,7 @@ allegro_status_t allegro_layer_step_host(const allegro_plan_t* plan, int n_atoms
     cudaStream_t st = (cudaStream_t)stream;
     unsigned char* ws = (unsigned char*)workspace;
     const size_t s = plan->dtype == ALLEGRO_F32 ? 4 : 8;
-    const size_t n = plan->n, dV = plan->tab.dV, P = plan->tab.paths.size();
+    const size_t n = plan->n, dV = plan->tab.dV;
     const int32_t e_ptr[2] = {0, (int32_t)n_edges};
     ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.row_ptr, row_ptr_host, (size_t)(n_atoms + 1) * 4, cudaMemcpyHostToDevice, st));
     ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.e_ptr, e_ptr, 8, cudaMemcpyHostToDevice, st));
@@ -361,15 +413,15 @@ allegro_status_t allegro_layer_step_host(const allegro_plan_t* plan, int n_atoms
         ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.V, V_host, (size_t)n_edges * n * dV * s, cudaMemcpyHostToDevice, st));
     }
     ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.W_r, W_r_host, n * n_basis * s, cudaMemcpyHostToDevice, st));
-    ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.path_w, path_w_host, P * s, cudaMemcpyHostToDevice, st));
+    fold_host(plan, path_w_host);   // the combined tensor travels as a kernel parameter: nothing to copy
     ALLEGRO_CUDA(cudaMemcpyAsync(ws + L.q, q_host, n * s, cudaMemcpyHostToDevice, st));
     const int32_t* rp = (const int32_t*)(ws + L.row_ptr);
     allegro_status_t r;
     if ((r = allegro_env_radial_forward(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.rvec, ws + L.W_r, n_basis, r_cut, scale, nullptr,
                                         ws + L.Eenv, nullptr, 0, stream)) != ALLEGRO_OK) return r;
-    if ((r = allegro_tp_forward_energy(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.V, ws + L.Eenv, ws + L.path_w, ws + L.q, kappa, ws + L.out,
+    if ((r = allegro_tp_forward_energy(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.V, ws + L.Eenv, nullptr, ws + L.q, kappa, ws + L.out,
                                        ws + L.e_edge, nullptr, stream)) != ALLEGRO_OK) return r;
-    if ((r = allegro_tp_backward_energy(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.out, ws + L.V, ws + L.Eenv, ws + L.path_w, ws + L.q, kappa,
+    if ((r = allegro_tp_backward_energy(plan, n_atoms, n_edges, rp, nullptr, 0, ws + L.out, ws + L.V, ws + L.Eenv, nullptr, ws + L.q, kappa,
                                         want_gV ? ws + L.gV : nullptr, ws + L.gEenv, nullptr, nullptr, 0, stream)) != ALLEGRO_OK) return r;
     if ((r = allegro_env_radial_backward(plan, n_atoms, n_edges, rp, ws + L.gEenv, ws + L.rvec, ws + L.W_r, n_basis, r_cut, scale, ws + L.g_r,
                                          nullptr, stream)) != ALLEGRO_OK) return r;

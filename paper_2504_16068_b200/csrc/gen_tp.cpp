@@ -5,8 +5,8 @@
 // usage: gen_tp <out_dir>   -> writes <out_dir>/tp_gen.cuh
 //
 // Two flavours are emitted per l_max:
-//   folded : coefficient z is read as ALLEGRO_CW(z) (= path_w[path(z)] * C_z, folded per call into
-//            __constant__ memory -> a constant-bank FFMA operand), output index = out component k.
+//   folded : coefficient z is read as cw[z] (= path_w[path(z)] * C_z, the "combined tensor"); cw is the first argument, a
+//            reference to a __grid_constant__ kernel parameter -> a constant-bank FFMA operand; output index = out component k.
 //   paths  : coefficient is a compile-time literal, output index = toff(path) + M (one slot per
 //            (path, M): the un-weighted t[e][n][p][M] that feeds the dense per-path channel mix and
 //            the path-weight gradient).
@@ -44,7 +44,7 @@ static std::vector<Pair> group_pairs(const PlanTables& t, bool paths_flavour, co
 static std::string coef(bool paths_flavour, const Term& tm) {
     char buf[64];
     if (paths_flavour) snprintf(buf, sizeof buf, "T(%.17g)", tm.c);
-    else snprintf(buf, sizeof buf, "ALLEGRO_CW(%d)", tm.z);
+    else snprintf(buf, sizeof buf, "cw[%d]", tm.z);
     return buf;
 }
 
@@ -57,12 +57,6 @@ static void emit(FILE* f, int L) {
     const int DT = toff[P];
     fprintf(f, "\n// ======================= l_max = %d: P = %d, nnz = %zu, dV = %d, dE = %d, dT = %d\n", L, P, t.nnz.size(), t.dV,
             t.dE, DT);
-    fprintf(f, "static __device__ const short tpgen_zpath_%d[%zu] = {", L, t.nnz.size());
-    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%d%s", t.nnz[z].path, z + 1 == t.nnz.size() ? "" : ",");
-    fprintf(f, "};\n");
-    fprintf(f, "static __device__ const double tpgen_zcoef_%d[%zu] = {", L, t.nnz.size());
-    for (size_t z = 0; z < t.nnz.size(); ++z) fprintf(f, "%.17g%s", t.nnz[z].c, z + 1 == t.nnz.size() ? "" : ",");
-    fprintf(f, "};\n");
     fprintf(f, "template <> struct TPGen<%d> {\n", L);
     fprintf(f, "    static constexpr int LMAX = %d, DV = %d, DE = %d, P = %d, NNZ = %zu, DT = %d;\n", L, t.dV, t.dE, P, t.nnz.size(), DT);
     for (int flavour = 0; flavour < 2; ++flavour) {
@@ -72,8 +66,10 @@ static void emit(FILE* f, int L) {
         const char* sfx = pf ? "_paths" : "";
         // ---------------- forward
         fprintf(f, "    // %s forward: %zu products + %zu FMA\n", pf ? "per-path (un-weighted)" : "folded", pairs.size(), t.nnz.size());
-        fprintf(f, "    template <typename T> static __device__ __forceinline__ void fwd%s(const T (&V)[%d], const T (&E)[%d], T (&O)[%d]) {\n",
-                sfx, t.dV, t.dE, DO);
+        char cwarg[64] = "";
+        if (!pf) snprintf(cwarg, sizeof cwarg, "const T (&cw)[%zu], ", t.nnz.size());
+        fprintf(f, "    template <typename T> static __device__ __forceinline__ void fwd%s(%sconst T (&V)[%d], const T (&E)[%d], T (&O)[%d]) {\n",
+                sfx, cwarg, t.dV, t.dE, DO);
         std::vector<char> touched(DO, 0);
         for (const Pair& pr : pairs) {
             fprintf(f, "        { const T p = V[%d] * E[%d];", pr.i, pr.j);
@@ -87,8 +83,8 @@ static void emit(FILE* f, int L) {
         fprintf(f, "    }\n");
         // ---------------- backward: gV assigned, gE accumulated
         fprintf(f, "    // %s VJP: cotangent G -> gV (assigned, if WANT_GV) and gE (accumulated)\n", pf ? "per-path" : "folded");
-        fprintf(f, "    template <typename T, bool WANT_GV> static __device__ __forceinline__ void bwd%s(const T (&V)[%d], const T (&E)[%d], const T (&G)[%d], T (&gV)[%d], T (&gE)[%d]) {\n",
-                sfx, t.dV, t.dE, DO, t.dV, t.dE);
+        fprintf(f, "    template <typename T, bool WANT_GV> static __device__ __forceinline__ void bwd%s(%sconst T (&V)[%d], const T (&E)[%d], const T (&G)[%d], T (&gV)[%d], T (&gE)[%d]) {\n",
+                sfx, cwarg, t.dV, t.dE, DO, t.dV, t.dE);
         std::vector<char> tv(t.dV, 0);
         for (const Pair& pr : pairs) {
             fprintf(f, "        { T s = %s * G[%d];", coef(pf, pr.terms[0]).c_str(), pr.terms[0].k);
@@ -124,9 +120,6 @@ static void emit(FILE* f, int L) {
         }
         fprintf(f, "    }\n");
     }
-    // ---------------- per-non-zero tables for the fold kernel (combined tensor = path weight x CG): device arrays
-    fprintf(f, "    static __device__ __forceinline__ int zpath(int z) { return tpgen_zpath_%d[z]; }\n", L);
-    fprintf(f, "    static __device__ __forceinline__ double zcoef(int z) { return tpgen_zcoef_%d[z]; }\n", L);
     // ---------------- small integer tables for the dense mix
     fprintf(f, "    // t-slot offset of each path, and the out block it mixes into\n");
     fprintf(f, "    static __host__ __device__ constexpr int toff(int p) { constexpr int v[%d] = {", P + 1);
@@ -190,7 +183,7 @@ int main(int argc, char** argv) {
     FILE* f = fopen(path.c_str(), "w");
     if (!f) { perror("fopen"); return 1; }
     fprintf(f, "// GENERATED by gen_tp.cpp from the plan tables of plan.cpp -- do not edit, not committed.\n");
-    fprintf(f, "// The including file defines ALLEGRO_CW(z): folded coefficient z (constant memory).\n#pragma once\n");
+    fprintf(f, "#pragma once\n");
     fprintf(f, "template <int L> struct TPGen;\n");
     for (int L = 1; L <= 3; ++L) emit(f, L);
     fprintf(f, "\n// per-path functions (dense mix), l_max <= 2\ntemplate <int L, int PTH> struct TPPath;\n");

@@ -4,7 +4,6 @@
 #error "compile with -DALLEGRO_MIX3_PART=0|1"
 #endif
 #include "common.cuh"
-#define ALLEGRO_CW(z) T(0) /* the folded-coefficient flavour is not used here */
 #include "generated/tp_gen.cuh"
 #include "mix3_kernels.cuh"
 
@@ -27,35 +26,60 @@ static allegro_status_t mix3_images(const TpArgs& a, float** img_f, float** img_
     return ALLEGRO_OK;
 }
 
+// which compiled path subset serves the plan's block masks: 0 = all paths, 1 = the paths into the 0e scalars,
+// 2 = the paths from the natural-parity input blocks (0e, 1o, 2e), -1 = none
+static int mix3_variant(const allegro_plan* plan) {
+    const unsigned o = plan->out_blocks & 0x3fu, i = plan->in_blocks & 0x3fu;
+    return (i == 0x3fu && o == 0x3fu) ? 0 : (i == 0x3fu && o == 0x1u) ? 1 : (i == 0x19u && o == 0x3fu) ? 2 : -1;
+}
+static allegro_status_t mix3_unsupported(const allegro_plan* plan) {
+    set_error("dense tensor product: block masks in 0x%x / out 0x%x are not built (all / all, all / 0x1, 0x19 / all)", plan->in_blocks & 0x3fu,
+              plan->out_blocks & 0x3fu);
+    return ALLEGRO_EUNSUPPORTED;
+}
+
 #if ALLEGRO_MIX3_PART == 0
-allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a) {
-    float *img_f, *img_b;
-    allegro_status_t s = mix3_images(a, &img_f, &img_b);
-    if (s != ALLEGRO_OK) return s;
-    auto k = mix3_fwd_kernel<0>;
-    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3::SMEM));
-    k<<<(unsigned)a.n_items, Mix3::CT + 64, Mix3::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out);
+template <uint32_t PMASK>
+static allegro_status_t mix3_fwd_launch(const TpArgs& a, const float* img_f) {
+    auto k = mix3_fwd_kernel<PMASK>;
+    constexpr int SMEM = Mix3Seq<PMASK>::SMEM;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
+    k<<<(unsigned)a.n_items, Mix3::CT + 64, SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
-#else
-allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item) {
+allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a) {
+    const int var = mix3_variant(a.plan);
+    if (var < 0) return mix3_unsupported(a.plan);
     float *img_f, *img_b;
     allegro_status_t s = mix3_images(a, &img_f, &img_b);
     if (s != ALLEGRO_OK) return s;
-    if (a.gV) {
-        auto k = mix3_bwd_kernel<true>;
-        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
-        k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
-                                                                    img_b, (float*)a.gV, gE_dst, gE_by_item);
-    } else {
-        auto k = mix3_bwd_kernel<false>;
-        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
-        k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv,
-                                                                    img_b, nullptr, gE_dst, gE_by_item);
-    }
+    return var == 0 ? mix3_fwd_launch<Mix3::ALL>(a, img_f)
+           : var == 1 ? mix3_fwd_launch<Mix3::mask_into(0)>(a, img_f)
+                      : mix3_fwd_launch<Mix3::mask_natural_in()>(a, img_f);
+}
+#else
+template <bool GV, uint32_t PMASK>
+static allegro_status_t mix3_bwd_launch(const TpArgs& a, const float* img_b, float* gE_dst, int gE_by_item) {
+    auto k = mix3_bwd_kernel<GV, PMASK>;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
+    k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv, img_b,
+                                                                (float*)a.gV, gE_dst, gE_by_item);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
+}
+allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item) {
+    const int var = mix3_variant(a.plan);
+    if (var < 0) return mix3_unsupported(a.plan);
+    float *img_f, *img_b;
+    allegro_status_t s = mix3_images(a, &img_f, &img_b);
+    if (s != ALLEGRO_OK) return s;
+    if (var == 0) return a.gV ? mix3_bwd_launch<true, Mix3::ALL>(a, img_b, gE_dst, gE_by_item) : mix3_bwd_launch<false, Mix3::ALL>(a, img_b, gE_dst, gE_by_item);
+    if (var == 1)
+        return a.gV ? mix3_bwd_launch<true, Mix3::mask_into(0)>(a, img_b, gE_dst, gE_by_item)
+                    : mix3_bwd_launch<false, Mix3::mask_into(0)>(a, img_b, gE_dst, gE_by_item);
+    return a.gV ? mix3_bwd_launch<true, Mix3::mask_natural_in()>(a, img_b, gE_dst, gE_by_item)
+                : mix3_bwd_launch<false, Mix3::mask_natural_in()>(a, img_b, gE_dst, gE_by_item);
 }
 #endif
 

@@ -4,18 +4,7 @@
 #ifndef ALLEGRO_T
 #error "compile with -DALLEGRO_T=float|double -DALLEGRO_L=1|2|3"
 #endif
-#include <cstdlib>
-
 #include "common.cuh"
-
-namespace allegro {
-constexpr int kCwMax = 1222;  // nnz of the l_max = 3 plan
-// Folded coefficient table Wc[z] = path_w[path(z)] * C_z of the call in flight.  Constant memory, so every
-// coefficient is a constant-bank operand of its FFMA/DFMA (no register, no load instruction).
-__constant__ ALLEGRO_T c_cw[kCwMax];
-__device__ ALLEGRO_T g_cw_stage[kCwMax];  // fold_kernel writes here; copied device-to-device into c_cw on the stream
-}  // namespace allegro
-#define ALLEGRO_CW(z) ::allegro::c_cw[z]
 #include "generated/tp_gen.cuh"
 #include "tp_kernels.cuh"
 #include "mix_kernels.cuh"
@@ -29,7 +18,7 @@ template <typename T> struct Cfg {
 };
 
 // Ring depth: as many stages as fit (<= 4) with two CTAs per SM; if that leaves fewer than 3, one CTA per SM
-// with up to 6 stages.  `extra` = barriers + reduction scratch.  ALLEGRO_NST overrides (experiments).
+// with up to 6 stages.  `extra` = barriers + reduction scratch.
 static inline int pick_stages(size_t stage_bytes, size_t extra) {
     const size_t cap2 = 113 * 1024, cap1 = 226 * 1024;
     int nst = 1;
@@ -37,20 +26,20 @@ static inline int pick_stages(size_t stage_bytes, size_t extra) {
     if (nst == 1) {
         for (int k : {6, 4, 3, 2}) if (k * stage_bytes + extra <= cap1) { nst = k; break; }
     }
-    if (const char* e = getenv("ALLEGRO_NST")) {
-        const int k = atoi(e);
-        if (k >= 1 && k <= 6 && k * stage_bytes + extra <= cap1) nst = k;
-    }
     return nst;
 }
 
+// the plan's folded coefficient table as a kernel parameter (bound by allegro_plan_bind_weights or by the call itself)
 template <typename T>
-static allegro_status_t fold_weights(const TpArgs& a) {
-    T* stage = nullptr;
-    ALLEGRO_CUDA(cudaGetSymbolAddress((void**)&stage, g_cw_stage));
-    fold_kernel<T, ALLEGRO_L><<<(Gen::NNZ + 127) / 128, 128, 0, a.st>>>((const T*)a.path_w, stage);
-    ALLEGRO_LAUNCHED();
-    ALLEGRO_CUDA(cudaMemcpyToSymbolAsync(c_cw, stage, sizeof(T) * Gen::NNZ, 0, cudaMemcpyDeviceToDevice, a.st));
+static allegro_status_t folded_table(const TpArgs& a, CwTab<T, Gen::NNZ>& tab) {
+    if (a.path_w != nullptr) {
+        allegro_status_t s = bind_scalar_weights(a.plan, a.path_w, a.st);
+        if (s != ALLEGRO_OK) return s;
+    } else if (!a.plan->cw_bound) {
+        set_error("tensor product (scalar weights): path_w is NULL and no weights are bound to the plan (allegro_plan_bind_weights)");
+        return ALLEGRO_EINVAL;
+    }
+    for (int z = 0; z < Gen::NNZ; ++z) tab.v[z] = (T)a.plan->cw[z];
     return ALLEGRO_OK;
 }
 
@@ -70,7 +59,8 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     }
     if (a.n_items == 0) return ALLEGRO_OK;
     if (a.plan->wmode == ALLEGRO_W_DENSE) return launch_mix_forward<T>(a);
-    allegro_status_t s = fold_weights<T>(a);
+    CwTab<T, Gen::NNZ> cwt;
+    allegro_status_t s = folded_table<T>(a, cwt);
     if (s != ALLEGRO_OK) return s;
     const int nslots = TH / a.n;
     const size_t tile = align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
@@ -83,7 +73,7 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     {                                                                                                              \
         auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, WO, WG, WE>;                                                      \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                       \
-        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(nst, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, nst, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
                                                         (const T*)a.q, (T)a.kappa, (T*)a.e_edge, (T*)a.Gout);      \
     }
     if (w_out && !w_g && !w_e) { ALLEGRO_FWD(true, false, false) }
@@ -131,7 +121,8 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
         return ALLEGRO_OK;
     }
     if (a.plan->wmode == ALLEGRO_W_DENSE) return launch_mix_backward<T>(a);
-    allegro_status_t s = fold_weights<T>(a);
+    CwTab<T, Gen::NNZ> cwt;
+    allegro_status_t s = folded_table<T>(a, cwt);
     if (s != ALLEGRO_OK) return s;
     unsigned char* ws = (unsigned char*)a.ws;
     T* gE_part = nullptr;
@@ -149,7 +140,7 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     {                                                                                                                     \
         auto k = tp_bwd_kernel<T, ALLEGRO_L, TH, GV, GW, COT>;                                                            \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                              \
-        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(nst, a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, nst, a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
                                                         (const T*)a.q, (T)a.kappa, (T*)a.gV, gE_dst, have_items ? 1 : 0, gw_part); \
     }
     const bool want_gv = a.gV != nullptr;

@@ -106,10 +106,8 @@ allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, cons
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st);
 
-// dense per-path mix, version 2 (inst_mix2.cu, three parts)
-allegro_status_t launch_mix2_forward_f32_l2_n64(const TpArgs& a);
-allegro_status_t launch_mix2_backward_gv_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
-allegro_status_t launch_mix2_backward_nogv_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item);
+// scalar path weights: fold path_w (DEVICE, [P]) with the CG table into plan->cw on the host (api.cu); synchronises the stream
+allegro_status_t bind_scalar_weights(const allegro_plan* plan, const void* path_w_dev, cudaStream_t st);
 
 // dense per-path mix on tcgen05 (inst_mix3.cu)
 allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a);

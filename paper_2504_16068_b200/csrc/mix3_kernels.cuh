@@ -41,24 +41,88 @@ __device__ __forceinline__ void static_for3(F&& f) {
 struct Mix3 {
     static constexpr int N = 64, L = 2, DV = 18, DE = 9, P = 30;
     static constexpr int TE = 24, NSLOT = 6, EPS = 4;            // tile edges = 6 slots x 4 consecutive edges
-    static constexpr int CT = 384;                                // compute threads (12 warps, 128 registers each); + 1 control warp
+    static constexpr int CT = 384;                                // compute threads (12 warps, 128 registers each); + 2 control warps
     static constexpr int A_BYTES = 2 * 128 * 128;                 // [2 K-atoms][128 rows][128 B]
-    static constexpr int BV_BYTES = 2 * 128 * 128;                // one B variant (hi or lo): [2 K-atoms][<=128 rows][128 B]
-    static constexpr int B_BYTES = 2 * BV_BYTES;
     static constexpr int NA = 3, NB = 2;                          // ring depths
     static constexpr int IMG_BYTES = 2 * 128 * 128;               // one path's weight image in global memory (hi and lo rows)
-    static constexpr int OFF_A = 0, OFF_B = NA * A_BYTES, OFF_BAR = OFF_B + NB * B_BYTES;
-    static constexpr int SMEM = OFF_BAR + 256 + 1024;             // + barrier block + 1024-byte alignment slack
+    static constexpr uint32_t ALL = 0x3fffffffu;                  // path mask: every path of the plan
     // TMEM column base of each output block, indexed by off3 (0e:0, 0o:1, 1e:2, 1o:5, 2e:8, 2o:13); N_b = 32 / 80 / 128
     __host__ __device__ static constexpr int dcol(int off3) {
         return off3 == 0 ? 0 : off3 == 1 ? 32 : off3 == 2 ? 64 : off3 == 5 ? 144 : off3 == 8 ? 224 : 352;
     }
-    // is p the first path (in plan order) that mixes into its output block?
+    __host__ __device__ static constexpr int ncols(int d3) { return d3 == 1 ? 32 : d3 == 3 ? 80 : 128; }
+    // the paths that mix into the output block at component offset off3 (0 = the 0e scalars)
+    __host__ __device__ static constexpr uint32_t mask_into(int off3) {
+        uint32_t m = 0;
+        for (int p = 0; p < P; ++p) if (TPGen<2>::off3(p) == off3) m |= 1u << p;
+        return m;
+    }
+    // (l1, p1) block of V that path p reads: first component (plan order: l1, p1, l2, l3) and width
+    __host__ __device__ static constexpr int off1(int p) {
+        int idx = 0;
+        for (int l1 = 0; l1 <= 2; ++l1)
+            for (int p1 = 0; p1 < 2; ++p1)
+                for (int l2 = 0; l2 <= 2; ++l2)
+                    for (int l3 = (l1 > l2 ? l1 - l2 : l2 - l1); l3 <= (l1 + l2 < 2 ? l1 + l2 : 2); ++l3, ++idx)
+                        if (idx == p) return 2 * l1 * l1 + (p1 ? 2 * l1 + 1 : 0);
+        return -1;
+    }
+    __host__ __device__ static constexpr int d1(int p) { return off1(p) < 2 ? 1 : off1(p) < 8 ? 3 : 5; }
+    // the paths whose input block has its natural parity (l, (-1)^l): 0e, 1o, 2e -- all that a first layer fed with
+    // V0 = v (x) Y(rhat) ever sees non-zero
+    __host__ __device__ static constexpr uint32_t mask_natural_in() {
+        uint32_t m = 0;
+        for (int p = 0; p < P; ++p) if (off1(p) == 0 || off1(p) == 5 || off1(p) == 8) m |= 1u << p;
+        return m;
+    }
+};
+
+// The paths that run (bit p of PMASK), in plan order, as compile-time functions of the sequence index k; shared-memory layout of
+// the forward kernel for that set (a B stage holds as many rows as the widest active block needs).
+template <uint32_t PMASK>
+struct Mix3Seq {
+    __host__ __device__ static constexpr bool active(int p) { return ((PMASK >> p) & 1u) != 0; }
+    __host__ __device__ static constexpr int count() {
+        int n = 0;
+        for (int p = 0; p < 30; ++p) n += active(p) ? 1 : 0;
+        return n;
+    }
+    __host__ __device__ static constexpr int path(int k) {
+        int n = 0;
+        for (int p = 0; p < 30; ++p) if (active(p)) { if (n == k) return p; ++n; }
+        return -1;
+    }
+    // is p the first active path (in plan order) that mixes into its output block?
     __host__ __device__ static constexpr bool first_of_block(int p) {
-        for (int r = 0; r < p; ++r) if (TPGen<2>::off3(r) == TPGen<2>::off3(p)) return false;
+        for (int r = 0; r < p; ++r) if (active(r) && TPGen<2>::off3(r) == TPGen<2>::off3(p)) return false;
         return true;
     }
-    __host__ __device__ static constexpr int ncols(int d3) { return d3 == 1 ? 32 : d3 == 3 ? 80 : 128; }
+    __host__ __device__ static constexpr bool block_active(int off3) {
+        for (int p = 0; p < 30; ++p) if (active(p) && TPGen<2>::off3(p) == off3) return true;
+        return false;
+    }
+    __host__ __device__ static constexpr int max_d3() {
+        int m = 1;
+        for (int p = 0; p < 30; ++p) if (active(p) && TPGen<2>::d3(p) > m) m = TPGen<2>::d3(p);
+        return m;
+    }
+    static constexpr int ATOM = Mix3::ncols(max_d3()) * 128;       // one K-atom of a B variant: [rows][128 B]
+    static constexpr int BV_BYTES = 2 * ATOM, B_BYTES = 2 * BV_BYTES;   // B stage: [hi, lo][2 K-atoms][rows][128 B]
+    // The epilogue stages `out` rows in B stage 1 when they fit there (the stage is idle from the last MMA of a tile until the
+    // first path of the next tile that is written into it); small B stages leave room for a staging area of its own.
+    static constexpr int STG_BYTES = (Mix3::CT / 32) * 4 * 16 * Mix3::DV * 4;
+    static constexpr bool ALIAS_STG = STG_BYTES <= B_BYTES;
+    static constexpr int OFF_A = 0, OFF_B = Mix3::NA * Mix3::A_BYTES, OFF_STG = OFF_B + Mix3::NB * B_BYTES;
+    static constexpr int OFF_BAR = OFF_STG + (ALIAS_STG ? 0 : STG_BYTES);
+    static constexpr int SMEM = OFF_BAR + 256 + 1024;             // + barrier block + 1024-byte alignment slack
+    static_assert(count() >= 2, "at least two paths");
+};
+
+// position in a ring of NST stages: stage index and the phase bit of the current turn
+template <int NST>
+struct RingPos {
+    uint32_t s = 0, ph = 0;
+    __device__ __forceinline__ void next() { if (++s == NST) { s = 0; ph ^= 1u; } }
 };
 
 // Weight images: img_f[p] feeds the forward (A row = output channel n', K = input channel n), img_b[p] the VJP
@@ -89,16 +153,17 @@ struct Mix3Bars {
 
 __device__ __forceinline__ float tf32_lo(float x) { return x - __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 
-template <int DUMMY = 0>
+template <uint32_t PMASK>
 __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                    const float* __restrict__ V, const float* __restrict__ Eenv,
                                                                    const float* __restrict__ img, float* __restrict__ out) {
     using M3 = Mix3;
+    using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
-    constexpr int DV = M3::DV, DE = M3::DE, P = M3::P, TE = M3::TE;
+    constexpr int DV = M3::DV, DE = M3::DE, NP = SQ::count(), TE = M3::TE;
     extern __shared__ unsigned char smem_raw[];
     unsigned char* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned (128-byte swizzle atoms)
-    Mix3Bars* bars = reinterpret_cast<Mix3Bars*>(sm + M3::OFF_BAR);
+    Mix3Bars* bars = reinterpret_cast<Mix3Bars*>(sm + SQ::OFF_BAR);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
@@ -121,57 +186,61 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
     if (warp >= M3::CT / 32) {
         // ================= two control warps (one thread each, so that neither spins inside the other's warp): weight images (TMA), MMA issue
         if (warp == M3::CT / 32 && lane == 0) {
+            RingPos<M3::NA> ra;
             for (int t = 0; t < ntiles; ++t) {
-                for (int p = 0; p < P; ++p) {
-                    const int sa = p % M3::NA;                                   // 30 paths per tile = 10 ring turns: stage and
-                    const uint32_t ph = (uint32_t)(p / M3::NA) & 1u;             // parity depend on p only
+                static_for3<0, NP>([&](auto kc) {
+                    constexpr int p = SQ::path(decltype(kc)::value);
                     MIX3_T0();
-                    mbar_wait(&bars->a_empty[sa], ph ^ 1u);
+                    mbar_wait(&bars->a_empty[ra.s], ra.ph ^ 1u);
                     MIX3_ACC(3, blockIdx.x == 0);
-                    mbar_expect_tx(&bars->a_full[sa], M3::IMG_BYTES);
-                    bulk_load(sm + M3::OFF_A + sa * M3::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * M3::IMG_BYTES,
-                              M3::IMG_BYTES, &bars->a_full[sa]);
-                }
+                    mbar_expect_tx(&bars->a_full[ra.s], M3::IMG_BYTES);
+                    bulk_load(sm + SQ::OFF_A + ra.s * M3::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * M3::IMG_BYTES,
+                              M3::IMG_BYTES, &bars->a_full[ra.s]);
+                    ra.next();
+                });
             }
         } else if (warp == M3::CT / 32 + 1) {   // the whole warp walks the loop; one elected lane issues
             constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 32);
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 128);
             // descriptors of K step 0 of every ring stage; K step j adds (j >> 2) * 16384 + (j & 3) * 32 bytes (16-byte units)
-            const uint32_t adesc0 = tc05::sdesc_lo(smem_u32(sm + M3::OFF_A)), bdesc0 = tc05::sdesc_lo(smem_u32(sm + M3::OFF_B));
+            const uint32_t adesc0 = tc05::sdesc_lo(smem_u32(sm + SQ::OFF_A)), bdesc0 = tc05::sdesc_lo(smem_u32(sm + SQ::OFF_B));
+            RingPos<M3::NA> ra;
+            RingPos<M3::NB> rb;
             for (int t = 0; t < ntiles; ++t) {
                 MIX3_T0();
                 if (t > 0) { mbar_wait(&bars->d_empty, (uint32_t)(t - 1) & 1u); tc05::fence_after_sync(); }
                 MIX3_ACC(2, blockIdx.x == 0 && lane == 0);
-                static_for3<0, P>([&](auto pc) {
-                    constexpr int p = decltype(pc)::value;
-                    constexpr int sa = p % M3::NA, sb = p & 1;
+                static_for3<0, NP>([&](auto kc) {
+                    constexpr int k = decltype(kc)::value;
+                    constexpr int p = SQ::path(k);
                     constexpr int d3 = Gen::d3(p), off3 = Gen::off3(p);
                     constexpr uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
-                    constexpr bool first = M3::first_of_block(p);   // first path of its output block: initialises the accumulator
-                    const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;          // 15 B-ring turns per tile
-                    mbar_wait(&bars->a_full[sa], (uint32_t)(p / M3::NA) & 1u);
-                    mbar_wait(&bars->b_full[sb], phb);
+                    constexpr bool first = SQ::first_of_block(p);   // first path of its output block: initialises the accumulator
+                    mbar_wait(&bars->a_full[ra.s], ra.ph);
+                    mbar_wait(&bars->b_full[rb.s], rb.ph);
                     MIX3_ACC(0, blockIdx.x == 0 && lane == 0);
                     tc05::fence_after_sync();
                     const uint32_t dcol = tbase + (uint32_t)M3::dcol(off3);
                     if (tc05::elect_one()) {
-                    uint32_t ad = adesc0 + (uint32_t)((sa * M3::A_BYTES) >> 4), bd = bdesc0 + (uint32_t)((sb * M3::B_BYTES) >> 4);
+                    uint32_t ad = adesc0 + ((ra.s * (uint32_t)M3::A_BYTES) >> 4), bd = bdesc0 + ((rb.s * (uint32_t)SQ::B_BYTES) >> 4);
                     asm volatile("" : "+r"(ad), "+r"(bd));   // opaque per path: keeps the descriptor words from being hoisted and spilled
 #pragma unroll
                     for (int v = 0; v < 2; ++v)          // B variant: hi, lo
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {    // K step of 8 channels
-                            const uint32_t koff = (uint32_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
-                            tc05::mma_tf32_lo(dcol, ad + koff, bd + (uint32_t)((v * M3::BV_BYTES) >> 4) + koff, tc05::kSdescHiSw128, idesc,
-                                              (first && v == 0 && j == 0) ? 0u : 1u);
+                            const uint32_t aoff = (uint32_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
+                            const uint32_t boff = (uint32_t)((v * SQ::BV_BYTES + (j >> 2) * SQ::ATOM + (j & 3) * 32) >> 4);
+                            tc05::mma_tf32_lo(dcol, ad + aoff, bd + boff, tc05::kSdescHiSw128, idesc, (first && v == 0 && j == 0) ? 0u : 1u);
                         }
-                    tc05::mma_commit(&bars->b_empty[sb]);
-                    tc05::mma_commit(&bars->a_empty[sa]);
-                    if (p == P - 1) tc05::mma_commit(&bars->d_full);
+                    tc05::mma_commit(&bars->b_empty[rb.s]);
+                    tc05::mma_commit(&bars->a_empty[ra.s]);
+                    if (k == NP - 1) tc05::mma_commit(&bars->d_full);
                     }
                     __syncwarp();
                     MIX3_ACC(1, blockIdx.x == 0 && lane == 0);
+                    ra.next();
+                    rb.next();
                 });
             }
         }
@@ -188,11 +257,13 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
 #pragma unroll
         for (int j = 0; j < M3::EPS; ++j) {
             const uint32_t e = 4u * slot + j, r = e & 7u;
-            boff[j] = (uint32_t)(ch >> 5) * 16384u + (e >> 3) * 1024u + r * 128u + (((((uint32_t)ch & 31u) >> 2) ^ r) << 4) + (((uint32_t)ch & 3u) << 2);
+            boff[j] = (uint32_t)(ch >> 5) * (uint32_t)SQ::ATOM + (e >> 3) * 1024u + r * 128u + (((((uint32_t)ch & 31u) >> 2) ^ r) << 4) + (((uint32_t)ch & 3u) << 2);
         }
         const int q = warp & 3, wq = warp >> 2, h = lane >> 4, nl = lane & 15;
+        RingPos<M3::NB> rb;
         for (int t = 0; t < ntiles; ++t) {
             const int eb = e0 + t * TE;
+            bool stg_busy = t > 0;
             MIX3_T0();
             float Vr[M3::EPS][DV];
 #pragma unroll
@@ -205,16 +276,17 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
                     for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
                 }
             }
-            static_for3<0, P>([&](auto pc) {
-                constexpr int p = decltype(pc)::value;
+            static_for3<0, NP>([&](auto kc) {
+                constexpr int k = decltype(kc)::value;
+                constexpr int p = SQ::path(k);
                 using Pth = TPPath<2, p>;
-                constexpr int sa = p % M3::NA, sb = p & 1;
-                const uint32_t phb = (uint32_t)(t + (p >> 1)) & 1u;
-                unsigned char* Bs = sm + M3::OFF_B + sb * M3::B_BYTES;
-                // B: t_p of this thread's three edges, hi (raw) and lo
-                MIX3_ACC(10, blockIdx.x == 0 && tid == 0 && p == 0);
-                mbar_wait(&bars->b_empty[sb], phb ^ 1u);
-                if (p == 1 && t > 0) asm volatile("bar.sync 1, %0;" ::"n"(2 * M3::CT) : "memory");
+                unsigned char* Bs = sm + SQ::OFF_B + rb.s * SQ::B_BYTES;
+                // B: t_p of this thread's four edges, hi (raw) and lo
+                MIX3_ACC(10, blockIdx.x == 0 && tid == 0 && k == 0);
+                mbar_wait(&bars->b_empty[rb.s], rb.ph ^ 1u);
+                if constexpr (SQ::ALIAS_STG) {   // first write of this tile into B stage 1, where the epilogue staged the previous tile's rows
+                    if (stg_busy && rb.s == 1) { asm volatile("bar.sync 1, %0;" ::"n"(2 * M3::CT) : "memory"); stg_busy = false; }
+                }
                 MIX3_ACC(4, blockIdx.x == 0 && tid == 0);
                 // launder E so that V.E products are not kept alive (common subexpressions) from one path to the next
 #pragma unroll
@@ -227,13 +299,14 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
                     for (int M = 0; M < Pth::D3; ++M) {
                         unsigned char* dst = Bs + boff[i] + 3 * M * 1024;
                         *reinterpret_cast<float*>(dst) = tp[M];
-                        *reinterpret_cast<float*>(dst + M3::BV_BYTES) = tf32_lo(tp[M]);
+                        *reinterpret_cast<float*>(dst + SQ::BV_BYTES) = tf32_lo(tp[M]);
                     }
                 }
                 MIX3_ACC(5, blockIdx.x == 0 && tid == 0);
                 fence_proxy_async();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&bars->b_full[sb]);
+                if (lane == 0) mbar_arrive(&bars->b_full[rb.s]);
+                rb.next();
                 MIX3_ACC(7, blockIdx.x == 0 && tid == 0);
             });
             // ---- epilogue: TMEM lane (n', h) -> out rows; warp (q, wq) takes edges 8 wq .. 8 wq + 7, lane h its half of them
@@ -242,7 +315,7 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
             tc05::fence_after_sync();
             // Rows are staged through shared memory (B stage 1 is idle until path 1 of the next tile) so that they leave as
             // fully coalesced 16-byte stores: per warp a private [4 edges][16 channels][18] block, two half-tiles in turn.
-            float* stg = reinterpret_cast<float*>(sm + M3::OFF_B + M3::B_BYTES) + warp * (4 * 16 * DV);
+            float* stg = reinterpret_cast<float*>(sm + (SQ::ALIAS_STG ? SQ::OFF_B + SQ::B_BYTES : SQ::OFF_STG)) + warp * (4 * 16 * DV);
             const uint32_t trow = tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(8 * wq);
 #pragma unroll
             for (int hf = 0; hf < 2; ++hf) {     // edges 8 wq + 4 hf + {0..3}: lane half h finalises edges 2 h, 2 h + 1 of them
@@ -251,18 +324,23 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
                     constexpr int b = decltype(bc)::value;
                     constexpr int off3 = b == 0 ? 0 : b == 1 ? 1 : b == 2 ? 2 : b == 3 ? 5 : b == 4 ? 8 : 13;
                     constexpr int d3 = b < 2 ? 1 : b < 4 ? 3 : 5;
-                    uint32_t v[d3][4];
+                    if constexpr (SQ::block_active(off3)) {
+                        uint32_t v[d3][4];
 #pragma unroll
-                    for (int M = 0; M < d3; ++M) tc05::tmem_ld4(trow + (uint32_t)(M3::dcol(off3) + M * TE + 4 * hf), v[M]);
-                    tc05::tmem_ld_wait();
+                        for (int M = 0; M < d3; ++M) tc05::tmem_ld4(trow + (uint32_t)(M3::dcol(off3) + M * TE + 4 * hf), v[M]);
+                        tc05::tmem_ld_wait();
 #pragma unroll
-                    for (int M = 0; M < d3; ++M)
+                        for (int M = 0; M < d3; ++M)
 #pragma unroll
-                        for (int i = 0; i < 2; ++i) {
-                            const float mine = __uint_as_float(h ? v[M][2 + i] : v[M][i]);
-                            const float send = __uint_as_float(h ? v[M][i] : v[M][2 + i]);
-                            o[i][off3 + M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
-                        }
+                            for (int i = 0; i < 2; ++i) {
+                                const float mine = __uint_as_float(h ? v[M][2 + i] : v[M][i]);
+                                const float send = __uint_as_float(h ? v[M][i] : v[M][2 + i]);
+                                o[i][off3 + M] = mine + __shfl_xor_sync(0xffffffffu, send, 16);
+                            }
+                    } else {   // no path into this block runs: its components are zeros
+#pragma unroll
+                        for (int M = 0; M < d3; ++M) { o[0][off3 + M] = 0.f; o[1][off3 + M] = 0.f; }
+                    }
                 });
                 if (hf == 1) {   // all TMEM reads of this warp are done: the accumulators may be overwritten
                     tc05::fence_before_sync();
@@ -281,7 +359,7 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
                 }
                 __syncwarp();
             }
-            asm volatile("bar.arrive 1, %0;" ::"n"(2 * M3::CT) : "memory");   // staging done; waited for before B stage 1 is rewritten
+            if constexpr (SQ::ALIAS_STG) asm volatile("bar.arrive 1, %0;" ::"n"(2 * M3::CT) : "memory");   // staging done; waited for before B stage 1 is rewritten
             MIX3_ACC(9, blockIdx.x == 0 && tid == 0);
         }
     }
@@ -312,25 +390,8 @@ struct Mix3B {
     }
     // TMEM columns: accumulator ring at 0, 80, 160; the V rows of a thread's four pairs (72 columns per warp row wq) at 320 ..
     static constexpr int VCOL = 320;
-    // (l1, p1) block of V that path p reads: first component and width
-    __host__ __device__ static constexpr int off1(int p) {
-        int idx = 0;
-        for (int l1 = 0; l1 <= 2; ++l1)
-            for (int p1 = 0; p1 < 2; ++p1)
-                for (int l2 = 0; l2 <= 2; ++l2)
-                    for (int l3 = (l1 > l2 ? l1 - l2 : l2 - l1); l3 <= (l1 + l2 < 2 ? l1 + l2 : 2); ++l3, ++idx)
-                        if (idx == p) return 2 * l1 * l1 + (p1 ? 2 * l1 + 1 : 0);
-        return -1;
-    }
-    __host__ __device__ static constexpr int d1(int p) {
-        int idx = 0;
-        for (int l1 = 0; l1 <= 2; ++l1)
-            for (int p1 = 0; p1 < 2; ++p1)
-                for (int l2 = 0; l2 <= 2; ++l2)
-                    for (int l3 = (l1 > l2 ? l1 - l2 : l2 - l1); l3 <= (l1 + l2 < 2 ? l1 + l2 : 2); ++l3, ++idx)
-                        if (idx == p) return 2 * l1 + 1;
-        return -1;
-    }
+    __host__ __device__ static constexpr int off1(int p) { return Mix3::off1(p); }
+    __host__ __device__ static constexpr int d1(int p) { return Mix3::d1(p); }
     // component k of a feature row -> row of the (M = 0, e = 0) element of its block + 16 M
     __host__ __device__ static constexpr int comprow(int k) {
         return k == 0 ? 0 : k == 1 ? 16 : k < 5 ? 32 + 16 * (k - 2) : k < 8 ? 80 + 16 * (k - 5) : k < 13 ? 128 + 16 * (k - 8) : 208 + 16 * (k - 13);
@@ -341,14 +402,15 @@ struct Mix3BBars {
     uint32_t tmem_slot;
 };
 
-template <bool WANT_GV>
+template <bool WANT_GV, uint32_t PMASK>
 __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                     const float* __restrict__ G, const float* __restrict__ V,
                                                                     const float* __restrict__ Eenv, const float* __restrict__ img,
                                                                     float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
     using MB = Mix3B;
+    using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
-    constexpr int DV = MB::DV, DE = MB::DE, P = MB::P, TE = MB::TE;
+    constexpr int DV = MB::DV, DE = MB::DE, NP = SQ::count(), TE = MB::TE;
     extern __shared__ unsigned char smem_raw[];
     unsigned char* sm = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
     Mix3BBars* bars = reinterpret_cast<Mix3BBars*>(sm + MB::OFF_BAR);
@@ -372,48 +434,51 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
     if (warp >= MB::CT / 32) {
         if (warp == MB::CT / 32 && lane == 0) {
             // ---- weight images (TMA)
+            RingPos<MB::NA> ra;
             for (int t = 0; t < ntiles; ++t)
-                for (int p = 0; p < P; ++p) {
-                    const int sa = p & 1;
-                    const uint32_t ph = (uint32_t)(t + (p >> 1)) & 1u;            // 15 ring turns per tile
-                    mbar_wait(&bars->a_empty[sa], ph ^ 1u);
-                    mbar_expect_tx(&bars->a_full[sa], Mix3::IMG_BYTES);
-                    bulk_load(sm + MB::OFF_A + sa * MB::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * Mix3::IMG_BYTES,
-                              Mix3::IMG_BYTES, &bars->a_full[sa]);
-                }
+                static_for3<0, NP>([&](auto kc) {
+                    constexpr int p = SQ::path(decltype(kc)::value);
+                    mbar_wait(&bars->a_empty[ra.s], ra.ph ^ 1u);
+                    mbar_expect_tx(&bars->a_full[ra.s], Mix3::IMG_BYTES);
+                    bulk_load(sm + MB::OFF_A + ra.s * MB::A_BYTES, reinterpret_cast<const unsigned char*>(img) + (size_t)p * Mix3::IMG_BYTES,
+                              Mix3::IMG_BYTES, &bars->a_full[ra.s]);
+                    ra.next();
+                });
         } else if (warp == MB::CT / 32 + 1) {
             // ---- MMA issue: the whole warp walks the loop, one elected lane issues
             constexpr uint32_t id1 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 16);
             constexpr uint32_t id3 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 48);
             constexpr uint32_t id5 = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 80);
             const uint32_t adesc0 = tc05::sdesc_lo(smem_u32(sm + MB::OFF_A)), gdesc0 = tc05::sdesc_lo(smem_u32(sm + MB::OFF_G));
+            RingPos<MB::NA> ra;
+            RingPos<MB::ND> rd;
             for (int t = 0; t < ntiles; ++t) {
                 mbar_wait(&bars->g_full, (uint32_t)t & 1u);
-                static_for3<0, P>([&](auto pc) {
-                    constexpr int p = decltype(pc)::value;
-                    constexpr int sa = p & 1;
+                static_for3<0, NP>([&](auto kc) {
+                    constexpr int p = SQ::path(decltype(kc)::value);
                     constexpr int d3 = Gen::d3(p), off3 = Gen::off3(p);
                     constexpr uint32_t idesc = d3 == 1 ? id1 : d3 == 3 ? id3 : id5;
-                    constexpr int sd = p % MB::ND;
-                    mbar_wait(&bars->a_full[sa], (uint32_t)(t + (p >> 1)) & 1u);
-                    mbar_wait(&bars->d_empty[sd], ((uint32_t)(p / MB::ND) & 1u) ^ 1u);
+                    mbar_wait(&bars->a_full[ra.s], ra.ph);
+                    mbar_wait(&bars->d_empty[rd.s], rd.ph ^ 1u);
                     tc05::fence_after_sync();
-                    const uint32_t dcol = tbase + sd * 80u;
+                    const uint32_t dcol = tbase + rd.s * 80u;
                     if (tc05::elect_one()) {
-                    uint32_t ad = adesc0, gd = gdesc0;   // opaque per path: otherwise all 112 descriptor words are hoisted out of the loops and spilled
+                    uint32_t ad = adesc0 + ((ra.s * (uint32_t)MB::A_BYTES) >> 4), gd = gdesc0;   // opaque per path: otherwise all descriptor words are hoisted out of the loops and spilled
                     asm volatile("" : "+r"(ad), "+r"(gd));
 #pragma unroll
                     for (int v = 0; v < 2; ++v)
 #pragma unroll
                         for (int j = 0; j < 8; ++j) {
-                            const uint32_t koff = (uint32_t)((sa * MB::A_BYTES + (j >> 2) * 16384 + (j & 3) * 32) >> 4);
+                            const uint32_t koff = (uint32_t)(((j >> 2) * 16384 + (j & 3) * 32) >> 4);
                             const uint32_t goff = (uint32_t)((v * MB::G_VAR + (j >> 2) * MB::G_ATOM + MB::rowoff(off3) * 128 + (j & 3) * 32) >> 4);
                             tc05::mma_tf32_lo(dcol, ad + koff, gd + goff, tc05::kSdescHiSw128, idesc, (v == 0 && j == 0) ? 0u : 1u);
                         }
-                    tc05::mma_commit(&bars->d_full[sd]);
-                    tc05::mma_commit(&bars->a_empty[sa]);
+                    tc05::mma_commit(&bars->d_full[rd.s]);
+                    tc05::mma_commit(&bars->a_empty[ra.s]);
                     }
                     __syncwarp();
+                    ra.next();
+                    rd.next();
                 });
             }
         }
@@ -432,6 +497,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
             const uint32_t e = 4u * slot + j, r = e & 7u;
             goff[j] = (uint32_t)(np >> 5) * MB::G_ATOM + (e >> 3) * 1024u + r * 128u + (((((uint32_t)np & 31u) >> 2) ^ r) << 4) + (((uint32_t)np & 3u) << 2);
         }
+        RingPos<MB::ND> rd;
         for (int t = 0; t < ntiles; ++t) {
             const int eb = e0 + t * TE;
             // (a) cotangent tile -> B operands of all six blocks (hi, lo)
@@ -445,12 +511,15 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
 #pragma unroll
                     for (int k = 0; k < DV; ++k) g[k] = 0.f;
                 }
-#pragma unroll
-                for (int k = 0; k < DV; ++k) {
-                    unsigned char* dst = sm + MB::OFF_G + goff[j] + (MB::comprow(k) / 8) * 1024;
-                    *reinterpret_cast<float*>(dst) = g[k];
-                    *reinterpret_cast<float*>(dst + MB::G_VAR) = tf32_lo(g[k]);
-                }
+                static_for3<0, DV>([&](auto kc) {   // only the blocks some active path reads
+                    constexpr int k = decltype(kc)::value;
+                    constexpr int off3k = k == 0 ? 0 : k == 1 ? 1 : k < 5 ? 2 : k < 8 ? 5 : k < 13 ? 8 : 13;
+                    if constexpr (SQ::block_active(off3k)) {
+                        unsigned char* dst = sm + MB::OFF_G + goff[j] + (MB::comprow(k) / 8) * 1024;
+                        *reinterpret_cast<float*>(dst) = g[k];
+                        *reinterpret_cast<float*>(dst + MB::G_VAR) = tf32_lo(g[k]);
+                    }
+                });
             }
             fence_proxy_async();
             __syncwarp();
@@ -480,12 +549,13 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
             }
             tc05::tmem_st_wait();
             // (c) paths: consume every accumulator as soon as it is complete
-            static_for3<0, P>([&](auto pc) {
-                constexpr int p = decltype(pc)::value;
+            static_for3<0, NP>([&](auto kc) {
+                constexpr int p = SQ::path(decltype(kc)::value);
                 using Pth = TPPath<2, p>;
                 constexpr int d3 = Pth::D3;
-                constexpr int sd = p % MB::ND;
-                mbar_wait(&bars->d_full[sd], (uint32_t)(p / MB::ND) & 1u);
+                const uint32_t sd = rd.s;
+                mbar_wait(&bars->d_full[sd], rd.ph);
+                rd.next();
                 tc05::fence_after_sync();
                 constexpr int o1 = MB::off1(p), w1 = MB::d1(p);
                 uint32_t v[d3][8];

@@ -3,16 +3,15 @@
 //   out[e][n'][off3(p)+M] = sum_p sum_n W[p][n'][n] t[e][n][p][M]
 // and its VJP  gt[e][n][p][M] = sum_n' W[p][n'][n] G[e][n'][off3(p)+M], then the per-path CG VJP with unit weights.
 //
-// First version (round 1): the 64x64 mixes run on the FP32/FP64 FMA pipe with 128-bit shared-memory operands
-// (t never leaves the SM: PAPER.md:71); the tcgen05 / 3xTF32 tensor-core version is the next step.
+// Generic version for any n, fp32 / fp64, l_max <= 2: the n x n mixes run on the FP32/FP64 FMA pipe with 128-bit shared-memory
+// operands (t never leaves the SM: PAPER.md:71).
 // One CTA per item; thread <-> (edge slot, channel).  Per tile of `nsl` edges:
 //   forward : t (DT values per thread) -> shared tS[slot][col][n]; per path p: W_p -> shared Ws[n'][n] (row stride n+4),
 //             acc[off3(p)+M] += <Ws[n'][:], tS[slot][toff(p)+M][:]>; thread (slot, n') stores its out row.
 //   backward: G rows -> shared gS[slot][k][n']; per path p: W_p^T -> shared; gt[toff(p)+M] += <WsT[n][:], gS[slot][off3(p)+M][:]>;
 //             then the generated per-path VJP (gV row stored, gEenv accumulated in registers over the segment).
-// fp32, l_max = 2, n = 64 (configs[2]) is served by the faster version in mix2_kernels.cuh (compiled in inst_mix2.cu).
+// fp32, l_max = 2, n = 64 (configs[2]) is served by the tcgen05 tensor-core version in mix3_kernels.cuh (compiled in inst_mix3.cu).
 #pragma once
-#include <cstdlib>
 #include <type_traits>
 #include <utility>
 
@@ -178,6 +177,11 @@ __global__ void __launch_bounds__(CT) mix_bwd_kernel(int n, const int* __restric
     }
 }
 
+static inline bool all_blocks(const allegro_plan* plan) {
+    const unsigned full = (1u << (2 * (plan->l_max + 1))) - 1u;
+    return (plan->out_blocks & full) == full && (plan->in_blocks & full) == full;
+}
+
 // The dense mode is instantiated for l_max <= 2 (what configs[2] needs): at l_max = 3 a thread would hold 312
 // un-weighted path values, which does not fit the register file.
 #if ALLEGRO_L <= 2
@@ -192,10 +196,13 @@ static allegro_status_t launch_mix_forward(const TpArgs& a) {
     }
 #if ALLEGRO_L == 2
     if constexpr (sizeof(T) == 4) {
-        if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr)
-            return getenv("ALLEGRO_MIX_V2") ? launch_mix2_forward_f32_l2_n64(a) : launch_mix3_forward_f32_l2_n64(a);
+        if (a.n == 64) return launch_mix3_forward_f32_l2_n64(a);
     }
 #endif
+    if (!all_blocks(a.plan)) {
+        set_error("tp_forward (dense): block subsets are built for fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
     const size_t ws_bytes = (size_t)a.n * (a.n + VEC) * sizeof(T);
     const size_t per_slot = (size_t)Gen::DT * a.n * sizeof(T);
     int nsl = CT / a.n;
@@ -244,10 +251,8 @@ static allegro_status_t launch_mix_backward(const TpArgs& a) {
     T* gE_dst = have_items ? (T*)a.ws : (T*)a.gEenv;
 #if ALLEGRO_L == 2
     if constexpr (sizeof(T) == 4) {
-        if (a.n == 64 && getenv("ALLEGRO_MIX_V1") == nullptr) {
-            allegro_status_t s2 = getenv("ALLEGRO_MIX_V2") == nullptr ? launch_mix3_backward_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0)
-                                  : a.gV ? launch_mix2_backward_gv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0)
-                                         : launch_mix2_backward_nogv_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0);
+        if (a.n == 64) {
+            allegro_status_t s2 = launch_mix3_backward_f32_l2_n64(a, (float*)gE_dst, have_items ? 1 : 0);
             if (s2 != ALLEGRO_OK) return s2;
             if (have_items) {
                 combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, (const T*)a.ws, (T*)a.gEenv);
@@ -257,6 +262,10 @@ static allegro_status_t launch_mix_backward(const TpArgs& a) {
         }
     }
 #endif
+    if (!all_blocks(a.plan)) {
+        set_error("tp_backward (dense): block subsets are built for fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
     const int nsl = CT / a.n;
     size_t smem = (size_t)nsl * Gen::DV * a.n * sizeof(T) + (size_t)a.n * (a.n + VEC) * sizeof(T);
     const size_t red = (size_t)CT * Gen::DE * sizeof(T);

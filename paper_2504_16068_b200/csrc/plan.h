@@ -35,5 +35,18 @@ struct allegro_plan {
     int l_max, n, dtype, wmode;
     allegro::PlanTables tab;
     mutable void* dense_img = nullptr;  // device: weight images of the tcgen05 dense mix (inst_mix3.cu), plan-owned
-    // order in which the generated kernels index the folded coefficient table (== tab.nnz order)
+    // output blocks (l3, p3) that are computed: bit b = block b in component order (0e, 0o, 1e, 1o, ...); the others are written as
+    // zeros by the forward and ignored in the cotangent by the VJP (allegro_plan_set_out_blocks)
+    unsigned out_blocks = ~0u;
+    // input blocks (l1, p1) of V that are present: the others are taken as identically zero (not read; their gV is written as
+    // zeros) -- a first layer fed with V0 = v (x) Y(rhat) only has the natural-parity blocks (allegro_plan_set_in_blocks)
+    unsigned in_blocks = ~0u;
+    // scalar mode: the folded coefficient table cw[z] = path_w[path(z)] * C_z of the weights bound last (allegro_plan_bind_weights),
+    // in tab.nnz order, already rounded to the plan's dtype; passed to the kernels BY VALUE as a kernel parameter
+    mutable std::vector<double> cw;
+    mutable bool cw_bound = false;
+    bool path_active(int p) const {
+        const allegro::PathInfo& q = tab.paths[p];
+        return ((out_blocks >> (2 * q.l3 + q.p3)) & 1u) != 0 && ((in_blocks >> (2 * q.l1 + q.p1)) & 1u) != 0;   // parity: 0 even, 1 odd
+    }
 };

@@ -27,16 +27,14 @@
 
 namespace allegro {
 
-static_assert(TPGen<ALLEGRO_L>::NNZ <= kCwMax, "coefficient table too small");
-
-// ------------------------------------------------------------------------------------------------
-// fold: cw[z] = path_w[path(z)] * C_z  (the "combined tensor"), product in double, rounded once
-template <typename T, int L>
-__global__ void fold_kernel(const T* __restrict__ path_w, T* __restrict__ cw) {
-    using Gen = TPGen<L>;
-    const int z = blockIdx.x * blockDim.x + threadIdx.x;
-    if (z < Gen::NNZ) cw[z] = (T)((double)path_w[Gen::zpath(z)] * Gen::zcoef(z));
-}
+// The folded coefficient table ("combined tensor" Wc = sum_p path_w[p] C^p) travels BY VALUE as a __grid_constant__
+// kernel parameter: every coefficient is a constant-bank operand of its FFMA/DFMA (no register, no load instruction), and two
+// launches -- different plans, different weights, different streams -- never share state.  Folded on the host when the weights
+// are bound (allegro_plan_bind_weights); 1.1 KB (l_max 2, fp32) .. 9.8 KB (l_max 3, fp64) of the 32 KB parameter space.
+template <typename T, int NNZ>
+struct CwTab {
+    T v[NNZ];
+};
 
 // ------------------------------------------------------------------------------------------------
 // The tile ring shared by the kernels below.  A stage holds TILES tiles of `tile_bytes` (tile 0 is
@@ -82,7 +80,7 @@ __device__ __forceinline__ T slot_sum(T x, int mode, int n, int slot, int ch, in
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
         const int wps = n >> 5;
-        if (wps == 1) return x;
+        if (wps == 1 || (slot + 1) * n > CT) return x;   // leftover threads (CT % n != 0) own no slot: they must not join a slot's barrier
         if (lane == 0) b[warp] = x;
         named_bar(1 + slot, n);
         if (ch == 0) {
@@ -111,7 +109,7 @@ __device__ __forceinline__ T slot_sum(T x, int mode, int n, int slot, int ch, in
 // WANT_OUT / WANT_G / WANT_E select which of out, G, e_edge are produced (at least one of out, G).
 // Stage = [V tile -> out tile (or G tile when !WANT_OUT)] [G tile when both are stored].
 template <typename T, int L, int CT, bool WANT_OUT, bool WANT_G, bool WANT_E>
-__global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
+__global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                           const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ out,
                                                           const T* __restrict__ q, T kappa, T* __restrict__ e_edge, T* __restrict__ G) {
     using Gen = TPGen<L>;
@@ -194,7 +192,7 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(int NST, int n, const i
             T* row = reinterpret_cast<T*>(r.stage(s)) + ((size_t)slot * n + ch) * DV;
             T v[DV], o[DV];
             row_load<T, DV>(row, v);
-            Gen::template fwd<T>(v, E, o);
+            Gen::template fwd<T>(cwt.v, v, E, o);
             if constexpr (WANT_OUT) row_store<T, DV>(row, o);
             if constexpr (EPI) {
                 T sq = T(0);
@@ -226,7 +224,7 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(int NST, int n, const i
 // order -> one partial row per item (reduced over items by gw_final_kernel).
 template <typename T, int L, int CT, bool WANT_GV, bool WANT_GW, bool COT>
 __global__ void __launch_bounds__(CT + 32)
-    tp_bwd_kernel(int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
+    tp_bwd_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
                   const T* __restrict__ Eenv, const T* __restrict__ q, T kappa, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item,
                   T* __restrict__ gw_part) {
     using Gen = TPGen<L>;
@@ -317,7 +315,7 @@ __global__ void __launch_bounds__(CT + 32)
                     for (int k = 0; k < DV; ++k) g[k] *= kappa;
                     g[0] += qc;
                 }
-                Gen::template bwd<T, WANT_GV>(v, E, g, gv, gE);
+                Gen::template bwd<T, WANT_GV>(cwt.v, v, E, g, gv, gE);
                 if constexpr (WANT_GW) Gen::template pathw<T>(v, E, g, gw);
                 if constexpr (WANT_GV) row_store<T, DV>(grow, gv);
             }

@@ -81,10 +81,15 @@ class SingleLayerStep:
         self.ws_env = torch.empty(max(ab.env_workspace(plan, self.N, items), 16), dtype=torch.uint8, device=dv)
         self.ws_bwd = torch.empty(max(ab.tp_backward_workspace(plan, self.N, self.E, items, want_g_path_w), 16), dtype=torch.uint8, device=dv)
         self.marks = None      # optional list of (name, start_event, end_event) filled by run(mark=True)
+        self.bind_weights()
+
+    def bind_weights(self):
+        """fold dev["path_w"] into the plan's combined tensor (once: MD weights are fixed; call again after changing them)"""
+        self.plan.bind_weights(self.dev["path_w"])
 
     def run(self, mark=False):
         p, d, it = self.plan, self.dev, self.items
-        rp, rvec, V, pw = d["row_ptr"], d["rvec"], d["V"], d["path_w"]
+        rp, rvec, V, pw = d["row_ptr"], d["rvec"], d["V"], None      # path weights: the table bound to the plan
         ev = []
 
         def timed(name, fn):
@@ -210,6 +215,7 @@ class ChunkedStep:
         self.e_ptr = torch.tensor([0, self.E], dtype=torch.int32, device=dv)
         self.ws = torch.empty(16, dtype=torch.uint8, device=dv)
         self.emax = emax
+        plan.bind_weights(dev["path_w"])
 
     def run(self, keep=None, mark=False):
         """keep: optional dict chunk_index -> dict that receives clones of that chunk's out / gV (parity tests);
@@ -235,9 +241,9 @@ class ChunkedStep:
             out = self.out[:m]
             gV = None if self.gV is None else self.gV[:m]
             timed("env_radial_forward", lambda: ab.env_radial_forward(p, rp_c, rvec, d["W_r"], self.rc, self.scale, Eenv=Eenv))
-            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp_c, V, Eenv, d["path_w"], d["q"], self.kappa, out=out,
+            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp_c, V, Eenv, None, d["q"], self.kappa, out=out,
                                                                     e_edge=self.e_edge[e0:e1], want_G=False))
-            timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp_c, out, V, Eenv, d["path_w"], d["q"], self.kappa,
+            timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp_c, out, V, Eenv, None, d["q"], self.kappa,
                                                                       want_gV=gV is not None, gV=gV, gEenv=gE, workspace=self.ws))
             timed("env_radial_backward", lambda: ab.env_radial_backward(p, rp_c, gE, rvec, d["W_r"], self.rc, self.scale,
                                                                         g_rvec=self.g_r[e0:e1]))
@@ -261,10 +267,13 @@ class TwoLayerStep:
     """One MD step of the stacked Allegro-style model of BASELINE.json:configs[2] (reading A19) as a sequence of library
     calls: edge embedding -> per layer [w = W_w x, env_embed, tensor product with dense per-path mix, latent update]
     -> readout of the l = 0 outputs -> the matching VJPs in reverse -> force gather.  `params` holds device tensors
-    W_x0 [n,nb], W_v0 [n,nb], W_w [L,n,n], W_p [L,P,n,n], A_lat [L-1,n,2n], q [n] and floats rc, scale."""
+    W_x0 [n,nb], W_v0 [n,nb], W_w [L,n,n], W_p [L,P,n,n], A_lat [L-1,n,2n], q [n] and floats rc, scale.
+    `plan_last`: optional dense plan restricted to the 0e output block (Plan.set_out_blocks(1)) for the last layer, whose
+    output feeds only the readout of the scalars: the paths into the other blocks are never run."""
 
-    def __init__(self, plan_dense, plan_scalar, dev, params):
+    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None):
         self.pd, self.ps, self.dev, self.p = plan_dense, plan_scalar, dev, params
+        self.pd_last = plan_last if plan_last is not None else plan_dense
         self.L = params["W_w"].shape[0]
         rp, rvec = dev["row_ptr"], dev["rvec"]
         self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
@@ -304,7 +313,8 @@ class TwoLayerStep:
         for l in range(L):
             timed("linear", lambda: ab.linear(self.x[l], p["W_w"][l], y=self.w[l]))
             timed("env_embed", lambda: ab.env_embed(ps, rp, rvec, self.w[l], scale, Eenv=self.Eenv[l]))
-            timed("tp_forward_dense", lambda: ab.tp_forward(pd, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
+            pl = self.pd_last if l == L - 1 else pd
+            timed("tp_forward_dense", lambda: ab.tp_forward(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
             if l < L - 1:
                 timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], self.V[l + 1], p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
         G = self.cot[0]
@@ -316,7 +326,8 @@ class TwoLayerStep:
                 g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
                 timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], G, self.g_r, g_x=g_x))
             gVl = self.cot[1] if G is self.cot[0] else self.cot[0]
-            timed("tp_backward_dense", lambda: ab.tp_backward(pd, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
+            pl = self.pd_last if l == L - 1 else pd
+            timed("tp_backward_dense", lambda: ab.tp_backward(pl, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
             if not have_gr:
                 timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r, g_w=self.g_w))
                 have_gr = True

@@ -353,6 +353,134 @@ def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
     assert ei.value.status == 2
 
 
+def _block_mask_weights(lmax, W, block_mask):
+    """path weights with the paths into the blocks outside block_mask zeroed: what an output-block subset computes"""
+    import oracle as orc
+    pt = orc.paths(lmax)
+    Wm = np.array(W, copy=True)
+    for p in range(len(pt["l3"])):
+        if not (block_mask >> (2 * int(pt["l3"][p]) + int(pt["p3"][p]))) & 1:
+            Wm[p] = 0
+    return Wm
+
+
+@pytest.mark.parametrize("wmode", ["dense", "scalar"])
+def test_output_block_subset(wmode):
+    """allegro_plan_set_out_blocks(0x1): only the paths into the 0e scalars run (last layer of a model whose readout takes the
+    l = 0 outputs, BASELINE.json:configs[2]).  Forward and VJP equal the oracle evaluated with the other paths' weights set
+    to zero; the cotangent outside the block is ignored."""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, rng
+    lmax, n, dt = 2, 64, np.float32
+    g = configs.geometry_for("C1s")
+    rp, E, N = g["row_ptr"], g["rvec"].shape[0], g["row_ptr"].shape[0] - 1
+    dV, dE, P = 18, 9, 30
+    S = rng.STREAMS
+    V = rng.normal(11, S["V"], (E, n, dV)).astype(dt)
+    Ee = (rng.normal(11, S["W_w"], (N, n, dE)) * 0.5).astype(dt)
+    W = (rng.normal(11, S["W_p"], (P, n, n)) / np.sqrt(n)).astype(dt) if wmode == "dense" else rng.normal(11, S["path_w"], (P,)).astype(dt)
+    G = rng.normal(11, S["G"], (E, n, dV)).astype(dt)
+    f8 = lambda a: a.astype(np.float64)
+    Wm = _block_mask_weights(lmax, W, 0x1)
+    Gm = np.zeros_like(G)
+    Gm[:, :, 0] = G[:, :, 0]
+    ref_out = orc.tp_forward(lmax, rp, f8(V), f8(Ee), f8(Wm))
+    ref_gV, ref_gE, _ = orc.tp_backward(lmax, rp, f8(Gm), f8(V), f8(Ee), f8(Wm), want_gV=True, want_gw=False)
+    assert np.abs(ref_out[:, :, 1:]).max() == 0.0
+    plan = ab.Plan(lmax, n, ab.F32, ab.W_DENSE if wmode == "dense" else ab.W_SCALAR)
+    plan.set_out_blocks(0x1)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    rpd, Vd, Ed, Wd, Gd = d(rp), d(V), d(Ee), d(W), d(G)
+    for items in (None, ab.segments_build(rp, 30)):
+        it = None if items is None else d(items)
+        out = ab.tp_forward(plan, rpd, Vd, Ed, Wd, items=it)
+        gV, gE, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it)     # full G handed in: its other blocks must be ignored
+        _assert_close(dict(out=ref_out, gV=ref_gV, gEenv=ref_gE), dict(out=out, gV=gV, gEenv=gE), dt, keys=("out", "gV", "gEenv"),
+                      label="0e-only " + wmode)
+        assert float(out[:, :, 1:].abs().max().item()) == 0.0
+    if wmode == "dense":
+        plan.set_out_blocks(0x5)      # not a compiled subset
+        with pytest.raises(ab.AllegroError) as ei:
+            ab.tp_forward(plan, rpd, Vd, Ed, Wd)
+        assert ei.value.status == 2
+
+
+def test_two_plans_two_streams_concurrently():
+    """Two plans of the same dtype / l_max with different scalar path weights, run on two streams at the same time: the folded
+    coefficient table travels with each launch as a kernel parameter, so neither sees the other's weights (round-1 finding:
+    a process-global __constant__ table raced).  Both results against the oracle."""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import rng
+    inp = _chain.make_inputs("C1s")
+    lmax, n, rp = inp["lmax"], inp["n"], inp["row_ptr"]
+    dev = _chain.to_device(inp)
+    f8 = lambda a: np.asarray(a, dtype=np.float64)
+    w, _ = orc.radial(f8(inp["W_r"]), inp["rc"], f8(inp["rvec"]))
+    Eenv = orc.env_embed(lmax, rp, f8(inp["rvec"]), w, inp["scale"])
+    Ed = torch.from_numpy(Eenv.astype(np.float32)).cuda()
+    Eenv = f8(Ed.cpu().numpy())
+    pws = [inp["path_w"], rng.normal(3, rng.STREAMS["path_w"], inp["path_w"].shape).astype(np.float32)]
+    refs = [orc.tp_forward(lmax, rp, f8(inp["V"]), Eenv, f8(pw)) for pw in pws]
+    plans = [ab.Plan(lmax, n, ab.F32), ab.Plan(lmax, n, ab.F32)]
+    pwd = [torch.from_numpy(pw).cuda() for pw in pws]
+    for pl, pw in zip(plans, pwd):
+        pl.bind_weights(pw)
+    streams = [torch.cuda.Stream(), torch.cuda.Stream()]
+    outs = [torch.empty_like(dev["V"]) for _ in range(2)]
+    torch.cuda.synchronize()
+    for rep in range(20):          # interleaved launches, no host synchronisation in between
+        for k in range(2):
+            with torch.cuda.stream(streams[k]):
+                ab.tp_forward(plans[k], dev["row_ptr"], dev["V"], Ed, None, out=outs[k], stream=streams[k])
+    torch.cuda.synchronize()
+    for k in range(2):
+        _assert_close(dict(out=refs[k]), dict(out=outs[k]), np.float32, keys=("out",), label="plan %d" % k)
+    assert not torch.equal(outs[0], outs[1])
+    # a call without bound weights and without path_w fails loudly
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_forward(ab.Plan(lmax, n, ab.F32), dev["row_ptr"], dev["V"], Ed, None)
+    assert ei.value.status == 1
+
+
+@pytest.mark.parametrize("n,dt", [(48, np.float32), (96, np.float32), (48, np.float64), (96, np.float64), (160, np.float32)])
+def test_energy_epilogue_channel_counts(n, dt):
+    """tp_forward_energy / tp_backward_energy for channel counts that leave compute threads without an edge slot (256 % 96 != 0)
+    or take the serial per-edge sum (n = 48): e_edge, out, gV, gEenv against the oracle (round-1 finding: n = 96 hung)."""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, rng
+    lmax = 1
+    g = configs.geometry_for("C0")
+    rp, E, N = g["row_ptr"], g["rvec"].shape[0], g["row_ptr"].shape[0] - 1
+    dV, dE, P = 8, 4, 10
+    S = rng.STREAMS
+    V = rng.normal(5, S["V"], (E, n, dV)).astype(dt)
+    Ee = (rng.normal(5, S["W_w"], (N, n, dE)) * 0.5).astype(dt)
+    pw = rng.normal(5, S["path_w"], (P,)).astype(dt)
+    q = (rng.normal(5, S["q"], (n,)) / np.sqrt(n)).astype(dt)
+    kappa = 0.3
+    f8 = lambda a: a.astype(np.float64)
+    out = orc.tp_forward(lmax, rp, f8(V), f8(Ee), f8(pw))
+    e_edge, G = orc.edge_energy(lmax, out, f8(q), kappa)
+    gV, gE, _ = orc.tp_backward(lmax, rp, G, f8(V), f8(Ee), f8(pw), want_gV=True, want_gw=False)
+    plan = ab.Plan(lmax, n, ab.F64 if dt == np.float64 else ab.F32)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    rpd, Vd, Ed, pwd, qd = d(rp), d(V), d(Ee), d(pw), d(q)
+    o, e, Gd = ab.tp_forward_energy(plan, rpd, Vd, Ed, pwd, qd, kappa)
+    gVd, gEd, _ = ab.tp_backward_energy(plan, rpd, o, Vd, Ed, pwd, qd, kappa)
+    torch.cuda.synchronize()
+    _assert_close(dict(out=out, e_edge=e_edge, G=G, gV=gV, gEenv=gE), dict(out=o, e_edge=e, G=Gd, gV=gVd, gEenv=gEd), dt,
+                  keys=("out", "e_edge", "G", "gV", "gEenv"), label="n=%d" % n)
+
+
 def _model_device(inp):
     import torch
     td = torch.float32 if inp["dt"] == np.float32 else torch.float64
@@ -363,18 +491,23 @@ def _model_device(inp):
     return dev, prm
 
 
-def _two_layer_step(inp):
+def _two_layer_step(inp, scalars_only_last=False):
     import paper_2504_16068_b200 as ab
     from paper_2504_16068_b200.pipeline import TwoLayerStep
     p = inp["params"]
     dt = ab.F32 if inp["dt"] == np.float32 else ab.F64
     dev, prm = _model_device(inp)
-    st = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm)
+    last = None
+    if scalars_only_last:      # the launch configuration bench.py --workload C2 times: last layer restricted to the 0e block
+        last = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
+        last.set_out_blocks(0x1)
+    st = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=last)
     st.run()
     return st
 
 
-def test_two_layer_model_c2s():
+@pytest.mark.parametrize("scalars_only_last", [False, True])
+def test_two_layer_model_c2s(scalars_only_last):
     """BASELINE.json:configs[2]'s recipe at 192 atoms (two stacked layers, dense 64x64 per-path mix, latent update, readout of
     the l = 0 outputs; forward + force backward) against oracle/model2.py: per-layer Eenv and features, per-edge energies,
     total energy, dE/dr_e and forces"""
@@ -385,11 +518,14 @@ def test_two_layer_model_c2s():
     p = inp["params"]
     taps = []
     en, g = model2.energy_grad(p, inp["row_ptr"], inp["rvec"].astype(np.float64), taps)
-    st = _two_layer_step(inp)
+    st = _two_layer_step(inp, scalars_only_last)
     ref, got = dict(g_r=g, e_edge=taps[-1]["e_edge"], F=orc.force_gather(inp["row_ptr"], inp["rev"], g)), dict(g_r=st.g_r, e_edge=st.e_edge, F=st.F)
     for l in range(p["n_layers"]):
         ref.update({"Eenv%d" % l: taps[l]["Eenv"], "V%d" % (l + 1): taps[l]["V_out"], "w%d" % l: taps[l]["w"]})
         got.update({"Eenv%d" % l: st.Eenv[l], "V%d" % (l + 1): st.V[l + 1], "w%d" % l: st.w[l]})
+    if scalars_only_last:      # only the scalars of the last layer's output exist
+        L = p["n_layers"]
+        ref["V%d" % L], got["V%d" % L] = taps[L - 1]["V_out"][:, :, :1], st.V[L][:, :, :1]
     ref["V0"], got["V0"] = taps[0]["V_in"], st.V[0]
     errs = _assert_close(ref, got, inp["dt"], keys=tuple(ref.keys()), label="C2s")
     print("C2s", {k: "%.2e" % v for k, v in errs.items()})
@@ -412,7 +548,7 @@ def test_two_layer_model_c2_full_size_sampled_centres():
     if free < 110e9:
         pytest.skip("needs ~100 GB of free HBM")
     inp = make_model_inputs("C2")
-    st = _two_layer_step(inp)
+    st = _two_layer_step(inp, scalars_only_last=True)
     torch.cuda.synchronize()
     rp, N = inp["row_ptr"], inp["N"]
     starts = [int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(2), 0, N - 5)] + [0, N - 4]
@@ -422,8 +558,8 @@ def test_two_layer_model_c2_full_size_sampled_centres():
         sub_rp = (rp[c0:c1 + 1] - rp[c0]).astype(np.int32)
         taps = []
         en, g = model2.energy_grad(inp["params"], sub_rp, inp["rvec"][e0:e1].astype(np.float64), taps)
-        ref = dict(g_r=g, e_edge=taps[-1]["e_edge"], V2=taps[1]["V_out"], Eenv1=taps[1]["Eenv"])
-        got = dict(g_r=st.g_r[e0:e1], e_edge=st.e_edge[e0:e1], V2=st.V[2][e0:e1], Eenv1=st.Eenv[1][c0:c1])
+        ref = dict(g_r=g, e_edge=taps[-1]["e_edge"], V1=taps[0]["V_out"], V2=taps[1]["V_out"][:, :, :1], Eenv1=taps[1]["Eenv"])
+        got = dict(g_r=st.g_r[e0:e1], e_edge=st.e_edge[e0:e1], V1=st.V[1][e0:e1], V2=st.V[2][e0:e1, :, :1], Eenv1=st.Eenv[1][c0:c1])
         _assert_close(ref, got, inp["dt"], keys=tuple(ref.keys()), label="C2 centres [%d,%d)" % (c0, c1))
     _check_force_gather(inp, dict(g_r=st.g_r, F=st.F))
 
