@@ -332,7 +332,11 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
     # last layer: its output feeds only the readout of the l = 0 outputs (configs[2]), so the plan is restricted to the 0e block
     plan_last = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
     plan_last.set_out_blocks(0x1)
-    step = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=plan_last)
+    # first layer: V0 = v (x) Y(rhat) has the natural-parity blocks only (reading A19), the paths from the other blocks never run
+    plan_first = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
+    plan_first.set_in_blocks(0x19)
+    step = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=plan_last,
+                        plan_first=plan_first)
     E, N = step.E, step.N
 
     def barrier():

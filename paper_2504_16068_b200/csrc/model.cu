@@ -1,11 +1,53 @@
 // model.cu -- dtype-only pieces of the two-layer model of BASELINE.json:configs[2] (reading A19) that are not part
 // of the tensor-product hot path: the per-edge linear maps (w = W_w x and its transpose), the scalar latent update
-// x' = u(r/r_c) SiLU(A [x ; V[:,0e]]) with its VJP, and an in-place add.  Small-K GEMMs ([E x 64] x [64 x 64..128]):
-// the weight matrix sits in shared memory (row stride +1: conflict-free), one thread per output element.
+// x' = u(r/r_c) SiLU(A [x ; V[:,0e]]) with its VJP, and an in-place add.  Small-K GEMMs ([E x 64] x [64 x 64..128]) in the
+// method's own precision (fp32 / fp64 FMA): register-tiled, both operands K-major in shared memory.
 #include "common.cuh"
 #include "launch.h"
 
 namespace allegro {
+
+// ---------------------------------------------------------------------------------------------- register-tiled small GEMM
+// All three maps are [E x K] . [K x n_out] products with K, n_out in {64, 128}: HBM-light, FMA-heavy.  One CTA (256 threads) owns
+// a tile of TILE_E = 128 edges and walks the outputs in chunks of 64; thread (ty, tx) = (tid / 16, tid % 16) accumulates 8 edges
+// (8 ty .. 8 ty + 7) x 4 outputs (4 tx .. 4 tx + 3) in registers.  Both operands sit in shared memory K-major -- xs[k][128 edges],
+// Ws[k][64 outputs] -- so one k step is two 128-bit loads of x (a broadcast inside each half-warp), one of W and 32 FMAs.
+constexpr int kTileE = 128, kTileO = 64;
+
+template <typename T>
+__device__ __forceinline__ void tile_mac(const T* __restrict__ xs, const T* __restrict__ Ws, int K, int ty, int tx, T (&acc)[8][4]) {
+#pragma unroll 4
+    for (int k = 0; k < K; ++k) {
+        T xv[8], wv[4];
+#pragma unroll
+        for (int i = 0; i < 8; ++i) xv[i] = xs[k * kTileE + 8 * ty + i];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) wv[j] = Ws[k * kTileO + 4 * tx + j];
+#pragma unroll
+        for (int i = 0; i < 8; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j] = fma(xv[i], wv[j], acc[i][j]);
+    }
+}
+// Ws[k][o] = W[o0 + o][k] (transpose_w == 0, W [n_out][ldw = K]) or W[k][o0 + o] (transpose_w == 1, W [K][ldw = n_out]); columns beyond
+// n_out are zero
+template <typename T>
+__device__ __forceinline__ void tile_load_w(T* __restrict__ Ws, const T* __restrict__ W, int K, int n_out, int o0, int transpose_w, int tid) {
+    for (int idx = tid; idx < K * kTileO; idx += 256) {
+        int k, o;
+        if (transpose_w) { k = idx / kTileO; o = idx - k * kTileO; } else { o = idx / K; k = idx - o * K; }
+        const int og = o0 + o;
+        Ws[k * kTileO + o] = og < n_out ? (transpose_w ? W[(size_t)k * n_out + og] : W[(size_t)og * K + k]) : T(0);
+    }
+}
+// xs[k][le] = x[eb + le][k] for k < K (rows beyond E are zero): lanes run over edges, so the shared-memory writes are conflict-free
+template <typename T>
+__device__ __forceinline__ void tile_load_x(T* __restrict__ xs, const T* __restrict__ x, long E, long eb, int K, int k0, int ldx, int kstride, int tid) {
+    for (int idx = tid; idx < K * kTileE; idx += 256) {
+        const int k = idx / kTileE, le = idx - k * kTileE;
+        xs[(k0 + k) * kTileE + le] = eb + le < E ? x[(size_t)(eb + le) * ldx + (size_t)k * kstride] : T(0);
+    }
+}
 
 // y[e][o] (+)= sum_i x[e][i] Wm[o][i]            (transpose_w == 0, Wm = W [n_out][n_in])
 // y[e][o] (+)= sum_i x[e][i] W[i][o]             (transpose_w == 1, W [n_in][n_out]: the VJP of the map above)
@@ -13,25 +55,38 @@ template <typename T>
 __global__ void __launch_bounds__(256) linear_kernel(long E, int n_out, int n_in, const T* __restrict__ x, const T* __restrict__ W, int transpose_w,
                                                       int accumulate, T* __restrict__ y) {
     extern __shared__ __align__(16) unsigned char lin_raw[];
-    T* Ws = reinterpret_cast<T*>(lin_raw);                 // [n_out][n_in + 1]
-    const int ld = n_in + 1;
-    T* xs = Ws + (size_t)n_out * ld;                       // [epb][n_in]
-    const int epb = 256 / n_out;                           // edges per pass
-    for (int idx = threadIdx.x; idx < n_out * n_in; idx += 256) {
-        const int o = idx / n_in, i = idx - o * n_in;
-        Ws[o * ld + i] = transpose_w ? W[(size_t)i * n_out + o] : W[idx];
-    }
-    const int le = threadIdx.x / n_out, o = threadIdx.x - le * n_out;
-    for (long eb = (long)blockIdx.x * epb; eb < E; eb += (long)gridDim.x * epb) {
+    T* xs = reinterpret_cast<T*>(lin_raw);            // [n_in][128]
+    T* Ws = xs + (size_t)n_in * kTileE;               // [n_in][64]
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    const int nchunk = (n_out + kTileO - 1) / kTileO;
+    for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
-        const int cnt = (int)min((long)epb, E - eb);
-        for (int idx = threadIdx.x; idx < cnt * n_in; idx += 256) xs[idx] = x[(size_t)eb * n_in + idx];
-        __syncthreads();
-        if (le < cnt) {
-            T acc = T(0);
-            for (int i = 0; i < n_in; ++i) acc = fma(xs[le * n_in + i], Ws[o * ld + i], acc);
-            T* dst = y + (size_t)(eb + le) * n_out + o;
-            *dst = accumulate ? *dst + acc : acc;
+        tile_load_x<T>(xs, x, E, eb, n_in, 0, n_in, 1, tid);
+        for (int c = 0; c < nchunk; ++c) {
+            if (c > 0 || nchunk > 1 || eb == (long)blockIdx.x * kTileE) {   // one output chunk: W stays resident over the tiles
+                __syncthreads();
+                tile_load_w<T>(Ws, W, n_in, n_out, c * kTileO, transpose_w, tid);
+            }
+            __syncthreads();
+            T acc[8][4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = T(0);
+            tile_mac<T>(xs, Ws, n_in, ty, tx, acc);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const long e = eb + 8 * ty + i;
+                if (e >= E) continue;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int o = c * kTileO + 4 * tx + j;
+                    if (o < n_out) {
+                        T* dst = y + (size_t)e * n_out + o;
+                        *dst = accumulate ? *dst + acc[i][j] : acc[i][j];
+                    }
+                }
+            }
         }
     }
 }
@@ -50,35 +105,56 @@ template <typename T>
 __global__ void __launch_bounds__(256) latent_fwd_kernel(long E, int n, int dV, T rc, const T* __restrict__ rvec, const T* __restrict__ x,
                                                           const T* __restrict__ V, const T* __restrict__ A, T* __restrict__ z, T* __restrict__ x_new) {
     extern __shared__ __align__(16) unsigned char lin_raw[];
-    const int K = 2 * n, ld = K + 1;
-    T* As = reinterpret_cast<T*>(lin_raw);  // [n][2n + 1]
-    T* in = As + (size_t)n * ld;            // [epb][2n]
-    const int epb = 256 / n;
-    for (int idx = threadIdx.x; idx < n * K; idx += 256) As[(idx / K) * ld + (idx % K)] = A[idx];
-    const int le = threadIdx.x / n, o = threadIdx.x - le * n;
-    for (long eb = (long)blockIdx.x * epb; eb < E; eb += (long)gridDim.x * epb) {
+    const int K = 2 * n;
+    T* xs = reinterpret_cast<T*>(lin_raw);            // [2n][128]: rows 0..n-1 = x, rows n..2n-1 = V[:, :, 0]
+    T* Ws = xs + (size_t)K * kTileE;                  // [2n][64]
+    T* us = Ws + (size_t)K * kTileO;                  // [128] cutoff u(|r|/rc)
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    const int nchunk = (n + kTileO - 1) / kTileO;
+    for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
-        const int cnt = (int)min((long)epb, E - eb);
-        for (int idx = threadIdx.x; idx < cnt * n; idx += 256) {
-            const int l2 = idx / n, i = idx - l2 * n;
-            in[l2 * K + i] = x[(size_t)(eb + l2) * n + i];
-            in[l2 * K + n + i] = V[((size_t)(eb + l2) * n + i) * dV];
+        tile_load_x<T>(xs, x, E, eb, n, 0, n, 1, tid);
+        tile_load_x<T>(xs, V, E, eb, n, n, n * dV, dV, tid);   // V[e][k][0]
+        if (tid < kTileE) {
+            const long e = eb + tid;
+            T du, u = T(0);
+            if (e < E) {
+                const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+                u = cutoff_u<T>(sqrt(rx * rx + ry * ry + rz * rz) / rc, du);
+            }
+            us[tid] = u;
         }
-        __syncthreads();
-        if (le < cnt) {
-            const size_t e = (size_t)(eb + le);
-            T acc = T(0);
-            for (int i = 0; i < K; ++i) acc = fma(in[le * K + i], As[o * ld + i], acc);
-            const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
-            T du;
-            const T u = cutoff_u<T>(sqrt(rx * rx + ry * ry + rz * rz) / rc, du);
-            const T sg = T(1) / (T(1) + exp(-acc));
-            z[e * n + o] = acc;
-            x_new[e * n + o] = u * acc * sg;
+        for (int c = 0; c < nchunk; ++c) {
+            if (c > 0 || nchunk > 1 || eb == (long)blockIdx.x * kTileE) {
+                __syncthreads();
+                tile_load_w<T>(Ws, A, K, n, c * kTileO, 0, tid);
+            }
+            __syncthreads();
+            T acc[8][4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = T(0);
+            tile_mac<T>(xs, Ws, K, ty, tx, acc);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const long e = eb + 8 * ty + i;
+                if (e >= E) continue;
+                const T u = us[8 * ty + i];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int o = c * kTileO + 4 * tx + j;
+                    if (o < n) {
+                        const T a = acc[i][j];
+                        const T sg = T(1) / (T(1) + exp(-a));
+                        z[(size_t)e * n + o] = a;
+                        x_new[(size_t)e * n + o] = u * a * sg;
+                    }
+                }
+            }
         }
     }
 }
-
 // VJP: g_z = g_xnew u SiLU'(z);  g_x[e][i] = sum_o g_z[o] A[o][i] (overwritten);  gV[e][i][0] += sum_o g_z[o] A[o][n+i];
 //      g_rvec[e] += (sum_o g_xnew[o] SiLU(z[o])) u'(x)/r_c rhat_e
 template <typename T>
@@ -86,44 +162,71 @@ __global__ void __launch_bounds__(256) latent_bwd_kernel(long E, int n, int dV, 
                                                           const T* __restrict__ g_xnew, const T* __restrict__ A, T* __restrict__ g_x,
                                                           T* __restrict__ gV, T* __restrict__ g_rvec) {
     extern __shared__ __align__(16) unsigned char lin_raw[];
-    const int K = 2 * n;
-    T* As = reinterpret_cast<T*>(lin_raw);  // [n][2n] (read along o for fixed i: consecutive threads i -> consecutive banks)
-    T* gz = As + (size_t)n * K;             // [epb][n]
-    T* rs = gz + 256;                       // [epb][n] g_xnew * SiLU(z) for the radial term
-    const int epb = 256 / n;
-    for (int idx = threadIdx.x; idx < n * K; idx += 256) As[idx] = A[idx];
-    const int le = threadIdx.x / n, i = threadIdx.x - le * n;
-    for (long eb = (long)blockIdx.x * epb; eb < E; eb += (long)gridDim.x * epb) {
+    T* xs = reinterpret_cast<T*>(lin_raw);            // [n][128]: g_z, K-major (K = the n outputs of the forward map)
+    T* Ws = xs + (size_t)n * kTileE;                  // [n][64]: A[o][chunk of the 2n inputs]
+    T* us = Ws + (size_t)n * kTileO;                  // [128] u, [128] u'/rc/|r|, [2][128] partial radial sums
+    T* dus = us + kTileE;
+    T* rs = dus + kTileE;
+    const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
+    const int nchunk = (2 * n + kTileO - 1) / kTileO;
+    for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
-        const int cnt = (int)min((long)epb, E - eb);
-        T u = T(0), du = T(0), rx = T(0), ry = T(0), rz = T(0), r = T(1);
-        if (le < cnt) {
-            const size_t e = (size_t)(eb + le);
-            rx = rvec[3 * e]; ry = rvec[3 * e + 1]; rz = rvec[3 * e + 2];
-            r = sqrt(rx * rx + ry * ry + rz * rz);
-            u = cutoff_u<T>(r / rc, du);
-            const T zz = z[e * n + i], g = g_xnew[e * n + i];
-            const T sg = T(1) / (T(1) + exp(-zz));
-            gz[le * n + i] = g * u * (sg * (T(1) + zz * (T(1) - sg)));
-            rs[le * n + i] = g * zz * sg;
+        if (tid < kTileE) {
+            const long e = eb + tid;
+            T u = T(0), du = T(0), r = T(1);
+            if (e < E) {
+                const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+                r = sqrt(rx * rx + ry * ry + rz * rz);
+                u = cutoff_u<T>(r / rc, du);
+            }
+            us[tid] = u;
+            dus[tid] = du / rc / r;
         }
         __syncthreads();
-        if (le < cnt) {
-            const size_t e = (size_t)(eb + le);
-            T a0 = T(0), a1 = T(0);
-            for (int o = 0; o < n; ++o) {
-                const T g = gz[le * n + o];
-                a0 = fma(g, As[o * K + i], a0);
-                a1 = fma(g, As[o * K + n + i], a1);
+        {   // g_z = g_xnew u SiLU'(z) -> xs[o][le]; this thread's edge le = tid % 128 is the same in every iteration
+            const int le = tid & (kTileE - 1);
+            const long e = eb + le;
+            T part = T(0);
+            for (int o = tid >> 7; o < n; o += 2) {
+                T gzv = T(0);
+                if (e < E) {
+                    const T zz = z[(size_t)e * n + o], g = g_xnew[(size_t)e * n + o];
+                    const T sg = T(1) / (T(1) + exp(-zz));
+                    gzv = g * us[le] * (sg * (T(1) + zz * (T(1) - sg)));
+                    part += g * zz * sg;
+                }
+                xs[o * kTileE + le] = gzv;
             }
-            g_x[e * n + i] = a0;
-            gV[(e * n + i) * dV] += a1;
-            if (i < 3) {
-                T s = T(0);
-                for (int o = 0; o < n; ++o) s += rs[le * n + o];
-                const T comp = i == 0 ? rx : (i == 1 ? ry : rz);
-                g_rvec[3 * e + i] += s * du / rc * comp / r;
+            rs[(tid >> 7) * kTileE + le] = part;
+        }
+        for (int c = 0; c < nchunk; ++c) {
+            __syncthreads();
+            tile_load_w<T>(Ws, A, n, 2 * n, c * kTileO, 1, tid);
+            __syncthreads();
+            T acc[8][4];
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) acc[i][j] = T(0);
+            tile_mac<T>(xs, Ws, n, ty, tx, acc);
+#pragma unroll
+            for (int i = 0; i < 8; ++i) {
+                const long e = eb + 8 * ty + i;
+                if (e >= E) continue;
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    const int o = c * kTileO + 4 * tx + j;
+                    if (o < n) g_x[(size_t)e * n + o] = acc[i][j];
+                    else if (o < 2 * n) gV[((size_t)e * n + (o - n)) * dV] += acc[i][j];
+                }
             }
+        }
+        if (tid < kTileE && eb + tid < E) {   // radial term: rs was written before the first barrier of the chunk loop
+            const long e = eb + tid;
+            const T sc = (rs[tid] + rs[kTileE + tid]) * dus[tid];
+            g_rvec[3 * e] += sc * rvec[3 * e];
+            g_rvec[3 * e + 1] += sc * rvec[3 * e + 1];
+            g_rvec[3 * e + 2] += sc * rvec[3 * e + 2];
         }
     }
 }
@@ -134,44 +237,41 @@ __global__ void add_inplace_kernel(long count, T* __restrict__ y, const T* __res
 }
 
 // ------------------------------------------------------------------------------------------------ launchers
-static inline unsigned model_grid(long E, int epb) {
-    const long want = (E + epb - 1) / epb;
-    return (unsigned)(want < 148 * 8 ? (want < 1 ? 1 : want) : 148 * 8);
+static inline unsigned model_grid(long E) {
+    const long want = (E + kTileE - 1) / kTileE;
+    return (unsigned)(want < 148 * 2 ? (want < 1 ? 1 : want) : 148 * 2);
 }
 
 template <typename T>
 allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st) {
-    if (n_out > 256 || n_in > 512) { set_error("linear: n_out = %d, n_in = %d unsupported (<= 256, <= 512)", n_out, n_in); return ALLEGRO_EUNSUPPORTED; }
+    if (n_out > 1024 || n_in > 256) { set_error("linear: n_out = %d, n_in = %d unsupported (<= 1024, <= 256)", n_out, n_in); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
-    const int epb = 256 / n_out;
-    const size_t smem = ((size_t)n_out * (n_in + 1) + (size_t)epb * n_in) * sizeof(T);
+    const size_t smem = (size_t)n_in * (kTileE + kTileO) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(linear_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    linear_kernel<T><<<model_grid(E, epb), 256, smem, st>>>(E, n_out, n_in, (const T*)x, (const T*)W, transpose_w, accumulate, (T*)y);
+    linear_kernel<T><<<model_grid(E), 256, smem, st>>>(E, n_out, n_in, (const T*)x, (const T*)W, transpose_w, accumulate, (T*)y);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
 template <typename T>
 allegro_status_t launch_latent_forward(long E, int n, int dV, double rc, const void* rvec, const void* x, const void* V, const void* A, void* z,
                                        void* x_new, cudaStream_t st) {
-    if (n > 128 || n < 3) { set_error("latent_forward: n = %d unsupported (3 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
+    if (n > 128 || n < 1) { set_error("latent_forward: n = %d unsupported (1 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
-    const int epb = 256 / n;
-    const size_t smem = ((size_t)n * (2 * n + 1) + (size_t)epb * 2 * n) * sizeof(T);
+    const size_t smem = ((size_t)2 * n * (kTileE + kTileO) + kTileE) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(latent_fwd_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    latent_fwd_kernel<T><<<model_grid(E, epb), 256, smem, st>>>(E, n, dV, (T)rc, (const T*)rvec, (const T*)x, (const T*)V, (const T*)A, (T*)z, (T*)x_new);
+    latent_fwd_kernel<T><<<model_grid(E), 256, smem, st>>>(E, n, dV, (T)rc, (const T*)rvec, (const T*)x, (const T*)V, (const T*)A, (T*)z, (T*)x_new);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
 template <typename T>
 allegro_status_t launch_latent_backward(long E, int n, int dV, double rc, const void* rvec, const void* z, const void* g_xnew, const void* A,
                                         void* g_x, void* gV, void* g_rvec, cudaStream_t st) {
-    if (n > 128 || n < 3) { set_error("latent_backward: n = %d unsupported (3 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
+    if (n > 256 || n < 1) { set_error("latent_backward: n = %d unsupported (1 <= n <= 256)", n); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
-    const int epb = 256 / n;
-    const size_t smem = ((size_t)n * 2 * n + 512) * sizeof(T);
+    const size_t smem = ((size_t)n * (kTileE + kTileO) + 4 * kTileE) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(latent_bwd_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    latent_bwd_kernel<T><<<model_grid(E, epb), 256, smem, st>>>(E, n, dV, (T)rc, (const T*)rvec, (const T*)z, (const T*)g_xnew, (const T*)A, (T*)g_x,
-                                                               (T*)gV, (T*)g_rvec);
+    latent_bwd_kernel<T><<<model_grid(E), 256, smem, st>>>(E, n, dV, (T)rc, (const T*)rvec, (const T*)z, (const T*)g_xnew, (const T*)A, (T*)g_x,
+                                                          (T*)gV, (T*)g_rvec);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

@@ -269,11 +269,14 @@ class TwoLayerStep:
     -> readout of the l = 0 outputs -> the matching VJPs in reverse -> force gather.  `params` holds device tensors
     W_x0 [n,nb], W_v0 [n,nb], W_w [L,n,n], W_p [L,P,n,n], A_lat [L-1,n,2n], q [n] and floats rc, scale.
     `plan_last`: optional dense plan restricted to the 0e output block (Plan.set_out_blocks(1)) for the last layer, whose
-    output feeds only the readout of the scalars: the paths into the other blocks are never run."""
+    output feeds only the readout of the scalars: the paths into the other blocks are never run.
+    `plan_first`: optional dense plan restricted to the natural-parity input blocks (Plan.set_in_blocks(0x19)) for the first
+    layer, whose input V0 = v (x) Y has zeros in the other blocks (reading A19): half of the paths never run."""
 
-    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None):
+    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None):
         self.pd, self.ps, self.dev, self.p = plan_dense, plan_scalar, dev, params
         self.pd_last = plan_last if plan_last is not None else plan_dense
+        self.pd_first = plan_first if plan_first is not None else plan_dense
         self.L = params["W_w"].shape[0]
         rp, rvec = dev["row_ptr"], dev["rvec"]
         self.N, self.E = rp.shape[0] - 1, rvec.shape[0]
@@ -313,7 +316,7 @@ class TwoLayerStep:
         for l in range(L):
             timed("linear", lambda: ab.linear(self.x[l], p["W_w"][l], y=self.w[l]))
             timed("env_embed", lambda: ab.env_embed(ps, rp, rvec, self.w[l], scale, Eenv=self.Eenv[l]))
-            pl = self.pd_last if l == L - 1 else pd
+            pl = self.pd_last if l == L - 1 else (self.pd_first if l == 0 else pd)
             timed("tp_forward_dense", lambda: ab.tp_forward(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
             if l < L - 1:
                 timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], self.V[l + 1], p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
@@ -326,7 +329,7 @@ class TwoLayerStep:
                 g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
                 timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], G, self.g_r, g_x=g_x))
             gVl = self.cot[1] if G is self.cot[0] else self.cot[0]
-            pl = self.pd_last if l == L - 1 else pd
+            pl = self.pd_last if l == L - 1 else (self.pd_first if l == 0 else pd)
             timed("tp_backward_dense", lambda: ab.tp_backward(pl, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
             if not have_gr:
                 timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r, g_w=self.g_w))

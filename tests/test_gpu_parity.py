@@ -353,15 +353,57 @@ def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
     assert ei.value.status == 2
 
 
-def _block_mask_weights(lmax, W, block_mask):
-    """path weights with the paths into the blocks outside block_mask zeroed: what an output-block subset computes"""
+def _block_mask_weights(lmax, W, out_mask, in_mask=0xffff):
+    """path weights with the paths into blocks outside out_mask / from blocks outside in_mask zeroed: what a block subset computes"""
     import oracle as orc
     pt = orc.paths(lmax)
     Wm = np.array(W, copy=True)
     for p in range(len(pt["l3"])):
-        if not (block_mask >> (2 * int(pt["l3"][p]) + int(pt["p3"][p]))) & 1:
+        if not ((out_mask >> (2 * int(pt["l3"][p]) + int(pt["p3"][p]))) & 1 and (in_mask >> (2 * int(pt["l1"][p]) + int(pt["p1"][p]))) & 1):
             Wm[p] = 0
     return Wm
+
+
+@pytest.mark.parametrize("wmode", ["dense", "scalar"])
+def test_input_block_subset(wmode):
+    """allegro_plan_set_in_blocks(0x19): V has the natural-parity blocks (0e, 1o, 2e) only -- the first layer of the two-layer
+    model, V0 = v (x) Y.  The other blocks of V are never read (they hold garbage here), the paths from them never run, their gV
+    components come back as zeros; everything else equals the oracle on V with those blocks zeroed."""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, rng
+    lmax, n, dt = 2, 64, np.float32
+    g = configs.geometry_for("C1s")
+    rp, E, N = g["row_ptr"], g["rvec"].shape[0], g["row_ptr"].shape[0] - 1
+    dV, dE, P = 18, 9, 30
+    S = rng.STREAMS
+    V = rng.normal(13, S["V"], (E, n, dV)).astype(dt)
+    Ee = (rng.normal(13, S["W_w"], (N, n, dE)) * 0.5).astype(dt)
+    W = (rng.normal(13, S["W_p"], (P, n, n)) / np.sqrt(n)).astype(dt) if wmode == "dense" else rng.normal(13, S["path_w"], (P,)).astype(dt)
+    G = rng.normal(13, S["G"], (E, n, dV)).astype(dt)
+    natural = [0, 5, 6, 7, 8, 9, 10, 11, 12]                  # components of 0e, 1o, 2e
+    other = [k for k in range(dV) if k not in natural]
+    Vz = V.copy()
+    Vz[:, :, other] = 0
+    f8 = lambda a: a.astype(np.float64)
+    ref_out = orc.tp_forward(lmax, rp, f8(Vz), f8(Ee), f8(W))
+    ref_gV, ref_gE, _ = orc.tp_backward(lmax, rp, f8(G), f8(Vz), f8(Ee), f8(W), want_gV=True, want_gw=False)
+    ref_gV[:, :, other] = 0
+    plan = ab.Plan(lmax, n, ab.F32, ab.W_DENSE if wmode == "dense" else ab.W_SCALAR)
+    plan.set_in_blocks(0x19)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    Vg = V.copy()
+    Vg[:, :, other] = 1e30                                    # must never be read
+    rpd, Vd, Ed, Wd, Gd = d(rp), d(Vg), d(Ee), d(W), d(G)
+    for items in (None, ab.segments_build(rp, 30)):
+        it = None if items is None else d(items)
+        out = ab.tp_forward(plan, rpd, Vd, Ed, Wd, items=it)
+        gV, gE, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it)
+        _assert_close(dict(out=ref_out, gV=ref_gV, gEenv=ref_gE), dict(out=out, gV=gV, gEenv=gE), dt, keys=("out", "gV", "gEenv"),
+                      label="natural-parity inputs " + wmode)
+        assert float(gV[:, :, other].abs().max().item()) == 0.0
 
 
 @pytest.mark.parametrize("wmode", ["dense", "scalar"])
@@ -497,11 +539,14 @@ def _two_layer_step(inp, scalars_only_last=False):
     p = inp["params"]
     dt = ab.F32 if inp["dt"] == np.float32 else ab.F64
     dev, prm = _model_device(inp)
-    last = None
-    if scalars_only_last:      # the launch configuration bench.py --workload C2 times: last layer restricted to the 0e block
+    last = first = None
+    if scalars_only_last:      # the launch configuration bench.py --workload C2 times: block subsets for the first and last layer
         last = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
         last.set_out_blocks(0x1)
-    st = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=last)
+        first = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
+        first.set_in_blocks(0x19)
+    st = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=last,
+                      plan_first=first)
     st.run()
     return st
 
