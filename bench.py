@@ -108,29 +108,52 @@ class ClockSampler:
 
 
 # ------------------------------------------------------------------------------------------------ oracle arm
-def _oracle_sample_step(inp, n_centres):
-    """One oracle step (the chain of tests/_chain.oracle_chain without forces) on the first n_centres centres with
-    their complete neighbourhoods (exact sub-problem: every per-edge / per-centre quantity depends on one centre)."""
+def _oracle_range(inp, c0, c1):
+    """One oracle step (the chain of tests/_chain.oracle_chain without forces) on centres [c0, c1) with their complete
+    neighbourhoods (exact sub-problem: every per-edge / per-centre quantity depends on one centre).  -> (edges, seconds)"""
     import _chain
     from workloads.inputs import sub_inputs
-    sub = sub_inputs(inp, 0, n_centres)
+    sub = sub_inputs(inp, c0, c1)
     t0 = time.perf_counter()
     _chain.oracle_chain(sub, want_gw=False, forces=False)
     return sub["E"], time.perf_counter() - t0
 
 
+def _oracle_sample_step(inp, n_centres):
+    return _oracle_range(inp, 0, n_centres)
+
+
+def _oracle_all_cores(inp, n_centres, cores):
+    """the same single-threaded oracle over `cores` disjoint centre ranges at once (the C++ oracle runs outside the GIL)
+    -> (edges, wall seconds)"""
+    import concurrent.futures as cf
+    from workloads.inputs import sub_inputs
+    bounds = [n_centres * k // cores for k in range(cores + 1)]
+    ranges = [(a, b) for a, b in zip(bounds[:-1], bounds[1:]) if b > a]
+    subs = [sub_inputs(inp, a, b) for a, b in ranges]          # slicing is not part of the timed work
+    import _chain
+    t0 = time.perf_counter()
+    with cf.ThreadPoolExecutor(max_workers=len(subs)) as ex:
+        list(ex.map(lambda sb: _chain.oracle_chain(sb, want_gw=False, forces=False), subs))
+    return sum(sb["E"] for sb in subs), time.perf_counter() - t0, len(subs)
+
+
 def cpu_baseline(inp, seconds):
-    """The float64 oracle, as it stands, on a bounded sample: calibrate on 4 centres, then size the sample for
-    about `seconds` of single-threaded CPU work."""
+    """The float64 oracle, as it stands, on a bounded sample of the workload: calibrate on 4 centres, one single-threaded leg
+    of about seconds / 2, then the same function on all host cores (sched_getaffinity) over disjoint centre ranges."""
     N = inp["N"]
     e_cal, t_cal = _oracle_sample_step(inp, min(4, N))
     rate = e_cal / max(t_cal, 1e-9)
     deg = inp["E"] / max(N, 1)
-    nc = int(max(4, min(N, rate * seconds / deg)))
-    e, t = _oracle_sample_step(inp, nc)
-    return {"value": e / t, "unit": UNIT, "cores": 1, "kind": "oracle",
-            "sample": "float64 C++ oracle chain (radial, env-embed, TP fwd, energy, TP VJP, env VJP; no force gather) on the first "
-                      "%d centres = %d edges of %s, %.1f s, single thread" % (nc, e, inp["name"], t)}
+    nc = int(max(4, min(N, rate * 0.5 * seconds / deg)))
+    e1, t1 = _oracle_sample_step(inp, nc)
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
+    nca = int(max(cores, min(N, nc * cores)))
+    ea, ta, used = _oracle_all_cores(inp, nca, cores)
+    return {"value": ea / ta, "unit": UNIT, "cores": used, "kind": "oracle", "value_1core": e1 / t1,
+            "sample": "float64 C++ oracle chain (radial, env-embed, TP fwd, energy, TP VJP, env VJP; no force gather): all-cores leg on the "
+                      "first %d centres = %d edges of %s split into %d ranges, %.1f s wall; single-thread leg on the first %d centres = %d "
+                      "edges, %.1f s" % (nca, ea, inp["name"], used, ta, nc, e1, t1)}
 
 
 def run_reference(args):
@@ -144,23 +167,24 @@ def run_reference(args):
     name = args.workload
     inp = make_inputs(name, features="lazy")
     steps = max(1, args.steps)
-    per_step = max(0.5, min(10.0, 120.0 / (steps + args.warmup)))
+    per_step = max(0.5, min(10.0, 120.0 / (steps + args.warmup)))     # wall seconds of oracle work per step
+    cores = len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1)
     e_cal, t_cal = _oracle_sample_step(inp, 4)
-    nc = int(max(4, min(inp["N"], (e_cal / t_cal) * per_step / (inp["E"] / inp["N"]))))
+    nc = int(max(cores, min(inp["N"], cores * (e_cal / t_cal) * per_step / (inp["E"] / inp["N"]))))
     for _ in range(args.warmup):
-        _oracle_sample_step(inp, nc)
-    tot_e, tot_t = 0, 0.0
+        _oracle_all_cores(inp, nc, cores)
+    tot_e, tot_t, used = 0, 0.0, cores
     for _ in range(steps):
-        e, t = _oracle_sample_step(inp, nc)
+        e, t, used = _oracle_all_cores(inp, nc, cores)
         tot_e += e
         tot_t += t
     v = tot_e / tot_t
-    sample = "first %d centres (%d edges) of %s per step, float64 C++ oracle, single thread" % (nc, tot_e // steps, name)
+    sample = "first %d centres (%d edges) of %s per step split into %d ranges, float64 C++ oracle, one thread per range" % (nc, tot_e // steps, name, used)
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": steps, "warmup": args.warmup,
         "ms_per_step": 1e3 * tot_t / steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
         "data": "synthetic", "config": {"workload": name, "sample": sample},
-        "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": used, "kind": "oracle", "sample": sample},
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
@@ -259,13 +283,34 @@ def run_ours(args):
     top = max(per_call_ms, key=per_call_ms.get)
     ach = abytes[top] / (per_call_ms[top] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": _ncu_traffic(name, top) if (args.mode == "onthefly" and not args.force_only) else None, "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top],
-                "ms_per_launch": per_call_ms[top]}
+                "traffic": _ncu_traffic(name, top) if (args.mode == "onthefly" and not args.force_only) else None,
+                "traffic_source": "committed ncu --set full capture, profiles/traffic.txt (not re-measured by this run)",
+                "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top], "ms_per_launch": per_call_ms[top],
+                "timing": "eager pass of the same %d steps with CUDA events around every call, run right after the timed graph replays "
+                          "(a replay cannot be split per kernel); the calls' sum can exceed ms_per_step by the launch gaps" % args.steps}
+    peaks = ab.measure_peaks()
+    peaks["hbm_gbs"] = peak
+    # forward only (configs[1]: "forward only, then forward+force VJP")
+    fwd = None
+    if not chunked:
+        for _ in range(3):
+            step.run_forward()
+        barrier()
+        f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        f0.record()
+        for _ in range(args.steps):
+            step.run_forward()
+        f1.record()
+        barrier()
+        fms = f0.elapsed_time(f1) / args.steps
+        fwd = {"ms_per_step": fms, "edges_per_s": E / (fms * 1e-3), "GBps_algorithmic": step.forward_bytes() / (fms * 1e-3) / 1e9,
+               "frac_of_hbm_peak": step.forward_bytes() / (fms * 1e-3) / 1e9 / peak, "launch": "eager"}
     step_bytes = sum(abytes[k] for k in per_call_ms)
     calls = {k: {"ms": round(per_call_ms[k], 4), "GB/s": round(abytes[k] / (per_call_ms[k] * 1e-3) / 1e9, 1),
                  "share": round(per_call_ms[k] / sum(per_call_ms.values()), 4)} for k in per_call_ms}
 
     # ---------------- end to end: host buffers in, forces + energy out, copies inside the timed region
+    e2e_md = None
     if chunked:
         e2e = None      # the host copy of V alone (86 GB at C3) does not fit pinned memory on the box: no end-to-end arm
     else:
@@ -285,7 +330,38 @@ def run_ours(args):
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
         e2e_ms = float(t.item()) / k_e2e
         e2e = {"value": E_all / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.h2d_bytes, "d2h_bytes_per_step": host.d2h_bytes,
-               "ms_per_step": e2e_ms, "steps": k_e2e}
+               "ms_per_step": e2e_ms, "steps": k_e2e,
+               "note": "allegro_layer_step_host: EVERY input of the step, the %.2f GB feature tensor V included, is copied from pinned host memory each "
+                       "step (PCIe-bound); e2e_md is the MD-shaped variant" % (E * inp["n"] * plan.dV * (4 if inp["dt"] == np.float32 else 8) / 1e9)}
+        # MD-shaped end to end: positions (edge vectors) in, forces + energy out, features and weights resident
+        h_rvec = torch.empty(dev["rvec"].shape, dtype=dev["rvec"].dtype, pin_memory=True).copy_(dev["rvec"])
+        h_F = torch.empty(step.F.shape, dtype=step.F.dtype, pin_memory=True)
+        h_e = torch.empty(step.e_tot.shape, dtype=step.e_tot.dtype, pin_memory=True)
+
+        def md_step():
+            dev["rvec"].copy_(h_rvec, non_blocking=True)
+            runner.run()
+            h_F.copy_(step.F, non_blocking=True)
+            h_e.copy_(step.e_tot, non_blocking=True)
+            torch.cuda.current_stream().synchronize()
+
+        for _ in range(3):
+            md_step()
+        barrier()
+        m0, m1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        m0.record()
+        for _ in range(args.steps):
+            md_step()
+        m1.record()
+        barrier()
+        t = torch.tensor([m0.elapsed_time(m1)], dtype=torch.float64, device="cuda")
+        if world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        md_ms = float(t.item()) / args.steps
+        e2e_md = {"value": E_all / (md_ms * 1e-3), "unit": UNIT, "ms_per_step": md_ms, "steps": args.steps,
+                  "h2d_bytes_per_step": int(h_rvec.numel() * h_rvec.element_size()),
+                  "d2h_bytes_per_step": int(h_F.numel() * h_F.element_size() + h_e.numel() * h_e.element_size()),
+                  "note": "edge vectors in from pinned host memory, forces and total energy out, host synchronised every step"}
 
     if rank == 0:
         line = {
@@ -300,7 +376,8 @@ def run_ours(args):
                        "fused_geometry": not args.separate_geometry},
             "atom_steps_per_s": N_all / (ms_step * 1e-3),
             "step_GBps_algorithmic": step_bytes / (ms_step * 1e-3) / 1e9, "step_frac_of_hbm_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
-            "roofline": roofline, "calls": calls, "clocks": clk, "e2e": e2e, "gpu_launches": int(launches),
+            "roofline": roofline, "calls": calls, "clocks": clk, "e2e": e2e, "e2e_md": e2e_md, "forward_only": fwd, "peaks": peaks,
+            "gpu_launches": int(launches),
         }
         line["config"]["launch"] = "eager call sequence" if args.no_graph else "CUDA graph replay of the step (%d kernels per step)" % runner.kernels_per_step
         if world == 1 and not args.no_cpu_baseline:

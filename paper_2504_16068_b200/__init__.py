@@ -66,6 +66,8 @@ SIGNATURES = {
     "allegro_latent_forward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_latent_backward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_add_inplace": (C.c_int, [C.c_long, C.c_int, _vp, _vp, _vp]),
+    "allegro_measure_fp32_fma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
+    "allegro_measure_tf32_mma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
     "allegro_status_str": (C.c_char_p, [C.c_int]),
     "allegro_last_error": (C.c_char_p, []),
     "allegro_launch_count": (C.c_long, []),
@@ -407,6 +409,14 @@ def latent_backward(rvec, r_cut, z, g_xnew, A, gV, g_rvec, g_x=None, stream=None
 def add_inplace(y, x, stream=None):
     _check(lib().allegro_add_inplace(y.numel(), _dt(y), _ptr(y), _ptr(x), _stream(stream)))
     return y
+
+
+def measure_peaks(stream=None):
+    """-> dict(fp32_fma_tflops, tf32_mma_tflops): roofline denominators measured on the current device"""
+    a, b = C.c_double(0.0), C.c_double(0.0)
+    _check(lib().allegro_measure_fp32_fma_peak(_stream(stream), C.byref(a)))
+    _check(lib().allegro_measure_tf32_mma_peak(_stream(stream), C.byref(b)))
+    return dict(fp32_fma_tflops=a.value, tf32_mma_tflops=b.value)
 
 
 def layer_step_host_workspace(plan, n_atoms, n_edges, n_basis, want_gV=True):

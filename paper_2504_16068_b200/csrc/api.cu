@@ -283,8 +283,8 @@ allegro_status_t allegro_tp_backward_energy(const allegro_plan_t* plan, int n_at
     ALLEGRO_CHECK_ARG(aligned16(out) && aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace),
                       "tensor not 16-byte aligned");
     ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
-    if (plan->wmode != ALLEGRO_W_SCALAR) {
-        set_error("allegro_tp_backward_energy: scalar path weights only");
+    if (plan->wmode != ALLEGRO_W_SCALAR && !(plan->dtype == ALLEGRO_F32 && plan->l_max == 2 && plan->n == 64 && path_w != nullptr && g_path_w == nullptr)) {
+        set_error("allegro_tp_backward_energy: scalar path weights, or dense weights with fp32, l_max = 2, n = 64");
         return ALLEGRO_EUNSUPPORTED;
     }
     TpArgs a{};

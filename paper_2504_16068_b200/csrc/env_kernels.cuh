@@ -477,6 +477,20 @@ __device__ __forceinline__ constexpr int natural_slot(int j) {  // Eenv-style in
     return 2 * l * l + ((l & 1) ? 2 * l + 1 : 0) + (j - l * l);
 }
 
+// Feature rows of 32 consecutive channels of one edge are ONE contiguous byte range in HBM: they are staged per warp in shared
+// memory and cross HBM as 16-byte vectors, lanes consecutive (a lane's own 72-byte row written or read directly costs nine
+// strided 8-byte requests per warp: 4x the transactions).
+template <typename T>
+__device__ __forceinline__ void warp_copy(T* __restrict__ dst, const T* __restrict__ src, int nelem, int lane) {
+    const bool vec = ((reinterpret_cast<uintptr_t>(dst) | reinterpret_cast<uintptr_t>(src)) & 15u) == 0 && (nelem * (int)sizeof(T)) % 16 == 0;
+    if (vec) {
+        const int nv = nelem * (int)sizeof(T) / 16;
+        for (int i = lane; i < nv; i += 32) reinterpret_cast<int4*>(dst)[i] = reinterpret_cast<const int4*>(src)[i];
+    } else {
+        for (int i = lane; i < nelem; i += 32) dst[i] = src[i];
+    }
+}
+
 template <typename T, int L, int NB>
 __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_x0,
                                                           const T* __restrict__ W_v0, T* __restrict__ x0, T* __restrict__ V0) {
@@ -486,25 +500,32 @@ __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double r
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long cb = (long)blockIdx.x * kGeoChunk;
     const int cnt = (int)min((long)kGeoChunk, E - cb);
+    T* stg = reinterpret_cast<T*>(geo_raw + ((sizeof(GeoSmem<T, L, NB>) + 15) / 16) * 16) + (size_t)warp * 32 * DV;   // [32 channels][DV] per warp
     if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
     __syncthreads();
     for (int le = warp; le < cnt; le += 8) {
         const size_t e = (size_t)(cb + le);
-        for (int ch = lane; ch < n; ch += 32) {
-            double sx = 0.0, sv = 0.0;
-            for (int b = 0; b < nb; ++b) {
-                const double bu = sm.Bs[le][b];
-                sx = fma((double)W_x0[ch * nb + b], bu, sx);
-                sv = fma((double)W_v0[ch * nb + b], bu, sv);
+        for (int ch0 = 0; ch0 < n; ch0 += 32) {
+            const int ch = ch0 + lane;
+            if (ch < n) {
+                double sx = 0.0, sv = 0.0;
+                for (int b = 0; b < nb; ++b) {
+                    const double bu = sm.Bs[le][b];
+                    sx = fma((double)W_x0[ch * nb + b], bu, sx);
+                    sv = fma((double)W_v0[ch * nb + b], bu, sv);
+                }
+                x0[e * n + ch] = (T)sx;
+                const T v0 = (T)sv;
+                T row[DV];
+#pragma unroll
+                for (int k = 0; k < DV; ++k) row[k] = T(0);
+#pragma unroll
+                for (int j = 0; j < DE; ++j) row[natural_slot<L>(j)] = v0 * sm.Ys[le][j];
+                row_store<T, DV>(stg + lane * DV, row);
             }
-            x0[e * n + ch] = (T)sx;
-            const T v0 = (T)sv;
-            T row[DV];
-#pragma unroll
-            for (int k = 0; k < DV; ++k) row[k] = T(0);
-#pragma unroll
-            for (int j = 0; j < DE; ++j) row[natural_slot<L>(j)] = v0 * sm.Ys[le][j];
-            row_store<T, DV>(V0 + (e * n + ch) * DV, row);
+            __syncwarp();
+            warp_copy<T>(V0 + (e * n + ch0) * DV, stg, min(32, n - ch0) * DV, lane);
+            __syncwarp();
         }
     }
 }
@@ -521,6 +542,7 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const long cb = (long)blockIdx.x * kGeoChunk;
     const int cnt = (int)min((long)kGeoChunk, E - cb);
+    T* stg = reinterpret_cast<T*>(geo_raw + ((sizeof(GeoSmem<T, L, NB>) + 15) / 16) * 16) + (size_t)warp * 32 * DV;   // [32 channels][DV] per warp
     if (tid < cnt) geo_phase1<T, L, NB, true>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
     __syncthreads();
     for (int le = warp; le < cnt; le += 8) {
@@ -529,9 +551,14 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
         double gbp[16];
 #pragma unroll
         for (int j = 0; j < 16; ++j) { gYp[j] = T(0); gbp[j] = 0.0; }
-        for (int ch = lane; ch < n; ch += 32) {
+        for (int ch0 = 0; ch0 < n; ch0 += 32) {
+            __syncwarp();
+            warp_copy<T>(stg, gV0 + (e * n + ch0) * DV, min(32, n - ch0) * DV, lane);
+            __syncwarp();
+            const int ch = ch0 + lane;
+            if (ch >= n) continue;
             T row[DV];
-            row_load<T, DV>(gV0 + (e * n + ch) * DV, row);
+            row_load<T, DV>(stg + lane * DV, row);
             double sv = 0.0;
             for (int b = 0; b < nb; ++b) sv = fma((double)W_v0[ch * nb + b], sm.Bs[le][b], sv);
             const T v0 = (T)sv;

@@ -59,14 +59,20 @@ allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a) {
                       : mix3_fwd_launch<Mix3::mask_natural_in()>(a, img_f);
 }
 #else
-template <bool GV, uint32_t PMASK>
+template <bool GV, uint32_t PMASK, bool COT>
 static allegro_status_t mix3_bwd_launch(const TpArgs& a, const float* img_b, float* gE_dst, int gE_by_item) {
-    auto k = mix3_bwd_kernel<GV, PMASK>;
+    auto k = mix3_bwd_kernel<GV, PMASK, COT>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
     k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv, img_b,
-                                                                (float*)a.gV, gE_dst, gE_by_item);
+                                                                (float*)a.gV, gE_dst, gE_by_item, (const float*)a.q, (float)a.kappa);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
+}
+template <uint32_t PMASK>
+static allegro_status_t mix3_bwd_pick(const TpArgs& a, const float* img_b, float* gE_dst, int gE_by_item) {
+    if (a.q != nullptr)   // allegro_tp_backward_energy: a.G is the forward result
+        return a.gV ? mix3_bwd_launch<true, PMASK, true>(a, img_b, gE_dst, gE_by_item) : mix3_bwd_launch<false, PMASK, true>(a, img_b, gE_dst, gE_by_item);
+    return a.gV ? mix3_bwd_launch<true, PMASK, false>(a, img_b, gE_dst, gE_by_item) : mix3_bwd_launch<false, PMASK, false>(a, img_b, gE_dst, gE_by_item);
 }
 allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst, int gE_by_item) {
     const int var = mix3_variant(a.plan);
@@ -74,12 +80,9 @@ allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst,
     float *img_f, *img_b;
     allegro_status_t s = mix3_images(a, &img_f, &img_b);
     if (s != ALLEGRO_OK) return s;
-    if (var == 0) return a.gV ? mix3_bwd_launch<true, Mix3::ALL>(a, img_b, gE_dst, gE_by_item) : mix3_bwd_launch<false, Mix3::ALL>(a, img_b, gE_dst, gE_by_item);
-    if (var == 1)
-        return a.gV ? mix3_bwd_launch<true, Mix3::mask_into(0)>(a, img_b, gE_dst, gE_by_item)
-                    : mix3_bwd_launch<false, Mix3::mask_into(0)>(a, img_b, gE_dst, gE_by_item);
-    return a.gV ? mix3_bwd_launch<true, Mix3::mask_natural_in()>(a, img_b, gE_dst, gE_by_item)
-                : mix3_bwd_launch<false, Mix3::mask_natural_in()>(a, img_b, gE_dst, gE_by_item);
+    return var == 0 ? mix3_bwd_pick<Mix3::ALL>(a, img_b, gE_dst, gE_by_item)
+           : var == 1 ? mix3_bwd_pick<Mix3::mask_into(0)>(a, img_b, gE_dst, gE_by_item)
+                      : mix3_bwd_pick<Mix3::mask_natural_in()>(a, img_b, gE_dst, gE_by_item);
 }
 #endif
 

@@ -129,6 +129,13 @@ __global__ void __launch_bounds__(256) edge_energy_kernel(int n, int dV, long E,
     const T* o = out + (size_t)e * len;
     T* g = G ? G + (size_t)e * len : nullptr;
     T acc = T(0);
+    if (kappa == T(0) && g == nullptr) {   // pure linear readout of the scalars: only component 0 of every row is touched
+        for (int ch = lane; ch < n; ch += 32) acc = fma(q[ch], o[(size_t)ch * dV], acc);
+#pragma unroll
+        for (int o2 = 16; o2 > 0; o2 >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o2);
+        if (lane == 0 && e_edge) e_edge[e] = acc;
+        return;
+    }
     for (int idx = lane; idx < len; idx += 32) {
         const T v = o[idx];
         const int ch = idx / dV, k = idx - ch * dV;

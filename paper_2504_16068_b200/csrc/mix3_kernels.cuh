@@ -402,11 +402,14 @@ struct Mix3BBars {
     uint32_t tmem_slot;
 };
 
-template <bool WANT_GV, uint32_t PMASK>
+// COT: G points at the forward result `out` and the cotangent of the A12 energy, q (x) delta_{k,0} + kappa out, is formed while the
+// tile is staged (G never exists in HBM).
+template <bool WANT_GV, uint32_t PMASK, bool COT>
 __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                     const float* __restrict__ G, const float* __restrict__ V,
                                                                     const float* __restrict__ Eenv, const float* __restrict__ img,
-                                                                    float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item) {
+                                                                    float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item,
+                                                                    const float* __restrict__ qvec, float kappa) {
     using MB = Mix3B;
     using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
@@ -491,6 +494,8 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
         for (int j = 0; j < DE; ++j) { E[j] = Eenv[((size_t)c * 64 + n) * DE + j]; gE[j] = 0.f; }
         // operand mapping: thread = (slot, n'), rows of edges 4 slot + j; byte offset of element (row of e, k = n') for M = 0, block row 0
         const int np = tid & 63, slot = tid >> 6;
+        float qn = 0.f;
+        if constexpr (COT) qn = qvec[np];
         uint32_t goff[4];
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
@@ -507,6 +512,11 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
                 float g[DV];
                 if (e < e1) {
                     row_load<float, DV>(G + ((size_t)e * 64 + np) * DV, g);
+                    if constexpr (COT) {
+#pragma unroll
+                        for (int k = 0; k < DV; ++k) g[k] *= kappa;
+                        g[0] += qn;
+                    }
                 } else {
 #pragma unroll
                     for (int k = 0; k < DV; ++k) g[k] = 0.f;

@@ -132,6 +132,25 @@ class SingleLayerStep:
             self.marks = ev
         return self.F, self.e_tot
 
+    def run_forward(self):
+        """forward only (BASELINE.json:configs[1]: "forward only, then forward+force VJP"): embedding, tensor product with the
+        energy epilogue, energy sum"""
+        p, d, it = self.plan, self.dev, self.items
+        rp, rvec, V = d["row_ptr"], d["rvec"], d["V"]
+        if self.fused_geometry:
+            ab.env_radial_forward(p, rp, rvec, d["W_r"], self.rc, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env)
+        else:
+            ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w)
+            ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env)
+        ab.tp_forward_energy(p, rp, V, self.Eenv, None, d["q"], self.kappa, items=it, out=self.out, e_edge=self.e_edge, want_G=False)
+        ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot)
+        return self.e_tot
+
+    def forward_bytes(self):
+        b = self.algorithmic_bytes()
+        return (b["env_radial_forward"] if self.fused_geometry else b["radial_forward"] + b["env_embed"]) + 2 * self.E * self.plan.n * self.plan.dV * (
+            4 if self.plan.dtype == ab.F32 else 8) + b["segment_sum"]
+
     def algorithmic_bytes(self):
         """HBM bytes each call must move at least once: dict name -> bytes per step"""
         p = self.plan
@@ -320,8 +339,11 @@ class TwoLayerStep:
             timed("tp_forward_dense", lambda: ab.tp_forward(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
             if l < L - 1:
                 timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], self.V[l + 1], p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
-        G = self.cot[0]
-        timed("edge_energy", lambda: ab.edge_energy(pd, self.V[L], p["q"], 0.0, e_edge=self.e_edge, G=G))
+        # readout E = sum_e sum_n q[n] V_L[e][n][0e]; its cotangent q (x) delta_{k,0} is formed inside the last layer's VJP when
+        # that kernel exists (fp32, l_max 2, n 64), otherwise materialised here
+        fused_cot = pd.dtype == ab.F32 and pd.l_max == 2 and pd.n == 64
+        G = self.V[L] if fused_cot else self.cot[0]
+        timed("edge_energy", lambda: ab.edge_energy(pd, self.V[L], p["q"], 0.0, e_edge=self.e_edge, want_G=not fused_cot, G=None if fused_cot else G))
         g_x_next, have_gr = None, False
         for l in reversed(range(L)):
             g_x = None
@@ -330,7 +352,11 @@ class TwoLayerStep:
                 timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], G, self.g_r, g_x=g_x))
             gVl = self.cot[1] if G is self.cot[0] else self.cot[0]
             pl = self.pd_last if l == L - 1 else (self.pd_first if l == 0 else pd)
-            timed("tp_backward_dense", lambda: ab.tp_backward(pl, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
+            if l == L - 1 and fused_cot:
+                timed("tp_backward_dense", lambda: ab.tp_backward_energy(pl, rp, self.V[L], self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, gV=gVl,
+                                                                         gEenv=self.gEenv, workspace=self.ws))
+            else:
+                timed("tp_backward_dense", lambda: ab.tp_backward(pl, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
             if not have_gr:
                 timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r, g_w=self.g_w))
                 have_gr = True
@@ -348,6 +374,14 @@ class TwoLayerStep:
         timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
         self.marks = ev
         return self.F, self.e_tot
+
+    def algorithmic_bytes(self):
+        """HBM bytes the dense tensor-product calls must move at least once (V in, out out; VJP: cotangent and V in,
+        gV out; Eenv / gEenv per centre), summed over layers"""
+        pd = self.pd
+        s = 4 if pd.dtype == ab.F32 else 8
+        feat, env = self.E * pd.n * pd.dV * s, self.N * pd.n * pd.dE * s
+        return {"tp_forward_dense": self.L * (2 * feat + env), "tp_backward_dense": self.L * (3 * feat + 2 * env)}
 
     def algorithmic_flops(self):
         """FP32 flops the dense tensor-product calls must execute (sparse CG 806 flop per channel-edge forward,
