@@ -45,6 +45,7 @@ def parse_args():
     ap.add_argument("--chunks", type=int, default=1, help="process the centres in this many chunks (C3 defaults to 16)")
     ap.add_argument("--no-graph", action="store_true", help="time the eager call sequence instead of CUDA-graph replays of the step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--replicas", action="store_true", help="N > 1: one independent system per rank (weak scaling) instead of one sharded system")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
     return ap.parse_args()
 
@@ -210,18 +211,28 @@ def run_ours(args):
     name = args.workload
     if name in ("C2", "C2s"):
         return run_two_layer(args, rank, world, local, dist, barrier_factory=None)
-    # multi-GPU: the path partitions over independent systems -- rank r owns the system of seed r;
-    # no data-path collective, weak scaling
-    inp = make_inputs(name, seed=rank, features="device")
-    dev = to_device(inp)
+    # multi-GPU: ONE system (seed 0) sharded by centre atom over the ranks -- every rank runs the kernels on its own CSR
+    # rows, the only exchange is the halo of cut-edge g_r rows before the owners gather their forces (sharding.py): strong scaling.
+    # --replicas: rank r owns the independent system of seed r instead (no data-path collective, weak scaling); C3 (chunked) always.
+    sharded = world > 1 and not args.replicas and name != "C3" and args.chunks <= 1
+    inp = make_inputs(name, seed=0 if sharded else rank, features="device")
     plan = ab.Plan(inp["lmax"], inp["n"], ab.F64 if inp["dt"] == np.float64 else ab.F32, ab.W_SCALAR)
+    sh = None
+    if sharded:
+        from paper_2504_16068_b200.pipeline import shard_to_device
+        from paper_2504_16068_b200.sharding import ShardedForces
+        sh = ShardedForces(inp["row_ptr"], inp["rev"], device="cuda", dtype=plan.tdtype)
+        dev = shard_to_device(inp, sh)
+        args.no_graph = True          # the halo exchange (NCCL send / recv) stays outside a captured graph
+    else:
+        dev = to_device(inp)
     chunked = name == "C3" or args.chunks > 1
     if chunked:      # feature tensors that do not fit HBM four times: V resident, work buffers per centre chunk
         step = ChunkedStep(plan, dev, inp["row_ptr"], inp["rc"], inp["kappa"], inp["scale"], n_chunks=max(args.chunks, 16 if name == "C3" else 1),
                            want_gV=not args.force_only)
     else:
         step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only, mode=args.mode,
-                               fused_geometry=not args.separate_geometry)
+                               fused_geometry=not args.separate_geometry, sharded=sh)
     E, N = step.E, step.N
 
     def barrier():
@@ -263,7 +274,7 @@ def run_ours(args):
     if world > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
     ms_step = float(t.item()) / args.steps
-    tot = torch.tensor([float(E), float(N)], dtype=torch.float64, device="cuda")     # every rank owns its own system (seed = rank)
+    tot = torch.tensor([float(E), float(N)], dtype=torch.float64, device="cuda")     # rank-local edges / atoms: the sum is the whole job
     if world > 1:
         dist.all_reduce(tot, op=dist.ReduceOp.SUM)
     E_all, N_all = float(tot[0].item()), float(tot[1].item())
@@ -314,23 +325,25 @@ def run_ours(args):
     if chunked:
         e2e = None      # the host copy of V alone (86 GB at C3) does not fit pinned memory on the box: no end-to-end arm
     else:
-        host = HostStep(step, inp)
-        for _ in range(3):
-            host.run()
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        host = None if sharded else HostStep(step, inp)     # the one-call host entry point is single-GPU
         k_e2e = max(3, min(args.steps, 10))
-        e0.record()
-        for _ in range(k_e2e):
-            host.run()
-        e1.record()
-        barrier()
-        t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
-        if world > 1:
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item()) / k_e2e
-        e2e = {"value": E_all / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.h2d_bytes, "d2h_bytes_per_step": host.d2h_bytes,
-               "ms_per_step": e2e_ms, "steps": k_e2e,
+        e2e_ms = float("nan")
+        if host is not None:
+            for _ in range(3):
+                host.run()
+            barrier()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(k_e2e):
+                host.run()
+            e1.record()
+            barrier()
+            t = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+            if world > 1:
+                dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_ms = float(t.item()) / k_e2e
+        e2e = None if host is None else {"value": E_all / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": host.h2d_bytes, "d2h_bytes_per_step": host.d2h_bytes,
+                                         "ms_per_step": e2e_ms, "steps": k_e2e,
                "note": "allegro_layer_step_host: EVERY input of the step, the %.2f GB feature tensor V included, is copied from pinned host memory each "
                        "step (PCIe-bound); e2e_md is the MD-shaped variant" % (E * inp["n"] * plan.dV * (4 if inp["dt"] == np.float32 else 8) / 1e9)}
         # MD-shaped end to end: positions (edge vectors) in, forces + energy out, features and weights resident
@@ -362,16 +375,21 @@ def run_ours(args):
                   "h2d_bytes_per_step": int(h_rvec.numel() * h_rvec.element_size()),
                   "d2h_bytes_per_step": int(h_F.numel() * h_F.element_size() + h_e.numel() * h_e.element_size()),
                   "note": "edge vectors in from pinned host memory, forces and total energy out, host synchronised every step"}
+        if sharded:      # the end-to-end arm of a sharded run is the MD-shaped one (every rank: its edge vectors in, its atoms' forces out)
+            e2e, e2e_md = e2e_md, None
 
     if rank == 0:
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
             "dtype": "f32" if inp["dt"] == np.float32 else "f64", "data": "synthetic",
-            "config": {"workload": "%s: BASELINE.json configs recipe, %d atoms, %d directed edges per GPU, l_max=%d, n=%d, "
-                                   "single TP layer forward + %s" % (name, N, E, inp["lmax"], inp["n"],
+            "config": {"workload": "%s: BASELINE.json configs recipe, %d atoms, %d directed edges %s, l_max=%d, n=%d, "
+                                   "single TP layer forward + %s" % (name, int(N_all) if sharded else N, int(E_all) if sharded else E,
+                                                                     "in ONE system sharded over the GPUs" if sharded else "per GPU", inp["lmax"], inp["n"],
                                                                      "force-only VJP" if args.force_only else "full VJP (gV, gEenv) + forces"),
-                       "atoms": N, "edges": E, "l_max": inp["lmax"], "n_channels": inp["n"], "parallelism": "independent systems per GPU", "mode": args.mode,
+                       "atoms": int(N_all) if sharded else N, "edges": int(E_all) if sharded else E, "l_max": inp["lmax"], "n_channels": inp["n"],
+                       "parallelism": ("centres of one system sharded over %d GPUs, halo exchange of %d bytes of cut-edge g_r per step from rank 0"
+                                       % (world, sh.halo_bytes)) if sharded else "independent systems per GPU", "mode": args.mode,
                        "l2": "not flushed: every feature tensor (%.2f GB) exceeds the 126 MB L2" % (E * inp["n"] * plan.dV * (4 if inp["dt"] == np.float32 else 8) / 1e9),
                        "fused_geometry": not args.separate_geometry},
             "atom_steps_per_s": N_all / (ms_step * 1e-3),
@@ -399,10 +417,18 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
     from paper_2504_16068_b200.pipeline import TwoLayerStep
     from workloads.inputs import make_model_inputs
     name = args.workload
-    inp = make_model_inputs(name, seed=rank)
+    sharded = world > 1 and not args.replicas      # one system, centres sharded over the ranks (strong scaling); see run_ours
+    inp = make_model_inputs(name, seed=0 if sharded else rank)
     p = inp["params"]
     td = torch.float32 if inp["dt"] == np.float32 else torch.float64
-    dev = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).cuda() for k in ("row_ptr", "rev", "rvec")}
+    sh = None
+    if sharded:
+        from paper_2504_16068_b200.pipeline import shard_to_device
+        from paper_2504_16068_b200.sharding import ShardedForces
+        sh = ShardedForces(inp["row_ptr"], inp["rev"], device="cuda", dtype=td)
+        dev = shard_to_device(inp, sh, keys_edge=("rvec",), keys_full=())
+    else:
+        dev = {k: torch.from_numpy(np.ascontiguousarray(inp[k])).cuda() for k in ("row_ptr", "rev", "rvec")}
     prm = {k: torch.from_numpy(np.ascontiguousarray(p[k])).to(td).cuda() for k in ("W_x0", "W_v0", "W_w", "W_p", "A_lat", "q")}
     prm.update(rc=p["rc"], scale=p["scale"])
     dt = ab.F32 if inp["dt"] == np.float32 else ab.F64
@@ -413,8 +439,12 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
     plan_first = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
     plan_first.set_in_blocks(0x19)
     step = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=plan_last,
-                        plan_first=plan_first)
+                        plan_first=plan_first, sharded=sh)
     E, N = step.E, step.N
+    tot = torch.tensor([float(E), float(N)], dtype=torch.float64, device="cuda")     # rank-local edges / atoms: the sum is the whole job
+    if world > 1:
+        dist.all_reduce(tot, op=dist.ReduceOp.SUM)
+    E_all, N_all = float(tot[0].item()), float(tot[1].item())
 
     def barrier():
         torch.cuda.synchronize()
@@ -452,15 +482,16 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
     per_call_ms = {k: sum(v) / len(v) for k, v in per_call.items()}
     flops = step.algorithmic_flops()
     top = max(per_call_ms, key=per_call_ms.get)
-    # the dense per-path mix runs on the tensor cores (mma.sync TF32, 3xTF32 split): tensor roofline for TF32 = the measured
-    # bf16 GEMM peak x the guide's nominal ratio 1.1 / 2.25 (B200_PROFILING.md); `achieved` counts ALGORITHMIC fp32 flops
-    # (one multiply-add per weight element and column), not the three TF32 MMAs each of them costs
-    mp = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(mp):
-        with open(mp) as f:
-            peak, peak_src = float(json.load(f)["bf16_tflops"]) * 1.1 / 2.25, "measured bf16_tflops (MEASURED_PEAKS.json) x 1.1/2.25 nominal tf32/bf16 ratio"
-    else:
-        peak, peak_src = 1590.0 * 1.1 / 2.25, "fallback 1.59 PFLOP/s bf16 (B200_PROFILING.md) x 1.1/2.25"
+    # The dense per-path mix runs on the tensor cores (tcgen05.mma kind::tf32, fp32 operands split hi / lo, four products per
+    # multiply-add).  Tensor roofline: the TF32 tcgen05 rate measured in this run (M 128, N 256, one CTA per SM); `achieved`
+    # counts ALGORITHMIC fp32 flops (one multiply-add per weight element and column), not the four TF32 MMAs each of them costs.
+    peaks = ab.measure_peaks()
+    hbm_peak, hbm_src = measured_peaks()
+    peaks["hbm_gbs"] = hbm_peak
+    peak, peak_src = peaks["tf32_mma_tflops"], "measured in this run: tcgen05.mma kind::tf32, M 128 x N 256 x K 8, one CTA per SM (allegro_measure_tf32_mma_peak)"
+    abytes = step.algorithmic_bytes()
+    tp_ms = per_call_ms.get("tp_forward_dense", 0.0) + per_call_ms.get("tp_backward_dense", 0.0)
+    tp_bytes = abytes["tp_forward_dense"] + abytes["tp_backward_dense"]
     ach = flops.get(top, 0) / (per_call_ms[top] * 1e-3) / 1e12
     # end to end: rvec (the positions) in from pinned host memory, forces and energy out, every step
     h_rvec = torch.empty(dev["rvec"].shape, dtype=dev["rvec"].dtype, pin_memory=True).copy_(dev["rvec"])
@@ -486,18 +517,29 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
     e2e_ms = e0.elapsed_time(e1) / k_e2e
     if rank == 0:
         line = {
-            "metric": METRIC, "value": world * E / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32" if inp["dt"] == np.float32 else "f64",
+            "metric": METRIC, "value": E_all / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if sharded else "weak", "vs_baseline": None,
+            "dtype": "f32" if inp["dt"] == np.float32 else "f64",
             "data": "synthetic",
             "config": {"workload": "%s: BASELINE.json configs[2] recipe, %d atoms, %d directed edges per GPU, l_max=%d, n=%d, %d layers with dense "
                                    "per-path mix, forward + force backward as one MD step" % (name, N, E, p["lmax"], p["n"], p["n_layers"]),
-                       "atoms": N, "edges": E, "l2": "not flushed: feature tensors (%.2f GB each) exceed the 126 MB L2" % (E * p["n"] * step.pd.dV * 4 / 1e9)},
-            "atom_steps_per_s": world * N / (ms_step * 1e-3),
+                       "atoms": int(N_all) if sharded else N, "edges": int(E_all) if sharded else E,
+                       "parallelism": ("centres of one system sharded over %d GPUs, halo exchange of cut-edge g_r" % world) if sharded else "independent systems per GPU",
+                       "block_subsets": "first layer: paths from the natural-parity blocks of V0 only (15 of 30); last layer: paths into 0e only (3 of 30)",
+                       "l2": "not flushed: feature tensors (%.2f GB each) exceed the 126 MB L2" % (E * p["n"] * step.pd.dV * 4 / 1e9)},
+            "atom_steps_per_s": N_all / (ms_step * 1e-3),
             "roofline": {"bound": "tensor", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
-                         "peak_source": peak_src, "note": "tf32 via legacy mma.sync with a 3xTF32 split; algorithmic fp32 flops"},
+                         "peak_source": peak_src, "note": "algorithmic fp32 flops of all layers' calls of this name; every multiply-add costs four TF32 MMAs "
+                                                          "(hi / lo split of both operands) on tcgen05",
+                         "timing": "CUDA events around every call inside the timed steps"},
+            # reading A15 holds the tensor-product part of C2 to the HBM roofline as well: bytes the dense TP calls must move / their time
+            "tp_hbm_roofline": {"bound": "hbm", "calls": ["tp_forward_dense", "tp_backward_dense"], "algorithmic_bytes_per_step": tp_bytes,
+                                "ms_per_step": tp_ms, "achieved": tp_bytes / (tp_ms * 1e-3) / 1e9 if tp_ms > 0 else None, "peak": hbm_peak, "unit": "GB/s",
+                                "frac": tp_bytes / (tp_ms * 1e-3) / 1e9 / hbm_peak if tp_ms > 0 else None, "peak_source": hbm_src},
+            "peaks": peaks,
             "calls": {k: {"ms": round(v, 4), "share": round(v / sum(per_call_ms.values()), 4)} for k, v in per_call_ms.items()},
             "clocks": clk,
-            "e2e": {"value": world * E / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h_rvec.numel() * h_rvec.element_size()),
+            "e2e": {"value": E_all / (e2e_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h_rvec.numel() * h_rvec.element_size()),
                     "d2h_bytes_per_step": int(h_F.numel() * h_F.element_size() + h_e.numel() * h_e.element_size()), "ms_per_step": e2e_ms, "steps": k_e2e},
             "gpu_launches": int(launches),
         }

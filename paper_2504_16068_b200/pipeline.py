@@ -56,8 +56,13 @@ class SingleLayerStep:
     `fused_geometry`: env_radial_forward / env_radial_backward (w and g_w never exist in HBM) instead of
     radial_forward + env_embed / env_embed_backward + radial_backward."""
 
-    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, mode="onthefly", fused_geometry=True):
+    def __init__(self, plan, dev, rc, kappa, scale=1.0, want_gV=True, want_g_path_w=False, items=None, mode="onthefly", fused_geometry=True,
+                 sharded=None):
+        """sharded: a sharding.ShardedForces when `dev` holds ONE RANK'S rows of a system split over several GPUs (row_ptr / rev are the
+        rank-local index arrays of its HaloPlan): g_r is written into its extended array, the halo exchange runs before the force
+        gather, energies (and g_path_w) are summed over the ranks"""
         assert mode in ("separate", "epilogue", "onthefly")
+        self.sharded = sharded
         self.plan, self.dev, self.rc, self.kappa, self.scale, self.mode = plan, dev, rc, kappa, scale, mode
         self.fused_geometry = fused_geometry
         rp, rvec, V = dev["row_ptr"], dev["rvec"], dev["V"]
@@ -73,7 +78,7 @@ class SingleLayerStep:
         self.gV = torch.empty_like(V) if want_gV else None
         self.gEenv = torch.empty_like(self.Eenv)
         self.g_path_w = torch.empty((plan.P,), dtype=dt, device=dv) if want_g_path_w else None
-        self.g_r = torch.empty_like(rvec)
+        self.g_r = torch.empty_like(rvec) if sharded is None else sharded.g_local
         self.g_w = None if fused_geometry else torch.empty_like(self.w)
         self.F = torch.empty((self.N, 3), dtype=dt, device=dv)
         self.e_tot = torch.empty((1,), dtype=dt, device=dv)
@@ -126,8 +131,16 @@ class SingleLayerStep:
         else:
             timed("env_embed_backward", lambda: ab.env_embed_backward(p, rp, self.gEenv, rvec, self.w, self.scale, g_rvec=self.g_r, g_w=self.g_w))
             timed("radial_backward", lambda: ab.radial_backward(rvec, d["W_r"], self.rc, self.g_w, self.g_r))
-        timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
-        timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        if self.sharded is None:
+            timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
+            timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        else:
+            timed("halo_exchange", self.sharded.exchange)
+            timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.sharded.g_ext, F=self.F))
+            timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+            timed("energy_all_reduce", lambda: self.sharded.reduce_sum(self.e_tot))
+            if self.g_path_w is not None:
+                self.sharded.reduce_sum(self.g_path_w)
         if mark:
             self.marks = ev
         return self.F, self.e_tot
@@ -292,8 +305,9 @@ class TwoLayerStep:
     `plan_first`: optional dense plan restricted to the natural-parity input blocks (Plan.set_in_blocks(0x19)) for the first
     layer, whose input V0 = v (x) Y has zeros in the other blocks (reading A19): half of the paths never run."""
 
-    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None):
+    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None, sharded=None):
         self.pd, self.ps, self.dev, self.p = plan_dense, plan_scalar, dev, params
+        self.sharded = sharded      # sharding.ShardedForces: `dev` holds one rank's rows (see SingleLayerStep)
         self.pd_last = plan_last if plan_last is not None else plan_dense
         self.pd_first = plan_first if plan_first is not None else plan_dense
         self.L = params["W_w"].shape[0]
@@ -310,7 +324,7 @@ class TwoLayerStep:
         self.gEenv = new(N, n, plan_dense.dE)
         self.cot = [new(E, n, dV), new(E, n, dV)]          # ping-pong cotangents of V_l
         self.g_w, self.g_x, self.g_x2 = new(E, n), new(E, n), new(E, n)
-        self.g_r, self.g_r_tmp = new(E, 3), new(E, 3)
+        self.g_r, self.g_r_tmp = (new(E, 3) if sharded is None else sharded.g_local), new(E, 3)
         self.e_edge, self.e_tot, self.F = new(E), new(1), new(N, 3)
         self.e_ptr = torch.tensor([0, E], dtype=torch.int32, device=dv)
         self.ws = torch.empty(16, dtype=torch.uint8, device=dv)
@@ -370,8 +384,14 @@ class TwoLayerStep:
                 timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x, accumulate=True))
             G, g_x_next = gVl, g_x
         timed("edge_embed_backward", lambda: ab.edge_embed_backward(pd, rvec, p["W_x0"], p["W_v0"], rc, g_x_next, G, self.g_r))
-        timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
-        timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        if self.sharded is None:
+            timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
+            timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+        else:
+            timed("halo_exchange", self.sharded.exchange)
+            timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.sharded.g_ext, F=self.F))
+            timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
+            timed("energy_all_reduce", lambda: self.sharded.reduce_sum(self.e_tot))
         self.marks = ev
         return self.F, self.e_tot
 
@@ -392,6 +412,22 @@ class TwoLayerStep:
         dT = {1: 22, 2: 102, 3: 312}[pd.l_max]
         mix = 2 * n * n * dT
         return {"tp_forward_dense": L * self.E * (cg_fwd + mix), "tp_backward_dense": L * self.E * (2 * cg_fwd + mix)}
+
+
+def shard_to_device(inp, sharded, keys_edge=("rvec", "V"), keys_full=("W_r", "path_w", "q"), device="cuda"):
+    """One rank's rows of the host problem `inp` as device tensors: row_ptr / rev become the rank-local index arrays of the
+    HaloPlan, per-edge tensors are sliced to the rank's edge range [e0, e1), parameters are replicated."""
+    hp = sharded.plan
+    dev = dict(row_ptr=torch.from_numpy(hp.row_ptr_loc).to(device), rev=torch.from_numpy(hp.rev_loc).to(device))
+    for k in keys_edge:
+        if inp.get(k) is not None:
+            v = inp[k][hp.e0:hp.e1]
+            dev[k] = (v if hasattr(v, "detach") else torch.from_numpy(np.ascontiguousarray(v))).to(device).contiguous()
+    for k in keys_full:
+        if inp.get(k) is not None:
+            v = inp[k]
+            dev[k] = (v if hasattr(v, "detach") else torch.from_numpy(np.ascontiguousarray(v))).to(device)
+    return dev
 
 
 class GraphedStep:

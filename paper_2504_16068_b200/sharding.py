@@ -1,12 +1,16 @@
-"""Multi-GPU host logic: Allegro is strictly local, E_tot = sum_i eps_i(edges of centre i), so the
-path shards by CENTRE ATOM with no data-path collective in the forward pass or in the tensor-product / embedding
-VJPs.  The one exchange is the force assembly: atom a needs g_r of the reverse edges of its row, which other ranks
-own.  Here every rank all-gathers the per-edge gradients g_r[E,3] (12 bytes per edge: 4.4 MB at C1, 35 MB at C2;
-latency-bound over NVLink/NVSwitch) and then gathers the forces of ITS OWN atoms with the deterministic CSR
-force_gather (no scatter-add, no float atomics), as a spatial-decomposition MD code keeps forces with the owner.
+"""Multi-GPU (spatial decomposition with a halo exchange per step): Allegro is strictly
+local, E_tot = sum_i eps_i(edges of centre i), so ONE system shards by CENTRE ATOM -- contiguous CSR row ranges balanced by
+edge count -- with no data-path collective in the forward pass or in the tensor-product / embedding VJPs: every rank runs the
+library's kernels on its own rows.  The one exchange is the force assembly (row a7): atom a needs g_r of the REVERSE edges of
+its row, and the reverse of a cut edge (a -> j, j owned elsewhere) lives on j's owner.  Each rank therefore sends the g_r rows
+of its cut edges to the ranks that own their far ends (12 bytes per cut edge, point to point: NCCL send/recv over
+NVLink/NVSwitch on GPUs, gloo on CPU), appends what it receives to its own g_r and gathers the forces of ITS OWN atoms with the
+same deterministic CSR force_gather kernel as the single-GPU path.  The owner's forces are bitwise those of a single-GPU
+run: same kernel, same per-atom order, same operand bits.  (How many edges are cut depends on how the atoms are numbered: a
+spatially sorted numbering cuts a surface layer, the random numbering of the synthetic boxes cuts about (1 - 1/world) of them.)
 
-The compute itself is injected (`compute_g_r`): on a GPU box it is the library's kernels on the rank's rows, in the
-CPU tests it is the oracle; only the partition, the padding and the collective live here.
+The compute itself is injected by the caller (pipeline.ShardedStep binds the CUDA kernels; the CPU tests bind the oracle or a
+stub): only the partition, the index lists and the exchange live here.
 """
 import numpy as np
 import torch
@@ -23,32 +27,89 @@ def partition_centres(row_ptr, world):
     return [(cuts[r], cuts[r + 1]) for r in range(world)]
 
 
-class ShardedForces:
-    """rank-local piece of one MD step: run compute_g_r on the rank's centres, exchange g_r, gather own forces.
+class HaloPlan:
+    """Index lists of one rank (host integers, built once per neighbour list).
 
-    compute_g_r(c_lo, c_hi) -> (g_r_local [E_local, 3] tensor, energy_local 0-d tensor)
-    force_gather(row_ptr_slice, rev, g_r_all) -> F_local [c_hi - c_lo, 3] tensor   (row_ptr_slice keeps GLOBAL edge offsets)
+    local edge k = global edge e0 + k.  rev_loc[k] indexes the EXTENDED array [own g_r rows (E_loc) ; halo rows (n_halo)]:
+    the own row of the reverse edge when it is local, else the halo slot that the owner's row is received into.
+    send_idx[d]: local edge offsets (ascending) whose g_r rows rank d needs; recv_off[s] / recv_cnt[s]: the halo slice filled
+    by rank s.  Both sides enumerate a rank pair's rows in ascending order of the SENDER's global edge index."""
+
+    def __init__(self, row_ptr, rev, world, rank):
+        rp = np.asarray(row_ptr, dtype=np.int64)
+        rev = np.asarray(rev, dtype=np.int64)
+        self.world, self.rank = world, rank
+        self.parts = partition_centres(rp, world)
+        self.edge_ranges = [(int(rp[a]), int(rp[b])) for a, b in self.parts]
+        self.c_lo, self.c_hi = self.parts[rank]
+        self.e0, self.e1 = self.edge_ranges[rank]
+        self.n_local = self.e1 - self.e0
+        starts = np.array([er[0] for er in self.edge_ranges] + [int(rp[-1])], dtype=np.int64)
+        r_loc = rev[self.e0:self.e1]                                   # global index of every own edge's reverse
+        owner = np.searchsorted(starts, r_loc, side="right") - 1       # rank that owns it (empty ranges own nothing)
+        rev_loc = np.where(owner == rank, r_loc - self.e0, -1)
+        self.recv_off, self.recv_cnt, self.send_idx = [0] * world, [0] * world, [np.zeros(0, dtype=np.int64)] * world
+        off = self.n_local
+        for s in range(world):
+            if s == rank:
+                continue
+            mine = np.nonzero(owner == s)[0]                           # own edges whose reverse lives on s
+            need = r_loc[mine]                                         # ... the rows of s that this rank needs
+            order = np.argsort(need, kind="stable")
+            self.recv_off[s], self.recv_cnt[s] = off, int(mine.shape[0])
+            rev_loc[mine[order]] = off + np.arange(mine.shape[0])
+            off += int(mine.shape[0])
+            # s needs exactly the reverses of those edges: this rank's edges `mine` themselves, in ascending order
+            self.send_idx[s] = np.sort(mine)
+        self.n_halo = off - self.n_local
+        assert (rev_loc >= 0).all()
+        self.rev_loc = rev_loc.astype(np.int32)
+        self.row_ptr_loc = (rp[self.c_lo:self.c_hi + 1] - self.e0).astype(np.int32)
+
+
+class ShardedForces:
+    """rank-local state of the force assembly: the extended g_r array, the exchange, the energy reduction.
+
+        sh = ShardedForces(row_ptr, rev, device=..., dtype=...)
+        ... write the g_r rows of the rank's own edges into sh.g_local (a view of sh.g_ext) ...
+        sh.exchange()                       # halo rows arrive in sh.g_ext[n_local:]
+        F_loc = force_gather(sh.plan.row_ptr_loc, sh.plan.rev_loc, sh.g_ext)      # forces of atoms [c_lo, c_hi)
     """
 
-    def __init__(self, row_ptr, rev, compute_g_r, force_gather, group=None):
+    def __init__(self, row_ptr, rev, device="cpu", dtype=torch.float64, group=None):
         self.group = group
         self.world, self.rank = dist.get_world_size(group), dist.get_rank(group)
-        self.row_ptr = np.asarray(row_ptr, dtype=np.int32)
-        self.rev = rev
-        self.parts = partition_centres(self.row_ptr, self.world)
-        self.edge_ranges = [(int(self.row_ptr[a]), int(self.row_ptr[b])) for a, b in self.parts]
-        self.pad = max(e1 - e0 for e0, e1 in self.edge_ranges)
-        self.compute_g_r, self.force_gather = compute_g_r, force_gather
+        self.plan = HaloPlan(row_ptr, rev, self.world, self.rank)
+        p = self.plan
+        self.g_ext = torch.zeros((p.n_local + p.n_halo, 3), dtype=dtype, device=device)
+        self.g_local = self.g_ext[:p.n_local]
+        self.send_idx = [torch.from_numpy(ix).to(device) for ix in p.send_idx]
+        self.send_buf = [torch.empty((ix.shape[0], 3), dtype=dtype, device=device) for ix in p.send_idx]
+        self.halo_bytes = int(sum(b.numel() * b.element_size() for b in self.send_buf))
 
-    def run(self):
-        c_lo, c_hi = self.parts[self.rank]
-        g_loc, e_loc = self.compute_g_r(c_lo, c_hi)
-        buf = torch.zeros((self.pad, 3), dtype=g_loc.dtype, device=g_loc.device)
-        buf[: g_loc.shape[0]] = g_loc
-        gathered = [torch.empty_like(buf) for _ in range(self.world)]
-        dist.all_gather(gathered, buf, group=self.group)
-        g_all = torch.cat([gathered[r][: e1 - e0] for r, (e0, e1) in enumerate(self.edge_ranges)], dim=0)
-        e_tot = e_loc.clone().reshape(1)
-        dist.all_reduce(e_tot, op=dist.ReduceOp.SUM, group=self.group)
-        F_loc = self.force_gather(self.row_ptr[c_lo:c_hi + 1], self.rev, g_all)
-        return F_loc, e_tot, (c_lo, c_hi)
+    def exchange(self):
+        """point-to-point halo exchange of the cut edges' g_r rows (asynchronous on the device for NCCL; waits for completion)"""
+        p, ops = self.plan, []
+        for d in range(self.world):
+            if d == self.rank:
+                continue
+            if p.recv_cnt[d]:
+                ops.append(dist.P2POp(dist.irecv, self.g_ext[p.recv_off[d]:p.recv_off[d] + p.recv_cnt[d]], d, self.group))
+            if self.send_buf[d].shape[0]:
+                torch.index_select(self.g_local, 0, self.send_idx[d], out=self.send_buf[d])
+                ops.append(dist.P2POp(dist.isend, self.send_buf[d], d, self.group))
+        if ops:
+            for w in dist.batch_isend_irecv(ops):
+                w.wait()
+
+    def reduce_sum(self, t):
+        """sum a small tensor (energy, path-weight gradient) over the ranks, in place"""
+        if self.world > 1:
+            dist.all_reduce(t, op=dist.ReduceOp.SUM, group=self.group)
+        return t
+
+    def gather_forces(self, F_loc, n_atoms):
+        """owners' force rows -> the full [N, 3] array on every rank (optional: an MD code keeps forces with the owner)"""
+        F = torch.zeros((n_atoms, 3), dtype=F_loc.dtype, device=F_loc.device)
+        F[self.plan.c_lo:self.plan.c_hi] = F_loc
+        return self.reduce_sum(F)

@@ -655,3 +655,38 @@ def test_cuda_graph_replay_matches_eager():
     st.run()
     torch.cuda.synchronize()
     assert torch.equal(st.F, F1) and not torch.equal(F1, F0)
+
+
+def test_sharded_step_single_rank_matches_unsharded():
+    """pipeline / sharding binding on the GPU with a one-rank process group (the box has one GPU): ShardedForces' index arrays,
+    the extended g_r array and the owner's force gather give bitwise the forces of the unsharded step; the multi-rank exchange
+    itself is covered on CPU by tests/test_sharding_gloo.py (world_size 2 and 3, bitwise against the oracle)."""
+    import os
+
+    import torch
+    import torch.distributed as dist
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import SingleLayerStep, shard_to_device
+    from paper_2504_16068_b200.sharding import ShardedForces
+    inp = _chain.make_inputs("C1s")
+    plan = ab.Plan(inp["lmax"], inp["n"], ab.F32)
+    st0 = SingleLayerStep(plan, _chain.to_device(inp), inp["rc"], inp["kappa"], inp["scale"])
+    st0.run()
+    created = False
+    if not dist.is_initialized():
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        os.environ.setdefault("MASTER_PORT", str(29600 + os.getpid() % 2000))
+        dist.init_process_group("gloo", rank=0, world_size=1)
+        created = True
+    try:
+        sh = ShardedForces(inp["row_ptr"], inp["rev"], device="cuda", dtype=torch.float32)
+        dev = shard_to_device(inp, sh)
+        st1 = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], sharded=sh)
+        st1.run(mark=True)
+        torch.cuda.synchronize()
+        assert torch.equal(st1.F, st0.F) and torch.equal(st1.e_tot, st0.e_tot) and torch.equal(st1.g_r, st0.g_r)
+        assert {"halo_exchange", "energy_all_reduce"} <= {nm for nm, _, _ in st1.marks}
+    finally:
+        if created:
+            dist.destroy_process_group()

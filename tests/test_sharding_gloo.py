@@ -32,6 +32,31 @@ def test_partition_balanced_and_covering():
                 assert max(edges) <= rp[-1] / world + 40          # within one row of perfectly balanced
 
 
+def test_halo_plan_index_lists():
+    """HaloPlan without any process group: for every rank of worlds 1..5 the extended array [own rows ; received rows] indexed by
+    rev_loc reproduces g_r[rev[e]] for every own edge, and the two sides of every rank pair agree on count and order"""
+    import _chain
+    from paper_2504_16068_b200.sharding import HaloPlan
+    inp = _chain.make_inputs("C4s")
+    rp, rev = inp["row_ptr"], inp["rev"]
+    E = int(rp[-1])
+    g = np.arange(3 * E, dtype=np.float64).reshape(E, 3)            # row e identifies global edge e
+    for world in (1, 2, 3, 5):
+        plans = [HaloPlan(rp, rev, world, r) for r in range(world)]
+        for r, pr in enumerate(plans):
+            ext = np.full((pr.n_local + pr.n_halo, 3), -1.0)
+            ext[:pr.n_local] = g[pr.e0:pr.e1]
+            for s_, ps in enumerate(plans):
+                if s_ == r:
+                    continue
+                rows = g[ps.e0 + ps.send_idx[r]]                     # what s sends to r, in s's order
+                assert rows.shape[0] == pr.recv_cnt[s_]
+                ext[pr.recv_off[s_]:pr.recv_off[s_] + pr.recv_cnt[s_]] = rows
+            assert np.array_equal(ext[pr.rev_loc], g[rev[pr.e0:pr.e1]])
+            assert pr.row_ptr_loc[0] == 0 and pr.row_ptr_loc[-1] == pr.n_local
+        assert sum(pr.n_local for pr in plans) == E
+
+
 def _worker(rank, world, port, name, q):
     os.environ["MASTER_ADDR"] = "127.0.0.1"
     os.environ["MASTER_PORT"] = str(port)
@@ -41,26 +66,33 @@ def _worker(rank, world, port, name, q):
     from paper_2504_16068_b200.sharding import ShardedForces
     from workloads.inputs import sub_inputs
     inp = _chain.make_inputs(name)
-
-    def compute(c_lo, c_hi):
-        if c_hi == c_lo:
-            return torch.zeros((0, 3), dtype=torch.float64), torch.zeros((), dtype=torch.float64)
-        sub = sub_inputs(inp, c_lo, c_hi)
-        r = _chain.oracle_chain(sub, want_gw=False, forces=False)
-        return torch.from_numpy(r["g_r"]), torch.tensor(float(np.sum(r["e_edge"])), dtype=torch.float64)
-
-    def gather(rp_slice, rev, g_all):
-        return torch.from_numpy(orc.force_gather(rp_slice, rev, g_all.numpy()))
-
-    sh = ShardedForces(inp["row_ptr"], inp["rev"], compute, gather)
-    F_loc, e_tot, (c_lo, c_hi) = sh.run()
-    q.put((rank, c_lo, c_hi, F_loc.numpy(), float(e_tot.item())))
+    sh = ShardedForces(inp["row_ptr"], inp["rev"], device="cpu", dtype=torch.float64)
+    hp = sh.plan
+    # (1) stub compute: row e of g_r names global edge e; after the exchange every own edge must see its reverse's row
+    sh.g_local.copy_(torch.arange(3 * hp.e0, 3 * hp.e1, dtype=torch.float64).reshape(-1, 3))
+    sh.exchange()
+    want = np.arange(3 * int(inp["row_ptr"][-1]), dtype=np.float64).reshape(-1, 3)[inp["rev"][hp.e0:hp.e1]]
+    stub_ok = bool(np.array_equal(sh.g_ext.numpy()[hp.rev_loc], want))
+    # (2) the oracle as the compute on the rank's centres
+    if hp.c_hi > hp.c_lo:
+        r = _chain.oracle_chain(sub_inputs(inp, hp.c_lo, hp.c_hi), want_gw=False, forces=False)
+        sh.g_local.copy_(torch.from_numpy(r["g_r"]))
+        e_loc = torch.tensor([float(np.sum(r["e_edge"]))], dtype=torch.float64)
+    else:
+        e_loc = torch.zeros(1, dtype=torch.float64)
+    sh.exchange()
+    F_loc = orc.force_gather(hp.row_ptr_loc, hp.rev_loc, sh.g_ext.numpy())
+    e_tot = sh.reduce_sum(e_loc)
+    F_all = sh.gather_forces(torch.from_numpy(F_loc), inp["N"])
+    q.put((rank, hp.c_lo, hp.c_hi, F_loc, float(e_tot.item()), stub_ok, F_all.numpy(), sh.halo_bytes))
     dist.barrier()
     dist.destroy_process_group()
 
 
 @pytest.mark.parametrize("name,world", [("C1s", 2), ("C4s", 3)])
 def test_sharded_forces_match_single_process(name, world):
+    """world_size-2 / 3 gloo processes: halo exchange of the cut edges' g_r rows, forces gathered by the owners.  The owners'
+    forces are BITWISE the single-process oracle's (same per-atom order, same operands); the energy is a sum over ranks."""
     import _chain
     inp = _chain.make_inputs(name)
     ref = _chain.oracle_chain(inp, want_gw=False)
@@ -75,7 +107,10 @@ def test_sharded_forces_match_single_process(name, world):
         p.join(timeout=60)
         assert p.exitcode == 0
     F = np.zeros_like(ref["F"])
-    for rank, c_lo, c_hi, F_loc, e_tot in got:
+    for rank, c_lo, c_hi, F_loc, e_tot, stub_ok, F_all, halo_bytes in got:
+        assert stub_ok
         F[c_lo:c_hi] = F_loc
         assert abs(e_tot - float(np.sum(ref["e_edge"]))) <= 1e-9 * abs(float(np.sum(ref["e_edge"])))
-    assert np.max(np.abs(F - ref["F"])) <= 1e-12 * np.max(np.abs(ref["F"]))
+        assert np.array_equal(F_all, ref["F"])
+        assert halo_bytes > 0
+    assert np.array_equal(F, ref["F"])
