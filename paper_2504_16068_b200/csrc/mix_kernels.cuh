@@ -177,6 +177,127 @@ __global__ void __launch_bounds__(CT) mix_bwd_kernel(int n, const int* __restric
     }
 }
 
+// ------------------------------------------------------------------------------------------------------------------
+// Gradient with respect to the dense path weights (training; PAPER.md:69 leaves the training kernels to future work):
+//   g_W[p][n'][n] = sum_e sum_M G[e][n'][off3(p) + M] * t_p[e][n][M]
+// One CTA per (path p, split s of the centres): the n x n accumulator of ONE path lives in registers (4 x 4 blocks per thread),
+// so no partial matrix is ever flushed per centre; the CTA walks its centres, recomputes t_p of nsl edges at a time into shared
+// memory next to the matching cotangent components, and adds their outer product.  Per centre the sum runs in T, across
+// centres in double; the kGwSplits partial matrices are added in split order by gw_dense_final_kernel (no atomics: the
+// result is bitwise reproducible).  The CTAs of the 30 paths of a split run side by side and share V / G / Eenv through L2.
+constexpr int kGwSplits = 16;
+constexpr int kGwMaxBlocks = 4;      // 4 x 4 blocks per thread: n <= 128 with 256 threads
+
+template <typename T, int L, int CT>
+__global__ void __launch_bounds__(CT) mix_gw_kernel(int n, int n_centres, const int* __restrict__ row_ptr, const T* __restrict__ G,
+                                                     const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ part) {
+    using Gen = TPGen<L>;
+    constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P, D3MAX = 2 * L + 1;
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const int nsl = CT / n;
+    T* ts = reinterpret_cast<T*>(smem_raw);            // [nsl][D3MAX][n]   t_p of the tile
+    T* gS = ts + (size_t)nsl * D3MAX * n;             // [nsl][D3MAX][n]   G[e][.][off3 + M]
+    const int tid = threadIdx.x;
+    const int p = blockIdx.x % P, split = blockIdx.x / P;
+    const int c_lo = (int)((long)n_centres * split / kGwSplits), c_hi = (int)((long)n_centres * (split + 1) / kGwSplits);
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = slot < nsl;
+    const int nq = n / 4, nblk = nq * nq;              // 4 x 4 blocks of the n x n matrix, block b -> (n' = 4 (b / nq), n = 4 (b % nq))
+    double acc[kGwMaxBlocks][16];
+#pragma unroll
+    for (int k = 0; k < kGwMaxBlocks; ++k)
+#pragma unroll
+        for (int i = 0; i < 16; ++i) acc[k][i] = 0.0;
+    int d3 = 1, off3 = 0;
+    static_for<0, P>([&](auto pc) {
+        constexpr int pp = decltype(pc)::value;
+        if (pp == p) { d3 = Gen::d3(pp); off3 = Gen::off3(pp); }
+    });
+
+    for (int c = c_lo; c < c_hi; ++c) {
+        const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+        T E[DE];
+#pragma unroll
+        for (int j = 0; j < DE; ++j) E[j] = active ? Eenv[((size_t)c * n + ch) * DE + j] : T(0);
+        T part_c[kGwMaxBlocks][16];
+#pragma unroll
+        for (int k = 0; k < kGwMaxBlocks; ++k)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) part_c[k][i] = T(0);
+        for (int eb = e0; eb < e1; eb += nsl) {
+            __syncthreads();
+            if (active) {
+                const int e = eb + slot;
+                T t[D3MAX], g[D3MAX];
+#pragma unroll
+                for (int M = 0; M < D3MAX; ++M) { t[M] = T(0); g[M] = T(0); }
+                if (e < e1) {
+                    const T* vrow = V + ((size_t)e * n + ch) * DV;
+                    const T* grow = G + ((size_t)e * n + ch) * DV;
+                    static_for<0, P>([&](auto pc) {
+                        constexpr int pp = decltype(pc)::value;
+                        using Pth = TPPath<L, pp>;
+                        if (pp == p) {
+                            T tp[Pth::D3];
+                            Pth::template fwd<T>(vrow, E, tp);
+#pragma unroll
+                            for (int M = 0; M < Pth::D3; ++M) { t[M] = tp[M]; g[M] = grow[Pth::OFF3 + M]; }
+                        }
+                    });
+                }
+#pragma unroll
+                for (int M = 0; M < D3MAX; ++M) {
+                    ts[((size_t)slot * D3MAX + M) * n + ch] = t[M];
+                    gS[((size_t)slot * D3MAX + M) * n + ch] = g[M];
+                }
+            }
+            __syncthreads();
+#pragma unroll
+            for (int k = 0; k < kGwMaxBlocks; ++k) {
+                const int b = tid + k * CT;
+                if (b < nblk) {
+                    const int r0 = 4 * (b / nq), c0 = 4 * (b - (b / nq) * nq);
+                    for (int sl = 0; sl < nsl; ++sl)
+                        for (int M = 0; M < d3; ++M) {
+                            const T* gp = gS + ((size_t)sl * D3MAX + M) * n + r0;
+                            const T* tp = ts + ((size_t)sl * D3MAX + M) * n + c0;
+#pragma unroll
+                            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                                for (int j = 0; j < 4; ++j) part_c[k][4 * i + j] = fma(gp[i], tp[j], part_c[k][4 * i + j]);
+                        }
+                }
+            }
+        }
+#pragma unroll
+        for (int k = 0; k < kGwMaxBlocks; ++k)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) acc[k][i] += (double)part_c[k][i];
+    }
+    T* dst = part + ((size_t)split * P + p) * n * n;
+#pragma unroll
+    for (int k = 0; k < kGwMaxBlocks; ++k) {
+        const int b = tid + k * CT;
+        if (b < nblk) {
+            const int r0 = 4 * (b / nq), c0 = 4 * (b - (b / nq) * nq);
+#pragma unroll
+            for (int i = 0; i < 4; ++i)
+#pragma unroll
+                for (int j = 0; j < 4; ++j) dst[(size_t)(r0 + i) * n + c0 + j] = (T)acc[k][4 * i + j];
+        }
+    }
+}
+
+// g_W = the split partials added in split order
+template <typename T>
+__global__ void gw_dense_final_kernel(long count, const T* __restrict__ part, T* __restrict__ g_W) {
+    const long i = (long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= count) return;
+    double a = 0.0;
+    for (int s = 0; s < kGwSplits; ++s) a += (double)part[(size_t)s * count + i];
+    g_W[i] = (T)a;
+}
+
 static inline bool all_blocks(const allegro_plan* plan) {
     const unsigned full = (1u << (2 * (plan->l_max + 1))) - 1u;
     return (plan->out_blocks & full) == full && (plan->in_blocks & full) == full;
@@ -227,10 +348,12 @@ static allegro_status_t launch_mix_forward(const TpArgs&) {
 }
 #endif
 
+// workspace layout of tp_backward (dense mode): [gE partial rows, one per item (only with items)] [kGwSplits partial g_W (only with g_path_w)]
 template <typename T>
 static size_t mix_backward_workspace(int n, long n_items, bool have_items, bool want_gw) {
-    (void)want_gw;
-    return have_items ? align_up((size_t)n_items * n * TPGen<ALLEGRO_L>::DE * sizeof(T), 256) : 0;
+    size_t b = have_items ? align_up((size_t)n_items * n * TPGen<ALLEGRO_L>::DE * sizeof(T), 256) : 0;
+    if (want_gw) b += align_up((size_t)kGwSplits * TPGen<ALLEGRO_L>::P * n * n * sizeof(T), 256);
+    return b;
 }
 
 #if ALLEGRO_L <= 2
@@ -243,12 +366,24 @@ static allegro_status_t launch_mix_backward(const TpArgs& a) {
         set_error("tp_backward (dense): n = %d unsupported (n %% %d == 0, n <= %d)", a.n, VEC, CT);
         return ALLEGRO_EUNSUPPORTED;
     }
-    if (a.g_path_w != nullptr) {
-        set_error("tp_backward (dense): the gradient with respect to the dense path weights is not built (forces need only gV, gEenv)");
-        return ALLEGRO_EUNSUPPORTED;
-    }
     const bool have_items = a.items != nullptr;
     T* gE_dst = have_items ? (T*)a.ws : (T*)a.gEenv;
+    if (a.g_path_w != nullptr) {   // training: gradient with respect to W_p (all blocks, explicit cotangent)
+        if (!all_blocks(a.plan) || a.q != nullptr || a.n % 4 != 0 || (a.n / 4) * (a.n / 4) > kGwMaxBlocks * CT) {
+            set_error("tp_backward (dense): g_path_w needs all blocks, an explicit cotangent and n %% 4 == 0, n <= 128");
+            return ALLEGRO_EUNSUPPORTED;
+        }
+        T* part = (T*)((unsigned char*)a.ws + (have_items ? align_up((size_t)a.n_items * a.n * Gen::DE * sizeof(T), 256) : 0));
+        const int nsl = CT / a.n;
+        const size_t smem_gw = 2 * (size_t)nsl * (2 * ALLEGRO_L + 1) * a.n * sizeof(T);
+        auto kg = mix_gw_kernel<T, ALLEGRO_L, CT>;
+        ALLEGRO_CUDA(cudaFuncSetAttribute(kg, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_gw));
+        kg<<<(unsigned)(Gen::P * kGwSplits), CT, smem_gw, a.st>>>(a.n, a.n_atoms, a.row_ptr, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, part);
+        ALLEGRO_LAUNCHED();
+        const long count = (long)Gen::P * a.n * a.n;
+        gw_dense_final_kernel<T><<<(unsigned)((count + 255) / 256), 256, 0, a.st>>>(count, part, (T*)a.g_path_w);
+        ALLEGRO_LAUNCHED();
+    }
 #if ALLEGRO_L == 2
     if constexpr (sizeof(T) == 4) {
         if (a.n == 64) {

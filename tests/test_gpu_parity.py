@@ -336,21 +336,21 @@ def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
     G = rng.normal(7, S["G"], (E, n, dV)).astype(dt)
     f8 = lambda a: a.astype(np.float64)
     ref_out = orc.tp_forward(lmax, rp, f8(V), f8(Ee), f8(W))
-    ref_gV, ref_gE, _ = orc.tp_backward(lmax, rp, f8(G), f8(V), f8(Ee), f8(W), want_gV=True, want_gw=False)
+    ref_gV, ref_gE, ref_gW = orc.tp_backward(lmax, rp, f8(G), f8(V), f8(Ee), f8(W), want_gV=True, want_gw=True)
+    assert ref_gW.shape == W.shape
     plan = ab.Plan(lmax, n, ab.F64 if dt == np.float64 else ab.F32, ab.W_DENSE)
     d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
     rpd, Vd, Ed, Wd, Gd = d(rp), d(V), d(Ee), d(W), d(G)
     for items in (None, ab.segments_build(rp, 6)):
         it = None if items is None else d(items)
         out = ab.tp_forward(plan, rpd, Vd, Ed, Wd, items=it)
-        gV, gE, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it)
-        _assert_close(dict(out=ref_out, gV=ref_gV, gEenv=ref_gE), dict(out=out, gV=gV, gEenv=gE), dt, keys=("out", "gV", "gEenv"),
-                      label="dense l%d n%d" % (lmax, n))
+        gV, gE, gW = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it, want_g_path_w=True)      # training: dE/dW_p as well (row f2)
+        _assert_close(dict(out=ref_out, gV=ref_gV, gEenv=ref_gE, g_path_w=ref_gW), dict(out=out, gV=gV, gEenv=gE, g_path_w=gW), dt,
+                      keys=("out", "gV", "gEenv", "g_path_w"), label="dense l%d n%d" % (lmax, n))
+        gW2 = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it, want_g_path_w=True)[2]
+        assert torch.equal(gW, gW2)                                                             # fixed-order reduction: reproducible bits
         _, gE2, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it, want_gV=False)
         _assert_close(dict(gEenv=ref_gE), dict(gEenv=gE2), dt, keys=("gEenv",), label="dense force-only")
-    with pytest.raises(ab.AllegroError) as ei:
-        ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, want_g_path_w=True)
-    assert ei.value.status == 2
 
 
 def _block_mask_weights(lmax, W, out_mask, in_mask=0xffff):
