@@ -301,6 +301,16 @@ def run_ours(args):
                           "(a replay cannot be split per kernel); the calls' sum can exceed ms_per_step by the launch gaps" % args.steps}
     peaks = ab.measure_peaks()
     peaks["hbm_gbs"] = peak
+    # FP32 / FP64 instruction co-limit of the sparse CG contraction: FMA + MUL instructions per channel-edge of the generated
+    # code (forward nnz + pairs, VJP nnz + 2 pairs) against the FMA-pipe instruction rate measured in this run (fp32 only)
+    nnz, pairs = {1: (32, 32), 2: (274, 258), 3: (1222, 1082)}[inp["lmax"]]
+    instr_edge = ((nnz + pairs) + (nnz + 2 * pairs)) * inp["n"]
+    alu = None
+    if inp["dt"] == np.float32:
+        rate = peaks["fp32_fma_tflops"] * 1e12 / 2.0
+        alu = {"bound": "alu", "achieved": instr_edge * E_all / world / (ms_step * 1e-3), "peak": rate, "unit": "FP32 lane-instructions/s per GPU",
+               "frac": instr_edge * E_all / world / (ms_step * 1e-3) / rate, "instructions_per_edge": instr_edge,
+               "peak_source": "measured in this run (allegro_measure_fp32_fma_peak: %.1f TFLOP/s = 2 flops per FFMA)" % peaks["fp32_fma_tflops"]}
     # forward only (configs[1]: "forward only, then forward+force VJP")
     fwd = None
     if not chunked:
@@ -394,7 +404,7 @@ def run_ours(args):
                        "fused_geometry": not args.separate_geometry},
             "atom_steps_per_s": N_all / (ms_step * 1e-3),
             "step_GBps_algorithmic": step_bytes / (ms_step * 1e-3) / 1e9, "step_frac_of_hbm_peak": step_bytes / (ms_step * 1e-3) / 1e9 / peak,
-            "roofline": roofline, "calls": calls, "clocks": clk, "e2e": e2e, "e2e_md": e2e_md, "forward_only": fwd, "peaks": peaks,
+            "roofline": roofline, "alu_roofline": alu, "calls": calls, "clocks": clk, "e2e": e2e, "e2e_md": e2e_md, "forward_only": fwd, "peaks": peaks,
             "gpu_launches": int(launches),
         }
         line["config"]["launch"] = "eager call sequence" if args.no_graph else "CUDA graph replay of the step (%d kernels per step)" % runner.kernels_per_step

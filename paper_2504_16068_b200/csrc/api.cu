@@ -71,6 +71,33 @@ allegro_status_t bind_scalar_weights(const allegro_plan* plan, const void* path_
     return ALLEGRO_OK;
 }
 
+allegro_status_t make_row128_map(CUtensorMap* map, const void* base, unsigned long long rows, unsigned box_rows) {
+    typedef CUresult (*encode_fn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+    static encode_fn encode = nullptr;
+    if (encode == nullptr) {
+        void* fn = nullptr;
+        cudaDriverEntryPointQueryResult qres;
+        ALLEGRO_CUDA(cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres));
+        if (fn == nullptr || qres != cudaDriverEntryPointSuccess) {
+            set_error("cuTensorMapEncodeTiled is not available from this driver");
+            return ALLEGRO_ECUDA;
+        }
+        encode = (encode_fn)fn;
+    }
+    const cuuint64_t dims[2] = {32, rows};
+    const cuuint64_t strides[1] = {128};           // bytes between rows
+    const cuuint32_t box[2] = {32, box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    const CUresult r = encode(map, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE,
+                              CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_NONE, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+    if (r != CUDA_SUCCESS) {
+        set_error("cuTensorMapEncodeTiled failed (%d) for %llu rows, box of %u rows", (int)r, rows, box_rows);
+        return ALLEGRO_ECUDA;
+    }
+    return ALLEGRO_OK;
+}
+
 }  // namespace allegro
 
 using namespace allegro;

@@ -1,5 +1,6 @@
 // common.cuh -- shared device/host helpers of the product kernels (sm_100a).
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <atomic>
@@ -80,6 +81,17 @@ __device__ __forceinline__ void bulk_store(void* dst_gmem, const void* src_smem,
     asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst_gmem), "r"(smem_u32(src_smem)), "r"(bytes)
                  : "memory");
 }
+// 2-D tiled TMA copies through a tensor map (SASS: UTMALDG / UTMASTG); c0 = element index in a row, c1 = row index
+__device__ __forceinline__ void tma_load_2d(void* dst_smem, const CUtensorMap* tmap, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(smem_u32(dst_smem)),
+                 "l"(tmap), "r"(c0), "r"(c1), "r"(smem_u32(bar))
+                 : "memory");
+}
+__device__ __forceinline__ void tma_store_2d(const CUtensorMap* tmap, int c0, int c1, const void* src_smem) {
+    asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];" ::"l"(tmap), "r"(c0), "r"(c1),
+                 "r"(smem_u32(src_smem))
+                 : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() {
@@ -138,6 +150,30 @@ __device__ __forceinline__ void row_store(T* __restrict__ p, const T (&r)[DV]) {
 #pragma unroll
         for (int i = 0; i < RB / 8; ++i) q[i] = v[i];
     }
+}
+
+// Rows of exactly 128 bytes (l_max = 3, fp32) moved by 2-D TMA with the 128-byte swizzle: the 16-byte chunk j of row r sits at chunk
+// position j ^ (r & 7) of the row's 128 bytes (tile base 1024-byte aligned).  `row` points at the row's first byte, sw = (r & 7) << 4.
+// A quarter-warp's eight 128-bit accesses then hit eight different bank groups instead of one (linear rows: 8-way conflict).
+template <typename T, int DV>
+__device__ __forceinline__ void row_load_sw(const unsigned char* __restrict__ row, uint32_t sw, T (&r)[DV]) {
+    static_assert(DV * sizeof(T) == 128, "swizzled rows are 128 bytes");
+    int4 v[8];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) v[j] = *reinterpret_cast<const int4*>(row + (((uint32_t)j << 4) ^ sw));
+    const T* s = reinterpret_cast<const T*>(v);
+#pragma unroll
+    for (int i = 0; i < DV; ++i) r[i] = s[i];
+}
+template <typename T, int DV>
+__device__ __forceinline__ void row_store_sw(unsigned char* __restrict__ row, uint32_t sw, const T (&r)[DV]) {
+    static_assert(DV * sizeof(T) == 128, "swizzled rows are 128 bytes");
+    int4 v[8];
+    T* s = reinterpret_cast<T*>(v);
+#pragma unroll
+    for (int i = 0; i < DV; ++i) s[i] = r[i];
+#pragma unroll
+    for (int j = 0; j < 8; ++j) *reinterpret_cast<int4*>(row + (((uint32_t)j << 4) ^ sw)) = v[j];
 }
 
 // item it -> (centre, e0, e1); items == nullptr means one item per centre

@@ -29,6 +29,10 @@ static inline int pick_stages(size_t stage_bytes, size_t extra) {
     return nst;
 }
 
+// Swizzled 2-D TMA variant: feature rows of exactly 128 bytes (l_max = 3 in fp32), box = one edge = n rows (n % 8 == 0, n <= 256)
+template <typename T>
+static bool use_swizzle(int n) { return sizeof(T) * Gen::DV == 128 && n % 8 == 0 && n <= 256; }
+
 // the plan's folded coefficient table as a kernel parameter (bound by allegro_plan_bind_weights or by the call itself)
 template <typename T>
 static allegro_status_t folded_table(const TpArgs& a, CwTab<T, Gen::NNZ>& tab) {
@@ -66,15 +70,29 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     const size_t tile = align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
     const bool w_out = a.out != nullptr, w_g = a.Gout != nullptr, w_e = a.e_edge != nullptr;
     const size_t stage = ((w_out && w_g) ? 2 : 1) * tile;
-    const size_t extra = 2 * 6 * 8 + 2 * TH * sizeof(T) + 64;
+    const bool sw = use_swizzle<T>(a.n);
+    const size_t extra = 2 * 6 * 8 + 2 * TH * sizeof(T) + 64 + (sw ? 1024 : 0);
     const int nst = pick_stages(stage, extra);
     const size_t smem = nst * stage + extra;
+    TpMaps tm{};
+    if (sw) {
+        const unsigned long long rows = (unsigned long long)a.n_edges * a.n;
+        if ((s = make_row128_map(&tm.a, a.V, rows, a.n)) != ALLEGRO_OK) return s;
+        if (w_out && (s = make_row128_map(&tm.b, a.out, rows, a.n)) != ALLEGRO_OK) return s;
+        if (w_g && (s = make_row128_map(&tm.c, a.Gout, rows, a.n)) != ALLEGRO_OK) return s;
+    }
+#define ALLEGRO_FWD_SW(WO, WG, WE, SW)                                                                             \
+    {                                                                                                              \
+        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, WO, WG, WE, SW>;                                                  \
+        if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                       \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, tm, nst, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
+                                                        (const T*)a.q, (T)a.kappa, (T*)a.e_edge, (T*)a.Gout);      \
+    }
 #define ALLEGRO_FWD(WO, WG, WE)                                                                                    \
     {                                                                                                              \
-        auto k = tp_fwd_kernel<T, ALLEGRO_L, TH, WO, WG, WE>;                                                      \
-        if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                       \
-        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, nst, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (T*)a.out, \
-                                                        (const T*)a.q, (T)a.kappa, (T*)a.e_edge, (T*)a.Gout);      \
+        if constexpr (sizeof(T) * Gen::DV == 128) {                                                                \
+            if (sw) ALLEGRO_FWD_SW(WO, WG, WE, true) else ALLEGRO_FWD_SW(WO, WG, WE, false)                        \
+        } else ALLEGRO_FWD_SW(WO, WG, WE, false)                                                                   \
     }
     if (w_out && !w_g && !w_e) { ALLEGRO_FWD(true, false, false) }
     else if (w_out && w_g && w_e) { ALLEGRO_FWD(true, true, true) }
@@ -85,6 +103,7 @@ allegro_status_t launch_tp_forward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
         return ALLEGRO_EUNSUPPORTED;
     }
 #undef ALLEGRO_FWD
+#undef ALLEGRO_FWD_SW
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -132,18 +151,32 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
 
     const int nslots = TH / a.n;
     const size_t stage = 2 * (size_t)align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
-    const size_t extra = 2 * 6 * 8 + 64;
+    const bool sw = use_swizzle<T>(a.n);
+    const size_t extra = 2 * 6 * 8 + 64 + (sw ? 1024 : 0);
     const int nst = pick_stages(stage, extra);
     const size_t smem = nst * stage + extra;
     const bool cot = a.q != nullptr;  // tile 0 is `out`; the A12 cotangent is formed in registers
-#define ALLEGRO_BWD(GV, GW, COT)                                                                                          \
+    const bool want_gv = a.gV != nullptr;
+    TpMaps tm{};
+    if (sw) {
+        const unsigned long long rows = (unsigned long long)a.n_edges * a.n;
+        if ((s = make_row128_map(&tm.a, a.V, rows, a.n)) != ALLEGRO_OK) return s;
+        if ((s = make_row128_map(&tm.c, a.G, rows, a.n)) != ALLEGRO_OK) return s;
+        if (want_gv && (s = make_row128_map(&tm.b, a.gV, rows, a.n)) != ALLEGRO_OK) return s;
+    }
+#define ALLEGRO_BWD_SW(GV, GW, COT, SW)                                                                                   \
     {                                                                                                                     \
-        auto k = tp_bwd_kernel<T, ALLEGRO_L, TH, GV, GW, COT>;                                                            \
+        auto k = tp_bwd_kernel<T, ALLEGRO_L, TH, GV, GW, COT, SW>;                                                        \
         if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                              \
-        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, nst, a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, tm, nst, a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, \
                                                         (const T*)a.q, (T)a.kappa, (T*)a.gV, gE_dst, have_items ? 1 : 0, gw_part); \
     }
-    const bool want_gv = a.gV != nullptr;
+#define ALLEGRO_BWD(GV, GW, COT)                                                                                          \
+    {                                                                                                                     \
+        if constexpr (sizeof(T) * Gen::DV == 128) {                                                                       \
+            if (sw) ALLEGRO_BWD_SW(GV, GW, COT, true) else ALLEGRO_BWD_SW(GV, GW, COT, false)                             \
+        } else ALLEGRO_BWD_SW(GV, GW, COT, false)                                                                         \
+    }
     if (cot) {
         if (want_gv && want_gw) { ALLEGRO_BWD(true, true, true) }
         else if (want_gv) { ALLEGRO_BWD(true, false, true) }
@@ -156,6 +189,7 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
         else { ALLEGRO_BWD(false, false, false) }
     }
 #undef ALLEGRO_BWD
+#undef ALLEGRO_BWD_SW
     ALLEGRO_LAUNCHED();
     if (have_items) {
         combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, gE_part, (T*)a.gEenv);

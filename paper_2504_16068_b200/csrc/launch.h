@@ -1,6 +1,7 @@
 // launch.h -- argument packs and launcher declarations shared by api.cu (dispatch) and the
 // per-(dtype, l_max) instantiation units inst_tp.cu / inst_env.cu.  Internal, not part of the ABI.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 
 #include <cstddef>
@@ -105,6 +106,10 @@ template <typename T>
 allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, const void* q, double kappa, void* e_edge, void* G, cudaStream_t st);
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st);
+
+// 2-D tensor map over a feature tensor whose rows are exactly 128 bytes: [rows][32 x 4 B], box = box_rows rows, 128-byte swizzle
+// (api.cu; cuTensorMapEncodeTiled through cudaGetDriverEntryPoint, no link-time dependency on libcuda)
+allegro_status_t make_row128_map(CUtensorMap* map, const void* base, unsigned long long rows, unsigned box_rows);
 
 // scalar path weights: fold path_w (DEVICE, [P]) with the CG table into plan->cw on the host (api.cu); synchronises the stream
 allegro_status_t bind_scalar_weights(const allegro_plan* plan, const void* path_w_dev, cudaStream_t st);

@@ -36,6 +36,13 @@ struct CwTab {
     T v[NNZ];
 };
 
+// Tensor maps of the swizzled variant (SW: feature rows of exactly 128 bytes, i.e. l_max = 3 in fp32): every feature tensor is a
+// 2-D array [E n rows][32 floats], box = one edge (n rows), 128-byte swizzle.  a = V, b = the tensor that is stored (out / gV),
+// c = the second stored tensor of the forward (G) or the cotangent that the VJP loads (G / out).  Unused (zero) when !SW.
+struct alignas(64) TpMaps {
+    CUtensorMap a, b, c;
+};
+
 // ------------------------------------------------------------------------------------------------
 // The tile ring shared by the kernels below.  A stage holds TILES tiles of `tile_bytes` (tile 0 is
 // overwritten in place by the result that is stored back).  full[s]: the stage's loads have landed
@@ -108,8 +115,8 @@ __device__ __forceinline__ T slot_sum(T x, int mode, int n, int slot, int ch, in
 //   e_edge[e] = sum_ch ( q[ch] out[e][ch][0] + kappa/2 sum_k out[e][ch][k]^2 ),   G = q (x) delta_{k,0} + kappa out
 // WANT_OUT / WANT_G / WANT_E select which of out, G, e_edge are produced (at least one of out, G).
 // Stage = [V tile -> out tile (or G tile when !WANT_OUT)] [G tile when both are stored].
-template <typename T, int L, int CT, bool WANT_OUT, bool WANT_G, bool WANT_E>
-__global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
+template <typename T, int L, int CT, bool WANT_OUT, bool WANT_G, bool WANT_E, bool SW>
+__global__ void __launch_bounds__(CT + 32, 2) tp_fwd_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, const __grid_constant__ TpMaps tm, int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                           const T* __restrict__ V, const T* __restrict__ Eenv, T* __restrict__ out,
                                                           const T* __restrict__ q, T kappa, T* __restrict__ e_edge, T* __restrict__ G) {
     using Gen = TPGen<L>;
@@ -117,7 +124,8 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__
     constexpr bool EPI = WANT_G || WANT_E;
     constexpr int TILES = (WANT_OUT && WANT_G) ? 2 : 1;
     static_assert(WANT_OUT || WANT_G, "nothing to store");
-    extern __shared__ __align__(128) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    unsigned char* smem_raw = SW ? smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u) : smem_dyn;   // swizzle atoms are 1024-byte aligned
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nslots = CT / n;
     const uint32_t row_bytes = (uint32_t)n * DV * sizeof(T);
@@ -141,9 +149,14 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__
         auto issue = [&](int t) {
             const int s = t % NST;
             const int eb = e0 + t * nslots;
-            const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
+            const int ne = min(nslots, e1 - eb);
+            const uint32_t bytes = (uint32_t)ne * row_bytes;
             mbar_expect_tx(&r.full[s], bytes);
-            bulk_load(r.stage(s), V + (size_t)eb * n * DV, bytes, &r.full[s]);
+            if constexpr (SW) {
+                for (int i = 0; i < ne; ++i) tma_load_2d(r.stage(s) + (size_t)i * row_bytes, &tm.a, 0, (eb + i) * n, &r.full[s]);
+            } else {
+                bulk_load(r.stage(s), V + (size_t)eb * n * DV, bytes, &r.full[s]);
+            }
         };
         const int pre = ntiles < NST ? ntiles : NST;
         for (int t = 0; t < pre; ++t) issue(t);
@@ -151,9 +164,17 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__
             const int s = u % NST;
             mbar_wait(&r.done[s], (uint32_t)(u / NST) & 1u);
             const int eb = e0 + u * nslots;
-            const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-            if constexpr (WANT_OUT) bulk_store(out + (size_t)eb * n * DV, r.stage(s), bytes);
-            if constexpr (WANT_G) bulk_store(G + (size_t)eb * n * DV, r.stage(s) + (TILES - 1) * r.tile_bytes, bytes);
+            const int ne = min(nslots, e1 - eb);
+            const uint32_t bytes = (uint32_t)ne * row_bytes;
+            if constexpr (SW) {
+                for (int i = 0; i < ne; ++i) {
+                    if constexpr (WANT_OUT) tma_store_2d(&tm.b, 0, (eb + i) * n, r.stage(s) + (size_t)i * row_bytes);
+                    if constexpr (WANT_G) tma_store_2d(&tm.c, 0, (eb + i) * n, r.stage(s) + (TILES - 1) * r.tile_bytes + (size_t)i * row_bytes);
+                }
+            } else {
+                if constexpr (WANT_OUT) bulk_store(out + (size_t)eb * n * DV, r.stage(s), bytes);
+                if constexpr (WANT_G) bulk_store(G + (size_t)eb * n * DV, r.stage(s) + (TILES - 1) * r.tile_bytes, bytes);
+            }
             bulk_commit();  // one group per tile
             if (NST == 1) {
                 if (u + 1 < ntiles) { bulk_wait_read<0>(); issue(u + 1); }
@@ -190,10 +211,15 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__
         T epart = T(0);
         if (valid) {
             T* row = reinterpret_cast<T*>(r.stage(s)) + ((size_t)slot * n + ch) * DV;
+            [[maybe_unused]] const uint32_t sw = ((uint32_t)(slot * n + ch) & 7u) << 4;
             T v[DV], o[DV];
-            row_load<T, DV>(row, v);
+            if constexpr (SW) row_load_sw<T, DV>(reinterpret_cast<const unsigned char*>(row), sw, v);
+            else row_load<T, DV>(row, v);
             Gen::template fwd<T>(cwt.v, v, E, o);
-            if constexpr (WANT_OUT) row_store<T, DV>(row, o);
+            if constexpr (WANT_OUT) {
+                if constexpr (SW) row_store_sw<T, DV>(reinterpret_cast<unsigned char*>(row), sw, o);
+                else row_store<T, DV>(row, o);
+            }
             if constexpr (EPI) {
                 T sq = T(0);
 #pragma unroll
@@ -203,7 +229,8 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__
 #pragma unroll
                     for (int k = 0; k < DV; ++k) o[k] *= kappa;
                     o[0] += qc;
-                    row_store<T, DV>(reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(row) + (TILES - 1) * r.tile_bytes), o);
+                    if constexpr (SW) row_store_sw<T, DV>(reinterpret_cast<unsigned char*>(row) + (TILES - 1) * r.tile_bytes, sw, o);
+                    else row_store<T, DV>(reinterpret_cast<T*>(reinterpret_cast<unsigned char*>(row) + (TILES - 1) * r.tile_bytes), o);
                 }
             }
         }
@@ -222,14 +249,15 @@ __global__ void __launch_bounds__(CT + 32) tp_fwd_kernel(const __grid_constant__
 // kappa out, is formed in registers (G never exists in HBM).
 // WANT_GW adds the path-weight gradient: per-thread accumulators -> fixed-shape warp tree -> warps in
 // order -> one partial row per item (reduced over items by gw_final_kernel).
-template <typename T, int L, int CT, bool WANT_GV, bool WANT_GW, bool COT>
+template <typename T, int L, int CT, bool WANT_GV, bool WANT_GW, bool COT, bool SW>
 __global__ void __launch_bounds__(CT + 32)
-    tp_bwd_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
+    tp_bwd_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, const __grid_constant__ TpMaps tm, int NST, int n, const int* __restrict__ row_ptr, const int* __restrict__ items, const T* __restrict__ G, const T* __restrict__ V,
                   const T* __restrict__ Eenv, const T* __restrict__ q, T kappa, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item,
                   T* __restrict__ gw_part) {
     using Gen = TPGen<L>;
     constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P;
-    extern __shared__ __align__(128) unsigned char smem_raw[];
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    unsigned char* smem_raw = SW ? smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u) : smem_dyn;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int nslots = CT / n;
     const uint32_t row_bytes = (uint32_t)n * DV * sizeof(T);
@@ -261,10 +289,18 @@ __global__ void __launch_bounds__(CT + 32)
             auto issue = [&](int t) {
                 const int s = t % NST;
                 const int eb = e0 + t * nslots;
-                const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
+                const int ne = min(nslots, e1 - eb);
+                const uint32_t bytes = (uint32_t)ne * row_bytes;
                 mbar_expect_tx(&r.full[s], 2 * bytes);
-                bulk_load(r.stage(s), G + (size_t)eb * n * DV, bytes, &r.full[s]);
-                bulk_load(r.stage(s) + r.tile_bytes, V + (size_t)eb * n * DV, bytes, &r.full[s]);
+                if constexpr (SW) {
+                    for (int i = 0; i < ne; ++i) {
+                        tma_load_2d(r.stage(s) + (size_t)i * row_bytes, &tm.c, 0, (eb + i) * n, &r.full[s]);
+                        tma_load_2d(r.stage(s) + r.tile_bytes + (size_t)i * row_bytes, &tm.a, 0, (eb + i) * n, &r.full[s]);
+                    }
+                } else {
+                    bulk_load(r.stage(s), G + (size_t)eb * n * DV, bytes, &r.full[s]);
+                    bulk_load(r.stage(s) + r.tile_bytes, V + (size_t)eb * n * DV, bytes, &r.full[s]);
+                }
             };
             const int pre = ntiles < NST ? ntiles : NST;
             for (int t = 0; t < pre; ++t) issue(t);
@@ -273,8 +309,13 @@ __global__ void __launch_bounds__(CT + 32)
                 mbar_wait(&r.done[s], (uint32_t)(u / NST) & 1u);
                 if constexpr (WANT_GV) {
                     const int eb = e0 + u * nslots;
-                    const uint32_t bytes = (uint32_t)min(nslots, e1 - eb) * row_bytes;
-                    bulk_store(gV + (size_t)eb * n * DV, r.stage(s), bytes);
+                    const int ne = min(nslots, e1 - eb);
+                    const uint32_t bytes = (uint32_t)ne * row_bytes;
+                    if constexpr (SW) {
+                        for (int i = 0; i < ne; ++i) tma_store_2d(&tm.b, 0, (eb + i) * n, r.stage(s) + (size_t)i * row_bytes);
+                    } else {
+                        bulk_store(gV + (size_t)eb * n * DV, r.stage(s), bytes);
+                    }
                     bulk_commit();
                     if (NST == 1) {
                         if (u + 1 < ntiles) { bulk_wait_read<0>(); issue(u + 1); }
@@ -307,9 +348,15 @@ __global__ void __launch_bounds__(CT + 32)
             if (active && eb + slot < e1) {
                 T* grow = reinterpret_cast<T*>(r.stage(s)) + ((size_t)slot * n + ch) * DV;
                 const T* vrow = reinterpret_cast<const T*>(r.stage(s) + r.tile_bytes) + ((size_t)slot * n + ch) * DV;
+                [[maybe_unused]] const uint32_t sw = ((uint32_t)(slot * n + ch) & 7u) << 4;
                 T v[DV], g[DV], gv[DV];
-                row_load<T, DV>(grow, g);
-                row_load<T, DV>(vrow, v);
+                if constexpr (SW) {
+                    row_load_sw<T, DV>(reinterpret_cast<const unsigned char*>(grow), sw, g);
+                    row_load_sw<T, DV>(reinterpret_cast<const unsigned char*>(vrow), sw, v);
+                } else {
+                    row_load<T, DV>(grow, g);
+                    row_load<T, DV>(vrow, v);
+                }
                 if constexpr (COT) {
 #pragma unroll
                     for (int k = 0; k < DV; ++k) g[k] *= kappa;
@@ -317,7 +364,10 @@ __global__ void __launch_bounds__(CT + 32)
                 }
                 Gen::template bwd<T, WANT_GV>(cwt.v, v, E, g, gv, gE);
                 if constexpr (WANT_GW) Gen::template pathw<T>(v, E, g, gw);
-                if constexpr (WANT_GV) row_store<T, DV>(grow, gv);
+                if constexpr (WANT_GV) {
+                    if constexpr (SW) row_store_sw<T, DV>(reinterpret_cast<unsigned char*>(grow), sw, gv);
+                    else row_store<T, DV>(grow, gv);
+                }
             }
             ring_release(&r.done[s], lane);
         }
