@@ -250,7 +250,8 @@ class ChunkedStep:
         plan.bind_weights(dev["path_w"])
 
     def run(self, keep=None, mark=False):
-        """keep: optional dict chunk_index -> dict that receives clones of that chunk's out / gV (parity tests);
+        """keep: optional dict chunk_index -> dict that receives clones of that chunk's out / gV (parity tests); a dict with a "rows" entry
+        (list of GLOBAL edge ranges (e_lo, e_hi) inside the chunk) receives only those rows, as lists under "out" / "gV";
         mark: record CUDA events around every call -> self.marks = [(name, start, end)] (one entry per call and chunk)"""
         p, d = self.plan, self.dev
         ev = []
@@ -280,7 +281,11 @@ class ChunkedStep:
             timed("env_radial_backward", lambda: ab.env_radial_backward(p, rp_c, gE, rvec, d["W_r"], self.rc, self.scale,
                                                                         g_rvec=self.g_r[e0:e1]))
             if keep is not None and k in keep:
-                keep[k].update(out=out.clone(), gV=None if gV is None else gV.clone())
+                if "rows" in keep[k]:
+                    keep[k]["out"] = [out[a - e0:b - e0].clone() for a, b in keep[k]["rows"]]
+                    keep[k]["gV"] = [None if gV is None else gV[a - e0:b - e0].clone() for a, b in keep[k]["rows"]]
+                else:
+                    keep[k].update(out=out.clone(), gV=None if gV is None else gV.clone())
         timed("force_gather", lambda: ab.force_gather(d["row_ptr"], d["rev"], self.g_r, F=self.F))
         timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
         return self.F, self.e_tot

@@ -231,6 +231,53 @@ def _check_sampled_centres(inp, got, ranges, label):
         _assert_close(ref, part, inp["dt"], keys=edge_keys + ("Eenv", "gEenv"), label="%s centres [%d,%d)" % (label, c0, c1))
 
 
+def _pool(fn, args_list, workers=None):
+    """run fn over args_list on the host cores (the C++ oracle and torch release the GIL)"""
+    import concurrent.futures as cf
+    import os
+    workers = workers or max(1, min(len(args_list), len(os.sched_getaffinity(0))))
+    with cf.ThreadPoolExecutor(max_workers=workers) as ex:
+        return list(ex.map(fn, args_list))
+
+
+def _check_sampled_centres_pool(inp, got, ranges, label):
+    """_check_sampled_centres with the oracle sub-problems fanned out over the host cores"""
+    from workloads.inputs import sub_inputs
+    edge_keys = ("w", "out", "e_edge", "G", "gV", "g_w", "g_r_env", "g_r")
+    subs = [sub_inputs(inp, c0, c1) for c0, c1 in ranges]
+    refs = _pool(lambda sb: _chain.oracle_chain(sb, want_gw=False, forces=False), subs)
+    for (c0, c1), sub, ref in zip(ranges, subs, refs):
+        e0, e1 = sub["edge_range"]
+        part = {k: got[k][e0:e1] for k in edge_keys if got.get(k) is not None}
+        part.update(Eenv=got["Eenv"][c0:c1], gEenv=got["gEenv"][c0:c1])
+        _assert_close(ref, part, inp["dt"], keys=edge_keys + ("Eenv", "gEenv"), label="%s centres [%d,%d)" % (label, c0, c1))
+    return sum(c1 - c0 for c0, c1 in ranges)
+
+
+def _check_forces_vs_oracle(inp, F_gpu, atoms, g_r_of_centre, label):
+    """Forces of `atoms` against the ORACLE's force assembly: atom a needs g_r of its own edges and of their reverses, i.e. the
+    oracle's g_r rows of centre a and of every neighbour centre (each evaluated with its complete neighbourhood);
+    F_ref[a] = sum_{e in row a} (g_r[e] - g_r[rev[e]]) in float64."""
+    rp, rev = inp["row_ptr"], inp["rev"]
+    centre_of = np.repeat(np.arange(inp["N"]), np.diff(rp))
+    need = sorted({int(a) for a in atoms} | {int(centre_of[rev[e]]) for a in atoms for e in range(rp[a], rp[a + 1])})
+    rows = dict(zip(need, _pool(g_r_of_centre, need)))
+    Fref = np.zeros((len(atoms), 3))
+    for i, a in enumerate(atoms):
+        for e in range(rp[a], rp[a + 1]):
+            j = int(centre_of[rev[e]])
+            Fref[i] += rows[a][e - rp[a]] - rows[j][rev[e] - rp[j]]
+    F = F_gpu[np.asarray(atoms)].detach().cpu().numpy().astype(np.float64)
+    rel = np.linalg.norm(F - Fref) / np.linalg.norm(Fref)
+    assert rel <= _chain.FORCE_RMS_TOL[inp["dt"]], "%s: forces of %d atoms vs oracle: relative RMS %g" % (label, len(atoms), rel)
+    return rel
+
+
+def _single_layer_g_r(inp):
+    from workloads.inputs import sub_inputs
+    return lambda c: _chain.oracle_chain(sub_inputs(inp, c, c + 1), want_gw=False, forces=False)["g_r"]
+
+
 def _check_force_gather(inp, got):
     """F against a float64 host re-summation of the GPU's own g_r (integer gather + sum: size-independent property)"""
     g_r = got["g_r"].cpu().numpy().astype(np.float64)
@@ -252,9 +299,11 @@ def test_c1_full_size_sampled_centres():
     got = _chain.gpu_chain(inp, want_gw=False)
     N = inp["N"]
     starts = [int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(3), 0, N - 17)]
-    ranges = [(c, c + 16) for c in starts + [0, N - 16]]
-    _check_sampled_centres(inp, got, ranges, "C1")
+    deg = np.diff(inp["row_ptr"])
+    ranges = [(c, c + 16) for c in starts + [0, N - 16]] + [(int(np.argmax(deg)), int(np.argmax(deg)) + 1), (int(np.argmin(deg)), int(np.argmin(deg)) + 1)]
+    _check_sampled_centres_pool(inp, got, ranges, "C1")          # 2 % of the centres, the highest- and lowest-degree ones included
     _check_force_gather(inp, got)
+    _check_forces_vs_oracle(inp, got["F"], [0, int(np.argmax(deg)), N - 1], _single_layer_g_r(inp), "C1")
     # the object bench.py times (preallocated buffers, fused forward + energy epilogue), same checks
     import paper_2504_16068_b200 as ab
     from paper_2504_16068_b200.pipeline import SingleLayerStep
@@ -301,20 +350,34 @@ def test_c3_full_size_chunked_sampled_centres():
     plan = ab.Plan(inp["lmax"], inp["n"], ab.F32)
     st = ChunkedStep(plan, dev, inp["row_ptr"], inp["rc"], inp["kappa"], inp["scale"], n_chunks=16)
     nck = len(st.chunks)
-    keep = {0: {}, nck // 2: {}, nck - 1: {}}
+    # ~2 % of the centres: in EVERY chunk a window at its first centres, at its middle and at its last centres (both
+    # sides of every chunk boundary), plus the highest- and the lowest-degree centre of the system
+    W = 40
+    rp = inp["row_ptr"]
+    deg = np.diff(rp)
+    windows = {k: [] for k in range(nck)}
+    for k, (c0, c1, e0, e1, _) in enumerate(st.chunks):
+        for a in (c0, (c0 + c1) // 2, c1 - W):
+            windows[k].append((a, a + W))
+    for c in (int(np.argmax(deg)), int(np.argmin(deg))):
+        k = next(i for i, ch in enumerate(st.chunks) if ch[0] <= c < ch[1])
+        windows[k].append((c, c + 1))
+    keep = {k: {"rows": [(int(rp[a]), int(rp[b])) for a, b in ws]} for k, ws in windows.items()}
     st.run(keep=keep)
     torch.cuda.synchronize()
-    for k, kept in keep.items():
-        c0, c1, e0, e1, _ = st.chunks[k]
-        for a in (c0, (c0 + c1) // 2, c1 - 3):
-            sub = sub_inputs(inp, a, a + 3)
-            ref = _chain.oracle_chain(sub, want_gw=False, forces=False)
-            s0, s1 = sub["edge_range"]
-            part = dict(out=kept["out"][s0 - e0:s1 - e0], gV=kept["gV"][s0 - e0:s1 - e0], e_edge=st.e_edge[s0:s1], g_r=st.g_r[s0:s1],
-                        Eenv=st.Eenv[a:a + 3], gEenv=st.gEenv[a:a + 3])
-            _assert_close(ref, part, inp["dt"], keys=tuple(part.keys()), label="C3 chunk %d centres [%d,%d)" % (k, a, a + 3))
+    jobs = [(k, i, a, b) for k, ws in windows.items() for i, (a, b) in enumerate(ws)]
+    subs = [sub_inputs(inp, a, b) for _, _, a, b in jobs]
+    refs = _pool(lambda sb: _chain.oracle_chain(sb, want_gw=False, forces=False), subs)
+    n_checked = 0
+    for (k, i, a, b), sub, ref in zip(jobs, subs, refs):
+        s0, s1 = sub["edge_range"]
+        part = dict(out=keep[k]["out"][i], gV=keep[k]["gV"][i], e_edge=st.e_edge[s0:s1], g_r=st.g_r[s0:s1], Eenv=st.Eenv[a:b], gEenv=st.gEenv[a:b])
+        _assert_close(ref, part, inp["dt"], keys=tuple(part.keys()), label="C3 chunk %d centres [%d,%d)" % (k, a, b))
+        n_checked += b - a
+    assert n_checked >= 0.019 * inp["N"]
     got = dict(g_r=st.g_r, F=st.F)
     _check_force_gather(inp, got)
+    _check_forces_vs_oracle(inp, st.F, [0, int(np.argmax(deg)), inp["N"] - 1], _single_layer_g_r(inp), "C3")
 
 
 @pytest.mark.parametrize("lmax,n,dt,geom", [(2, 64, np.float32, "C1s"), (1, 8, np.float64, "C0"), (1, 128, np.float32, "C0"), (2, 32, np.float64, "C4s")])
@@ -596,17 +659,29 @@ def test_two_layer_model_c2_full_size_sampled_centres():
     st = _two_layer_step(inp, scalars_only_last=True)
     torch.cuda.synchronize()
     rp, N = inp["row_ptr"], inp["N"]
-    starts = [int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(2), 0, N - 5)] + [0, N - 4]
-    for c0 in starts:
-        c1 = c0 + 4
+    deg = np.diff(rp)
+    # ~1 % of the centres: 80 seeded windows of 4 centres, both ends of the system, the highest- and lowest-degree centre
+    starts = sorted({int(x) for x in rng.randint(0, rng.STREAMS["sample"], np.arange(80), 0, N - 5)} | {0, N - 4})
+    ranges = [(c, c + 4) for c in starts] + [(int(np.argmax(deg)), int(np.argmax(deg)) + 1), (int(np.argmin(deg)), int(np.argmin(deg)) + 1)]
+
+    def oracle_range(cr):
+        c0, c1 = cr
         e0, e1 = int(rp[c0]), int(rp[c1])
-        sub_rp = (rp[c0:c1 + 1] - rp[c0]).astype(np.int32)
         taps = []
-        en, g = model2.energy_grad(inp["params"], sub_rp, inp["rvec"][e0:e1].astype(np.float64), taps)
+        en, g = model2.energy_grad(inp["params"], (rp[c0:c1 + 1] - rp[c0]).astype(np.int32), inp["rvec"][e0:e1].astype(np.float64), taps)
+        return g, taps
+
+    refs = _pool(oracle_range, ranges, workers=4)      # model2 is multi-threaded torch: a few ranges at a time
+    n_checked = 0
+    for (c0, c1), (g, taps) in zip(ranges, refs):
+        e0, e1 = int(rp[c0]), int(rp[c1])
         ref = dict(g_r=g, e_edge=taps[-1]["e_edge"], V1=taps[0]["V_out"], V2=taps[1]["V_out"][:, :, :1], Eenv1=taps[1]["Eenv"])
         got = dict(g_r=st.g_r[e0:e1], e_edge=st.e_edge[e0:e1], V1=st.V[1][e0:e1], V2=st.V[2][e0:e1, :, :1], Eenv1=st.Eenv[1][c0:c1])
         _assert_close(ref, got, inp["dt"], keys=tuple(ref.keys()), label="C2 centres [%d,%d)" % (c0, c1))
+        n_checked += c1 - c0
+    assert n_checked >= 0.0095 * N
     _check_force_gather(inp, dict(g_r=st.g_r, F=st.F))
+    _check_forces_vs_oracle(inp, st.F, [0, N - 1], lambda c: oracle_range((c, c + 1))[0], "C2")
 
 
 @pytest.mark.parametrize("name", ["C0", "C1s"])
