@@ -60,6 +60,13 @@ SIGNATURES = {
     "allegro_layer_step_host_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_int, C.c_int]),
     "allegro_layer_step_host": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, C.c_double, C.c_double,
                                           C.c_int, _vp, _vp, _vp, C.c_size_t, _vp]),
+    "allegro_layer_step_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_int]),
+    "allegro_layer_step_create": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, C.c_double, C.c_double, C.c_int,
+                                            _vp, _vp, _vp, C.c_size_t, C.POINTER(_vp)]),
+    "allegro_layer_step_launch": (C.c_int, [_vp, _vp]),
+    "allegro_layer_step_buffer": (_vp, [_vp, C.c_char_p]),
+    "allegro_layer_step_num_kernels": (C.c_int, [_vp]),
+    "allegro_layer_step_destroy": (None, [_vp]),
     "allegro_edge_embed": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp]),
     "allegro_edge_embed_backward": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp, _vp]),
     "allegro_linear": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_int, _vp, _vp, C.c_int, C.c_int, _vp, _vp]),
@@ -409,6 +416,43 @@ def latent_backward(rvec, r_cut, z, g_xnew, A, gV, g_rvec, g_x=None, stream=None
 def add_inplace(y, x, stream=None):
     _check(lib().allegro_add_inplace(y.numel(), _dt(y), _ptr(y), _ptr(x), _stream(stream)))
     return y
+
+
+class LayerStepGraph:
+    """allegro_step_t: the single-layer MD step for device-resident buffers, captured into a CUDA graph INSIDE the library and
+    replayed with one launch.  `plan` must have its weights bound; F [N,3] and e_tot [1] are written by every launch."""
+
+    def __init__(self, plan, row_ptr, rev, rvec, V, W_r, r_cut, q, kappa, scale, F, e_tot, want_gV=True):
+        self.plan = plan
+        self.N, self.E = row_ptr.shape[0] - 1, rvec.shape[0]
+        self.refs = (row_ptr, rev, rvec, V, W_r, q, F, e_tot)          # the graph holds their addresses
+        nbytes = lib().allegro_layer_step_workspace(plan.h, self.N, self.E, int(bool(want_gV)))
+        self.ws = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=rvec.device)
+        h = _vp()
+        _check(lib().allegro_layer_step_create(plan.h, self.N, self.E, _ptr(row_ptr), _ptr(rev), _ptr(rvec), _ptr(V), _ptr(W_r), W_r.shape[1],
+                                               float(r_cut), _ptr(q), float(kappa), float(scale), int(bool(want_gV)), _ptr(F), _ptr(e_tot),
+                                               _ptr(self.ws), self.ws.numel(), C.byref(h)))
+        self.h = h
+        self.F, self.e_tot = F, e_tot
+        self.kernels_per_step = lib().allegro_layer_step_num_kernels(h)
+
+    def buffer(self, name, shape, dtype):
+        """view of a workspace buffer ("Eenv", "gEenv", "out", "gV", "e_edge", "g_rvec") as a tensor"""
+        p = lib().allegro_layer_step_buffer(self.h, name.encode())
+        if not p:
+            return None
+        off = p - self.ws.data_ptr()
+        n = int(np.prod(shape)) * torch.empty((), dtype=dtype).element_size()
+        return self.ws[off:off + n].view(dtype).view(*shape)
+
+    def run(self, stream=None, mark=False):
+        _check(lib().allegro_layer_step_launch(self.h, _stream(stream)))
+        return self.F, self.e_tot
+
+    def __del__(self):
+        if getattr(self, "h", None) and _lib is not None:
+            _lib.allegro_layer_step_destroy(self.h)
+            self.h = None
 
 
 def measure_peaks(stream=None):

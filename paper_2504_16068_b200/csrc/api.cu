@@ -462,6 +462,124 @@ allegro_status_t allegro_layer_step_host(const allegro_plan_t* plan, int n_atoms
     return ALLEGRO_OK;
 }
 
+// ---------------------------------------------------------------------------------------------- one-launch MD step (CUDA graph inside the library)
+struct allegro_step {
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    unsigned char* ws = nullptr;
+    size_t off_Eenv = 0, off_gEenv = 0, off_out = 0, off_gV = 0, off_e_edge = 0, off_g_r = 0, off_e_ptr = 0, total = 0;
+    bool have_gV = false;
+    int kernels = 0;
+};
+namespace {
+void graph_step_layout(const allegro_plan_t* plan, int N, long E, int want_gV, allegro_step& L) {
+    const size_t s = plan->dtype == ALLEGRO_F32 ? 4 : 8;
+    const size_t n = plan->n, dV = plan->tab.dV, dE = plan->tab.dE;
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += allegro::align_up(bytes ? bytes : 1, 256); return o; };
+    L.off_e_ptr = take(8);
+    L.off_Eenv = take((size_t)N * n * dE * s); L.off_gEenv = take((size_t)N * n * dE * s); L.off_out = take((size_t)E * n * dV * s);
+    L.off_gV = want_gV ? take((size_t)E * n * dV * s) : 0;
+    L.off_e_edge = take((size_t)E * s); L.off_g_r = take((size_t)E * 3 * s);
+    L.total = off;
+    L.have_gV = want_gV != 0;
+}
+}  // namespace
+
+size_t allegro_layer_step_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges, int want_gV) {
+    if (!plan || n_atoms < 0 || n_edges < 0) return 0;
+    allegro_step L;
+    graph_step_layout(plan, n_atoms, n_edges, want_gV, L);
+    return L.total;
+}
+
+allegro_status_t allegro_layer_step_create(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* rev,
+                                           const void* rvec, const void* V, const void* W_r, int n_basis, double r_cut, const void* q, double kappa,
+                                           double scale, int want_gV, void* F, void* e_tot, void* workspace, size_t workspace_bytes,
+                                           allegro_step_t** out) {
+    ALLEGRO_CHECK_ARG(out != nullptr, "out is NULL");
+    *out = nullptr;
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_atoms >= 0 && n_edges >= 0 && n_edges < 2147483647L, "bad plan / sizes");
+    ALLEGRO_CHECK_ARG(plan->wmode == ALLEGRO_W_SCALAR, "scalar path weights only");
+    ALLEGRO_CHECK_ARG(plan->cw_bound, "bind the path weights first (allegro_plan_bind_weights)");
+    ALLEGRO_CHECK_ARG(row_ptr && W_r && q && F && e_tot, "NULL argument");
+    ALLEGRO_CHECK_ARG((rev && rvec && V) || n_edges == 0, "NULL tensor");
+    allegro_step* st = new (std::nothrow) allegro_step();
+    if (!st) { set_error("allegro_layer_step_create: out of host memory"); return ALLEGRO_ENOMEM; }
+    graph_step_layout(plan, n_atoms, n_edges, want_gV, *st);
+    if (workspace == nullptr || workspace_bytes < st->total || !aligned16(workspace)) {
+        set_error("allegro_layer_step_create: workspace too small or misaligned (%zu < %zu bytes)", workspace_bytes, st->total);
+        delete st;
+        return ALLEGRO_ENOMEM;
+    }
+    st->ws = (unsigned char*)workspace;
+    unsigned char* ws = st->ws;
+    cudaStream_t cs = nullptr;
+    allegro_status_t r = ALLEGRO_OK;
+    auto fail = [&](allegro_status_t code) {
+        if (cs) cudaStreamDestroy(cs);
+        allegro_layer_step_destroy(st);
+        return code;
+    };
+    if (cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking) != cudaSuccess) { set_error("allegro_layer_step_create: cudaStreamCreate failed"); return fail(ALLEGRO_ECUDA); }
+    const int32_t e_ptr[2] = {0, (int32_t)n_edges};
+    if (cudaMemcpyAsync(ws + st->off_e_ptr, e_ptr, 8, cudaMemcpyHostToDevice, cs) != cudaSuccess || cudaStreamSynchronize(cs) != cudaSuccess) {
+        set_error("allegro_layer_step_create: workspace is not device memory?");
+        return fail(ALLEGRO_ECUDA);
+    }
+    auto sequence = [&](void* stream) -> allegro_status_t {
+        allegro_status_t s;
+        if ((s = allegro_env_radial_forward(plan, n_atoms, n_edges, row_ptr, nullptr, 0, rvec, W_r, n_basis, r_cut, scale, nullptr, ws + st->off_Eenv,
+                                            nullptr, 0, stream)) != ALLEGRO_OK) return s;
+        if ((s = allegro_tp_forward_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, V, ws + st->off_Eenv, nullptr, q, kappa, ws + st->off_out,
+                                           ws + st->off_e_edge, nullptr, stream)) != ALLEGRO_OK) return s;
+        if ((s = allegro_tp_backward_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, ws + st->off_out, V, ws + st->off_Eenv, nullptr, q, kappa,
+                                            want_gV ? ws + st->off_gV : nullptr, ws + st->off_gEenv, nullptr, nullptr, 0, stream)) != ALLEGRO_OK) return s;
+        if ((s = allegro_env_radial_backward(plan, n_atoms, n_edges, row_ptr, ws + st->off_gEenv, rvec, W_r, n_basis, r_cut, scale, ws + st->off_g_r,
+                                             nullptr, stream)) != ALLEGRO_OK) return s;
+        if ((s = allegro_force_gather(n_atoms, n_edges, row_ptr, rev, ws + st->off_g_r, (allegro_dtype_t)plan->dtype, F, stream)) != ALLEGRO_OK) return s;
+        return allegro_segment_sum((const int32_t*)(ws + st->off_e_ptr), 1, ws + st->off_e_edge, (allegro_dtype_t)plan->dtype, e_tot, stream);
+    };
+    // one eager pass first: it sets every kernel's attributes outside the capture and proves the arguments
+    if ((r = sequence(cs)) != ALLEGRO_OK) return fail(r);
+    if (cudaStreamSynchronize(cs) != cudaSuccess) { set_error("allegro_layer_step_create: the eager pass failed: %s", cudaGetErrorString(cudaGetLastError())); return fail(ALLEGRO_ECUDA); }
+    const long k0 = g_launches.load();
+    if (cudaStreamBeginCapture(cs, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { set_error("allegro_layer_step_create: cudaStreamBeginCapture failed"); return fail(ALLEGRO_ECUDA); }
+    r = sequence(cs);
+    const cudaError_t ce = cudaStreamEndCapture(cs, &st->graph);
+    st->kernels = (int)(g_launches.load() - k0);
+    if (r != ALLEGRO_OK) return fail(r);
+    if (ce != cudaSuccess || st->graph == nullptr) { set_error("allegro_layer_step_create: capture failed: %s", cudaGetErrorString(ce)); return fail(ALLEGRO_ECUDA); }
+    if (cudaGraphInstantiate(&st->exec, st->graph, 0) != cudaSuccess) { set_error("allegro_layer_step_create: cudaGraphInstantiate failed"); return fail(ALLEGRO_ECUDA); }
+    cudaStreamDestroy(cs);
+    *out = st;
+    return ALLEGRO_OK;
+}
+
+allegro_status_t allegro_layer_step_launch(allegro_step_t* step, void* stream) {
+    ALLEGRO_CHECK_ARG(step != nullptr && step->exec != nullptr, "step is NULL");
+    ALLEGRO_CUDA(cudaGraphLaunch(step->exec, (cudaStream_t)stream));
+    g_launches.fetch_add(step->kernels);
+    return ALLEGRO_OK;
+}
+void* allegro_layer_step_buffer(const allegro_step_t* step, const char* name) {
+    if (!step || !name) return nullptr;
+    if (!strcmp(name, "Eenv")) return step->ws + step->off_Eenv;
+    if (!strcmp(name, "gEenv")) return step->ws + step->off_gEenv;
+    if (!strcmp(name, "out")) return step->ws + step->off_out;
+    if (!strcmp(name, "gV")) return step->have_gV ? step->ws + step->off_gV : nullptr;
+    if (!strcmp(name, "e_edge")) return step->ws + step->off_e_edge;
+    if (!strcmp(name, "g_rvec")) return step->ws + step->off_g_r;
+    return nullptr;
+}
+int allegro_layer_step_num_kernels(const allegro_step_t* step) { return step ? step->kernels : -1; }
+void allegro_layer_step_destroy(allegro_step_t* step) {
+    if (!step) return;
+    if (step->exec) cudaGraphExecDestroy(step->exec);
+    if (step->graph) cudaGraphDestroy(step->graph);
+    delete step;
+}
+
 // ---------------------------------------------------------------------------------------------- two-layer model helpers
 allegro_status_t allegro_edge_embed(const allegro_plan_t* plan, long n_edges, const void* rvec, const void* W_x0, const void* W_v0, int n_basis,
                                     double r_cut, void* x0, void* V0, void* stream) {

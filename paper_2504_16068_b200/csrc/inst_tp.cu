@@ -15,6 +15,8 @@ using Gen = TPGen<ALLEGRO_L>;
 
 template <typename T> struct Cfg {
     static constexpr int THREADS = sizeof(T) == 4 ? 256 : 128;  // compute threads; one producer warp is added at launch
+    // VJP at l_max = 3, fp32: 168 registers per thread allow one CTA per SM only, so that CTA gets 12 compute warps instead of 8
+    static constexpr int THREADS_BWD = (sizeof(T) == 4 && ALLEGRO_L == 3) ? 384 : THREADS;
 };
 
 // Ring depth: as many stages as fit (<= 4) with two CTAs per SM; if that leaves fewer than 3, one CTA per SM
@@ -123,7 +125,7 @@ size_t tp_backward_workspace<ALLEGRO_T, ALLEGRO_L>(int n, int n_atoms, long n_it
 template <>
 allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     using T = ALLEGRO_T;
-    constexpr int TH = Cfg<T>::THREADS;
+    constexpr int TH = Cfg<T>::THREADS_BWD;
     if (a.n > TH || ((size_t)a.n * Gen::DV * sizeof(T)) % 16 != 0) {
         set_error("tp_backward: n = %d unsupported (need n <= %d and n*dV*sizeof(T) %% 16 == 0)", a.n, TH);
         return ALLEGRO_EUNSUPPORTED;

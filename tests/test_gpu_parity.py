@@ -765,3 +765,37 @@ def test_sharded_step_single_rank_matches_unsharded():
     finally:
         if created:
             dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("name", ["C0", "C4s"])
+def test_library_graph_step_matches_eager(name):
+    """allegro_layer_step_create / _launch: the step captured into a CUDA graph INSIDE the library (no torch graph, one launch per
+    MD step) gives the bits of the eager call sequence, also after the edge vectors change in place; buffers are reachable"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from paper_2504_16068_b200.pipeline import SingleLayerStep
+    inp = _chain.make_inputs(name)
+    dev = _chain.to_device(inp)
+    dt = ab.F64 if inp["dt"] == np.float64 else ab.F32
+    plan = ab.Plan(inp["lmax"], inp["n"], dt)
+    st = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"])
+    st.run()
+    F0, e0, gV0 = st.F.clone(), st.e_tot.clone(), st.gV.clone()
+    F, e = torch.empty_like(st.F), torch.empty_like(st.e_tot)
+    g = ab.LayerStepGraph(plan, dev["row_ptr"], dev["rev"], dev["rvec"], dev["V"], dev["W_r"], inp["rc"], dev["q"], inp["kappa"], inp["scale"], F, e)
+    assert g.kernels_per_step == 6
+    F.zero_()
+    g.run()
+    torch.cuda.synchronize()
+    assert torch.equal(F, F0) and torch.equal(e, e0)
+    assert torch.equal(g.buffer("gV", tuple(st.gV.shape), st.gV.dtype), gV0)
+    dev["rvec"].mul_(1.01)
+    g.run()
+    st.run()
+    torch.cuda.synchronize()
+    assert torch.equal(F, st.F) and not torch.equal(F, F0)
+    with pytest.raises(ab.AllegroError) as ei:          # weights must be bound before the capture
+        ab.LayerStepGraph(ab.Plan(inp["lmax"], inp["n"], dt), dev["row_ptr"], dev["rev"], dev["rvec"], dev["V"], dev["W_r"], inp["rc"], dev["q"],
+                          inp["kappa"], inp["scale"], F, e)
+    assert ei.value.status == 1
