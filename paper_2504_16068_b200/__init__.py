@@ -75,6 +75,7 @@ SIGNATURES = {
     "allegro_add_inplace": (C.c_int, [C.c_long, C.c_int, _vp, _vp, _vp]),
     "allegro_measure_fp32_fma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
     "allegro_measure_tf32_mma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
+    "allegro_measure_tf32_mma_rate": (C.c_int, [C.c_int, _vp, C.POINTER(C.c_double)]),
     "allegro_status_str": (C.c_char_p, [C.c_int]),
     "allegro_last_error": (C.c_char_p, []),
     "allegro_launch_count": (C.c_long, []),
@@ -460,7 +461,12 @@ def measure_peaks(stream=None):
     a, b = C.c_double(0.0), C.c_double(0.0)
     _check(lib().allegro_measure_fp32_fma_peak(_stream(stream), C.byref(a)))
     _check(lib().allegro_measure_tf32_mma_peak(_stream(stream), C.byref(b)))
-    return dict(fp32_fma_tflops=a.value, tf32_mma_tflops=b.value)
+    by_n = {}
+    for n in (32, 80, 128, 256):
+        c = C.c_double(0.0)
+        _check(lib().allegro_measure_tf32_mma_rate(n, _stream(stream), C.byref(c)))
+        by_n[str(n)] = c.value
+    return dict(fp32_fma_tflops=a.value, tf32_mma_tflops=b.value, tf32_mma_tflops_by_N=by_n)
 
 
 def layer_step_host_workspace(plan, n_atoms, n_edges, n_basis, want_gV=True):

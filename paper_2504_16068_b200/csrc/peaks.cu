@@ -23,7 +23,8 @@ __global__ void __launch_bounds__(1024) ffma_peak_kernel(int iters, float a, flo
     if (s == 123.456f) sink[0] = s;   // never true: keeps the chains alive
 }
 
-// one CTA per SM; one thread issues `iters` x 8 tcgen05.mma kind::tf32, M = 128, N = 256, K = 8 each, operands in shared memory
+// one CTA per SM; one thread issues `iters` x 8 tcgen05.mma kind::tf32, M = 128, N = NCOLS, K = 8 each, operands in shared memory
+template <int NCOLS>
 __global__ void __launch_bounds__(128, 1) tf32_mma_peak_kernel(int iters) {
     extern __shared__ unsigned char peak_smem_raw[];
     unsigned char* sm = peak_smem_raw + ((1024u - (smem_u32(peak_smem_raw) & 1023u)) & 1023u);
@@ -39,7 +40,7 @@ __global__ void __launch_bounds__(128, 1) tf32_mma_peak_kernel(int iters) {
     tc05::fence_after_sync();
     const uint32_t tb = slot;
     if (tid == 0) {
-        constexpr uint32_t idesc = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 256);
+        constexpr uint32_t idesc = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, NCOLS);
         const uint32_t a0 = tc05::sdesc_lo(smem_u32(sm)), b0 = tc05::sdesc_lo(smem_u32(sm + 32768));   // A: 128 rows, B: 256 rows, two K-atoms each
         for (int it = 0; it < iters; ++it) {
 #pragma unroll
@@ -93,33 +94,56 @@ allegro_status_t allegro_measure_fp32_fma_peak(void* stream, double* tflops) {
     return ALLEGRO_OK;
 }
 
-allegro_status_t allegro_measure_tf32_mma_peak(void* stream, double* tflops) {
-    ALLEGRO_CHECK_ARG(tflops != nullptr, "tflops is NULL");
-    cudaStream_t st = (cudaStream_t)stream;
+}  // extern "C"
+
+template <int NCOLS>
+static allegro_status_t measure_tf32(cudaStream_t st, double* tflops) {
     int dev = 0, sms = 0;
     ALLEGRO_CUDA(cudaGetDevice(&dev));
     ALLEGRO_CUDA(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int smem = 100 * 1024, iters = 2000;
-    ALLEGRO_CUDA(cudaFuncSetAttribute(tf32_mma_peak_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    ALLEGRO_CUDA(cudaFuncSetAttribute(tf32_mma_peak_kernel<NCOLS>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     cudaEvent_t e0, e1;
     ALLEGRO_CUDA(cudaEventCreate(&e0));
     ALLEGRO_CUDA(cudaEventCreate(&e1));
     double best = 0.0;
     for (int rep = 0; rep < 4; ++rep) {
         ALLEGRO_CUDA(cudaEventRecord(e0, st));
-        tf32_mma_peak_kernel<<<sms, 128, smem, st>>>(iters);
+        tf32_mma_peak_kernel<NCOLS><<<sms, 128, smem, st>>>(iters);
         ALLEGRO_LAUNCHED();
         ALLEGRO_CUDA(cudaEventRecord(e1, st));
         ALLEGRO_CUDA(cudaEventSynchronize(e1));
         float ms = 0.f;
         ALLEGRO_CUDA(cudaEventElapsedTime(&ms, e0, e1));
-        const double tf = 2.0 * 128.0 * 256.0 * 8.0 * 8.0 * iters * sms / (ms * 1e-3) / 1e12;
+        const double tf = 2.0 * 128.0 * NCOLS * 8.0 * 8.0 * iters * sms / (ms * 1e-3) / 1e12;
         if (rep > 0 && tf > best) best = tf;
     }
     cudaEventDestroy(e0);
     cudaEventDestroy(e1);
     *tflops = best;
     return ALLEGRO_OK;
+}
+
+extern "C" {
+
+allegro_status_t allegro_measure_tf32_mma_peak(void* stream, double* tflops) {
+    ALLEGRO_CHECK_ARG(tflops != nullptr, "tflops is NULL");
+    return measure_tf32<256>((cudaStream_t)stream, tflops);
+}
+
+allegro_status_t allegro_measure_tf32_mma_rate(int n_cols, void* stream, double* tflops) {
+    ALLEGRO_CHECK_ARG(tflops != nullptr, "tflops is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    switch (n_cols) {
+        case 16: return measure_tf32<16>(st, tflops);
+        case 32: return measure_tf32<32>(st, tflops);
+        case 48: return measure_tf32<48>(st, tflops);
+        case 80: return measure_tf32<80>(st, tflops);
+        case 128: return measure_tf32<128>(st, tflops);
+        case 256: return measure_tf32<256>(st, tflops);
+    }
+    set_error("allegro_measure_tf32_mma_rate: N = %d is not one of 16, 32, 48, 80, 128, 256", n_cols);
+    return ALLEGRO_EINVAL;
 }
 
 }  // extern "C"
