@@ -40,7 +40,8 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="C1")
     ap.add_argument("--force-only", action="store_true", help="skip dE/dV (valid when V does not depend on positions)")
-    ap.add_argument("--mode", default="onthefly", choices=["separate", "epilogue", "onthefly"], help="call sequence (pipeline.SingleLayerStep)")
+    ap.add_argument("--mode", default="auto", choices=["auto", "separate", "epilogue", "onthefly", "fused"],
+                    help="call sequence (pipeline.SingleLayerStep); auto = fused (one kernel for forward + energy + VJP) for l_max <= 2, onthefly for l_max = 3")
     ap.add_argument("--separate-geometry", action="store_true", help="radial / env-embed as four kernels instead of the two fused ones")
     ap.add_argument("--chunks", type=int, default=1, help="process the centres in this many chunks (C3 defaults to 16)")
     ap.add_argument("--no-graph", action="store_true", help="time the eager call sequence instead of CUDA-graph replays of the step")
@@ -226,9 +227,11 @@ def run_ours(args):
         args.no_graph = True          # the halo exchange (NCCL send / recv) stays outside a captured graph
     else:
         dev = to_device(inp)
+    if args.mode == "auto":      # at l_max = 3 the fused kernel needs 168 registers for one CTA of 8 warps per SM and is slower than the two kernels
+        args.mode = "fused" if inp["lmax"] <= 2 else "onthefly"
     chunked = name == "C3" or args.chunks > 1
     if chunked:      # feature tensors that do not fit HBM four times: V resident, work buffers per centre chunk
-        step = ChunkedStep(plan, dev, inp["row_ptr"], inp["rc"], inp["kappa"], inp["scale"], n_chunks=max(args.chunks, 16 if name == "C3" else 1),
+        step = ChunkedStep(plan, dev, inp["row_ptr"], inp["rc"], inp["kappa"], inp["scale"], n_chunks=max(args.chunks, 16 if name == "C3" else 1), fused=args.mode == "fused",
                            want_gV=not args.force_only)
     else:
         step = SingleLayerStep(plan, dev, inp["rc"], inp["kappa"], inp["scale"], want_gV=not args.force_only, mode=args.mode,
@@ -249,7 +252,7 @@ def run_ours(args):
     runner = step
     lib_graph = False
     if not args.no_graph:
-        if not chunked and args.mode == "onthefly" and not args.separate_geometry:
+        if not chunked and args.mode in ("fused", "onthefly") and not args.separate_geometry:
             # the graph is captured INSIDE the library (allegro_layer_step_create): one C-ABI call per MD step, no framework graph
             runner = ab.LayerStepGraph(plan, dev["row_ptr"], dev["rev"], dev["rvec"], dev["V"], dev["W_r"], inp["rc"], dev["q"], inp["kappa"], inp["scale"],
                                        step.F, step.e_tot, want_gV=not args.force_only)
@@ -301,7 +304,7 @@ def run_ours(args):
     top = max(per_call_ms, key=per_call_ms.get)
     ach = abytes[top] / (per_call_ms[top] * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": top, "achieved": ach, "peak": peak, "unit": "GB/s", "frac": ach / peak,
-                "traffic": _ncu_traffic(name, top) if (args.mode == "onthefly" and not args.force_only) else None,
+                "traffic": _ncu_traffic(name, top) if (args.mode in ("onthefly", "fused") and not args.force_only) else None,
                 "traffic_source": "committed ncu --set full capture, profiles/traffic.txt (not re-measured by this run)",
                 "peak_source": peak_src, "algorithmic_bytes_per_launch": abytes[top], "ms_per_launch": per_call_ms[top],
                 "timing": "eager pass of the same %d steps with CUDA events around every call, run right after the timed graph replays "

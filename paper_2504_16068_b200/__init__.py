@@ -46,6 +46,8 @@ SIGNATURES = {
     "allegro_tp_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_backward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp,
                                              C.c_size_t, _vp]),
+    "allegro_tp_fused_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp, _vp,
+                                          C.c_size_t, _vp]),
     "allegro_tp_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_long, C.c_int]),
     "allegro_env_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
     "allegro_env_embed_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp]),
@@ -278,6 +280,26 @@ def tp_backward_energy(plan, row_ptr, out, V, Eenv, path_w, q, kappa, items=None
                                             _ptr(Eenv), _ptr(path_w), _ptr(q), float(kappa), _ptr(gV), _ptr(gEenv), _ptr(g_path_w),
                                             _ptr(workspace), workspace.numel(), _stream(stream)))
     return gV, gEenv, g_path_w
+
+
+def tp_fused_energy(plan, row_ptr, V, Eenv, path_w, q, kappa, items=None, want_gV=True, want_g_path_w=False, e_edge=None, gV=None, gEenv=None,
+                    g_path_w=None, workspace=None, stream=None):
+    """forward + energy + VJP in one kernel -> (e_edge, gV or None, gEenv, g_path_w or None); `out` never exists"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    if e_edge is None:
+        e_edge = torch.empty((n_edges,), dtype=V.dtype, device=V.device)
+    if gV is None and want_gV:
+        gV = torch.empty_like(V)
+    if gEenv is None:
+        gEenv = torch.empty_like(Eenv)
+    if g_path_w is None and want_g_path_w:
+        g_path_w = torch.empty((plan.P,), dtype=V.dtype, device=V.device)
+    if workspace is None:
+        workspace = _ws(tp_backward_workspace(plan, n_atoms, n_edges, items, g_path_w is not None), V.device)
+    _check(lib().allegro_tp_fused_energy(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(V), _ptr(Eenv), _ptr(path_w),
+                                         _ptr(q), float(kappa), _ptr(e_edge), _ptr(gV), _ptr(gEenv), _ptr(g_path_w), _ptr(workspace),
+                                         workspace.numel(), _stream(stream)))
+    return e_edge, gV, gEenv, g_path_w
 
 
 def env_embed_backward(plan, row_ptr, gEenv, rvec, w, scale=1.0, want_g_w=True, g_rvec=None, g_w=None, stream=None):

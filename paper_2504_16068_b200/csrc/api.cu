@@ -27,6 +27,7 @@ void set_error(const char* fmt, ...) {
     template <> allegro_status_t launch_env_embed_backward<T, L>(const EnvBwdArgs&);           \
     template <> allegro_status_t launch_tp_forward<T, L>(const TpArgs&);                       \
     template <> allegro_status_t launch_tp_backward<T, L>(const TpArgs&);                      \
+    template <> allegro_status_t launch_tp_fused<T, L>(const TpArgs&);                         \
     template <> size_t tp_backward_workspace<T, L>(int, int, long, bool, int, bool);
 ALLEGRO_DECL(float, 1) ALLEGRO_DECL(float, 2) ALLEGRO_DECL(float, 3)
 ALLEGRO_DECL(double, 1) ALLEGRO_DECL(double, 2) ALLEGRO_DECL(double, 3)
@@ -322,6 +323,28 @@ allegro_status_t allegro_tp_backward_energy(const allegro_plan_t* plan, int n_at
     return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
 }
 
+allegro_status_t allegro_tp_fused_energy(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                         long n_items, const void* V, const void* Eenv, const void* path_w, const void* q, double kappa, void* e_edge,
+                                         void* gV, void* gEenv, void* g_path_w, void* workspace, size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((V && e_edge) || n_edges == 0, "V / e_edge is NULL");
+    ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
+    ALLEGRO_CHECK_ARG(q != nullptr, "q is NULL");
+    ALLEGRO_CHECK_ARG(gV == nullptr || gV != V, "gV aliases V");
+    ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace), "tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (plan->wmode != ALLEGRO_W_SCALAR) {
+        set_error("allegro_tp_fused_energy: scalar path weights only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.q = q; a.kappa = kappa; a.e_edge = e_edge; a.gV = gV; a.gEenv = gEenv; a.g_path_w = g_path_w;
+    a.ws = workspace; a.ws_bytes = workspace_bytes; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_fused, a);
+}
+
 size_t allegro_tp_backward_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges, long n_items, int want_g_path_w) {
     (void)n_edges;
     if (!plan) return 0;
@@ -468,6 +491,7 @@ struct allegro_step {
     cudaGraphExec_t exec = nullptr;
     unsigned char* ws = nullptr;
     size_t off_Eenv = 0, off_gEenv = 0, off_out = 0, off_gV = 0, off_e_edge = 0, off_g_r = 0, off_e_ptr = 0, total = 0;
+    bool fused = true;   // l_max <= 2: forward + energy + VJP in one kernel (no `out`); l_max = 3: two kernels (the fused one is slower there)
     bool have_gV = false;
     int kernels = 0;
 };
@@ -478,7 +502,9 @@ void graph_step_layout(const allegro_plan_t* plan, int N, long E, int want_gV, a
     size_t off = 0;
     auto take = [&](size_t bytes) { const size_t o = off; off += allegro::align_up(bytes ? bytes : 1, 256); return o; };
     L.off_e_ptr = take(8);
-    L.off_Eenv = take((size_t)N * n * dE * s); L.off_gEenv = take((size_t)N * n * dE * s); L.off_out = take((size_t)E * n * dV * s);
+    L.fused = plan->l_max <= 2;
+    L.off_Eenv = take((size_t)N * n * dE * s); L.off_gEenv = take((size_t)N * n * dE * s);
+    L.off_out = L.fused ? 0 : take((size_t)E * n * dV * s);
     L.off_gV = want_gV ? take((size_t)E * n * dV * s) : 0;
     L.off_e_edge = take((size_t)E * s); L.off_g_r = take((size_t)E * 3 * s);
     L.total = off;
@@ -531,10 +557,15 @@ allegro_status_t allegro_layer_step_create(const allegro_plan_t* plan, int n_ato
         allegro_status_t s;
         if ((s = allegro_env_radial_forward(plan, n_atoms, n_edges, row_ptr, nullptr, 0, rvec, W_r, n_basis, r_cut, scale, nullptr, ws + st->off_Eenv,
                                             nullptr, 0, stream)) != ALLEGRO_OK) return s;
-        if ((s = allegro_tp_forward_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, V, ws + st->off_Eenv, nullptr, q, kappa, ws + st->off_out,
-                                           ws + st->off_e_edge, nullptr, stream)) != ALLEGRO_OK) return s;
-        if ((s = allegro_tp_backward_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, ws + st->off_out, V, ws + st->off_Eenv, nullptr, q, kappa,
-                                            want_gV ? ws + st->off_gV : nullptr, ws + st->off_gEenv, nullptr, nullptr, 0, stream)) != ALLEGRO_OK) return s;
+        if (st->fused) {
+            if ((s = allegro_tp_fused_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, V, ws + st->off_Eenv, nullptr, q, kappa, ws + st->off_e_edge,
+                                             want_gV ? ws + st->off_gV : nullptr, ws + st->off_gEenv, nullptr, nullptr, 0, stream)) != ALLEGRO_OK) return s;
+        } else {
+            if ((s = allegro_tp_forward_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, V, ws + st->off_Eenv, nullptr, q, kappa, ws + st->off_out,
+                                               ws + st->off_e_edge, nullptr, stream)) != ALLEGRO_OK) return s;
+            if ((s = allegro_tp_backward_energy(plan, n_atoms, n_edges, row_ptr, nullptr, 0, ws + st->off_out, V, ws + st->off_Eenv, nullptr, q, kappa,
+                                                want_gV ? ws + st->off_gV : nullptr, ws + st->off_gEenv, nullptr, nullptr, 0, stream)) != ALLEGRO_OK) return s;
+        }
         if ((s = allegro_env_radial_backward(plan, n_atoms, n_edges, row_ptr, ws + st->off_gEenv, rvec, W_r, n_basis, r_cut, scale, ws + st->off_g_r,
                                              nullptr, stream)) != ALLEGRO_OK) return s;
         if ((s = allegro_force_gather(n_atoms, n_edges, row_ptr, rev, ws + st->off_g_r, (allegro_dtype_t)plan->dtype, F, stream)) != ALLEGRO_OK) return s;
@@ -566,7 +597,7 @@ void* allegro_layer_step_buffer(const allegro_step_t* step, const char* name) {
     if (!step || !name) return nullptr;
     if (!strcmp(name, "Eenv")) return step->ws + step->off_Eenv;
     if (!strcmp(name, "gEenv")) return step->ws + step->off_gEenv;
-    if (!strcmp(name, "out")) return step->ws + step->off_out;
+    if (!strcmp(name, "out")) return step->fused ? nullptr : step->ws + step->off_out;
     if (!strcmp(name, "gV")) return step->have_gV ? step->ws + step->off_gV : nullptr;
     if (!strcmp(name, "e_edge")) return step->ws + step->off_e_edge;
     if (!strcmp(name, "g_rvec")) return step->ws + step->off_g_r;

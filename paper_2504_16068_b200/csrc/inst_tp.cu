@@ -204,4 +204,80 @@ allegro_status_t launch_tp_backward<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
     return ALLEGRO_OK;
 }
 
+// forward + energy + VJP in one pass (scalar weights); workspace as for tp_backward
+template <>
+allegro_status_t launch_tp_fused<ALLEGRO_T, ALLEGRO_L>(const TpArgs& a) {
+    using T = ALLEGRO_T;
+    constexpr int TH = Cfg<T>::THREADS;
+    if (a.n > TH || ((size_t)a.n * Gen::DV * sizeof(T)) % 16 != 0) {
+        set_error("tp_fused: n = %d unsupported (need n <= %d and n*dV*sizeof(T) %% 16 == 0)", a.n, TH);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    const bool have_items = a.items != nullptr;
+    const bool want_gw = a.g_path_w != nullptr;
+    const size_t need = tp_backward_workspace<T, ALLEGRO_L>(a.n, a.n_atoms, a.n_items, have_items, a.plan->wmode, want_gw);
+    if (need > a.ws_bytes || (need > 0 && a.ws == nullptr)) {
+        set_error("tp_fused: workspace too small (%zu < %zu bytes)", a.ws_bytes, need);
+        return ALLEGRO_ENOMEM;
+    }
+    if (a.n_items == 0) {
+        if (want_gw) ALLEGRO_CUDA(cudaMemsetAsync(a.g_path_w, 0, sizeof(T) * Gen::P, a.st));
+        return ALLEGRO_OK;
+    }
+    CwTab<T, Gen::NNZ> cwt;
+    allegro_status_t s = folded_table<T>(a, cwt);
+    if (s != ALLEGRO_OK) return s;
+    unsigned char* ws = (unsigned char*)a.ws;
+    T* gE_part = nullptr;
+    if (have_items) { gE_part = (T*)ws; ws += align_up((size_t)a.n_items * a.n * Gen::DE * sizeof(T), 256); }
+    T* gw_part = want_gw ? (T*)ws : nullptr;
+    T* gE_dst = have_items ? gE_part : (T*)a.gEenv;
+
+    const int nslots = TH / a.n;
+    const size_t stage = (size_t)align128((size_t)nslots * a.n * Gen::DV * sizeof(T));
+    const bool sw = use_swizzle<T>(a.n);
+    const size_t extra = 2 * 6 * 8 + 2 * TH * sizeof(T) + 64 + (sw ? 1024 : 0);
+    size_t red = (size_t)TH * Gen::DE * sizeof(T);          // the gEenv / g_path_w reductions reuse the ring
+    if (want_gw && (size_t)(TH / 32) * Gen::P * sizeof(T) > red) red = (size_t)(TH / 32) * Gen::P * sizeof(T);
+    int nst = pick_stages(stage, extra);
+    while (nst * stage < red) ++nst;
+    const size_t smem = nst * stage + extra;
+    const bool want_gv = a.gV != nullptr;
+    TpMaps tm{};
+    if (sw) {
+        const unsigned long long rows = (unsigned long long)a.n_edges * a.n;
+        if ((s = make_row128_map(&tm.a, a.V, rows, a.n)) != ALLEGRO_OK) return s;
+        if (want_gv && (s = make_row128_map(&tm.b, a.gV, rows, a.n)) != ALLEGRO_OK) return s;
+    }
+#define ALLEGRO_FUSED_SW(GV, GW, SW)                                                                                       \
+    {                                                                                                                     \
+        auto k = tp_fused_kernel<T, ALLEGRO_L, TH, GV, GW, SW>;                                                           \
+        if ((s = set_smem(k, smem)) != ALLEGRO_OK) return s;                                                              \
+        k<<<(unsigned)a.n_items, TH + 32, smem, a.st>>>(cwt, cwt, tm, nst, a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (const T*)a.q, \
+                                                        (T)a.kappa, (T*)a.e_edge, (T*)a.gV, gE_dst, have_items ? 1 : 0, gw_part); \
+    }
+#define ALLEGRO_FUSED(GV, GW)                                                                                             \
+    {                                                                                                                     \
+        if constexpr (sizeof(T) * Gen::DV == 128) {                                                                       \
+            if (sw) ALLEGRO_FUSED_SW(GV, GW, true) else ALLEGRO_FUSED_SW(GV, GW, false)                                   \
+        } else ALLEGRO_FUSED_SW(GV, GW, false)                                                                            \
+    }
+    if (want_gv && want_gw) { ALLEGRO_FUSED(true, true) }
+    else if (want_gv) { ALLEGRO_FUSED(true, false) }
+    else if (want_gw) { ALLEGRO_FUSED(false, true) }
+    else { ALLEGRO_FUSED(false, false) }
+#undef ALLEGRO_FUSED
+#undef ALLEGRO_FUSED_SW
+    ALLEGRO_LAUNCHED();
+    if (have_items) {
+        combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, gE_part, (T*)a.gEenv);
+        ALLEGRO_LAUNCHED();
+    }
+    if (want_gw) {
+        gw_final_kernel<T><<<Gen::P, 256, 0, a.st>>>(gw_part, a.n_items, Gen::P, (T*)a.g_path_w);
+        ALLEGRO_LAUNCHED();
+    }
+    return ALLEGRO_OK;
+}
+
 }  // namespace allegro

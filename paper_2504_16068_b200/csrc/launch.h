@@ -92,6 +92,7 @@ template <typename T, int L> allegro_status_t launch_env_embed(const EnvArgs& a)
 template <typename T, int L> allegro_status_t launch_env_embed_backward(const EnvBwdArgs& a);
 template <typename T, int L> allegro_status_t launch_tp_forward(const TpArgs& a);
 template <typename T, int L> allegro_status_t launch_tp_backward(const TpArgs& a);
+template <typename T, int L> allegro_status_t launch_tp_fused(const TpArgs& a);
 template <typename T, int L> size_t tp_backward_workspace(int n, int n_atoms, long n_items, bool have_items, int wmode, bool want_gw);
 
 // dtype-only helpers (misc.cu)

@@ -410,6 +410,182 @@ __global__ void __launch_bounds__(CT + 32)
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Forward + energy + first derivative in ONE pass over V (fusion is the paper's whole argument -- "costly
+// intermediate memory reads and writes").  Per (edge, channel) row: out = Wc (V (x) Eenv) stays in registers,
+// e_edge and the cotangent G = q (x) delta_{k,0} + kappa out of the A12 energy are formed from it, and the VJP
+// gV = Wc^T (G (x) Eenv), gEenv += Wc^T (V (x) G) follows at once: V crosses HBM once, gV once, `out` and G never
+// (23.9 KB -> 9.4 KB per edge at C1).  Stage = [V tile -> gV tile in place].  The kernel is then bound by instruction issue
+// (1,322 + ~60 FP32 instructions per channel-edge at l_max = 2), not by HBM.
+template <typename T, int L, int CT, bool WANT_GV, bool WANT_GW, bool SW>
+__global__ void __launch_bounds__(CT + 32, (L >= 3 ? 1 : 2))
+    tp_fused_kernel(const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt, const __grid_constant__ CwTab<T, TPGen<L>::NNZ> cwt2,
+                    const __grid_constant__ TpMaps tm, int NST, int n, const int* __restrict__ row_ptr,
+                    const int* __restrict__ items, const T* __restrict__ V, const T* __restrict__ Eenv, const T* __restrict__ q, T kappa,
+                    T* __restrict__ e_edge, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item, T* __restrict__ gw_part) {
+    using Gen = TPGen<L>;
+    constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P;
+    extern __shared__ __align__(128) unsigned char smem_dyn[];
+    unsigned char* smem_raw = SW ? smem_dyn + ((1024u - (smem_u32(smem_dyn) & 1023u)) & 1023u) : smem_dyn;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int nslots = CT / n;
+    const uint32_t row_bytes = (uint32_t)n * DV * sizeof(T);
+    Ring r;
+    r.base = smem_raw;
+    r.tile_bytes = align128((size_t)nslots * row_bytes);
+    r.stage_bytes = r.tile_bytes;
+    r.full = reinterpret_cast<uint64_t*>(smem_raw + (size_t)NST * r.stage_bytes);
+    r.done = r.full + NST;
+    T* ebuf = reinterpret_cast<T*>(r.done + NST);  // [2][CT]
+
+    int c, e0, e1;
+    get_item(items, row_ptr, blockIdx.x, c, e0, e1);
+    const int ntiles = (e1 - e0 + nslots - 1) / nslots;   // 0 for an empty item: only the zero gEenv row is written
+    ring_init(r, tid, CT / 32, NST);
+
+    const bool compute = warp < CT / 32;
+    const int slot = tid / n, ch = tid - slot * n;
+    const bool active = compute && slot < nslots;
+    T gE[DE];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) gE[j] = T(0);
+    T gw[WANT_GW ? P : 1];
+#pragma unroll
+    for (int p = 0; p < (WANT_GW ? P : 1); ++p) gw[p] = T(0);
+
+    if (!compute) {
+        // ---------------------------------------------------------------- producer
+        if (lane == 0) {
+            auto issue = [&](int t) {
+                const int s = t % NST;
+                const int eb = e0 + t * nslots;
+                const int ne = min(nslots, e1 - eb);
+                const uint32_t bytes = (uint32_t)ne * row_bytes;
+                mbar_expect_tx(&r.full[s], bytes);
+                if constexpr (SW) {
+                    for (int i = 0; i < ne; ++i) tma_load_2d(r.stage(s) + (size_t)i * row_bytes, &tm.a, 0, (eb + i) * n, &r.full[s]);
+                } else {
+                    bulk_load(r.stage(s), V + (size_t)eb * n * DV, bytes, &r.full[s]);
+                }
+            };
+            const int pre = ntiles < NST ? ntiles : NST;
+            for (int t = 0; t < pre; ++t) issue(t);
+            for (int u = 0; u < ntiles; ++u) {
+                const int s = u % NST;
+                mbar_wait(&r.done[s], (uint32_t)(u / NST) & 1u);
+                if constexpr (WANT_GV) {
+                    const int eb = e0 + u * nslots;
+                    const int ne = min(nslots, e1 - eb);
+                    if constexpr (SW) {
+                        for (int i = 0; i < ne; ++i) tma_store_2d(&tm.b, 0, (eb + i) * n, r.stage(s) + (size_t)i * row_bytes);
+                    } else {
+                        bulk_store(gV + (size_t)eb * n * DV, r.stage(s), (uint32_t)ne * row_bytes);
+                    }
+                    bulk_commit();
+                    if (NST == 1) {
+                        if (u + 1 < ntiles) { bulk_wait_read<0>(); issue(u + 1); }
+                    } else if (u >= 1 && u - 1 + NST < ntiles) {
+                        bulk_wait_read<1>();
+                        issue(u - 1 + NST);
+                    }
+                } else {
+                    if (u + NST < ntiles) issue(u + NST);  // every warp is done with stage s
+                }
+            }
+            if constexpr (WANT_GV) bulk_wait_read<0>();
+        }
+    } else {
+        // ---------------------------------------------------------------- compute warps
+        T E[DE];
+        T qc = T(0);
+#pragma unroll
+        for (int j = 0; j < DE; ++j) E[j] = T(0);
+        if (active) {
+            const T* er = Eenv + ((size_t)c * n + ch) * DE;
+#pragma unroll
+            for (int j = 0; j < DE; ++j) E[j] = er[j];
+            qc = q[ch];
+        }
+        const int mode = slot_sum_mode(n);
+        for (int t = 0; t < ntiles; ++t) {
+            const int s = t % NST;
+            mbar_wait(&r.full[s], (uint32_t)(t / NST) & 1u);
+            const int eb = e0 + t * nslots;
+            const bool valid = active && eb + slot < e1;
+            T epart = T(0);
+            if (valid) {
+                T* row = reinterpret_cast<T*>(r.stage(s)) + ((size_t)slot * n + ch) * DV;
+                [[maybe_unused]] const uint32_t sw = ((uint32_t)(slot * n + ch) & 7u) << 4;
+                T v[DV], g[DV], gv[DV];
+                if constexpr (SW) row_load_sw<T, DV>(reinterpret_cast<const unsigned char*>(row), sw, v);
+                else row_load<T, DV>(row, v);
+                Gen::template fwd<T>(cwt.v, v, E, g);                 // g = out
+                T sq = T(0);
+#pragma unroll
+                for (int k = 0; k < DV; ++k) sq = fma(g[k], g[k], sq);
+                epart = fma(T(0.5) * kappa, sq, qc * g[0]);
+#pragma unroll
+                for (int k = 0; k < DV; ++k) g[k] *= kappa;            // g = cotangent of the A12 energy
+                g[0] += qc;
+                // scheduling fence: the VJP below starts from complete g / v rows (otherwise the two unrolled contractions are
+                // interleaved for ILP and their live ranges no longer fit the register file)
+#pragma unroll
+                for (int k = 0; k < DV; ++k) {
+                    if constexpr (sizeof(T) == 4) asm volatile("" : "+f"(g[k]), "+f"(v[k]));
+                    else asm volatile("" : "+d"(g[k]), "+d"(v[k]));
+                }
+                // cwt2 is a second copy of the same table: read through the first one, every coefficient would be kept alive from
+                // its forward use to its VJP use (274 .. 1222 values) and spilled
+                Gen::template bwd<T, WANT_GV>(cwt2.v, v, E, g, gv, gE);
+                if constexpr (WANT_GW) Gen::template pathw<T>(v, E, g, gw);
+                if constexpr (WANT_GV) {
+                    if constexpr (SW) row_store_sw<T, DV>(reinterpret_cast<unsigned char*>(row), sw, gv);
+                    else row_store<T, DV>(row, gv);
+                }
+            }
+            ring_release(&r.done[s], lane);
+            const T tot = slot_sum<T, CT>(epart, mode, n, slot, ch, tid, t, ebuf);
+            if (valid && ch == 0) e_edge[eb + slot] = tot;
+        }
+    }
+    __syncthreads();  // all tiles are computed and every store has left shared memory: the ring can be reused
+
+    // ---- gEenv: slots summed in slot order
+    T* red = reinterpret_cast<T*>(smem_raw);  // [CT][DE], then [warps][P]
+    if (active) {
+#pragma unroll
+        for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = gE[j];
+    }
+    __syncthreads();
+    if (compute && slot == 0) {
+        T* dst = gE_dst + ((size_t)(gE_by_item ? (long)blockIdx.x : (long)c) * n + ch) * DE;
+#pragma unroll
+        for (int j = 0; j < DE; ++j) {
+            T acc = red[(size_t)ch * DE + j];
+            for (int sl = 1; sl < nslots; ++sl) acc += red[((size_t)sl * n + ch) * DE + j];
+            dst[j] = acc;
+        }
+    }
+    if constexpr (WANT_GW) {
+        __syncthreads();
+        if (compute) {
+#pragma unroll
+            for (int p = 0; p < P; ++p) {
+                T a = gw[p];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) a += __shfl_xor_sync(0xffffffffu, a, o);
+                if (lane == 0) red[warp * P + p] = a;
+            }
+        }
+        __syncthreads();
+        if (tid < P) {
+            T acc = red[tid];
+            for (int wv = 1; wv < CT / 32; ++wv) acc += red[wv * P + tid];
+            gw_part[(size_t)blockIdx.x * P + tid] = acc;
+        }
+    }
+}
+
 // g_path_w[p] = sum over items of the partial rows: each thread adds a strided subset in order (double),
 // then a fixed-shape shared-memory tree.  One CTA per path.
 template <typename T>

@@ -53,6 +53,8 @@ class SingleLayerStep:
       "epilogue" : tp_forward_energy (out, e_edge, G from one kernel) -> tp_backward
       "onthefly" : tp_forward_energy (out, e_edge) -> tp_backward_energy (cotangent formed from out in registers;
                    G never exists in HBM)
+      "fused"    : tp_fused_energy: forward, energy and VJP in ONE kernel (V read once, gV written once, out and G never
+                   exist in HBM; self.out stays unwritten)
     `fused_geometry`: env_radial_forward / env_radial_backward (w and g_w never exist in HBM) instead of
     radial_forward + env_embed / env_embed_backward + radial_backward."""
 
@@ -61,7 +63,7 @@ class SingleLayerStep:
         """sharded: a sharding.ShardedForces when `dev` holds ONE RANK'S rows of a system split over several GPUs (row_ptr / rev are the
         rank-local index arrays of its HaloPlan): g_r is written into its extended array, the halo exchange runs before the force
         gather, energies (and g_path_w) are summed over the ranks"""
-        assert mode in ("separate", "epilogue", "onthefly")
+        assert mode in ("separate", "epilogue", "onthefly", "fused")
         self.sharded = sharded
         self.plan, self.dev, self.rc, self.kappa, self.scale, self.mode = plan, dev, rc, kappa, scale, mode
         self.fused_geometry = fused_geometry
@@ -72,9 +74,9 @@ class SingleLayerStep:
         n = plan.n
         self.w = None if fused_geometry else torch.empty((self.E, n), dtype=dt, device=dv)
         self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
-        self.out = torch.empty_like(V)
+        self.out = torch.empty_like(V) if mode != "fused" else None
         self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
-        self.G = torch.empty_like(V) if mode != "onthefly" else None
+        self.G = torch.empty_like(V) if mode in ("separate", "epilogue") else None
         self.gV = torch.empty_like(V) if want_gV else None
         self.gEenv = torch.empty_like(self.Eenv)
         self.g_path_w = torch.empty((plan.P,), dtype=dt, device=dv) if want_g_path_w else None
@@ -122,10 +124,12 @@ class SingleLayerStep:
             timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it, out=self.out,
                                                                     e_edge=self.e_edge, G=self.G))
             timed("tp_backward", lambda: ab.tp_backward(p, rp, self.G, V, self.Eenv, pw, **bw))
-        else:
+        elif self.mode == "onthefly":
             timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, items=it, out=self.out,
                                                                     e_edge=self.e_edge, want_G=False))
             timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp, self.out, V, self.Eenv, pw, d["q"], self.kappa, **bw))
+        else:
+            timed("tp_fused_energy", lambda: ab.tp_fused_energy(p, rp, V, self.Eenv, pw, d["q"], self.kappa, e_edge=self.e_edge, **bw))
         if self.fused_geometry:
             timed("env_radial_backward", lambda: ab.env_radial_backward(p, rp, self.gEenv, rvec, d["W_r"], self.rc, self.scale, g_rvec=self.g_r))
         else:
@@ -155,6 +159,8 @@ class SingleLayerStep:
         else:
             ab.radial_forward(rvec, d["W_r"], self.rc, w=self.w)
             ab.env_embed(p, rp, rvec, self.w, self.scale, items=it, Eenv=self.Eenv, workspace=self.ws_env)
+        if self.out is None:       # mode "fused" never materialises `out`: the forward-only timing needs a buffer of its own
+            self.out = torch.empty_like(V)
         ab.tp_forward_energy(p, rp, V, self.Eenv, None, d["q"], self.kappa, items=it, out=self.out, e_edge=self.e_edge, want_G=False)
         ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot)
         return self.e_tot
@@ -179,6 +185,7 @@ class SingleLayerStep:
             "tp_forward_energy": (3 if self.G is not None else 2) * feat + env + E * s + (N + 1) * 4,
             "tp_backward": bwd,
             "tp_backward_energy": bwd,
+            "tp_fused_energy": (2 if self.gV is not None else 1) * feat + 2 * env + E * s + (N + 1) * 4,
             "env_radial_forward": E * 3 * s + env + (N + 1) * 4,
             "env_radial_backward": env + 2 * E * 3 * s + (N + 1) * 4,
             "env_embed_backward": env + E * 3 * s + wrow + wrow + E * 3 * s + (N + 1) * 4,
@@ -218,11 +225,14 @@ class ChunkedStep:
     resident, the centres are processed in `n_chunks` contiguous ranges that reuse one set of chunk-sized work buffers
     (out, gV), and the per-edge results that the force assembly needs (g_r, e_edge) are written into full-size arrays.
     Chunks are independent because every per-edge / per-centre quantity depends on one centre (strict locality).
-    Call sequence per chunk: env_radial_forward -> tp_forward_energy -> tp_backward_energy -> env_radial_backward;
-    then one force_gather and one segment_sum over the whole system."""
+    Call sequence per chunk: env_radial_forward -> tp_fused_energy (forward + energy + VJP in one kernel: no `out` buffer at
+    all) -> env_radial_backward; then one force_gather and one segment_sum over the whole system.  fused=False keeps the two-kernel
+    sequence tp_forward_energy -> tp_backward_energy with a chunk-sized `out` buffer (parity tests read it)."""
 
-    def __init__(self, plan, dev, row_ptr_host, rc, kappa, scale=1.0, n_chunks=8, want_gV=True):
+    def __init__(self, plan, dev, row_ptr_host, rc, kappa, scale=1.0, n_chunks=8, want_gV=True, fused=None):
         from .sharding import partition_centres
+        fused = plan.l_max <= 2 if fused is None else fused      # at l_max = 3 the two-kernel sequence is faster (DESIGN.md section 6)
+        self.fused = fused
         self.plan, self.dev, self.rc, self.kappa, self.scale = plan, dev, rc, kappa, scale
         rp_h = np.asarray(row_ptr_host, dtype=np.int64)
         self.N, self.E = rp_h.shape[0] - 1, int(rp_h[-1])
@@ -238,8 +248,8 @@ class ChunkedStep:
         n = plan.n
         self.Eenv = torch.empty((self.N, n, plan.dE), dtype=dt, device=dv)
         self.gEenv = torch.empty_like(self.Eenv)
-        self.out = torch.empty((emax, n, plan.dV), dtype=dt, device=dv)
-        self.gV = torch.empty_like(self.out) if want_gV else None
+        self.out = None if fused else torch.empty((emax, n, plan.dV), dtype=dt, device=dv)
+        self.gV = torch.empty((emax, n, plan.dV), dtype=dt, device=dv) if want_gV else None
         self.e_edge = torch.empty((self.E,), dtype=dt, device=dv)
         self.g_r = torch.empty((self.E, 3), dtype=dt, device=dv)
         self.F = torch.empty((self.N, 3), dtype=dt, device=dv)
@@ -271,21 +281,25 @@ class ChunkedStep:
             m = e1 - e0
             rvec, V = d["rvec"][e0:e1], d["V"][e0:e1]
             Eenv, gE = self.Eenv[c0:c1], self.gEenv[c0:c1]
-            out = self.out[:m]
+            out = None if self.out is None else self.out[:m]
             gV = None if self.gV is None else self.gV[:m]
             timed("env_radial_forward", lambda: ab.env_radial_forward(p, rp_c, rvec, d["W_r"], self.rc, self.scale, Eenv=Eenv))
-            timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp_c, V, Eenv, None, d["q"], self.kappa, out=out,
-                                                                    e_edge=self.e_edge[e0:e1], want_G=False))
-            timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp_c, out, V, Eenv, None, d["q"], self.kappa,
-                                                                      want_gV=gV is not None, gV=gV, gEenv=gE, workspace=self.ws))
+            if self.fused:
+                timed("tp_fused_energy", lambda: ab.tp_fused_energy(p, rp_c, V, Eenv, None, d["q"], self.kappa, e_edge=self.e_edge[e0:e1],
+                                                                    want_gV=gV is not None, gV=gV, gEenv=gE, workspace=self.ws))
+            else:
+                timed("tp_forward_energy", lambda: ab.tp_forward_energy(p, rp_c, V, Eenv, None, d["q"], self.kappa, out=out,
+                                                                        e_edge=self.e_edge[e0:e1], want_G=False))
+                timed("tp_backward_energy", lambda: ab.tp_backward_energy(p, rp_c, out, V, Eenv, None, d["q"], self.kappa,
+                                                                          want_gV=gV is not None, gV=gV, gEenv=gE, workspace=self.ws))
             timed("env_radial_backward", lambda: ab.env_radial_backward(p, rp_c, gE, rvec, d["W_r"], self.rc, self.scale,
                                                                         g_rvec=self.g_r[e0:e1]))
             if keep is not None and k in keep:
                 if "rows" in keep[k]:
-                    keep[k]["out"] = [out[a - e0:b - e0].clone() for a, b in keep[k]["rows"]]
+                    keep[k]["out"] = [None if out is None else out[a - e0:b - e0].clone() for a, b in keep[k]["rows"]]
                     keep[k]["gV"] = [None if gV is None else gV[a - e0:b - e0].clone() for a, b in keep[k]["rows"]]
                 else:
-                    keep[k].update(out=out.clone(), gV=None if gV is None else gV.clone())
+                    keep[k].update(out=None if out is None else out.clone(), gV=None if gV is None else gV.clone())
         timed("force_gather", lambda: ab.force_gather(d["row_ptr"], d["rev"], self.g_r, F=self.F))
         timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))
         return self.F, self.e_tot
@@ -296,7 +310,8 @@ class ChunkedStep:
         E, N, n, dV, dE = self.E, self.N, p.n, p.dV, p.dE
         feat, env = E * n * dV * s, N * n * dE * s
         return {"env_radial_forward": E * 3 * s + env, "tp_forward_energy": 2 * feat + env + E * s,
-                "tp_backward_energy": (3 if self.gV is not None else 2) * feat + 2 * env, "env_radial_backward": env + 2 * E * 3 * s,
+                "tp_backward_energy": (3 if self.gV is not None else 2) * feat + 2 * env,
+                "tp_fused_energy": (2 if self.gV is not None else 1) * feat + 2 * env + E * s, "env_radial_backward": env + 2 * E * 3 * s,
                 "force_gather": 2 * E * 3 * s + E * 4 + N * 3 * s, "segment_sum": E * s}
 
 

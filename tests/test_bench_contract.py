@@ -24,7 +24,7 @@ def _run(args):
 def test_reference_arm_line():
     d = _run(["--impl", "reference", "--workload", "C1s", "--steps", "1", "--warmup", "0"])
     assert BASE_KEYS <= set(d) and d["impl"] == "reference"
-    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] == 1 and d["cpu_baseline"]["value"] == d["value"]
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1 and d["cpu_baseline"]["value"] == d["value"]
     assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
     assert d["value"] > 0 and d["vs_baseline"] is None and d["config"]["workload"] == "C1s"
 

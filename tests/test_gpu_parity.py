@@ -66,7 +66,7 @@ def test_forward_energy_epilogue(name, want_out):
 
 
 @pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
-@pytest.mark.parametrize("mode,fused_geometry", [("separate", False), ("epilogue", False), ("onthefly", False), ("onthefly", True)])
+@pytest.mark.parametrize("mode,fused_geometry", [("separate", False), ("epilogue", False), ("onthefly", False), ("onthefly", True), ("fused", True)])
 def test_single_layer_step_modes(name, mode, fused_geometry):
     """the three call sequences of pipeline.SingleLayerStep (the object bench.py times) give the oracle's forces,
     energies and gradients; "onthefly" exercises tp_backward_energy (cotangent formed from out in registers)"""
@@ -584,6 +584,12 @@ def test_energy_epilogue_channel_counts(n, dt):
     torch.cuda.synchronize()
     _assert_close(dict(out=out, e_edge=e_edge, G=G, gV=gV, gEenv=gE), dict(out=o, e_edge=e, G=Gd, gV=gVd, gEenv=gEd), dt,
                   keys=("out", "e_edge", "G", "gV", "gEenv"), label="n=%d" % n)
+    # the same through the single fused kernel (forward + energy + VJP), also with centres split into items
+    for items in (None, ab.segments_build(rp, 5)):
+        it = None if items is None else d(items)
+        e2, gV2, gE2, _ = ab.tp_fused_energy(plan, rpd, Vd, Ed, pwd, qd, kappa, items=it)
+        torch.cuda.synchronize()
+        _assert_close(dict(e_edge=e_edge, gV=gV, gEenv=gE), dict(e_edge=e2, gV=gV2, gEenv=gE2), dt, keys=("e_edge", "gV", "gEenv"), label="fused n=%d" % n)
 
 
 def _model_device(inp):
@@ -784,7 +790,7 @@ def test_library_graph_step_matches_eager(name):
     F0, e0, gV0 = st.F.clone(), st.e_tot.clone(), st.gV.clone()
     F, e = torch.empty_like(st.F), torch.empty_like(st.e_tot)
     g = ab.LayerStepGraph(plan, dev["row_ptr"], dev["rev"], dev["rvec"], dev["V"], dev["W_r"], inp["rc"], dev["q"], inp["kappa"], inp["scale"], F, e)
-    assert g.kernels_per_step == 6
+    assert g.kernels_per_step == 5
     F.zero_()
     g.run()
     torch.cuda.synchronize()
