@@ -220,6 +220,14 @@ def force_gather(row_ptr, rev, g_rvec):
     return F
 
 
+def virial(rvec, g_rvec):
+    """W[a][b] = sum_e g_rvec[e][a] rvec[e][b] (reading A25) -> [3,3]"""
+    rvec, g_rvec = _f64(rvec), _f64(g_rvec)
+    W = np.zeros((3, 3))
+    lib().orc_virial(C.c_int64(rvec.shape[0]), _d(rvec), _d(g_rvec), _d(W))
+    return W
+
+
 def edge_energy(lmax, out, q, kappa, want_G=True):
     """-> (e_edge[E], G or None)"""
     out, q = _f64(out), _f64(q)

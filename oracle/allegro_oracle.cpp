@@ -611,6 +611,17 @@ void orc_force_gather(int N, const int32_t* row_ptr, const int32_t* rev, const d
     }
 }
 
+/* Virial of an energy that depends on the positions only through the edge vectors (reading A25): under the homogeneous
+   deformation r_e -> (I + eps) r_e,  dE/d eps[a][b] = sum_e g_rvec[e][a] * r_e[b] =: W[a][b] (sum over DIRECTED edges: each is its
+   own term of E_tot).  Pressure = -trace(W) / (3 volume).  (the MD integration consumes forces; stress is the
+   companion quantity for constant-pressure MD.) */
+void orc_virial(int64_t E, const double* rvec, const double* g_rvec, double* W) {
+    for (int i = 0; i < 9; ++i) W[i] = 0.0;
+    for (int64_t e = 0; e < E; ++e)
+        for (int a = 0; a < 3; ++a)
+            for (int b = 0; b < 3; ++b) W[3 * a + b] += g_rvec[3 * (size_t)e + a] * rvec[3 * (size_t)e + b];
+}
+
 void orc_edge_energy(int lmax, int n, int64_t E, const double* out, const double* q, double kappa,
                      double* e_edge, double* G) {
     int dV = orc_dim_v(lmax);

@@ -95,6 +95,8 @@ void    orc_edge_energy(int lmax, int n, int64_t E, const double* out, const dou
                         double kappa, double* e_edge, double* G);
 /* out[s] = sum_{i = ptr[s]}^{ptr[s+1]-1} vals[i], sequential */
 void    orc_segment_sum(const int32_t* ptr, int nseg, const double* vals, double* out);
+/* W[a][b] = sum_e g_rvec[e][a] rvec[e][b]  (reading A25: dE/d(strain), directed edges) */
+void    orc_virial(int64_t E, const double* rvec, const double* g_rvec, double* W);
 
 
 #ifdef __cplusplus

@@ -343,3 +343,32 @@ def test_generated_neighbour_lists_are_valid():
         ii, jj = np.nonzero(adj)
         assert np.array_equal(ii, ctr) and np.array_equal(jj, col)
         assert np.allclose(d[ii, jj], rv, atol=1e-12)
+
+
+def test_virial_is_the_strain_derivative_of_the_energy():
+    """orc.virial (reading A25) pinned by central finite differences: deform every edge vector by r -> (I + h e_a e_b^T) r, re-evaluate
+    the whole chain's energy (radial weights, embedding, tensor product, energy) and difference; all nine components, plus the
+    closed form trace(W) = sum_e r_e . g_r[e] = dE/d(ln scale).  The configs' boxes play no role: the energy sees positions only
+    through the edge vectors."""
+    import _chain
+    inp = _chain.make_inputs("C0")
+    base = _chain.oracle_chain(inp, want_gw=False)
+    W = oracle.virial(inp["rvec"].astype(np.float64), base["g_r"])
+    assert W.shape == (3, 3)
+    assert abs(np.trace(W) - float(np.sum(inp["rvec"].astype(np.float64) * base["g_r"]))) <= 1e-12 * abs(np.trace(W))
+
+    def energy(defo):
+        sub = dict(inp)
+        sub["rvec"] = inp["rvec"].astype(np.float64) @ defo.T
+        return float(np.sum(_chain.oracle_chain(sub, want_gw=False, forces=False)["e_edge"]))
+
+    h = 1e-6
+    for a in range(3):
+        for b in range(3):
+            d = np.zeros((3, 3))
+            d[a, b] = h
+            fd = (energy(np.eye(3) + d) - energy(np.eye(3) - d)) / (2 * h)
+            assert abs(fd - W[a, b]) <= 2e-7 * np.abs(W).max(), (a, b, fd, W[a, b])
+    # W is NOT symmetric here (V ~ N(0,1) does not rotate with the geometry, so E_tot is not rotation invariant): a transposed
+    # definition fails the off-diagonal finite differences above
+    assert np.abs(W - W.T).max() > 1e-3 * np.abs(W).max()
