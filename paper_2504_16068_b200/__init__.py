@@ -59,6 +59,7 @@ SIGNATURES = {
     "allegro_env_radial_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, C.c_double, C.c_double, _vp, _vp, _vp]),
     "allegro_edge_energy": (C.c_int, [_vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_segment_sum": (C.c_int, [_vp, C.c_int, _vp, C.c_int, _vp, _vp]),
+    "allegro_virial": (C.c_int, [C.c_long, _vp, _vp, C.c_int, _vp, _vp]),
     "allegro_layer_step_host_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_int, C.c_int]),
     "allegro_layer_step_host": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, C.c_double, C.c_double,
                                           C.c_int, _vp, _vp, _vp, C.c_size_t, _vp]),
@@ -75,6 +76,10 @@ SIGNATURES = {
     "allegro_latent_forward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_latent_backward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_add_inplace": (C.c_int, [C.c_long, C.c_int, _vp, _vp, _vp]),
+    "allegro_neighbour_workspace": (C.c_size_t, [C.c_int]),
+    "allegro_neighbour_count": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, _vp, C.c_size_t, _vp, C.POINTER(C.c_long)]),
+    "allegro_neighbour_fill": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, C.c_long, _vp, _vp, _vp, C.c_int, _vp,
+                                         C.c_size_t, _vp]),
     "allegro_measure_fp32_fma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
     "allegro_measure_tf32_mma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
     "allegro_measure_tf32_mma_rate": (C.c_int, [C.c_int, _vp, C.POINTER(C.c_double)]),
@@ -379,6 +384,14 @@ def edge_energy(plan, out, q, kappa, want_e=True, want_G=True, e_edge=None, G=No
     return e_edge, G
 
 
+def virial(rvec, g_rvec, W=None, stream=None):
+    """-> W [3,3]: W[a][b] = sum_e g_rvec[e][a] rvec[e][b]"""
+    if W is None:
+        W = torch.empty((3, 3), dtype=rvec.dtype, device=rvec.device)
+    _check(lib().allegro_virial(rvec.shape[0], _ptr(rvec), _ptr(g_rvec), _dt(rvec), _ptr(W), _stream(stream)))
+    return W
+
+
 def segment_sum(ptr, vals, out=None, stream=None):
     nseg = ptr.shape[0] - 1
     if out is None:
@@ -476,6 +489,32 @@ class LayerStepGraph:
         if getattr(self, "h", None) and _lib is not None:
             _lib.allegro_layer_step_destroy(self.h)
             self.h = None
+
+
+def neighbour_list(pos, r_cut, box=None, mol_id=None, dtype=F32, stream=None):
+    """positions (device, float64 [N,3]) -> dict(row_ptr, col, rev, rvec) on the device (allegro_neighbour_count / _fill).
+    box: cubic periodic box edge, or None for an open system (the bounding box is taken from the positions)."""
+    assert pos.dtype == torch.float64 and pos.is_cuda
+    N = pos.shape[0]
+    ws = torch.empty(max(lib().allegro_neighbour_workspace(N), 16), dtype=torch.uint8, device=pos.device)
+    row_ptr = torch.empty((N + 1,), dtype=torch.int32, device=pos.device)
+    lo = hi = None
+    if box is None:
+        lo = np.ascontiguousarray(pos.min(0).values.cpu().numpy() if N else np.zeros(3))
+        hi = np.ascontiguousarray(pos.max(0).values.cpu().numpy() if N else np.ones(3))
+    plo = None if lo is None else lo.ctypes.data_as(_f64p)
+    phi = None if hi is None else hi.ctypes.data_as(_f64p)
+    n_edges = C.c_long(0)
+    b = float(box) if box is not None else 0.0
+    _check(lib().allegro_neighbour_count(N, _ptr(pos), b, plo, phi, float(r_cut), _ptr(mol_id), _ptr(row_ptr), _ptr(ws), ws.numel(),
+                                         _stream(stream), C.byref(n_edges)))
+    E = n_edges.value
+    col = torch.empty((E,), dtype=torch.int32, device=pos.device)
+    rev = torch.empty((E,), dtype=torch.int32, device=pos.device)
+    rvec = torch.empty((E, 3), dtype=torch_dtype(dtype), device=pos.device)
+    _check(lib().allegro_neighbour_fill(N, _ptr(pos), b, plo, phi, float(r_cut), _ptr(mol_id), _ptr(row_ptr), E, _ptr(col), _ptr(rev), _ptr(rvec),
+                                        dtype, _ptr(ws), ws.numel(), _stream(stream)))
+    return dict(row_ptr=row_ptr, col=col, rev=rev, rvec=rvec)
 
 
 def measure_peaks(stream=None):

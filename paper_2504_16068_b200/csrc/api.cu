@@ -404,6 +404,13 @@ allegro_status_t allegro_edge_energy(const allegro_plan_t* plan, long n_edges, c
                : launch_edge_energy<double>(plan->n, plan->tab.dV, n_edges, out, q, kappa, e_edge, G, (cudaStream_t)stream);
 }
 
+allegro_status_t allegro_virial(long n_edges, const void* rvec, const void* g_rvec, allegro_dtype_t dtype, void* W, void* stream) {
+    ALLEGRO_CHECK_ARG(n_edges >= 0 && W != nullptr && ((rvec && g_rvec) || n_edges == 0), "bad argument");
+    ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
+    return dtype == ALLEGRO_F32 ? launch_virial<float>(n_edges, rvec, g_rvec, W, (cudaStream_t)stream)
+                                : launch_virial<double>(n_edges, rvec, g_rvec, W, (cudaStream_t)stream);
+}
+
 allegro_status_t allegro_segment_sum(const int32_t* ptr, int n_segments, const void* vals, allegro_dtype_t dtype, void* out, void* stream) {
     ALLEGRO_CHECK_ARG(n_segments >= 0 && ((ptr && out) || n_segments == 0), "bad argument");
     ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");

@@ -106,6 +106,8 @@ allegro_status_t launch_force_gather(int n_atoms, long E, const int32_t* row_ptr
 template <typename T>
 allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, const void* q, double kappa, void* e_edge, void* G, cudaStream_t st);
 template <typename T>
+allegro_status_t launch_virial(long E, const void* rvec, const void* g_rvec, void* W, cudaStream_t st);
+template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st);
 
 // 2-D tensor map over a feature tensor whose rows are exactly 128 bytes: [rows][32 x 4 B], box = box_rows rows, 128-byte swizzle

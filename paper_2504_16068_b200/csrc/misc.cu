@@ -235,6 +235,66 @@ allegro_status_t launch_edge_energy(int n, int dV, long E, const void* out, cons
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
+// W[a][b] = sum_e g_rvec[e][a] rvec[e][b] (reading A25).  One 8-CTA cluster: every thread adds a strided subset of the edges in
+// double, each CTA folds its threads with a fixed shared-memory tree per component, CTA 0 adds the CTAs' partials in rank order
+// through distributed shared memory (deterministic, no workspace, no atomics).
+template <typename T>
+__global__ void __launch_bounds__(kSegThreads) virial_kernel(long E, const T* __restrict__ rvec, const T* __restrict__ g, T* __restrict__ W) {
+    namespace cg = cooperative_groups;
+    cg::cluster_group cluster = cg::this_cluster();
+    __shared__ double sh[9][kSegThreads];
+    const int rank = (int)cluster.block_rank();
+    double acc[9];
+#pragma unroll
+    for (int i = 0; i < 9; ++i) acc[i] = 0.0;
+    for (long e = (long)rank * kSegThreads + threadIdx.x; e < E; e += (long)kSegThreads * kSegCluster) {
+        const double r0 = (double)rvec[3 * e], r1 = (double)rvec[3 * e + 1], r2 = (double)rvec[3 * e + 2];
+#pragma unroll
+        for (int a = 0; a < 3; ++a) {
+            const double ga = (double)g[3 * e + a];
+            acc[3 * a] = fma(ga, r0, acc[3 * a]);
+            acc[3 * a + 1] = fma(ga, r1, acc[3 * a + 1]);
+            acc[3 * a + 2] = fma(ga, r2, acc[3 * a + 2]);
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < 9; ++i) sh[i][threadIdx.x] = acc[i];
+    __syncthreads();
+    for (int o = kSegThreads / 2; o > 0; o >>= 1) {
+        if ((int)threadIdx.x < o) {
+#pragma unroll
+            for (int i = 0; i < 9; ++i) sh[i][threadIdx.x] += sh[i][threadIdx.x + o];
+        }
+        __syncthreads();
+    }
+    cluster.sync();
+    if (rank == 0 && threadIdx.x < 9) {
+        double tot = sh[threadIdx.x][0];
+        for (int r = 1; r < kSegCluster; ++r) tot += *cluster.map_shared_rank(&sh[threadIdx.x][0], r);
+        W[threadIdx.x] = (T)tot;
+    }
+    cluster.sync();  // keep every CTA's shared memory alive until CTA 0 has read it
+}
+
+template <typename T>
+allegro_status_t launch_virial(long E, const void* rvec, const void* g_rvec, void* W, cudaStream_t st) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(kSegCluster);
+    cfg.blockDim = dim3(kSegThreads);
+    cfg.dynamicSmemBytes = 0;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = kSegCluster;
+    attr[0].val.clusterDim.y = 1;
+    attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    ALLEGRO_CUDA(cudaLaunchKernelEx(&cfg, virial_kernel<T>, E, (const T*)rvec, (const T*)g_rvec, (T*)W));
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
 template <typename T>
 allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* vals, void* out, cudaStream_t st) {
     if (nseg == 0) return ALLEGRO_OK;
@@ -260,6 +320,7 @@ allegro_status_t launch_segment_sum(const int32_t* ptr, int nseg, const void* va
     template allegro_status_t launch_radial_backward<T>(int, int, double, long, const void*, const void*, const void*, void*, cudaStream_t); \
     template allegro_status_t launch_force_gather<T>(int, long, const int32_t*, const int32_t*, const void*, void*, cudaStream_t);    \
     template allegro_status_t launch_edge_energy<T>(int, int, long, const void*, const void*, double, void*, void*, cudaStream_t);    \
+    template allegro_status_t launch_virial<T>(long, const void*, const void*, void*, cudaStream_t);                                   \
     template allegro_status_t launch_segment_sum<T>(const int32_t*, int, const void*, void*, cudaStream_t);
 ALLEGRO_INST(float)
 ALLEGRO_INST(double)

@@ -805,3 +805,45 @@ def test_library_graph_step_matches_eager(name):
         ab.LayerStepGraph(ab.Plan(inp["lmax"], inp["n"], dt), dev["row_ptr"], dev["rev"], dev["rvec"], dev["V"], dev["W_r"], inp["rc"], dev["q"],
                           inp["kappa"], inp["scale"], F, e)
     assert ei.value.status == 1
+
+
+@pytest.mark.parametrize("name", ["C0", "C1s", "C4s"])
+def test_virial(name):
+    """allegro_virial against the oracle's (reading A25), on the g_r of the GPU chain; bitwise reproducible"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    inp = _chain.make_inputs(name)
+    got = _chain.gpu_chain(inp, want_gw=False)
+    dev = _chain.to_device(inp)
+    W = ab.virial(dev["rvec"], got["g_r"])
+    ref = orc.virial(inp["rvec"].astype(np.float64), got["g_r"].cpu().numpy().astype(np.float64))
+    assert np.max(np.abs(W.cpu().numpy().astype(np.float64) - ref)) <= _chain.TOL[inp["dt"]] * np.max(np.abs(ref))
+    assert torch.equal(W, ab.virial(dev["rvec"], got["g_r"]))
+    ref_full = orc.virial(inp["rvec"].astype(np.float64), _chain.oracle_chain(inp, want_gw=False, forces=False)["g_r"])
+    assert np.max(np.abs(W.cpu().numpy().astype(np.float64) - ref_full)) <= 10 * _chain.TOL[inp["dt"]] * np.max(np.abs(ref_full))
+
+
+@pytest.mark.parametrize("name", ["C0", "C1s", "C4s", "C1"])
+def test_gpu_neighbour_list_bit_exact(name):
+    """allegro_neighbour_count / _fill: the cell-list builder on the GPU gives the CSR list of workloads/geometry.py (k-d tree on the
+    host) bit for bit -- row_ptr, neighbour indices, reverse-edge permutation -- and the same edge vectors after the one rounding
+    to the config's dtype (readings A7, A9, A17); C0's box holds two cells per direction (all-pairs path), C4s is open with a
+    molecule filter, C1 is the full 4,096-atom box"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs
+    g = configs.geometry_for(name)
+    dt = np.float64 if g["spec"]["dtype"] == "f64" else np.float32
+    pos = torch.from_numpy(np.ascontiguousarray(g["pos"])).cuda()
+    mol = None
+    if g["mol_ptr"] is not None:
+        mol = torch.from_numpy((np.searchsorted(g["mol_ptr"], np.arange(pos.shape[0]), side="right") - 1).astype(np.int32)).cuda()
+    nl = ab.neighbour_list(pos, g["spec"]["rc"], box=g["box"], mol_id=mol, dtype=ab.F64 if dt == np.float64 else ab.F32)
+    torch.cuda.synchronize()
+    assert np.array_equal(nl["row_ptr"].cpu().numpy(), g["row_ptr"])
+    assert np.array_equal(nl["col"].cpu().numpy(), g["col"])
+    assert np.array_equal(nl["rev"].cpu().numpy(), g["rev"])
+    assert np.array_equal(nl["rvec"].cpu().numpy(), g["rvec"].astype(dt))
