@@ -220,6 +220,16 @@ def force_gather(row_ptr, rev, g_rvec):
     return F
 
 
+def tp_double_backward(lmax, row_ptr, G, V, Eenv, path_w, aV, bE):
+    """gradients of S = <aV, gV> + <bE, gEenv> (outputs of tp_backward, scalar weights) -> (dG, dV, dEenv, dw)  (reading A26)"""
+    row_ptr, G, V, Eenv, path_w, aV, bE = _i32(row_ptr), _f64(G), _f64(V), _f64(Eenv), _f64(path_w), _f64(aV), _f64(bE)
+    assert path_w.ndim == 1
+    N, n = row_ptr.shape[0] - 1, V.shape[1]
+    dG, dV, dE, dw = np.zeros_like(V), np.zeros_like(V), np.zeros_like(Eenv), np.zeros_like(path_w)
+    lib().orc_tp_double_backward(lmax, n, N, _i(row_ptr), _d(G), _d(V), _d(Eenv), _d(path_w), _d(aV), _d(bE), _d(dG), _d(dV), _d(dE), _d(dw))
+    return dG, dV, dE, dw
+
+
 def virial(rvec, g_rvec):
     """W[a][b] = sum_e g_rvec[e][a] rvec[e][b] (reading A25) -> [3,3]"""
     rvec, g_rvec = _f64(rvec), _f64(g_rvec)

@@ -601,6 +601,47 @@ void orc_env_embed_backward(int lmax, int n, int N, const int32_t* row_ptr, int 
     }
 }
 
+/* Second derivative of the tensor product ("the additional kernels required for training are left for future work";
+   SURVEY 8.f2: VJP-of-VJP for a force-matching loss).  The first derivative (scalar weights, Wc = sum_p w_p C^p) is
+       gV[e,n,i] = sum_{jk} Wc[ijk] E[c,n,j] G[e,n,k],      gE[c,n,j] = sum_{e in row c} sum_{ik} Wc[ijk] V[e,n,i] G[e,n,k].
+   For cotangents aV (of gV) and bE (of gE) the scalar S = <aV, gV> + <bE, gE> has the gradients written out below, term by term
+   over the non-zero list (reading A26: S is trilinear in (aV | bE, V | E, G) and linear in w):
+       dG[e,n,k] = sum_{ij} Wc[ijk] (aV[e,n,i] E[c,n,j] + V[e,n,i] bE[c,n,j])
+       dV[e,n,i] = sum_{jk} Wc[ijk] bE[c,n,j] G[e,n,k]
+       dE[c,n,j] = sum_{e in row c} sum_{ik} Wc[ijk] aV[e,n,i] G[e,n,k]
+       dw[p]     = sum_{e,n} sum_{(ijk) in p} C^p[ijk] G[e,n,k] (aV[e,n,i] E[c,n,j] + V[e,n,i] bE[c,n,j])                       */
+void orc_tp_double_backward(int lmax, int n, int N, const int32_t* row_ptr, const double* G, const double* V, const double* Eenv,
+                            const double* path_w, const double* aV, const double* bE, double* dG, double* dV_, double* dE_, double* dw) {
+    const std::vector<Path>& P = paths_for(lmax);
+    const std::vector<Nz>& L = nz_for(lmax);
+    int dV = orc_dim_v(lmax), dE = orc_dim_e(lmax);
+    for (size_t p = 0; p < P.size(); ++p) dw[p] = 0.0;
+    for (int c = 0; c < N; ++c) {
+        const double* Ec = Eenv + (size_t)c * n * dE;
+        const double* bc = bE + (size_t)c * n * dE;
+        double* dEc = dE_ + (size_t)c * n * dE;
+        for (int q = 0; q < n * dE; ++q) dEc[q] = 0.0;
+        for (int e = row_ptr[c]; e < row_ptr[c + 1]; ++e) {
+            const double* Ve = V + (size_t)e * n * dV;
+            const double* Ge = G + (size_t)e * n * dV;
+            const double* ae = aV + (size_t)e * n * dV;
+            double* dGe = dG + (size_t)e * n * dV;
+            double* dVe = dV_ + (size_t)e * n * dV;
+            for (int q = 0; q < n * dV; ++q) { dGe[q] = 0.0; dVe[q] = 0.0; }
+            for (int ch = 0; ch < n; ++ch)
+                for (size_t z = 0; z < L.size(); ++z) {
+                    const double cw = path_w[L[z].path] * L[z].c;
+                    const int i = ch * dV + L[z].i, j = ch * dE + L[z].j, k = ch * dV + L[z].k;
+                    const double mix = ae[i] * Ec[j] + Ve[i] * bc[j];
+                    dGe[k] += cw * mix;
+                    dVe[i] += cw * bc[j] * Ge[k];
+                    dEc[j] += cw * ae[i] * Ge[k];
+                    dw[L[z].path] += L[z].c * Ge[k] * mix;
+                }
+        }
+    }
+}
+
 /* F[a] = sum_{e in row a} (g_r[e] - g_r[rev[e]])  (r_e = x_nbr - x_centre + shift, F = -dE/dx) */
 void orc_force_gather(int N, const int32_t* row_ptr, const int32_t* rev, const double* g_rvec, double* F) {
     for (int a = 0; a < N; ++a) {

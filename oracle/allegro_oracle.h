@@ -95,6 +95,9 @@ void    orc_edge_energy(int lmax, int n, int64_t E, const double* out, const dou
                         double kappa, double* e_edge, double* G);
 /* out[s] = sum_{i = ptr[s]}^{ptr[s+1]-1} vals[i], sequential */
 void    orc_segment_sum(const int32_t* ptr, int nseg, const double* vals, double* out);
+/* gradients of S = <aV, gV> + <bE, gE> of orc_tp_backward's outputs (scalar weights) with respect to G, V, Eenv, path_w (reading A26) */
+void    orc_tp_double_backward(int lmax, int n, int N, const int32_t* row_ptr, const double* G, const double* V, const double* Eenv,
+                               const double* path_w, const double* aV, const double* bE, double* dG, double* dV, double* dE, double* dw);
 /* W[a][b] = sum_e g_rvec[e][a] rvec[e][b]  (reading A25: dE/d(strain), directed edges) */
 void    orc_virial(int64_t E, const double* rvec, const double* g_rvec, double* W);
 

@@ -372,3 +372,38 @@ def test_virial_is_the_strain_derivative_of_the_energy():
     # W is NOT symmetric here (V ~ N(0,1) does not rotate with the geometry, so E_tot is not rotation invariant): a transposed
     # definition fails the off-diagonal finite differences above
     assert np.abs(W - W.T).max() > 1e-3 * np.abs(W).max()
+
+
+@pytest.mark.parametrize("lmax", [1, 2])
+def test_tp_double_backward_is_the_gradient_of_the_vjp(lmax):
+    """orc.tp_double_backward (reading A26) pinned through the already pinned first derivative: S(G, V, E, w) = <aV, gV> + <bE, gE> with
+    (gV, gE) = orc.tp_backward; central differences of S along random directions of each argument equal <gradient, direction>.
+    S is linear in each argument, so the differences are exact up to rounding; a swapped pair of cotangents or a dropped term fails."""
+    g = _small_graph("C0")
+    rp = g["row_ptr"]
+    E, N = g["rvec"].shape[0], rp.shape[0] - 1
+    n, dV, dE, P = 3, oracle.dim_v(lmax), oracle.dim_e(lmax), len(oracle.paths(lmax)["l1"])
+    rs = np.random.RandomState(5)
+    G, V, aV = rs.randn(E, n, dV), rs.randn(E, n, dV), rs.randn(E, n, dV)
+    Ee, bE = rs.randn(N, n, dE), rs.randn(N, n, dE)
+    w = rs.randn(P)
+
+    def S(G_, V_, E_, w_):
+        gV, gE, _ = oracle.tp_backward(lmax, rp, G_, V_, E_, w_, want_gV=True, want_gw=False)
+        return float(np.sum(aV * gV) + np.sum(bE * gE))
+
+    dG, dVv, dEe, dw = oracle.tp_double_backward(lmax, rp, G, V, Ee, w, aV, bE)
+    h = 1e-3
+    scale = abs(S(G, V, Ee, w)) + 1.0
+    for name, grad, shape in (("G", dG, G.shape), ("V", dVv, V.shape), ("E", dEe, Ee.shape), ("w", dw, w.shape)):
+        d = rs.randn(*shape)
+        args_p = dict(G=G, V=V, E=Ee, w=w)
+        args_m = dict(args_p)
+        args_p[name] = args_p[name] + h * d
+        args_m[name] = args_m[name] - h * d
+        fd = (S(args_p["G"], args_p["V"], args_p["E"], args_p["w"]) - S(args_m["G"], args_m["V"], args_m["E"], args_m["w"])) / (2 * h)
+        assert abs(fd - float(np.sum(grad * d))) <= 1e-9 * scale * 100, (name, fd, float(np.sum(grad * d)))
+    # the two cotangents are not interchangeable: zeroing bE leaves dV = 0 and dG = fwd(aV, E)
+    dG0, dV0, dE0, _ = oracle.tp_double_backward(lmax, rp, G, V, Ee, w, aV, np.zeros_like(bE))
+    assert np.abs(dV0).max() == 0.0
+    assert np.allclose(dG0, oracle.tp_forward(lmax, rp, aV, Ee, w), rtol=0, atol=1e-12 * np.abs(dG0).max())
