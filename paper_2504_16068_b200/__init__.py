@@ -48,6 +48,8 @@ SIGNATURES = {
                                              C.c_size_t, _vp]),
     "allegro_tp_fused_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp, _vp,
                                           C.c_size_t, _vp]),
+    "allegro_tp_double_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
+    "allegro_tp_double_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_long, C.c_int]),
     "allegro_env_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
     "allegro_env_embed_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp]),
@@ -305,6 +307,17 @@ def tp_fused_energy(plan, row_ptr, V, Eenv, path_w, q, kappa, items=None, want_g
                                          _ptr(q), float(kappa), _ptr(e_edge), _ptr(gV), _ptr(gEenv), _ptr(g_path_w), _ptr(workspace),
                                          workspace.numel(), _stream(stream)))
     return e_edge, gV, gEenv, g_path_w
+
+
+def tp_double_backward(plan, row_ptr, G, V, Eenv, path_w, aV, bE, want_d_path_w=True, stream=None):
+    """second derivative (training): gradients of <aV, gV> + <bE, gEenv> -> (dG, dV, dEenv, d_path_w or None)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    dG, dV, dE = torch.empty_like(V), torch.empty_like(V), torch.empty_like(Eenv)
+    dw = torch.empty((plan.P,), dtype=V.dtype, device=V.device) if want_d_path_w else None
+    ws = _ws(lib().allegro_tp_double_backward_workspace(plan.h, n_atoms, n_edges), V.device)
+    _check(lib().allegro_tp_double_backward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(G), _ptr(V), _ptr(Eenv), _ptr(path_w), _ptr(aV), _ptr(bE),
+                                            _ptr(dG), _ptr(dV), _ptr(dE), _ptr(dw), _ptr(ws), ws.numel(), _stream(stream)))
+    return dG, dV, dE, dw
 
 
 def env_embed_backward(plan, row_ptr, gEenv, rvec, w, scale=1.0, want_g_w=True, g_rvec=None, g_w=None, stream=None):

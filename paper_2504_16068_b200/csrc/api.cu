@@ -345,6 +345,65 @@ allegro_status_t allegro_tp_fused_energy(const allegro_plan_t* plan, int n_atoms
     return ALLEGRO_DISPATCH(plan, launch_tp_fused, a);
 }
 
+// ---- second derivative (training): a composition of the first-derivative and forward kernels, see the header
+namespace {
+struct Dbw { size_t tmp_feat, tmp_env, gw2, bwd, bwd_bytes, total; };
+Dbw dbw_layout(const allegro_plan_t* plan, int N, long E) {
+    const size_t s = plan->dtype == ALLEGRO_F32 ? 4 : 8;
+    const size_t n = plan->n, dV = plan->tab.dV, dE = plan->tab.dE, P = plan->tab.paths.size();
+    Dbw L{};
+    size_t off = 0;
+    auto take = [&](size_t bytes) { const size_t o = off; off += allegro::align_up(bytes ? bytes : 1, 256); return o; };
+    L.tmp_feat = take((size_t)E * n * dV * s); L.tmp_env = take((size_t)N * n * dE * s); L.gw2 = take(P * s);
+    L.bwd_bytes = allegro_tp_backward_workspace(plan, N, E, 0, 1);
+    L.bwd = take(L.bwd_bytes);
+    L.total = off;
+    return L;
+}
+}  // namespace
+
+size_t allegro_tp_double_backward_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges) {
+    if (!plan || n_atoms < 0 || n_edges < 0) return 0;
+    return dbw_layout(plan, n_atoms, n_edges).total;
+}
+
+allegro_status_t allegro_tp_double_backward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const void* G, const void* V,
+                                            const void* Eenv, const void* path_w, const void* aV, const void* bE, void* dG, void* dV, void* dEenv,
+                                            void* d_path_w, void* workspace, size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((G && V && aV && dG && dV) || n_edges == 0, "NULL edge tensor");
+    ALLEGRO_CHECK_ARG((Eenv && bE && dEenv) || n_atoms == 0, "NULL centre tensor");
+    if (plan->wmode != ALLEGRO_W_SCALAR) {
+        set_error("allegro_tp_double_backward: scalar path weights only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    const Dbw L = dbw_layout(plan, n_atoms, n_edges);
+    if (workspace == nullptr || workspace_bytes < L.total || !aligned16(workspace)) {
+        set_error("allegro_tp_double_backward: workspace too small or misaligned (%zu < %zu bytes)", workspace_bytes, L.total);
+        return ALLEGRO_ENOMEM;
+    }
+    if (path_w != nullptr) {       // bind once; the four launches below use the bound table
+        allegro_status_t b = bind_scalar_weights(plan, path_w, (cudaStream_t)stream);
+        if (b != ALLEGRO_OK) return b;
+    }
+    unsigned char* ws = (unsigned char*)workspace;
+    const allegro_dtype_t dt = (allegro_dtype_t)plan->dtype;
+    const long feat = n_edges * plan->n * plan->tab.dV;
+    allegro_status_t r;
+    // dG = fwd(aV, Eenv) + fwd(V, bE)
+    if ((r = allegro_tp_forward(plan, n_atoms, n_edges, row_ptr, nullptr, 0, aV, Eenv, nullptr, dG, stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_tp_forward(plan, n_atoms, n_edges, row_ptr, nullptr, 0, V, bE, nullptr, ws + L.tmp_feat, stream)) != ALLEGRO_OK) return r;
+    if ((r = allegro_add_inplace(feat, dt, dG, ws + L.tmp_feat, stream)) != ALLEGRO_OK) return r;
+    // dEenv = the gEenv output of the first derivative with aV in V's place; its path-weight output is sum C aV Eenv G
+    if ((r = allegro_tp_backward(plan, n_atoms, n_edges, row_ptr, nullptr, 0, G, aV, Eenv, nullptr, nullptr, dEenv, d_path_w, ws + L.bwd, L.bwd_bytes,
+                                 stream)) != ALLEGRO_OK) return r;
+    // dV = the gV output of the first derivative with bE in Eenv's place; its path-weight output is sum C V bE G
+    if ((r = allegro_tp_backward(plan, n_atoms, n_edges, row_ptr, nullptr, 0, G, V, bE, nullptr, dV, ws + L.tmp_env, d_path_w ? ws + L.gw2 : nullptr,
+                                 ws + L.bwd, L.bwd_bytes, stream)) != ALLEGRO_OK) return r;
+    if (d_path_w) return allegro_add_inplace((long)plan->tab.paths.size(), dt, d_path_w, ws + L.gw2, stream);
+    return ALLEGRO_OK;
+}
+
 size_t allegro_tp_backward_workspace(const allegro_plan_t* plan, int n_atoms, long n_edges, long n_items, int want_g_path_w) {
     (void)n_edges;
     if (!plan) return 0;

@@ -847,3 +847,31 @@ def test_gpu_neighbour_list_bit_exact(name):
     assert np.array_equal(nl["col"].cpu().numpy(), g["col"])
     assert np.array_equal(nl["rev"].cpu().numpy(), g["rev"])
     assert np.array_equal(nl["rvec"].cpu().numpy(), g["rvec"].astype(dt))
+
+
+@pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
+def test_tp_double_backward(name):
+    """allegro_tp_double_backward (training, row f2; reading A26) against the oracle's term-by-term second derivative on every
+    single-layer config shape (fp64 l_max 1, fp32 l_max 2 / 3)"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import rng
+    inp = _chain.make_inputs(name)
+    lmax, n, dt, rp = inp["lmax"], inp["n"], inp["dt"], inp["row_ptr"]
+    E, N = inp["E"], inp["N"]
+    dV, dE = 2 * (lmax + 1) ** 2, (lmax + 1) ** 2
+    S = rng.STREAMS
+    V, pw = inp["V"], inp["path_w"]
+    G = rng.normal(21, S["G"], (E, n, dV)).astype(dt)
+    aV = rng.normal(22, S["V"], (E, n, dV)).astype(dt)
+    Ee = (rng.normal(23, S["W_w"], (N, n, dE)) * 0.5).astype(dt)
+    bE = (rng.normal(24, S["W_w"], (N, n, dE)) * 0.5).astype(dt)
+    f8 = lambda a: np.asarray(a, dtype=np.float64)
+    ref = dict(zip(("dG", "dV", "dE", "dw"), orc.tp_double_backward(lmax, rp, f8(G), f8(V), f8(Ee), f8(pw), f8(aV), f8(bE))))
+    plan = ab.Plan(lmax, n, ab.F64 if dt == np.float64 else ab.F32)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    got = dict(zip(("dG", "dV", "dE", "dw"), ab.tp_double_backward(plan, d(rp), d(G), d(V), d(Ee), d(pw), d(aV), d(bE))))
+    torch.cuda.synchronize()
+    _assert_close(ref, got, dt, keys=("dG", "dV", "dE", "dw"), label="double backward " + name)
