@@ -261,14 +261,14 @@ allegro_status_t allegro_tp_forward_energy(const allegro_plan_t* plan, int n_ato
                                            void* out, void* e_edge, void* G, void* stream) {
     ALLEGRO_CHECK_GRAPH();
     ALLEGRO_CHECK_ARG(V || n_edges == 0, "V is NULL");
-    ALLEGRO_CHECK_ARG(out || G, "out and G are both NULL");
+    ALLEGRO_CHECK_ARG(out || G || (plan->wmode == ALLEGRO_W_DENSE && e_edge), "out and G are both NULL");
     ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
     ALLEGRO_CHECK_ARG(q != nullptr, "q is NULL");
     ALLEGRO_CHECK_ARG((V != out && V != G && (out != G || !out)) || n_edges == 0, "out / G alias V or each other");
     ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(out) && aligned16(G) && aligned16(Eenv), "feature tensor not 16-byte aligned");
     ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
-    if (plan->wmode != ALLEGRO_W_SCALAR) {
-        set_error("allegro_tp_forward_energy: scalar path weights only");
+    if (plan->wmode != ALLEGRO_W_SCALAR && !(plan->dtype == ALLEGRO_F32 && plan->l_max == 2 && plan->n == 64 && path_w != nullptr && G == nullptr && e_edge != nullptr)) {
+        set_error("allegro_tp_forward_energy: scalar path weights, or dense weights with fp32, l_max = 2, n = 64, e_edge and no G");
         return ALLEGRO_EUNSUPPORTED;
     }
     TpArgs a{};
@@ -304,7 +304,8 @@ allegro_status_t allegro_tp_backward_energy(const allegro_plan_t* plan, int n_at
                                             double kappa, void* gV, void* gEenv, void* g_path_w, void* workspace, size_t workspace_bytes,
                                             void* stream) {
     ALLEGRO_CHECK_GRAPH();
-    ALLEGRO_CHECK_ARG((out && V) || n_edges == 0, "out / V is NULL");
+    ALLEGRO_CHECK_ARG(V || n_edges == 0, "V is NULL");
+    ALLEGRO_CHECK_ARG(out || n_edges == 0 || (plan->wmode == ALLEGRO_W_DENSE && kappa == 0.0), "out is NULL (allowed in dense mode with kappa == 0 only)");
     ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
     ALLEGRO_CHECK_ARG(q != nullptr, "q is NULL");
     ALLEGRO_CHECK_ARG(gV == nullptr || (gV != out && gV != V), "gV aliases an input");

@@ -44,7 +44,8 @@ static allegro_status_t mix3_fwd_launch(const TpArgs& a, const float* img_f) {
     auto k = mix3_fwd_kernel<PMASK>;
     constexpr int SMEM = Mix3Seq<PMASK>::SMEM;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
-    k<<<(unsigned)a.n_items, Mix3::CT + 64, SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out);
+    k<<<(unsigned)a.n_items, Mix3::CT + 64, SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out,
+                                                          (const float*)a.q, (float)a.kappa, (float*)a.e_edge);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

@@ -114,7 +114,8 @@ struct Mix3Seq {
     static constexpr bool ALIAS_STG = STG_BYTES <= B_BYTES;
     static constexpr int OFF_A = 0, OFF_B = Mix3::NA * Mix3::A_BYTES, OFF_STG = OFF_B + Mix3::NB * B_BYTES;
     static constexpr int OFF_BAR = OFF_STG + (ALIAS_STG ? 0 : STG_BYTES);
-    static constexpr int SMEM = OFF_BAR + 256 + 1024;             // + barrier block + 1024-byte alignment slack
+    static constexpr int OFF_RED = OFF_BAR + 256;                 // [2][4 lane quarters][24 edges] partial edge energies
+    static constexpr int SMEM = OFF_RED + 2 * 4 * Mix3::TE * 4 + 1024;   // + barrier block + energy partials + 1024-byte alignment slack
     static_assert(count() >= 2, "at least two paths");
 };
 
@@ -153,10 +154,14 @@ struct Mix3Bars {
 
 __device__ __forceinline__ float tf32_lo(float x) { return x - __uint_as_float(__float_as_uint(x) & 0xffffe000u); }
 
+// Energy epilogue (e_edge != NULL): e_edge[e] = sum_n' ( q[n'] out[e][n'][0] + kappa/2 sum_k out[e][n'][k]^2 ) of reading A12, formed
+// from the rows while they are in registers; `out` may then be NULL (the rows are never stored: a last layer whose output feeds
+// only the readout).
 template <uint32_t PMASK>
 __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                    const float* __restrict__ V, const float* __restrict__ Eenv,
-                                                                   const float* __restrict__ img, float* __restrict__ out) {
+                                                                   const float* __restrict__ img, float* __restrict__ out,
+                                                                   const float* __restrict__ qvec, float kappa, float* __restrict__ e_edge) {
     using M3 = Mix3;
     using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
@@ -260,6 +265,8 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
             boff[j] = (uint32_t)(ch >> 5) * (uint32_t)SQ::ATOM + (e >> 3) * 1024u + r * 128u + (((((uint32_t)ch & 31u) >> 2) ^ r) << 4) + (((uint32_t)ch & 3u) << 2);
         }
         const int q = warp & 3, wq = warp >> 2, h = lane >> 4, nl = lane & 15;
+        const float qn = e_edge != nullptr ? qvec[16 * q + nl] : 0.f;
+        float* red = reinterpret_cast<float*>(sm + SQ::OFF_RED);
         RingPos<M3::NB> rb;
         for (int t = 0; t < ntiles; ++t) {
             const int eb = e0 + t * TE;
@@ -347,17 +354,38 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
                     __syncwarp();
                     if (lane == 0) mbar_arrive(&bars->d_empty);
                 }
+                if (e_edge != nullptr) {   // energy partial of this lane quarter's 16 channels, per edge: xor tree inside the half-warp
 #pragma unroll
-                for (int i = 0; i < 2; ++i) row_store<float, DV>(stg + ((2 * h + i) * 16 + nl) * DV, o[i]);
-                __syncwarp();
-                const int ebase = eb + 8 * wq + 4 * hf;
+                    for (int i = 0; i < 2; ++i) {
+                        float sq = 0.f;
 #pragma unroll
-                for (int r = 0; r < 9; ++r) {    // 4 edges x 288 floats = 288 float4
-                    const int idx = lane + 32 * r, el = idx / 72, w4 = idx - el * 72;
-                    if (ebase + el < e1)
-                        *reinterpret_cast<float4*>(out + ((size_t)(ebase + el) * 64 + 16 * q) * DV + 4 * w4) = reinterpret_cast<const float4*>(stg)[idx];
+                        for (int k = 0; k < DV; ++k) sq = fmaf(o[i][k], o[i][k], sq);
+                        float ep = fmaf(0.5f * kappa, sq, qn * o[i][0]);
+#pragma unroll
+                        for (int sft = 8; sft > 0; sft >>= 1) ep += __shfl_xor_sync(0xffffffffu, ep, sft);
+                        if (nl == 0) red[((t & 1) * 4 + q) * TE + 8 * wq + 4 * hf + 2 * h + i] = ep;
+                    }
                 }
-                __syncwarp();
+                if (out != nullptr) {
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) row_store<float, DV>(stg + ((2 * h + i) * 16 + nl) * DV, o[i]);
+                    __syncwarp();
+                    const int ebase = eb + 8 * wq + 4 * hf;
+#pragma unroll
+                    for (int r = 0; r < 9; ++r) {    // 4 edges x 288 floats = 288 float4
+                        const int idx = lane + 32 * r, el = idx / 72, w4 = idx - el * 72;
+                        if (ebase + el < e1)
+                            *reinterpret_cast<float4*>(out + ((size_t)(ebase + el) * 64 + 16 * q) * DV + 4 * w4) = reinterpret_cast<const float4*>(stg)[idx];
+                    }
+                    __syncwarp();
+                }
+            }
+            if (e_edge != nullptr) {       // the four lane quarters' partials in order (double-buffered by tile parity)
+                asm volatile("bar.sync 2, %0;" ::"n"(M3::CT) : "memory");
+                if (tid < TE && eb + tid < e1) {
+                    const float* rp4 = red + (t & 1) * 4 * TE + tid;
+                    e_edge[eb + tid] = ((rp4[0] + rp4[TE]) + rp4[2 * TE]) + rp4[3 * TE];
+                }
             }
             if constexpr (SQ::ALIAS_STG) asm volatile("bar.arrive 1, %0;" ::"n"(2 * M3::CT) : "memory");   // staging done; waited for before B stage 1 is rewritten
             MIX3_ACC(9, blockIdx.x == 0 && tid == 0);
@@ -511,11 +539,17 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
                 const int e = eb + 4 * slot + j;
                 float g[DV];
                 if (e < e1) {
-                    row_load<float, DV>(G + ((size_t)e * 64 + np) * DV, g);
-                    if constexpr (COT) {
+                    if (COT && G == nullptr) {       // kappa == 0: the cotangent is q (x) delta_{k,0}, nothing to read
 #pragma unroll
-                        for (int k = 0; k < DV; ++k) g[k] *= kappa;
-                        g[0] += qn;
+                        for (int k = 0; k < DV; ++k) g[k] = 0.f;
+                        g[0] = qn;
+                    } else {
+                        row_load<float, DV>(G + ((size_t)e * 64 + np) * DV, g);
+                        if constexpr (COT) {
+#pragma unroll
+                            for (int k = 0; k < DV; ++k) g[k] *= kappa;
+                            g[0] += qn;
+                        }
                     }
                 } else {
 #pragma unroll

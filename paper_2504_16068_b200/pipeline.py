@@ -325,9 +325,13 @@ class TwoLayerStep:
     `plan_first`: optional dense plan restricted to the natural-parity input blocks (Plan.set_in_blocks(0x19)) for the first
     layer, whose input V0 = v (x) Y has zeros in the other blocks (reading A19): half of the paths never run."""
 
-    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None, sharded=None):
+    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None, sharded=None, fuse_readout=None):
         self.pd, self.ps, self.dev, self.p = plan_dense, plan_scalar, dev, params
         self.sharded = sharded      # sharding.ShardedForces: `dev` holds one rank's rows (see SingleLayerStep)
+        # fuse_readout: the readout E = sum q . V_L[:, :, 0e] is taken in the last layer's forward epilogue and its cotangent formed inside
+        # the last layer's VJP, so V_L is never stored (default: whenever the tcgen05 kernels serve the shape and plan_last is given)
+        tc = plan_dense.dtype == ab.F32 and plan_dense.l_max == 2 and plan_dense.n == 64
+        self.fuse_readout = (tc and plan_last is not None) if fuse_readout is None else (fuse_readout and tc)
         self.pd_last = plan_last if plan_last is not None else plan_dense
         self.pd_first = plan_first if plan_first is not None else plan_dense
         self.L = params["W_w"].shape[0]
@@ -338,7 +342,7 @@ class TwoLayerStep:
         new = lambda *shape: torch.empty(shape, dtype=dt, device=dv)
         self.x = [new(E, n) for _ in range(L)]            # x_0 .. x_{L-1}
         self.z = [new(E, n) for _ in range(L - 1)]
-        self.V = [new(E, n, dV) for _ in range(L + 1)]    # V_0 .. V_L
+        self.V = [new(E, n, dV) for _ in range(L)] + [None if self.fuse_readout else new(E, n, dV)]    # V_0 .. V_L
         self.w = [new(E, n) for _ in range(L)]
         self.Eenv = [new(N, n, plan_dense.dE) for _ in range(L)]
         self.gEenv = new(N, n, plan_dense.dE)
@@ -370,14 +374,19 @@ class TwoLayerStep:
             timed("linear", lambda: ab.linear(self.x[l], p["W_w"][l], y=self.w[l]))
             timed("env_embed", lambda: ab.env_embed(ps, rp, rvec, self.w[l], scale, Eenv=self.Eenv[l]))
             pl = self.pd_last if l == L - 1 else (self.pd_first if l == 0 else pd)
-            timed("tp_forward_dense", lambda: ab.tp_forward(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
+            if l == L - 1 and self.fuse_readout:
+                timed("tp_forward_dense", lambda: ab.tp_forward_energy(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, want_out=False,
+                                                                       want_G=False, e_edge=self.e_edge))
+            else:
+                timed("tp_forward_dense", lambda: ab.tp_forward(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
             if l < L - 1:
                 timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], self.V[l + 1], p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
         # readout E = sum_e sum_n q[n] V_L[e][n][0e]; its cotangent q (x) delta_{k,0} is formed inside the last layer's VJP when
         # that kernel exists (fp32, l_max 2, n 64), otherwise materialised here
         fused_cot = pd.dtype == ab.F32 and pd.l_max == 2 and pd.n == 64
         G = self.V[L] if fused_cot else self.cot[0]
-        timed("edge_energy", lambda: ab.edge_energy(pd, self.V[L], p["q"], 0.0, e_edge=self.e_edge, want_G=not fused_cot, G=None if fused_cot else G))
+        if not self.fuse_readout:
+            timed("edge_energy", lambda: ab.edge_energy(pd, self.V[L], p["q"], 0.0, e_edge=self.e_edge, want_G=not fused_cot, G=None if fused_cot else G))
         g_x_next, have_gr = None, False
         for l in reversed(range(L)):
             g_x = None
