@@ -92,6 +92,10 @@ __device__ __forceinline__ void tma_store_2d(const CUtensorMap* tmap, int c0, in
                  "r"(smem_u32(src_smem))
                  : "memory");
 }
+// ask the L2 to fetch a contiguous range ahead of its use (no completion to wait for; size a multiple of 16 bytes)
+__device__ __forceinline__ void bulk_prefetch_l2(const void* src_gmem, uint32_t bytes) {
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src_gmem), "r"(bytes) : "memory");
+}
 __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
 template <int N>
 __device__ __forceinline__ void bulk_wait_read() {

@@ -272,6 +272,8 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
             const int eb = e0 + t * TE;
             bool stg_busy = t > 0;
             MIX3_T0();
+            if (tid == 0 && eb + TE < e1)     // the next tile's V rows (one contiguous range) are pulled into L2 while this tile computes
+                bulk_prefetch_l2(V + (size_t)(eb + TE) * 64 * DV, (uint32_t)min(TE, e1 - eb - TE) * 64 * DV * 4);
             float Vr[M3::EPS][DV];
 #pragma unroll
             for (int i = 0; i < M3::EPS; ++i) {
@@ -533,6 +535,11 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
         RingPos<MB::ND> rd;
         for (int t = 0; t < ntiles; ++t) {
             const int eb = e0 + t * TE;
+            if (tid == 0 && eb + TE < e1) {   // the next tile's cotangent and V rows are pulled into L2 while this tile computes
+                const uint32_t nb = (uint32_t)min(TE, e1 - eb - TE) * 64 * DV * 4;
+                if (G != nullptr) bulk_prefetch_l2(G + (size_t)(eb + TE) * 64 * DV, nb);
+                bulk_prefetch_l2(V + (size_t)(eb + TE) * 64 * DV, nb);
+            }
             // (a) cotangent tile -> B operands of all six blocks (hi, lo)
 #pragma unroll
             for (int j = 0; j < 4; ++j) {
