@@ -138,6 +138,19 @@ def radial(Wr, rc, rvec):
     return w, dw
 
 
+def radial_typed(Wr, rc_edge, rvec):
+    """radial() with a cutoff radius per edge (per-edge-type cutoffs, reading A27): the pinned orc_radial evaluated on the edges of
+    every distinct cutoff value in turn -> (w [E,n], dwdr [E,n])"""
+    rc_edge = np.asarray(rc_edge, dtype=np.float64)
+    rvec = _f64(rvec)
+    w = np.zeros((rvec.shape[0], np.asarray(Wr).shape[0]))
+    dw = np.zeros_like(w)
+    for rc in np.unique(rc_edge):
+        m = rc_edge == rc
+        w[m], dw[m] = radial(Wr, float(rc), rvec[m])
+    return w, dw
+
+
 def radial_backward(rvec, g_w, dwdr, g_rvec):
     """g_rvec += (sum_n g_w dwdr) rhat, in place; returns g_rvec"""
     rvec, g_w, dwdr = _f64(rvec), _f64(g_w), _f64(dwdr)

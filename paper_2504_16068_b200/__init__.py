@@ -79,9 +79,13 @@ SIGNATURES = {
     "allegro_latent_backward": (C.c_int, [C.c_long, C.c_int, C.c_int, C.c_double, C.c_int, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_add_inplace": (C.c_int, [C.c_long, C.c_int, _vp, _vp, _vp]),
     "allegro_neighbour_workspace": (C.c_size_t, [C.c_int]),
-    "allegro_neighbour_count": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, _vp, C.c_size_t, _vp, C.POINTER(C.c_long)]),
-    "allegro_neighbour_fill": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, C.c_long, _vp, _vp, _vp, C.c_int, _vp,
-                                         C.c_size_t, _vp]),
+    "allegro_neighbour_count": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, C.c_int, _vp, _vp, _vp, C.c_size_t, _vp,
+                                          C.POINTER(C.c_long)]),
+    "allegro_neighbour_fill": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, C.c_int, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp,
+                                         C.c_int, _vp, C.c_size_t, _vp]),
+    "allegro_env_radial_forward_typed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp,
+                                                   C.c_size_t, _vp]),
+    "allegro_env_radial_backward_typed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_measure_fp32_fma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
     "allegro_measure_tf32_mma_peak": (C.c_int, [_vp, C.POINTER(C.c_double)]),
     "allegro_measure_tf32_mma_rate": (C.c_int, [C.c_int, _vp, C.POINTER(C.c_double)]),
@@ -504,9 +508,10 @@ class LayerStepGraph:
             self.h = None
 
 
-def neighbour_list(pos, r_cut, box=None, mol_id=None, dtype=F32, stream=None):
-    """positions (device, float64 [N,3]) -> dict(row_ptr, col, rev, rvec) on the device (allegro_neighbour_count / _fill).
-    box: cubic periodic box edge, or None for an open system (the bounding box is taken from the positions)."""
+def neighbour_list(pos, r_cut, box=None, mol_id=None, dtype=F32, species=None, rc_table=None, stream=None):
+    """positions (device, float64 [N,3]) -> dict(row_ptr, col, rev, rvec[, rc_edge]) on the device (allegro_neighbour_count / _fill).
+    box: cubic periodic box edge, or None for an open system (the bounding box is taken from the positions).
+    species (int32 [N]) + rc_table (float64 [S,S], symmetric, <= r_cut): per-edge-type cutoffs; rc_edge [E] is returned as well."""
     assert pos.dtype == torch.float64 and pos.is_cuda
     N = pos.shape[0]
     ws = torch.empty(max(lib().allegro_neighbour_workspace(N), 16), dtype=torch.uint8, device=pos.device)
@@ -519,15 +524,49 @@ def neighbour_list(pos, r_cut, box=None, mol_id=None, dtype=F32, stream=None):
     phi = None if hi is None else hi.ctypes.data_as(_f64p)
     n_edges = C.c_long(0)
     b = float(box) if box is not None else 0.0
-    _check(lib().allegro_neighbour_count(N, _ptr(pos), b, plo, phi, float(r_cut), _ptr(mol_id), _ptr(row_ptr), _ptr(ws), ws.numel(),
-                                         _stream(stream), C.byref(n_edges)))
+    typed = species is not None and rc_table is not None
+    ns = int(rc_table.shape[0]) if typed else 0
+    _check(lib().allegro_neighbour_count(N, _ptr(pos), b, plo, phi, float(r_cut), _ptr(mol_id), _ptr(species) if typed else None, ns,
+                                         _ptr(rc_table) if typed else None, _ptr(row_ptr), _ptr(ws), ws.numel(), _stream(stream), C.byref(n_edges)))
     E = n_edges.value
     col = torch.empty((E,), dtype=torch.int32, device=pos.device)
     rev = torch.empty((E,), dtype=torch.int32, device=pos.device)
     rvec = torch.empty((E, 3), dtype=torch_dtype(dtype), device=pos.device)
-    _check(lib().allegro_neighbour_fill(N, _ptr(pos), b, plo, phi, float(r_cut), _ptr(mol_id), _ptr(row_ptr), E, _ptr(col), _ptr(rev), _ptr(rvec),
+    rc_edge = torch.empty((E,), dtype=torch_dtype(dtype), device=pos.device) if typed else None
+    _check(lib().allegro_neighbour_fill(N, _ptr(pos), b, plo, phi, float(r_cut), _ptr(mol_id), _ptr(species) if typed else None, ns,
+                                        _ptr(rc_table) if typed else None, _ptr(row_ptr), E, _ptr(col), _ptr(rev), _ptr(rvec), _ptr(rc_edge),
                                         dtype, _ptr(ws), ws.numel(), _stream(stream)))
-    return dict(row_ptr=row_ptr, col=col, rev=rev, rvec=rvec)
+    out = dict(row_ptr=row_ptr, col=col, rev=rev, rvec=rvec)
+    if typed:
+        out["rc_edge"] = rc_edge
+    return out
+
+
+def env_radial_forward_typed(plan, row_ptr, rvec, W_r, rc_edge, scale=1.0, items=None, want_w=False, w=None, Eenv=None, workspace=None, stream=None):
+    """env_radial_forward with a cutoff radius per edge (per-edge-type cutoffs, reading A27) -> (Eenv, w or None)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if Eenv is None:
+        Eenv = torch.empty((n_atoms, plan.n, plan.dE), dtype=rvec.dtype, device=rvec.device)
+    if w is None and want_w:
+        w = torch.empty((n_edges, plan.n), dtype=rvec.dtype, device=rvec.device)
+    if workspace is None:
+        workspace = _ws(env_workspace(plan, n_atoms, items), rvec.device)
+    _check(lib().allegro_env_radial_forward_typed(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(rvec), _ptr(W_r),
+                                                  W_r.shape[1], _ptr(rc_edge), float(scale), _ptr(w), _ptr(Eenv), _ptr(workspace), workspace.numel(),
+                                                  _stream(stream)))
+    return Eenv, w
+
+
+def env_radial_backward_typed(plan, row_ptr, gEenv, rvec, W_r, rc_edge, scale=1.0, want_g_w=False, g_rvec=None, g_w=None, stream=None):
+    """VJP of env_radial_forward_typed -> (g_rvec, g_w or None)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if g_rvec is None:
+        g_rvec = torch.empty_like(rvec)
+    if g_w is None and want_g_w:
+        g_w = torch.empty((n_edges, plan.n), dtype=rvec.dtype, device=rvec.device)
+    _check(lib().allegro_env_radial_backward_typed(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(gEenv), _ptr(rvec), _ptr(W_r), W_r.shape[1],
+                                                   _ptr(rc_edge), float(scale), _ptr(g_rvec), _ptr(g_w), _stream(stream)))
+    return g_rvec, g_w
 
 
 def measure_peaks(stream=None):

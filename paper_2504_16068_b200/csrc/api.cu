@@ -239,6 +239,36 @@ allegro_status_t allegro_env_radial_backward(const allegro_plan_t* plan, int n_a
     return ALLEGRO_DISPATCH(plan, launch_env_embed_backward, a);
 }
 
+allegro_status_t allegro_env_radial_forward_typed(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                                  long n_items, const void* rvec, const void* W_r, int n_basis, const void* rc_edge, double scale,
+                                                  void* w, void* Eenv, void* workspace, size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && rc_edge) || n_edges == 0, "rvec / rc_edge is NULL");
+    ALLEGRO_CHECK_ARG(W_r != nullptr && n_basis >= 1, "W_r is NULL or bad n_basis");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    ALLEGRO_CHECK_ARG(aligned16(Eenv) && aligned16(w), "Eenv / w not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    const size_t need = allegro_env_workspace(plan, n_atoms, items ? n_items : 0);
+    if (items && (workspace == nullptr || workspace_bytes < need)) {
+        set_error("allegro_env_radial_forward_typed: workspace too small (%zu < %zu bytes)", workspace_bytes, need);
+        return ALLEGRO_ENOMEM;
+    }
+    EnvArgs a{plan->n, n_atoms, n_edges, row_ptr, items, items ? n_items : (long)n_atoms, rvec, nullptr, scale, Eenv, workspace,
+              (cudaStream_t)stream, W_r, n_basis, 1.0, w, rc_edge};
+    return ALLEGRO_DISPATCH(plan, launch_env_embed, a);
+}
+
+allegro_status_t allegro_env_radial_backward_typed(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const void* gEenv,
+                                                   const void* rvec, const void* W_r, int n_basis, const void* rc_edge, double scale, void* g_rvec,
+                                                   void* g_w, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && g_rvec && rc_edge) || n_edges == 0, "rvec / g_rvec / rc_edge is NULL");
+    ALLEGRO_CHECK_ARG(W_r != nullptr && n_basis >= 1, "W_r is NULL or bad n_basis");
+    ALLEGRO_CHECK_ARG(gEenv || n_atoms == 0, "gEenv is NULL");
+    EnvBwdArgs a{plan->n, n_atoms, n_edges, row_ptr, gEenv, rvec, nullptr, scale, g_rvec, g_w, (cudaStream_t)stream, W_r, n_basis, 1.0, rc_edge};
+    return ALLEGRO_DISPATCH(plan, launch_env_embed_backward, a);
+}
+
 allegro_status_t allegro_tp_forward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
                                     long n_items, const void* V, const void* Eenv, const void* path_w, void* out, void* stream) {
     ALLEGRO_CHECK_GRAPH();

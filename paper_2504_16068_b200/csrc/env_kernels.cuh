@@ -229,7 +229,7 @@ __device__ __forceinline__ void geo_phase1(GeoSmem<T, L, NB>& sm, int le, const 
 }
 
 template <typename T, int L, int CPL, int NB>
-__global__ void __launch_bounds__(256) env_radial_fwd_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr, const int* __restrict__ items,
+__global__ void __launch_bounds__(256) env_radial_fwd_kernel(int n, int nb, double rc, const T* __restrict__ rc_edge, const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                               const T* __restrict__ rvec, const T* __restrict__ W_r, T scale,
                                                               T* __restrict__ w_out, T* __restrict__ dst, int by_item) {
     constexpr int DE = (L + 1) * (L + 1);
@@ -252,7 +252,7 @@ __global__ void __launch_bounds__(256) env_radial_fwd_kernel(int n, int nb, doub
 
     for (int cb = e0; cb < e1; cb += kGeoChunk) {
         const int cnt = min(kGeoChunk, e1 - cb);
-        if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+        if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc_edge ? (double)rc_edge[(size_t)(cb + tid)] : rc, nb);
         __syncthreads();
         for (int le = warp; le < cnt; le += 8) {
             double Bv[NB];
@@ -293,7 +293,7 @@ __global__ void __launch_bounds__(256) env_radial_fwd_kernel(int n, int nb, doub
 }
 
 template <typename T, int L, int CPL, int NB>
-__global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
+__global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, double rc, const T* __restrict__ rc_edge, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
                                                               const T* __restrict__ rvec, const T* __restrict__ W_r, T scale,
                                                               T* __restrict__ g_rvec, T* __restrict__ g_w) {
     constexpr int DE = (L + 1) * (L + 1);
@@ -317,7 +317,7 @@ __global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, doub
     }
     for (int cb = e0; cb < e1; cb += kGeoChunk) {
         const int cnt = min(kGeoChunk, e1 - cb);
-        if (tid < cnt) geo_phase1<T, L, NB, true>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+        if (tid < cnt) geo_phase1<T, L, NB, true>(sm, tid, rvec, (size_t)(cb + tid), rc_edge ? (double)rc_edge[(size_t)(cb + tid)] : rc, nb);
         __syncthreads();
         for (int le = warp; le < cnt; le += 8) {
             const size_t e = (size_t)(cb + le);
@@ -371,7 +371,7 @@ __global__ void __launch_bounds__(256) env_radial_bwd_kernel(int n, int nb, doub
 //   sum_ch g_w[e][ch] dw[e][ch]/dr = sum_j Y_j(e) sum_b dBu_e[b] M_c[b][j]
 // Per-edge work no longer scales with the channel count (72 FMAs instead of n x 17), and everything is in double.
 template <typename T, int L, int NB>
-__global__ void __launch_bounds__(kGeoChunk) env_radial_fwd_fact_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr,
+__global__ void __launch_bounds__(kGeoChunk) env_radial_fwd_fact_kernel(int n, int nb, double rc, const T* __restrict__ rc_edge, const int* __restrict__ row_ptr,
                                                                          const int* __restrict__ items, const T* __restrict__ rvec,
                                                                          const T* __restrict__ W_r, double scale, T* __restrict__ dst, int by_item) {
     constexpr int DE = (L + 1) * (L + 1);
@@ -387,7 +387,7 @@ __global__ void __launch_bounds__(kGeoChunk) env_radial_fwd_fact_kernel(int n, i
     for (int r = 0; r < R; ++r) sacc[r] = 0.0;
     for (int cb = e0; cb < e1; cb += kGeoChunk) {
         const int cnt = min(kGeoChunk, e1 - cb);
-        if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
+        if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc_edge ? (double)rc_edge[(size_t)(cb + tid)] : rc, nb);
         __syncthreads();
 #pragma unroll
         for (int r = 0; r < R; ++r) {
@@ -413,7 +413,7 @@ __global__ void __launch_bounds__(kGeoChunk) env_radial_fwd_fact_kernel(int n, i
 }
 
 template <typename T, int L, int NB>
-__global__ void __launch_bounds__(kGeoChunk) env_radial_bwd_fact_kernel(int n, int nb, double rc, const int* __restrict__ row_ptr,
+__global__ void __launch_bounds__(kGeoChunk) env_radial_bwd_fact_kernel(int n, int nb, double rc, const T* __restrict__ rc_edge, const int* __restrict__ row_ptr,
                                                                          const T* __restrict__ gEenv, const T* __restrict__ rvec,
                                                                          const T* __restrict__ W_r, double scale, T* __restrict__ g_rvec) {
     constexpr int DE = (L + 1) * (L + 1);
@@ -440,7 +440,7 @@ __global__ void __launch_bounds__(kGeoChunk) env_radial_bwd_fact_kernel(int n, i
         const double dx = (double)rx, dy = (double)ry, dz = (double)rz;
         const double rr = sqrt(dx * dx + dy * dy + dz * dz);
         double Bu[kMaxBasis], dBu[kMaxBasis];
-        radial_basis<true>(rr, rc, nb, Bu, dBu);
+        radial_basis<true>(rr, rc_edge ? (double)rc_edge[e] : rc, nb, Bu, dBu);
         const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
         const T x = rx * inv, y = ry * inv, z = rz * inv;
         T Y[DE], gY[DE];

@@ -33,13 +33,13 @@ allegro_status_t launch_env_embed<ALLEGRO_T, ALLEGRO_L>(const EnvArgs& a) {
             set_error("env_radial_forward: n = %d, n_basis = %d unsupported (n <= 128, n_basis <= %d)", a.n, a.nb, kMaxBasis);
             return ALLEGRO_EUNSUPPORTED;
         }
-        if (a.w_out == nullptr && getenv("ALLEGRO_GEO_UNFACTORISED") == nullptr) {   // w not requested: factorised form
+        if (a.w_out == nullptr) {   // w not requested: factorised form
 #define ALLEGRO_GEOFF(NB)                                                                                                  \
     {                                                                                                                      \
         auto k = env_radial_fwd_fact_kernel<T, ALLEGRO_L, NB>;                                                             \
         const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>) + (size_t)NB * DE * sizeof(double);                          \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
-        k<<<(unsigned)a.n_items, kGeoChunk, smem, a.st>>>(a.n, a.nb, a.rc, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.W_r, \
+        k<<<(unsigned)a.n_items, kGeoChunk, smem, a.st>>>(a.n, a.nb, a.rc, (const T*)a.rc_edge, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.W_r, \
                                                           a.scale, dst, have_items ? 1 : 0);                               \
     }
             if (a.nb <= 8) ALLEGRO_GEOFF(8) else ALLEGRO_GEOFF(16)
@@ -50,7 +50,7 @@ allegro_status_t launch_env_embed<ALLEGRO_T, ALLEGRO_L>(const EnvArgs& a) {
         auto k = env_radial_fwd_kernel<T, ALLEGRO_L, CPL, NB>;                                                             \
         const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>) + (size_t)32 * CPL * DE * sizeof(T);                         \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
-        k<<<(unsigned)a.n_items, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.W_r, \
+        k<<<(unsigned)a.n_items, 256, smem, a.st>>>(a.n, a.nb, a.rc, (const T*)a.rc_edge, a.row_ptr, a.items, (const T*)a.rvec, (const T*)a.W_r, \
                                                     (T)a.scale, (T*)a.w_out, dst, have_items ? 1 : 0);                     \
     }
         if (a.nb <= 8) {
@@ -86,11 +86,11 @@ allegro_status_t launch_env_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EnvBwdArg
             set_error("env_radial_backward: n = %d, n_basis = %d unsupported (n <= 128, n_basis <= %d)", a.n, a.nb, kMaxBasis);
             return ALLEGRO_EUNSUPPORTED;
         }
-        if (a.g_w == nullptr && getenv("ALLEGRO_GEO_UNFACTORISED") == nullptr) {   // g_w not requested: factorised form
+        if (a.g_w == nullptr) {   // g_w not requested: factorised form
             constexpr int DEb = (ALLEGRO_L + 1) * (ALLEGRO_L + 1);
 #define ALLEGRO_GEOBF(NB)                                                                                                  \
     env_radial_bwd_fact_kernel<T, ALLEGRO_L, NB><<<(unsigned)a.n_atoms, kGeoChunk, (size_t)a.n * (DEb + a.nb) * sizeof(T), a.st>>>( \
-        a.n, a.nb, a.rc, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.W_r, a.scale, (T*)a.g_rvec);
+        a.n, a.nb, a.rc, (const T*)a.rc_edge, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.W_r, a.scale, (T*)a.g_rvec);
             if (a.nb <= 8) { ALLEGRO_GEOBF(8) } else { ALLEGRO_GEOBF(16) }
 #undef ALLEGRO_GEOBF
             ALLEGRO_LAUNCHED();
@@ -101,7 +101,7 @@ allegro_status_t launch_env_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EnvBwdArg
         auto k = env_radial_bwd_kernel<T, ALLEGRO_L, CPL, NB>;                                                             \
         const size_t smem = sizeof(GeoSmem<T, ALLEGRO_L, NB>);                                                             \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                      \
-        k<<<(unsigned)a.n_atoms, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec,       \
+        k<<<(unsigned)a.n_atoms, 256, smem, a.st>>>(a.n, a.nb, a.rc, (const T*)a.rc_edge, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec,       \
                                                     (const T*)a.W_r, (T)a.scale, (T*)a.g_rvec, (T*)a.g_w);                 \
     }
         if (a.nb <= 8) {

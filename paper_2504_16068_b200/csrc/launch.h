@@ -29,6 +29,7 @@ struct EnvArgs {
     int nb;
     double rc;
     void* w_out;
+    const void* rc_edge;  // nullable: per-edge cutoff radii T[E] (per-edge-type cutoffs, reading A27); overrides rc
 };
 struct EnvBwdArgs {
     int n, n_atoms;
@@ -45,6 +46,7 @@ struct EnvBwdArgs {
     const void* W_r;
     int nb;
     double rc;
+    const void* rc_edge;  // nullable: per-edge cutoff radii T[E]
 };
 struct TpArgs {
     const allegro_plan* plan;

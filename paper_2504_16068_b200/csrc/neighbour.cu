@@ -19,6 +19,9 @@ struct NbrGrid {
     double box, rc, cell[3], lo[3];
     int nc[3];
     int periodic, brute;
+    const int* species;        // nullable: per-edge-type cutoffs (reading A27)
+    const double* rc_table;    // [n_species][n_species]
+    int n_species;
 };
 
 __device__ __forceinline__ int nbr_cell_of(const NbrGrid& g, const double* __restrict__ p, int d) {
@@ -26,7 +29,11 @@ __device__ __forceinline__ int nbr_cell_of(const NbrGrid& g, const double* __res
     return c < 0 ? 0 : (c >= g.nc[d] ? g.nc[d] - 1 : c);
 }
 
-// edge vector of the ordered pair (a < b) as the host computes it; returns true when 0 < |d| < rc
+__device__ __forceinline__ double nbr_rc(const NbrGrid& g, int a, int b) {
+    return g.species ? g.rc_table[g.species[a] * g.n_species + g.species[b]] : g.rc;
+}
+
+// edge vector of the ordered pair (a < b) as the host computes it; returns true when 0 < |d| < rc (the pair's own cutoff)
 __device__ __forceinline__ bool nbr_pair(const NbrGrid& g, const double* __restrict__ pos, int a, int b, double (&d)[3]) {
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
@@ -36,7 +43,7 @@ __device__ __forceinline__ bool nbr_pair(const NbrGrid& g, const double* __restr
     }
     const double r2 = __dadd_rn(__dadd_rn(__dmul_rn(d[0], d[0]), __dmul_rn(d[1], d[1])), __dmul_rn(d[2], d[2]));
     const double r = __dsqrt_rn(r2);
-    return r > 0.0 && r < g.rc;
+    return r > 0.0 && r < nbr_rc(g, a, b);
 }
 
 __global__ void nbr_cell_kernel(NbrGrid g, int N, const double* __restrict__ pos, int* __restrict__ cell_id, int* __restrict__ cell_cnt) {
@@ -123,7 +130,8 @@ __global__ void nbr_count_kernel(NbrGrid g, int N, const double* __restrict__ po
 
 template <typename T>
 __global__ void nbr_fill_kernel(NbrGrid g, int N, const double* __restrict__ pos, const int* __restrict__ mol_id, const int* __restrict__ cell_start,
-                                const int* __restrict__ sorted, const int* __restrict__ row_ptr, int* __restrict__ col, T* __restrict__ rvec) {
+                                const int* __restrict__ sorted, const int* __restrict__ row_ptr, int* __restrict__ col, T* __restrict__ rvec,
+                                T* __restrict__ rc_edge) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= N) return;
     const int r0 = row_ptr[i], r1 = row_ptr[i + 1];
@@ -146,6 +154,7 @@ __global__ void nbr_fill_kernel(NbrGrid g, int N, const double* __restrict__ pos
         const double sgn = i < j ? 1.0 : -1.0;
 #pragma unroll
         for (int k = 0; k < 3; ++k) rvec[3 * (size_t)e + k] = (T)(sgn * d[k]);
+        if (rc_edge) rc_edge[e] = (T)nbr_rc(g, i, j);
     }
 }
 
@@ -178,8 +187,11 @@ static NbrWs nbr_layout(void* ws, int N, long ncells) {
 static const long kNbrMaxCells = 1L << 21;
 
 // grid geometry from the box (periodic) or from a caller-given bounding box (open)
-static allegro_status_t nbr_grid(int N, double box, double rc, const double* lo, const double* hi, NbrGrid& g) {
+static allegro_status_t nbr_grid(int N, double box, double rc, const double* lo, const double* hi, const int32_t* species, int n_species,
+                                 const double* rc_table, NbrGrid& g) {
     g.box = box; g.rc = rc; g.periodic = box > 0.0 ? 1 : 0; g.brute = 0;
+    g.species = (species && rc_table && n_species > 0) ? species : nullptr;
+    g.rc_table = rc_table; g.n_species = n_species;
     long cells = 1;
     for (int d = 0; d < 3; ++d) {
         const double ext = g.periodic ? box : (hi[d] - lo[d]);
@@ -213,14 +225,14 @@ size_t allegro_neighbour_workspace(int n_atoms) {
 }
 
 allegro_status_t allegro_neighbour_count(int n_atoms, const double* pos, double box, const double* bbox_lo_host, const double* bbox_hi_host, double r_cut,
-                                         const int32_t* mol_id, int32_t* row_ptr, void* workspace, size_t workspace_bytes, void* stream,
-                                         long* n_edges_host) {
+                                         const int32_t* mol_id, const int32_t* species, int n_species, const double* rc_table, int32_t* row_ptr,
+                                         void* workspace, size_t workspace_bytes, void* stream, long* n_edges_host) {
     ALLEGRO_CHECK_ARG(n_atoms >= 0 && r_cut > 0 && row_ptr != nullptr && n_edges_host != nullptr, "bad argument");
     ALLEGRO_CHECK_ARG(pos != nullptr || n_atoms == 0, "pos is NULL");
     ALLEGRO_CHECK_ARG(box > 0.0 || (bbox_lo_host && bbox_hi_host), "open systems need a bounding box");
     cudaStream_t st = (cudaStream_t)stream;
     NbrGrid g;
-    allegro_status_t s = nbr_grid(n_atoms, box, r_cut, bbox_lo_host, bbox_hi_host, g);
+    allegro_status_t s = nbr_grid(n_atoms, box, r_cut, bbox_lo_host, bbox_hi_host, species, n_species, rc_table, g);
     if (s != ALLEGRO_OK) return s;
     const long ncells = (long)g.nc[0] * g.nc[1] * g.nc[2];
     const NbrWs L = nbr_layout(workspace, n_atoms, kNbrMaxCells);
@@ -251,15 +263,16 @@ allegro_status_t allegro_neighbour_count(int n_atoms, const double* pos, double 
 }
 
 allegro_status_t allegro_neighbour_fill(int n_atoms, const double* pos, double box, const double* bbox_lo_host, const double* bbox_hi_host, double r_cut,
-                                        const int32_t* mol_id, const int32_t* row_ptr, long n_edges, int32_t* col, int32_t* rev, void* rvec,
-                                        allegro_dtype_t dtype, void* workspace, size_t workspace_bytes, void* stream) {
+                                        const int32_t* mol_id, const int32_t* species, int n_species, const double* rc_table, const int32_t* row_ptr,
+                                        long n_edges, int32_t* col, int32_t* rev, void* rvec, void* rc_edge, allegro_dtype_t dtype, void* workspace,
+                                        size_t workspace_bytes, void* stream) {
     ALLEGRO_CHECK_ARG(n_atoms >= 0 && r_cut > 0 && row_ptr != nullptr && n_edges >= 0, "bad argument");
     ALLEGRO_CHECK_ARG((col && rev && rvec) || n_edges == 0, "NULL output");
     ALLEGRO_CHECK_ARG(box > 0.0 || (bbox_lo_host && bbox_hi_host), "open systems need a bounding box");
     ALLEGRO_CHECK_ARG(dtype == ALLEGRO_F32 || dtype == ALLEGRO_F64, "bad dtype");
     cudaStream_t st = (cudaStream_t)stream;
     NbrGrid g;
-    allegro_status_t s = nbr_grid(n_atoms, box, r_cut, bbox_lo_host, bbox_hi_host, g);
+    allegro_status_t s = nbr_grid(n_atoms, box, r_cut, bbox_lo_host, bbox_hi_host, species, n_species, rc_table, g);
     if (s != ALLEGRO_OK) return s;
     const NbrWs L = nbr_layout(workspace, n_atoms, kNbrMaxCells);
     if (workspace == nullptr || workspace_bytes < L.total) {
@@ -268,8 +281,8 @@ allegro_status_t allegro_neighbour_fill(int n_atoms, const double* pos, double b
     }
     if (n_atoms == 0 || n_edges == 0) return ALLEGRO_OK;
     const unsigned nb = (unsigned)((n_atoms + 127) / 128);
-    if (dtype == ALLEGRO_F32) nbr_fill_kernel<float><<<nb, 128, 0, st>>>(g, n_atoms, pos, mol_id, L.cell_start, L.sorted, row_ptr, col, (float*)rvec);
-    else nbr_fill_kernel<double><<<nb, 128, 0, st>>>(g, n_atoms, pos, mol_id, L.cell_start, L.sorted, row_ptr, col, (double*)rvec);
+    if (dtype == ALLEGRO_F32) nbr_fill_kernel<float><<<nb, 128, 0, st>>>(g, n_atoms, pos, mol_id, L.cell_start, L.sorted, row_ptr, col, (float*)rvec, (float*)rc_edge);
+    else nbr_fill_kernel<double><<<nb, 128, 0, st>>>(g, n_atoms, pos, mol_id, L.cell_start, L.sorted, row_ptr, col, (double*)rvec, (double*)rc_edge);
     ALLEGRO_LAUNCHED();
     nbr_rev_kernel<<<(unsigned)n_atoms, 64, 0, st>>>(n_atoms, row_ptr, col, rev);
     ALLEGRO_LAUNCHED();

@@ -891,3 +891,49 @@ def test_tp_double_backward(name):
     got = dict(zip(("dG", "dV", "dE", "dw"), ab.tp_double_backward(plan, d(rp), d(G), d(V), d(Ee), d(pw), d(aV), d(bE))))
     torch.cuda.synchronize()
     _assert_close(ref, got, dt, keys=("dG", "dV", "dE", "dw"), label="double backward " + name)
+
+
+def test_per_edge_type_cutoffs():
+    """PAPER.md:156 per-edge-type cutoff radii (reading A27): the GPU neighbour builder with a species table gives the host builder's
+    list and per-edge cutoffs bit for bit; the fused geometry kernels with a cutoff per edge (allegro_env_radial_forward_typed /
+    _backward_typed, factorised and un-factorised forms) match the oracle's radial_typed -> env_embed chain and its VJP"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, geometry, rng
+    g = configs.geometry_for("C1s")
+    pos, box, species = g["pos"], g["box"], g["species"].astype(np.int32)
+    S = int(species.max()) + 1
+    tab = 4.0 + 2.0 * rng.uniform(0, rng.STREAMS["rot"], np.arange(S * S)).reshape(S, S)
+    tab = np.maximum(tab, tab.T)
+    tab[0, 0] = 6.0
+    ref = geometry.neighbour_list_periodic_typed(pos, box, species, tab)
+    dt = np.float32
+    nl = ab.neighbour_list(torch.from_numpy(pos).cuda(), 6.0, box=box, dtype=ab.F32, species=torch.from_numpy(species).cuda(),
+                           rc_table=torch.from_numpy(np.ascontiguousarray(tab)).cuda())
+    torch.cuda.synchronize()
+    for k in ("row_ptr", "col", "rev"):
+        assert np.array_equal(nl[k].cpu().numpy(), ref[k]), k
+    assert np.array_equal(nl["rvec"].cpu().numpy(), ref["rvec"].astype(dt))
+    assert np.array_equal(nl["rc_edge"].cpu().numpy(), ref["rc_edge"].astype(dt))
+    assert ref["row_ptr"][-1] < g["row_ptr"][-1]          # fewer edges than with the single 6 A cutoff
+    # geometry pass with per-edge cutoffs
+    lmax, n = 2, 64
+    rp, rvec, rce = ref["row_ptr"], ref["rvec"].astype(dt), ref["rc_edge"].astype(dt)
+    N = rp.shape[0] - 1
+    Wr = (rng.normal(3, rng.STREAMS["W_r"], (n, 8)) / np.sqrt(8)).astype(dt)
+    gE = rng.normal(3, rng.STREAMS["G"], (N, n, 9)).astype(dt)
+    f8 = lambda a: np.asarray(a, dtype=np.float64)
+    w, dwdr = orc.radial_typed(f8(Wr), f8(rce), f8(rvec))
+    Eenv = orc.env_embed(lmax, rp, f8(rvec), w, 0.7)
+    g_r, g_w = orc.env_embed_backward(lmax, rp, f8(gE), f8(rvec), w, 0.7)
+    orc.radial_backward(f8(rvec), g_w, dwdr, g_r)
+    plan = ab.Plan(lmax, n, ab.F32)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    for want in (False, True):          # factorised form; un-factorised form (w / g_w requested)
+        E2, w2 = ab.env_radial_forward_typed(plan, d(rp), d(rvec), d(Wr), d(rce), 0.7, want_w=want)
+        gr2, gw2 = ab.env_radial_backward_typed(plan, d(rp), d(gE), d(rvec), d(Wr), d(rce), 0.7, want_g_w=want)
+        torch.cuda.synchronize()
+        _assert_close(dict(Eenv=Eenv, w=w, g_r=g_r, g_w=g_w), dict(Eenv=E2, w=w2, g_r=gr2, g_w=gw2), dt, keys=("Eenv", "w", "g_r", "g_w"),
+                      label="typed cutoffs want_w=%s" % want)

@@ -407,3 +407,24 @@ def test_tp_double_backward_is_the_gradient_of_the_vjp(lmax):
     dG0, dV0, dE0, _ = oracle.tp_double_backward(lmax, rp, G, V, Ee, w, aV, np.zeros_like(bE))
     assert np.abs(dV0).max() == 0.0
     assert np.allclose(dG0, oracle.tp_forward(lmax, rp, aV, Ee, w), rtol=0, atol=1e-12 * np.abs(dG0).max())
+
+
+def test_radial_typed_is_radial_per_cutoff_class():
+    """oracle.radial_typed (reading A27: a cutoff radius per edge) is the pinned radial() applied per class of edges: with one class it
+    is radial() itself, with two classes every edge gets the value radial() gives it at its own cutoff, and the envelope vanishes at
+    each edge's own cutoff"""
+    g = _small_graph("C0")
+    rvec = g["rvec"].astype(np.float64)
+    rs = np.random.RandomState(2)
+    Wr = rs.randn(5, 8) / np.sqrt(8)
+    w0, d0 = oracle.radial(Wr, 4.0, rvec)
+    w1, d1 = oracle.radial_typed(Wr, np.full(rvec.shape[0], 4.0), rvec)
+    assert np.array_equal(w0, w1) and np.array_equal(d0, d1)
+    rce = np.where(np.arange(rvec.shape[0]) % 2 == 0, 4.0, 4.5)
+    w2, d2 = oracle.radial_typed(Wr, rce, rvec)
+    wa, da = oracle.radial(Wr, 4.0, rvec)
+    wb, db = oracle.radial(Wr, 4.5, rvec)
+    assert np.array_equal(w2[0::2], wa[0::2]) and np.array_equal(w2[1::2], wb[1::2]) and np.array_equal(d2[1::2], db[1::2])
+    edge = np.array([[0.0, 0.0, 4.5 - 1e-9], [0.0, 4.0 - 1e-9, 0.0]])
+    wz, _ = oracle.radial_typed(Wr, np.array([4.5, 4.0]), edge)
+    assert np.abs(wz).max() < 1e-20

@@ -102,6 +102,21 @@ def neighbour_list_periodic(pos, box, rc):
     return _csr_from_pairs(pos.shape[0], i, j, rvec)
 
 
+def neighbour_list_periodic_typed(pos, box, species, rc_table):
+    """Per-edge-type cutoffs: the pair (i, j) is an edge iff 0 < |r| < rc_table[species[i], species[j]] (symmetric
+    table).  Built from the plain list at the largest cutoff by dropping the edges beyond their own cutoff -> the same dict plus
+    rc_edge[E], the cutoff of every edge."""
+    rc_table = np.asarray(rc_table, dtype=np.float64)
+    full = neighbour_list_periodic(pos, box, float(rc_table.max()))
+    i, j, d = full["centre"].astype(np.int64), full["col"].astype(np.int64), full["rvec"]
+    r = np.sqrt((d * d).sum(1))
+    rce = rc_table[species[i], species[j]]
+    keep = r < rce
+    out = _csr_from_pairs(pos.shape[0], i[keep], j[keep], d[keep])
+    out["rc_edge"] = rc_table[species[out["centre"]], species[out["col"]]]
+    return out
+
+
 def neighbour_list_open(pos, rc, mol_ptr=None):
     """Non-periodic; with mol_ptr, no edges between different molecules."""
     n = pos.shape[0]
