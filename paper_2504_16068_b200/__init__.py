@@ -51,6 +51,8 @@ SIGNATURES = {
     "allegro_tp_double_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
     "allegro_tp_double_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_backward_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_long, C.c_int]),
+    "allegro_tp_backward_static_capacity": (C.c_size_t, []),
+    "allegro_tp_backward_static": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_env_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long]),
     "allegro_env_embed_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_force_gather": (C.c_int, [C.c_int, C.c_long, _vp, _vp, _vp, C.c_int, _vp, _vp]),
@@ -272,6 +274,15 @@ def tp_backward(plan, row_ptr, G, V, Eenv, path_w, items=None, want_gV=True, wan
     _check(lib().allegro_tp_backward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(V),
                                      _ptr(Eenv), _ptr(path_w), _ptr(gV), _ptr(gEenv), _ptr(g_path_w), _ptr(workspace),
                                      workspace.numel(), _stream(stream)))
+    return gV, gEenv, g_path_w
+
+
+def tp_backward_static(plan, row_ptr, G, V, Eenv, path_w, gV, gEenv, g_path_w=None, items=None, stream=None):
+    """allegro_tp_backward_static: the VJP with its scratch in the library's static device array -- no allocation anywhere, so
+    every output tensor is the caller's (gV may be None).  -> (gV, gEenv, g_path_w)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    _check(lib().allegro_tp_backward_static(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(V), _ptr(Eenv),
+                                            _ptr(path_w), _ptr(gV), _ptr(gEenv), _ptr(g_path_w), _stream(stream)))
     return gV, gEenv, g_path_w
 
 
