@@ -42,6 +42,8 @@ SIGNATURES = {
     "allegro_segments_build": (C.c_int, [_i32p, C.c_int, C.c_int, _i32p, C.c_long, C.POINTER(C.c_long)]),
     "allegro_env_embed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_tp_forward_aux": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_tp_backward_aux": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_forward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp]),
     "allegro_tp_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_backward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp,
@@ -242,6 +244,24 @@ def tp_forward(plan, row_ptr, V, Eenv, path_w, items=None, out=None, stream=None
     _check(lib().allegro_tp_forward(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(V), _ptr(Eenv),
                                     _ptr(path_w), _ptr(out), _stream(stream)))
     return out
+
+
+def tp_forward_aux(plan, row_ptr, V, Eenv, path_w, out, out_scalars, items=None, stream=None):
+    """dense tp_forward that also writes the compact 0e scalars out_scalars[e][n] = out[e][n][0]"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    _check(lib().allegro_tp_forward_aux(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(V), _ptr(Eenv), _ptr(path_w),
+                                        _ptr(out), _ptr(out_scalars), _stream(stream)))
+    return out, out_scalars
+
+
+def tp_backward_aux(plan, row_ptr, G, g_scalars, V, Eenv, path_w, gV, gEenv, items=None, workspace=None, stream=None):
+    """dense tp_backward with the cotangent G + g_scalars (x) delta_0e (g_scalars [E, n] compact, may be None)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, V.shape[0]
+    if workspace is None:
+        workspace = _ws(tp_backward_workspace(plan, n_atoms, n_edges, items, False), V.device)
+    _check(lib().allegro_tp_backward_aux(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(g_scalars), _ptr(V),
+                                         _ptr(Eenv), _ptr(path_w), _ptr(gV), _ptr(gEenv), _ptr(workspace), workspace.numel(), _stream(stream)))
+    return gV, gEenv
 
 
 def tp_forward_energy(plan, row_ptr, V, Eenv, path_w, q, kappa, items=None, want_out=True, want_e=True, want_G=True, out=None, e_edge=None,

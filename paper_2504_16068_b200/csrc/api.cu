@@ -286,6 +286,55 @@ allegro_status_t allegro_tp_forward(const allegro_plan_t* plan, int n_atoms, lon
     return ALLEGRO_DISPATCH(plan, launch_tp_forward, a);
 }
 
+// tensor-core dense kernels exist for this shape only (inst_mix3.cu)
+static bool dense_tc_shape(const allegro_plan_t* plan) {
+    return plan->wmode == ALLEGRO_W_DENSE && plan->dtype == ALLEGRO_F32 && plan->l_max == 2 && plan->n == 64;
+}
+
+allegro_status_t allegro_tp_forward_aux(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                        long n_items, const void* V, const void* Eenv, const void* path_w, void* out, void* out_scalars,
+                                        void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((V && out) || n_edges == 0, "V / out is NULL");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr && aligned16(path_w), "path_w is NULL or not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(V != out || n_edges == 0, "out aliases V");
+    ALLEGRO_CHECK_ARG(aligned16(V) && aligned16(out) && aligned16(Eenv), "feature tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (!dense_tc_shape(plan)) {
+        set_error("allegro_tp_forward_aux: dense weights with fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.out = out; a.scalars_out = out_scalars; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_forward, a);
+}
+
+allegro_status_t allegro_tp_backward_aux(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                         long n_items, const void* G, const void* g_scalars, const void* V, const void* Eenv, const void* path_w,
+                                         void* gV, void* gEenv, void* workspace, size_t workspace_bytes, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((G && V) || n_edges == 0, "G / V is NULL");
+    ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr && aligned16(path_w), "path_w is NULL or not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(gV == nullptr || (gV != G && gV != V), "gV aliases an input");
+    ALLEGRO_CHECK_ARG(aligned16(G) && aligned16(V) && aligned16(gV) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace),
+                      "tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (!dense_tc_shape(plan)) {
+        set_error("allegro_tp_backward_aux: dense weights with fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.G = G; a.g_scalars = g_scalars; a.V = V; a.Eenv = Eenv; a.path_w = path_w; a.gV = gV; a.gEenv = gEenv;
+    a.ws = workspace; a.ws_bytes = workspace_bytes; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
+}
+
 allegro_status_t allegro_tp_forward_energy(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
                                            long n_items, const void* V, const void* Eenv, const void* path_w, const void* q, double kappa,
                                            void* out, void* e_edge, void* G, void* stream) {

@@ -45,7 +45,7 @@ static allegro_status_t mix3_fwd_launch(const TpArgs& a, const float* img_f) {
     constexpr int SMEM = Mix3Seq<PMASK>::SMEM;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
     k<<<(unsigned)a.n_items, Mix3::CT + 64, SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out,
-                                                          (const float*)a.q, (float)a.kappa, (float*)a.e_edge);
+                                                          (const float*)a.q, (float)a.kappa, (float*)a.e_edge, (float*)a.scalars_out);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -65,7 +65,7 @@ static allegro_status_t mix3_bwd_launch(const TpArgs& a, const float* img_b, flo
     auto k = mix3_bwd_kernel<GV, PMASK, COT>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
     k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv, img_b,
-                                                                (float*)a.gV, gE_dst, gE_by_item, (const float*)a.q, (float)a.kappa);
+                                                                (float*)a.gV, gE_dst, gE_by_item, (const float*)a.q, (float)a.kappa, (const float*)a.g_scalars);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

@@ -72,6 +72,9 @@ struct TpArgs {
     void* ws;
     size_t ws_bytes;
     cudaStream_t st;
+    // dense mode, fp32 / l_max 2 / n 64 only (allegro_tp_forward_aux / _backward_aux): compact side channel of the 0e scalars
+    void* scalars_out;      // forward: T[E][n] copy of out[:, :, 0e]
+    const void* g_scalars;  // backward: T[E][n] added to G[:, :, 0e]
 };
 
 struct EmbedArgs {

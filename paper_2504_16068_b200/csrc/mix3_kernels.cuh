@@ -156,12 +156,14 @@ __device__ __forceinline__ float tf32_lo(float x) { return x - __uint_as_float(_
 
 // Energy epilogue (e_edge != NULL): e_edge[e] = sum_n' ( q[n'] out[e][n'][0] + kappa/2 sum_k out[e][n'][k]^2 ) of reading A12, formed
 // from the rows while they are in registers; `out` may then be NULL (the rows are never stored: a last layer whose output feeds
-// only the readout).
+// only the readout).  s_out (nullable, [E][64]): compact copy of the 0e scalars out[e][n'][0], what a scalar latent update reads
+// (as a 72-byte-strided gather from `out` it costs 8 x the sectors).
 template <uint32_t PMASK>
 __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                    const float* __restrict__ V, const float* __restrict__ Eenv,
                                                                    const float* __restrict__ img, float* __restrict__ out,
-                                                                   const float* __restrict__ qvec, float kappa, float* __restrict__ e_edge) {
+                                                                   const float* __restrict__ qvec, float kappa, float* __restrict__ e_edge,
+                                                                   float* __restrict__ s_out) {
     using M3 = Mix3;
     using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
@@ -368,6 +370,13 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
                         if (nl == 0) red[((t & 1) * 4 + q) * TE + 8 * wq + 4 * hf + 2 * h + i] = ep;
                     }
                 }
+                if (s_out != nullptr) {
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        const int e = eb + 8 * wq + 4 * hf + 2 * h + i;
+                        if (e < e1) s_out[(size_t)e * 64 + 16 * q + nl] = o[i][0];
+                    }
+                }
                 if (out != nullptr) {
 #pragma unroll
                     for (int i = 0; i < 2; ++i) row_store<float, DV>(stg + ((2 * h + i) * 16 + nl) * DV, o[i]);
@@ -433,13 +442,14 @@ struct Mix3BBars {
 };
 
 // COT: G points at the forward result `out` and the cotangent of the A12 energy, q (x) delta_{k,0} + kappa out, is formed while the
-// tile is staged (G never exists in HBM).
+// tile is staged (G never exists in HBM).  g_s (nullable, [E][64]): a compact cotangent of the 0e scalars that is ADDED to
+// G[e][n'][0] while the tile is staged (the scalar latent update's VJP writes it; G itself is not modified).
 template <bool WANT_GV, uint32_t PMASK, bool COT>
 __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                     const float* __restrict__ G, const float* __restrict__ V,
                                                                     const float* __restrict__ Eenv, const float* __restrict__ img,
                                                                     float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item,
-                                                                    const float* __restrict__ qvec, float kappa) {
+                                                                    const float* __restrict__ qvec, float kappa, const float* __restrict__ g_s) {
     using MB = Mix3B;
     using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
@@ -558,6 +568,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
                             g[0] += qn;
                         }
                     }
+                    if (g_s != nullptr) g[0] += g_s[(size_t)e * 64 + np];
                 } else {
 #pragma unroll
                     for (int k = 0; k < DV; ++k) g[k] = 0.f;

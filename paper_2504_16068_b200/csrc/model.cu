@@ -1,7 +1,7 @@
 // model.cu -- dtype-only pieces of the two-layer model of BASELINE.json:configs[2] (reading A19) that are not part
 // of the tensor-product hot path: the per-edge linear maps (w = W_w x and its transpose), the scalar latent update
 // x' = u(r/r_c) SiLU(A [x ; V[:,0e]]) with its VJP, and an in-place add.  Small-K GEMMs ([E x 64] x [64 x 64..128]) in the
-// method's own precision (fp32 / fp64 FMA): register-tiled, both operands K-major in shared memory.
+// method's own precision (fp32 / fp64 FMA): register-tiled, operands in shared memory.
 #include "common.cuh"
 #include "launch.h"
 
@@ -9,44 +9,75 @@ namespace allegro {
 
 // ---------------------------------------------------------------------------------------------- register-tiled small GEMM
 // All three maps are [E x K] . [K x n_out] products with K, n_out in {64, 128}: HBM-light, FMA-heavy.  One CTA (256 threads) owns
-// a tile of TILE_E = 128 edges and walks the outputs in chunks of 64; thread (ty, tx) = (tid / 16, tid % 16) accumulates 8 edges
-// (8 ty .. 8 ty + 7) x 4 outputs (4 tx .. 4 tx + 3) in registers.  Both operands sit in shared memory K-major -- xs[k][128 edges],
-// Ws[k][64 outputs] -- so one k step is two 128-bit loads of x (a broadcast inside each half-warp), one of W and 32 FMAs.
+// a tile of kTileE = 128 edges and walks the outputs in chunks of 64; thread (ty, tx) = (tid / 16, tid % 16) accumulates 8 edges
+// (ty + 16 i) x 4 outputs (4 tx .. 4 tx + 3) in registers.  The x tile sits in shared memory ROW-major, xs[edge][Kp + VEC] (Kp = K
+// rounded up to the 16-byte vector width VEC, the pad columns zero): global rows are read with lanes running along K (fully
+// coalesced, conflict-free stores), and the multiply loop reads one 16-byte vector of VEC consecutive k per edge -- the two
+// edges of a warp are adjacent rows, Kp + VEC words apart, so their vectors fall into different banks, and the 16 tx lanes
+// share the address (broadcast).  W sits K-major, Ws[k][64 outputs].  One step of VEC k's: 8 + VEC vector loads, 32 VEC FMAs.
 constexpr int kTileE = 128, kTileO = 64;
 
+template <typename T> struct TileVec { static constexpr int N = 16 / (int)sizeof(T); };
+__host__ __device__ static inline int tile_kp(int K, int vec) { return (K + vec - 1) / vec * vec; }
+
 template <typename T>
-__device__ __forceinline__ void tile_mac(const T* __restrict__ xs, const T* __restrict__ Ws, int K, int ty, int tx, T (&acc)[8][4]) {
-#pragma unroll 4
-    for (int k = 0; k < K; ++k) {
-        T xv[8], wv[4];
+__device__ __forceinline__ void tile_mac(const T* __restrict__ xs, const T* __restrict__ Ws, int Kp, int ty, int tx, T (&acc)[8][4]) {
+    constexpr int VEC = TileVec<T>::N;
+    constexpr int WV = 4 / VEC;                       // 16-byte vectors per 4 outputs: 1 (float) or 2 (double)
+    const int ld = Kp + VEC;
+    for (int k = 0; k < Kp; k += VEC) {
+        T xv[8][VEC], wv[VEC][4];
 #pragma unroll
-        for (int i = 0; i < 8; ++i) xv[i] = xs[k * kTileE + 8 * ty + i];
+        for (int i = 0; i < 8; ++i) {
+            const int4 v = *reinterpret_cast<const int4*>(xs + (size_t)(ty + 16 * i) * ld + k);
+            const T* sv = reinterpret_cast<const T*>(&v);
 #pragma unroll
-        for (int j = 0; j < 4; ++j) wv[j] = Ws[k * kTileO + 4 * tx + j];
+            for (int q = 0; q < VEC; ++q) xv[i][q] = sv[q];
+        }
 #pragma unroll
-        for (int i = 0; i < 8; ++i)
+        for (int q = 0; q < VEC; ++q) {
+            const T* wrow = Ws + (size_t)(k + q) * kTileO + 4 * tx;
 #pragma unroll
-            for (int j = 0; j < 4; ++j) acc[i][j] = fma(xv[i], wv[j], acc[i][j]);
+            for (int h = 0; h < WV; ++h) {
+                const int4 v = *reinterpret_cast<const int4*>(wrow + h * VEC);
+                const T* sv = reinterpret_cast<const T*>(&v);
+#pragma unroll
+                for (int jj = 0; jj < VEC; ++jj) wv[q][h * VEC + jj] = sv[jj];
+            }
+        }
+#pragma unroll
+        for (int q = 0; q < VEC; ++q)
+#pragma unroll
+            for (int i = 0; i < 8; ++i)
+#pragma unroll
+                for (int jj = 0; jj < 4; ++jj) acc[i][jj] = fma(xv[i][q], wv[q][jj], acc[i][jj]);
     }
 }
-// Ws[k][o] = W[o0 + o][k] (transpose_w == 0, W [n_out][ldw = K]) or W[k][o0 + o] (transpose_w == 1, W [K][ldw = n_out]); columns beyond
-// n_out are zero
+// Ws[k][o] = W[o0 + o][k] (transpose_w == 0, W [n_out][K]) or W[k][o0 + o] (transpose_w == 1, W [K][n_out]); rows k >= K and columns
+// beyond n_out are zero
 template <typename T>
-__device__ __forceinline__ void tile_load_w(T* __restrict__ Ws, const T* __restrict__ W, int K, int n_out, int o0, int transpose_w, int tid) {
-    for (int idx = tid; idx < K * kTileO; idx += 256) {
+__device__ __forceinline__ void tile_load_w(T* __restrict__ Ws, const T* __restrict__ W, int K, int Kp, int n_out, int o0, int transpose_w, int tid) {
+    for (int idx = tid; idx < Kp * kTileO; idx += 256) {
         int k, o;
-        if (transpose_w) { k = idx / kTileO; o = idx - k * kTileO; } else { o = idx / K; k = idx - o * K; }
+        if (transpose_w) { k = idx / kTileO; o = idx - k * kTileO; } else { o = idx / Kp; k = idx - o * Kp; }
         const int og = o0 + o;
-        Ws[k * kTileO + o] = og < n_out ? (transpose_w ? W[(size_t)k * n_out + og] : W[(size_t)og * K + k]) : T(0);
+        Ws[k * kTileO + o] = (og < n_out && k < K) ? (transpose_w ? W[(size_t)k * n_out + og] : W[(size_t)og * K + k]) : T(0);
     }
 }
-// xs[k][le] = x[eb + le][k] for k < K (rows beyond E are zero): lanes run over edges, so the shared-memory writes are conflict-free
+// xs[le][k0 + k] = x[(eb + le) * ldx + k * kstride] for k < K (rows beyond E are zero): lanes run along k
 template <typename T>
-__device__ __forceinline__ void tile_load_x(T* __restrict__ xs, const T* __restrict__ x, long E, long eb, int K, int k0, int ldx, int kstride, int tid) {
+__device__ __forceinline__ void tile_load_x(T* __restrict__ xs, int ld, const T* __restrict__ x, long E, long eb, int K, int k0, size_t ldx, int kstride,
+                                            int tid) {
     for (int idx = tid; idx < K * kTileE; idx += 256) {
-        const int k = idx / kTileE, le = idx - k * kTileE;
-        xs[(k0 + k) * kTileE + le] = eb + le < E ? x[(size_t)(eb + le) * ldx + (size_t)k * kstride] : T(0);
+        const int le = idx / K, k = idx - le * K;
+        xs[(size_t)le * ld + k0 + k] = eb + le < E ? x[(size_t)(eb + le) * ldx + (size_t)k * kstride] : T(0);
     }
+}
+// zero the pad columns [K, ld) of every row (once per CTA: the tile loads never touch them)
+template <typename T>
+__device__ __forceinline__ void tile_zero_pad(T* __restrict__ xs, int ld, int K, int tid) {
+    const int w = ld - K;
+    for (int idx = tid; idx < w * kTileE; idx += 256) xs[(size_t)(idx / w) * ld + K + idx % w] = T(0);
 }
 
 // y[e][o] (+)= sum_i x[e][i] Wm[o][i]            (transpose_w == 0, Wm = W [n_out][n_in])
@@ -54,18 +85,21 @@ __device__ __forceinline__ void tile_load_x(T* __restrict__ xs, const T* __restr
 template <typename T>
 __global__ void __launch_bounds__(256) linear_kernel(long E, int n_out, int n_in, const T* __restrict__ x, const T* __restrict__ W, int transpose_w,
                                                       int accumulate, T* __restrict__ y) {
+    constexpr int VEC = TileVec<T>::N;
     extern __shared__ __align__(16) unsigned char lin_raw[];
-    T* xs = reinterpret_cast<T*>(lin_raw);            // [n_in][128]
-    T* Ws = xs + (size_t)n_in * kTileE;               // [n_in][64]
+    const int Kp = tile_kp(n_in, VEC), ld = Kp + VEC;
+    T* xs = reinterpret_cast<T*>(lin_raw);            // [128][ld]
+    T* Ws = xs + (size_t)kTileE * ld;                 // [Kp][64]
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int nchunk = (n_out + kTileO - 1) / kTileO;
+    tile_zero_pad<T>(xs, ld, n_in, tid);
     for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
-        tile_load_x<T>(xs, x, E, eb, n_in, 0, n_in, 1, tid);
+        tile_load_x<T>(xs, ld, x, E, eb, n_in, 0, (size_t)n_in, 1, tid);
         for (int c = 0; c < nchunk; ++c) {
             if (c > 0 || nchunk > 1 || eb == (long)blockIdx.x * kTileE) {   // one output chunk: W stays resident over the tiles
                 __syncthreads();
-                tile_load_w<T>(Ws, W, n_in, n_out, c * kTileO, transpose_w, tid);
+                tile_load_w<T>(Ws, W, n_in, Kp, n_out, c * kTileO, transpose_w, tid);
             }
             __syncthreads();
             T acc[8][4];
@@ -73,10 +107,10 @@ __global__ void __launch_bounds__(256) linear_kernel(long E, int n_out, int n_in
             for (int i = 0; i < 8; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) acc[i][j] = T(0);
-            tile_mac<T>(xs, Ws, n_in, ty, tx, acc);
+            tile_mac<T>(xs, Ws, Kp, ty, tx, acc);
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const long e = eb + 8 * ty + i;
+                const long e = eb + ty + 16 * i;
                 if (e >= E) continue;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
@@ -105,16 +139,18 @@ template <typename T>
 __global__ void __launch_bounds__(256) latent_fwd_kernel(long E, int n, int dV, T rc, const T* __restrict__ rvec, const T* __restrict__ x,
                                                           const T* __restrict__ V, const T* __restrict__ A, T* __restrict__ z, T* __restrict__ x_new) {
     extern __shared__ __align__(16) unsigned char lin_raw[];
-    const int K = 2 * n;
-    T* xs = reinterpret_cast<T*>(lin_raw);            // [2n][128]: rows 0..n-1 = x, rows n..2n-1 = V[:, :, 0]
-    T* Ws = xs + (size_t)K * kTileE;                  // [2n][64]
-    T* us = Ws + (size_t)K * kTileO;                  // [128] cutoff u(|r|/rc)
+    constexpr int VEC = TileVec<T>::N;
+    const int K = 2 * n, Kp = tile_kp(K, VEC), ld = Kp + VEC;
+    T* xs = reinterpret_cast<T*>(lin_raw);            // [128][ld]: columns 0..n-1 = x, n..2n-1 = V[:, :, 0]
+    T* Ws = xs + (size_t)kTileE * ld;                 // [Kp][64]
+    T* us = Ws + (size_t)Kp * kTileO;                 // [128] cutoff u(|r|/rc)
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int nchunk = (n + kTileO - 1) / kTileO;
+    tile_zero_pad<T>(xs, ld, K, tid);
     for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
-        tile_load_x<T>(xs, x, E, eb, n, 0, n, 1, tid);
-        tile_load_x<T>(xs, V, E, eb, n, n, n * dV, dV, tid);   // V[e][k][0]
+        tile_load_x<T>(xs, ld, x, E, eb, n, 0, (size_t)n, 1, tid);
+        tile_load_x<T>(xs, ld, V, E, eb, n, n, (size_t)n * dV, dV, tid);   // V[e][k][0]
         if (tid < kTileE) {
             const long e = eb + tid;
             T du, u = T(0);
@@ -127,7 +163,7 @@ __global__ void __launch_bounds__(256) latent_fwd_kernel(long E, int n, int dV, 
         for (int c = 0; c < nchunk; ++c) {
             if (c > 0 || nchunk > 1 || eb == (long)blockIdx.x * kTileE) {
                 __syncthreads();
-                tile_load_w<T>(Ws, A, K, n, c * kTileO, 0, tid);
+                tile_load_w<T>(Ws, A, K, Kp, n, c * kTileO, 0, tid);
             }
             __syncthreads();
             T acc[8][4];
@@ -135,12 +171,12 @@ __global__ void __launch_bounds__(256) latent_fwd_kernel(long E, int n, int dV, 
             for (int i = 0; i < 8; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) acc[i][j] = T(0);
-            tile_mac<T>(xs, Ws, K, ty, tx, acc);
+            tile_mac<T>(xs, Ws, Kp, ty, tx, acc);
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const long e = eb + 8 * ty + i;
+                const long e = eb + ty + 16 * i;
                 if (e >= E) continue;
-                const T u = us[8 * ty + i];
+                const T u = us[ty + 16 * i];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
                     const int o = c * kTileO + 4 * tx + j;
@@ -162,13 +198,16 @@ __global__ void __launch_bounds__(256) latent_bwd_kernel(long E, int n, int dV, 
                                                           const T* __restrict__ g_xnew, const T* __restrict__ A, T* __restrict__ g_x,
                                                           T* __restrict__ gV, T* __restrict__ g_rvec) {
     extern __shared__ __align__(16) unsigned char lin_raw[];
-    T* xs = reinterpret_cast<T*>(lin_raw);            // [n][128]: g_z, K-major (K = the n outputs of the forward map)
-    T* Ws = xs + (size_t)n * kTileE;                  // [n][64]: A[o][chunk of the 2n inputs]
-    T* us = Ws + (size_t)n * kTileO;                  // [128] u, [128] u'/rc/|r|, [2][128] partial radial sums
+    constexpr int VEC = TileVec<T>::N;
+    const int Kp = tile_kp(n, VEC), ld = Kp + VEC, ld2 = n + 1;
+    T* xs = reinterpret_cast<T*>(lin_raw);            // [128][ld]: g_z, row-major (K = the n outputs of the forward map)
+    T* Ws = xs + (size_t)kTileE * ld;                 // [Kp][64]: A[o][chunk of the 2n inputs]
+    T* ss = Ws + (size_t)Kp * kTileO;                 // [128][n + 1]: g_xnew SiLU(z), summed over o per edge for the radial term
+    T* us = ss + (size_t)kTileE * ld2;                // [128] u, [128] u'/rc/|r|
     T* dus = us + kTileE;
-    T* rs = dus + kTileE;
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int nchunk = (2 * n + kTileO - 1) / kTileO;
+    tile_zero_pad<T>(xs, ld, n, tid);
     for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
         if (tid < kTileE) {
@@ -183,35 +222,33 @@ __global__ void __launch_bounds__(256) latent_bwd_kernel(long E, int n, int dV, 
             dus[tid] = du / rc / r;
         }
         __syncthreads();
-        {   // g_z = g_xnew u SiLU'(z) -> xs[o][le]; this thread's edge le = tid % 128 is the same in every iteration
-            const int le = tid & (kTileE - 1);
+        // g_z = g_xnew u SiLU'(z) -> xs[le][o], g_xnew SiLU(z) -> ss[le][o]; lanes run along o (coalesced)
+        for (int idx = tid; idx < n * kTileE; idx += 256) {
+            const int le = idx / n, o = idx - le * n;
             const long e = eb + le;
-            T part = T(0);
-            for (int o = tid >> 7; o < n; o += 2) {
-                T gzv = T(0);
-                if (e < E) {
-                    const T zz = z[(size_t)e * n + o], g = g_xnew[(size_t)e * n + o];
-                    const T sg = T(1) / (T(1) + exp(-zz));
-                    gzv = g * us[le] * (sg * (T(1) + zz * (T(1) - sg)));
-                    part += g * zz * sg;
-                }
-                xs[o * kTileE + le] = gzv;
+            T gzv = T(0), sv = T(0);
+            if (e < E) {
+                const T zz = z[(size_t)e * n + o], g = g_xnew[(size_t)e * n + o];
+                const T sg = T(1) / (T(1) + exp(-zz));
+                gzv = g * us[le] * (sg * (T(1) + zz * (T(1) - sg)));
+                sv = g * zz * sg;
             }
-            rs[(tid >> 7) * kTileE + le] = part;
+            xs[(size_t)le * ld + o] = gzv;
+            ss[(size_t)le * ld2 + o] = sv;
         }
         for (int c = 0; c < nchunk; ++c) {
             __syncthreads();
-            tile_load_w<T>(Ws, A, n, 2 * n, c * kTileO, 1, tid);
+            tile_load_w<T>(Ws, A, n, Kp, 2 * n, c * kTileO, 1, tid);
             __syncthreads();
             T acc[8][4];
 #pragma unroll
             for (int i = 0; i < 8; ++i)
 #pragma unroll
                 for (int j = 0; j < 4; ++j) acc[i][j] = T(0);
-            tile_mac<T>(xs, Ws, n, ty, tx, acc);
+            tile_mac<T>(xs, Ws, Kp, ty, tx, acc);
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
-                const long e = eb + 8 * ty + i;
+                const long e = eb + ty + 16 * i;
                 if (e >= E) continue;
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
@@ -221,9 +258,11 @@ __global__ void __launch_bounds__(256) latent_bwd_kernel(long E, int n, int dV, 
                 }
             }
         }
-        if (tid < kTileE && eb + tid < E) {   // radial term: rs was written before the first barrier of the chunk loop
+        if (tid < kTileE && eb + tid < E) {   // radial term: ss was written before the first barrier of the chunk loop; o in order
             const long e = eb + tid;
-            const T sc = (rs[tid] + rs[kTileE + tid]) * dus[tid];
+            T tot = T(0);
+            for (int o = 0; o < n; ++o) tot += ss[(size_t)tid * ld2 + o];
+            const T sc = tot * dus[tid];
             g_rvec[3 * e] += sc * rvec[3 * e];
             g_rvec[3 * e + 1] += sc * rvec[3 * e + 1];
             g_rvec[3 * e + 2] += sc * rvec[3 * e + 2];
@@ -246,7 +285,8 @@ template <typename T>
 allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st) {
     if (n_out > 1024 || n_in > 256) { set_error("linear: n_out = %d, n_in = %d unsupported (<= 1024, <= 256)", n_out, n_in); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
-    const size_t smem = (size_t)n_in * (kTileE + kTileO) * sizeof(T);
+    const int vec = TileVec<T>::N, Kp = tile_kp(n_in, vec);
+    const size_t smem = ((size_t)kTileE * (Kp + vec) + (size_t)Kp * kTileO) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(linear_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     linear_kernel<T><<<model_grid(E), 256, smem, st>>>(E, n_out, n_in, (const T*)x, (const T*)W, transpose_w, accumulate, (T*)y);
     ALLEGRO_LAUNCHED();
@@ -257,7 +297,8 @@ allegro_status_t launch_latent_forward(long E, int n, int dV, double rc, const v
                                        void* x_new, cudaStream_t st) {
     if (n > 128 || n < 1) { set_error("latent_forward: n = %d unsupported (1 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
-    const size_t smem = ((size_t)2 * n * (kTileE + kTileO) + kTileE) * sizeof(T);
+    const int vec = TileVec<T>::N, Kp = tile_kp(2 * n, vec);
+    const size_t smem = ((size_t)kTileE * (Kp + vec) + (size_t)Kp * kTileO + kTileE) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(latent_fwd_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     latent_fwd_kernel<T><<<model_grid(E), 256, smem, st>>>(E, n, dV, (T)rc, (const T*)rvec, (const T*)x, (const T*)V, (const T*)A, (T*)z, (T*)x_new);
     ALLEGRO_LAUNCHED();
@@ -266,9 +307,10 @@ allegro_status_t launch_latent_forward(long E, int n, int dV, double rc, const v
 template <typename T>
 allegro_status_t launch_latent_backward(long E, int n, int dV, double rc, const void* rvec, const void* z, const void* g_xnew, const void* A,
                                         void* g_x, void* gV, void* g_rvec, cudaStream_t st) {
-    if (n > 256 || n < 1) { set_error("latent_backward: n = %d unsupported (1 <= n <= 256)", n); return ALLEGRO_EUNSUPPORTED; }
+    if (n > 128 || n < 1) { set_error("latent_backward: n = %d unsupported (1 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
-    const size_t smem = ((size_t)n * (kTileE + kTileO) + 4 * kTileE) * sizeof(T);
+    const int vec = TileVec<T>::N, Kp = tile_kp(n, vec);
+    const size_t smem = ((size_t)kTileE * (Kp + vec) + (size_t)Kp * kTileO + (size_t)kTileE * (n + 1) + 2 * kTileE) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(latent_bwd_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     latent_bwd_kernel<T><<<model_grid(E), 256, smem, st>>>(E, n, dV, (T)rc, (const T*)rvec, (const T*)z, (const T*)g_xnew, (const T*)A, (T*)g_x,
                                                           (T*)gV, (T*)g_rvec);

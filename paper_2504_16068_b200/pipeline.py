@@ -332,6 +332,7 @@ class TwoLayerStep:
         # the last layer's VJP, so V_L is never stored (default: whenever the tcgen05 kernels serve the shape and plan_last is given)
         tc = plan_dense.dtype == ab.F32 and plan_dense.l_max == 2 and plan_dense.n == 64
         self.fuse_readout = (tc and plan_last is not None) if fuse_readout is None else (fuse_readout and tc)
+        self.tc = tc      # tensor-core dense kernels: the 0e scalars travel between the layers in compact [E, n] side arrays
         self.pd_last = plan_last if plan_last is not None else plan_dense
         self.pd_first = plan_first if plan_first is not None else plan_dense
         self.L = params["W_w"].shape[0]
@@ -348,6 +349,8 @@ class TwoLayerStep:
         self.gEenv = new(N, n, plan_dense.dE)
         self.cot = [new(E, n, dV), new(E, n, dV)]          # ping-pong cotangents of V_l
         self.g_w, self.g_x, self.g_x2 = new(E, n), new(E, n), new(E, n)
+        self.s = [new(E, n, 1) if self.tc else None for _ in range(L - 1)]      # compact V_{l+1}[:, :, 0e] for the latent update
+        self.gs = new(E, n, 1) if (self.tc and L > 1) else None                  # compact cotangent of those scalars
         self.g_r, self.g_r_tmp = (new(E, 3) if sharded is None else sharded.g_local), new(E, 3)
         self.e_edge, self.e_tot, self.F = new(E), new(1), new(N, 3)
         self.e_ptr = torch.tensor([0, E], dtype=torch.int32, device=dv)
@@ -377,10 +380,13 @@ class TwoLayerStep:
             if l == L - 1 and self.fuse_readout:
                 timed("tp_forward_dense", lambda: ab.tp_forward_energy(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, want_out=False,
                                                                        want_G=False, e_edge=self.e_edge))
+            elif self.tc and l < L - 1:
+                timed("tp_forward_dense", lambda: ab.tp_forward_aux(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], self.V[l + 1], self.s[l]))
             else:
                 timed("tp_forward_dense", lambda: ab.tp_forward(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], out=self.V[l + 1]))
             if l < L - 1:
-                timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], self.V[l + 1], p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
+                Vs = self.s[l] if self.tc else self.V[l + 1]
+                timed("latent_forward", lambda: ab.latent_forward(rvec, rc, self.x[l], Vs, p["A_lat"][l], z=self.z[l], x_new=self.x[l + 1]))
         # readout E = sum_e sum_n q[n] V_L[e][n][0e]; its cotangent q (x) delta_{k,0} is formed inside the last layer's VJP when
         # that kernel exists (fp32, l_max 2, n 64), otherwise materialised here
         fused_cot = pd.dtype == ab.F32 and pd.l_max == 2 and pd.n == 64
@@ -392,12 +398,19 @@ class TwoLayerStep:
             g_x = None
             if l < L - 1:     # x_{l+1} = u SiLU(A [x_l ; V_{l+1}[:,0e]]): cotangent g_x_next; adds to G[:, :, 0] and g_r
                 g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
-                timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], G, self.g_r, g_x=g_x))
+                if self.tc:      # the scalars' cotangent goes into the compact side array; the dense VJP adds it to G while staging
+                    self.gs.zero_()
+                    timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], self.gs, self.g_r, g_x=g_x))
+                else:
+                    timed("latent_backward", lambda: ab.latent_backward(rvec, rc, self.z[l], g_x_next, p["A_lat"][l], G, self.g_r, g_x=g_x))
             gVl = self.cot[1] if G is self.cot[0] else self.cot[0]
             pl = self.pd_last if l == L - 1 else (self.pd_first if l == 0 else pd)
             if l == L - 1 and fused_cot:
                 timed("tp_backward_dense", lambda: ab.tp_backward_energy(pl, rp, self.V[L], self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, gV=gVl,
                                                                          gEenv=self.gEenv, workspace=self.ws))
+            elif self.tc and l < L - 1:
+                timed("tp_backward_dense", lambda: ab.tp_backward_aux(pl, rp, G, self.gs, self.V[l], self.Eenv[l], p["W_p"][l], gVl, self.gEenv,
+                                                                      workspace=self.ws))
             else:
                 timed("tp_backward_dense", lambda: ab.tp_backward(pl, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
             if not have_gr:

@@ -414,6 +414,17 @@ def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
         assert torch.equal(gW, gW2)                                                             # fixed-order reduction: reproducible bits
         _, gE2, _ = ab.tp_backward(plan, rpd, Gd, Vd, Ed, Wd, items=it, want_gV=False)
         _assert_close(dict(gEenv=ref_gE), dict(gEenv=gE2), dt, keys=("gEenv",), label="dense force-only")
+        if lmax == 2 and n == 64 and dt == np.float32:
+            # compact side channel of the 0e scalars (allegro_tp_forward_aux / _backward_aux): bitwise the plain calls' results
+            out2, sc = torch.empty_like(out), torch.empty((E, n, 1), dtype=out.dtype, device="cuda")
+            ab.tp_forward_aux(plan, rpd, Vd, Ed, Wd, out2, sc, items=it)
+            assert torch.equal(out2, out) and torch.equal(sc[:, :, 0], out[:, :, 0])
+            gs = torch.from_numpy(rng.normal(8, S["q"], (E, n, 1)).astype(dt)).cuda()
+            G2 = Gd.clone()
+            G2[:, :, 0] += gs[:, :, 0]
+            gV_a, gE_a, _ = ab.tp_backward(plan, rpd, G2, Vd, Ed, Wd, items=it)
+            gV_b, gE_b = ab.tp_backward_aux(plan, rpd, Gd, gs, Vd, Ed, Wd, torch.empty_like(Vd), torch.empty_like(Ed), items=it)
+            assert torch.equal(gV_a, gV_b) and torch.equal(gE_a, gE_b)
 
 
 def _block_mask_weights(lmax, W, out_mask, in_mask=0xffff):
