@@ -501,6 +501,15 @@ __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double r
     const long cb = (long)blockIdx.x * kGeoChunk;
     const int cnt = (int)min((long)kGeoChunk, E - cb);
     T* stg = reinterpret_cast<T*>(geo_raw + ((sizeof(GeoSmem<T, L, NB>) + 15) / 16) * 16) + (size_t)warp * 32 * DV;   // [32 channels][DV] per warp
+    // the two weight matrices transposed to [b][ch] in double: lanes run over channels, so the reads below are conflict-free (read
+    // from global memory as W[ch][b] they cost 32 sectors per request)
+    double* Wxs = reinterpret_cast<double*>(geo_raw + ((sizeof(GeoSmem<T, L, NB>) + 15) / 16) * 16 + (size_t)8 * 32 * DV * sizeof(T));
+    double* Wvs = Wxs + (size_t)nb * n;
+    for (int idx = tid; idx < n * nb; idx += 256) {
+        const int ch = idx / nb, b = idx - ch * nb;
+        Wxs[b * n + ch] = (double)W_x0[idx];
+        Wvs[b * n + ch] = (double)W_v0[idx];
+    }
     if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
     __syncthreads();
     for (int le = warp; le < cnt; le += 8) {
@@ -511,8 +520,8 @@ __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double r
                 double sx = 0.0, sv = 0.0;
                 for (int b = 0; b < nb; ++b) {
                     const double bu = sm.Bs[le][b];
-                    sx = fma((double)W_x0[ch * nb + b], bu, sx);
-                    sv = fma((double)W_v0[ch * nb + b], bu, sv);
+                    sx = fma(Wxs[b * n + ch], bu, sx);
+                    sv = fma(Wvs[b * n + ch], bu, sv);
                 }
                 x0[e * n + ch] = (T)sx;
                 const T v0 = (T)sv;
@@ -543,6 +552,13 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
     const long cb = (long)blockIdx.x * kGeoChunk;
     const int cnt = (int)min((long)kGeoChunk, E - cb);
     T* stg = reinterpret_cast<T*>(geo_raw + ((sizeof(GeoSmem<T, L, NB>) + 15) / 16) * 16) + (size_t)warp * 32 * DV;   // [32 channels][DV] per warp
+    double* Wxs = reinterpret_cast<double*>(geo_raw + ((sizeof(GeoSmem<T, L, NB>) + 15) / 16) * 16 + (size_t)8 * 32 * DV * sizeof(T));   // [b][ch]
+    double* Wvs = Wxs + (size_t)nb * n;
+    for (int idx = tid; idx < n * nb; idx += 256) {
+        const int ch = idx / nb, b = idx - ch * nb;
+        Wxs[b * n + ch] = (double)W_x0[idx];
+        Wvs[b * n + ch] = (double)W_v0[idx];
+    }
     if (tid < cnt) geo_phase1<T, L, NB, true>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
     __syncthreads();
     for (int le = warp; le < cnt; le += 8) {
@@ -560,7 +576,7 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
             T row[DV];
             row_load<T, DV>(stg + lane * DV, row);
             double sv = 0.0;
-            for (int b = 0; b < nb; ++b) sv = fma((double)W_v0[ch * nb + b], sm.Bs[le][b], sv);
+            for (int b = 0; b < nb; ++b) sv = fma(Wvs[b * n + ch], sm.Bs[le][b], sv);
             const T v0 = (T)sv;
             T gv0 = T(0);
 #pragma unroll
@@ -572,7 +588,7 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
             const double gx = (double)g_x0[e * n + ch];
 #pragma unroll
             for (int b = 0; b < NB; ++b)
-                if (b < nb) gbp[b] += gx * (double)W_x0[ch * nb + b] + (double)gv0 * (double)W_v0[ch * nb + b];
+                if (b < nb) gbp[b] += gx * Wxs[b * n + ch] + (double)gv0 * Wvs[b * n + ch];
         }
         warp_reduce16<T>(gYp, lane);
         warp_reduce16<double>(gbp, lane);

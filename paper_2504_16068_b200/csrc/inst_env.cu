@@ -137,7 +137,7 @@ allegro_status_t launch_edge_embed<ALLEGRO_T, ALLEGRO_L>(const EmbedArgs& a) {
 #define ALLEGRO_EMB(NB)                                                                                                     \
     {                                                                                                                       \
         auto k = edge_embed_kernel<T, ALLEGRO_L, NB>;                                                                       \
-        const size_t smem = (sizeof(GeoSmem<T, ALLEGRO_L, NB>) + 15) / 16 * 16 + 8 * 32 * 2 * (ALLEGRO_L + 1) * (ALLEGRO_L + 1) * sizeof(T); \
+        const size_t smem = (sizeof(GeoSmem<T, ALLEGRO_L, NB>) + 15) / 16 * 16 + 8 * 32 * 2 * (ALLEGRO_L + 1) * (ALLEGRO_L + 1) * sizeof(T) + (size_t)2 * a.nb * a.n * sizeof(double); \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
         k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0, (T*)a.x0, (T*)a.V0); \
     }
@@ -159,7 +159,7 @@ allegro_status_t launch_edge_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EmbedArg
 #define ALLEGRO_EMBB(NB)                                                                                                    \
     {                                                                                                                       \
         auto k = edge_embed_bwd_kernel<T, ALLEGRO_L, NB>;                                                                   \
-        const size_t smem = (sizeof(GeoSmem<T, ALLEGRO_L, NB>) + 15) / 16 * 16 + 8 * 32 * 2 * (ALLEGRO_L + 1) * (ALLEGRO_L + 1) * sizeof(T); \
+        const size_t smem = (sizeof(GeoSmem<T, ALLEGRO_L, NB>) + 15) / 16 * 16 + 8 * 32 * 2 * (ALLEGRO_L + 1) * (ALLEGRO_L + 1) * sizeof(T) + (size_t)2 * a.nb * a.n * sizeof(double); \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
         k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0,     \
                                      (const T*)a.g_x0, (const T*)a.gV0, (T*)a.g_rvec);                                     \

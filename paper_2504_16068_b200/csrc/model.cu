@@ -73,6 +73,21 @@ __device__ __forceinline__ void tile_load_x(T* __restrict__ xs, int ld, const T*
         xs[(size_t)le * ld + k0 + k] = eb + le < E ? x[(size_t)(eb + le) * ldx + (size_t)k * kstride] : T(0);
     }
 }
+// store 4 consecutive outputs of one edge: one 16-byte vector when the row allows it (float, n_out % 4 == 0), else scalars
+template <typename T>
+__device__ __forceinline__ void tile_store4(T* __restrict__ dst, const T (&v)[4], int o, int n_out, bool vec) {
+    if (vec) {
+        if constexpr (sizeof(T) == 4) {
+            *reinterpret_cast<float4*>(dst) = make_float4(v[0], v[1], v[2], v[3]);
+        } else {
+            *reinterpret_cast<double2*>(dst) = make_double2(v[0], v[1]);
+            *reinterpret_cast<double2*>(dst + 2) = make_double2(v[2], v[3]);
+        }
+    } else {
+#pragma unroll
+        for (int j = 0; j < 4; ++j) if (o + j < n_out) dst[j] = v[j];
+    }
+}
 // zero the pad columns [K, ld) of every row (once per CTA: the tile loads never touch them)
 template <typename T>
 __device__ __forceinline__ void tile_zero_pad(T* __restrict__ xs, int ld, int K, int tid) {
@@ -92,6 +107,7 @@ __global__ void __launch_bounds__(256) linear_kernel(long E, int n_out, int n_in
     T* Ws = xs + (size_t)kTileE * ld;                 // [Kp][64]
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int nchunk = (n_out + kTileO - 1) / kTileO;
+    const bool vec_out = n_out % 4 == 0 && (reinterpret_cast<uintptr_t>(y) & 15u) == 0;
     tile_zero_pad<T>(xs, ld, n_in, tid);
     for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
@@ -111,15 +127,14 @@ __global__ void __launch_bounds__(256) linear_kernel(long E, int n_out, int n_in
 #pragma unroll
             for (int i = 0; i < 8; ++i) {
                 const long e = eb + ty + 16 * i;
-                if (e >= E) continue;
+                const int o = c * kTileO + 4 * tx;
+                if (e >= E || o >= n_out) continue;
+                T* dst = y + (size_t)e * n_out + o;
+                if (accumulate) {
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int o = c * kTileO + 4 * tx + j;
-                    if (o < n_out) {
-                        T* dst = y + (size_t)e * n_out + o;
-                        *dst = accumulate ? *dst + acc[i][j] : acc[i][j];
-                    }
+                    for (int j = 0; j < 4; ++j) if (o + j < n_out) acc[i][j] += dst[j];
                 }
+                tile_store4<T>(dst, acc[i], o, n_out, vec_out);
             }
         }
     }
@@ -146,6 +161,7 @@ __global__ void __launch_bounds__(256) latent_fwd_kernel(long E, int n, int dV, 
     T* us = Ws + (size_t)Kp * kTileO;                 // [128] cutoff u(|r|/rc)
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int nchunk = (n + kTileO - 1) / kTileO;
+    const bool vec_out = n % 4 == 0 && ((reinterpret_cast<uintptr_t>(z) | reinterpret_cast<uintptr_t>(x_new)) & 15u) == 0;
     tile_zero_pad<T>(xs, ld, K, tid);
     for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
@@ -177,16 +193,16 @@ __global__ void __launch_bounds__(256) latent_fwd_kernel(long E, int n, int dV, 
                 const long e = eb + ty + 16 * i;
                 if (e >= E) continue;
                 const T u = us[ty + 16 * i];
+                const int o = c * kTileO + 4 * tx;
+                if (o >= n) continue;
+                T xn[4];
 #pragma unroll
                 for (int j = 0; j < 4; ++j) {
-                    const int o = c * kTileO + 4 * tx + j;
-                    if (o < n) {
-                        const T a = acc[i][j];
-                        const T sg = T(1) / (T(1) + exp(-a));
-                        z[(size_t)e * n + o] = a;
-                        x_new[(size_t)e * n + o] = u * a * sg;
-                    }
+                    const T a = acc[i][j];
+                    xn[j] = u * a * (T(1) / (T(1) + exp(-a)));
                 }
+                tile_store4<T>(z + (size_t)e * n + o, acc[i], o, n, vec_out);
+                tile_store4<T>(x_new + (size_t)e * n + o, xn, o, n, vec_out);
             }
         }
     }
@@ -207,6 +223,7 @@ __global__ void __launch_bounds__(256) latent_bwd_kernel(long E, int n, int dV, 
     T* dus = us + kTileE;
     const int tid = threadIdx.x, ty = tid >> 4, tx = tid & 15;
     const int nchunk = (2 * n + kTileO - 1) / kTileO;
+    const bool vec_out = n % 4 == 0 && ((reinterpret_cast<uintptr_t>(g_x) | reinterpret_cast<uintptr_t>(gV)) & 15u) == 0;
     tile_zero_pad<T>(xs, ld, n, tid);
     for (long eb = (long)blockIdx.x * kTileE; eb < E; eb += (long)gridDim.x * kTileE) {
         __syncthreads();
@@ -250,11 +267,21 @@ __global__ void __launch_bounds__(256) latent_bwd_kernel(long E, int n, int dV, 
             for (int i = 0; i < 8; ++i) {
                 const long e = eb + ty + 16 * i;
                 if (e >= E) continue;
+                const int o0 = c * kTileO + 4 * tx;
+                if (vec_out && o0 + 3 < n) {
+                    tile_store4<T>(g_x + (size_t)e * n + o0, acc[i], o0, n, true);
+                } else if (vec_out && dV == 1 && o0 >= n && o0 + 3 < 2 * n) {      // compact scalar cotangent: contiguous
+                    T* dst = gV + (size_t)e * n + (o0 - n);
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int o = c * kTileO + 4 * tx + j;
-                    if (o < n) g_x[(size_t)e * n + o] = acc[i][j];
-                    else if (o < 2 * n) gV[((size_t)e * n + (o - n)) * dV] += acc[i][j];
+                    for (int j = 0; j < 4; ++j) acc[i][j] += dst[j];
+                    tile_store4<T>(dst, acc[i], o0 - n, n, true);
+                } else {
+#pragma unroll
+                    for (int j = 0; j < 4; ++j) {
+                        const int o = o0 + j;
+                        if (o < n) g_x[(size_t)e * n + o] = acc[i][j];
+                        else if (o < 2 * n) gV[((size_t)e * n + (o - n)) * dV] += acc[i][j];
+                    }
                 }
             }
         }
