@@ -87,6 +87,8 @@ SIGNATURES = {
                                           C.POINTER(C.c_long)]),
     "allegro_neighbour_fill": (C.c_int, [C.c_int, _vp, C.c_double, _f64p, _f64p, C.c_double, _vp, _vp, C.c_int, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp,
                                          C.c_int, _vp, C.c_size_t, _vp]),
+    "allegro_env_linear_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp]),
+    "allegro_env_linear_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, C.c_int, _vp, C.c_int, _vp]),
     "allegro_env_radial_forward_typed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp,
                                                    C.c_size_t, _vp]),
     "allegro_env_radial_backward_typed": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, C.c_int, _vp, C.c_double, _vp, _vp, _vp]),
@@ -571,6 +573,25 @@ def neighbour_list(pos, r_cut, box=None, mol_id=None, dtype=F32, species=None, r
     if typed:
         out["rc_edge"] = rc_edge
     return out
+
+
+def env_linear_forward(plan, row_ptr, rvec, x, W, scale=1.0, Eenv=None, stream=None):
+    """Eenv of the linear per-edge weights w = x W^T without forming w (allegro_env_linear_forward)"""
+    n_atoms = row_ptr.shape[0] - 1
+    if Eenv is None:
+        Eenv = torch.empty((n_atoms, plan.n, plan.dE), dtype=rvec.dtype, device=rvec.device)
+    _check(lib().allegro_env_linear_forward(plan.h, n_atoms, rvec.shape[0], _ptr(row_ptr), _ptr(rvec), _ptr(x), _ptr(W), x.shape[1], float(scale),
+                                            _ptr(Eenv), _stream(stream)))
+    return Eenv
+
+
+def env_linear_backward(plan, row_ptr, gEenv, rvec, x, W, scale, g_rvec, g_x, accumulate_g_rvec=False, accumulate_g_x=False, stream=None):
+    """VJP of env_linear_forward: g_rvec [E,3] and g_x [E,n_in] are overwritten or accumulated into"""
+    n_atoms = row_ptr.shape[0] - 1
+    _check(lib().allegro_env_linear_backward(plan.h, n_atoms, rvec.shape[0], _ptr(row_ptr), _ptr(gEenv), _ptr(rvec), _ptr(x), _ptr(W), x.shape[1],
+                                             float(scale), _ptr(g_rvec), int(bool(accumulate_g_rvec)), _ptr(g_x), int(bool(accumulate_g_x)),
+                                             _stream(stream)))
+    return g_rvec, g_x
 
 
 def env_radial_forward_typed(plan, row_ptr, rvec, W_r, rc_edge, scale=1.0, items=None, want_w=False, w=None, Eenv=None, workspace=None, stream=None):

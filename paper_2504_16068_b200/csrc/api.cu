@@ -25,6 +25,8 @@ void set_error(const char* fmt, ...) {
     template <> allegro_status_t launch_edge_embed<T, L>(const EmbedArgs&);                    \
     template <> allegro_status_t launch_edge_embed_backward<T, L>(const EmbedArgs&);           \
     template <> allegro_status_t launch_env_embed_backward<T, L>(const EnvBwdArgs&);           \
+    template <> allegro_status_t launch_env_linear<T, L>(const EnvLinArgs&);                   \
+    template <> allegro_status_t launch_env_linear_backward<T, L>(const EnvLinArgs&);          \
     template <> allegro_status_t launch_tp_forward<T, L>(const TpArgs&);                       \
     template <> allegro_status_t launch_tp_backward<T, L>(const TpArgs&);                      \
     template <> allegro_status_t launch_tp_fused<T, L>(const TpArgs&);                         \
@@ -237,6 +239,32 @@ allegro_status_t allegro_env_radial_backward(const allegro_plan_t* plan, int n_a
     ALLEGRO_CHECK_ARG(gEenv || n_atoms == 0, "gEenv is NULL");
     EnvBwdArgs a{plan->n, n_atoms, n_edges, row_ptr, gEenv, rvec, nullptr, scale, g_rvec, g_w, (cudaStream_t)stream, W_r, n_basis, r_cut};
     return ALLEGRO_DISPATCH(plan, launch_env_embed_backward, a);
+}
+
+allegro_status_t allegro_env_linear_forward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const void* rvec,
+                                            const void* x, const void* W, int n_in, double scale, void* Eenv, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && x) || n_edges == 0, "rvec / x is NULL");
+    ALLEGRO_CHECK_ARG(W != nullptr && n_in >= 1, "W is NULL or bad n_in");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    EnvLinArgs a{};
+    a.n_out = plan->n; a.n_in = n_in; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.rvec = rvec; a.x = x; a.W = W;
+    a.scale = scale; a.Eenv = Eenv; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_env_linear, a);
+}
+
+allegro_status_t allegro_env_linear_backward(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const void* gEenv,
+                                             const void* rvec, const void* x, const void* W, int n_in, double scale, void* g_rvec,
+                                             int accumulate_g_rvec, void* g_x, int accumulate_g_x, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && x && g_rvec && g_x) || n_edges == 0, "rvec / x / g_rvec / g_x is NULL");
+    ALLEGRO_CHECK_ARG(W != nullptr && n_in >= 1, "W is NULL or bad n_in");
+    ALLEGRO_CHECK_ARG(gEenv || n_atoms == 0, "gEenv is NULL");
+    EnvLinArgs a{};
+    a.n_out = plan->n; a.n_in = n_in; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.rvec = rvec; a.x = x; a.W = W;
+    a.scale = scale; a.gEenv = gEenv; a.g_rvec = g_rvec; a.acc_g_rvec = accumulate_g_rvec; a.g_x = g_x; a.acc_g_x = accumulate_g_x;
+    a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_env_linear_backward, a);
 }
 
 allegro_status_t allegro_env_radial_forward_typed(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,

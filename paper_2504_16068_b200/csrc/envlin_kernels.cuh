@@ -1,0 +1,162 @@
+// envlin_kernels.cuh -- environment embedding of LINEAR per-edge weights, w[e][n] = sum_m W[n][m] x[e][m] (the per-edge linear
+// map of the stacked model, reading A19), without ever forming w: the sums over edges and over m commute, so per centre c
+//   forward : S_c[m][j] = sum_{e in row c} x[e][m] Y_j(rhat_e)              (n_in x dE),   Eenv[c][n][j] = scale sum_m W[n][m] S_c[m][j]
+//   VJP     : M_c[m][j] = scale sum_n W[n][m] gEenv[c][n][j]                (n_in x dE)
+//             g_x[e][m]  (+)= sum_j M_c[m][j] Y_j(rhat_e)                    (= sum_n W[n][m] g_w[e][n])
+//             gY_e[j]      = sum_m M_c[m][j] x[e][m],   g_rvec[e] (+)= (I - rhat rhat^T) J^T gY_e / |r_e|
+// The per-edge n_in x n GEMM (and its transpose in the VJP) becomes one n x n_in x dE product per CENTRE: ~deg / dE times fewer
+// FMAs, and neither w[E][n] nor g_w[E][n] crosses HBM.  One CTA (256 threads) per centre; every sum has a fixed order.
+// Included by inst_env.cu once per (ALLEGRO_T, ALLEGRO_L).
+#pragma once
+#include "common.cuh"
+#include "launch.h"
+
+namespace allegro {
+
+constexpr int kEnvLinThreads = 256, kEnvLinChunk = 128;
+
+template <typename T, int L>
+__global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_out, int n_in, const int* __restrict__ row_ptr, const T* __restrict__ rvec,
+                                                                         const T* __restrict__ x, const T* __restrict__ W, T scale,
+                                                                         T* __restrict__ Eenv) {
+    constexpr int DE = (L + 1) * (L + 1);
+    extern __shared__ __align__(16) unsigned char envlin_raw[];
+    T* Ys = reinterpret_cast<T*>(envlin_raw);                 // [chunk][DE]
+    T* red = Ys + kEnvLinChunk * DE;                           // [threads][DE] per-slot partial sums, then S[n_in][DE] in its first rows
+    T* Wt = red + kEnvLinThreads * DE;                         // [n_in][n_out]: W transposed (lanes run over n in the last phase)
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x;
+    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+    const int nslots = kEnvLinThreads / n_in;
+    const int slot = tid / n_in, m = tid - slot * n_in;
+    const bool active = slot < nslots;
+    for (int idx = tid; idx < n_out * n_in; idx += kEnvLinThreads) {
+        const int n = idx / n_in, mm = idx - n * n_in;
+        Wt[mm * n_out + n] = W[idx];
+    }
+    T acc[DE];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) acc[j] = T(0);
+    for (int cb = e0; cb < e1; cb += kEnvLinChunk) {
+        const int cnt = min(kEnvLinChunk, e1 - cb);
+        __syncthreads();
+        if (tid < cnt) {
+            const size_t e = (size_t)(cb + tid);
+            const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+            const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+            T Y[DE];
+            sph_harm<T, L>(rx * inv, ry * inv, rz * inv, Y);
+#pragma unroll
+            for (int j = 0; j < DE; ++j) Ys[tid * DE + j] = Y[j];
+        }
+        __syncthreads();
+        if (active) {
+            for (int le = slot; le < cnt; le += nslots) {
+                const T xv = x[(size_t)(cb + le) * n_in + m];
+#pragma unroll
+                for (int j = 0; j < DE; ++j) acc[j] = fma(xv, Ys[le * DE + j], acc[j]);
+            }
+        }
+    }
+    __syncthreads();
+#pragma unroll
+    for (int j = 0; j < DE; ++j) red[tid * DE + j] = acc[j];
+    __syncthreads();
+    if (slot == 0) {     // S[m][j]: slots in slot order (into the first n_in rows; thread m only touches row m and rows sl * n_in + m)
+#pragma unroll
+        for (int j = 0; j < DE; ++j) {
+            T s = red[m * DE + j];
+            for (int sl = 1; sl < nslots; ++sl) s += red[(sl * n_in + m) * DE + j];
+            acc[j] = s;
+        }
+    }
+    __syncthreads();
+    if (slot == 0) {
+#pragma unroll
+        for (int j = 0; j < DE; ++j) red[m * DE + j] = acc[j];
+    }
+    __syncthreads();
+    // Eenv[c][n][j] = scale sum_m W[n][m] S[m][j]
+    for (int idx = tid; idx < n_out * DE; idx += kEnvLinThreads) {
+        const int j = idx / n_out, n = idx - j * n_out;
+        T s = T(0);
+        for (int mm = 0; mm < n_in; ++mm) s = fma(Wt[mm * n_out + n], red[mm * DE + j], s);
+        Eenv[((size_t)c * n_out + n) * DE + j] = scale * s;
+    }
+}
+
+template <typename T, int L>
+__global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_out, int n_in, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
+                                                                         const T* __restrict__ rvec, const T* __restrict__ x, const T* __restrict__ W,
+                                                                         T scale, T* __restrict__ g_rvec, int acc_g_rvec, T* __restrict__ g_x, int acc_g_x) {
+    constexpr int DE = (L + 1) * (L + 1);
+    extern __shared__ __align__(16) unsigned char envlin_raw[];
+    T* Ys = reinterpret_cast<T*>(envlin_raw);                 // [chunk][DE]
+    T* geo = Ys + kEnvLinChunk * DE;                           // [chunk][4]: unit vector, 1/|r|
+    T* gEs = geo + kEnvLinChunk * 4;                           // [n_out][DE]
+    T* Ms = gEs + n_out * DE;                                  // [n_in][DE]
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x;
+    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+    const int nslots = kEnvLinThreads / n_in;
+    const int slot = tid / n_in, m = tid - slot * n_in;
+    const bool active = slot < nslots;
+    for (int idx = tid; idx < n_out * DE; idx += kEnvLinThreads) gEs[idx] = gEenv[(size_t)c * n_out * DE + idx];
+    __syncthreads();
+    // M[m][j] = scale sum_n W[n][m] gE[n][j]: lanes run over m (coalesced rows of W)
+    for (int idx = tid; idx < n_in * DE; idx += kEnvLinThreads) {
+        const int j = idx / n_in, mm = idx - j * n_in;
+        T s = T(0);
+        for (int n = 0; n < n_out; ++n) s = fma(W[(size_t)n * n_in + mm], gEs[n * DE + j], s);
+        Ms[mm * DE + j] = scale * s;
+    }
+    for (int cb = e0; cb < e1; cb += kEnvLinChunk) {
+        const int cnt = min(kEnvLinChunk, e1 - cb);
+        __syncthreads();
+        if (tid < cnt) {
+            const size_t e = (size_t)(cb + tid);
+            const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+            const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+            const T ux = rx * inv, uy = ry * inv, uz = rz * inv;
+            T Y[DE];
+            sph_harm<T, L>(ux, uy, uz, Y);
+#pragma unroll
+            for (int j = 0; j < DE; ++j) Ys[tid * DE + j] = Y[j];
+            geo[tid * 4] = ux; geo[tid * 4 + 1] = uy; geo[tid * 4 + 2] = uz; geo[tid * 4 + 3] = inv;
+        }
+        __syncthreads();
+        if (active) {        // g_x[e][m] = sum_j M[m][j] Y_j(e)
+            T Mr[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) Mr[j] = Ms[m * DE + j];
+            for (int le = slot; le < cnt; le += nslots) {
+                T s = T(0);
+#pragma unroll
+                for (int j = 0; j < DE; ++j) s = fma(Mr[j], Ys[le * DE + j], s);
+                T* dst = g_x + (size_t)(cb + le) * n_in + m;
+                *dst = acc_g_x ? *dst + s : s;
+            }
+        }
+        if (tid < cnt) {     // gY_e[j] = sum_m M[m][j] x[e][m], then through Y_lm and the normalisation
+            const size_t e = (size_t)(cb + tid);
+            T gY[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) gY[j] = T(0);
+            const T* xr = x + e * n_in;
+            for (int mm = 0; mm < n_in; ++mm) {
+                const T xv = xr[mm];
+#pragma unroll
+                for (int j = 0; j < DE; ++j) gY[j] = fma(Ms[mm * DE + j], xv, gY[j]);
+            }
+            const T ux = geo[tid * 4], uy = geo[tid * 4 + 1], uz = geo[tid * 4 + 2], inv = geo[tid * 4 + 3];
+            T g[3];
+            sph_harm_vjp<T, L>(ux, uy, uz, gY, g);
+            const T dot = g[0] * ux + g[1] * uy + g[2] * uz;
+            const T r0 = (g[0] - dot * ux) * inv, r1 = (g[1] - dot * uy) * inv, r2 = (g[2] - dot * uz) * inv;
+            T* dst = g_rvec + 3 * e;
+            if (acc_g_rvec) { dst[0] += r0; dst[1] += r1; dst[2] += r2; } else { dst[0] = r0; dst[1] = r1; dst[2] = r2; }
+        }
+    }
+}
+
+}  // namespace allegro

@@ -5,6 +5,7 @@
 #include <cstdlib>
 
 #include "env_kernels.cuh"
+#include "envlin_kernels.cuh"
 
 namespace allegro {
 
@@ -166,6 +167,42 @@ allegro_status_t launch_edge_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EmbedArg
     }
     if (a.nb <= 8) ALLEGRO_EMBB(8) else ALLEGRO_EMBB(16)
 #undef ALLEGRO_EMBB
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
+template <>
+allegro_status_t launch_env_linear<ALLEGRO_T, ALLEGRO_L>(const EnvLinArgs& a) {
+    using T = ALLEGRO_T;
+    constexpr int DE = (ALLEGRO_L + 1) * (ALLEGRO_L + 1);
+    if (a.n_in < 1 || a.n_in > kEnvLinThreads || a.n_out > 256) {
+        set_error("env_linear_forward: n_in = %d, n = %d unsupported (n_in <= %d, n <= 256)", a.n_in, a.n_out, kEnvLinThreads);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (a.n_atoms == 0) return ALLEGRO_OK;
+    const size_t smem = ((size_t)kEnvLinChunk * DE + (size_t)kEnvLinThreads * DE + (size_t)a.n_in * a.n_out) * sizeof(T);
+    auto k = env_linear_fwd_kernel<T, ALLEGRO_L>;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k<<<(unsigned)a.n_atoms, kEnvLinThreads, smem, a.st>>>(a.n_out, a.n_in, a.row_ptr, (const T*)a.rvec, (const T*)a.x, (const T*)a.W, (T)a.scale,
+                                                           (T*)a.Eenv);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
+template <>
+allegro_status_t launch_env_linear_backward<ALLEGRO_T, ALLEGRO_L>(const EnvLinArgs& a) {
+    using T = ALLEGRO_T;
+    constexpr int DE = (ALLEGRO_L + 1) * (ALLEGRO_L + 1);
+    if (a.n_in < 1 || a.n_in > kEnvLinThreads || a.n_out > 256) {
+        set_error("env_linear_backward: n_in = %d, n = %d unsupported (n_in <= %d, n <= 256)", a.n_in, a.n_out, kEnvLinThreads);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (a.n_atoms == 0) return ALLEGRO_OK;
+    const size_t smem = ((size_t)kEnvLinChunk * (DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE) * sizeof(T);
+    auto k = env_linear_bwd_kernel<T, ALLEGRO_L>;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    k<<<(unsigned)a.n_atoms, kEnvLinThreads, smem, a.st>>>(a.n_out, a.n_in, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.x, (const T*)a.W,
+                                                           (T)a.scale, (T*)a.g_rvec, a.acc_g_rvec, (T*)a.g_x, a.acc_g_x);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

@@ -48,6 +48,22 @@ struct EnvBwdArgs {
     double rc;
     const void* rc_edge;  // nullable: per-edge cutoff radii T[E]
 };
+struct EnvLinArgs {
+    int n_out, n_in, n_atoms;
+    long n_edges;
+    const int32_t* row_ptr;
+    const void* rvec;
+    const void* x;
+    const void* W;        // [n_out][n_in]
+    double scale;
+    void* Eenv;           // forward output
+    const void* gEenv;    // backward input
+    void* g_rvec;
+    int acc_g_rvec;
+    void* g_x;
+    int acc_g_x;
+    cudaStream_t st;
+};
 struct TpArgs {
     const allegro_plan* plan;
     int n, n_atoms;
@@ -95,6 +111,8 @@ template <typename T, int L> allegro_status_t launch_edge_embed(const EmbedArgs&
 template <typename T, int L> allegro_status_t launch_edge_embed_backward(const EmbedArgs& a);
 template <typename T, int L> allegro_status_t launch_env_embed(const EnvArgs& a);
 template <typename T, int L> allegro_status_t launch_env_embed_backward(const EnvBwdArgs& a);
+template <typename T, int L> allegro_status_t launch_env_linear(const EnvLinArgs& a);
+template <typename T, int L> allegro_status_t launch_env_linear_backward(const EnvLinArgs& a);
 template <typename T, int L> allegro_status_t launch_tp_forward(const TpArgs& a);
 template <typename T, int L> allegro_status_t launch_tp_backward(const TpArgs& a);
 template <typename T, int L> allegro_status_t launch_tp_fused(const TpArgs& a);

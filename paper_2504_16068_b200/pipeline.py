@@ -325,13 +325,14 @@ class TwoLayerStep:
     `plan_first`: optional dense plan restricted to the natural-parity input blocks (Plan.set_in_blocks(0x19)) for the first
     layer, whose input V0 = v (x) Y has zeros in the other blocks (reading A19): half of the paths never run."""
 
-    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None, sharded=None, fuse_readout=None):
+    def __init__(self, plan_dense, plan_scalar, dev, params, plan_last=None, plan_first=None, sharded=None, fuse_readout=None, factorised_env=True):
         self.pd, self.ps, self.dev, self.p = plan_dense, plan_scalar, dev, params
         self.sharded = sharded      # sharding.ShardedForces: `dev` holds one rank's rows (see SingleLayerStep)
         # fuse_readout: the readout E = sum q . V_L[:, :, 0e] is taken in the last layer's forward epilogue and its cotangent formed inside
         # the last layer's VJP, so V_L is never stored (default: whenever the tcgen05 kernels serve the shape and plan_last is given)
         tc = plan_dense.dtype == ab.F32 and plan_dense.l_max == 2 and plan_dense.n == 64
         self.fuse_readout = (tc and plan_last is not None) if fuse_readout is None else (fuse_readout and tc)
+        self.factorised_env = factorised_env      # env-embed of the linear weights without forming w (False: linear + env_embed, the named calls)
         self.tc = tc      # tensor-core dense kernels: the 0e scalars travel between the layers in compact [E, n] side arrays
         self.pd_last = plan_last if plan_last is not None else plan_dense
         self.pd_first = plan_first if plan_first is not None else plan_dense
@@ -374,8 +375,11 @@ class TwoLayerStep:
 
         timed("edge_embed", lambda: ab.edge_embed(pd, rvec, p["W_x0"], p["W_v0"], rc, x0=self.x[0], V0=self.V[0]))
         for l in range(L):
-            timed("linear", lambda: ab.linear(self.x[l], p["W_w"][l], y=self.w[l]))
-            timed("env_embed", lambda: ab.env_embed(ps, rp, rvec, self.w[l], scale, Eenv=self.Eenv[l]))
+            if self.factorised_env:      # w = W_w x is never formed: the linear map is applied once per centre (allegro_env_linear_forward)
+                timed("env_linear_forward", lambda: ab.env_linear_forward(ps, rp, rvec, self.x[l], p["W_w"][l], scale, Eenv=self.Eenv[l]))
+            else:
+                timed("linear", lambda: ab.linear(self.x[l], p["W_w"][l], y=self.w[l]))
+                timed("env_embed", lambda: ab.env_embed(ps, rp, rvec, self.w[l], scale, Eenv=self.Eenv[l]))
             pl = self.pd_last if l == L - 1 else (self.pd_first if l == 0 else pd)
             if l == L - 1 and self.fuse_readout:
                 timed("tp_forward_dense", lambda: ab.tp_forward_energy(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, want_out=False,
@@ -413,17 +417,25 @@ class TwoLayerStep:
                                                                       workspace=self.ws))
             else:
                 timed("tp_backward_dense", lambda: ab.tp_backward(pl, rp, G, self.V[l], self.Eenv[l], p["W_p"][l], gV=gVl, gEenv=self.gEenv, workspace=self.ws))
-            if not have_gr:
-                timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r, g_w=self.g_w))
+            if self.factorised_env:
+                acc_x = g_x is not None
+                if g_x is None:
+                    g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
+                timed("env_linear_backward", lambda: ab.env_linear_backward(ps, rp, self.gEenv, rvec, self.x[l], p["W_w"][l], scale, self.g_r, g_x,
+                                                                            accumulate_g_rvec=have_gr, accumulate_g_x=acc_x))
                 have_gr = True
             else:
-                timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r_tmp, g_w=self.g_w))
-                timed("add_inplace", lambda: ab.add_inplace(self.g_r, self.g_r_tmp))
-            if g_x is None:
-                g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
-                timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x))
-            else:
-                timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x, accumulate=True))
+                if not have_gr:
+                    timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r, g_w=self.g_w))
+                    have_gr = True
+                else:
+                    timed("env_embed_backward", lambda: ab.env_embed_backward(ps, rp, self.gEenv, rvec, self.w[l], scale, g_rvec=self.g_r_tmp, g_w=self.g_w))
+                    timed("add_inplace", lambda: ab.add_inplace(self.g_r, self.g_r_tmp))
+                if g_x is None:
+                    g_x = self.g_x if g_x_next is not self.g_x else self.g_x2
+                    timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x))
+                else:
+                    timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x, accumulate=True))
             G, g_x_next = gVl, g_x
         timed("edge_embed_backward", lambda: ab.edge_embed_backward(pd, rvec, p["W_x0"], p["W_v0"], rc, g_x_next, G, self.g_r))
         if self.sharded is None:

@@ -639,7 +639,7 @@ def _two_layer_step(inp, scalars_only_last=False):
         first = ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE)
         first.set_in_blocks(0x19)
     st = TwoLayerStep(ab.Plan(p["lmax"], p["n"], dt, ab.W_DENSE), ab.Plan(p["lmax"], p["n"], dt, ab.W_SCALAR), dev, prm, plan_last=last,
-                      plan_first=first, fuse_readout=(scalars_only_last == "fused_readout"))
+                      plan_first=first, fuse_readout=(scalars_only_last == "fused_readout"), factorised_env=bool(scalars_only_last))
     st.run()
     return st
 
@@ -659,8 +659,10 @@ def test_two_layer_model_c2s(scalars_only_last):
     st = _two_layer_step(inp, scalars_only_last)
     ref, got = dict(g_r=g, e_edge=taps[-1]["e_edge"], F=orc.force_gather(inp["row_ptr"], inp["rev"], g)), dict(g_r=st.g_r, e_edge=st.e_edge, F=st.F)
     for l in range(p["n_layers"]):
-        ref.update({"Eenv%d" % l: taps[l]["Eenv"], "V%d" % (l + 1): taps[l]["V_out"], "w%d" % l: taps[l]["w"]})
-        got.update({"Eenv%d" % l: st.Eenv[l], "V%d" % (l + 1): st.V[l + 1], "w%d" % l: st.w[l]})
+        ref.update({"Eenv%d" % l: taps[l]["Eenv"], "V%d" % (l + 1): taps[l]["V_out"]})
+        got.update({"Eenv%d" % l: st.Eenv[l], "V%d" % (l + 1): st.V[l + 1]})
+        if not st.factorised_env:      # the per-edge weights w = W_w x exist only on the un-factorised path
+            ref["w%d" % l], got["w%d" % l] = taps[l]["w"], st.w[l]
     if scalars_only_last:      # only the scalars of the last layer's output exist
         L = p["n_layers"]
         if st.V[L] is None:    # readout fused into the last layer's forward: V_L is never stored
@@ -948,3 +950,37 @@ def test_per_edge_type_cutoffs():
         torch.cuda.synchronize()
         _assert_close(dict(Eenv=Eenv, w=w, g_r=g_r, g_w=g_w), dict(Eenv=E2, w=w2, g_r=gr2, g_w=gw2), dt, keys=("Eenv", "w", "g_r", "g_w"),
                       label="typed cutoffs want_w=%s" % want)
+
+
+@pytest.mark.parametrize("geom,lmax,n,n_in,dt", [("C1s", 2, 64, 64, np.float32), ("C0", 1, 8, 12, np.float64), ("C4s", 3, 32, 64, np.float32)])
+def test_env_linear_forward_and_vjp(geom, lmax, n, n_in, dt):
+    """allegro_env_linear_forward / _backward (embedding of the linear weights w = x W^T with the linear map applied once per centre)
+    against the oracle's plain chain: w = x W^T -> env_embed; VJP: env_embed_backward -> g_x = g_w W; also accumulating"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, rng
+    g = configs.geometry_for(geom)
+    rp, rvec = g["row_ptr"], g["rvec"].astype(dt)
+    E, N = rvec.shape[0], rp.shape[0] - 1
+    dE = (lmax + 1) ** 2
+    S = rng.STREAMS
+    x = rng.normal(17, S["V"], (E, n_in)).astype(dt)
+    W = (rng.normal(17, S["W_w"], (n, n_in)) / np.sqrt(n_in)).astype(dt)
+    gE = rng.normal(17, S["G"], (N, n, dE)).astype(dt)
+    f8 = lambda a: np.asarray(a, dtype=np.float64)
+    w = f8(x) @ f8(W).T
+    Eenv = orc.env_embed(lmax, rp, f8(rvec), w, 0.8)
+    g_r, g_w = orc.env_embed_backward(lmax, rp, f8(gE), f8(rvec), w, 0.8)
+    g_x = g_w @ f8(W)
+    plan = ab.Plan(lmax, n, ab.F64 if dt == np.float64 else ab.F32)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    rpd, rd, xd, Wd, gEd = d(rp), d(rvec), d(x), d(W), d(gE)
+    E2 = ab.env_linear_forward(plan, rpd, rd, xd, Wd, 0.8)
+    gr2, gx2 = ab.env_linear_backward(plan, rpd, gEd, rd, xd, Wd, 0.8, torch.empty_like(rd), torch.empty_like(xd))
+    torch.cuda.synchronize()
+    _assert_close(dict(Eenv=Eenv, g_r=g_r, g_x=g_x), dict(Eenv=E2, g_r=gr2, g_x=gx2), dt, keys=("Eenv", "g_r", "g_x"), label="env_linear " + geom)
+    gr3, gx3 = torch.ones_like(rd), torch.ones_like(xd)
+    ab.env_linear_backward(plan, rpd, gEd, rd, xd, Wd, 0.8, gr3, gx3, accumulate_g_rvec=True, accumulate_g_x=True)
+    _assert_close(dict(g_r=g_r + 1.0, g_x=g_x + 1.0), dict(g_r=gr3, g_x=gx3), dt, keys=("g_r", "g_x"), label="env_linear accumulate " + geom)
