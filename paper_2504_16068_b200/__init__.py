@@ -44,6 +44,11 @@ SIGNATURES = {
     "allegro_tp_forward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp]),
     "allegro_tp_forward_aux": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp]),
     "allegro_tp_backward_aux": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
+    "allegro_tp_forward_outer": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
+    "allegro_tp_backward_outer": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t,
+                                            _vp]),
+    "allegro_edge_embed_factors": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp]),
+    "allegro_edge_embed_factors_backward": (C.c_int, [_vp, C.c_long, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, _vp, _vp, _vp]),
     "allegro_tp_forward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp]),
     "allegro_tp_backward": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp, C.c_size_t, _vp]),
     "allegro_tp_backward_energy": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_double, _vp, _vp, _vp, _vp,
@@ -264,6 +269,38 @@ def tp_backward_aux(plan, row_ptr, G, g_scalars, V, Eenv, path_w, gV, gEenv, ite
     _check(lib().allegro_tp_backward_aux(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(g_scalars), _ptr(V),
                                          _ptr(Eenv), _ptr(path_w), _ptr(gV), _ptr(gEenv), _ptr(workspace), workspace.numel(), _stream(stream)))
     return gV, gEenv
+
+
+def tp_forward_outer(plan, row_ptr, rvec, v0, Eenv, path_w, out, out_scalars=None, items=None, stream=None):
+    """dense tp_forward whose input V0 = v0 (x) Y(rhat) is generated on chip (layer-1 specialisation)"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    _check(lib().allegro_tp_forward_outer(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(rvec), _ptr(v0), _ptr(Eenv),
+                                          _ptr(path_w), _ptr(out), _ptr(out_scalars), _stream(stream)))
+    return out, out_scalars
+
+
+def tp_backward_outer(plan, row_ptr, G, g_scalars, rvec, v0, Eenv, path_w, g_v0, gY, gEenv, items=None, workspace=None, stream=None):
+    """VJP of tp_forward_outer: g_v0 [E, n], gY [E, dE] (the contractions of gV0 with Y and with v0), gEenv"""
+    n_atoms, n_edges = row_ptr.shape[0] - 1, rvec.shape[0]
+    if workspace is None:
+        workspace = _ws(tp_backward_workspace(plan, n_atoms, n_edges, items, False), rvec.device)
+    _check(lib().allegro_tp_backward_outer(plan.h, n_atoms, n_edges, _ptr(row_ptr), _ptr(items), _n_items(items), _ptr(G), _ptr(g_scalars), _ptr(rvec),
+                                           _ptr(v0), _ptr(Eenv), _ptr(path_w), _ptr(g_v0), _ptr(gY), _ptr(gEenv), _ptr(workspace), workspace.numel(),
+                                           _stream(stream)))
+    return g_v0, gY, gEenv
+
+
+def edge_embed_factors(plan, rvec, W_x0, W_v0, r_cut, x0, v0, stream=None):
+    _check(lib().allegro_edge_embed_factors(plan.h, rvec.shape[0], _ptr(rvec), _ptr(W_x0), _ptr(W_v0), W_x0.shape[1], float(r_cut), _ptr(x0), _ptr(v0),
+                                            _stream(stream)))
+    return x0, v0
+
+
+def edge_embed_factors_backward(plan, rvec, W_x0, W_v0, r_cut, g_x0, g_v0, gY, g_rvec, stream=None):
+    """g_rvec is accumulated into"""
+    _check(lib().allegro_edge_embed_factors_backward(plan.h, rvec.shape[0], _ptr(rvec), _ptr(W_x0), _ptr(W_v0), W_x0.shape[1], float(r_cut), _ptr(g_x0),
+                                                     _ptr(g_v0), _ptr(gY), _ptr(g_rvec), _stream(stream)))
+    return g_rvec
 
 
 def tp_forward_energy(plan, row_ptr, V, Eenv, path_w, q, kappa, items=None, want_out=True, want_e=True, want_G=True, out=None, e_edge=None,

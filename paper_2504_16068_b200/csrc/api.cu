@@ -363,6 +363,48 @@ allegro_status_t allegro_tp_backward_aux(const allegro_plan_t* plan, int n_atoms
     return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
 }
 
+allegro_status_t allegro_tp_forward_outer(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                          long n_items, const void* rvec, const void* v0, const void* Eenv, const void* path_w, void* out,
+                                          void* out_scalars, void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((rvec && v0 && out) || n_edges == 0, "rvec / v0 / out is NULL");
+    ALLEGRO_CHECK_ARG(Eenv || n_atoms == 0, "Eenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr && aligned16(path_w), "path_w is NULL or not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(aligned16(out) && aligned16(Eenv), "feature tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (!dense_tc_shape(plan)) {
+        set_error("allegro_tp_forward_outer: dense weights with fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.rvec = rvec; a.v0 = v0; a.Eenv = Eenv; a.path_w = path_w; a.out = out; a.scalars_out = out_scalars; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_forward, a);
+}
+
+allegro_status_t allegro_tp_backward_outer(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
+                                           long n_items, const void* G, const void* g_scalars, const void* rvec, const void* v0, const void* Eenv,
+                                           const void* path_w, void* g_v0, void* gY, void* gEenv, void* workspace, size_t workspace_bytes,
+                                           void* stream) {
+    ALLEGRO_CHECK_GRAPH();
+    ALLEGRO_CHECK_ARG((G && rvec && v0 && g_v0 && gY) || n_edges == 0, "G / rvec / v0 / g_v0 / gY is NULL");
+    ALLEGRO_CHECK_ARG((Eenv && gEenv) || n_atoms == 0, "Eenv / gEenv is NULL");
+    ALLEGRO_CHECK_ARG(path_w != nullptr && aligned16(path_w), "path_w is NULL or not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(aligned16(G) && aligned16(Eenv) && aligned16(gEenv) && aligned16(workspace), "tensor not 16-byte aligned");
+    ALLEGRO_CHECK_ARG(items == nullptr || n_items >= n_atoms, "n_items < n_atoms");
+    if (!dense_tc_shape(plan)) {
+        set_error("allegro_tp_backward_outer: dense weights with fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    TpArgs a{};
+    a.plan = plan; a.n = plan->n; a.n_atoms = n_atoms; a.n_edges = n_edges; a.row_ptr = row_ptr; a.items = items;
+    a.n_items = items ? n_items : (long)n_atoms;
+    a.G = G; a.g_scalars = g_scalars; a.rvec = rvec; a.v0 = v0; a.Eenv = Eenv; a.path_w = path_w; a.g_v0 = g_v0; a.gYe = gY; a.gEenv = gEenv;
+    a.ws = workspace; a.ws_bytes = workspace_bytes; a.st = (cudaStream_t)stream;
+    return ALLEGRO_DISPATCH(plan, launch_tp_backward, a);
+}
+
 allegro_status_t allegro_tp_forward_energy(const allegro_plan_t* plan, int n_atoms, long n_edges, const int32_t* row_ptr, const int32_t* items,
                                            long n_items, const void* V, const void* Eenv, const void* path_w, const void* q, double kappa,
                                            void* out, void* e_edge, void* G, void* stream) {
@@ -802,6 +844,25 @@ allegro_status_t allegro_edge_embed_backward(const allegro_plan_t* plan, long n_
     ALLEGRO_CHECK_ARG(W_x0 && W_v0 && n_basis >= 1 && r_cut > 0, "bad weights / n_basis / r_cut");
     ALLEGRO_CHECK_ARG(aligned16(gV0), "gV0 not 16-byte aligned");
     EmbedArgs a{plan->n, n_basis, r_cut, n_edges, rvec, W_x0, W_v0, nullptr, nullptr, g_x0, gV0, g_rvec, (cudaStream_t)stream};
+    return ALLEGRO_DISPATCH(plan, launch_edge_embed_backward, a);
+}
+allegro_status_t allegro_edge_embed_factors(const allegro_plan_t* plan, long n_edges, const void* rvec, const void* W_x0, const void* W_v0, int n_basis,
+                                            double r_cut, void* x0, void* v0, void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_edges >= 0, "plan is NULL or n_edges < 0");
+    ALLEGRO_CHECK_ARG((rvec && x0 && v0) || n_edges == 0, "NULL tensor");
+    ALLEGRO_CHECK_ARG(W_x0 && W_v0 && n_basis >= 1 && r_cut > 0, "bad weights / n_basis / r_cut");
+    EmbedArgs a{plan->n, n_basis, r_cut, n_edges, rvec, W_x0, W_v0, x0, nullptr, nullptr, nullptr, nullptr, (cudaStream_t)stream};
+    a.v0_out = v0;
+    return ALLEGRO_DISPATCH(plan, launch_edge_embed, a);
+}
+allegro_status_t allegro_edge_embed_factors_backward(const allegro_plan_t* plan, long n_edges, const void* rvec, const void* W_x0, const void* W_v0,
+                                                     int n_basis, double r_cut, const void* g_x0, const void* g_v0, const void* gY, void* g_rvec,
+                                                     void* stream) {
+    ALLEGRO_CHECK_ARG(plan != nullptr && n_edges >= 0, "plan is NULL or n_edges < 0");
+    ALLEGRO_CHECK_ARG((rvec && g_x0 && g_v0 && gY && g_rvec) || n_edges == 0, "NULL tensor");
+    ALLEGRO_CHECK_ARG(W_x0 && W_v0 && n_basis >= 1 && r_cut > 0, "bad weights / n_basis / r_cut");
+    EmbedArgs a{plan->n, n_basis, r_cut, n_edges, rvec, W_x0, W_v0, nullptr, nullptr, g_x0, nullptr, g_rvec, (cudaStream_t)stream};
+    a.g_v0 = g_v0; a.gYe = gY;
     return ALLEGRO_DISPATCH(plan, launch_edge_embed_backward, a);
 }
 allegro_status_t allegro_linear(long n_rows, int n_out, int n_in, allegro_dtype_t dtype, const void* x, const void* W, int transpose_w,

@@ -493,7 +493,7 @@ __device__ __forceinline__ void warp_copy(T* __restrict__ dst, const T* __restri
 
 template <typename T, int L, int NB>
 __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec, const T* __restrict__ W_x0,
-                                                          const T* __restrict__ W_v0, T* __restrict__ x0, T* __restrict__ V0) {
+                                                          const T* __restrict__ W_v0, T* __restrict__ x0, T* __restrict__ V0, T* __restrict__ v0_out) {
     constexpr int DE = (L + 1) * (L + 1), DV = 2 * DE;
     extern __shared__ __align__(16) unsigned char geo_raw[];
     GeoSmem<T, L, NB>& sm = *reinterpret_cast<GeoSmem<T, L, NB>*>(geo_raw);
@@ -525,16 +525,21 @@ __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double r
                 }
                 x0[e * n + ch] = (T)sx;
                 const T v0 = (T)sv;
-                T row[DV];
+                if (v0_out != nullptr) v0_out[e * n + ch] = v0;      // the factor alone (V0 = v0 (x) Y is generated on chip by its consumer)
+                if (V0 != nullptr) {
+                    T row[DV];
 #pragma unroll
-                for (int k = 0; k < DV; ++k) row[k] = T(0);
+                    for (int k = 0; k < DV; ++k) row[k] = T(0);
 #pragma unroll
-                for (int j = 0; j < DE; ++j) row[natural_slot<L>(j)] = v0 * sm.Ys[le][j];
-                row_store<T, DV>(stg + lane * DV, row);
+                    for (int j = 0; j < DE; ++j) row[natural_slot<L>(j)] = v0 * sm.Ys[le][j];
+                    row_store<T, DV>(stg + lane * DV, row);
+                }
             }
-            __syncwarp();
-            warp_copy<T>(V0 + (e * n + ch0) * DV, stg, min(32, n - ch0) * DV, lane);
-            __syncwarp();
+            if (V0 != nullptr) {
+                __syncwarp();
+                warp_copy<T>(V0 + (e * n + ch0) * DV, stg, min(32, n - ch0) * DV, lane);
+                __syncwarp();
+            }
         }
     }
 }
@@ -543,7 +548,10 @@ __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double r
 template <typename T, int L, int NB>
 __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec,
                                                               const T* __restrict__ W_x0, const T* __restrict__ W_v0, const T* __restrict__ g_x0,
-                                                              const T* __restrict__ gV0, T* __restrict__ g_rvec) {
+                                                              const T* __restrict__ gV0, T* __restrict__ g_rvec, const T* __restrict__ g_v0c,
+                                                              const T* __restrict__ gYc) {
+    // gV0 == NULL: the cotangent of V0 = v0 (x) Y arrives already contracted (allegro_tp_backward_outer): g_v0c[e][ch] = <gV0[e][ch], Y>,
+    // gYc[e][j] = sum_ch gV0[e][ch][slot j] v0[e][ch]
     constexpr int DE = (L + 1) * (L + 1), DV = 2 * DE;
     static_assert(DE <= 16 && NB <= 16, "warp_reduce16");
     extern __shared__ __align__(16) unsigned char geo_raw[];
@@ -568,22 +576,27 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
 #pragma unroll
         for (int j = 0; j < 16; ++j) { gYp[j] = T(0); gbp[j] = 0.0; }
         for (int ch0 = 0; ch0 < n; ch0 += 32) {
-            __syncwarp();
-            warp_copy<T>(stg, gV0 + (e * n + ch0) * DV, min(32, n - ch0) * DV, lane);
-            __syncwarp();
-            const int ch = ch0 + lane;
-            if (ch >= n) continue;
-            T row[DV];
-            row_load<T, DV>(stg + lane * DV, row);
-            double sv = 0.0;
-            for (int b = 0; b < nb; ++b) sv = fma(Wvs[b * n + ch], sm.Bs[le][b], sv);
-            const T v0 = (T)sv;
             T gv0 = T(0);
+            const int ch = ch0 + lane;
+            if (gV0 != nullptr) {
+                __syncwarp();
+                warp_copy<T>(stg, gV0 + (e * n + ch0) * DV, min(32, n - ch0) * DV, lane);
+                __syncwarp();
+                if (ch >= n) continue;
+                T row[DV];
+                row_load<T, DV>(stg + lane * DV, row);
+                double sv = 0.0;
+                for (int b = 0; b < nb; ++b) sv = fma(Wvs[b * n + ch], sm.Bs[le][b], sv);
+                const T v0 = (T)sv;
 #pragma unroll
-            for (int j = 0; j < DE; ++j) {
-                const T gj = row[natural_slot<L>(j)];
-                gv0 = fma(gj, sm.Ys[le][j], gv0);
-                gYp[j] = fma(gj, v0, gYp[j]);
+                for (int j = 0; j < DE; ++j) {
+                    const T gj = row[natural_slot<L>(j)];
+                    gv0 = fma(gj, sm.Ys[le][j], gv0);
+                    gYp[j] = fma(gj, v0, gYp[j]);
+                }
+            } else {
+                if (ch >= n) continue;
+                gv0 = g_v0c[e * n + ch];
             }
             const double gx = (double)g_x0[e * n + ch];
 #pragma unroll
@@ -595,6 +608,10 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
         T gY[DE];
 #pragma unroll
         for (int j = 0; j < DE; ++j) gY[j] = __shfl_sync(0xffffffffu, gYp[0], 2 * j);
+        if (gV0 == nullptr) {
+#pragma unroll
+            for (int j = 0; j < DE; ++j) gY[j] = gYc[e * DE + j];
+        }
         double rad = 0.0;
 #pragma unroll
         for (int b = 0; b < NB; ++b) {

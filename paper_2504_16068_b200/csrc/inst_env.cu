@@ -140,7 +140,8 @@ allegro_status_t launch_edge_embed<ALLEGRO_T, ALLEGRO_L>(const EmbedArgs& a) {
         auto k = edge_embed_kernel<T, ALLEGRO_L, NB>;                                                                       \
         const size_t smem = (sizeof(GeoSmem<T, ALLEGRO_L, NB>) + 15) / 16 * 16 + 8 * 32 * 2 * (ALLEGRO_L + 1) * (ALLEGRO_L + 1) * sizeof(T) + (size_t)2 * a.nb * a.n * sizeof(double); \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
-        k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0, (T*)a.x0, (T*)a.V0); \
+        k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0, (T*)a.x0, (T*)a.V0, \
+                                     (T*)a.v0_out); \
     }
     if (a.nb <= 8) ALLEGRO_EMB(8) else ALLEGRO_EMB(16)
 #undef ALLEGRO_EMB
@@ -163,7 +164,7 @@ allegro_status_t launch_edge_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EmbedArg
         const size_t smem = (sizeof(GeoSmem<T, ALLEGRO_L, NB>) + 15) / 16 * 16 + 8 * 32 * 2 * (ALLEGRO_L + 1) * (ALLEGRO_L + 1) * sizeof(T) + (size_t)2 * a.nb * a.n * sizeof(double); \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
         k<<<grid, 256, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0,     \
-                                     (const T*)a.g_x0, (const T*)a.gV0, (T*)a.g_rvec);                                     \
+                                     (const T*)a.g_x0, (const T*)a.gV0, (T*)a.g_rvec, (const T*)a.g_v0, (const T*)a.gYe);   \
     }
     if (a.nb <= 8) ALLEGRO_EMBB(8) else ALLEGRO_EMBB(16)
 #undef ALLEGRO_EMBB

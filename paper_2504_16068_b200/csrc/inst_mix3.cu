@@ -39,13 +39,24 @@ static allegro_status_t mix3_unsupported(const allegro_plan* plan) {
 }
 
 #if ALLEGRO_MIX3_PART == 0
+static allegro_status_t mix3_fwd_launch_outer(const TpArgs& a, const float* img_f) {
+    constexpr uint32_t PMASK = Mix3::mask_natural_in();
+    auto k = mix3_fwd_kernel<PMASK, true>;
+    constexpr int SMEM = Mix3Seq<PMASK>::SMEM;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
+    k<<<(unsigned)a.n_items, Mix3::CT + 64, SMEM, a.st>>>(a.row_ptr, a.items, nullptr, (const float*)a.Eenv, img_f, (float*)a.out, (const float*)a.q,
+                                                          (float)a.kappa, (float*)a.e_edge, (float*)a.scalars_out, (const float*)a.rvec,
+                                                          (const float*)a.v0);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
 template <uint32_t PMASK>
 static allegro_status_t mix3_fwd_launch(const TpArgs& a, const float* img_f) {
     auto k = mix3_fwd_kernel<PMASK>;
     constexpr int SMEM = Mix3Seq<PMASK>::SMEM;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM));
     k<<<(unsigned)a.n_items, Mix3::CT + 64, SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.V, (const float*)a.Eenv, img_f, (float*)a.out,
-                                                          (const float*)a.q, (float)a.kappa, (float*)a.e_edge, (float*)a.scalars_out);
+                                                          (const float*)a.q, (float)a.kappa, (float*)a.e_edge, (float*)a.scalars_out, nullptr, nullptr);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -55,6 +66,10 @@ allegro_status_t launch_mix3_forward_f32_l2_n64(const TpArgs& a) {
     float *img_f, *img_b;
     allegro_status_t s = mix3_images(a, &img_f, &img_b);
     if (s != ALLEGRO_OK) return s;
+    if (a.v0 != nullptr) {
+        if (var != 2) { set_error("tp_forward_outer: the plan must be restricted to the natural-parity input blocks (set_in_blocks(0x19))"); return ALLEGRO_EINVAL; }
+        return mix3_fwd_launch_outer(a, img_f);
+    }
     return var == 0 ? mix3_fwd_launch<Mix3::ALL>(a, img_f)
            : var == 1 ? mix3_fwd_launch<Mix3::mask_into(0)>(a, img_f)
                       : mix3_fwd_launch<Mix3::mask_natural_in()>(a, img_f);
@@ -65,7 +80,17 @@ static allegro_status_t mix3_bwd_launch(const TpArgs& a, const float* img_b, flo
     auto k = mix3_bwd_kernel<GV, PMASK, COT>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
     k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, (const float*)a.V, (const float*)a.Eenv, img_b,
-                                                                (float*)a.gV, gE_dst, gE_by_item, (const float*)a.q, (float)a.kappa, (const float*)a.g_scalars);
+                                                                (float*)a.gV, gE_dst, gE_by_item, (const float*)a.q, (float)a.kappa, (const float*)a.g_scalars, nullptr, nullptr,
+                                                                nullptr, nullptr);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+static allegro_status_t mix3_bwd_launch_outer(const TpArgs& a, const float* img_b, float* gE_dst, int gE_by_item) {
+    auto k = mix3_bwd_kernel<true, Mix3::mask_natural_in(), false, true>;
+    ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, Mix3B::SMEM));
+    k<<<(unsigned)a.n_items, Mix3B::CT + 64, Mix3B::SMEM, a.st>>>(a.row_ptr, a.items, (const float*)a.G, nullptr, (const float*)a.Eenv, img_b, nullptr,
+                                                                gE_dst, gE_by_item, nullptr, 0.f, (const float*)a.g_scalars, (const float*)a.rvec,
+                                                                (const float*)a.v0, (float*)a.g_v0, (float*)a.gYe);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
@@ -81,6 +106,10 @@ allegro_status_t launch_mix3_backward_f32_l2_n64(const TpArgs& a, float* gE_dst,
     float *img_f, *img_b;
     allegro_status_t s = mix3_images(a, &img_f, &img_b);
     if (s != ALLEGRO_OK) return s;
+    if (a.v0 != nullptr) {
+        if (var != 2) { set_error("tp_backward_outer: the plan must be restricted to the natural-parity input blocks (set_in_blocks(0x19))"); return ALLEGRO_EINVAL; }
+        return mix3_bwd_launch_outer(a, img_b, gE_dst, gE_by_item);
+    }
     return var == 0 ? mix3_bwd_pick<Mix3::ALL>(a, img_b, gE_dst, gE_by_item)
            : var == 1 ? mix3_bwd_pick<Mix3::mask_into(0)>(a, img_b, gE_dst, gE_by_item)
                       : mix3_bwd_pick<Mix3::mask_natural_in()>(a, img_b, gE_dst, gE_by_item);

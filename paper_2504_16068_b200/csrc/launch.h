@@ -91,6 +91,11 @@ struct TpArgs {
     // dense mode, fp32 / l_max 2 / n 64 only (allegro_tp_forward_aux / _backward_aux): compact side channel of the 0e scalars
     void* scalars_out;      // forward: T[E][n] copy of out[:, :, 0e]
     const void* g_scalars;  // backward: T[E][n] added to G[:, :, 0e]
+    // layer-1 specialisation (allegro_tp_forward_outer / _backward_outer): V = v0 (x) Y(rhat) generated on chip, V == NULL
+    const void* rvec;       // T[E][3]
+    const void* v0;         // T[E][n]
+    void* g_v0;             // backward: T[E][n]
+    void* gYe;              // backward: T[E][dE]
 };
 
 struct EmbedArgs {
@@ -106,6 +111,9 @@ struct EmbedArgs {
     const void* gV0;
     void* g_rvec;      // backward: accumulated into
     cudaStream_t st;
+    void* v0_out;      // forward, nullable: the factor v0[e][n] of V0 = v0 (x) Y (V0 itself is then optional)
+    const void* g_v0;  // backward, with gV0 == NULL: <gV0[e][n], Y(e)>            (allegro_tp_backward_outer)
+    const void* gYe;   // backward, with gV0 == NULL: sum_n gV0[e][n][slot j] v0[e][n]
 };
 template <typename T, int L> allegro_status_t launch_edge_embed(const EmbedArgs& a);
 template <typename T, int L> allegro_status_t launch_edge_embed_backward(const EmbedArgs& a);

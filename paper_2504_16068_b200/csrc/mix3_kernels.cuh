@@ -119,6 +119,18 @@ struct Mix3Seq {
     static_assert(count() >= 2, "at least two paths");
 };
 
+// OUTER mode (layer-1 specialisation): the input features are not read from HBM but generated on chip as the outer product
+// V0[e][n][(l, (-1)^l), m] = v0[e][n] Y_lm(rhat_e) of reading A19 (other-parity slots zero).  Y for l <= 2 in the convention of reading
+// A1 (real, component-normalised, m = -l..l; Y_1 = sqrt3 (y, z, x)), index j = l^2 + l + m; feature slot of j: 0e -> 0, 1o -> 5..7, 2e -> 8..12.
+__device__ __forceinline__ void mix3_sph9(float x, float y, float z, float (&Y)[9]) {
+    const float s3 = 1.7320508075688772f, s15 = 3.8729833462074170f, s5h = 1.1180339887498949f;
+    Y[0] = 1.f;
+    Y[1] = s3 * y; Y[2] = s3 * z; Y[3] = s3 * x;
+    Y[4] = s15 * x * y; Y[5] = s15 * y * z; Y[6] = s5h * (3.f * z * z - 1.f); Y[7] = s15 * x * z; Y[8] = 0.5f * s15 * (x * x - y * y);
+}
+__host__ __device__ constexpr int mix3_nat_slot(int j) { return j == 0 ? 0 : j < 4 ? 4 + j : 4 + j; }   // j 1..3 -> 5..7, j 4..8 -> 8..12
+__host__ __device__ constexpr int mix3_nat_j(int slot) { return slot == 0 ? 0 : slot - 4; }             // inverse on the natural slots
+
 // position in a ring of NST stages: stage index and the phase bit of the current turn
 template <int NST>
 struct RingPos {
@@ -158,12 +170,14 @@ __device__ __forceinline__ float tf32_lo(float x) { return x - __uint_as_float(_
 // from the rows while they are in registers; `out` may then be NULL (the rows are never stored: a last layer whose output feeds
 // only the readout).  s_out (nullable, [E][64]): compact copy of the 0e scalars out[e][n'][0], what a scalar latent update reads
 // (as a 72-byte-strided gather from `out` it costs 8 x the sectors).
-template <uint32_t PMASK>
+// OUTER: V is not read; the rows are generated from rvec [E][3] and v0 [E][64] (see mix3_sph9).
+template <uint32_t PMASK, bool OUTER = false>
 __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                    const float* __restrict__ V, const float* __restrict__ Eenv,
                                                                    const float* __restrict__ img, float* __restrict__ out,
                                                                    const float* __restrict__ qvec, float kappa, float* __restrict__ e_edge,
-                                                                   float* __restrict__ s_out) {
+                                                                   float* __restrict__ s_out, const float* __restrict__ rvec = nullptr,
+                                                                   const float* __restrict__ v0 = nullptr) {
     using M3 = Mix3;
     using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
@@ -274,14 +288,26 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
             const int eb = e0 + t * TE;
             bool stg_busy = t > 0;
             MIX3_T0();
-            if (tid == 0 && eb + TE < e1)     // the next tile's V rows (one contiguous range) are pulled into L2 while this tile computes
+            if (!OUTER && tid == 0 && eb + TE < e1)     // the next tile's V rows (one contiguous range) are pulled into L2 while this tile computes
                 bulk_prefetch_l2(V + (size_t)(eb + TE) * 64 * DV, (uint32_t)min(TE, e1 - eb - TE) * 64 * DV * 4);
             float Vr[M3::EPS][DV];
 #pragma unroll
             for (int i = 0; i < M3::EPS; ++i) {
                 const int e = eb + 4 * slot + i;
                 if (e < e1) {
-                    row_load<float, DV>(V + ((size_t)e * 64 + ch) * DV, Vr[i]);
+                    if constexpr (OUTER) {
+                        const float rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+                        const float inv = 1.f / sqrtf(rx * rx + ry * ry + rz * rz);
+                        float Y[9];
+                        mix3_sph9(rx * inv, ry * inv, rz * inv, Y);
+                        const float v = v0[(size_t)e * 64 + ch];
+#pragma unroll
+                        for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
+#pragma unroll
+                        for (int j = 0; j < 9; ++j) Vr[i][mix3_nat_slot(j)] = v * Y[j];
+                    } else {
+                        row_load<float, DV>(V + ((size_t)e * 64 + ch) * DV, Vr[i]);
+                    }
                 } else {
 #pragma unroll
                     for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
@@ -422,7 +448,8 @@ struct Mix3B {
     static constexpr int G_ATOM = ROWS * 128, G_VAR = 2 * G_ATOM, G_BYTES = 2 * G_VAR;   // hi, lo: [2 K-atoms][288 rows][128 B]
     static constexpr int A_BYTES = 2 * 128 * 128, NA = 2, ND = 3;   // 30 paths = 10 turns of the accumulator ring: slot and parity depend on p only
     static constexpr int OFF_G = 0, OFF_A = G_BYTES, OFF_BAR = OFF_A + NA * A_BYTES;
-    static constexpr int SMEM = OFF_BAR + 256 + 1024;
+    static constexpr int OFF_YS = OFF_BAR + 256;                    // OUTER mode: Y_j(rhat_e) of the tile's edges, [TE][9] floats
+    static constexpr int SMEM = OFF_YS + 640 + 1024;
     // first row of a block's B operand, indexed by off3
     __host__ __device__ static constexpr int rowoff(int off3) {
         return off3 == 0 ? 0 : off3 == 1 ? 16 : off3 == 2 ? 32 : off3 == 5 ? 80 : off3 == 8 ? 128 : 208;
@@ -444,12 +471,18 @@ struct Mix3BBars {
 // COT: G points at the forward result `out` and the cotangent of the A12 energy, q (x) delta_{k,0} + kappa out, is formed while the
 // tile is staged (G never exists in HBM).  g_s (nullable, [E][64]): a compact cotangent of the 0e scalars that is ADDED to
 // G[e][n'][0] while the tile is staged (the scalar latent update's VJP writes it; G itself is not modified).
-template <bool WANT_GV, uint32_t PMASK, bool COT>
+// OUTER (layer-1 specialisation): V = v0 (x) Y(rhat) is generated on chip from rvec [E][3] and v0 [E][64] (see mix3_sph9) and gV is not
+// stored: it is contracted at once into g_v0[e][n] = sum_j gV[e][n][slot j] Y_j(rhat_e) ([E][64]) and gYe[e][j] = sum_n gV[e][n][slot j]
+// v0[e][n] ([E][9]; lanes by a fixed xor tree, the four lane quarters in order), what the edge embedding's VJP needs.
+template <bool WANT_GV, uint32_t PMASK, bool COT, bool OUTER = false>
 __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* __restrict__ row_ptr, const int* __restrict__ items,
                                                                     const float* __restrict__ G, const float* __restrict__ V,
                                                                     const float* __restrict__ Eenv, const float* __restrict__ img,
                                                                     float* __restrict__ gV, float* __restrict__ gE_dst, int gE_by_item,
-                                                                    const float* __restrict__ qvec, float kappa, const float* __restrict__ g_s) {
+                                                                    const float* __restrict__ qvec, float kappa, const float* __restrict__ g_s,
+                                                                    const float* __restrict__ rvec = nullptr, const float* __restrict__ v0 = nullptr,
+                                                                    float* __restrict__ g_v0 = nullptr, float* __restrict__ gYe = nullptr) {
+    static_assert(!OUTER || (WANT_GV && PMASK == Mix3::mask_natural_in()), "OUTER mode: natural-parity input paths, gV accumulated");
     using MB = Mix3B;
     using SQ = Mix3Seq<PMASK>;
     using Gen = TPGen<2>;
@@ -548,7 +581,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
             if (tid == 0 && eb + TE < e1) {   // the next tile's cotangent and V rows are pulled into L2 while this tile computes
                 const uint32_t nb = (uint32_t)min(TE, e1 - eb - TE) * 64 * DV * 4;
                 if (G != nullptr) bulk_prefetch_l2(G + (size_t)(eb + TE) * 64 * DV, nb);
-                bulk_prefetch_l2(V + (size_t)(eb + TE) * 64 * DV, nb);
+                if (!OUTER) bulk_prefetch_l2(V + (size_t)(eb + TE) * 64 * DV, nb);
             }
             // (a) cotangent tile -> B operands of all six blocks (hi, lo)
 #pragma unroll
@@ -590,6 +623,33 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
             // hold the gV accumulators; each path reads back only the (l1, p1) block it contracts
             float gv[4][DV];
             const uint32_t vrow = tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(MB::VCOL + 72 * wq);
+            [[maybe_unused]] float v0r[4];
+            [[maybe_unused]] const float* Ys = reinterpret_cast<const float*>(sm + MB::OFF_YS);
+            if constexpr (OUTER) {
+                if (tid < TE) {      // Y_j of the tile's edges, once per tile
+                    float* Yw = reinterpret_cast<float*>(sm + MB::OFF_YS) + tid * 9;
+                    const int e = eb + tid;
+                    float Y[9];
+                    if (e < e1) {
+                        const float rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+                        const float inv = 1.f / sqrtf(rx * rx + ry * ry + rz * rz);
+                        mix3_sph9(rx * inv, ry * inv, rz * inv, Y);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 9; ++j) Y[j] = 0.f;
+                    }
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) Yw[j] = Y[j];
+                }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int e = eb + 8 * wq + 4 * h + i;
+                    v0r[i] = e < e1 ? v0[(size_t)e * 64 + n] : 0.f;
+#pragma unroll
+                    for (int k = 0; k < DV; ++k) gv[i][k] = 0.f;
+                }
+                named_bar(1, MB::CT);   // Ys visible to every compute warp
+            } else {
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
                 const int e = eb + 8 * wq + 4 * h + i;
@@ -610,6 +670,7 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
                 for (int k = 0; k < DV; ++k) gv[i][k] = 0.f;
             }
             tc05::tmem_st_wait();
+            }
             // (c) paths: consume every accumulator as soon as it is complete
             static_for3<0, NP>([&](auto kc) {
                 constexpr int p = SQ::path(decltype(kc)::value);
@@ -627,7 +688,10 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
                 float Vb[4][DV];   // only components o1 .. o1 + w1 - 1 are read by this path's code
 #pragma unroll
                 for (int i = 0; i < 4; ++i) {
-                    if constexpr (w1 == 1) {
+                    if constexpr (OUTER) {
+#pragma unroll
+                        for (int k = 0; k < w1; ++k) Vb[i][o1 + k] = v0r[i] * Ys[(8 * wq + 4 * h + i) * 9 + mix3_nat_j(o1 + k)];
+                    } else if constexpr (w1 == 1) {
                         uint32_t x[1];
                         tc05::tmem_ld1(vrow + (uint32_t)(18 * i + o1), x);
                         Vb[i][o1] = __uint_as_float(x[0]);
@@ -663,8 +727,32 @@ __global__ void __launch_bounds__(Mix3B::CT + 64, 1) mix3_bwd_kernel(const int* 
                     Pth::template bwd<float, WANT_GV>(Vb[i], E, gt, gv[i], gE);
                 }
             });
-            // (d) gV rows: staged per warp in the (now idle) operand region, stored as coalesced 16-byte vectors
-            if constexpr (WANT_GV) {
+            // (d) OUTER: gV is contracted with Y (-> g_v0) and with v0 over the 64 channels (-> gYe) instead of being stored
+            if constexpr (OUTER) {
+                float* redY = reinterpret_cast<float*>(sm + MB::OFF_G);   // [4 lane quarters][TE][9] in the (now idle) operand region
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const int el = 8 * wq + 4 * h + i, e = eb + el;
+                    float sv = 0.f;
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) sv = fmaf(gv[i][mix3_nat_slot(j)], Ys[el * 9 + j], sv);
+                    if (e < e1) g_v0[(size_t)e * 64 + n] = sv;
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) {
+                        float pj = gv[i][mix3_nat_slot(j)] * v0r[i];
+#pragma unroll
+                        for (int o = 8; o > 0; o >>= 1) pj += __shfl_xor_sync(0xffffffffu, pj, o);
+                        if (nl == 0) redY[(q * TE + el) * 9 + j] = pj;
+                    }
+                }
+                named_bar(1, MB::CT);
+                if (tid < TE * 9) {
+                    const int el = tid / 9, j = tid - el * 9;
+                    if (eb + el < e1)
+                        gYe[(size_t)(eb + el) * 9 + j] = ((redY[(0 * TE + el) * 9 + j] + redY[(1 * TE + el) * 9 + j]) + redY[(2 * TE + el) * 9 + j]) +
+                                                         redY[(3 * TE + el) * 9 + j];
+                }
+            } else if constexpr (WANT_GV) {
                 float* stg = reinterpret_cast<float*>(sm + MB::OFF_G) + warp * (8 * 16 * DV);
 #pragma unroll
                 for (int i = 0; i < 4; ++i) row_store<float, DV>(stg + ((4 * h + i) * 16 + nl) * DV, gv[i]);

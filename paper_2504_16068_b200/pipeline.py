@@ -332,6 +332,9 @@ class TwoLayerStep:
         # the last layer's VJP, so V_L is never stored (default: whenever the tcgen05 kernels serve the shape and plan_last is given)
         tc = plan_dense.dtype == ab.F32 and plan_dense.l_max == 2 and plan_dense.n == 64
         self.fuse_readout = (tc and plan_last is not None) if fuse_readout is None else (fuse_readout and tc)
+        # layer-1 specialisation: V_0 = v0 (x) Y is generated on chip by the first layer's kernels (never stored), its cotangent arrives
+        # contracted (g_v0, gY); needs the tensor-core kernels and a first-layer plan restricted to the natural-parity input blocks
+        self.outer = tc and plan_first is not None and factorised_env and params["W_w"].shape[0] > 1
         self.factorised_env = factorised_env      # env-embed of the linear weights without forming w (False: linear + env_embed, the named calls)
         self.tc = tc      # tensor-core dense kernels: the 0e scalars travel between the layers in compact [E, n] side arrays
         self.pd_last = plan_last if plan_last is not None else plan_dense
@@ -345,6 +348,9 @@ class TwoLayerStep:
         self.x = [new(E, n) for _ in range(L)]            # x_0 .. x_{L-1}
         self.z = [new(E, n) for _ in range(L - 1)]
         self.V = [new(E, n, dV) for _ in range(L)] + [None if self.fuse_readout else new(E, n, dV)]    # V_0 .. V_L
+        if self.outer:
+            self.V[0] = None
+            self.v0, self.g_v0, self.gY = new(E, n), new(E, n), new(E, plan_dense.dE)
         self.w = [new(E, n) for _ in range(L)]
         self.Eenv = [new(N, n, plan_dense.dE) for _ in range(L)]
         self.gEenv = new(N, n, plan_dense.dE)
@@ -373,7 +379,10 @@ class TwoLayerStep:
             ev.append((name, a, b))
             return r
 
-        timed("edge_embed", lambda: ab.edge_embed(pd, rvec, p["W_x0"], p["W_v0"], rc, x0=self.x[0], V0=self.V[0]))
+        if self.outer:
+            timed("edge_embed", lambda: ab.edge_embed_factors(pd, rvec, p["W_x0"], p["W_v0"], rc, self.x[0], self.v0))
+        else:
+            timed("edge_embed", lambda: ab.edge_embed(pd, rvec, p["W_x0"], p["W_v0"], rc, x0=self.x[0], V0=self.V[0]))
         for l in range(L):
             if self.factorised_env:      # w = W_w x is never formed: the linear map is applied once per centre (allegro_env_linear_forward)
                 timed("env_linear_forward", lambda: ab.env_linear_forward(ps, rp, rvec, self.x[l], p["W_w"][l], scale, Eenv=self.Eenv[l]))
@@ -384,6 +393,8 @@ class TwoLayerStep:
             if l == L - 1 and self.fuse_readout:
                 timed("tp_forward_dense", lambda: ab.tp_forward_energy(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, want_out=False,
                                                                        want_G=False, e_edge=self.e_edge))
+            elif self.outer and l == 0 and l < L - 1:
+                timed("tp_forward_dense", lambda: ab.tp_forward_outer(pl, rp, rvec, self.v0, self.Eenv[l], p["W_p"][l], self.V[l + 1], self.s[l]))
             elif self.tc and l < L - 1:
                 timed("tp_forward_dense", lambda: ab.tp_forward_aux(pl, rp, self.V[l], self.Eenv[l], p["W_p"][l], self.V[l + 1], self.s[l]))
             else:
@@ -412,6 +423,9 @@ class TwoLayerStep:
             if l == L - 1 and fused_cot:
                 timed("tp_backward_dense", lambda: ab.tp_backward_energy(pl, rp, self.V[L], self.V[l], self.Eenv[l], p["W_p"][l], p["q"], 0.0, gV=gVl,
                                                                          gEenv=self.gEenv, workspace=self.ws))
+            elif self.outer and l == 0 and l < L - 1:
+                timed("tp_backward_dense", lambda: ab.tp_backward_outer(pl, rp, G, self.gs, rvec, self.v0, self.Eenv[l], p["W_p"][l], self.g_v0, self.gY,
+                                                                        self.gEenv, workspace=self.ws))
             elif self.tc and l < L - 1:
                 timed("tp_backward_dense", lambda: ab.tp_backward_aux(pl, rp, G, self.gs, self.V[l], self.Eenv[l], p["W_p"][l], gVl, self.gEenv,
                                                                       workspace=self.ws))
@@ -437,7 +451,10 @@ class TwoLayerStep:
                 else:
                     timed("linear", lambda: ab.linear(self.g_w, p["W_w"][l], transpose_w=True, y=g_x, accumulate=True))
             G, g_x_next = gVl, g_x
-        timed("edge_embed_backward", lambda: ab.edge_embed_backward(pd, rvec, p["W_x0"], p["W_v0"], rc, g_x_next, G, self.g_r))
+        if self.outer and L > 1:
+            timed("edge_embed_backward", lambda: ab.edge_embed_factors_backward(pd, rvec, p["W_x0"], p["W_v0"], rc, g_x_next, self.g_v0, self.gY, self.g_r))
+        else:
+            timed("edge_embed_backward", lambda: ab.edge_embed_backward(pd, rvec, p["W_x0"], p["W_v0"], rc, g_x_next, G, self.g_r))
         if self.sharded is None:
             timed("force_gather", lambda: ab.force_gather(rp, d["rev"], self.g_r, F=self.F))
             timed("segment_sum", lambda: ab.segment_sum(self.e_ptr, self.e_edge, out=self.e_tot))

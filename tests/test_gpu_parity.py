@@ -984,3 +984,57 @@ def test_env_linear_forward_and_vjp(geom, lmax, n, n_in, dt):
     gr3, gx3 = torch.ones_like(rd), torch.ones_like(xd)
     ab.env_linear_backward(plan, rpd, gEd, rd, xd, Wd, 0.8, gr3, gx3, accumulate_g_rvec=True, accumulate_g_x=True)
     _assert_close(dict(g_r=g_r + 1.0, g_x=g_x + 1.0), dict(g_r=gr3, g_x=gx3), dt, keys=("g_r", "g_x"), label="env_linear accumulate " + geom)
+
+
+def test_layer1_outer_product_input():
+    """allegro_tp_forward_outer / _backward_outer / allegro_edge_embed_factors(_backward): the first layer with its input
+    V0 = v0 (x) Y(rhat) generated on chip equals the same layer fed with the materialised V0 (allegro_edge_embed -> allegro_tp_forward /
+    _backward), and the contracted cotangents g_v0, gY equal the contractions of that path's gV with the ORACLE's Y_lm; then the
+    embedding's VJP from the factors equals the one from gV0"""
+    import oracle as orc
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs, rng
+    lmax, n, dt = 2, 64, np.float32
+    g = configs.geometry_for("C1s")
+    rp, rvec = g["row_ptr"], g["rvec"].astype(dt)
+    E, N = rvec.shape[0], rp.shape[0] - 1
+    S = rng.STREAMS
+    W_x0 = (rng.normal(19, S["W_x0"], (n, 8)) / np.sqrt(8)).astype(dt)
+    W_v0 = (rng.normal(19, S["W_v0"], (n, 8)) / np.sqrt(8)).astype(dt)
+    Ee = (rng.normal(19, S["W_w"], (N, n, 9)) * 0.5).astype(dt)
+    W = (rng.normal(19, S["W_p"], (30, n, n)) / np.sqrt(n)).astype(dt)
+    G = rng.normal(19, S["G"], (E, n, 18)).astype(dt)
+    gs = rng.normal(20, S["q"], (E, n, 1)).astype(dt)
+    g_x0 = rng.normal(21, S["q"], (E, n)).astype(dt)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    rpd, rd, Ed, Wd, Gd, gsd, Wx, Wv, gx0 = d(rp), d(rvec), d(Ee), d(W), d(G), d(gs), d(W_x0), d(W_v0), d(g_x0)
+    plan = ab.Plan(lmax, n, ab.F32, ab.W_DENSE)
+    plan.set_in_blocks(0x19)
+    rc = 6.0
+    # materialised path
+    x0, V0 = ab.edge_embed(plan, rd, Wx, Wv, rc)
+    out_a, sc_a = torch.empty_like(V0), torch.empty((E, n, 1), dtype=V0.dtype, device="cuda")
+    ab.tp_forward_aux(plan, rpd, V0, Ed, Wd, out_a, sc_a)
+    gV_a, gE_a = ab.tp_backward_aux(plan, rpd, Gd, gsd, V0, Ed, Wd, torch.empty_like(V0), torch.empty_like(Ed))
+    gr_a = torch.zeros_like(rd)
+    ab.edge_embed_backward(plan, rd, Wx, Wv, rc, gx0, gV_a, gr_a)
+    # on-chip path
+    x0b, v0 = ab.edge_embed_factors(plan, rd, Wx, Wv, rc, torch.empty_like(x0), torch.empty_like(x0))
+    assert torch.equal(x0b, x0)
+    out_b, sc_b = torch.empty_like(V0), torch.empty_like(sc_a)
+    ab.tp_forward_outer(plan, rpd, rd, v0, Ed, Wd, out_b, sc_b)
+    g_v0, gY, gE_b = ab.tp_backward_outer(plan, rpd, Gd, gsd, rd, v0, Ed, Wd, torch.empty_like(x0), torch.empty((E, 9), dtype=V0.dtype, device="cuda"),
+                                          torch.empty_like(Ed))
+    gr_b = torch.zeros_like(rd)
+    ab.edge_embed_factors_backward(plan, rd, Wx, Wv, rc, gx0, g_v0, gY, gr_b)
+    torch.cuda.synchronize()
+    Y = np.stack([orc.sph_harm(lmax, rvec[e].astype(np.float64))[0] for e in range(E)])
+    slots = [0, 5, 6, 7, 8, 9, 10, 11, 12]
+    gVn = gV_a.double().cpu().numpy()[:, :, slots]
+    ref = dict(out=out_a, sc=sc_a, gEenv=gE_a, g_r=gr_a, g_v0=np.einsum("enj,ej->en", gVn, Y),
+               gY=np.einsum("enj,en->ej", gVn, v0.double().cpu().numpy()))
+    ref = {k: (v.double().cpu().numpy() if hasattr(v, "cpu") else v) for k, v in ref.items()}
+    got = dict(out=out_b, sc=sc_b, gEenv=gE_b, g_r=gr_b, g_v0=g_v0, gY=gY)
+    _assert_close(ref, got, dt, keys=tuple(ref.keys()), label="layer-1 outer")
