@@ -630,4 +630,56 @@ __global__ void __launch_bounds__(256) edge_embed_bwd_kernel(int n, int nb, doub
     }
 }
 
+// VJP of the edge embedding from the FACTORS of the cotangent of V0 = v0 (x) Y (allegro_edge_embed_factors_backward): thread per edge,
+//   g_b[b] = sum_ch ( g_x0[e][ch] W_x0[ch][b] + g_v0[e][ch] W_v0[ch][b] ),   g_rvec[e] += (sum_b g_b dBu_b/dr) rhat_e + proj(J^T gY[e]) / |r_e|
+// with the weights broadcast from shared memory ([b][ch], double); no cross-lane reduction at all.
+template <typename T, int L, int NB>
+__global__ void __launch_bounds__(kGeoChunk) edge_embed_factors_bwd_kernel(int n, int nb, double rc, long E, const T* __restrict__ rvec,
+                                                                           const T* __restrict__ W_x0, const T* __restrict__ W_v0,
+                                                                           const T* __restrict__ g_x0, const T* __restrict__ g_v0,
+                                                                           const T* __restrict__ gYc, T* __restrict__ g_rvec) {
+    constexpr int DE = (L + 1) * (L + 1);
+    extern __shared__ __align__(16) unsigned char geo_raw[];
+    double* Wxs = reinterpret_cast<double*>(geo_raw);   // [ch][NB] (ch-major: one thread walks ch, all threads read the same address)
+    double* Wvs = Wxs + (size_t)n * NB;
+    const int tid = threadIdx.x;
+    for (int idx = tid; idx < n * NB; idx += kGeoChunk) {
+        const int ch = idx / NB, b = idx - ch * NB;
+        Wxs[idx] = b < nb ? (double)W_x0[ch * nb + b] : 0.0;
+        Wvs[idx] = b < nb ? (double)W_v0[ch * nb + b] : 0.0;
+    }
+    __syncthreads();
+    const long e = (long)blockIdx.x * kGeoChunk + tid;
+    if (e >= E) return;
+    const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+    const double dx = (double)rx, dy = (double)ry, dz = (double)rz;
+    const double rr = sqrt(dx * dx + dy * dy + dz * dz);
+    double Bu[kMaxBasis], dBu[kMaxBasis];
+    radial_basis<true>(rr, rc, nb, Bu, dBu);
+    double gb[NB];
+#pragma unroll
+    for (int b = 0; b < NB; ++b) gb[b] = 0.0;
+    const T* gx = g_x0 + (size_t)e * n;
+    const T* gv = g_v0 + (size_t)e * n;
+    for (int ch = 0; ch < n; ++ch) {
+        const double a = (double)gx[ch], c = (double)gv[ch];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) gb[b] = fma(a, Wxs[ch * NB + b], fma(c, Wvs[ch * NB + b], gb[b]));
+    }
+    double rad = 0.0;
+#pragma unroll
+    for (int b = 0; b < NB; ++b)
+        if (b < nb) rad = fma(gb[b], dBu[b], rad);
+    const T inv = T(1) / sqrt(rx * rx + ry * ry + rz * rz);
+    const T x = rx * inv, y = ry * inv, z = rz * inv;
+    T gY[DE], g[3];
+#pragma unroll
+    for (int j = 0; j < DE; ++j) gY[j] = gYc[(size_t)e * DE + j];
+    sph_harm_vjp<T, L>(x, y, z, gY, g);
+    const T dot = g[0] * x + g[1] * y + g[2] * z;
+    g_rvec[3 * e] = (T)((double)g_rvec[3 * e] + (double)((g[0] - dot * x) * inv) + rad * (dx / rr));
+    g_rvec[3 * e + 1] = (T)((double)g_rvec[3 * e + 1] + (double)((g[1] - dot * y) * inv) + rad * (dy / rr));
+    g_rvec[3 * e + 2] = (T)((double)g_rvec[3 * e + 2] + (double)((g[2] - dot * z) * inv) + rad * (dz / rr));
+}
+
 }  // namespace allegro

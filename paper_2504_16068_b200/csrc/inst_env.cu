@@ -158,6 +158,20 @@ allegro_status_t launch_edge_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EmbedArg
     }
     if (a.n_edges == 0) return ALLEGRO_OK;
     const unsigned grid = (unsigned)((a.n_edges + kGeoChunk - 1) / kGeoChunk);
+    if (a.gV0 == nullptr && a.g_v0 != nullptr) {      // factor form of the cotangent: thread per edge, no reductions
+#define ALLEGRO_EMBF(NB)                                                                                                    \
+    {                                                                                                                       \
+        auto k = edge_embed_factors_bwd_kernel<T, ALLEGRO_L, NB>;                                                           \
+        const size_t smem = (size_t)2 * a.n * NB * sizeof(double);                                                          \
+        ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
+        k<<<grid, kGeoChunk, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0,  \
+                                           (const T*)a.g_x0, (const T*)a.g_v0, (const T*)a.gYe, (T*)a.g_rvec);              \
+    }
+        if (a.nb <= 8) ALLEGRO_EMBF(8) else ALLEGRO_EMBF(16)
+#undef ALLEGRO_EMBF
+        ALLEGRO_LAUNCHED();
+        return ALLEGRO_OK;
+    }
 #define ALLEGRO_EMBB(NB)                                                                                                    \
     {                                                                                                                       \
         auto k = edge_embed_bwd_kernel<T, ALLEGRO_L, NB>;                                                                   \
