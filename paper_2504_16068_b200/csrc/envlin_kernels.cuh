@@ -16,24 +16,25 @@ namespace allegro {
 constexpr int kEnvLinThreads = 256, kEnvLinChunk = 128;
 
 template <typename T, int L>
-__global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_out, int n_in, const int* __restrict__ row_ptr, const T* __restrict__ rvec,
+__global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_atoms, int n_out, int n_in, const int* __restrict__ row_ptr, const T* __restrict__ rvec,
                                                                          const T* __restrict__ x, const T* __restrict__ W, T scale,
                                                                          T* __restrict__ Eenv) {
     constexpr int DE = (L + 1) * (L + 1);
     extern __shared__ __align__(16) unsigned char envlin_raw[];
     T* Ys = reinterpret_cast<T*>(envlin_raw);                 // [chunk][DE]
     T* red = Ys + kEnvLinChunk * DE;                           // [threads][DE] per-slot partial sums, then S[n_in][DE] in its first rows
-    T* Wt = red + kEnvLinThreads * DE;                         // [n_in][n_out]: W transposed (lanes run over n in the last phase)
+    T* Wt = red + kEnvLinThreads * DE;                         // [n_in][n_out + 1]: W transposed, rows padded (conflict-free both ways)
     const int tid = threadIdx.x;
-    const int c = blockIdx.x;
-    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
+    const int ldw = n_out + 1;
     const int nslots = kEnvLinThreads / n_in;
     const int slot = tid / n_in, m = tid - slot * n_in;
     const bool active = slot < nslots;
-    for (int idx = tid; idx < n_out * n_in; idx += kEnvLinThreads) {
+    for (int idx = tid; idx < n_out * n_in; idx += kEnvLinThreads) {     // once per CTA: the CTA walks centres blockIdx.x, + gridDim.x, ...
         const int n = idx / n_in, mm = idx - n * n_in;
-        Wt[mm * n_out + n] = W[idx];
+        Wt[mm * ldw + n] = W[idx];
     }
+    for (int c = blockIdx.x; c < n_atoms; c += gridDim.x) {
+    const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
     T acc[DE];
 #pragma unroll
     for (int j = 0; j < DE; ++j) acc[j] = T(0);
@@ -80,8 +81,10 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_ou
     for (int idx = tid; idx < n_out * DE; idx += kEnvLinThreads) {
         const int j = idx / n_out, n = idx - j * n_out;
         T s = T(0);
-        for (int mm = 0; mm < n_in; ++mm) s = fma(Wt[mm * n_out + n], red[mm * DE + j], s);
+        for (int mm = 0; mm < n_in; ++mm) s = fma(Wt[mm * ldw + n], red[mm * DE + j], s);
         Eenv[((size_t)c * n_out + n) * DE + j] = scale * s;
+    }
+    __syncthreads();     // red / Ys are rewritten by the next centre
     }
 }
 
@@ -95,6 +98,7 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
     T* geo = Ys + kEnvLinChunk * DE;                           // [chunk][4]: unit vector, 1/|r|
     T* gEs = geo + kEnvLinChunk * 4;                           // [n_out][DE]
     T* Ms = gEs + n_out * DE;                                  // [n_in][DE]
+    T* part = Ms + n_in * DE;                                  // [chunk][DE]: the second half-sum of gY
     const int tid = threadIdx.x;
     const int c = blockIdx.x;
     const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
@@ -137,17 +141,34 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
                 *dst = acc_g_x ? *dst + s : s;
             }
         }
-        if (tid < cnt) {     // gY_e[j] = sum_m M[m][j] x[e][m], then through Y_lm and the normalisation
+        {   // gY_e[j] = sum_m M[m][j] x[e][m]: thread (half, edge) sums one half of the m range; halves added in order
+            const int half = tid / kEnvLinChunk, le = tid - half * kEnvLinChunk;
+            const int m0 = half ? n_in / 2 : 0, m1 = half ? n_in : n_in / 2;
+            T gYh[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) gYh[j] = T(0);
+            if (le < cnt) {
+                const T* xr = x + (size_t)(cb + le) * n_in;
+                for (int mm = m0; mm < m1; ++mm) {
+                    const T xv = xr[mm];
+#pragma unroll
+                    for (int j = 0; j < DE; ++j) gYh[j] = fma(Ms[mm * DE + j], xv, gYh[j]);
+                }
+                if (half) {
+#pragma unroll
+                    for (int j = 0; j < DE; ++j) part[le * DE + j] = gYh[j];
+                }
+            }
+            __syncthreads();
+            if (half == 0 && le < cnt) {
+#pragma unroll
+                for (int j = 0; j < DE; ++j) gYh[j] += part[le * DE + j];
+            }
+            if (half != 0 || le >= cnt) continue;
             const size_t e = (size_t)(cb + tid);
             T gY[DE];
 #pragma unroll
-            for (int j = 0; j < DE; ++j) gY[j] = T(0);
-            const T* xr = x + e * n_in;
-            for (int mm = 0; mm < n_in; ++mm) {
-                const T xv = xr[mm];
-#pragma unroll
-                for (int j = 0; j < DE; ++j) gY[j] = fma(Ms[mm * DE + j], xv, gY[j]);
-            }
+            for (int j = 0; j < DE; ++j) gY[j] = gYh[j];
             const T ux = geo[tid * 4], uy = geo[tid * 4 + 1], uz = geo[tid * 4 + 2], inv = geo[tid * 4 + 3];
             T g[3];
             sph_harm_vjp<T, L>(ux, uy, uz, gY, g);

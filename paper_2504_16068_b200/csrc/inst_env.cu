@@ -195,10 +195,11 @@ allegro_status_t launch_env_linear<ALLEGRO_T, ALLEGRO_L>(const EnvLinArgs& a) {
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
-    const size_t smem = ((size_t)kEnvLinChunk * DE + (size_t)kEnvLinThreads * DE + (size_t)a.n_in * a.n_out) * sizeof(T);
+    const size_t smem = ((size_t)kEnvLinChunk * DE + (size_t)kEnvLinThreads * DE + (size_t)a.n_in * (a.n_out + 1)) * sizeof(T);
     auto k = env_linear_fwd_kernel<T, ALLEGRO_L>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    k<<<(unsigned)a.n_atoms, kEnvLinThreads, smem, a.st>>>(a.n_out, a.n_in, a.row_ptr, (const T*)a.rvec, (const T*)a.x, (const T*)a.W, (T)a.scale,
+    const unsigned grid = (unsigned)(a.n_atoms < 148 * 6 ? a.n_atoms : 148 * 6);      // persistent: W^T is staged once per CTA
+    k<<<grid, kEnvLinThreads, smem, a.st>>>(a.n_atoms, a.n_out, a.n_in, a.row_ptr, (const T*)a.rvec, (const T*)a.x, (const T*)a.W, (T)a.scale,
                                                            (T*)a.Eenv);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
@@ -213,7 +214,7 @@ allegro_status_t launch_env_linear_backward<ALLEGRO_T, ALLEGRO_L>(const EnvLinAr
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
-    const size_t smem = ((size_t)kEnvLinChunk * (DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE) * sizeof(T);
+    const size_t smem = ((size_t)kEnvLinChunk * (2 * DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE) * sizeof(T);
     auto k = env_linear_bwd_kernel<T, ALLEGRO_L>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k<<<(unsigned)a.n_atoms, kEnvLinThreads, smem, a.st>>>(a.n_out, a.n_in, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.x, (const T*)a.W,
