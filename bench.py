@@ -567,7 +567,9 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
                        "block_subsets": "first layer: paths from the natural-parity blocks of V0 only (15 of 30); last layer: paths into 0e only (3 of 30)",
                        "l2": "not flushed: feature tensors (%.2f GB each) exceed the 126 MB L2" % (E * p["n"] * step.pd.dV * 4 / 1e9)},
             "atom_steps_per_s": N_all / (ms_step * 1e-3),
-            "roofline": {"bound": "tensor", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+            "roofline": {"bound": "tensor", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak,
+                         "traffic": _ncu_traffic(name, top), "traffic_source": "committed ncu --set full capture, profiles/traffic.txt: dram bytes of "
+                                                                               "both layers' launches of this call per step (not re-measured by this run)",
                          "peak_source": peak_src, "note": "algorithmic fp32 flops of all layers' calls of this name; every multiply-add costs four TF32 MMAs "
                                                           "(hi / lo split of both operands) on tcgen05",
                          "timing": "CUDA events around every call inside the timed steps"},

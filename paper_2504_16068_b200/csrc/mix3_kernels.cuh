@@ -115,7 +115,9 @@ struct Mix3Seq {
     static constexpr int OFF_A = 0, OFF_B = Mix3::NA * Mix3::A_BYTES, OFF_STG = OFF_B + Mix3::NB * B_BYTES;
     static constexpr int OFF_BAR = OFF_STG + (ALIAS_STG ? 0 : STG_BYTES);
     static constexpr int OFF_RED = OFF_BAR + 256;                 // [2][4 lane quarters][24 edges] partial edge energies
-    static constexpr int SMEM = OFF_RED + 2 * 4 * Mix3::TE * 4 + 1024;   // + barrier block + energy partials + 1024-byte alignment slack
+    static constexpr int OFF_YS = OFF_RED + 2 * 4 * Mix3::TE * 4;       // OUTER mode: Y_j(rhat_e) of the tile's edges, [TE][9] floats
+    static constexpr int SMEM = OFF_YS + 896 + 1024;             // + barrier block + energy partials + Ys + 1024-byte alignment slack
+    static_assert(SMEM <= 232448, "shared memory of the forward kernel");
     static_assert(count() >= 2, "at least two paths");
 };
 
@@ -291,27 +293,47 @@ __global__ void __launch_bounds__(Mix3::CT + 64, 1) mix3_fwd_kernel(const int* _
             if (!OUTER && tid == 0 && eb + TE < e1)     // the next tile's V rows (one contiguous range) are pulled into L2 while this tile computes
                 bulk_prefetch_l2(V + (size_t)(eb + TE) * 64 * DV, (uint32_t)min(TE, e1 - eb - TE) * 64 * DV * 4);
             float Vr[M3::EPS][DV];
+            if constexpr (OUTER) {      // Y_j of the tile's edges once per tile (shared memory), then the rows v0 (x) Y in registers
+                float* Ysw = reinterpret_cast<float*>(sm + SQ::OFF_YS);
+                if (tid < TE) {
+                    const int e = eb + tid;
+                    float Y[9];
+                    if (e < e1) {
+                        const float rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
+                        const float inv = 1.f / sqrtf(rx * rx + ry * ry + rz * rz);
+                        mix3_sph9(rx * inv, ry * inv, rz * inv, Y);
+                    } else {
+#pragma unroll
+                        for (int j = 0; j < 9; ++j) Y[j] = 0.f;
+                    }
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) Ysw[tid * 9 + j] = Y[j];
+                }
+                float vv[M3::EPS];
+#pragma unroll
+                for (int i = 0; i < M3::EPS; ++i) {
+                    const int e = eb + 4 * slot + i;
+                    vv[i] = e < e1 ? v0[(size_t)e * 64 + ch] : 0.f;
+                }
+                asm volatile("bar.sync 3, %0;" ::"n"(M3::CT) : "memory");
+#pragma unroll
+                for (int i = 0; i < M3::EPS; ++i) {
+#pragma unroll
+                    for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
+#pragma unroll
+                    for (int j = 0; j < 9; ++j) Vr[i][mix3_nat_slot(j)] = vv[i] * Ysw[(4 * slot + i) * 9 + j];
+                }
+            } else {
 #pragma unroll
             for (int i = 0; i < M3::EPS; ++i) {
                 const int e = eb + 4 * slot + i;
                 if (e < e1) {
-                    if constexpr (OUTER) {
-                        const float rx = rvec[3 * (size_t)e], ry = rvec[3 * (size_t)e + 1], rz = rvec[3 * (size_t)e + 2];
-                        const float inv = 1.f / sqrtf(rx * rx + ry * ry + rz * rz);
-                        float Y[9];
-                        mix3_sph9(rx * inv, ry * inv, rz * inv, Y);
-                        const float v = v0[(size_t)e * 64 + ch];
-#pragma unroll
-                        for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
-#pragma unroll
-                        for (int j = 0; j < 9; ++j) Vr[i][mix3_nat_slot(j)] = v * Y[j];
-                    } else {
-                        row_load<float, DV>(V + ((size_t)e * 64 + ch) * DV, Vr[i]);
-                    }
+                    row_load<float, DV>(V + ((size_t)e * 64 + ch) * DV, Vr[i]);
                 } else {
 #pragma unroll
                     for (int k = 0; k < DV; ++k) Vr[i][k] = 0.f;
                 }
+            }
             }
             static_for3<0, NP>([&](auto kc) {
                 constexpr int k = decltype(kc)::value;
