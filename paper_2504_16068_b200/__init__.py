@@ -71,6 +71,7 @@ SIGNATURES = {
     "allegro_edge_energy": (C.c_int, [_vp, C.c_long, _vp, _vp, C.c_double, _vp, _vp, _vp]),
     "allegro_segment_sum": (C.c_int, [_vp, C.c_int, _vp, C.c_int, _vp, _vp]),
     "allegro_virial": (C.c_int, [C.c_long, _vp, _vp, C.c_int, _vp, _vp]),
+    "allegro_check_graph": (C.c_int, [C.c_int, C.c_long, _vp, _vp, C.c_long, _vp, _vp, _vp, C.c_int, C.POINTER(C.c_long), _vp]),
     "allegro_layer_step_host_workspace": (C.c_size_t, [_vp, C.c_int, C.c_long, C.c_int, C.c_int]),
     "allegro_layer_step_host": (C.c_int, [_vp, C.c_int, C.c_long, _vp, _vp, _vp, _vp, _vp, C.c_int, C.c_double, _vp, _vp, C.c_double, C.c_double,
                                           C.c_int, _vp, _vp, _vp, C.c_size_t, _vp]),
@@ -477,6 +478,16 @@ def virial(rvec, g_rvec, W=None, stream=None):
         W = torch.empty((3, 3), dtype=rvec.dtype, device=rvec.device)
     _check(lib().allegro_virial(rvec.shape[0], _ptr(rvec), _ptr(g_rvec), _dt(rvec), _ptr(W), _stream(stream)))
     return W
+
+
+def check_graph(row_ptr, n_edges, items=None, rev=None, col=None, rvec=None, stream=None):
+    """debugging aid (allegro_check_graph): number of violations in the step's index lists; raises AllegroError when there is one"""
+    n_bad = C.c_long(-1)
+    dt = _dt(rvec) if rvec is not None else F32
+    n_items = 0 if items is None else items.numel() // 3
+    _check(lib().allegro_check_graph(row_ptr.shape[0] - 1, int(n_edges), _ptr(row_ptr), _ptr(items), n_items, _ptr(rev), _ptr(col), _ptr(rvec), dt,
+                                     C.byref(n_bad), _stream(stream)))
+    return n_bad.value
 
 
 def segment_sum(ptr, vals, out=None, stream=None):

@@ -62,7 +62,7 @@ def generate(force=False):
 
 
 def _jobs():
-    jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("model.o", "model.cu", []), ("peaks.o", "peaks.cu", []), ("neighbour.o", "neighbour.cu", []), ("noalloc.o", "noalloc.cu", []), ("plan.o", "plan.cpp", [])]
+    jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("model.o", "model.cu", []), ("peaks.o", "peaks.cu", []), ("neighbour.o", "neighbour.cu", []), ("noalloc.o", "noalloc.cu", []), ("check.o", "check.cu", []), ("plan.o", "plan.cpp", [])]
     for part in (0, 1):
         jobs.insert(0, ("inst_mix3_p%d.o" % part, "inst_mix3.cu", ["-DALLEGRO_MIX3_PART=%d" % part]))
     for tag, ctype in DTYPES:
@@ -70,7 +70,12 @@ def _jobs():
             d = ["-DALLEGRO_T=%s" % ctype, "-DALLEGRO_L=%d" % L]
             jobs.append(("inst_tp_%s_l%d.o" % (tag, L), "inst_tp.cu", d))
             jobs.append(("inst_env_%s_l%d.o" % (tag, L), "inst_env.cu", d))
-    return jobs
+    # slowest files first (the pool starts jobs in list order): the l_max = 3 units, the dense l_max = 3 kernels, the tcgen05 mix
+    for tag, ctype in DTYPES:
+        for part in (3, 2, 1, 0):
+            jobs.insert(0, ("inst_mixp_%s_p%d.o" % (tag, part), "inst_mixp.cu", ["-DALLEGRO_T=%s" % ctype, "-DALLEGRO_MIXP_PART=%d" % part]))
+    slow = [j for j in jobs if j[0].startswith("inst_tp_") and j[0].endswith("_l3.o")]
+    return slow + [j for j in jobs if j not in slow]
 
 
 def build(force=False, jobs=None, verbose=False):

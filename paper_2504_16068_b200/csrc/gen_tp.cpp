@@ -134,7 +134,7 @@ static void emit(FILE* f, int L) {
     fprintf(f, "};\n");
 }
 
-// Per-path device functions for the dense per-path channel mix (l_max <= 2): un-weighted t_p = C^p (V (x) E) of ONE path and
+// Per-path device functions for the dense per-path channel mix: un-weighted t_p = C^p (V (x) E) of ONE path and
 // its VJP, with the feature row read through a pointer (shared memory) so that only the path's V block is touched.
 static void emit_paths(FILE* f, int L) {
     PlanTables t;
@@ -144,7 +144,8 @@ static void emit_paths(FILE* f, int L) {
     size_t z = 0;
     for (int p = 0; p < P; ++p) {
         const int d3 = 2 * t.paths[p].l3 + 1, off3 = t.paths[p].off3;
-        fprintf(f, "template <> struct TPPath<%d, %d> {\n    static constexpr int D3 = %d, TOFF = %d, OFF3 = %d;\n", L, p, d3, toff, off3);
+        const int d1 = 2 * t.paths[p].l1 + 1, off1 = t.paths[p].off1;
+        fprintf(f, "template <> struct TPPath<%d, %d> {\n    static constexpr int D3 = %d, TOFF = %d, OFF3 = %d, D1 = %d, OFF1 = %d;\n", L, p, d3, toff, off3, d1, off1);
         std::vector<Pair> pairs;
         std::map<std::pair<int, int>, int> idx;
         for (; z < t.nnz.size() && t.nnz[z].path == p; ++z) {
@@ -172,6 +173,18 @@ static void emit_paths(FILE* f, int L) {
             for (size_t q = 1; q < pr.terms.size(); ++q) fprintf(f, " s = fma(T(%.17g), gt[%d], s);", pr.terms[q].c, pr.terms[q].k);
             fprintf(f, " gE[%d] = fma(s, V[%d], gE[%d]); if (WANT_GV) gV[%d] = fma(s, E[%d], gV[%d]); }\n", pr.j, pr.i, pr.j, pr.i, pr.j, pr.i);
         }
+        fprintf(f, "    }\n");
+        // the same VJP with the feature cotangent of the path's OWN input block only (gv[i - OFF1], overwritten): the paths-outer kernels
+        fprintf(f, "    template <typename T, bool WANT_GV> static __device__ __forceinline__ void bwd_local(const T* __restrict__ V, const T (&E)[%d], const T (&gt)[%d], T (&gv)[%d], T (&gE)[%d]) {\n",
+                t.dE, d3, d1, t.dE);
+        fprintf(f, "        if (WANT_GV) {");
+        for (int i = 0; i < d1; ++i) fprintf(f, " gv[%d] = T(0);", i);
+        fprintf(f, " }\n");
+        for (const Pair& pr : pairs) {
+            fprintf(f, "        { T s = T(%.17g) * gt[%d];", pr.terms[0].c, pr.terms[0].k);
+            for (size_t q = 1; q < pr.terms.size(); ++q) fprintf(f, " s = fma(T(%.17g), gt[%d], s);", pr.terms[q].c, pr.terms[q].k);
+            fprintf(f, " gE[%d] = fma(s, V[%d], gE[%d]); if (WANT_GV) gv[%d] = fma(s, E[%d], gv[%d]); }\n", pr.j, pr.i, pr.j, pr.i - off1, pr.j, pr.i - off1);
+        }
         fprintf(f, "    }\n};\n");
         toff += d3;
     }
@@ -186,8 +199,8 @@ int main(int argc, char** argv) {
     fprintf(f, "#pragma once\n");
     fprintf(f, "template <int L> struct TPGen;\n");
     for (int L = 1; L <= 3; ++L) emit(f, L);
-    fprintf(f, "\n// per-path functions (dense mix), l_max <= 2\ntemplate <int L, int PTH> struct TPPath;\n");
-    for (int L = 1; L <= 2; ++L) emit_paths(f, L);
+    fprintf(f, "\n// per-path functions (dense mix)\ntemplate <int L, int PTH> struct TPPath;\n");
+    for (int L = 1; L <= 3; ++L) emit_paths(f, L);
     fclose(f);
     return 0;
 }

@@ -3,8 +3,8 @@
 //   out[e][n'][off3(p)+M] = sum_p sum_n W[p][n'][n] t[e][n][p][M]
 // and its VJP  gt[e][n][p][M] = sum_n' W[p][n'][n] G[e][n'][off3(p)+M], then the per-path CG VJP with unit weights.
 //
-// Generic version for any n, fp32 / fp64, l_max <= 2: the n x n mixes run on the FP32/FP64 FMA pipe with 128-bit shared-memory
-// operands (t never leaves the SM: PAPER.md:71).
+// Generic version for any n, fp32 / fp64: the n x n mixes run on the FP32/FP64 FMA pipe with 128-bit shared-memory
+// operands (t never leaves the SM: PAPER.md:71).  l_max <= 2 as described next; l_max = 3 with the loops exchanged (mixp_* below).
 // One CTA per item; thread <-> (edge slot, channel).  Per tile of `nsl` edges:
 //   forward : t (DT values per thread) -> shared tS[slot][col][n]; per path p: W_p -> shared Ws[n'][n] (row stride n+4),
 //             acc[off3(p)+M] += <Ws[n'][:], tS[slot][toff(p)+M][:]>; thread (slot, n') stores its out row.
@@ -303,8 +303,8 @@ static inline bool all_blocks(const allegro_plan* plan) {
     return (plan->out_blocks & full) == full && (plan->in_blocks & full) == full;
 }
 
-// The dense mode is instantiated for l_max <= 2 (what configs[2] needs): at l_max = 3 a thread would hold 312
-// un-weighted path values, which does not fit the register file.
+// l_max <= 2: all un-weighted path values of an (edge, channel) live in the thread (mix_fwd / mix_bwd); l_max = 3: the
+// paths-outer kernels above (312 values do not fit the register file).
 #if ALLEGRO_L <= 2
 template <typename T>
 static allegro_status_t launch_mix_forward(const TpArgs& a) {
@@ -341,10 +341,25 @@ static allegro_status_t launch_mix_forward(const TpArgs& a) {
 }
 
 #else
+// l_max = 3: the paths-outer kernels of mixp_kernels.cuh, compiled in their own translation units (inst_mixp.cu; the 68 unrolled
+// paths make them the slowest files of the build, so they do not sit behind the sparse kernels of this unit)
+template <typename T> allegro_status_t launch_mixp_forward(const TpArgs& a);
+template <typename T, bool WANT_GV> allegro_status_t launch_mixp_backward(const TpArgs& a, T* gE_dst, int gE_by_item);
+template <typename T> allegro_status_t launch_mixp_gw(const TpArgs& a, T* part);
+
 template <typename T>
-static allegro_status_t launch_mix_forward(const TpArgs&) {
-    set_error("tp_forward (dense): dense path weights are built for l_max <= 2");
-    return ALLEGRO_EUNSUPPORTED;
+static allegro_status_t launch_mix_forward(const TpArgs& a) {
+    constexpr int CT = sizeof(T) == 4 ? 256 : 128;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    if (a.n % VEC != 0 || a.n > CT) {
+        set_error("tp_forward (dense): n = %d unsupported (n %% %d == 0, n <= %d)", a.n, VEC, CT);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (!all_blocks(a.plan)) {
+        set_error("tp_forward (dense): block subsets are built for fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    return launch_mixp_forward<T>(a);
 }
 #endif
 
@@ -423,9 +438,37 @@ static allegro_status_t launch_mix_backward(const TpArgs& a) {
 }
 #else
 template <typename T>
-static allegro_status_t launch_mix_backward(const TpArgs&) {
-    set_error("tp_backward (dense): dense path weights are built for l_max <= 2");
-    return ALLEGRO_EUNSUPPORTED;
+static allegro_status_t launch_mix_backward(const TpArgs& a) {
+    using Gen = TPGen<ALLEGRO_L>;
+    constexpr int CT = sizeof(T) == 4 ? 256 : 128;
+    constexpr int VEC = 16 / (int)sizeof(T);
+    if (a.n % VEC != 0 || a.n > CT) {
+        set_error("tp_backward (dense): n = %d unsupported (n %% %d == 0, n <= %d)", a.n, VEC, CT);
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    if (!all_blocks(a.plan) || a.q != nullptr) {
+        set_error("tp_backward (dense): block subsets and the on-the-fly cotangent are built for fp32, l_max = 2, n = 64 only");
+        return ALLEGRO_EUNSUPPORTED;
+    }
+    const bool have_items = a.items != nullptr;
+    T* gE_dst = have_items ? (T*)a.ws : (T*)a.gEenv;
+    if (a.g_path_w != nullptr) {   // training: gradient with respect to W_p
+        if (a.n % 4 != 0 || (a.n / 4) * (a.n / 4) > kGwMaxBlocks * CT) {
+            set_error("tp_backward (dense): g_path_w needs n %% 4 == 0, n <= 128");
+            return ALLEGRO_EUNSUPPORTED;
+        }
+        T* part = (T*)((unsigned char*)a.ws + (have_items ? align_up((size_t)a.n_items * a.n * Gen::DE * sizeof(T), 256) : 0));
+        allegro_status_t sg = launch_mixp_gw<T>(a, part);
+        if (sg != ALLEGRO_OK) return sg;
+    }
+    allegro_status_t sb = a.gV != nullptr ? launch_mixp_backward<T, true>(a, gE_dst, have_items ? 1 : 0)
+                                          : launch_mixp_backward<T, false>(a, gE_dst, have_items ? 1 : 0);
+    if (sb != ALLEGRO_OK) return sb;
+    if (have_items) {
+        combine_items_kernel<T><<<(unsigned)a.n_items, 128, 0, a.st>>>(a.items, a.n_items, a.n * Gen::DE, (const T*)a.ws, (T*)a.gEenv);
+        ALLEGRO_LAUNCHED();
+    }
+    return ALLEGRO_OK;
 }
 #endif
 

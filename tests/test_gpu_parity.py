@@ -380,10 +380,12 @@ def test_c3_full_size_chunked_sampled_centres():
     _check_forces_vs_oracle(inp, st.F, [0, int(np.argmax(deg)), inp["N"] - 1], _single_layer_g_r(inp), "C3")
 
 
-@pytest.mark.parametrize("lmax,n,dt,geom", [(2, 64, np.float32, "C1s"), (1, 8, np.float64, "C0"), (1, 128, np.float32, "C0"), (2, 32, np.float64, "C4s")])
+@pytest.mark.parametrize("lmax,n,dt,geom", [(2, 64, np.float32, "C1s"), (1, 8, np.float64, "C0"), (1, 128, np.float32, "C0"), (2, 32, np.float64, "C4s"),
+                                            (3, 128, np.float32, "C0"), (3, 64, np.float32, "C0"), (3, 16, np.float64, "C0")])
 def test_dense_path_weights_forward_and_vjp(lmax, n, dt, geom):
     """ALLEGRO_W_DENSE (BASELINE.json:configs[2], reading A5): per-path n x n channel mix, forward and VJP (gV, gEenv),
-    against the oracle's dense mode on seeded inputs; also with centres split into items"""
+    against the oracle's dense mode on seeded inputs; also with centres split into items.  l_max = 3 (Table 1's medium / large
+    models: 68 paths, n = 64 / 128) runs the paths-outer kernels."""
     import oracle as orc
     import torch
 
@@ -876,6 +878,52 @@ def test_gpu_neighbour_list_bit_exact(name):
     assert np.array_equal(nl["col"].cpu().numpy(), g["col"])
     assert np.array_equal(nl["rev"].cpu().numpy(), g["rev"])
     assert np.array_equal(nl["rvec"].cpu().numpy(), g["rvec"].astype(dt))
+
+
+@pytest.mark.parametrize("name", ["C0", "C4s"])
+def test_check_graph_accepts_sound_lists_and_names_broken_ones(name):
+    """allegro_check_graph (debugging aid: the kernels index unchecked and compute-sanitizer is closed on this pool): the seeded
+    graphs and their segment plans pass; one corrupted entry in each list is counted and named"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import configs
+    g = configs.geometry_for(name)
+    dt = np.float64 if g["spec"]["dtype"] == "f64" else np.float32
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    rp, rev, col, rvec = d(g["row_ptr"]), d(g["rev"]), d(g["col"]), d(g["rvec"].astype(dt))
+    E, N = g["rvec"].shape[0], g["row_ptr"].shape[0] - 1
+    items = d(ab.segments_build(g["row_ptr"], 7))
+    assert ab.check_graph(rp, E, items=items, rev=rev, col=col, rvec=rvec) == 0
+    assert ab.check_graph(rp, E) == 0
+
+    def bad(match, **kw):
+        args = dict(items=items, rev=rev, col=col, rvec=rvec)
+        args.update(kw)
+        with pytest.raises(ab.AllegroError) as ei:
+            ab.check_graph(args.pop("rp", rp), args.pop("E", E), **args)
+        assert ei.value.status == 1 and match in str(ei.value), str(ei.value)
+
+    c = int(np.argmax(np.diff(g["row_ptr"])))                 # a centre with edges
+    e = int(g["row_ptr"][c])
+    rp2 = rp.clone(); rp2[c + 1] = rp2[c] - 1 if c > 0 else -1
+    bad("row_ptr", rp=rp2)
+    bad("row_ptr", E=E + 1)
+    it2 = items.clone(); it2[3, 2] += 1                        # an item reaching past its tile: the next one no longer continues it
+    bad("items", items=it2)
+    it3 = items[:-1].contiguous()                              # the last centre's last item is missing
+    bad("items", items=it3)
+    rev2 = rev.clone(); rev2[e] = rev[e + 1]                   # not an involution any more
+    bad("rev", rev=rev2)
+    rev3 = rev.clone(); rev3[e] = E                            # out of range
+    bad("rev", rev=rev3)
+    col2 = col.clone(); col2[e] = (int(col[e]) + 1) % N        # the reverse edge is not in the named neighbour's row
+    bad("rev / col", col=col2)
+    rv2 = rvec.clone(); rv2[e] = 0                             # zero-length edge: the kernels divide by |r|
+    bad("rvec", rvec=rv2)
+    rv3 = rvec.clone(); rv3[E - 1, 1] = float("nan")
+    bad("rvec", rvec=rv3)
+    assert ab.check_graph(rp, E, items=items, rev=rev, col=col, rvec=rvec) == 0      # the counters are reset by every call
 
 
 @pytest.mark.parametrize("name", ["C0", "C1s", "C3s", "C4s"])
