@@ -14,10 +14,18 @@ namespace allegro {
 using T = ALLEGRO_T;
 constexpr int CT = sizeof(T) == 4 ? 256 : 128;
 
+// one n x (n + VEC) weight image must fit next to the staged tile
+static inline allegro_status_t mixp_check_smem(size_t smem, int n) {
+    if (smem <= 226 * 1024) return ALLEGRO_OK;
+    set_error("dense path weights at l_max = 3: n = %d needs %zu bytes of shared memory (n <= 192 in fp32, n <= 128 in fp64)", n, smem);
+    return ALLEGRO_EUNSUPPORTED;
+}
+
 #if ALLEGRO_MIXP_PART == 0
 template <>
 allegro_status_t launch_mixp_forward<T>(const TpArgs& a) {
     const size_t smem = mixp_smem<T, 3>(a.n, CT);
+    if (mixp_check_smem(smem, a.n) != ALLEGRO_OK) return ALLEGRO_EUNSUPPORTED;
     auto k = mixp_fwd_kernel<T, 3, CT>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k<<<(unsigned)a.n_items, CT, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.V, (const T*)a.Eenv, (const T*)a.path_w, (T*)a.out);
@@ -28,6 +36,7 @@ allegro_status_t launch_mixp_forward<T>(const TpArgs& a) {
 template <>
 allegro_status_t launch_mixp_backward<T, ALLEGRO_MIXP_PART == 1>(const TpArgs& a, T* gE_dst, int gE_by_item) {
     const size_t smem = mixp_smem<T, 3>(a.n, CT);
+    if (mixp_check_smem(smem, a.n) != ALLEGRO_OK) return ALLEGRO_EUNSUPPORTED;
     auto k = mixp_bwd_kernel<T, 3, CT, ALLEGRO_MIXP_PART == 1>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k<<<(unsigned)a.n_items, CT, smem, a.st>>>(a.n, a.row_ptr, a.items, (const T*)a.G, (const T*)a.V, (const T*)a.Eenv, (const T*)a.path_w,

@@ -7,7 +7,7 @@ namespace allegro {
 
 // 68 paths, 312 un-weighted path values per (edge, channel): they do not fit a thread's registers, so the loops are exchanged --
 // PATHS OUTER, edges inner.  One CTA per item (a centre's run of at most `tile_edges` edges).  Per path p: W_p (forward) or W_p^T
-// (VJP) is staged ONCE per item in shared memory; per tile of nsl x kMixpEpt edges thread (slot, n) computes the path's 2 l3 + 1
+// (VJP) is staged ONCE per item in shared memory; per tile of nsl x EPT edges thread (slot, n) computes the path's 2 l3 + 1
 // un-weighted values of its edges into shared memory and thread (slot, n') adds the mixed values to ITS OWN out rows (a
 // read-modify-write of rows that only this thread touches, so program order is the only ordering needed; the first path into a
 // block writes).  The item's out / gV rows stay in L2 between paths.  Every sum has a fixed order.
@@ -18,20 +18,35 @@ __host__ __device__ constexpr bool mixp_first_out(int p) {
     return true;
 }
 
-constexpr int kMixpEpt = 4;      // edges per thread and tile: one 128-bit load of a W row serves 4 x (2 l3 + 1) dot products
+// Register tile of a thread: R output rows (channels c0 + r nth, nth = n / R) x EPT edges x (2 l3 + 1) components.  Per group of
+// four K columns a thread loads R 128-bit pieces of W rows and EPT x D3 pieces of staged values for 4 R EPT D3 FMAs; the shared-
+// memory port (128 B / clk / SM) is what bounds these kernels, so bytes per FMA is the figure of merit.
+#ifndef ALLEGRO_MIXP_R
+#define ALLEGRO_MIXP_R 2
+#endif
+#ifndef ALLEGRO_MIXP_EPT
+#define ALLEGRO_MIXP_EPT 4
+#endif
+template <typename T> struct MixpTile {
+    static constexpr int R = sizeof(T) == 4 ? ALLEGRO_MIXP_R : 1;     // fp64: one row (the VJP already needs 254 registers)
+    static constexpr int EPT = sizeof(T) == 4 ? ALLEGRO_MIXP_EPT : 4;
+};
 
-// acc[k][M] = <wrow[:], tS[slot + nsl k][M][:]>, k < EPT, M < D3: rows of length n in shared memory, 128-bit loads, W loaded once per 4 columns
-template <typename T, int D3, int D3MAX, int EPT>
-__device__ __forceinline__ void mixp_dots(const T* __restrict__ wrow, const T* __restrict__ tS, int slot, int nsl, int n, T (&acc)[EPT][D3]) {
+// acc[r][k][M] = <Ws[c0 + r nth][:], tS[slot + nsl k][M][:]>: rows of length n in shared memory, 128-bit loads
+template <typename T, int D3, int D3MAX, int R, int EPT>
+__device__ __forceinline__ void mixp_dots(const T* __restrict__ Ws, int ldw, int c0, int nth, const T* __restrict__ tS, int slot, int nsl, int n,
+                                          T (&acc)[R][EPT][D3]) {
     constexpr int VEC = 16 / (int)sizeof(T);
 #pragma unroll
-    for (int k = 0; k < EPT; ++k)
+    for (int r = 0; r < R; ++r)
 #pragma unroll
-        for (int M = 0; M < D3; ++M) acc[k][M] = T(0);
-    const int4* w4 = reinterpret_cast<const int4*>(wrow);
+        for (int k = 0; k < EPT; ++k)
+#pragma unroll
+            for (int M = 0; M < D3; ++M) acc[r][k][M] = T(0);
     for (int i = 0; i < n / VEC; ++i) {
-        const int4 wv = w4[i];
-        const T* ws = reinterpret_cast<const T*>(&wv);
+        int4 wv[R];
+#pragma unroll
+        for (int r = 0; r < R; ++r) wv[r] = reinterpret_cast<const int4*>(Ws + (size_t)(c0 + r * nth) * ldw)[i];
 #pragma unroll
         for (int k = 0; k < EPT; ++k)
 #pragma unroll
@@ -39,7 +54,11 @@ __device__ __forceinline__ void mixp_dots(const T* __restrict__ wrow, const T* _
                 const int4 tv = reinterpret_cast<const int4*>(tS + ((size_t)(slot + nsl * k) * D3MAX + M) * n)[i];
                 const T* ts = reinterpret_cast<const T*>(&tv);
 #pragma unroll
-                for (int q = 0; q < VEC; ++q) acc[k][M] = fma(ws[q], ts[q], acc[k][M]);
+                for (int r = 0; r < R; ++r) {
+                    const T* ws = reinterpret_cast<const T*>(&wv[r]);
+#pragma unroll
+                    for (int q = 0; q < VEC; ++q) acc[r][k][M] = fma(ws[q], ts[q], acc[r][k][M]);
+                }
             }
     }
 }
@@ -49,22 +68,24 @@ __global__ void __launch_bounds__(CT) mixp_fwd_kernel(int n, const int* __restri
                                                        const T* __restrict__ V, const T* __restrict__ Eenv, const T* __restrict__ W,
                                                        T* __restrict__ out) {
     using Gen = TPGen<L>;
-    constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P, D3MAX = 2 * L + 1, EPT = kMixpEpt;
+    constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P, D3MAX = 2 * L + 1, R = MixpTile<T>::R, EPT = MixpTile<T>::EPT;
     constexpr int VEC = 16 / (int)sizeof(T);
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int nsl = CT / n, te = nsl * EPT;            // a tile = te edges; thread (slot, ch) owns edges slot + nsl k of it
+    const int nth = n / R, nsl = CT / nth, te = nsl * EPT;   // a tile = te edges; thread (slot, c0) owns edges slot + nsl k, rows c0 + r nth
     T* Ws = reinterpret_cast<T*>(smem_raw);            // [n][n + VEC]
     const int ldw = n + VEC;
     T* tS = Ws + (size_t)n * ldw;                      // [te][D3MAX][n]
     const int tid = threadIdx.x;
-    const int slot = tid / n, ch = tid - slot * n;
+    const int slot = tid / nth, c0 = tid - slot * nth;
     const bool active = slot < nsl;
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
     const int ntiles = (e1 - e0 + te - 1) / te;
-    T E[DE];
+    T E[R][DE];
 #pragma unroll
-    for (int j = 0; j < DE; ++j) E[j] = active ? Eenv[((size_t)c * n + ch) * DE + j] : T(0);
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int j = 0; j < DE; ++j) E[r][j] = active ? Eenv[((size_t)c * n + c0 + r * nth) * DE + j] : T(0);
 
     static_for<0, P>([&](auto pc) {
         constexpr int p = decltype(pc)::value;
@@ -82,28 +103,35 @@ __global__ void __launch_bounds__(CT) mixp_fwd_kernel(int n, const int* __restri
 #pragma unroll
                 for (int k = 0; k < EPT; ++k) {
                     const int e = eb + nsl * k;
-                    T tp[Pth::D3];
-                    if (e < e1) {
-                        Pth::template fwd<T>(V + ((size_t)e * n + ch) * DV, E, tp);
-                    } else {
 #pragma unroll
-                        for (int M = 0; M < Pth::D3; ++M) tp[M] = T(0);
+                    for (int r = 0; r < R; ++r) {
+                        const int ch = c0 + r * nth;
+                        T tp[Pth::D3];
+                        if (e < e1) {
+                            Pth::template fwd<T>(V + ((size_t)e * n + ch) * DV, E[r], tp);
+                        } else {
+#pragma unroll
+                            for (int M = 0; M < Pth::D3; ++M) tp[M] = T(0);
+                        }
+#pragma unroll
+                        for (int M = 0; M < Pth::D3; ++M) tS[((size_t)(slot + nsl * k) * D3MAX + M) * n + ch] = tp[M];
                     }
-#pragma unroll
-                    for (int M = 0; M < Pth::D3; ++M) tS[((size_t)(slot + nsl * k) * D3MAX + M) * n + ch] = tp[M];
                 }
             }
             __syncthreads();
             if (active) {
-                T acc[EPT][Pth::D3];
-                mixp_dots<T, Pth::D3, D3MAX, EPT>(Ws + (size_t)ch * ldw, tS, slot, nsl, n, acc);
+                T acc[R][EPT][Pth::D3];
+                mixp_dots<T, Pth::D3, D3MAX, R, EPT>(Ws, ldw, c0, nth, tS, slot, nsl, n, acc);
 #pragma unroll
                 for (int k = 0; k < EPT; ++k) {
                     const int e = eb + nsl * k;
                     if (e < e1) {
-                        T* dst = out + ((size_t)e * n + ch) * DV + Pth::OFF3;
 #pragma unroll
-                        for (int M = 0; M < Pth::D3; ++M) dst[M] = first ? acc[k][M] : dst[M] + acc[k][M];
+                        for (int r = 0; r < R; ++r) {
+                            T* dst = out + ((size_t)e * n + c0 + r * nth) * DV + Pth::OFF3;
+#pragma unroll
+                            for (int M = 0; M < Pth::D3; ++M) dst[M] = first ? acc[r][k][M] : dst[M] + acc[r][k][M];
+                        }
                     }
                 }
             }
@@ -126,22 +154,24 @@ __global__ void __launch_bounds__(CT) mixp_bwd_kernel(int n, const int* __restri
                                                        const T* __restrict__ G, const T* __restrict__ V, const T* __restrict__ Eenv,
                                                        const T* __restrict__ W, T* __restrict__ gV, T* __restrict__ gE_dst, int gE_by_item) {
     using Gen = TPGen<L>;
-    constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P, D3MAX = 2 * L + 1, EPT = kMixpEpt;
+    constexpr int DV = Gen::DV, DE = Gen::DE, P = Gen::P, D3MAX = 2 * L + 1, R = MixpTile<T>::R, EPT = MixpTile<T>::EPT;
     constexpr int VEC = 16 / (int)sizeof(T);
     extern __shared__ __align__(128) unsigned char smem_raw[];
-    const int nsl = CT / n, te = nsl * EPT;
+    const int nth = n / R, nsl = CT / nth, te = nsl * EPT;
     T* WsT = reinterpret_cast<T*>(smem_raw);           // [n][n + VEC], WsT[a][b] = W_p[b][a]
     const int ldw = n + VEC;
     T* gS = WsT + (size_t)n * ldw;                     // [te][D3MAX][n]
     const int tid = threadIdx.x;
-    const int slot = tid / n, ch = tid - slot * n;
+    const int slot = tid / nth, c0 = tid - slot * nth;
     const bool active = slot < nsl;
     int c, e0, e1;
     get_item(items, row_ptr, blockIdx.x, c, e0, e1);
     const int ntiles = (e1 - e0 + te - 1) / te;
-    T E[DE], gE[DE];
+    T E[R][DE], gE[R][DE];
 #pragma unroll
-    for (int j = 0; j < DE; ++j) { E[j] = active ? Eenv[((size_t)c * n + ch) * DE + j] : T(0); gE[j] = T(0); }
+    for (int r = 0; r < R; ++r)
+#pragma unroll
+        for (int j = 0; j < DE; ++j) { E[r][j] = active ? Eenv[((size_t)c * n + c0 + r * nth) * DE + j] : T(0); gE[r][j] = T(0); }
 
     static_for<0, P>([&](auto pc) {
         constexpr int p = decltype(pc)::value;
@@ -162,25 +192,33 @@ __global__ void __launch_bounds__(CT) mixp_bwd_kernel(int n, const int* __restri
 #pragma unroll
                 for (int k = 0; k < EPT; ++k) {
                     const int e = eb + nsl * k;
-                    const T* grow = G + ((size_t)e * n + ch) * DV + Pth::OFF3;
 #pragma unroll
-                    for (int M = 0; M < Pth::D3; ++M) gS[((size_t)(slot + nsl * k) * D3MAX + M) * n + ch] = e < e1 ? grow[M] : T(0);
+                    for (int r = 0; r < R; ++r) {
+                        const int ch = c0 + r * nth;
+                        const T* grow = G + ((size_t)e * n + ch) * DV + Pth::OFF3;
+#pragma unroll
+                        for (int M = 0; M < Pth::D3; ++M) gS[((size_t)(slot + nsl * k) * D3MAX + M) * n + ch] = e < e1 ? grow[M] : T(0);
+                    }
                 }
             }
             __syncthreads();
             if (active) {
-                T gt[EPT][Pth::D3];
-                mixp_dots<T, Pth::D3, D3MAX, EPT>(WsT + (size_t)ch * ldw, gS, slot, nsl, n, gt);
+                T gt[R][EPT][Pth::D3];
+                mixp_dots<T, Pth::D3, D3MAX, R, EPT>(WsT, ldw, c0, nth, gS, slot, nsl, n, gt);
 #pragma unroll
                 for (int k = 0; k < EPT; ++k) {
                     const int e = eb + nsl * k;
                     if (e < e1) {
-                        T gv[Pth::D1];
-                        Pth::template bwd_local<T, WANT_GV>(V + ((size_t)e * n + ch) * DV, E, gt[k], gv, gE);
-                        if constexpr (WANT_GV) {
-                            T* dst = gV + ((size_t)e * n + ch) * DV + Pth::OFF1;
 #pragma unroll
-                            for (int i = 0; i < Pth::D1; ++i) dst[i] = first ? gv[i] : dst[i] + gv[i];
+                        for (int r = 0; r < R; ++r) {
+                            const int ch = c0 + r * nth;
+                            T gv[Pth::D1];
+                            Pth::template bwd_local<T, WANT_GV>(V + ((size_t)e * n + ch) * DV, E[r], gt[r][k], gv, gE[r]);
+                            if constexpr (WANT_GV) {
+                                T* dst = gV + ((size_t)e * n + ch) * DV + Pth::OFF1;
+#pragma unroll
+                                for (int i = 0; i < Pth::D1; ++i) dst[i] = first ? gv[i] : dst[i] + gv[i];
+                            }
                         }
                     }
                 }
@@ -192,16 +230,22 @@ __global__ void __launch_bounds__(CT) mixp_bwd_kernel(int n, const int* __restri
     __syncthreads();
     if (active) {
 #pragma unroll
-        for (int j = 0; j < DE; ++j) red[((size_t)slot * n + ch) * DE + j] = gE[j];
+        for (int r = 0; r < R; ++r)
+#pragma unroll
+            for (int j = 0; j < DE; ++j) red[((size_t)slot * n + c0 + r * nth) * DE + j] = gE[r][j];
     }
     __syncthreads();
     if (slot == 0) {
-        T* dst = gE_dst + ((size_t)(gE_by_item ? (long)blockIdx.x : (long)c) * n + ch) * DE;
 #pragma unroll
-        for (int j = 0; j < DE; ++j) {
-            T acc = red[(size_t)ch * DE + j];
-            for (int sl = 1; sl < nsl; ++sl) acc += red[((size_t)sl * n + ch) * DE + j];
-            dst[j] = acc;
+        for (int r = 0; r < R; ++r) {
+            const int ch = c0 + r * nth;
+            T* dst = gE_dst + ((size_t)(gE_by_item ? (long)blockIdx.x : (long)c) * n + ch) * DE;
+#pragma unroll
+            for (int j = 0; j < DE; ++j) {
+                T acc = red[(size_t)ch * DE + j];
+                for (int sl = 1; sl < nsl; ++sl) acc += red[((size_t)sl * n + ch) * DE + j];
+                dst[j] = acc;
+            }
         }
     }
 }
@@ -211,8 +255,9 @@ __global__ void __launch_bounds__(CT) mixp_bwd_kernel(int n, const int* __restri
 template <typename T, int L_>
 static size_t mixp_smem(int n, int CT) {
     constexpr int VEC = 16 / (int)sizeof(T);
-    const size_t b = ((size_t)n * (n + VEC) + (size_t)(CT / n) * kMixpEpt * (2 * L_ + 1) * n) * sizeof(T);
-    const size_t red = (size_t)CT * TPGen<L_>::DE * sizeof(T);
+    const int nsl = CT / (n / MixpTile<T>::R);
+    const size_t b = ((size_t)n * (n + VEC) + (size_t)nsl * MixpTile<T>::EPT * (2 * L_ + 1) * n) * sizeof(T);
+    const size_t red = (size_t)nsl * n * TPGen<L_>::DE * sizeof(T);
     return b > red ? b : red;
 }
 
