@@ -327,17 +327,21 @@ def run_ours(args):
         if top in per_ce:
             k_ach = per_ce[top] * inp["n"] * E / (per_call_ms[top] * 1e-3)
             alu["kernel"] = {"name": top, "achieved": k_ach, "frac": k_ach / rate, "instructions_per_channel_edge": per_ce[top]}
-    # The fused kernel moves 2.5x fewer bytes than the two kernels it replaces and is bound by instruction issue: its line reports the ALU
-    # roofline as `roofline` and keeps the HBM figures under `hbm_roofline`
+    # Which roof binds the dominant kernel follows from its arithmetic: algorithmic instructions / measured FMA rate against algorithmic
+    # bytes / measured HBM bandwidth.  The fused kernel (2.5x fewer bytes than the two kernels it replaces) and the l_max = 3 kernels
+    # (3,386 instructions per 384 bytes in the VJP) are instruction-bound: their line reports the ALU roofline as `roofline` and
+    # keeps the HBM figures under `hbm_roofline`; the two-kernel sequence at l_max <= 2 is HBM-bound.
     hbm_roofline = None
-    if top == "tp_fused_energy" and alu is not None and "kernel" in alu:
+    alu_binds = (alu is not None and "kernel" in alu and
+                 per_ce[top] * inp["n"] * E / rate > abytes[top] / (peak * 1e9))
+    if alu_binds:
         hbm_roofline = roofline
         roofline = {"bound": "alu", "kernel": top, "achieved": alu["kernel"]["achieved"] / 1e12, "peak": rate / 1e12, "unit": "T FP32 instructions/s",
                     "frac": alu["kernel"]["frac"], "traffic": hbm_roofline["traffic"], "traffic_source": hbm_roofline["traffic_source"],
                     "peak_source": src, "algorithmic_instructions_per_launch": per_ce[top] * inp["n"] * E, "ms_per_launch": per_call_ms[top],
                     "timing": hbm_roofline["timing"],
-                    "note": "forward + energy + VJP in one kernel: algorithmic FMA + MUL instructions of the sparse CG contraction / CUDA-event time; "
-                            "the kernel's HBM fraction is under hbm_roofline"}
+                    "note": "algorithmic FMA + MUL instructions of the sparse CG contraction / CUDA-event time; at the measured rates this "
+                            "kernel's instruction time exceeds its HBM time, so the ALU roof binds; its HBM fraction is under hbm_roofline"}
     # forward only (configs[1]: "forward only, then forward+force VJP")
     fwd = None
     if not chunked:
