@@ -252,7 +252,10 @@ def run_ours(args):
     runner = step
     lib_graph = False
     if not args.no_graph:
-        if not chunked and args.mode in ("fused", "onthefly") and not args.separate_geometry:
+        # the library's own step object runs the fused kernel at l_max <= 2 and the two-kernel sequence at l_max = 3: it is the runner
+        # only when that is the mode asked for, so that the timed steps and the per-call roofline pass run the same kernels
+        lib_mode = "fused" if inp["lmax"] <= 2 else "onthefly"
+        if not chunked and args.mode == lib_mode and not args.separate_geometry:
             # the graph is captured INSIDE the library (allegro_layer_step_create): one C-ABI call per MD step, no framework graph
             runner = ab.LayerStepGraph(plan, dev["row_ptr"], dev["rev"], dev["rvec"], dev["V"], dev["W_r"], inp["rc"], dev["q"], inp["kappa"], inp["scale"],
                                        step.F, step.e_tot, want_gV=not args.force_only)
