@@ -91,7 +91,8 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_at
 template <typename T, int L>
 __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_out, int n_in, const int* __restrict__ row_ptr, const T* __restrict__ gEenv,
                                                                          const T* __restrict__ rvec, const T* __restrict__ x, const T* __restrict__ W,
-                                                                         T scale, T* __restrict__ g_rvec, int acc_g_rvec, T* __restrict__ g_x, int acc_g_x) {
+                                                                         T scale, T* __restrict__ g_rvec, int acc_g_rvec, T* __restrict__ g_x, int acc_g_x,
+                                                                         int stage_x) {
     constexpr int DE = (L + 1) * (L + 1);
     extern __shared__ __align__(16) unsigned char envlin_raw[];
     T* Ys = reinterpret_cast<T*>(envlin_raw);                 // [chunk][DE]
@@ -99,6 +100,11 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
     T* gEs = geo + kEnvLinChunk * 4;                           // [n_out][DE]
     T* Ms = gEs + n_out * DE;                                  // [n_in][DE]
     T* part = Ms + n_in * DE;                                  // [chunk][DE]: the second half-sum of gY
+    // [chunk][n_in + 1] (stage_x): the chunk's x rows, loaded with lanes along m (coalesced).  The gY sum walks a ROW per thread:
+    // from global memory that is one 32-byte sector per lane and load (32 L1 wavefronts per request), from the padded rows here
+    // it is conflict-free
+    T* xs = part + kEnvLinChunk * DE;
+    const int ldx = n_in + 1;
     const int tid = threadIdx.x;
     const int c = blockIdx.x;
     const int e0 = row_ptr[c], e1 = row_ptr[c + 1];
@@ -128,6 +134,12 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
             for (int j = 0; j < DE; ++j) Ys[tid * DE + j] = Y[j];
             geo[tid * 4] = ux; geo[tid * 4 + 1] = uy; geo[tid * 4 + 2] = uz; geo[tid * 4 + 3] = inv;
         }
+        if (stage_x) {
+            for (int idx = tid; idx < cnt * n_in; idx += kEnvLinThreads) {
+                const int le = idx / n_in, mm = idx - le * n_in;
+                xs[le * ldx + mm] = x[(size_t)cb * n_in + idx];
+            }
+        }
         __syncthreads();
         if (active) {        // g_x[e][m] = sum_j M[m][j] Y_j(e)
             T Mr[DE];
@@ -148,7 +160,7 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
 #pragma unroll
             for (int j = 0; j < DE; ++j) gYh[j] = T(0);
             if (le < cnt) {
-                const T* xr = x + (size_t)(cb + le) * n_in;
+                const T* xr = stage_x ? xs + le * ldx : x + (size_t)(cb + le) * n_in;
                 for (int mm = m0; mm < m1; ++mm) {
                     const T xv = xr[mm];
 #pragma unroll

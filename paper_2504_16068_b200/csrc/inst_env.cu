@@ -214,11 +214,15 @@ allegro_status_t launch_env_linear_backward<ALLEGRO_T, ALLEGRO_L>(const EnvLinAr
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
-    const size_t smem = ((size_t)kEnvLinChunk * (2 * DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE) * sizeof(T);
+    size_t smem = ((size_t)kEnvLinChunk * (2 * DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE) * sizeof(T);
+    // the chunk's x rows are staged in shared memory when that still leaves two CTAs per SM
+    const size_t xs_bytes = (size_t)kEnvLinChunk * (a.n_in + 1) * sizeof(T);
+    const int stage_x = smem + xs_bytes <= 100 * 1024 ? 1 : 0;
+    if (stage_x) smem += xs_bytes;
     auto k = env_linear_bwd_kernel<T, ALLEGRO_L>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     k<<<(unsigned)a.n_atoms, kEnvLinThreads, smem, a.st>>>(a.n_out, a.n_in, a.row_ptr, (const T*)a.gEenv, (const T*)a.rvec, (const T*)a.x, (const T*)a.W,
-                                                           (T)a.scale, (T*)a.g_rvec, a.acc_g_rvec, (T*)a.g_x, a.acc_g_x);
+                                                           (T)a.scale, (T*)a.g_rvec, a.acc_g_rvec, (T*)a.g_x, a.acc_g_x, stage_x);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

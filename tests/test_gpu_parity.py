@@ -216,6 +216,21 @@ def test_unsupported_and_bad_arguments_fail_loudly():
     with pytest.raises(ab.AllegroError) as ei:        # workspace too small
         ab.tp_backward(plan, rp, V, V.clone(), E, pw, want_g_path_w=True, workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
     assert ei.value.status == 4
+    # dense mix at l_max = 3: one n x n weight image must fit shared memory next to the staged tile (n <= 192 in fp32)
+    dense = ab.Plan(3, 224, ab.F32, ab.W_DENSE)
+    V3 = torch.zeros((1, 224, 32), device="cuda")
+    E3 = torch.zeros((1, 224, 16), device="cuda")
+    W3 = torch.zeros((68, 224, 224), device="cuda")
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_forward(dense, rp, V3, E3, W3)
+    assert ei.value.status == 2 and "shared memory" in str(ei.value)
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_backward(dense, rp, V3, V3.clone(), E3, W3)
+    assert ei.value.status == 2
+    dense.set_out_blocks(0x1)                         # block subsets exist for the tensor-core shape only
+    with pytest.raises(ab.AllegroError) as ei:
+        ab.tp_forward(dense, rp, V3, E3, W3)
+    assert ei.value.status == 2
 
 
 def _check_sampled_centres(inp, got, ranges, label):
