@@ -26,6 +26,7 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_at
     T* Wt = red + kEnvLinThreads * DE;                         // [n_in][n_out + 1]: W transposed, rows padded (conflict-free both ways)
     const int tid = threadIdx.x;
     const int ldw = n_out + 1;
+    T* part = Wt + (size_t)n_in * ldw;                         // [threads / n_out][n_out][DE]: partial sums of the per-centre product
     const int nslots = kEnvLinThreads / n_in;
     const int slot = tid / n_in, m = tid - slot * n_in;
     const bool active = slot < nslots;
@@ -52,7 +53,17 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_at
         }
         __syncthreads();
         if (active) {
-            for (int le = slot; le < cnt; le += nslots) {
+            int le = slot;
+            for (; le + 3 * nslots < cnt; le += 4 * nslots) {      // four rows in flight: the loop is bound by the latency of the x loads
+                T xv[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) xv[u] = x[(size_t)(cb + le + u * nslots) * n_in + m];
+#pragma unroll
+                for (int u = 0; u < 4; ++u)
+#pragma unroll
+                    for (int j = 0; j < DE; ++j) acc[j] = fma(xv[u], Ys[(le + u * nslots) * DE + j], acc[j]);
+            }
+            for (; le < cnt; le += nslots) {
                 const T xv = x[(size_t)(cb + le) * n_in + m];
 #pragma unroll
                 for (int j = 0; j < DE; ++j) acc[j] = fma(xv, Ys[le * DE + j], acc[j]);
@@ -77,14 +88,32 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_fwd_kernel(int n_at
         for (int j = 0; j < DE; ++j) red[m * DE + j] = acc[j];
     }
     __syncthreads();
-    // Eenv[c][n][j] = scale sum_m W[n][m] S[m][j]
-    for (int idx = tid; idx < n_out * DE; idx += kEnvLinThreads) {
-        const int j = idx / n_out, n = idx - j * n_out;
-        T s = T(0);
-        for (int mm = 0; mm < n_in; ++mm) s = fma(Wt[mm * ldw + n], red[mm * DE + j], s);
-        Eenv[((size_t)c * n_out + n) * DE + j] = scale * s;
+    // Eenv[c][n][j] = scale sum_m W[n][m] S[m][j]: thread (q, n) holds the DE sums of output channel n over the q-th part of the m
+    // range (one W load and DE broadcast loads of S per DE FMAs); the parts are then added in q order
+    {
+        const int nq = kEnvLinThreads / n_out;                    // parts of the m range (4 at n = 64); n_out <= 256
+        const int q = tid / n_out, n = tid - q * n_out;
+        if (q < nq) {
+            const int m0 = (int)((long)n_in * q / nq), m1 = (int)((long)n_in * (q + 1) / nq);
+            T s[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) s[j] = T(0);
+            for (int mm = m0; mm < m1; ++mm) {
+                const T w = Wt[mm * ldw + n];
+#pragma unroll
+                for (int j = 0; j < DE; ++j) s[j] = fma(w, red[mm * DE + j], s[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < DE; ++j) part[((size_t)q * n_out + n) * DE + j] = s[j];
+        }
+        __syncthreads();
+        for (int idx = tid; idx < n_out * DE; idx += kEnvLinThreads) {     // idx = n * DE + j: the store is contiguous
+            T t = part[idx];
+            for (int qq = 1; qq < nq; ++qq) t += part[(size_t)qq * n_out * DE + idx];
+            Eenv[(size_t)c * n_out * DE + idx] = scale * t;
+        }
     }
-    __syncthreads();     // red / Ys are rewritten by the next centre
+    __syncthreads();     // red / Ys / part are rewritten by the next centre
     }
 }
 
@@ -103,7 +132,8 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
     // [chunk][n_in + 1] (stage_x): the chunk's x rows, loaded with lanes along m (coalesced).  The gY sum walks a ROW per thread:
     // from global memory that is one 32-byte sector per lane and load (32 L1 wavefronts per request), from the padded rows here
     // it is conflict-free
-    T* xs = part + kEnvLinChunk * DE;
+    T* mpart = part + kEnvLinChunk * DE;                       // [threads / n_in][n_in][DE]: partial sums of M
+    T* xs = mpart + kEnvLinThreads * DE;
     const int ldx = n_in + 1;
     const int tid = threadIdx.x;
     const int c = blockIdx.x;
@@ -113,12 +143,30 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
     const bool active = slot < nslots;
     for (int idx = tid; idx < n_out * DE; idx += kEnvLinThreads) gEs[idx] = gEenv[(size_t)c * n_out * DE + idx];
     __syncthreads();
-    // M[m][j] = scale sum_n W[n][m] gE[n][j]: lanes run over m (coalesced rows of W)
-    for (int idx = tid; idx < n_in * DE; idx += kEnvLinThreads) {
-        const int j = idx / n_in, mm = idx - j * n_in;
-        T s = T(0);
-        for (int n = 0; n < n_out; ++n) s = fma(W[(size_t)n * n_in + mm], gEs[n * DE + j], s);
-        Ms[mm * DE + j] = scale * s;
+    // M[m][j] = scale sum_n W[n][m] gE[n][j]: thread (q, m) holds the DE sums of row m over the q-th part of the n range (lanes run
+    // over m: coalesced rows of W, one load per DE FMAs); the parts are added in q order.
+    {
+        const int nq = kEnvLinThreads / n_in;
+        const int q = tid / n_in, mm = tid - q * n_in;
+        if (q < nq) {
+            const int n0 = (int)((long)n_out * q / nq), n1 = (int)((long)n_out * (q + 1) / nq);
+            T sacc[DE];
+#pragma unroll
+            for (int j = 0; j < DE; ++j) sacc[j] = T(0);
+            for (int n = n0; n < n1; ++n) {
+                const T w = W[(size_t)n * n_in + mm];
+#pragma unroll
+                for (int j = 0; j < DE; ++j) sacc[j] = fma(w, gEs[n * DE + j], sacc[j]);
+            }
+#pragma unroll
+            for (int j = 0; j < DE; ++j) mpart[((size_t)q * n_in + mm) * DE + j] = sacc[j];
+        }
+        __syncthreads();
+        for (int idx = tid; idx < n_in * DE; idx += kEnvLinThreads) {
+            T t = mpart[idx];
+            for (int qq = 1; qq < nq; ++qq) t += mpart[(size_t)qq * n_in * DE + idx];
+            Ms[idx] = scale * t;
+        }
     }
     for (int cb = e0; cb < e1; cb += kEnvLinChunk) {
         const int cnt = min(kEnvLinChunk, e1 - cb);
@@ -145,12 +193,27 @@ __global__ void __launch_bounds__(kEnvLinThreads) env_linear_bwd_kernel(int n_ou
             T Mr[DE];
 #pragma unroll
             for (int j = 0; j < DE; ++j) Mr[j] = Ms[m * DE + j];
-            for (int le = slot; le < cnt; le += nslots) {
-                T s = T(0);
-#pragma unroll
-                for (int j = 0; j < DE; ++j) s = fma(Mr[j], Ys[le * DE + j], s);
+            int le = slot;
+            for (; le + 3 * nslots < cnt; le += 4 * nslots) {      // four rows in flight (the accumulate variant waits on its loads)
                 T* dst = g_x + (size_t)(cb + le) * n_in + m;
-                *dst = acc_g_x ? *dst + s : s;
+                const size_t st = (size_t)nslots * n_in;
+                T old[4];
+#pragma unroll
+                for (int u = 0; u < 4; ++u) old[u] = acc_g_x ? dst[u * st] : T(0);
+#pragma unroll
+                for (int u = 0; u < 4; ++u) {
+                    T sv = T(0);
+#pragma unroll
+                    for (int j = 0; j < DE; ++j) sv = fma(Mr[j], Ys[(le + u * nslots) * DE + j], sv);
+                    dst[u * st] = old[u] + sv;
+                }
+            }
+            for (; le < cnt; le += nslots) {
+                T sv = T(0);
+#pragma unroll
+                for (int j = 0; j < DE; ++j) sv = fma(Mr[j], Ys[le * DE + j], sv);
+                T* dst = g_x + (size_t)(cb + le) * n_in + m;
+                *dst = acc_g_x ? *dst + sv : sv;
             }
         }
         {   // gY_e[j] = sum_m M[m][j] x[e][m]: thread (half, edge) sums one half of the m range; halves added in order

@@ -195,10 +195,16 @@ allegro_status_t launch_env_linear<ALLEGRO_T, ALLEGRO_L>(const EnvLinArgs& a) {
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
-    const size_t smem = ((size_t)kEnvLinChunk * DE + (size_t)kEnvLinThreads * DE + (size_t)a.n_in * (a.n_out + 1)) * sizeof(T);
+    const size_t smem = ((size_t)kEnvLinChunk * DE + 2 * (size_t)kEnvLinThreads * DE + (size_t)a.n_in * (a.n_out + 1)) * sizeof(T);
     auto k = env_linear_fwd_kernel<T, ALLEGRO_L>;
     ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    const unsigned grid = (unsigned)(a.n_atoms < 148 * 6 ? a.n_atoms : 148 * 6);      // persistent: W^T is staged once per CTA
+    // persistent: W^T is staged once per CTA; one wave of as many CTAs as are resident at this shared-memory size
+    int per_sm = 1, n_sm = 148, dev = 0;
+    ALLEGRO_CUDA(cudaGetDevice(&dev));
+    ALLEGRO_CUDA(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    ALLEGRO_CUDA(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k, kEnvLinThreads, smem));
+    if (per_sm < 1) per_sm = 1;
+    const unsigned grid = (unsigned)(a.n_atoms < n_sm * per_sm ? a.n_atoms : n_sm * per_sm);
     k<<<grid, kEnvLinThreads, smem, a.st>>>(a.n_atoms, a.n_out, a.n_in, a.row_ptr, (const T*)a.rvec, (const T*)a.x, (const T*)a.W, (T)a.scale,
                                                            (T*)a.Eenv);
     ALLEGRO_LAUNCHED();
@@ -214,7 +220,7 @@ allegro_status_t launch_env_linear_backward<ALLEGRO_T, ALLEGRO_L>(const EnvLinAr
         return ALLEGRO_EUNSUPPORTED;
     }
     if (a.n_atoms == 0) return ALLEGRO_OK;
-    size_t smem = ((size_t)kEnvLinChunk * (2 * DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE) * sizeof(T);
+    size_t smem = ((size_t)kEnvLinChunk * (2 * DE + 4) + (size_t)a.n_out * DE + (size_t)a.n_in * DE + (size_t)kEnvLinThreads * DE) * sizeof(T);
     // the chunk's x rows are staged in shared memory when that still leaves two CTAs per SM
     const size_t xs_bytes = (size_t)kEnvLinChunk * (a.n_in + 1) * sizeof(T);
     const int stage_x = smem + xs_bytes <= 100 * 1024 ? 1 : 0;
