@@ -48,6 +48,10 @@ def parse_args():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--replicas", action="store_true", help="N > 1: one independent system per rank (weak scaling) instead of one sharded system")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target CPU time of the oracle sample")
+    ap.add_argument("--dense-tp", action="store_true",
+                    help="side bench: allegro_tp_forward + allegro_tp_backward alone with DENSE per-path weights on the workload's graph, l_max and n "
+                         "(e.g. --workload C3m: the l_max = 3, n = 128 shape of Table 1's large model); not the headline metric")
+    ap.add_argument("--dense-edges", type=int, default=200000, help="--dense-tp: leading centres covering about this many edges")
     return ap.parse_args()
 
 
@@ -596,6 +600,77 @@ def run_two_layer(args, rank, world, local, dist, barrier_factory=None):
         dist.destroy_process_group()
 
 
+def run_dense_tp(args):
+    """Side bench (a4): the dense per-path channel mix alone -- tp_forward + tp_backward (gV, gEenv) with W_p[n, n]
+    per path -- on the leading centres of the workload's graph.  One JSON line; flops = 2 n^2 sum_p (2 l3 + 1) per edge and pass."""
+    import numpy as np
+    import torch
+
+    assert torch.cuda.is_available(), "bench.py needs a CUDA device (there is no CPU fallback)"
+    import paper_2504_16068_b200 as ab
+    from workloads import configs
+    g = configs.geometry_for(args.workload)
+    spec = g["spec"]
+    lmax, n = spec["lmax"], spec["n"]
+    dt = ab.F64 if spec["dtype"] == "f64" else ab.F32
+    rp = g["row_ptr"]
+    c = int(np.searchsorted(rp, min(args.dense_edges, int(rp[-1]))))
+    c = max(1, min(c, rp.shape[0] - 1))
+    E = int(rp[c])
+    plan = ab.Plan(lmax, n, dt, ab.W_DENSE)
+    td = plan.tdtype
+    gen = torch.Generator(device="cuda").manual_seed(0)
+    rnd = lambda *sh: torch.randn(*sh, generator=gen, device="cuda", dtype=td)
+    rpd = torch.from_numpy(np.ascontiguousarray(rp[:c + 1])).cuda()
+    V, G, Ee, W = rnd(E, n, plan.dV), rnd(E, n, plan.dV), rnd(c, n, plan.dE) * 0.5, rnd(plan.P, n, n) / n ** 0.5
+    items = torch.from_numpy(ab.segments_build(rp[:c + 1], 32)).cuda()
+    out, gV, gE = torch.empty_like(V), torch.empty_like(V), torch.empty_like(Ee)
+
+    def step():
+        ab.tp_forward(plan, rpd, V, Ee, W, out=out, items=items)
+        ab.tp_backward(plan, rpd, G, V, Ee, W, gV=gV, gEenv=gE, items=items)
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    clocks = ClockSampler(0)
+    clocks.start()
+    n0 = ab.launch_count()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    tf = tb = 0.0
+    for _ in range(args.steps):
+        ev[0].record()
+        ab.tp_forward(plan, rpd, V, Ee, W, out=out, items=items)
+        ev[1].record()
+        ab.tp_backward(plan, rpd, G, V, Ee, W, gV=gV, gEenv=gE, items=items)
+        ev[2].record()
+        torch.cuda.synchronize()
+        tf += ev[0].elapsed_time(ev[1])
+        tb += ev[1].elapsed_time(ev[2])
+    launches = ab.launch_count() - n0
+    clk = clocks.stop()
+    tf, tb = tf / args.steps, tb / args.steps
+    pt = plan.paths()
+    dT = int(sum(2 * int(l3) + 1 for l3 in pt["l3"]))
+    flops = 2.0 * n * n * dT * E
+    peaks = ab.measure_peaks()
+    tc = lmax == 2 and n == 64 and dt == ab.F32
+    peak = peaks["tf32_mma_tflops"] if tc else peaks["fp32_fma_tflops"]
+    top, ttop = ("tp_backward_dense", tb) if tb >= tf else ("tp_forward_dense", tf)
+    ach = flops / (ttop * 1e-3) / 1e12
+    line = {"metric": "edges/s for the dense per-path mix alone (tp_forward + tp_backward, W_p[n, n] per path)", "value": E / ((tf + tb) * 1e-3),
+            "unit": "edges/s", "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": tf + tb, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f64" if dt == ab.F64 else "f32", "data": "synthetic",
+            "config": {"workload": "%s graph (first %d centres, %d edges), l_max=%d, n=%d, %d paths, dense weights; side bench, not the headline "
+                                   "metric" % (args.workload, c, E, lmax, n, plan.P),
+                       "l2": "inputs of %.1f GB exceed the 126 MB L2" % (3 * V.numel() * V.element_size() / 1e9)},
+            "calls": {"tp_forward_dense": {"ms": tf, "TFLOP/s": flops / (tf * 1e-3) / 1e12}, "tp_backward_dense": {"ms": tb, "TFLOP/s": flops / (tb * 1e-3) / 1e12}},
+            "roofline": {"bound": "tensor" if tc else "alu", "kernel": top, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak, "traffic": None,
+                         "peak_source": "measured in this run (%s)" % ("allegro_measure_tf32_mma_peak" if tc else "allegro_measure_fp32_fma_peak"),
+                         "note": "algorithmic fp32 flops of the n x n mixes (the CG products before them are not counted)"},
+            "peaks": peaks, "clocks": clk, "e2e": None, "gpu_launches": launches}      # e2e: the host-buffer arm belongs to the headline step
+    print(json.dumps(line))
+
+
 def _ncu_traffic(workload, kernel):
     """dram bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/traffic.txt), or None"""
     p = os.path.join(ROOT, "profiles", "traffic.txt")
@@ -609,5 +684,7 @@ if __name__ == "__main__":
     a = parse_args()
     if a.impl == "reference":
         run_reference(a)
+    elif a.dense_tp:
+        run_dense_tp(a)
     else:
         run_ours(a)

@@ -43,3 +43,12 @@ def test_cuda_arm_line():
     assert d2["roofline"]["bound"] == "hbm" and d2["roofline"]["unit"] == "GB/s"
     assert d["gpu_launches"] > 0 and d["e2e"]["h2d_bytes_per_step"] > 0 and d["e2e"]["d2h_bytes_per_step"] > 0
     assert d["cpu_baseline"]["kind"] == "oracle" and "workload" in d["config"]
+
+
+@pytest.mark.gpu
+def test_dense_tp_side_bench_line():
+    """bench.py --dense-tp: the dense per-path mix alone on a workload's graph (l_max = 3 runs the paths-outer FMA kernels)"""
+    d = _run(["--workload", "C3s", "--dense-tp", "--steps", "2", "--warmup", "3"])
+    assert BASE_KEYS | {"roofline", "clocks", "calls"} <= set(d)
+    assert d["value"] > 0 and d["gpu_launches"] >= 4 and d["roofline"]["bound"] == "alu"
+    assert set(d["calls"]) == {"tp_forward_dense", "tp_backward_dense"} and "l_max=3" in d["config"]["workload"]
