@@ -69,6 +69,12 @@ def feature_offset(l, odd):
     return 2 * l * l + ((2 * l + 1) if odd else 0)
 
 
+def latent_update(x, s, A, u):
+    """scalar latent update between layers (reading A19): z = A [x ; s], x_new = u(r / r_c) SiLU(z); x, s [E, n], A [n, 2n], u [E]"""
+    z = torch.cat([x, s], dim=1) @ A.T
+    return z, u[:, None] * torch.nn.functional.silu(z)
+
+
 def forward(params, row_ptr, rvec, taps=None):
     """E_tot (0-d tensor) for rvec [E,3] (float64 tensor, may require grad).  params: lmax, n, nb, n_layers, rc, scale,
     W_x0 [n,nb], W_v0 [n,nb], W_w [L,n,n], W_p [L,P,n,n], A_lat [L-1,n,2n], q [n] (numpy or tensors)."""
@@ -108,8 +114,7 @@ def forward(params, row_ptr, rvec, taps=None):
             taps.append(dict(w=w.detach().numpy(), Eenv=Eenv.detach().numpy(), V_in=V.detach().numpy(), V_out=Vn.detach().numpy(),
                              x_in=x.detach().numpy()))
         if layer < L - 1:
-            z = torch.cat([x, Vn[:, :, 0]], dim=1) @ A_lat[layer].T
-            x = u[:, None] * torch.nn.functional.silu(z)
+            z, x = latent_update(x, Vn[:, :, 0], A_lat[layer], u)
         V = Vn
     e_edge = (V[:, :, 0] * q[None, :]).sum(1)
     if taps is not None:
