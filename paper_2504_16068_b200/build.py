@@ -62,7 +62,7 @@ def generate(force=False):
 
 
 def _jobs():
-    jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("model.o", "model.cu", []), ("peaks.o", "peaks.cu", []), ("neighbour.o", "neighbour.cu", []), ("noalloc.o", "noalloc.cu", []), ("check.o", "check.cu", []), ("plan.o", "plan.cpp", [])]
+    jobs = [("api.o", "api.cu", []), ("misc.o", "misc.cu", []), ("model.o", "model.cu", []), ("peaks.o", "peaks.cu", []), ("neighbour.o", "neighbour.cu", []), ("noalloc.o", "noalloc.cu", []), ("check.o", "check.cu", []), ("tclin.o", "tclin.cu", []), ("plan.o", "plan.cpp", [])]
     for part in (0, 1):
         jobs.insert(0, ("inst_mix3_p%d.o" % part, "inst_mix3.cu", ["-DALLEGRO_MIX3_PART=%d" % part]))
     for tag, ctype in DTYPES:

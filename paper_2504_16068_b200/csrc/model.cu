@@ -2,6 +2,8 @@
 // of the tensor-product hot path: the per-edge linear maps (w = W_w x and its transpose), the scalar latent update
 // x' = u(r/r_c) SiLU(A [x ; V[:,0e]]) with its VJP, and an in-place add.  Small-K GEMMs ([E x 64] x [64 x 64..128]) in the
 // method's own precision (fp32 / fp64 FMA): register-tiled, operands in shared memory.
+#include <initializer_list>
+
 #include "common.cuh"
 #include "launch.h"
 
@@ -319,11 +321,24 @@ allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }
+// tclin.cu: fp32, n = 64, compact scalars (dV == 1), 16-byte aligned rows -- the tcgen05 versions
+allegro_status_t launch_latent_forward_tc(long E, double rc, const void* rvec, const void* x, const void* s, const void* A, void* z, void* x_new,
+                                          cudaStream_t st);
+allegro_status_t launch_latent_backward_tc(long E, double rc, const void* rvec, const void* z, const void* g_xnew, const void* A, void* g_x, void* g_s,
+                                           void* g_rvec, cudaStream_t st);
+static inline bool tc_shape(size_t elem, int n, int dV, std::initializer_list<const void*> ptrs) {
+    if (elem != 4 || n != 64 || dV != 1) return false;
+    for (const void* p : ptrs)
+        if (!aligned16(p)) return false;
+    return true;
+}
+
 template <typename T>
 allegro_status_t launch_latent_forward(long E, int n, int dV, double rc, const void* rvec, const void* x, const void* V, const void* A, void* z,
                                        void* x_new, cudaStream_t st) {
     if (n > 128 || n < 1) { set_error("latent_forward: n = %d unsupported (1 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
+    if (tc_shape(sizeof(T), n, dV, {x, V, A, z, x_new})) return launch_latent_forward_tc(E, rc, rvec, x, V, A, z, x_new, st);
     const int vec = TileVec<T>::N, Kp = tile_kp(2 * n, vec);
     const size_t smem = ((size_t)kTileE * (Kp + vec) + (size_t)Kp * kTileO + kTileE) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(latent_fwd_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -336,6 +351,7 @@ allegro_status_t launch_latent_backward(long E, int n, int dV, double rc, const 
                                         void* g_x, void* gV, void* g_rvec, cudaStream_t st) {
     if (n > 128 || n < 1) { set_error("latent_backward: n = %d unsupported (1 <= n <= 128)", n); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
+    if (tc_shape(sizeof(T), n, dV, {z, g_xnew, A, g_x, gV})) return launch_latent_backward_tc(E, rc, rvec, z, g_xnew, A, g_x, gV, g_rvec, st);
     const int vec = TileVec<T>::N, Kp = tile_kp(n, vec);
     const size_t smem = ((size_t)kTileE * (Kp + vec) + (size_t)Kp * kTileO + (size_t)kTileE * (n + 1) + 2 * kTileE) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(latent_bwd_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

@@ -895,6 +895,56 @@ def test_gpu_neighbour_list_bit_exact(name):
     assert np.array_equal(nl["rvec"].cpu().numpy(), g["rvec"].astype(dt))
 
 
+@pytest.mark.parametrize("n,compact", [(64, True), (64, False), (32, True)])
+def test_latent_update_forward_and_vjp(n, compact):
+    """allegro_latent_forward / _backward (reading A19) against the oracle's latent_update and its autograd VJP.  fp32, n = 64 with the
+    compact scalar channel runs the tcgen05 kernels (tclin.cu: hi / lo tf32 split, TMEM accumulator), the other shapes the FMA tiles;
+    333 edges = two full 128-edge tiles and a ragged one"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from oracle import model2
+    from workloads import configs, rng
+    g = configs.geometry_for("C1s")
+    E, rc = 333, float(g["spec"]["rc"])
+    rvec = g["rvec"][:E].astype(np.float32)
+    S = rng.STREAMS
+    x = rng.normal(51, S["V"], (E, n)).astype(np.float32)
+    sc = rng.normal(52, S["G"], (E, n)).astype(np.float32)
+    A = (rng.normal(53, S["W_p"], (n, 2 * n)) / np.sqrt(2 * n)).astype(np.float32)
+    gx = rng.normal(54, S["q"], (E, n)).astype(np.float32)
+    gs0 = rng.normal(55, S["G"], (E, n)).astype(np.float32)          # the scalar cotangent and g_rvec are accumulated into
+    gr0 = rng.normal(56, S["V"], (E, 3)).astype(np.float32)
+    # oracle: float64, the VJP by autograd of <g_xnew, x_new>
+    t64 = lambda a, grad=False: torch.tensor(a.astype(np.float64), requires_grad=grad)
+    xo, so, ro = t64(x, True), t64(sc, True), t64(rvec, True)
+    r = torch.sqrt((ro * ro).sum(1)) / rc
+    u = 1.0 - 28.0 * r ** 6 + 48.0 * r ** 7 - 21.0 * r ** 8
+    z_ref, xn_ref = model2.latent_update(xo, so, t64(A), u)
+    (xn_ref * t64(gx)).sum().backward()
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    dV = 1 if compact else 18
+    V = torch.zeros((E, n, dV), device="cuda")
+    V[:, :, 0] = d(sc)
+    z, xn = ab.latent_forward(d(rvec), rc, d(x), V, d(A))
+    gV = torch.zeros((E, n, dV), device="cuda")
+    gV[:, :, 0] = d(gs0)
+    g_r = d(gr0).clone()
+    g_x = ab.latent_backward(d(rvec), rc, z, d(gx), d(A), gV, g_r)
+    torch.cuda.synchronize()
+    tol = 1e-5
+
+    def rel(a, b):
+        b = np.asarray(b, dtype=np.float64)
+        return float(np.abs(a.double().cpu().numpy() - b).max() / np.abs(b).max())
+    assert rel(z, z_ref.detach().numpy()) <= tol and rel(xn, xn_ref.detach().numpy()) <= tol
+    assert rel(g_x, xo.grad.numpy()) <= tol
+    assert rel(gV[:, :, 0] - d(gs0), so.grad.numpy()) <= 2 * tol
+    assert rel(g_r - d(gr0), ro.grad.numpy()) <= 4 * tol
+    if dV > 1:
+        assert float(gV[:, :, 1:].abs().max()) == 0.0
+
+
 @pytest.mark.parametrize("name", ["C0", "C4s"])
 def test_check_graph_accepts_sound_lists_and_names_broken_ones(name):
     """allegro_check_graph (debugging aid: the kernels index unchecked and compute-sanitizer is closed on this pool): the seeded
