@@ -90,15 +90,20 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_fwd_kernel(long E, fl
     const uint32_t idesc = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 64);
     const uint32_t sbase = smem_u32(sm);
     uint32_t phase = 0;
-    for (long eb = (long)blockIdx.x * kTcTile; eb < E; eb += (long)gridDim.x * kTcTile) {
-        // rows 16 warp .. + 15: lane l holds chunk l of [x ; s] (K = 4 l .. 4 l + 3): two fully coalesced 256-byte row halves
-        const float* src = lane < 16 ? x : s;
-        float4 v[16];
+    // rows 16 warp .. + 15: lane l holds chunk l of [x ; s] (K = 4 l .. 4 l + 3): two fully coalesced 256-byte row halves.  The rows of
+    // the NEXT tile are loaded into registers right after this tile's MMAs are issued, so that their latency hides behind the MMAs
+    // and the epilogue (one CTA per SM: nothing else would cover it)
+    const float* src = lane < 16 ? x : s;
+    float4 v[16];
+    auto load_rows = [&](long eb) {
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
             const long e = eb + 16 * warp + i;
             v[i] = e < E ? *reinterpret_cast<const float4*>(src + (size_t)e * 64 + 4 * (lane & 15)) : make_float4(0.f, 0.f, 0.f, 0.f);
         }
+    };
+    load_rows((long)blockIdx.x * kTcTile);
+    for (long eb = (long)blockIdx.x * kTcTile; eb < E; eb += (long)gridDim.x * kTcTile) {
 #pragma unroll
         for (int i = 0; i < 16; ++i) tc_store_split(sm + kFwdAhi, sm + kFwdAlo, kAtomA, 16 * warp + i, lane, v[i]);
         if (tid < kTcTile) {
@@ -120,6 +125,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_fwd_kernel(long E, fl
             }
             __syncwarp();
         }
+        load_rows(eb + (long)gridDim.x * kTcTile);
         mbar_wait(&bars->done, phase);
         phase ^= 1u;
         tc05::fence_after_sync();
@@ -158,8 +164,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_fwd_kernel(long E, fl
 
 // -------------------------------------------------------------------------------------------------------------------- VJP
 // A operand = g_z [128 edges][K = 64 outputs of the forward map], formed by the loading warps; B = A^T: row i (the 128 inputs), K = o.
-// shared memory: A_hi [2 slabs][128 x 128 B] | A_lo | B_hi [2 slabs][128 x 128 B] | B_lo | barriers
-constexpr int kBwdAhi = 0, kBwdAlo = 2 * kAtomA, kBwdBhi = 4 * kAtomA, kBwdBlo = 6 * kAtomA, kBwdBars = 8 * kAtomA, kBwdSmem = kBwdBars + 64 + 1024;
+// shared memory: A_hi [2 slabs][128 x 128 B] | A_lo | B_hi [2 slabs][128 x 128 B] | B_lo | radial factor per edge [128] | barriers
+constexpr int kBwdAhi = 0, kBwdAlo = 2 * kAtomA, kBwdBhi = 4 * kAtomA, kBwdBlo = 6 * kAtomA, kBwdSc = 8 * kAtomA, kBwdBars = kBwdSc + kTcTile * 4,
+              kBwdSmem = kBwdBars + 64 + 1024;
 
 __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, float rc, const float* __restrict__ rvec, const float* __restrict__ z,
                                                                        const float* __restrict__ g_xnew, const float* __restrict__ A,
@@ -167,6 +174,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
     extern __shared__ unsigned char tc_raw[];
     unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(tc_raw) + 1023) & ~(uintptr_t)1023);
     TcBars* bars = reinterpret_cast<TcBars*>(sm + kBwdBars);
+    float* scs = reinterpret_cast<float*>(sm + kBwdSc);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     if (warp == 0) {
         tc05::tmem_alloc(&bars->tmem_slot, 128);
@@ -192,10 +200,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
     const uint32_t idesc = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 128);
     const uint32_t sbase = smem_u32(sm);
     uint32_t phase = 0;
-    for (long eb = (long)blockIdx.x * kTcTile; eb < E; eb += (long)gridDim.x * kTcTile) {
-        // half-warp per row: rows 16 warp + 2 i + (lane >> 4), chunk c = lane & 15 (outputs 4 c .. 4 c + 3)
-        const int c = lane & 15;
-        float4 zv[8], gv[8];
+    // half-warp per row: rows 16 warp + 2 i + (lane >> 4), chunk c = lane & 15 (outputs 4 c .. 4 c + 3); the next tile's rows are
+    // prefetched into registers behind the MMAs and the epilogue, as in the forward kernel
+    const int c = lane & 15;
+    float4 zv[8], gv[8];
+    auto load_rows = [&](long eb) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const long e = eb + 16 * warp + 2 * i + (lane >> 4);
@@ -207,6 +216,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
                 gv[i] = zv[i];
             }
         }
+    };
+    load_rows((long)blockIdx.x * kTcTile);
+    for (long eb = (long)blockIdx.x * kTcTile; eb < E; eb += (long)gridDim.x * kTcTile) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
             const int r = 16 * warp + 2 * i + (lane >> 4);
@@ -231,12 +243,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
             // radial term: sum over the 64 outputs = fixed xor tree over the row's 16 lanes
 #pragma unroll
             for (int sft = 8; sft > 0; sft >>= 1) sv += __shfl_xor_sync(0xffffffffu, sv, sft);
-            if (c == 0 && e < E) {
-                const float sc = sv * dus;
-                g_rvec[3 * e] += sc * rx;
-                g_rvec[3 * e + 1] += sc * ry;
-                g_rvec[3 * e + 2] += sc * rz;
-            }
+            if (c == 0) scs[r] = sv * dus;      // the edge's g_rvec update follows below, one thread per edge (independent loads)
         }
         fence_proxy_async();
         __syncthreads();
@@ -248,30 +255,42 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
             }
             __syncwarp();
         }
+        // while the MMAs run: the radial term of this tile's edges, the old scalar cotangent rows of the warps that add to them,
+        // and the next tile's rows
+        if (tid < kTcTile && eb + tid < E) {
+            const long e = eb + tid;
+            const float sc = scs[tid];
+            g_rvec[3 * e] += sc * rvec[3 * e];
+            g_rvec[3 * e + 1] += sc * rvec[3 * e + 1];
+            g_rvec[3 * e + 2] += sc * rvec[3 * e + 2];
+        }
+        const int q = warp & 3, hc = warp >> 2;
+        const long er = eb + 32 * q + lane;
+        float* dst = (hc ? g_s : g_x) + (size_t)(er < E ? er : 0) * 64;
+        float4 old[16];
+        if (hc) {
+#pragma unroll
+            for (int k = 0; k < 16; ++k) old[k] = er < E ? reinterpret_cast<const float4*>(dst)[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        load_rows(eb + (long)gridDim.x * kTcTile);
         mbar_wait(&bars->done, phase);
         phase ^= 1u;
         tc05::fence_after_sync();
         // columns 0..63 = g_x (overwritten), 64..127 = the compact scalar cotangent (added to)
-        {
-            const int q = warp & 3, hc = warp >> 2, r = 32 * q + lane;
-            const long e = eb + r;
-            float* dst = (hc ? g_s : g_x) + (size_t)(e < E ? e : 0) * 64;
 #pragma unroll
-            for (int g = 0; g < 4; ++g) {
-                uint32_t w[16];
-                tc05::tmem_ld16(tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(64 * hc + 16 * g), w);
-                tc05::tmem_ld_wait();
-                if (e < E) {
-                    float4* d4 = reinterpret_cast<float4*>(dst + 16 * g);
+        for (int g = 0; g < 4; ++g) {
+            uint32_t w[16];
+            tc05::tmem_ld16(tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(64 * hc + 16 * g), w);
+            tc05::tmem_ld_wait();
+            if (er < E) {
+                float4* d4 = reinterpret_cast<float4*>(dst + 16 * g);
 #pragma unroll
-                    for (int k = 0; k < 4; ++k) {
-                        float4 o = make_float4(__uint_as_float(w[4 * k]), __uint_as_float(w[4 * k + 1]), __uint_as_float(w[4 * k + 2]), __uint_as_float(w[4 * k + 3]));
-                        if (hc) {
-                            const float4 old = d4[k];
-                            o.x += old.x; o.y += old.y; o.z += old.z; o.w += old.w;
-                        }
-                        d4[k] = o;
+                for (int k = 0; k < 4; ++k) {
+                    float4 o = make_float4(__uint_as_float(w[4 * k]), __uint_as_float(w[4 * k + 1]), __uint_as_float(w[4 * k + 2]), __uint_as_float(w[4 * k + 3]));
+                    if (hc) {
+                        o.x += old[4 * g + k].x; o.y += old[4 * g + k].y; o.z += old[4 * g + k].z; o.w += old[4 * g + k].w;
                     }
+                    d4[k] = o;
                 }
             }
         }
