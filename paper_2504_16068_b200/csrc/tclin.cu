@@ -65,7 +65,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_fwd_kernel(long E, fl
                                                                        const float* __restrict__ s, const float* __restrict__ A,
                                                                        float* __restrict__ z, float* __restrict__ x_new) {
     extern __shared__ unsigned char tc_raw[];
-    unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(tc_raw) + 1023) & ~(uintptr_t)1023);
+    unsigned char* sm = tc_raw + ((1024u - (smem_u32(tc_raw) & 1023u)) & 1023u);     // 1024-byte aligned, still a shared-window pointer (STS, not ST)
     float* us = reinterpret_cast<float*>(sm + kFwdU);
     TcBars* bars = reinterpret_cast<TcBars*>(sm + kFwdBars);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
@@ -172,7 +172,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
                                                                        const float* __restrict__ g_xnew, const float* __restrict__ A,
                                                                        float* __restrict__ g_x, float* __restrict__ g_s, float* __restrict__ g_rvec) {
     extern __shared__ unsigned char tc_raw[];
-    unsigned char* sm = reinterpret_cast<unsigned char*>((reinterpret_cast<uintptr_t>(tc_raw) + 1023) & ~(uintptr_t)1023);
+    unsigned char* sm = tc_raw + ((1024u - (smem_u32(tc_raw) & 1023u)) & 1023u);     // 1024-byte aligned, still a shared-window pointer (STS, not ST)
     TcBars* bars = reinterpret_cast<TcBars*>(sm + kBwdBars);
     float* scs = reinterpret_cast<float*>(sm + kBwdSc);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
