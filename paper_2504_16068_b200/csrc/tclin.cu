@@ -95,11 +95,15 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_fwd_kernel(long E, fl
     // and the epilogue (one CTA per SM: nothing else would cover it)
     const float* src = lane < 16 ? x : s;
     float4 v[16];
+    float r3[3] = {1.f, 0.f, 0.f};      // edge vector of row tid (threads 0..127 form the cutoff values)
     auto load_rows = [&](long eb) {
 #pragma unroll
         for (int i = 0; i < 16; ++i) {
             const long e = eb + 16 * warp + i;
             v[i] = e < E ? *reinterpret_cast<const float4*>(src + (size_t)e * 64 + 4 * (lane & 15)) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        if (tid < kTcTile && eb + tid < E) {
+            r3[0] = rvec[3 * (eb + tid)]; r3[1] = rvec[3 * (eb + tid) + 1]; r3[2] = rvec[3 * (eb + tid) + 2];
         }
     };
     load_rows((long)blockIdx.x * kTcTile);
@@ -107,12 +111,8 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_fwd_kernel(long E, fl
 #pragma unroll
         for (int i = 0; i < 16; ++i) tc_store_split(sm + kFwdAhi, sm + kFwdAlo, kAtomA, 16 * warp + i, lane, v[i]);
         if (tid < kTcTile) {
-            const long e = eb + tid;
             float du, u = 0.f;
-            if (e < E) {
-                const float rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
-                u = tc_cutoff<float>(sqrtf(rx * rx + ry * ry + rz * rz) / rc, du);
-            }
+            if (eb + tid < E) u = tc_cutoff<float>(sqrtf(r3[0] * r3[0] + r3[1] * r3[1] + r3[2] * r3[2]) / rc, du);
             us[tid] = u;
         }
         fence_proxy_async();
@@ -204,6 +204,7 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
     // prefetched into registers behind the MMAs and the epilogue, as in the forward kernel
     const int c = lane & 15;
     float4 zv[8], gv[8];
+    float rr3[8][3];
     auto load_rows = [&](long eb) {
 #pragma unroll
         for (int i = 0; i < 8; ++i) {
@@ -211,9 +212,11 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
             if (e < E) {
                 zv[i] = *reinterpret_cast<const float4*>(z + (size_t)e * 64 + 4 * c);
                 gv[i] = *reinterpret_cast<const float4*>(g_xnew + (size_t)e * 64 + 4 * c);
+                rr3[i][0] = rvec[3 * e]; rr3[i][1] = rvec[3 * e + 1]; rr3[i][2] = rvec[3 * e + 2];
             } else {
                 zv[i] = make_float4(0.f, 0.f, 0.f, 0.f);
                 gv[i] = zv[i];
+                rr3[i][0] = 1.f; rr3[i][1] = 0.f; rr3[i][2] = 0.f;
             }
         }
     };
@@ -223,10 +226,9 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
         for (int i = 0; i < 8; ++i) {
             const int r = 16 * warp + 2 * i + (lane >> 4);
             const long e = eb + r;
-            float u = 0.f, dus = 0.f, rx = 0.f, ry = 0.f, rz = 0.f;
+            float u = 0.f, dus = 0.f;
             if (e < E) {
-                rx = rvec[3 * e]; ry = rvec[3 * e + 1]; rz = rvec[3 * e + 2];
-                const float rr = sqrtf(rx * rx + ry * ry + rz * rz);
+                const float rr = sqrtf(rr3[i][0] * rr3[i][0] + rr3[i][1] * rr3[i][1] + rr3[i][2] * rr3[i][2]);
                 float du;
                 u = tc_cutoff<float>(rr / rc, du);
                 dus = du / rc / rr;
