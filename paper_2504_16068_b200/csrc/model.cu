@@ -310,10 +310,13 @@ static inline unsigned model_grid(long E) {
     return (unsigned)(want < 148 * 2 ? (want < 1 ? 1 : want) : 148 * 2);
 }
 
+allegro_status_t launch_linear64_tc(long E, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st);
+
 template <typename T>
 allegro_status_t launch_linear(long E, int n_out, int n_in, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st) {
     if (n_out > 1024 || n_in > 256) { set_error("linear: n_out = %d, n_in = %d unsupported (<= 1024, <= 256)", n_out, n_in); return ALLEGRO_EUNSUPPORTED; }
     if (E == 0) return ALLEGRO_OK;
+    if (sizeof(T) == 4 && n_out == 64 && n_in == 64 && aligned16(x) && aligned16(y)) return launch_linear64_tc(E, x, W, transpose_w, accumulate, y, st);
     const int vec = TileVec<T>::N, Kp = tile_kp(n_in, vec);
     const size_t smem = ((size_t)kTileE * (Kp + vec) + (size_t)Kp * kTileO) * sizeof(T);
     ALLEGRO_CUDA(cudaFuncSetAttribute(linear_kernel<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));

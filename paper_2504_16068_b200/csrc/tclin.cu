@@ -302,6 +302,100 @@ __global__ void __launch_bounds__(kTcThreads, 1) tc_latent_bwd_kernel(long E, fl
     if (warp == 0) tc05::tmem_dealloc(tbase, 128);
 }
 
+// ------------------------------------------------------------------------------------------------- linear map, K = N = 64
+// y[e][o] (+)= sum_i x[e][i] W[o][i] (transpose_w == 0) or sum_i x[e][i] W[i][o] (transpose_w == 1): the per-edge linear of the stacked
+// model when the embedding is not factorised (reading A19) and its VJP.  Same scheme as above; 96 KB of images: two CTAs per SM.
+constexpr int kLinAhi = 0, kLinAlo = 2 * kAtomA, kLinBhi = 4 * kAtomA, kLinBatom = 64 * 128, kLinBlo = kLinBhi + 2 * kLinBatom,
+              kLinBars = kLinBlo + 2 * kLinBatom, kLinSmem = kLinBars + 64 + 1024;
+
+__global__ void __launch_bounds__(kTcThreads, 2) tc_linear64_kernel(long E, const float* __restrict__ x, const float* __restrict__ W, int transpose_w,
+                                                                     int accumulate, float* __restrict__ y) {
+    extern __shared__ unsigned char tc_raw[];
+    unsigned char* sm = tc_raw + ((1024u - (smem_u32(tc_raw) & 1023u)) & 1023u);
+    TcBars* bars = reinterpret_cast<TcBars*>(sm + kLinBars);
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    if (warp == 0) {
+        tc05::tmem_alloc(&bars->tmem_slot, 64);
+        tc05::tmem_relinquish();
+    }
+    if (tid == 0) {
+        mbar_init(&bars->done, 1);
+        fence_mbar_init();
+    }
+    // B row o (an output), K position i (an input)
+    for (int idx = tid; idx < 64 * 64; idx += kTcThreads) {
+        const int o = transpose_w ? (idx & 63) : (idx >> 6), i = transpose_w ? (idx >> 6) : (idx & 63), c = i >> 2;
+        const float a = W[idx];
+        const uint32_t off = (uint32_t)(c >> 3) * (uint32_t)kLinBatom + tc05::sw128_off((uint32_t)o, (uint32_t)(c & 7)) + (uint32_t)(i & 3) * 4u;
+        *reinterpret_cast<float*>(sm + kLinBhi + off) = a;
+        *reinterpret_cast<float*>(sm + kLinBlo + off) = tc_lo(a);
+    }
+    fence_proxy_async();
+    tc05::fence_before_sync();
+    __syncthreads();
+    tc05::fence_after_sync();
+    const uint32_t tbase = bars->tmem_slot;
+    const uint32_t idesc = tc05::make_idesc(tc05::FMT_TF32, tc05::FMT_TF32, 128, 64);
+    const uint32_t sbase = smem_u32(sm);
+    uint32_t phase = 0;
+    const int c = lane & 15;
+    float4 xv[8];
+    auto load_rows = [&](long eb) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) {
+            const long e = eb + 16 * warp + 2 * i + (lane >> 4);
+            xv[i] = e < E ? *reinterpret_cast<const float4*>(x + (size_t)e * 64 + 4 * c) : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+    };
+    load_rows((long)blockIdx.x * kTcTile);
+    for (long eb = (long)blockIdx.x * kTcTile; eb < E; eb += (long)gridDim.x * kTcTile) {
+#pragma unroll
+        for (int i = 0; i < 8; ++i) tc_store_split(sm + kLinAhi, sm + kLinAlo, kAtomA, 16 * warp + 2 * i + (lane >> 4), c, xv[i]);
+        fence_proxy_async();
+        __syncthreads();
+        if (warp == 0) {
+            if (tc05::elect_one()) {
+                tc05::fence_after_sync();
+                tc_issue(tbase, sbase + kLinAhi, sbase + kLinAlo, sbase + kLinBhi, sbase + kLinBlo, kLinBatom, 8, idesc);
+                tc05::mma_commit(&bars->done);
+            }
+            __syncwarp();
+        }
+        load_rows(eb + (long)gridDim.x * kTcTile);
+        const int q = warp & 3, hc = warp >> 2;
+        const long er = eb + 32 * q + lane;
+        float* dst = y + (size_t)(er < E ? er : 0) * 64 + 32 * hc;
+        float4 old[8];
+        if (accumulate) {
+#pragma unroll
+            for (int k = 0; k < 8; ++k) old[k] = er < E ? reinterpret_cast<const float4*>(dst)[k] : make_float4(0.f, 0.f, 0.f, 0.f);
+        }
+        mbar_wait(&bars->done, phase);
+        phase ^= 1u;
+        tc05::fence_after_sync();
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+            uint32_t w[16];
+            tc05::tmem_ld16(tbase + ((uint32_t)(32 * q) << 16) + (uint32_t)(32 * hc + 16 * g), w);
+            tc05::tmem_ld_wait();
+            if (er < E) {
+                float4* d4 = reinterpret_cast<float4*>(dst + 16 * g);
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    float4 o = make_float4(__uint_as_float(w[4 * k]), __uint_as_float(w[4 * k + 1]), __uint_as_float(w[4 * k + 2]), __uint_as_float(w[4 * k + 3]));
+                    if (accumulate) {
+                        o.x += old[4 * g + k].x; o.y += old[4 * g + k].y; o.z += old[4 * g + k].z; o.w += old[4 * g + k].w;
+                    }
+                    d4[k] = o;
+                }
+            }
+        }
+        tc05::fence_before_sync();
+        __syncthreads();
+    }
+    if (warp == 0) tc05::tmem_dealloc(tbase, 64);
+}
+
 }  // namespace
 
 // ---------------------------------------------------------------------------------------------------------------- launchers
@@ -326,6 +420,17 @@ allegro_status_t launch_latent_backward_tc(long E, double rc, const void* rvec, 
     ALLEGRO_CUDA(cudaFuncSetAttribute(tc_latent_bwd_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kBwdSmem));
     tc_latent_bwd_kernel<<<tc_grid(E), kTcThreads, kBwdSmem, st>>>(E, (float)rc, (const float*)rvec, (const float*)z, (const float*)g_xnew,
                                                                    (const float*)A, (float*)g_x, (float*)g_s, (float*)g_rvec);
+    ALLEGRO_LAUNCHED();
+    return ALLEGRO_OK;
+}
+
+
+allegro_status_t launch_linear64_tc(long E, const void* x, const void* W, int transpose_w, int accumulate, void* y, cudaStream_t st) {
+    ALLEGRO_CUDA(cudaFuncSetAttribute(tc_linear64_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kLinSmem));
+    const long tiles = (E + kTcTile - 1) / kTcTile;
+    const unsigned g1 = tc_grid(E);
+    const unsigned grid = (unsigned)(tiles < 2L * g1 ? tiles : 2L * g1);      // two CTAs per SM
+    tc_linear64_kernel<<<grid, kTcThreads, kLinSmem, st>>>(E, (const float*)x, (const float*)W, transpose_w, accumulate, (float*)y);
     ALLEGRO_LAUNCHED();
     return ALLEGRO_OK;
 }

@@ -895,6 +895,36 @@ def test_gpu_neighbour_list_bit_exact(name):
     assert np.array_equal(nl["rvec"].cpu().numpy(), g["rvec"].astype(dt))
 
 
+@pytest.mark.parametrize("n_in,n_out", [(64, 64), (64, 128), (32, 64)])
+def test_linear_map_and_its_transpose(n_in, n_out):
+    """allegro_linear: y (+)= x W^T and the transposed map with accumulation (the per-edge linear of reading A19 and its VJP), against the
+    float64 matrix products.  fp32 with 64 inputs and 64 outputs runs on tcgen05 (tclin.cu), the other shapes on the FMA tiles;
+    333 rows = two full 128-row tiles and a ragged one"""
+    import torch
+
+    import paper_2504_16068_b200 as ab
+    from workloads import rng
+    S = rng.STREAMS
+    R = 333
+    x = rng.normal(61, S["V"], (R, n_in)).astype(np.float32)
+    W = (rng.normal(62, S["W_p"], (n_out, n_in)) / np.sqrt(n_in)).astype(np.float32)
+    g = rng.normal(63, S["G"], (R, n_out)).astype(np.float32)
+    y0 = rng.normal(64, S["q"], (R, n_in)).astype(np.float32)
+    d = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    f8 = lambda a: a.astype(np.float64)
+    y = ab.linear(d(x), d(W))
+    gx = ab.linear(d(g), d(W), transpose_w=True)
+    acc = d(y0).clone()
+    ab.linear(d(g), d(W), transpose_w=True, y=acc, accumulate=True)
+    torch.cuda.synchronize()
+
+    def rel(a, b):
+        return float(np.abs(a.double().cpu().numpy() - b).max() / np.abs(b).max())
+    assert rel(y, f8(x) @ f8(W).T) <= 1e-5
+    assert rel(gx, f8(g) @ f8(W)) <= 1e-5
+    assert rel(acc, f8(y0) + f8(g) @ f8(W)) <= 1e-5
+
+
 @pytest.mark.parametrize("n,compact", [(64, True), (64, False), (32, True)])
 def test_latent_update_forward_and_vjp(n, compact):
     """allegro_latent_forward / _backward (reading A19) against the oracle's latent_update and its autograd VJP.  fp32, n = 64 with the
