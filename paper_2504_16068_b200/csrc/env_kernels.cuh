@@ -512,16 +512,41 @@ __global__ void __launch_bounds__(256) edge_embed_kernel(int n, int nb, double r
     }
     if (tid < cnt) geo_phase1<T, L, NB, false>(sm, tid, rvec, (size_t)(cb + tid), rc, nb);
     __syncthreads();
+    // n <= 64: the weights of the lane's (at most two) channels live in registers for all of the warp's edges -- read from shared memory
+    // per edge they are 4 wavefronts per basis function and the kernel is bound by the shared-memory pipe
+    const bool wreg = n <= 64;
+    double wx[2][NB], wv[2][NB];
+#pragma unroll
+    for (int g = 0; g < 2; ++g)
+#pragma unroll
+        for (int b = 0; b < NB; ++b) {
+            const int ch = 32 * g + lane;
+            const bool ok = wreg && ch < n && b < nb;
+            wx[g][b] = ok ? Wxs[b * n + ch] : 0.0;
+            wv[g][b] = ok ? Wvs[b * n + ch] : 0.0;
+        }
     for (int le = warp; le < cnt; le += 8) {
         const size_t e = (size_t)(cb + le);
+        double bus[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) bus[b] = b < nb ? sm.Bs[le][b] : 0.0;
         for (int ch0 = 0; ch0 < n; ch0 += 32) {
             const int ch = ch0 + lane;
             if (ch < n) {
                 double sx = 0.0, sv = 0.0;
-                for (int b = 0; b < nb; ++b) {
-                    const double bu = sm.Bs[le][b];
-                    sx = fma(Wxs[b * n + ch], bu, sx);
-                    sv = fma(Wvs[b * n + ch], bu, sv);
+                if (wreg) {
+                    const int g = ch0 >> 5;
+#pragma unroll
+                    for (int b = 0; b < NB; ++b) {
+                        sx = fma(g ? wx[1][b] : wx[0][b], bus[b], sx);
+                        sv = fma(g ? wv[1][b] : wv[0][b], bus[b], sv);
+                    }
+                } else {
+                    for (int b = 0; b < nb; ++b) {      // (sm.Bs, not bus[b]: a run-time index would put bus into local memory)
+                        const double bu = sm.Bs[le][b];
+                        sx = fma(Wxs[b * n + ch], bu, sx);
+                        sv = fma(Wvs[b * n + ch], bu, sv);
+                    }
                 }
                 x0[e * n + ch] = (T)sx;
                 const T v0 = (T)sv;
@@ -648,10 +673,16 @@ __global__ void __launch_bounds__(kGeoChunk) edge_embed_factors_bwd_kernel(int n
         Wxs[idx] = b < nb ? (double)W_x0[ch * nb + b] : 0.0;
         Wvs[idx] = b < nb ? (double)W_v0[ch * nb + b] : 0.0;
     }
-    __syncthreads();
-    const long e = (long)blockIdx.x * kGeoChunk + tid;
-    if (e >= E) return;
-    const T rx = rvec[3 * e], ry = rvec[3 * e + 1], rz = rvec[3 * e + 2];
+    const long cb = (long)blockIdx.x * kGeoChunk;
+    const long e = cb + tid;
+    const bool live = e < E;
+    const int cnt = (int)min((long)kGeoChunk, E - cb);
+    // the chunk's cotangent rows, 32 channels at a time: loaded with lanes along the channels (coalesced), read back one ROW per thread
+    // from rows padded to 33 words (conflict-free).  Read straight from global memory a thread walks its own 256-byte row: one sector
+    // per lane and load, 32 wavefronts per request
+    T* xs = reinterpret_cast<T*>(Wvs + (size_t)n * NB);     // [chunk][33]
+    T* vs = xs + kGeoChunk * 33;
+    const T rx = live ? rvec[3 * e] : T(1), ry = live ? rvec[3 * e + 1] : T(0), rz = live ? rvec[3 * e + 2] : T(0);
     const double dx = (double)rx, dy = (double)ry, dz = (double)rz;
     const double rr = sqrt(dx * dx + dy * dy + dz * dz);
     double Bu[kMaxBasis], dBu[kMaxBasis];
@@ -659,13 +690,27 @@ __global__ void __launch_bounds__(kGeoChunk) edge_embed_factors_bwd_kernel(int n
     double gb[NB];
 #pragma unroll
     for (int b = 0; b < NB; ++b) gb[b] = 0.0;
-    const T* gx = g_x0 + (size_t)e * n;
-    const T* gv = g_v0 + (size_t)e * n;
-    for (int ch = 0; ch < n; ++ch) {
-        const double a = (double)gx[ch], c = (double)gv[ch];
+    for (int c0 = 0; c0 < n; c0 += 32) {
+        const int cw = min(32, n - c0);
+        __syncthreads();
+        for (int idx = tid; idx < cnt * 32; idx += kGeoChunk) {
+            const int le = idx >> 5, cc = idx & 31;
+            if (cc < cw) {
+                xs[le * 33 + cc] = g_x0[(size_t)(cb + le) * n + c0 + cc];
+                vs[le * 33 + cc] = g_v0[(size_t)(cb + le) * n + c0 + cc];
+            }
+        }
+        __syncthreads();
+        if (live) {
+            for (int cc = 0; cc < cw; ++cc) {
+                const double a = (double)xs[tid * 33 + cc], c = (double)vs[tid * 33 + cc];
+                const int ch = c0 + cc;
 #pragma unroll
-        for (int b = 0; b < NB; ++b) gb[b] = fma(a, Wxs[ch * NB + b], fma(c, Wvs[ch * NB + b], gb[b]));
+                for (int b = 0; b < NB; ++b) gb[b] = fma(a, Wxs[ch * NB + b], fma(c, Wvs[ch * NB + b], gb[b]));
+            }
+        }
     }
+    if (!live) return;
     double rad = 0.0;
 #pragma unroll
     for (int b = 0; b < NB; ++b)

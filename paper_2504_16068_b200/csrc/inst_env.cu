@@ -162,7 +162,7 @@ allegro_status_t launch_edge_embed_backward<ALLEGRO_T, ALLEGRO_L>(const EmbedArg
 #define ALLEGRO_EMBF(NB)                                                                                                    \
     {                                                                                                                       \
         auto k = edge_embed_factors_bwd_kernel<T, ALLEGRO_L, NB>;                                                           \
-        const size_t smem = (size_t)2 * a.n * NB * sizeof(double);                                                          \
+        const size_t smem = (size_t)2 * a.n * NB * sizeof(double) + (size_t)2 * kGeoChunk * 33 * sizeof(T);                  \
         ALLEGRO_CUDA(cudaFuncSetAttribute(k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));                       \
         k<<<grid, kGeoChunk, smem, a.st>>>(a.n, a.nb, a.rc, a.n_edges, (const T*)a.rvec, (const T*)a.W_x0, (const T*)a.W_v0,  \
                                            (const T*)a.g_x0, (const T*)a.g_v0, (const T*)a.gYe, (T*)a.g_rvec);              \
